@@ -1,0 +1,165 @@
+/*
+ * sdf.h -- C ABI of the B200-native CSC closest-point transform
+ * (narrow-band signed distance + closest-triangle grids from a closed triangle soup).
+ *
+ * Method: Roosing, Strickson, Nikiforakis, "Fast Distance Fields for Fluid Dynamics
+ * Mesh Generation on Graphics Hardware", arXiv:1903.00353.  Citations are lines of
+ * /root/reference/PAPER.md ("PAPER.md:<line>") plus the section / equation.
+ *
+ *   problem statement      PAPER.md:45   (eq.1: f(x) = min distance to the surface, signed)
+ *                          PAPER.md:63-77 (sec.2 pseudo-code: for each extrusion, for each cell
+ *                                          inside, keep the min-magnitude distance)
+ *   input                  PAPER.md:274-294 (sec.7: closed, consistently oriented STL triangle
+ *                                          soup, vertices counter-clockwise from outside,
+ *                                          arbitrary triangle order, duplicated vertices)
+ *   grid / output          PAPER.md:384  (sec.10: row-major 1-D float array; coordinates
+ *                                          recovered from the offset and the physical limits)
+ *   band                   PAPER.md:392  (distance written only if smaller than a user maximum)
+ *
+ * Every function returns an int status (0 = SDF_OK); none throws, aborts or prints.
+ * The library never falls back to a CPU implementation: without a CUDA device every
+ * compute entry point returns SDF_ECUDA.
+ */
+#ifndef PAPER_1903_00353_SDF_H
+#define PAPER_1903_00353_SDF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    SDF_OK          = 0,
+    SDF_EINVAL      = 1,  /* null pointer, ntri <= 0, h <= 0, band <= 0, bad dims, NaN/Inf input */
+    SDF_ENOTCLOSED  = 2,  /* an undirected edge without exactly two incident triangles */
+    SDF_EORIENT     = 3,  /* an edge traversed in the same direction by both triangles */
+    SDF_EDEGENERATE = 4,  /* zero-area triangle or repeated vertex in a triangle */
+    SDF_ENOMEM      = 5,  /* device (or host staging) allocation failed */
+    SDF_ECUDA       = 6   /* CUDA runtime error / no device; see sdf_last_cuda_error() */
+};
+
+/* Opaque handle: device-resident feature tables of one mesh.  Owned by the library,
+ * released by sdf_destroy. */
+typedef struct sdf_mesh sdf_mesh;
+
+/* Device-memory callbacks supplied by the caller (from Python: torch's caching
+ * allocator).  `alloc` returns a DEVICE pointer usable on `stream` (NULL on failure);
+ * `free` releases it.  Pass a NULL sdf_allocator* to let the library use the CUDA
+ * stream-ordered pool (cudaMallocAsync). The struct is copied; `user` must stay valid
+ * until sdf_destroy. */
+typedef struct sdf_allocator {
+    void *(*alloc)(size_t bytes, void *stream, void *user);
+    void  (*free)(void *ptr, void *user);
+    void  *user;
+} sdf_allocator;
+
+/* Counters of the feature builder and of the last sdf_compute (host values). */
+typedef struct sdf_stats_t {
+    int64_t F, V, E;                      /* triangles, welded vertices, undirected edges      */
+    int64_t edges_convex, edges_concave, edges_flat;      /* PAPER.md:352 discriminant         */
+    int64_t verts_pos_only, verts_neg_only, verts_both, verts_skipped; /* cone sides emitted   */
+    int64_t verts_hemisphere;             /* "ruff" vertices: cos_cone <= 0 */
+    int64_t weld_collisions;              /* hash-equal runs that held distinct vertices        */
+    /* last sdf_compute */
+    int64_t polyhedra;                    /* extrusions with a non-empty clipped bounding volume */
+    int64_t work_items;                   /* (polyhedron, grid row) items after the prefix sum  */
+    int64_t pairs_tested;                 /* (cell, polyhedron) pairs inside a clipped row span */
+    int64_t pairs_accepted;               /* of those: inside the polyhedron and d < band       */
+    int64_t bricks_active, bricks_total;  /* 8x8x8-cell bricks holding packed scratch           */
+    int64_t band_cells;                   /* populated output cells                             */
+    int64_t fp64_rechecks;                /* cells whose band / sign decision was redone in fp64 */
+} sdf_stats_t;
+
+/*
+ * sdf_create -- organise the unordered soup into features (sec.7: weld
+ * identical vertices, pair the two half-edges of every edge
+ * eq.8: angle-weighted pseudonormals; convex / concave /
+ * flat / saddle classification) and build the band-independent part of every
+ * characteristic polyhedron (eq.3-5, 344-364 sec.8).
+ *
+ *   tri_xyz   [ntri][3 vertices][x,y,z] fp32, counter-clockwise seen from outside
+ *             (PAPER.md:278).  HOST pointer when on_device == 0 (copied with
+ *             cudaMemcpyAsync), DEVICE pointer when on_device == 1.  Borrowed for the
+ *             duration of the call only.  Vertices are identical iff their three fp32
+ *             values are bit-identical (-0 == +0).
+ *   ntri      1 .. 2^30-1
+ *   a         device allocator, or NULL
+ *   stream    cudaStream_t (0 = legacy default stream).  The call synchronises the stream
+ *             once before returning (validation flags and the vertex count).
+ *   out       receives the handle on SDF_OK; set to NULL otherwise.
+ * Errors: SDF_EINVAL, SDF_ENOTCLOSED, SDF_EORIENT, SDF_EDEGENERATE, SDF_ENOMEM, SDF_ECUDA.
+ */
+int sdf_create(const float *tri_xyz, int64_t ntri, int on_device,
+               const sdf_allocator *a, void *stream, sdf_mesh **out);
+
+/*
+ * sdf_compute -- clip every characteristic polyhedron to the band and the grid
+ * (PAPER.md:344-364), scan-convert it into (polyhedron, grid-row) work items
+ * (sec.5, replacing the schedulers of PAPER.md:366-380), evaluate the
+ * exact feature distance for every cell inside and min-combine (PAPER.md:63-77, 374,
+ * 386-392), then sign every populated cell from the pseudonormal of its closest feature
+ * and write both grids.
+ *
+ *   origin    HOST pointer to 3 floats: position of sample (0,0,0).  Sample (i,j,k) sits at
+ *             origin + (i,j,k)*h (cell centres).
+ *   h         grid spacing > 0;  nx,ny,nz: 1 .. 32767 each;  band > 0 in length units.
+ *   dist_out  DEVICE, caller-owned, nx*ny*nz floats, linear index ((int64)k*ny + j)*nx + i
+ *             (x fastest).  Signed distance, negative inside, written iff
+ *             |d| < band; +INFINITY elsewhere.  Every element is
+ *             overwritten.
+ *   tri_out   DEVICE, caller-owned, nx*ny*nz int32: index (in the caller's soup order) of
+ *             the closest triangle, -1 outside the band.  Where several triangles are
+ *             equally close (closest point on a shared edge / vertex) the lowest index.
+ *   stream    cudaStream_t.  Work is enqueued on it; the call synchronises it once
+ *             mid-way (work-item and brick totals) and leaves the final kernels enqueued.
+ * May be called repeatedly on one handle with different grids / bands.
+ * Errors: SDF_EINVAL, SDF_ENOMEM, SDF_ECUDA.
+ */
+int sdf_compute(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz,
+                float band, float *dist_out, int32_t *tri_out, void *stream);
+
+/*
+ * sdf_compute_host -- same as sdf_compute but dist_out / tri_out are HOST buffers
+ * (pinned memory recommended): device grids are taken from the allocator, computed,
+ * copied back with cudaMemcpyAsync and the stream is synchronised before returning.
+ */
+int sdf_compute_host(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz,
+                     float band, float *dist_out_host, int32_t *tri_out_host, void *stream);
+
+/* Counters (host struct filled from the handle; synchronises `the last stream used` if a
+ * compute is still in flight). */
+int sdf_stats(sdf_mesh *m, sdf_stats_t *out);
+
+/*
+ * sdf_get_table -- copy one internal feature table to HOST memory (tests / inspection).
+ *   which: one of SDF_TABLE_*; dst: host buffer of `bytes` bytes, which must equal the
+ *   table size exactly (SDF_EINVAL otherwise).  Synchronous.
+ */
+enum {
+    SDF_TABLE_CORNER_VID   = 0,  /* int32 [3F]   corner -> welded vertex id                      */
+    SDF_TABLE_HALFEDGE_ADJ = 1,  /* int32 [3F]   half-edge 3t+k (corner k -> k+1) -> its opposite */
+    SDF_TABLE_FACE_NORMAL  = 2,  /* float [F][3] unit face normals                               */
+    SDF_TABLE_VERTEX_REC   = 3,  /* 32 B  [V]    {float pos[3], axis[3], cos_cone; int32 info}   */
+    SDF_TABLE_EDGE_REC     = 4,  /* 64 B  [E]    {float a[3], b[3], n1[3], n2[3]; int32 tri, cls, pad[2]} */
+    SDF_TABLE_VERTEX_MINTRI= 5   /* int32 [V]    lowest incident triangle id                     */
+};
+int sdf_get_table(sdf_mesh *m, int which, void *dst, size_t bytes);
+
+/* Release the handle and all its device memory (NULL is a no-op). */
+void sdf_destroy(sdf_mesh *m);
+
+/* Static string for a status code. */
+const char *sdf_strerror(int status);
+
+/* cudaError_t value of the last failing CUDA call seen by this library (0 if none). */
+int sdf_last_cuda_error(void);
+
+/* Library version, for the symbol / load test. */
+int sdf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PAPER_1903_00353_SDF_H */

@@ -1,0 +1,273 @@
+"""Thin ctypes binding over the C-ABI library of `include/sdf.h` (argument marshalling only).
+
+Same names as the C entry points: `sdf_create`, `sdf_compute`, `sdf_compute_host`,
+`sdf_stats`, `sdf_get_table`, `sdf_destroy`.  PyTorch supplies device memory (output
+tensors, and the library's workspace through torch's caching allocator) and the CUDA
+stream; every step of the method runs inside the library's kernels.  There is no CPU
+fallback: if the library is missing or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+STATUS_NAMES = {0: "SDF_OK", 1: "SDF_EINVAL", 2: "SDF_ENOTCLOSED", 3: "SDF_EORIENT",
+                4: "SDF_EDEGENERATE", 5: "SDF_ENOMEM", 6: "SDF_ECUDA"}
+SDF_OK, SDF_EINVAL, SDF_ENOTCLOSED, SDF_EORIENT, SDF_EDEGENERATE, SDF_ENOMEM, SDF_ECUDA = range(7)
+
+TABLE_CORNER_VID, TABLE_HALFEDGE_ADJ, TABLE_FACE_NORMAL, TABLE_VERTEX_REC, TABLE_EDGE_REC, \
+    TABLE_VERTEX_MINTRI = range(6)
+
+EXPORTS = ("sdf_create", "sdf_compute", "sdf_compute_host", "sdf_stats", "sdf_get_table",
+           "sdf_destroy", "sdf_strerror", "sdf_last_cuda_error", "sdf_version")
+
+VERTEX_REC_DTYPE = np.dtype([("pos", "<f4", 3), ("axis", "<f4", 3), ("cos_cone", "<f4"), ("info", "<i4")])
+EDGE_REC_DTYPE = np.dtype([("a", "<f4", 3), ("b", "<f4", 3), ("n1", "<f4", 3), ("n2", "<f4", 3),
+                           ("tri", "<i4"), ("cls", "<i4"), ("pad", "<i4", 2)])
+
+
+class SdfError(RuntimeError):
+    def __init__(self, status, where=""):
+        self.status = int(status)
+        msg = STATUS_NAMES.get(self.status, str(status))
+        try:
+            msg += ": " + lib().sdf_strerror(self.status).decode()
+            if self.status == SDF_ECUDA:
+                msg += " (cudaError %d)" % lib().sdf_last_cuda_error()
+        except Exception:
+            pass
+        super().__init__("%s failed with %s" % (where or "sdf call", msg))
+
+
+_ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
+_FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+
+class _Allocator(C.Structure):
+    _fields_ = [("alloc", _ALLOC_FN), ("free", _FREE_FN), ("user", C.c_void_p)]
+
+
+class Stats(C.Structure):
+    _fields_ = [(n, C.c_int64) for n in (
+        "F", "V", "E", "edges_convex", "edges_concave", "edges_flat",
+        "verts_pos_only", "verts_neg_only", "verts_both", "verts_skipped", "verts_hemisphere",
+        "weld_collisions", "polyhedra", "work_items", "pairs_tested", "pairs_accepted",
+        "bricks_active", "bricks_total", "band_cells", "fp64_rechecks")]
+
+    def as_dict(self):
+        return {n: int(getattr(self, n)) for n, _ in self._fields_}
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def lib():
+    """Load the shared library (building it with nvcc if the in-tree copy is missing or stale)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if os.environ.get("SDF_B200_NO_BUILD") != "1":
+        path = _build.build_library()
+    if not os.path.exists(path):
+        raise RuntimeError("CUDA library %s is missing; run `python -m paper_1903_00353_b200.build`" % path)
+    L = C.CDLL(path)
+    vp = C.c_void_p
+    L.sdf_create.argtypes = [vp, C.c_int64, C.c_int, C.POINTER(_Allocator), vp, C.POINTER(vp)]
+    L.sdf_create.restype = C.c_int
+    L.sdf_compute.argtypes = [vp, C.POINTER(C.c_float), C.c_float, C.c_int, C.c_int, C.c_int, C.c_float, vp, vp, vp]
+    L.sdf_compute.restype = C.c_int
+    L.sdf_compute_host.argtypes = L.sdf_compute.argtypes
+    L.sdf_compute_host.restype = C.c_int
+    L.sdf_stats.argtypes = [vp, C.POINTER(Stats)]
+    L.sdf_stats.restype = C.c_int
+    L.sdf_get_table.argtypes = [vp, C.c_int, vp, C.c_size_t]
+    L.sdf_get_table.restype = C.c_int
+    L.sdf_destroy.argtypes = [vp]
+    L.sdf_destroy.restype = None
+    L.sdf_strerror.argtypes = [C.c_int]
+    L.sdf_strerror.restype = C.c_char_p
+    L.sdf_last_cuda_error.argtypes = []
+    L.sdf_last_cuda_error.restype = C.c_int
+    L.sdf_version.argtypes = []
+    L.sdf_version.restype = C.c_int
+    _lib = L
+    return L
+
+
+# --------------------------------------------------------------------------------------
+# torch plumbing: device memory and streams only
+# --------------------------------------------------------------------------------------
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_1903_00353_b200 needs a CUDA device (there is no CPU fallback)")
+    return torch
+
+
+_torch_allocator = None
+
+
+def torch_allocator():
+    """sdf_allocator whose callbacks are torch's caching allocator."""
+    global _torch_allocator
+    if _torch_allocator is None:
+        torch = _torch()
+
+        def _alloc(nbytes, stream, user):
+            try:
+                return torch.cuda.caching_allocator_alloc(int(nbytes), stream=int(stream or 0))
+            except Exception:
+                return None
+
+        def _free(ptr, user):
+            if ptr:
+                torch.cuda.caching_allocator_delete(int(ptr))
+
+        a = _Allocator(_ALLOC_FN(_alloc), _FREE_FN(_free), None)
+        _torch_allocator = a
+    return _torch_allocator
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        return int(_torch().cuda.current_stream().cuda_stream)
+    if isinstance(stream, int):
+        return stream
+    return int(stream.cuda_stream)
+
+
+class Mesh:
+    """Owner of an `sdf_mesh*` handle."""
+
+    def __init__(self, handle, ntri):
+        self._h = handle
+        self.ntri = int(ntri)
+
+    def destroy(self):
+        if self._h:
+            lib().sdf_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    @property
+    def handle(self):
+        if not self._h:
+            raise RuntimeError("sdf_mesh already destroyed")
+        return self._h
+
+
+def sdf_create(tri_xyz, stream=None, use_torch_allocator=True) -> Mesh:
+    """tri_xyz: float32 [F,3,3] -- a torch CUDA tensor (device pointer, on_device=1) or a
+    numpy array / CPU tensor (host pointer, copied by the library)."""
+    L = lib()
+    torch = _torch()
+    if isinstance(tri_xyz, torch.Tensor):
+        t = tri_xyz.detach()
+        if t.dtype != torch.float32:
+            raise TypeError("tri_xyz must be float32")
+        t = t.contiguous()
+        ptr, on_dev, ntri, keep = t.data_ptr(), int(t.is_cuda), t.numel() // 9, t
+    else:
+        a = np.ascontiguousarray(tri_xyz, dtype=np.float32)
+        ptr, on_dev, ntri, keep = a.ctypes.data, 0, a.size // 9, a
+    if keep is not None and (keep.size if isinstance(keep, np.ndarray) else keep.numel()) != 9 * ntri:
+        raise ValueError("tri_xyz must hold 9 floats per triangle")
+    out = C.c_void_p()
+    alloc = C.byref(torch_allocator()) if use_torch_allocator else None
+    st = L.sdf_create(C.c_void_p(ptr), ntri, on_dev, alloc, C.c_void_p(_stream_ptr(stream)), C.byref(out))
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_create")
+    return Mesh(out, ntri)
+
+
+def _origin3(origin):
+    o = (C.c_float * 3)(*[float(v) for v in origin])
+    return o
+
+
+def sdf_compute(mesh: Mesh, origin, h, dims, band, dist_out=None, tri_out=None, stream=None):
+    """Returns (dist float32 [nz,ny,nx], tri int32 [nz,ny,nx]) CUDA tensors."""
+    L = lib()
+    torch = _torch()
+    nx, ny, nz = (int(v) for v in dims)
+    if dist_out is None:
+        dist_out = torch.empty((nz, ny, nx), dtype=torch.float32, device="cuda")
+    if tri_out is None:
+        tri_out = torch.empty((nz, ny, nx), dtype=torch.int32, device="cuda")
+    assert dist_out.is_cuda and tri_out.is_cuda and dist_out.is_contiguous() and tri_out.is_contiguous()
+    assert dist_out.numel() == nx * ny * nz and tri_out.numel() == nx * ny * nz
+    assert dist_out.dtype == torch.float32 and tri_out.dtype == torch.int32
+    st = L.sdf_compute(mesh.handle, _origin3(origin), float(h), nx, ny, nz, float(band),
+                       C.c_void_p(dist_out.data_ptr()), C.c_void_p(tri_out.data_ptr()),
+                       C.c_void_p(_stream_ptr(stream)))
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_compute")
+    return dist_out, tri_out
+
+
+def sdf_compute_host(mesh: Mesh, origin, h, dims, band, dist_out=None, tri_out=None, stream=None):
+    """Host-buffer variant: dist_out / tri_out are CPU tensors (pinned recommended)."""
+    L = lib()
+    torch = _torch()
+    nx, ny, nz = (int(v) for v in dims)
+    if dist_out is None:
+        dist_out = torch.empty((nz, ny, nx), dtype=torch.float32, pin_memory=True)
+    if tri_out is None:
+        tri_out = torch.empty((nz, ny, nx), dtype=torch.int32, pin_memory=True)
+    assert not dist_out.is_cuda and not tri_out.is_cuda
+    assert dist_out.numel() == nx * ny * nz and tri_out.numel() == nx * ny * nz
+    st = L.sdf_compute_host(mesh.handle, _origin3(origin), float(h), nx, ny, nz, float(band),
+                            C.c_void_p(dist_out.data_ptr()), C.c_void_p(tri_out.data_ptr()),
+                            C.c_void_p(_stream_ptr(stream)))
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_compute_host")
+    return dist_out, tri_out
+
+
+def sdf_stats(mesh: Mesh) -> dict:
+    s = Stats()
+    st = lib().sdf_stats(mesh.handle, C.byref(s))
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_stats")
+    return s.as_dict()
+
+
+def sdf_get_table(mesh: Mesh, which: int) -> np.ndarray:
+    s = sdf_stats(mesh)
+    F, V, E = s["F"], s["V"], s["E"]
+    shape_dtype = {
+        TABLE_CORNER_VID: ((F, 3), np.int32), TABLE_HALFEDGE_ADJ: ((F, 3), np.int32),
+        TABLE_FACE_NORMAL: ((F, 3), np.float32), TABLE_VERTEX_REC: ((V,), VERTEX_REC_DTYPE),
+        TABLE_EDGE_REC: ((E,), EDGE_REC_DTYPE), TABLE_VERTEX_MINTRI: ((V,), np.int32)}[which]
+    out = np.empty(shape_dtype[0], dtype=shape_dtype[1])
+    st = lib().sdf_get_table(mesh.handle, which, C.c_void_p(out.ctypes.data), out.nbytes)
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_get_table")
+    return out
+
+
+def sdf_destroy(mesh: Mesh):
+    mesh.destroy()
+
+
+def compute_workload(w, host_soup=False, stream=None):
+    """Convenience for tests / bench: sdf_create + sdf_compute on a `Workload`."""
+    torch = _torch()
+    soup = w.soup if host_soup else torch.from_numpy(np.ascontiguousarray(w.soup)).cuda()
+    m = sdf_create(soup, stream=stream)
+    d, t = sdf_compute(m, w.origin, w.h, w.dims, w.band, stream=stream)
+    return m, d, t

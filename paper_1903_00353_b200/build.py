@@ -1,0 +1,61 @@
+"""Build the CUDA C-ABI library (`libsdf_b200.so`) in-tree with nvcc for sm_100a.
+
+    python -m paper_1903_00353_b200.build [--force]
+
+nvcc cross-compiles without a GPU.  The shared object sits next to this file (it is
+git-ignored but travels to the GPU box with the repository snapshot).
+"""
+from __future__ import annotations
+
+import os
+import subprocess
+import sys
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(_HERE, "csrc")
+LIB = os.path.join(_HERE, "libsdf_b200.so")
+SOURCES = ["api.cu", "features.cu", "compute.cu"]
+HEADERS = ["common.cuh", "primitives.cuh", os.path.join("..", "..", "include", "sdf.h")]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+              "-Xcompiler", "-fPIC", "-shared", "--cudart", "static"]
+
+
+def _nvcc() -> str:
+    for cand in (os.environ.get("NVCC"), "/usr/local/cuda/bin/nvcc", "nvcc"):
+        if cand and (os.path.isabs(cand) and os.path.exists(cand) or not os.path.isabs(cand)):
+            return cand
+    return "nvcc"
+
+
+def source_hash() -> str:
+    """Content hash of everything the library is built from (mtimes do not survive the
+    snapshot copy to the GPU box)."""
+    import hashlib
+    h = hashlib.sha256()
+    h.update(" ".join(NVCC_FLAGS).encode())
+    for s in SOURCES + HEADERS:
+        with open(os.path.join(CSRC, s), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()
+
+
+def needs_build() -> bool:
+    if not os.path.exists(LIB) or not os.path.exists(LIB + ".hash"):
+        return True
+    with open(LIB + ".hash") as f:
+        return f.read().strip() != source_hash()
+
+
+def build_library(force: bool = False, verbose: bool = False) -> str:
+    if not force and not needs_build():
+        return LIB
+    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+          ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    subprocess.check_call(cmd)
+    with open(LIB + ".hash", "w") as f:
+        f.write(source_hash())
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build_library(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -1,0 +1,195 @@
+// api.cu -- the C ABI of include/sdf.h: argument checks, handle lifetime, allocator plumbing.
+#include "common.cuh"
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+
+int g_last_cuda_error = 0;
+
+int dev_alloc(const sdf_allocator *a, void **p, size_t bytes, cudaStream_t st) {
+    *p = nullptr;
+    if (bytes == 0) bytes = 16;
+    if (a && a->alloc) {
+        *p = a->alloc(bytes, (void *)st, a->user);
+        return *p ? SDF_OK : SDF_ENOMEM;
+    }
+    cudaError_t e = cudaMallocAsync(p, bytes, st);
+    if (e != cudaSuccess) {
+        g_last_cuda_error = (int)e;
+        (void)cudaGetLastError();
+        *p = nullptr;
+        return e == cudaErrorMemoryAllocation ? SDF_ENOMEM : SDF_ECUDA;
+    }
+    return SDF_OK;
+}
+
+void dev_free(const sdf_allocator *a, void *p, cudaStream_t st) {
+    if (!p) return;
+    if (a && a->alloc) { a->free(p, a->user); return; }
+    cudaFreeAsync(p, st);
+}
+
+static int have_device() {
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || n <= 0) {
+        g_last_cuda_error = (int)(e != cudaSuccess ? e : cudaErrorNoDevice);
+        (void)cudaGetLastError();
+        return 0;
+    }
+    return 1;
+}
+
+extern "C" {
+
+int sdf_version(void) { return 100; }
+int sdf_last_cuda_error(void) { return g_last_cuda_error; }
+
+const char *sdf_strerror(int s) {
+    switch (s) {
+    case SDF_OK: return "ok";
+    case SDF_EINVAL: return "invalid argument or non-finite input";
+    case SDF_ENOTCLOSED: return "surface not closed: an edge without exactly two triangles";
+    case SDF_EORIENT: return "inconsistent orientation: an edge traversed twice in the same direction";
+    case SDF_EDEGENERATE: return "degenerate triangle (zero area or repeated vertex)";
+    case SDF_ENOMEM: return "out of memory";
+    case SDF_ECUDA: return "CUDA error or no CUDA device";
+    default: return "unknown status";
+    }
+}
+
+void sdf_destroy(sdf_mesh *m) {
+    if (!m) return;
+    cudaStream_t st = m->last_stream;
+    cudaStreamSynchronize(st);
+    void *ptrs[] = {m->soup, m->fn, m->cvid, m->adj, m->vmint, m->vrec, m->erec, m->d_ctr, m->d_flags, m->hdr,
+                    m->offsets, m->scan_ws, m->brick_flag, m->brick_table, m->scratch};
+    for (size_t i = 0; i < sizeof(ptrs) / sizeof(ptrs[0]); i++) dev_free(&m->alloc, ptrs[i], st);
+    m->~sdf_mesh();
+    free(m);
+}
+
+int sdf_create(const float *tri_xyz, int64_t ntri, int on_device, const sdf_allocator *a, void *stream,
+               sdf_mesh **out) {
+    if (out) *out = nullptr;
+    if (!tri_xyz || !out || ntri <= 0 || ntri > ((int64_t)1 << 29)) return SDF_EINVAL;
+    if (a && (!a->alloc || !a->free)) return SDF_EINVAL;
+    if (!have_device()) return SDF_ECUDA;
+    void *mem = calloc(1, sizeof(sdf_mesh));
+    if (!mem) return SDF_ENOMEM;
+    sdf_mesh *m = new (mem) sdf_mesh;
+    memset(m, 0, sizeof(*m));
+    if (a) m->alloc = *a;
+    m->F = ntri;
+    m->last_stream = (cudaStream_t)stream;
+    int s = build_features(m, tri_xyz, on_device, (cudaStream_t)stream);
+    if (s != SDF_OK) {
+        sdf_destroy(m);
+        return s;
+    }
+    *out = m;
+    return SDF_OK;
+}
+
+static int make_grid(const float origin[3], float h, int nx, int ny, int nz, float band, const float *dist,
+                     const int32_t *tri, GridParams *g) {
+    if (!origin || !(h > 0.0f) || !(band > 0.0f) || !isfinite(h) || !isfinite(band)) return SDF_EINVAL;
+    if (nx <= 0 || ny <= 0 || nz <= 0 || nx > 32767 || ny > 32767 || nz > 32767) return SDF_EINVAL;
+    if (!isfinite(origin[0]) || !isfinite(origin[1]) || !isfinite(origin[2])) return SDF_EINVAL;
+    memset(g, 0, sizeof(*g));
+    g->ox = origin[0]; g->oy = origin[1]; g->oz = origin[2]; g->h = h;
+    g->dox = origin[0]; g->doy = origin[1]; g->doz = origin[2]; g->dh = h;
+    g->nx = nx; g->ny = ny; g->nz = nz;
+    g->nbx = (nx + BRICK - 1) / BRICK; g->nby = (ny + BRICK - 1) / BRICK; g->nbz = (nz + BRICK - 1) / BRICK;
+    g->band = band; g->dband = band;
+    // eps: tolerance of every inclusion test, the upper value of PAPER.md:386 (1e-3 dx)
+    g->eps = 1e-3f * h;
+    // guard: bound on the fp32 error of an evaluated distance; cells with |d - band| < guard
+    // are decided in fp64 by the emit pass
+    float maxabs = 0.0f;
+    const int n[3] = {nx, ny, nz};
+    for (int i = 0; i < 3; i++) {
+        float lo = fabsf(origin[i]), hi = fabsf(origin[i] + (n[i] - 1) * h);
+        maxabs = fmaxf(maxabs, fmaxf(lo, hi));
+    }
+    g->guard = 1e-3f * h + 1e-6f * maxabs;
+    g->rb = band + g->guard + g->eps;
+    const char *dbg = getenv("SDF_AABB_MODE");
+    g->aabb_mode = (dbg && dbg[0] == '1') ? 1 : 0;
+    g->vec4 = (nx % 4 == 0) && (((uintptr_t)dist & 15) == 0) && (((uintptr_t)tri & 15) == 0);
+    return SDF_OK;
+}
+
+int sdf_compute(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz, float band, float *dist_out,
+                int32_t *tri_out, void *stream) {
+    if (!m || !dist_out || !tri_out) return SDF_EINVAL;
+    GridParams g;
+    CKS(make_grid(origin, h, nx, ny, nz, band, dist_out, tri_out, &g));
+    return run_compute(m, g, dist_out, tri_out, (cudaStream_t)stream);
+}
+
+int sdf_compute_host(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz, float band,
+                     float *dist_out_host, int32_t *tri_out_host, void *stream) {
+    if (!m || !dist_out_host || !tri_out_host) return SDF_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    GridParams g;
+    CKS(make_grid(origin, h, nx, ny, nz, band, nullptr, nullptr, &g));
+    size_t n = (size_t)nx * ny * nz;
+    float *dd = nullptr;
+    int32_t *dt = nullptr;
+    int s = dev_alloc(&m->alloc, (void **)&dd, n * sizeof(float), st);
+    if (s == SDF_OK) s = dev_alloc(&m->alloc, (void **)&dt, n * sizeof(int32_t), st);
+    if (s == SDF_OK) s = run_compute(m, g, dd, dt, st);
+    if (s == SDF_OK) {
+        cudaError_t e = cudaMemcpyAsync(dist_out_host, dd, n * sizeof(float), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(tri_out_host, dt, n * sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { g_last_cuda_error = (int)e; (void)cudaGetLastError(); s = SDF_ECUDA; }
+    }
+    dev_free(&m->alloc, dd, st);
+    dev_free(&m->alloc, dt, st);
+    return s;
+}
+
+int sdf_stats(sdf_mesh *m, sdf_stats_t *o) {
+    if (!m || !o) return SDF_EINVAL;
+    CK(cudaStreamSynchronize(m->last_stream));
+    CK(cudaMemcpy(m->h_ctr, m->d_ctr, sizeof(u64) * CTR_COUNT, cudaMemcpyDeviceToHost));
+    const u64 *c = m->h_ctr;
+    memset(o, 0, sizeof(*o));
+    o->F = m->F; o->V = m->V; o->E = m->E;
+    o->edges_convex = (int64_t)c[CTR_E_CONVEX]; o->edges_concave = (int64_t)c[CTR_E_CONCAVE];
+    o->edges_flat = (int64_t)c[CTR_E_FLAT];
+    o->verts_pos_only = (int64_t)c[CTR_V_POS]; o->verts_neg_only = (int64_t)c[CTR_V_NEG];
+    o->verts_both = (int64_t)c[CTR_V_BOTH]; o->verts_skipped = (int64_t)c[CTR_V_SKIP];
+    o->verts_hemisphere = (int64_t)c[CTR_V_HEMI];
+    o->weld_collisions = (int64_t)c[CTR_WELD_BAD];
+    o->polyhedra = (int64_t)c[CTR_POLY]; o->work_items = (int64_t)c[CTR_ITEMS];
+    o->pairs_tested = (int64_t)c[CTR_TESTED]; o->pairs_accepted = (int64_t)c[CTR_ACCEPTED];
+    o->bricks_active = (int64_t)c[CTR_BRICKS];
+    o->bricks_total = m->last_bricks_total;
+    o->band_cells = (int64_t)c[CTR_BAND]; o->fp64_rechecks = (int64_t)c[CTR_RECHECK];
+    return SDF_OK;
+}
+
+int sdf_get_table(sdf_mesh *m, int which, void *dst, size_t bytes) {
+    if (!m || !dst) return SDF_EINVAL;
+    const void *src = nullptr;
+    size_t need = 0;
+    switch (which) {
+    case SDF_TABLE_CORNER_VID: src = m->cvid; need = sizeof(int) * 3 * (size_t)m->F; break;
+    case SDF_TABLE_HALFEDGE_ADJ: src = m->adj; need = sizeof(int) * 3 * (size_t)m->F; break;
+    case SDF_TABLE_FACE_NORMAL: src = m->fn; need = sizeof(float) * 3 * (size_t)m->F; break;
+    case SDF_TABLE_VERTEX_REC: src = m->vrec; need = sizeof(VertexRec) * (size_t)m->V; break;
+    case SDF_TABLE_EDGE_REC: src = m->erec; need = sizeof(EdgeRec) * (size_t)m->E; break;
+    case SDF_TABLE_VERTEX_MINTRI: src = m->vmint; need = sizeof(int) * (size_t)m->V; break;
+    default: return SDF_EINVAL;
+    }
+    if (bytes != need || !src) return SDF_EINVAL;
+    CK(cudaStreamSynchronize(m->last_stream));
+    CK(cudaMemcpy(dst, src, need, cudaMemcpyDeviceToHost));
+    return SDF_OK;
+}
+
+} // extern "C"

@@ -1,0 +1,121 @@
+// common.cuh -- shared declarations of the CUDA path (sm_100a).
+// Shares nothing with oracle/ (the CPU oracle is test infrastructure).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/sdf.h"
+
+typedef unsigned int u32;
+typedef unsigned long long u64;
+
+// ---------------------------------------------------------------------------------------
+// error handling: every CUDA call goes through CK(); the first failure is remembered
+// ---------------------------------------------------------------------------------------
+extern int g_last_cuda_error;
+#define CK(call)                                                   \
+    do {                                                           \
+        cudaError_t e__ = (call);                                  \
+        if (e__ != cudaSuccess) {                                  \
+            g_last_cuda_error = (int)e__;                          \
+            (void)cudaGetLastError();                              \
+            return (e__ == cudaErrorMemoryAllocation) ? SDF_ENOMEM : SDF_ECUDA; \
+        }                                                          \
+    } while (0)
+#define CKS(expr)                                                  \
+    do {                                                           \
+        int s__ = (expr);                                          \
+        if (s__ != SDF_OK) return s__;                             \
+    } while (0)
+
+// error bits raised by device code (sdf_mesh::d_flags[0])
+enum { ERRB_NONFINITE = 1, ERRB_NOTCLOSED = 2, ERRB_ORIENT = 4, ERRB_DEGENERATE = 8 };
+
+// device counters (sdf_mesh::d_ctr), 64-bit each
+enum {
+    CTR_V = 0, CTR_WELD_BAD, CTR_E_CONVEX, CTR_E_CONCAVE, CTR_E_FLAT,
+    CTR_V_POS, CTR_V_NEG, CTR_V_BOTH, CTR_V_SKIP, CTR_V_HEMI,
+    CTR_POLY, CTR_ITEMS, CTR_BRICKS, CTR_TESTED, CTR_ACCEPTED, CTR_BAND, CTR_RECHECK,
+    CTR_COUNT = 24
+};
+
+// ---------------------------------------------------------------------------------------
+// feature tables (HBM layout)
+// ---------------------------------------------------------------------------------------
+// Band-independent part of an edge wedge: end points in the direction the
+// half-edge is traversed in triangle t0 (normal n1), n2 = normal of the opposite triangle.
+struct __align__(16) EdgeRec {
+    float a[3], b[3], n1[3], n2[3];
+    int tri;     // min(t0, t1): the id written for cells closest to this edge
+    int cls;     // +1 convex, -1 concave, 0 flat (no wedge)
+    int pad[2];
+};
+static_assert(sizeof(EdgeRec) == 64, "EdgeRec must be 64 B");
+
+// Band-independent part of a vertex cone: apex, unit pseudonormal axis
+// (eq.8), cosine of the half angle (eq.9), info bits.
+struct __align__(16) VertexRec {
+    float pos[3], axis[3];
+    float cos_cone;
+    int info;    // bit0: emit +axis side, bit1: emit -axis side, bit2: hemisphere (ruff)
+};
+static_assert(sizeof(VertexRec) == 32, "VertexRec must be 32 B");
+
+// Band- and grid-dependent header of one polyhedron: its bounding volume in cell indices
+// clipped to the grid and the number of grid rows (j,k) it covers.
+struct __align__(16) PolyHdr {
+    short i0, i1, j0, j1, k0, k1;
+    u32 rows;
+};
+static_assert(sizeof(PolyHdr) == 16, "PolyHdr must be 16 B");
+
+#define BRICK 8                      // scratch bricks are 8x8x8 cells
+#define BRICK_CELLS 512
+#define PACK_EMPTY 0xFFFFFFFFFFFFFFFFull
+
+struct GridParams {
+    float ox, oy, oz, h;
+    double dox, doy, doz, dh;       // same values promoted (fp64 re-check paths)
+    int nx, ny, nz;
+    int nbx, nby, nbz;              // bricks per axis
+    float band, eps, guard, rb;     // rb = band + guard + eps : reach of every polyhedron
+    double dband;
+    int aabb_mode;                  // debug: candidates = band-expanded triangle AABBs only
+    int vec4;                       // 1: nx % 4 == 0 and outputs 16-B aligned -> 128-bit stores
+};
+
+// ---------------------------------------------------------------------------------------
+// handle
+// ---------------------------------------------------------------------------------------
+struct sdf_mesh {
+    sdf_allocator alloc;     // copied; alloc.alloc == nullptr -> cudaMallocAsync
+    int64_t F, E, V;
+    // feature tables (device)
+    float *soup;             // [F][9] canonicalised copy of the input
+    float *fn;               // [F][3] unit face normals
+    int *cvid;               // [3F]
+    int *adj;                // [3F]
+    int *vmint;              // [V]
+    VertexRec *vrec;         // [V]
+    EdgeRec *erec;           // [E]
+    u64 *d_ctr;              // [CTR_COUNT]
+    int *d_flags;            // [4]
+    // persistent per-compute workspace (grown on demand)
+    PolyHdr *hdr;  size_t hdr_cap;         // [F + E + 2V]
+    u64 *offsets;  size_t offsets_cap;     // [P + 1]
+    u64 *scan_ws;  size_t scan_ws_cap;
+    unsigned char *brick_flag; size_t brick_flag_cap;
+    int *brick_table; size_t brick_table_cap;
+    u64 *scratch;  size_t scratch_cap;     // bricks * 512 packed values
+    u64 h_ctr[CTR_COUNT];
+    int64_t last_bricks_total;
+    cudaStream_t last_stream;
+};
+
+// allocation through the handle's allocator
+int dev_alloc(const sdf_allocator *a, void **p, size_t bytes, cudaStream_t st);
+void dev_free(const sdf_allocator *a, void *p, cudaStream_t st);
+
+// stages (features.cu / compute.cu)
+int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st);
+int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st);
