@@ -1,0 +1,337 @@
+#!/usr/bin/env python
+"""bench.py -- narrow-band SDF throughput of the CSC hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one mesh+grid: sdf_create (A0-A4: weld,
+edge table, pseudonormals, classes) + sdf_compute (A5-A8: extrude, scan-convert, evaluate +
+min-combine, sign + emit) through the C ABI.  Default workload: BASELINE.json config C4
+(3,996,000-triangle star surface, 1024^3 grid, band 2h), the one north_star quotes the
+target on.  `value` = populated band cells / step time with the soup and both output grids
+resident in HBM; `e2e` = same metric with HOST buffers (pinned soup in, pinned grids out).
+
+The path does not shard (north_star: one GPU): --gpus N under torchrun runs N independent
+replicas, no collective on the data path ("replicas only").
+
+--impl reference times the CPU oracle (oracle/) on the host cores on a bounded z-slab
+sample of the same workload.  Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1903_00353_b200 import workloads as W  # noqa: E402
+
+METRIC = "narrow_band_sdf_cells_per_s"
+UNIT = "band cells/s"
+L2_BYTES = 126 * 1024 * 1024
+
+
+# --------------------------------------------------------------------------------------- #
+# helpers
+# --------------------------------------------------------------------------------------- #
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is not None:
+            self.p.terminate()
+            try:
+                self.p.wait(timeout=5)
+            except Exception:
+                self.p.kill()
+        try:
+            self.f.flush()
+            with open(self.f.name) as f:
+                rows = [r.strip().split(", ") for r in f if r.strip()]
+            os.unlink(self.f.name)
+        except Exception:
+            rows = []
+        sm, smax, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in rows:
+            if len(r) < 9:
+                continue
+            try:
+                sm.append(float(r[1]))
+                smax.append(float(r[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, r[5:9]):
+                if v.strip().lower() == "active":
+                    reasons.add(n)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(smax)), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def sample_slab(w, nslices):
+    """Bounded sample of the workload for the oracle: the central z-slab of `nslices` slices."""
+    nx, ny, nz = w.dims
+    ns = min(nslices, nz)
+    k0 = (nz - ns) // 2
+    return w.crop((0, 0, k0), (nx, ny, ns)), "central z-slab k in [%d,%d) of %d slices, full mesh" % (k0, k0 + ns, nz)
+
+
+# --------------------------------------------------------------------------------------- #
+# reference arm: the CPU oracle, as it stands, on the host cores
+# --------------------------------------------------------------------------------------- #
+def time_oracle(w, nslices, steps, warmup):
+    import oracle
+    oracle.build()
+    cores = oracle.default_threads()
+    t0 = time.perf_counter()
+    om = oracle.Mesh(w.soup)
+    build_s = time.perf_counter() - t0
+    c, what = sample_slab(w, nslices)
+    cells = 0
+    for _ in range(warmup):
+        om.sdf(c.origin, c.h, c.dims, c.band, cores)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        d, _t = om.sdf(c.origin, c.h, c.dims, c.band, cores)
+    dt = (time.perf_counter() - t0) / max(steps, 1)
+    cells = int(np.isfinite(d).sum())
+    return {"value": cells / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": what + "; %d band cells per step in %.2f s; one-off connectivity build %.1f s not included"
+                      % (cells, dt, build_s),
+            "build_s": build_s, "s_per_step": dt, "band_cells": cells}
+
+
+def run_reference(args):
+    rank, _lr, world = dist_env()
+    if rank != 0:
+        return
+    w = W.config(args.config)
+    r = time_oracle(w, args.ref_slices, args.steps, args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["s_per_step"] * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(w, args),
+            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(w, args):
+    nx, ny, nz = w.dims
+    return {"workload": "%s: %d triangles, grid %dx%dx%d, h=%g, band %gh (BASELINE.json configs[%d])"
+                        % (w.name, w.ntri, nx, ny, nz, w.h, w.band / w.h, W.CONFIG_NAMES.index(w.name)),
+            "triangles": w.ntri, "grid": [nx, ny, nz], "band_cells": w.band / w.h,
+            "parallelism": "replicas only (the path does not shard)" if args.gpus > 1 else "1 GPU",
+            "l2": "no flush needed: each step streams %.2f GB of output > %d MB L2"
+                  % (8.0 * w.ncells / 1e9, L2_BYTES >> 20)}
+
+
+# --------------------------------------------------------------------------------------- #
+# our arm: the CUDA path through the C ABI
+# --------------------------------------------------------------------------------------- #
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1903_00353_b200 import binding as B
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local_rank % torch.cuda.device_count())
+    dev = torch.device("cuda", torch.cuda.current_device())
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    w = W.config(args.config)
+    nx, ny, nz = w.dims
+    N = w.ncells
+    soup_host = torch.from_numpy(np.ascontiguousarray(w.soup)).pin_memory()
+    soup_dev = soup_host.to(dev)
+    dist_out = torch.empty((nz, ny, nx), dtype=torch.float32, device=dev)
+    tri_out = torch.empty((nz, ny, nx), dtype=torch.int32, device=dev)
+    need_flush = 8 * N < 2 * L2_BYTES
+    flush_buf = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev) if need_flush else None
+    stream = torch.cuda.current_stream()
+
+    def step_device():
+        m = B.sdf_create(soup_dev, stream=stream)
+        B.sdf_compute(m, w.origin, w.h, w.dims, w.band, dist_out, tri_out, stream=stream)
+        return m
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- warm-up (also sizes torch's caching allocator pools)
+    for _ in range(max(args.warmup, 0)):
+        step_device().destroy()
+    # ---- timed: K steps, device-resident inputs and outputs
+    B.sdf_enable_timing(True)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    stage_sum, stats = {}, None
+    clocks = ClockSampler(torch.cuda.current_device())
+    barrier()
+    clocks.start()
+    l0 = B.sdf_launch_count()
+    t_wall = time.perf_counter()
+    for i in range(args.steps):
+        if flush_buf is not None:
+            flush_buf.zero_()
+        ev[i][0].record(stream)
+        m = step_device()
+        ev[i][1].record(stream)
+        for k, v in B.sdf_get_timings(m).items():        # synchronises the stream
+            stage_sum[k] = stage_sum.get(k, 0.0) + v
+        if i == args.steps - 1:
+            stats = B.sdf_stats(m)
+        m.destroy()
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    launches = B.sdf_launch_count() - l0
+    clk = clocks.stop()
+    B.sdf_enable_timing(False)
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(step_ms))
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    band_cells = int(stats["band_cells"])
+    value = world * band_cells / (ms_per_step * 1e-3)
+
+    # ---- end to end: HOST buffers through the C ABI (H2D of the soup, D2H of both grids)
+    e2e = None
+    if not args.no_e2e:
+        dist_host = torch.empty((nz, ny, nx), dtype=torch.float32, pin_memory=True)
+        tri_host = torch.empty((nz, ny, nx), dtype=torch.int32, pin_memory=True)
+        soup_np = soup_host.numpy()
+
+        def step_host():
+            m = B.sdf_create(soup_np, stream=stream)                 # host pointer: copied by the library
+            B.sdf_compute_host(m, w.origin, w.h, w.dims, w.band, dist_host, tri_host, stream=stream)
+            m.destroy()
+
+        step_host()
+        ne = max(1, min(args.steps, args.e2e_steps))
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(ne):
+            step_host()
+        e1.record(stream)
+        barrier()
+        e_ms = e0.elapsed_time(e1) / ne
+        if world > 1:
+            t = torch.tensor([e_ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e_ms = float(t.item())
+        assert int(torch.isfinite(dist_host).sum()) == band_cells
+        e2e = {"value": world * band_cells / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": e_ms, "steps": ne,
+               "h2d_bytes_per_step": int(soup_host.numel() * 4), "d2h_bytes_per_step": int(8 * N)}
+        del dist_host, tri_host
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (stage durations from CUDA events on the launch stream)
+    peak, peak_src = measured_peaks()
+    stage_ms = {k: v / args.steps for k, v in stage_sum.items()}
+    dom = max(stage_ms, key=stage_ms.get)
+    alg_bytes = {"emit": 8.0 * N,                                   # 8 B per cell, written once
+                 "ingest_weld": 36.0 * w.ntri, "edges": 36.0 * w.ntri, "vertices": 36.0 * w.ntri}
+    emit_gbs = 8.0 * N / (stage_ms["emit"] * 1e-3) / 1e9 if stage_ms.get("emit") else 0.0
+    roofline = {"bound": "hbm", "kernel": "emit_kernel (A8 sign + dense write)", "achieved": emit_gbs, "peak": peak,
+                "unit": "GB/s", "frac": emit_gbs / peak, "traffic": args.traffic,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": 8.0 * N,
+                "ms_per_launch": stage_ms.get("emit"), "dominant_stage": dom}
+    step_bytes = 8.0 * N + 36.0 * w.ntri
+    roofline_step = {"bound": "hbm", "algorithmic_bytes": step_bytes, "ideal_ms": step_bytes / (peak * 1e9) * 1e3,
+                     "frac": step_bytes / (peak * 1e9) * 1e3 / ms_per_step}
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        r = time_oracle(w, args.cpu_slices, 1, 0)
+        cpu = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(w, args),
+            "band_cells": band_cells, "stage_ms": stage_ms, "step_ms_min": min(step_ms), "wall_ms_per_step":
+            t_wall * 1e3 / args.steps, "roofline": roofline, "roofline_step": roofline_step, "cpu_baseline": cpu,
+            "e2e": e2e, "gpu_launches": int(launches), "clocks": clk,
+            "stats": {k: stats[k] for k in ("polyhedra", "work_items", "pairs_tested", "pairs_accepted",
+                                            "bricks_active", "fp64_rechecks")}}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C4", choices=list(W.CONFIG_NAMES))
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-slices", type=int, default=256, help="z-slices of the oracle sample (cpu_baseline)")
+    ap.add_argument("--ref-slices", type=int, default=64, help="z-slices per step of --impl reference")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram bytes per emit launch from the committed ncu --set full capture (profiles/)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -147,6 +147,30 @@ enum {
 };
 int sdf_get_table(sdf_mesh *m, int which, void *dst, size_t bytes);
 
+/*
+ * Stage timing (measurement support).  sdf_enable_timing(1) makes every
+ * later sdf_create / sdf_compute record CUDA events around its stages ON THE STREAM IT WAS
+ * GIVEN (no extra synchronisation); sdf_get_timings synchronises that stream and returns
+ * the durations, in milliseconds, of the stages of the handle's sdf_create and of its last
+ * sdf_compute.  ms: HOST array of SDF_T_COUNT floats (n must equal SDF_T_COUNT); a stage
+ * that did not run reports 0.
+ */
+enum {
+    SDF_T_INGEST_WELD = 0,  /* A0+A1: copy/canonicalise, hash keys, radix sort, weld ids        */
+    SDF_T_EDGES       = 1,  /* A2+A3: triangle geometry, half-edge sort, pairing, edge classes  */
+    SDF_T_VERTICES    = 2,  /* A3+A4: pseudonormals, cone angles, vertex classes                */
+    SDF_T_CLIP_SCAN   = 3,  /* A5+A6: clip polyhedra, row counts, prefix sums, brick table      */
+    SDF_T_CLEAR       = 4,  /* scratch bricks reset to "empty"                                  */
+    SDF_T_EVALUATE    = 5,  /* A7: work items -> distances -> packed atomicMin                  */
+    SDF_T_EMIT        = 6,  /* A8: sign + dense write of both grids                             */
+    SDF_T_COUNT       = 7
+};
+int sdf_enable_timing(int on);
+int sdf_get_timings(sdf_mesh *m, float *ms, int n);
+
+/* Number of CUDA kernels this library has launched in this process so far. */
+int64_t sdf_launch_count(void);
+
 /* Release the handle and all its device memory (NULL is a no-op). */
 void sdf_destroy(sdf_mesh *m);
 

@@ -23,7 +23,10 @@ TABLE_CORNER_VID, TABLE_HALFEDGE_ADJ, TABLE_FACE_NORMAL, TABLE_VERTEX_REC, TABLE
     TABLE_VERTEX_MINTRI = range(6)
 
 EXPORTS = ("sdf_create", "sdf_compute", "sdf_compute_host", "sdf_stats", "sdf_get_table",
-           "sdf_destroy", "sdf_strerror", "sdf_last_cuda_error", "sdf_version")
+           "sdf_destroy", "sdf_strerror", "sdf_last_cuda_error", "sdf_version",
+           "sdf_enable_timing", "sdf_get_timings", "sdf_launch_count")
+
+TIMING_STAGES = ("ingest_weld", "edges", "vertices", "clip_scan", "clear", "evaluate", "emit")
 
 VERTEX_REC_DTYPE = np.dtype([("pos", "<f4", 3), ("axis", "<f4", 3), ("cos_cone", "<f4"), ("info", "<i4")])
 EDGE_REC_DTYPE = np.dtype([("a", "<f4", 3), ("b", "<f4", 3), ("n1", "<f4", 3), ("n2", "<f4", 3),
@@ -99,6 +102,12 @@ def lib():
     L.sdf_last_cuda_error.restype = C.c_int
     L.sdf_version.argtypes = []
     L.sdf_version.restype = C.c_int
+    L.sdf_enable_timing.argtypes = [C.c_int]
+    L.sdf_enable_timing.restype = C.c_int
+    L.sdf_get_timings.argtypes = [vp, C.POINTER(C.c_float), C.c_int]
+    L.sdf_get_timings.restype = C.c_int
+    L.sdf_launch_count.argtypes = []
+    L.sdf_launch_count.restype = C.c_int64
     _lib = L
     return L
 
@@ -258,6 +267,23 @@ def sdf_get_table(mesh: Mesh, which: int) -> np.ndarray:
     if st != SDF_OK:
         raise SdfError(st, "sdf_get_table")
     return out
+
+
+def sdf_enable_timing(on: bool):
+    lib().sdf_enable_timing(1 if on else 0)
+
+
+def sdf_get_timings(mesh: Mesh) -> dict:
+    """Stage durations (ms) of the handle's sdf_create and its last sdf_compute."""
+    ms = (C.c_float * len(TIMING_STAGES))()
+    st = lib().sdf_get_timings(mesh.handle, ms, len(TIMING_STAGES))
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_get_timings")
+    return {k: float(ms[i]) for i, k in enumerate(TIMING_STAGES)}
+
+
+def sdf_launch_count() -> int:
+    return int(lib().sdf_launch_count())
 
 
 def sdf_destroy(mesh: Mesh):

@@ -6,6 +6,19 @@
 #include <new>
 
 int g_last_cuda_error = 0;
+int g_timing = 0;
+long long g_launch_count = 0;
+
+void stage_mark(sdf_mesh *m, int stage, int which, cudaStream_t st) {
+    if (!g_timing) return;
+    if (!m->ev[stage][which] && cudaEventCreate(&m->ev[stage][which]) != cudaSuccess) {
+        m->ev[stage][which] = nullptr;
+        (void)cudaGetLastError();
+        return;
+    }
+    cudaEventRecord(m->ev[stage][which], st);
+    if (which == 1) m->ev_set[stage] = true;
+}
 
 int dev_alloc(const sdf_allocator *a, void **p, size_t bytes, cudaStream_t st) {
     *p = nullptr;
@@ -44,6 +57,18 @@ static int have_device() {
 extern "C" {
 
 int sdf_version(void) { return 100; }
+int64_t sdf_launch_count(void) { return (int64_t)g_launch_count; }
+int sdf_enable_timing(int on) { g_timing = on ? 1 : 0; return SDF_OK; }
+
+int sdf_get_timings(sdf_mesh *m, float *ms, int n) {
+    if (!m || !ms || n != SDF_T_COUNT) return SDF_EINVAL;
+    CK(cudaStreamSynchronize(m->last_stream));
+    for (int i = 0; i < SDF_T_COUNT; i++) {
+        ms[i] = 0.0f;
+        if (m->ev_set[i] && m->ev[i][0] && m->ev[i][1]) CK(cudaEventElapsedTime(&ms[i], m->ev[i][0], m->ev[i][1]));
+    }
+    return SDF_OK;
+}
 int sdf_last_cuda_error(void) { return g_last_cuda_error; }
 
 const char *sdf_strerror(int s) {
@@ -66,6 +91,9 @@ void sdf_destroy(sdf_mesh *m) {
     void *ptrs[] = {m->soup, m->fn, m->cvid, m->adj, m->vmint, m->vrec, m->erec, m->d_ctr, m->d_flags, m->hdr,
                     m->offsets, m->scan_ws, m->brick_flag, m->brick_table, m->scratch};
     for (size_t i = 0; i < sizeof(ptrs) / sizeof(ptrs[0]); i++) dev_free(&m->alloc, ptrs[i], st);
+    for (int i = 0; i < SDF_T_COUNT; i++)
+        for (int w = 0; w < 2; w++)
+            if (m->ev[i][w]) cudaEventDestroy(m->ev[i][w]);
     m->~sdf_mesh();
     free(m);
 }

@@ -13,6 +13,9 @@ typedef unsigned long long u64;
 // error handling: every CUDA call goes through CK(); the first failure is remembered
 // ---------------------------------------------------------------------------------------
 extern int g_last_cuda_error;
+extern int g_timing;                 // sdf_enable_timing
+extern long long g_launch_count;     // kernels launched by this library (sdf_launch_count)
+#define KL (++g_launch_count)        // written in front of every <<< >>> launch
 #define CK(call)                                                   \
     do {                                                           \
         cudaError_t e__ = (call);                                  \
@@ -108,6 +111,8 @@ struct sdf_mesh {
     int *brick_table; size_t brick_table_cap;
     u64 *scratch;  size_t scratch_cap;     // bricks * 512 packed values
     u64 h_ctr[CTR_COUNT];
+    cudaEvent_t ev[SDF_T_COUNT][2];   // stage begin / end events (created on first use)
+    bool ev_set[SDF_T_COUNT];
     int64_t last_bricks_total;
     cudaStream_t last_stream;
 };
@@ -115,6 +120,9 @@ struct sdf_mesh {
 // allocation through the handle's allocator
 int dev_alloc(const sdf_allocator *a, void **p, size_t bytes, cudaStream_t st);
 void dev_free(const sdf_allocator *a, void *p, cudaStream_t st);
+
+// stage timing: record the begin (which = 0) / end (which = 1) event of a stage on st
+void stage_mark(sdf_mesh *m, int stage, int which, cudaStream_t st);
 
 // stages (features.cu / compute.cu)
 int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st);

@@ -537,10 +537,12 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
     CK(cudaMemsetAsync(m->d_ctr + CTR_POLY, 0, sizeof(u64) * (CTR_COUNT - CTR_POLY), st));
 
     // A5 + A6: clip, count rows, mark bricks; prefix sums
-    clip_count_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(mv, g, m->hdr, m->brick_flag);
-    count_nonempty_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(m->hdr, P, m->d_ctr);
+    for (int i = SDF_T_CLIP_SCAN; i < SDF_T_COUNT; i++) m->ev_set[i] = false;
+    stage_mark(m, SDF_T_CLIP_SCAN, 0, st);
+    KL; clip_count_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(mv, g, m->hdr, m->brick_flag);
+    KL; count_nonempty_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(m->hdr, P, m->d_ctr);
     CKS(launch_scan(RowsIn{m->hdr}, RowsOut{m->offsets}, P, m->scan_ws, m->d_ctr + CTR_ITEMS, st));
-    set_last_offset_kernel<<<1, 1, 0, st>>>(m->offsets, P, m->d_ctr + CTR_ITEMS);
+    KL; set_last_offset_kernel<<<1, 1, 0, st>>>(m->offsets, P, m->d_ctr + CTR_ITEMS);
     CKS(launch_scan(BrickIn{m->brick_flag}, BrickOut{m->brick_table}, nbricks, m->scan_ws, m->d_ctr + CTR_BRICKS, st));
     CK(cudaGetLastError());
 
@@ -549,15 +551,20 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
     CK(cudaMemcpyAsync(tot, m->d_ctr + CTR_ITEMS, sizeof(tot), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     const u64 items = tot[0], bricks = tot[1];
+    stage_mark(m, SDF_T_CLIP_SCAN, 1, st);
     CKS(ensure(m, &m->scratch, &m->scratch_cap, (size_t)(bricks ? bricks : 1) * BRICK_CELLS, st));
+    stage_mark(m, SDF_T_CLEAR, 0, st);
     if (bricks) CK(cudaMemsetAsync(m->scratch, 0xFF, (size_t)bricks * BRICK_CELLS * sizeof(u64), st));
+    stage_mark(m, SDF_T_CLEAR, 1, st);
 
     // A7
     if (items) {
         u64 nblk = (items + EV_IPB - 1) / EV_IPB;
         if (nblk > 0x7FFFFFFFull) return SDF_EINVAL;
-        evaluate_kernel<<<(unsigned)nblk, EV_BT, 0, st>>>(mv, g, m->hdr, m->offsets, items, m->brick_table, m->scratch,
+        stage_mark(m, SDF_T_EVALUATE, 0, st);
+        KL; evaluate_kernel<<<(unsigned)nblk, EV_BT, 0, st>>>(mv, g, m->hdr, m->offsets, items, m->brick_table, m->scratch,
                                                          m->d_ctr);
+        stage_mark(m, SDF_T_EVALUATE, 1, st);
     }
     // A8
     {
@@ -567,10 +574,13 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
         int64_t ntiles = (int64_t)((g.ny + 7) / 8) * g.nz;
         int64_t grid = (int64_t)sms * 8;
         if (grid > ntiles) grid = ntiles;
+        stage_mark(m, SDF_T_EMIT, 0, st);
+        KL;
         if (g.vec4)
             emit_kernel<4><<<(unsigned)grid, 256, 0, st>>>(mv, g, m->brick_table, m->scratch, dist, tri, m->d_ctr);
         else
             emit_kernel<1><<<(unsigned)grid, 256, 0, st>>>(mv, g, m->brick_table, m->scratch, dist, tri, m->d_ctr);
+        stage_mark(m, SDF_T_EMIT, 1, st);
     }
     CK(cudaGetLastError());
     m->last_stream = st;

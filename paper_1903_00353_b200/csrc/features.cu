@@ -374,6 +374,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     CK(cudaMemsetAsync(m->adj, 0xFF, sizeof(int) * 3 * F, st));
 
     // ---- A0: ingest
+    stage_mark(m, SDF_T_INGEST_WELD, 0, st);
     const float *src = tri;
     float *staging = nullptr;
     if (!on_device) {
@@ -394,7 +395,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     CKS(tmp.get((void **)&scan_ws, sizeof(u64) * ws_elems));
     CKS(tmp.get((void **)&head, (size_t)nc));
     CKS(tmp.get((void **)&vcorner, sizeof(int) * nc));      // V <= 3F
-    ingest_kernel<<<blocks_for(nc), FB, 0, st>>>(src, m->soup, nc, k32a, va, m->d_flags);
+    KL; ingest_kernel<<<blocks_for(nc), FB, 0, st>>>(src, m->soup, nc, k32a, va, m->d_flags);
 
     // ---- A1: weld (radix sort of the hashed keys, exact compare of neighbours)
     {
@@ -402,12 +403,13 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
         bool first;
         CKS(radix_sort_pairs<u32>(k32a, va, k32b, vb, nc, shifts, 4, hist, scan_ws, st, &first));
         u32 *ks = first ? k32a : k32b, *vs = first ? va : vb;
-        weld_flags_kernel<<<blocks_for(nc), FB, 0, st>>>(m->soup, ks, vs, nc, head, m->d_ctr);
-        weld_fix_kernel<<<blocks_for(nc), FB, 0, st>>>(m->soup, ks, vs, nc, head, m->d_ctr);
+        KL; weld_flags_kernel<<<blocks_for(nc), FB, 0, st>>>(m->soup, ks, vs, nc, head, m->d_ctr);
+        KL; weld_fix_kernel<<<blocks_for(nc), FB, 0, st>>>(m->soup, ks, vs, nc, head, m->d_ctr);
         HeadIn hin{head};
         HeadOut hout{vs, m->cvid, vcorner};
         CKS(launch_scan(hin, hout, (int64_t)nc, scan_ws, m->d_ctr + CTR_V, st));
     }
+    stage_mark(m, SDF_T_INGEST_WELD, 1, st);
     // first host crossing: the vertex count sizes every per-vertex table
     CK(cudaMemcpyAsync(m->h_ctr, m->d_ctr, sizeof(u64) * CTR_COUNT, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
@@ -415,12 +417,13 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     const int V = (int)m->V;
 
     // ---- A3 (per triangle) + half-edge keys
+    stage_mark(m, SDF_T_EDGES, 0, st);
     u64 *vacc, *eka, *ekb;
     CKS(tmp.get((void **)&vacc, sizeof(u64) * 3 * (size_t)V));
     CKS(tmp.get((void **)&eka, sizeof(u64) * nc));
     CKS(tmp.get((void **)&ekb, sizeof(u64) * nc));
     CK(cudaMemsetAsync(vacc, 0, sizeof(u64) * 3 * (size_t)V, st));
-    tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, m->cvid, (int)F, m->fn, vacc, eka, va, m->d_flags);
+    KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, m->cvid, (int)F, m->fn, vacc, eka, va, m->d_flags);
 
     // ---- A2: edge table (radix sort of the (min,max) keys over their significant bits)
     {
@@ -439,12 +442,14 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
         }
         m->E = nc / 2;
         CKS(dev_alloc(al, (void **)&m->erec, sizeof(EdgeRec) * (size_t)(m->E > 0 ? m->E : 1), st));
-        edge_pair_kernel<<<blocks_for(nc), FB, 0, st>>>(ks, vs, nc & ~1, m->soup, m->fn, m->cvid, m->adj, m->erec,
+        KL; edge_pair_kernel<<<blocks_for(nc), FB, 0, st>>>(ks, vs, nc & ~1, m->soup, m->fn, m->cvid, m->adj, m->erec,
                                                         m->d_flags, m->d_ctr);
     }
     CK(cudaGetLastError());
+    stage_mark(m, SDF_T_EDGES, 1, st);
 
     // ---- A3/A4 vertices (garbage-in on invalid input is harmless: ids stay in range)
+    stage_mark(m, SDF_T_VERTICES, 0, st);
     double *vn64;
     long long *vcosq;
     int *vside;
@@ -453,13 +458,14 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     CKS(tmp.get((void **)&vside, sizeof(int) * (size_t)V));
     CKS(dev_alloc(al, (void **)&m->vmint, sizeof(int) * (size_t)V, st));
     CKS(dev_alloc(al, (void **)&m->vrec, sizeof(VertexRec) * (size_t)V, st));
-    vertex_normal_kernel<<<blocks_for(V), FB, 0, st>>>(vacc, V, vn64);
-    fill_i64_kernel<<<blocks_for(V), FB, 0, st>>>(vcosq, V, 0x7FFFFFFFFFFFFFFFll);
-    fill_i32_kernel<<<blocks_for(V), FB, 0, st>>>(m->vmint, V, 0x7FFFFFFF);
+    KL; vertex_normal_kernel<<<blocks_for(V), FB, 0, st>>>(vacc, V, vn64);
+    KL; fill_i64_kernel<<<blocks_for(V), FB, 0, st>>>(vcosq, V, 0x7FFFFFFFFFFFFFFFll);
+    KL; fill_i32_kernel<<<blocks_for(V), FB, 0, st>>>(m->vmint, V, 0x7FFFFFFF);
     CK(cudaMemsetAsync(vside, 0, sizeof(int) * (size_t)V, st));
-    vertex_cone_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, m->cvid, (int)F, vn64, vcosq, vside, m->vmint);
-    vertex_record_kernel<<<blocks_for(V), FB, 0, st>>>(m->soup, vcorner, vn64, vcosq, vside, V, m->vrec, m->d_ctr);
+    KL; vertex_cone_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, m->cvid, (int)F, vn64, vcosq, vside, m->vmint);
+    KL; vertex_record_kernel<<<blocks_for(V), FB, 0, st>>>(m->soup, vcorner, vn64, vcosq, vside, V, m->vrec, m->d_ctr);
     CK(cudaGetLastError());
+    stage_mark(m, SDF_T_VERTICES, 1, st);
     // second host crossing: validation flags + class counters
     int hflags[4];
     CK(cudaMemcpyAsync(hflags, m->d_flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));

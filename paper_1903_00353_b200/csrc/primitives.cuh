@@ -103,9 +103,9 @@ static int launch_scan(InF in, OutF out, int64_t n, u64 *ws, u64 *total, cudaStr
         return SDF_OK;
     }
     int64_t nb = (n + SCAN_TILE - 1) / SCAN_TILE;
-    scan_reduce_kernel<InF><<<(unsigned)nb, SCAN_BT, 0, st>>>(in, n, ws);
-    scan_partials_kernel<<<1, SCAN_BT, 0, st>>>(ws, nb, total);
-    scan_down_kernel<InF, OutF><<<(unsigned)nb, SCAN_BT, 0, st>>>(in, out, n, ws);
+    KL; scan_reduce_kernel<InF><<<(unsigned)nb, SCAN_BT, 0, st>>>(in, n, ws);
+    KL; scan_partials_kernel<<<1, SCAN_BT, 0, st>>>(ws, nb, total);
+    KL; scan_down_kernel<InF, OutF><<<(unsigned)nb, SCAN_BT, 0, st>>>(in, out, n, ws);
     CK(cudaGetLastError());
     return SDF_OK;
 }
@@ -213,11 +213,11 @@ static int radix_sort_pairs(K *k0, u32 *v0, K *k1, u32 *v1, int n, const int *sh
     K *ki = k0, *ko = k1;
     u32 *vi = v0, *vo = v1;
     for (int p = 0; p < npass; p++) {
-        radix_hist_kernel<K><<<nb, RS_BT, 0, st>>>(ki, n, shifts[p], hist, nb);
+        KL; radix_hist_kernel<K><<<nb, RS_BT, 0, st>>>(ki, n, shifts[p], hist, nb);
         HistIn hin{hist};
         HistOut hout{hist};
         CKS(launch_scan(hin, hout, (int64_t)nb * 256, scan_ws, (u64 *)nullptr, st));
-        radix_scatter_kernel<K><<<nb, RS_BT, 0, st>>>(ki, vi, ko, vo, n, shifts[p], hist, nb);
+        KL; radix_scatter_kernel<K><<<nb, RS_BT, 0, st>>>(ki, vi, ko, vo, n, shifts[p], hist, nb);
         K *tk = ki; ki = ko; ko = tk;
         u32 *tv = vi; vi = vo; vo = tv;
     }
