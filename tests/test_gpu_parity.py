@@ -102,7 +102,11 @@ def test_host_pointer_and_repeat_compute(oracle_mod):
     d2, t2 = B.sdf_compute(m, w.origin, w.h, w.dims, 0.5 * w.band)
     d1, t1, d2, t2 = (x.cpu().numpy() for x in (d1, t1, d2, t2))
     inner = np.abs(d1) < 0.5 * w.band * (1 - 1e-5)
-    assert np.array_equal(d2[inner], d1[inner]) and np.array_equal(t2[inner], t1[inner])
+    # ids are band-independent; distances too, except that cells near the (new) band edge are
+    # re-evaluated in fp64 by the emit pass and may differ in the last fp32 bit
+    assert np.array_equal(t2[inner], t1[inner])
+    assert np.max(np.abs(d2[inner] - d1[inner])) <= 1e-7
+    assert np.mean(d2[inner] == d1[inner]) > 0.98
     outer = ~(np.abs(d1) < 0.5 * w.band * (1 + 1e-5))
     assert np.all(np.isposinf(d2[outer]))
     dh, th = B.sdf_compute_host(m, w.origin, w.h, w.dims, w.band)
