@@ -162,8 +162,10 @@ enum {
     SDF_T_CLIP_SCAN   = 3,  /* A5+A6: clip polyhedra, row counts, prefix sums, brick table      */
     SDF_T_CLEAR       = 4,  /* scratch bricks reset to "empty"                                  */
     SDF_T_EVALUATE    = 5,  /* A7: work items -> distances -> packed atomicMin                  */
-    SDF_T_EMIT        = 6,  /* A8: sign + dense write of both grids                             */
-    SDF_T_COUNT       = 7
+    SDF_T_EMIT        = 6,  /* A8b: sign pass over the active bricks, written into both grids   */
+    SDF_T_FILL        = 7,  /* A8a: dense sentinel fill of both grids (library-owned side stream,
+                               concurrent with stages 3-5)                                     */
+    SDF_T_COUNT       = 8
 };
 int sdf_enable_timing(int on);
 int sdf_get_timings(sdf_mesh *m, float *ms, int n);

@@ -26,7 +26,7 @@ EXPORTS = ("sdf_create", "sdf_compute", "sdf_compute_host", "sdf_stats", "sdf_ge
            "sdf_destroy", "sdf_strerror", "sdf_last_cuda_error", "sdf_version",
            "sdf_enable_timing", "sdf_get_timings", "sdf_launch_count")
 
-TIMING_STAGES = ("ingest_weld", "edges", "vertices", "clip_scan", "clear", "evaluate", "emit")
+TIMING_STAGES = ("ingest_weld", "edges", "vertices", "clip_scan", "clear", "evaluate", "emit", "fill")
 
 VERTEX_REC_DTYPE = np.dtype([("pos", "<f4", 3), ("axis", "<f4", 3), ("cos_cone", "<f4"), ("info", "<i4")])
 EDGE_REC_DTYPE = np.dtype([("a", "<f4", 3), ("b", "<f4", 3), ("n1", "<f4", 3), ("n2", "<f4", 3),

@@ -88,8 +88,11 @@ void sdf_destroy(sdf_mesh *m) {
     if (!m) return;
     cudaStream_t st = m->last_stream;
     cudaStreamSynchronize(st);
+    if (m->side) { cudaStreamSynchronize(m->side); cudaStreamDestroy(m->side); }
+    if (m->ev_fork) cudaEventDestroy(m->ev_fork);
+    if (m->ev_join) cudaEventDestroy(m->ev_join);
     void *ptrs[] = {m->soup, m->fn, m->cvid, m->adj, m->vmint, m->vrec, m->erec, m->d_ctr, m->d_flags, m->hdr,
-                    m->offsets, m->scan_ws, m->brick_flag, m->brick_table, m->scratch};
+                    m->offsets, m->scan_ws, m->brick_flag, m->brick_table, m->brick_list, m->scratch};
     for (size_t i = 0; i < sizeof(ptrs) / sizeof(ptrs[0]); i++) dev_free(&m->alloc, ptrs[i], st);
     for (int i = 0; i < SDF_T_COUNT; i++)
         for (int w = 0; w < 2; w++)
@@ -154,7 +157,9 @@ int sdf_compute(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int
     if (!m || !dist_out || !tri_out) return SDF_EINVAL;
     GridParams g;
     CKS(make_grid(origin, h, nx, ny, nz, band, dist_out, tri_out, &g));
-    return run_compute(m, g, dist_out, tri_out, (cudaStream_t)stream);
+    int s = run_compute(m, g, dist_out, tri_out, (cudaStream_t)stream);
+    if (s != SDF_OK && m->side) cudaStreamSynchronize(m->side);   // never leave the fill in flight on failure
+    return s;
 }
 
 int sdf_compute_host(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz, float band,
@@ -169,6 +174,7 @@ int sdf_compute_host(sdf_mesh *m, const float origin[3], float h, int nx, int ny
     int s = dev_alloc(&m->alloc, (void **)&dd, n * sizeof(float), st);
     if (s == SDF_OK) s = dev_alloc(&m->alloc, (void **)&dt, n * sizeof(int32_t), st);
     if (s == SDF_OK) s = run_compute(m, g, dd, dt, st);
+    if (s != SDF_OK && m->side) cudaStreamSynchronize(m->side);
     if (s == SDF_OK) {
         cudaError_t e = cudaMemcpyAsync(dist_out_host, dd, n * sizeof(float), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaMemcpyAsync(tri_out_host, dt, n * sizeof(int32_t), cudaMemcpyDeviceToHost, st);

@@ -109,12 +109,15 @@ struct sdf_mesh {
     u64 *scan_ws;  size_t scan_ws_cap;
     unsigned char *brick_flag; size_t brick_flag_cap;
     int *brick_table; size_t brick_table_cap;
+    int *brick_list; size_t brick_list_cap;   // scratch slot -> brick index
     u64 *scratch;  size_t scratch_cap;     // bricks * 512 packed values
     u64 h_ctr[CTR_COUNT];
     cudaEvent_t ev[SDF_T_COUNT][2];   // stage begin / end events (created on first use)
     bool ev_set[SDF_T_COUNT];
     int64_t last_bricks_total;
     cudaStream_t last_stream;
+    cudaStream_t side;                // library-owned stream of the sentinel fill (A8a)
+    cudaEvent_t ev_fork, ev_join;
 };
 
 // allocation through the handle's allocator

@@ -194,8 +194,11 @@ struct BrickIn {
     __device__ u64 operator()(int64_t i) const { return flag[i]; }
 };
 struct BrickOut {
-    int *table;
-    __device__ void operator()(int64_t i, u64 ex, u64 v) const { table[i] = v ? (int)ex : -1; }
+    int *table, *list;        // brick -> scratch slot (-1 = inactive), slot -> brick
+    __device__ void operator()(int64_t i, u64 ex, u64 v) const {
+        table[i] = v ? (int)ex : -1;
+        if (v) list[ex] = (int)i;
+    }
 };
 __global__ void count_nonempty_kernel(const PolyHdr *__restrict__ hdr, int64_t P, u64 *__restrict__ ctr) {
     int64_t p = (int64_t)blockIdx.x * 256 + threadIdx.x;
@@ -400,15 +403,44 @@ __global__ void __launch_bounds__(EV_BT) evaluate_kernel(MeshView mv, GridParams
 }
 
 // ---------------------------------------------------------------------------------------
-// A8: sign + emit.  Persistent blocks walk tiles of 8 rows (one brick row in j, one k);
-// warp w writes row 8*tile_j + w with 128-bit stores; inactive bricks get sentinels.
+// A8: sign + emit.  Two kernels: (1) fill_kernel streams the sentinels (+inf, -1;
+// PAPER.md:66) over both dense grids at HBM write speed -- it depends on nothing, so it
+// runs on a side stream underneath A5-A7; (2) emit_bricks_kernel then overwrites the cells
+// of the active bricks: sign from the pseudonormal of the closest feature.
 // ---------------------------------------------------------------------------------------
+#define FILL_BT 512
+#define FILL_UNROLL 4
+
+__global__ void __launch_bounds__(FILL_BT) fill_kernel(float *__restrict__ dist, int *__restrict__ tri, int64_t n,
+                                                       int vec) {
+    const int64_t tid = (int64_t)blockIdx.x * FILL_BT + threadIdx.x, nth = (int64_t)gridDim.x * FILL_BT;
+    if (vec) {
+        const int64_t n4 = n >> 2;
+        const float4 dv = make_float4(INFINITY, INFINITY, INFINITY, INFINITY);
+        const int4 tv = make_int4(-1, -1, -1, -1);
+        float4 *d4 = (float4 *)dist;
+        int4 *t4 = (int4 *)tri;
+        // each block walks contiguous chunks of FILL_UNROLL * FILL_BT vectors (32 KiB per array)
+        const int64_t chunk = (int64_t)FILL_BT * FILL_UNROLL;
+        for (int64_t base = (int64_t)blockIdx.x * chunk; base < n4; base += (int64_t)gridDim.x * chunk) {
+#pragma unroll
+            for (int u = 0; u < FILL_UNROLL; u++) {
+                int64_t i = base + (int64_t)u * FILL_BT + threadIdx.x;
+                if (i < n4) { __stcs(d4 + i, dv); __stcs(t4 + i, tv); }
+            }
+        }
+        for (int64_t i = (n4 << 2) + tid; i < n; i += nth) { dist[i] = INFINITY; tri[i] = -1; }
+    } else {
+        for (int64_t i = tid; i < n; i += nth) { dist[i] = INFINITY; tri[i] = -1; }
+    }
+}
+
 struct CellOut { float d; int t; };
 
 // Populated cell: band decision (fp64 re-check near the band edge) and the sign from the
 // pseudonormal of the closest feature of the winning triangle.
-__device__ __noinline__ CellOut finish_cell(const MeshView &mv, const GridParams &g, int i, int j, int k, u64 pack,
-                                            u32 &recheck) {
+__device__ __forceinline__ CellOut finish_cell(const MeshView &mv, const GridParams &g, int i, int j, int k, u64 pack,
+                                               u32 &recheck) {
     CellOut o;
     o.d = INFINITY; o.t = -1;
     float d = __uint_as_float((u32)(pack >> 32));
@@ -449,58 +481,79 @@ __device__ __noinline__ CellOut finish_cell(const MeshView &mv, const GridParams
     return o;
 }
 
-template <int VEC>
-__global__ void __launch_bounds__(256) emit_kernel(MeshView mv, GridParams g, const int *__restrict__ table,
-                                                   const u64 *__restrict__ scratch, float *__restrict__ dist,
-                                                   int *__restrict__ tri, u64 *__restrict__ ctr) {
-    __shared__ u32 s_stat[2];
-    if (threadIdx.x == 0) s_stat[0] = s_stat[1] = 0;
+// One block per active brick (8x8x8 cells, 4 KiB of packed scratch).  Phase 1 loads the
+// brick and compacts its populated cells into a shared list; phase 2 spreads the list over
+// the threads (the sign pass is the expensive, divergent part); phase 3 writes the brick's
+// 64 row segments (8 cells = one 32-B sector each) into both grids.
+#define EB_BT 128
+__global__ void __launch_bounds__(EB_BT) emit_bricks_kernel(MeshView mv, GridParams g, const int *__restrict__ list,
+                                                            const u64 *__restrict__ scratch,
+                                                            float *__restrict__ dist, int *__restrict__ tri,
+                                                            u64 *__restrict__ ctr) {
+    __shared__ __align__(16) u64 s_pack[BRICK_CELLS];
+    __shared__ __align__(16) float s_d[BRICK_CELLS];
+    __shared__ __align__(16) int s_t[BRICK_CELLS];
+    __shared__ unsigned short s_list[BRICK_CELLS];
+    __shared__ u32 s_n, s_stat[2];
+    const int tid = threadIdx.x;
+    if (tid == 0) { s_n = 0; s_stat[0] = s_stat[1] = 0; }
     __syncthreads();
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int tiles_j = (g.ny + 7) >> 3;
-    const int64_t ntiles = (int64_t)tiles_j * g.nz;
+    const int slot = blockIdx.x;
+    const int b = list[slot];
+    const int bx = b % g.nbx, by = (b / g.nbx) % g.nby, bz = b / (g.nbx * g.nby);
+    {
+        const ulonglong2 *src = (const ulonglong2 *)(scratch + (size_t)slot * BRICK_CELLS) + 2 * tid;
+        ulonglong2 p01 = src[0], p23 = src[1];
+        const u64 p[4] = {p01.x, p01.y, p23.x, p23.y};
+        const int c0 = 4 * tid;
+        // warp-aggregated append of the populated cells
+        int cnt = (p[0] != PACK_EMPTY) + (p[1] != PACK_EMPTY) + (p[2] != PACK_EMPTY) + (p[3] != PACK_EMPTY);
+        const int lane = tid & 31;
+        int inc = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int v = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += v;
+        }
+        int base = 0;
+        if (lane == 31 && inc) base = (int)atomicAdd(&s_n, (u32)inc);
+        base = __shfl_sync(0xffffffffu, base, 31) + inc - cnt;
+#pragma unroll
+        for (int c = 0; c < 4; c++) {
+            s_d[c0 + c] = INFINITY; s_t[c0 + c] = -1;
+            if (p[c] != PACK_EMPTY) { s_pack[c0 + c] = p[c]; s_list[base++] = (unsigned short)(c0 + c); }
+        }
+    }
+    __syncthreads();
+    const int n = (int)s_n;
     u32 band = 0, recheck = 0;
-    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int k = (int)(tile / tiles_j), bj = (int)(tile - (int64_t)k * tiles_j);
-        const int j = bj * 8 + w;
-        if (j >= g.ny) continue;
-        const int *trow = table + ((size_t)(k >> 3) * g.nby + bj) * g.nbx;
-        const size_t rowbase = ((size_t)k * g.ny + j) * g.nx;
-        const int inb = ((k & 7) * 8 + (j & 7)) * 8;
-        if (VEC == 4) {
-            for (int i = lane * 4; i < g.nx; i += 128) {
-                float4 dv = make_float4(INFINITY, INFINITY, INFINITY, INFINITY);
-                int4 tv = make_int4(-1, -1, -1, -1);
-                int slot = trow[i >> 3];
-                if (slot >= 0) {
-                    const ulonglong2 *src = (const ulonglong2 *)(scratch + (size_t)slot * BRICK_CELLS + inb + (i & 7));
-                    ulonglong2 p01 = src[0], p23 = src[1];
-                    if (p01.x != PACK_EMPTY) { CellOut o = finish_cell(mv, g, i, j, k, p01.x, recheck); dv.x = o.d; tv.x = o.t; band += o.t >= 0; }
-                    if (p01.y != PACK_EMPTY) { CellOut o = finish_cell(mv, g, i + 1, j, k, p01.y, recheck); dv.y = o.d; tv.y = o.t; band += o.t >= 0; }
-                    if (p23.x != PACK_EMPTY) { CellOut o = finish_cell(mv, g, i + 2, j, k, p23.x, recheck); dv.z = o.d; tv.z = o.t; band += o.t >= 0; }
-                    if (p23.y != PACK_EMPTY) { CellOut o = finish_cell(mv, g, i + 3, j, k, p23.y, recheck); dv.w = o.d; tv.w = o.t; band += o.t >= 0; }
-                }
-                __stcs((float4 *)(dist + rowbase + i), dv);
-                __stcs((int4 *)(tri + rowbase + i), tv);
-            }
-        } else {
-            for (int i = lane; i < g.nx; i += 32) {
-                float dv = INFINITY;
-                int tv = -1;
-                int slot = trow[i >> 3];
-                if (slot >= 0) {
-                    u64 p = scratch[(size_t)slot * BRICK_CELLS + inb + (i & 7)];
-                    if (p != PACK_EMPTY) { CellOut o = finish_cell(mv, g, i, j, k, p, recheck); dv = o.d; tv = o.t; band += o.t >= 0; }
-                }
-                __stcs(dist + rowbase + i, dv);
-                __stcs(tri + rowbase + i, tv);
+    for (int q = tid; q < n; q += EB_BT) {
+        const int c = s_list[q];
+        const int i = bx * 8 + (c & 7), j = by * 8 + ((c >> 3) & 7), k = bz * 8 + (c >> 6);
+        CellOut o = finish_cell(mv, g, i, j, k, s_pack[c], recheck);
+        s_d[c] = o.d; s_t[c] = o.t;
+        band += o.t >= 0;
+    }
+    __syncthreads();
+    {
+        const int c0 = 4 * tid;
+        const int i = bx * 8 + (c0 & 7), j = by * 8 + ((c0 >> 3) & 7), k = bz * 8 + (c0 >> 6);
+        if (j < g.ny && k < g.nz) {
+            const size_t o = ((size_t)k * g.ny + j) * g.nx + i;
+            if (g.vec4 && i + 3 < g.nx) {
+                *(float4 *)(dist + o) = *(const float4 *)(s_d + c0);
+                *(int4 *)(tri + o) = *(const int4 *)(s_t + c0);
+            } else {
+#pragma unroll
+                for (int c = 0; c < 4; c++)
+                    if (i + c < g.nx) { dist[o + c] = s_d[c0 + c]; tri[o + c] = s_t[c0 + c]; }
             }
         }
     }
     if (band) atomicAdd(&s_stat[0], band);
     if (recheck) atomicAdd(&s_stat[1], recheck);
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (tid == 0) {
         if (s_stat[0]) atomicAdd(&ctr[CTR_BAND], (u64)s_stat[0]);
         if (s_stat[1]) atomicAdd(&ctr[CTR_RECHECK], (u64)s_stat[1]);
     }
@@ -533,17 +586,40 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
     CKS(ensure(m, &m->scan_ws, &m->scan_ws_cap, scan_ws_elems(scan_n), st));
     CKS(ensure(m, &m->brick_flag, &m->brick_flag_cap, (size_t)nbricks, st));
     CKS(ensure(m, &m->brick_table, &m->brick_table_cap, (size_t)nbricks, st));
+    CKS(ensure(m, &m->brick_list, &m->brick_list_cap, (size_t)nbricks, st));
+
+    // A8a: the sentinel fill depends on nothing: fork it onto the side stream so that it
+    // streams to HBM underneath A5-A7 (which are latency / atomic bound)
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    for (int i = SDF_T_CLIP_SCAN; i < SDF_T_COUNT; i++) m->ev_set[i] = false;
+    {
+        if (!m->side) CK(cudaStreamCreateWithFlags(&m->side, cudaStreamNonBlocking));
+        if (!m->ev_fork) CK(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
+        if (!m->ev_join) CK(cudaEventCreateWithFlags(&m->ev_join, cudaEventDisableTiming));
+        CK(cudaEventRecord(m->ev_fork, st));
+        CK(cudaStreamWaitEvent(m->side, m->ev_fork, 0));
+        const int64_t N = (int64_t)g.nx * g.ny * g.nz;
+        int64_t fb = (N / 4 + (int64_t)FILL_BT * FILL_UNROLL - 1) / ((int64_t)FILL_BT * FILL_UNROLL);
+        if (fb > (int64_t)sms * 2) fb = (int64_t)sms * 2;
+        if (fb < 1) fb = 1;
+        const int vec = (((uintptr_t)dist & 15) == 0) && (((uintptr_t)tri & 15) == 0);
+        stage_mark(m, SDF_T_FILL, 0, m->side);
+        KL; fill_kernel<<<(unsigned)fb, FILL_BT, 0, m->side>>>(dist, tri, N, vec);
+        stage_mark(m, SDF_T_FILL, 1, m->side);
+        CK(cudaEventRecord(m->ev_join, m->side));
+    }
     CK(cudaMemsetAsync(m->brick_flag, 0, (size_t)nbricks, st));
     CK(cudaMemsetAsync(m->d_ctr + CTR_POLY, 0, sizeof(u64) * (CTR_COUNT - CTR_POLY), st));
 
     // A5 + A6: clip, count rows, mark bricks; prefix sums
-    for (int i = SDF_T_CLIP_SCAN; i < SDF_T_COUNT; i++) m->ev_set[i] = false;
     stage_mark(m, SDF_T_CLIP_SCAN, 0, st);
     KL; clip_count_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(mv, g, m->hdr, m->brick_flag);
     KL; count_nonempty_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(m->hdr, P, m->d_ctr);
     CKS(launch_scan(RowsIn{m->hdr}, RowsOut{m->offsets}, P, m->scan_ws, m->d_ctr + CTR_ITEMS, st));
     KL; set_last_offset_kernel<<<1, 1, 0, st>>>(m->offsets, P, m->d_ctr + CTR_ITEMS);
-    CKS(launch_scan(BrickIn{m->brick_flag}, BrickOut{m->brick_table}, nbricks, m->scan_ws, m->d_ctr + CTR_BRICKS, st));
+    CKS(launch_scan(BrickIn{m->brick_flag}, BrickOut{m->brick_table, m->brick_list}, nbricks, m->scan_ws, m->d_ctr + CTR_BRICKS, st));
     CK(cudaGetLastError());
 
     // host crossing: totals size the launch and the scratch
@@ -566,20 +642,11 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
                                                          m->d_ctr);
         stage_mark(m, SDF_T_EVALUATE, 1, st);
     }
-    // A8
-    {
-        int dev = 0, sms = 148;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        int64_t ntiles = (int64_t)((g.ny + 7) / 8) * g.nz;
-        int64_t grid = (int64_t)sms * 8;
-        if (grid > ntiles) grid = ntiles;
+    // A8b: join the fill, then overwrite the active bricks
+    CK(cudaStreamWaitEvent(st, m->ev_join, 0));
+    if (bricks) {
         stage_mark(m, SDF_T_EMIT, 0, st);
-        KL;
-        if (g.vec4)
-            emit_kernel<4><<<(unsigned)grid, 256, 0, st>>>(mv, g, m->brick_table, m->scratch, dist, tri, m->d_ctr);
-        else
-            emit_kernel<1><<<(unsigned)grid, 256, 0, st>>>(mv, g, m->brick_table, m->scratch, dist, tri, m->d_ctr);
+        KL; emit_bricks_kernel<<<(unsigned)bricks, EB_BT, 0, st>>>(mv, g, m->brick_list, m->scratch, dist, tri, m->d_ctr);
         stage_mark(m, SDF_T_EMIT, 1, st);
     }
     CK(cudaGetLastError());

@@ -203,6 +203,19 @@ __global__ void __launch_bounds__(FB) edge_pair_kernel(const u64 *__restrict__ k
             adj[he1] = (int)he0;
             int t0 = he0 / 3, k0 = he0 % 3, t1 = he1 / 3;
             const float *A = soup + 9 * (size_t)t0 + 3 * k0, *B = soup + 9 * (size_t)t0 + 3 * ((k0 + 1) % 3);
+            {
+                // canonical direction a -> b = ascending exact position bits, so the record (and
+                // the fp32 rounding of every distance evaluated from it) does not depend on the
+                // order of the triangles in the soup; n1 stays the normal of the triangle that
+                // traverses a -> b
+                const u32 *pa = (const u32 *)A, *pb = (const u32 *)B;
+                bool swap = pa[0] != pb[0] ? pa[0] > pb[0] : (pa[1] != pb[1] ? pa[1] > pb[1] : pa[2] > pb[2]);
+                if (swap) {
+                    int k1 = he1 % 3;
+                    t0 = t1; t1 = he0 / 3; k0 = k1;
+                    A = soup + 9 * (size_t)t0 + 3 * k0; B = soup + 9 * (size_t)t0 + 3 * ((k0 + 1) % 3);
+                }
+            }
             const float *N1 = fn + 3 * (size_t)t0, *N2 = fn + 3 * (size_t)t1;
             EdgeRec r;
             double u[3], n1[3], n2[3], x[3];
