@@ -92,7 +92,7 @@ void sdf_destroy(sdf_mesh *m) {
     if (m->ev_fork) cudaEventDestroy(m->ev_fork);
     if (m->ev_join) cudaEventDestroy(m->ev_join);
     void *ptrs[] = {m->soup, m->fn, m->cvid, m->adj, m->vmint, m->vrec, m->erec, m->d_ctr, m->d_flags, m->hdr,
-                    m->offsets, m->scan_ws, m->brick_flag, m->brick_table, m->brick_list, m->scratch};
+                    m->scan_ws, m->brick_flag, m->brick_table, m->brick_list, m->big_list, m->scratch};
     for (size_t i = 0; i < sizeof(ptrs) / sizeof(ptrs[0]); i++) dev_free(&m->alloc, ptrs[i], st);
     for (int i = 0; i < SDF_T_COUNT; i++)
         for (int w = 0; w < 2; w++)
@@ -189,8 +189,16 @@ int sdf_compute_host(sdf_mesh *m, const float origin[3], float h, int nx, int ny
 int sdf_stats(sdf_mesh *m, sdf_stats_t *o) {
     if (!m || !o) return SDF_EINVAL;
     CK(cudaStreamSynchronize(m->last_stream));
-    CK(cudaMemcpy(m->h_ctr, m->d_ctr, sizeof(u64) * CTR_COUNT, cudaMemcpyDeviceToHost));
-    const u64 *c = m->h_ctr;
+    static u64 all[CTR_TOTAL];
+    CK(cudaMemcpy(all, m->d_ctr, sizeof(u64) * CTR_TOTAL, cudaMemcpyDeviceToHost));
+    memcpy(m->h_ctr, all, sizeof(u64) * CTR_COUNT);
+    u64 *c = m->h_ctr;
+    c[CTR_POLY] = c[CTR_TESTED] = c[CTR_ACCEPTED] = c[CTR_ITEMS] = 0;
+    for (int s = 0; s < CTR_SLOTS; s++) {
+        const u64 *q = all + CTR_SPREAD + s * 8;
+        c[CTR_POLY] += q[SP_POLY]; c[CTR_TESTED] += q[SP_TESTED];
+        c[CTR_ACCEPTED] += q[SP_ACCEPTED]; c[CTR_ITEMS] += q[SP_ROWS];
+    }
     memset(o, 0, sizeof(*o));
     o->F = m->F; o->V = m->V; o->E = m->E;
     o->edges_convex = (int64_t)c[CTR_E_CONVEX]; o->edges_concave = (int64_t)c[CTR_E_CONCAVE];

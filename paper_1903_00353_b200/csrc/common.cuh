@@ -39,8 +39,14 @@ enum {
     CTR_V = 0, CTR_WELD_BAD, CTR_E_CONVEX, CTR_E_CONCAVE, CTR_E_FLAT,
     CTR_V_POS, CTR_V_NEG, CTR_V_BOTH, CTR_V_SKIP, CTR_V_HEMI,
     CTR_POLY, CTR_ITEMS, CTR_BRICKS, CTR_TESTED, CTR_ACCEPTED, CTR_BAND, CTR_RECHECK,
-    CTR_COUNT = 24
+    CTR_BIG, CTR_BIG_NEXT,       // big-polyhedron list: length, dynamic fetch cursor
+    CTR_COUNT = 24,
+    // statistics that every warp adds to are spread over CTR_SLOTS lines of 8 counters
+    // (same-address atomics serialise in L2); sdf_stats sums the slots
+    CTR_SPREAD = CTR_COUNT, CTR_SLOTS = 64,
+    CTR_TOTAL = CTR_SPREAD + CTR_SLOTS * 8
 };
+enum { SP_POLY = 0, SP_TESTED, SP_ACCEPTED, SP_ROWS };
 
 // ---------------------------------------------------------------------------------------
 // feature tables (HBM layout)
@@ -71,6 +77,10 @@ struct __align__(16) PolyHdr {
     u32 rows;
 };
 static_assert(sizeof(PolyHdr) == 16, "PolyHdr must be 16 B");
+
+#define ROWS_BIG 0x80000000u         // PolyHdr::rows flag: taken by evaluate_big_kernel
+#define BIG_ROWS 256u                // ... when it has more rows than this
+#define BIG_NI 32                    // ... or rows at least this long
 
 #define BRICK 8                      // scratch bricks are 8x8x8 cells
 #define BRICK_CELLS 512
@@ -105,11 +115,11 @@ struct sdf_mesh {
     int *d_flags;            // [4]
     // persistent per-compute workspace (grown on demand)
     PolyHdr *hdr;  size_t hdr_cap;         // [F + E + 2V]
-    u64 *offsets;  size_t offsets_cap;     // [P + 1]
     u64 *scan_ws;  size_t scan_ws_cap;
     unsigned char *brick_flag; size_t brick_flag_cap;
     int *brick_table; size_t brick_table_cap;
     int *brick_list; size_t brick_list_cap;   // scratch slot -> brick index
+    u32 *big_list; size_t big_list_cap;       // polyhedra of evaluate_big_kernel
     u64 *scratch;  size_t scratch_cap;     // bricks * 512 packed values
     u64 h_ctr[CTR_COUNT];
     cudaEvent_t ev[SDF_T_COUNT][2];   // stage begin / end events (created on first use)

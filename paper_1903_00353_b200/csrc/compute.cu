@@ -100,13 +100,16 @@ __device__ __forceinline__ void cell_range(double mn, double mx, double o, doubl
 }
 
 __global__ void __launch_bounds__(256) clip_count_kernel(MeshView mv, GridParams g, PolyHdr *__restrict__ hdr,
-                                                         unsigned char *__restrict__ brick_flag) {
+                                                         unsigned char *__restrict__ brick_flag,
+                                                         u32 *__restrict__ big_list, u64 *__restrict__ ctr) {
     int64_t p = (int64_t)blockIdx.x * 256 + threadIdx.x;
-    if (p >= mv.P) return;
+    const bool live = p < mv.P;
+    if (!live) p = 0;
     float mn[3], mx[3];
-    bool emit = true;
+    bool emit = live;
     const float rb = g.rb, eps = g.eps;
-    if (p < mv.F) {
+    if (!live) {
+    } else if (p < mv.F) {
         // face slab: triangle swept by +-rb along its normal
         const float *T = mv.soup + 9 * p, *N = mv.fn + 3 * p;
 #pragma unroll
@@ -174,21 +177,22 @@ __global__ void __launch_bounds__(256) clip_count_kernel(MeshView mv, GridParams
             h.rows = (u32)(j1 - j0 + 1) * (u32)(k1 - k0 + 1);
             for (int bz = k0 >> 3; bz <= (k1 >> 3); bz++)
                 for (int by = j0 >> 3; by <= (j1 >> 3); by++)
-                    for (int bx = i0 >> 3; bx <= (i1 >> 3); bx++)
-                        brick_flag[((size_t)bz * g.nby + by) * g.nbx + bx] = 1;
+                    for (int bx = i0 >> 3; bx <= (i1 >> 3); bx++) {
+                        unsigned char *f = brick_flag + ((size_t)bz * g.nby + by) * g.nbx + bx;
+                        if (!*f) *f = 1;            // mostly already set: a cached read, not a write
+                    }
+            // big polyhedra (many rows or long rows) go to the block-per-polyhedron kernel
+            if (h.rows > BIG_ROWS || i1 - i0 >= BIG_NI) {
+                big_list[atomicAdd(&ctr[CTR_BIG], 1ull)] = (u32)p;
+                h.rows |= ROWS_BIG;
+            }
         }
     }
-    hdr[p] = h;
+    if (live) hdr[p] = h;
+    int c = __syncthreads_count(live && h.rows != 0);
+    if (threadIdx.x == 0 && c) atomicAdd(&ctr[CTR_SPREAD + (blockIdx.x & (CTR_SLOTS - 1)) * 8 + SP_POLY], (u64)c);
 }
 
-struct RowsIn {
-    const PolyHdr *hdr;
-    __device__ u64 operator()(int64_t i) const { return hdr[i].rows; }
-};
-struct RowsOut {
-    u64 *off;
-    __device__ void operator()(int64_t i, u64 ex, u64) const { off[i] = ex; }
-};
 struct BrickIn {
     const unsigned char *flag;
     __device__ u64 operator()(int64_t i) const { return flag[i]; }
@@ -200,24 +204,106 @@ struct BrickOut {
         if (v) list[ex] = (int)i;
     }
 };
-__global__ void count_nonempty_kernel(const PolyHdr *__restrict__ hdr, int64_t P, u64 *__restrict__ ctr) {
-    int64_t p = (int64_t)blockIdx.x * 256 + threadIdx.x;
-    int c = __syncthreads_count(p < P && hdr[p].rows > 0);
-    if (threadIdx.x == 0 && c) atomicAdd(&ctr[CTR_POLY], (u64)c);
+
+// ---------------------------------------------------------------------------------------
+// A6 + A7: scan conversion and evaluation.
+//
+// A polyhedron is turned into a 40-word record in shared memory: five row-clip constraints
+// (a convex body meets a grid row in one interval, so each half-space s(i,j,k) = A + gx*di +
+// gy*dj + gz*dk >= 0 clips the row's x-span analytically), the geometry the
+// per-cell tests and distances need, the triangle id and the AABV.  Work is flattened
+// WITHIN A WARP: lane l owns polyhedron 32*warp + l, the row counts are prefix-summed across
+// the lanes, and the warp then walks the flattened (polyhedron, row) list 32 rows at a time
+// -- the load balancing of PAPER.md:376-380 (dynamic parallelism) without child launches,
+// without a global work-item list and without a device-wide scan.  Polyhedra with many or
+// long rows are listed by clip_count_kernel and taken by evaluate_big_kernel, one block per
+// polyhedron with the lanes along x.
+// ---------------------------------------------------------------------------------------
+#define PR_GEO 20        // 13 geometry floats
+#define PR_ID 33
+#define PR_TYPE 34
+#define PR_I0 35
+#define PR_NI 36         // i1 - i0
+#define PR_J0 37
+#define PR_NJ 38         // j1 - j0 + 1
+#define PR_K0 39
+#define PR_WORDS 41      // odd stride: records of different owners fall in different banks
+
+__device__ __forceinline__ void set_con(float *rec, int c, f3 m, f3 r0, float lim, float h) {
+    const float gx = h * m.x;
+    rec[4 * c + 0] = dot(m, r0) - lim;                 // s >= lim at the AABV corner cell
+    rec[4 * c + 1] = h * m.y;
+    rec[4 * c + 2] = h * m.z;
+    rec[4 * c + 3] = gx != 0.0f ? 1.0f / gx : 0.0f;    // 0: the constraint does not depend on x
 }
-__global__ void set_last_offset_kernel(u64 *off, int64_t P, const u64 *total) { off[P] = *total; }
+__device__ __forceinline__ void no_con(float *rec, int c) {
+    rec[4 * c + 0] = 1.0f; rec[4 * c + 1] = 0.0f; rec[4 * c + 2] = 0.0f; rec[4 * c + 3] = 0.0f;
+}
 
-// ---------------------------------------------------------------------------------------
-// A7: flat (polyhedron, row) work items -> cells -> packed atomicMin
-// ---------------------------------------------------------------------------------------
-#define EV_BT 256
-#define EV_IPB 1024      // work items per block
-#define EV_CH 128        // polyhedra staged in shared memory per chunk
-
-struct __align__(16) Geo {
-    float f[12];
-    int id, type, pad0, pad1;
-};
+// A5: the polyhedron of feature p, clipped to the band, as a record
+__device__ __forceinline__ void build_record(const MeshView &mv, const GridParams &g, int64_t p, const PolyHdr &H,
+                                             float *rec) {
+    const float h = g.h, eps = g.eps, reach = g.band + g.guard;
+    const f3 x0 = mk<float>(fmaf((float)H.i0, h, g.ox), fmaf((float)H.j0, h, g.oy), fmaf((float)H.k0, h, g.oz));
+    int *ri = (int *)rec;
+    float *G = rec + PR_GEO;
+    if (p < mv.F) {
+        // face slab: three inward side planes through the edges + the slab
+        const float *T = mv.soup + 9 * p, *N = mv.fn + 3 * p;
+        const f3 a = ld3(T), e0 = ld3(T + 3) - a, ec = ld3(T + 6) - a, n = ld3(N);
+        const f3 r0 = x0 - a;
+        if (!g.aabb_mode) {
+            const f3 e1 = ec - e0;
+            const f3 m0 = cross(n, e0), m1 = cross(n, e1), m2 = cross(ec, n);          // inward, |m_i| = |edge_i|
+            const float t0 = eps * sqrtf(dot(e0, e0)), t1 = eps * sqrtf(dot(e1, e1)), t2 = eps * sqrtf(dot(ec, ec));
+            set_con(rec, 0, m0, r0, -2.0f * t0, h);
+            set_con(rec, 1, m1, r0 - e0, -2.0f * t1, h);
+            set_con(rec, 2, m2, r0 - ec, -2.0f * t2, h);
+            set_con(rec, 3, n, r0, -(reach + eps), h);
+            set_con(rec, 4, mk<float>(-n.x, -n.y, -n.z), r0, -(reach + eps), h);
+        } else {
+#pragma unroll
+            for (int c = 0; c < 5; c++) no_con(rec, c);
+        }
+        G[0] = a.x; G[1] = a.y; G[2] = a.z; G[3] = e0.x; G[4] = e0.y; G[5] = e0.z;
+        G[6] = ec.x; G[7] = ec.y; G[8] = ec.z; G[9] = n.x; G[10] = n.y; G[11] = n.z; G[12] = 0.0f;
+        ri[PR_ID] = (int)p; ri[PR_TYPE] = 0;
+    } else if (p < (int64_t)mv.F + mv.E) {
+        // edge wedge: beyond both faces' side planes, between the end caps
+        const EdgeRec &r = mv.erec[p - mv.F];
+        const f3 a = ld3(r.a), ab = ld3(r.b) - a, n1 = ld3(r.n1), n2 = ld3(r.n2);
+        const float L = sqrtf(dot(ab, ab));
+        const f3 u = (1.0f / L) * ab;
+        const f3 w1 = cross(u, n1), w2 = cross(n2, u);
+        const f3 r0 = x0 - a;
+        set_con(rec, 0, u, r0, -2.0f * eps, h);
+        set_con(rec, 1, mk<float>(-u.x, -u.y, -u.z), r0, -(L + 2.0f * eps), h);
+        set_con(rec, 2, w1, r0, -2.0f * eps, h);
+        set_con(rec, 3, w2, r0, -2.0f * eps, h);
+        no_con(rec, 4);
+        G[0] = a.x; G[1] = a.y; G[2] = a.z; G[3] = u.x; G[4] = u.y; G[5] = u.z; G[6] = L;
+        G[7] = w1.x; G[8] = w1.y; G[9] = w1.z; G[10] = w2.x; G[11] = w2.y; G[12] = w2.z;
+        ri[PR_ID] = r.tri; ri[PR_TYPE] = 1;
+    } else {
+        // vertex cone / hemisphere (eq.10, 362-364) inside the ball of radius reach
+        const int64_t q = p - mv.F - mv.E;
+        const VertexRec &r = mv.vrec[q >> 1];
+        const float sg = (q & 1) ? -1.0f : 1.0f;
+        const f3 v = ld3(r.pos), A = sg * ld3(r.axis);
+        const float c = r.cos_cone;
+        // a cone of half angle <= 90 degrees lies in the half space A.(x - v) >= 0
+        if (c >= 0.0f) set_con(rec, 0, A, x0 - v, -2.0f * eps, h); else no_con(rec, 0);
+#pragma unroll
+        for (int k = 1; k < 5; k++) no_con(rec, k);
+        G[0] = v.x; G[1] = v.y; G[2] = v.z; G[3] = A.x; G[4] = A.y; G[5] = A.z; G[6] = c;
+#pragma unroll
+        for (int k = 7; k < 13; k++) G[k] = 0.0f;
+        ri[PR_ID] = mv.vmint[q >> 1]; ri[PR_TYPE] = 2;
+    }
+    ri[PR_I0] = H.i0; ri[PR_NI] = H.i1 - H.i0;
+    ri[PR_J0] = H.j0; ri[PR_NJ] = H.j1 - H.j0 + 1;
+    ri[PR_K0] = H.k0;
+}
 
 __device__ __forceinline__ void put_min(const GridParams &g, const int *__restrict__ table, u64 *__restrict__ scratch,
                                         int i, int j, int k, float d, int id) {
@@ -226,180 +312,181 @@ __device__ __forceinline__ void put_min(const GridParams &g, const int *__restri
     atomicMin(cell, ((u64)__float_as_uint(d) << 32) | (u32)id);
 }
 
-// restrict t in [tlo, thi] to s0 + t*gx >= lim
-__device__ __forceinline__ void clip_ge(float s0, float gx, float lim, float &tlo, float &thi) {
-    float num = lim - s0;
-    if (gx > 0.0f) tlo = fmaxf(tlo, num / gx);
-    else if (gx < 0.0f) thi = fminf(thi, num / gx);
-    else if (num > 0.0f) thi = -1.0f;
-}
-
-__device__ __forceinline__ void process_row(const GridParams &g, const Geo &G, const PolyHdr &H, u32 row,
+// One grid row (j,k) of one polyhedron: clip the x-span, then test and evaluate its cells
+// i = ia + lane0, ia + lane0 + STRIDE, ...  (STRIDE 1: a lane owns the row; 32: a warp does).
+template <int STRIDE>
+__device__ __forceinline__ void process_row(const GridParams &g, const float *rec, u32 row, int lane0,
                                             const int *__restrict__ table, u64 *__restrict__ scratch, u32 &tested,
                                             u32 &accepted) {
-    const int nj = H.j1 - H.j0 + 1;
-    const int j = H.j0 + (int)(row % (u32)nj), k = H.k0 + (int)(row / (u32)nj);
-    const float y = fmaf((float)j, g.h, g.oy), z = fmaf((float)k, g.h, g.oz);
-    const float x0 = fmaf((float)H.i0, g.h, g.ox);
+    const int *ri = (const int *)rec;
+    const int nj = ri[PR_NJ];
+    const int dk = (int)(row / (u32)nj), dj = (int)(row - (u32)dk * (u32)nj);
+    const int i0 = ri[PR_I0], type = ri[PR_TYPE];
+    const float fj = (float)dj, fk = (float)dk;
+    float tlo = 0.0f, thi = (float)ri[PR_NI];
+    bool empty = false;
+#pragma unroll
+    for (int c = 0; c < 5; c++) {
+        const float s = fmaf(rec[4 * c + 2], fk, fmaf(rec[4 * c + 1], fj, rec[4 * c]));
+        const float inv = rec[4 * c + 3], t = -s * inv;
+        if (inv > 0.0f) tlo = fmaxf(tlo, t);
+        else if (inv < 0.0f) thi = fminf(thi, t);
+        else if (s < 0.0f) empty = true;
+    }
+    const int j = ri[PR_J0] + dj, k = ri[PR_K0] + dk;
+    const float h = g.h, eps = g.eps;
+    const float y = fmaf((float)j, h, g.oy), z = fmaf((float)k, h, g.oz);
     const float reach = g.band + g.guard;          // accept d < reach; the emit pass decides exactly
-    const float eps = g.eps, h = g.h;
-    float tlo = 0.0f, thi = (float)(H.i1 - H.i0);
-    if (G.type == 0) {
-        // ---- face slab: three inward side planes through the edges + the slab
-        f3 a = ld3(G.f), e0 = ld3(G.f + 3) - a, ec = ld3(G.f + 6) - a, n = ld3(G.f + 9);
-        f3 e1 = ec - e0;
-        f3 m0 = cross(n, e0), m1 = cross(n, e1), m2 = cross(ec, n);          // inward, |m_i| = |edge_i|
-        float t0 = eps * sqrtf(dot(e0, e0)), t1 = eps * sqrtf(dot(e1, e1)), t2 = eps * sqrtf(dot(ec, ec));
-        f3 r0 = mk<float>(x0 - a.x, y - a.y, z - a.z);
-        if (!g.aabb_mode) {
-            clip_ge(dot(m0, r0), h * m0.x, -2.0f * t0, tlo, thi);
-            clip_ge(dot(m1, r0 - e0), h * m1.x, -2.0f * t1, tlo, thi);
-            clip_ge(dot(m2, r0 - ec), h * m2.x, -2.0f * t2, tlo, thi);
-            float dn0 = dot(n, r0), gn = h * n.x;
-            clip_ge(dn0, gn, -(reach + eps), tlo, thi);
-            clip_ge(-dn0, -gn, -(reach + eps), tlo, thi);
-        }
-        if (!(tlo <= thi)) return;
-        int ia = H.i0 + (int)ceilf(tlo), ib = H.i0 + (int)floorf(thi);
-        for (int i = ia; i <= ib; i++) {
-            f3 r = mk<float>(fmaf((float)i, h, g.ox) - a.x, r0.y, r0.z);
+    const float *G = rec + PR_GEO;
+    if (type == 2) {
+        // ball of radius reach about the vertex
+        const float ry = y - G[1], rz = z - G[2];
+        const float rem = reach * reach - ry * ry - rz * rz;
+        if (rem < 0.0f) return;
+        const float xr = sqrtf(rem), inv_h = 1.0f / h, x0 = fmaf((float)i0, h, g.ox);
+        tlo = fmaxf(tlo, (G[0] - xr - x0) * inv_h - 1e-2f);
+        thi = fminf(thi, (G[0] + xr - x0) * inv_h + 1e-2f);
+    }
+    if (empty || !(tlo <= thi)) return;
+    const int ia = i0 + (int)ceilf(tlo), ib = i0 + (int)floorf(thi);
+    if (ia + lane0 > ib) return;
+    const int id = ri[PR_ID];
+    if (type == 0) {
+        const f3 a = ld3(G), e0 = ld3(G + 3), ec = ld3(G + 6), n = ld3(G + 9);
+        const f3 e1 = ec - e0;
+        const f3 m0 = cross(n, e0), m1 = cross(n, e1), m2 = cross(ec, n);
+        const float t0 = eps * sqrtf(dot(e0, e0)), t1 = eps * sqrtf(dot(e1, e1)), t2 = eps * sqrtf(dot(ec, ec));
+        const float ry = y - a.y, rz = z - a.z;
+        for (int i = ia + lane0; i <= ib; i += STRIDE) {
+            const f3 r = mk<float>(fmaf((float)i, h, g.ox) - a.x, ry, rz);
             tested++;
             float d;
             if (g.aabb_mode) {
                 int rg; f3 q;
                 d = tri_closest<float>(r, e0, ec, n, rg, q);
             } else {
-                float s0 = dot(m0, r), s1 = dot(m1, r - e0), s2 = dot(m2, r - ec);
+                const float s0 = dot(m0, r), s1 = dot(m1, r - e0), s2 = dot(m2, r - ec);
                 if (s0 < -t0 || s1 < -t1 || s2 < -t2) continue;
                 if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f) d = fabsf(dot(n, r));
                 else { int rg; f3 q; d = tri_closest<float>(r, e0, ec, n, rg, q); }   // eps margin: exact clamped distance
             }
-            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, G.id); }
+            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id); }
         }
-    } else if (G.type == 1) {
-        // ---- edge wedge: beyond both faces' side planes, between the end caps
-        f3 a = ld3(G.f), ab = ld3(G.f + 3) - a, n1 = ld3(G.f + 6), n2 = ld3(G.f + 9);
-        float L = sqrtf(dot(ab, ab));
-        f3 u = (1.0f / L) * ab;
-        f3 w1 = cross(u, n1), w2 = cross(n2, u);
-        f3 r0 = mk<float>(x0 - a.x, y - a.y, z - a.z);
-        float tu = dot(u, r0), gu = h * u.x;
-        clip_ge(tu, gu, -2.0f * eps, tlo, thi);
-        clip_ge(-tu, -gu, -(L + 2.0f * eps), tlo, thi);
-        clip_ge(dot(w1, r0), h * w1.x, -2.0f * eps, tlo, thi);
-        clip_ge(dot(w2, r0), h * w2.x, -2.0f * eps, tlo, thi);
-        if (!(tlo <= thi)) return;
-        int ia = H.i0 + (int)ceilf(tlo), ib = H.i0 + (int)floorf(thi);
-        for (int i = ia; i <= ib; i++) {
-            f3 r = mk<float>(fmaf((float)i, h, g.ox) - a.x, r0.y, r0.z);
+    } else if (type == 1) {
+        const f3 a = ld3(G), u = ld3(G + 3), w1 = ld3(G + 7), w2 = ld3(G + 10);
+        const float L = G[6];
+        const float ry = y - a.y, rz = z - a.z;
+        for (int i = ia + lane0; i <= ib; i += STRIDE) {
+            const f3 r = mk<float>(fmaf((float)i, h, g.ox) - a.x, ry, rz);
             tested++;
-            float t = dot(u, r);
+            const float t = dot(u, r);
             if (t < -eps || t > L + eps || dot(w1, r) < -eps || dot(w2, r) < -eps) continue;
-            float tc = fminf(fmaxf(t, 0.0f), L);
-            f3 q = r - tc * u;
-            float d = sqrtf(dot(q, q));
-            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, G.id); }
+            const float tc = fminf(fmaxf(t, 0.0f), L);
+            const f3 q = r - tc * u;
+            const float d = sqrtf(dot(q, q));
+            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id); }
         }
     } else {
-        // ---- vertex cone / hemisphere (eq.10, 362-364)
-        f3 v = ld3(G.f), A = ld3(G.f + 3);
-        float c = G.f[6];
-        float ry = y - v.y, rz = z - v.z;
-        float rem = reach * reach - ry * ry - rz * rz;
-        if (rem < 0.0f) return;
-        float xr = sqrtf(rem), inv_h = 1.0f / h;
-        tlo = fmaxf(tlo, (v.x - xr - x0) * inv_h - 1e-2f);
-        thi = fminf(thi, (v.x + xr - x0) * inv_h + 1e-2f);
-        if (!(tlo <= thi)) return;
-        int ia = H.i0 + (int)ceilf(tlo), ib = H.i0 + (int)floorf(thi);
-        for (int i = ia; i <= ib; i++) {
-            f3 r = mk<float>(fmaf((float)i, h, g.ox) - v.x, ry, rz);
+        const f3 v = ld3(G), A = ld3(G + 3);
+        const float c = G[6];
+        const float ry = y - v.y, rz = z - v.z;
+        for (int i = ia + lane0; i <= ib; i += STRIDE) {
+            const f3 r = mk<float>(fmaf((float)i, h, g.ox) - v.x, ry, rz);
             tested++;
-            float d = sqrtf(dot(r, r));
+            const float d = sqrtf(dot(r, r));
             if (d >= reach || dot(A, r) < c * d - eps) continue;
             accepted++;
-            put_min(g, table, scratch, i, j, k, d, G.id);
+            put_min(g, table, scratch, i, j, k, d, id);
         }
     }
 }
 
-__global__ void __launch_bounds__(EV_BT) evaluate_kernel(MeshView mv, GridParams g, const PolyHdr *__restrict__ hdr,
-                                                         const u64 *__restrict__ off, u64 total,
-                                                         const int *__restrict__ table, u64 *__restrict__ scratch,
-                                                         u64 *__restrict__ ctr) {
-    __shared__ u64 s_off[EV_CH + 1];
-    __shared__ PolyHdr s_hdr[EV_CH];
-    __shared__ Geo s_geo[EV_CH];
-    __shared__ int64_t s_plo, s_phi;
-    __shared__ u32 s_stat[2];
-    const u64 w0 = (u64)blockIdx.x * EV_IPB;
-    const u64 w1 = (w0 + EV_IPB < total) ? w0 + EV_IPB : total;
-    if (threadIdx.x < 2) {
-        // polyhedron holding item w: largest p with off[p] <= w (off is non-decreasing, off[P] = total)
-        u64 w = threadIdx.x == 0 ? w0 : w1 - 1;
-        int64_t lo = 0, hi = mv.P;          // invariant: off[lo] <= w < off[hi]
-        while (hi - lo > 1) {
-            int64_t mid = (lo + hi) >> 1;
-            if (off[mid] <= w) lo = mid; else hi = mid;
-        }
-        if (threadIdx.x == 0) { s_plo = lo; s_stat[0] = s_stat[1] = 0; } else s_phi = lo;
+__device__ __forceinline__ void add_stats(u64 *__restrict__ ctr, u32 tested, u32 accepted, u32 rows) {
+    // warp-reduced, spread over CTR_SLOTS lines: same-address atomics serialise in L2
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+        tested += __shfl_xor_sync(0xffffffffu, tested, o);
+        accepted += __shfl_xor_sync(0xffffffffu, accepted, o);
+        rows += __shfl_xor_sync(0xffffffffu, rows, o);
     }
-    __syncthreads();
-    const int64_t plo = s_plo, phi = s_phi;
+    if ((threadIdx.x & 31) == 0) {
+        u64 *s = ctr + CTR_SPREAD + ((blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) & (CTR_SLOTS - 1)) * 8;
+        if (tested) atomicAdd(s + SP_TESTED, (u64)tested);
+        if (accepted) atomicAdd(s + SP_ACCEPTED, (u64)accepted);
+        if (rows) atomicAdd(s + SP_ROWS, (u64)rows);
+    }
+}
+
+#define ES_WARPS 4
+__global__ void __launch_bounds__(32 * ES_WARPS) evaluate_small_kernel(MeshView mv, GridParams g,
+                                                                       const PolyHdr *__restrict__ hdr,
+                                                                       const int *__restrict__ table,
+                                                                       u64 *__restrict__ scratch, u64 *__restrict__ ctr) {
+    __shared__ float s_rec[ES_WARPS][32][PR_WORDS];
+    __shared__ int s_ex[ES_WARPS][33];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t p = ((int64_t)blockIdx.x * ES_WARPS + w) * 32 + lane;
+    int rows = 0;
+    if (p < mv.P) {
+        const PolyHdr H = hdr[p];
+        if (H.rows != 0 && !(H.rows & ROWS_BIG)) {
+            rows = (int)H.rows;
+            build_record(mv, g, p, H, s_rec[w][lane]);
+        }
+    }
+    int inc = rows;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int v = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += v;
+    }
+    const int total = __shfl_sync(0xffffffffu, inc, 31);
+    if (total == 0) return;
+    s_ex[w][lane] = inc - rows;
+    if (lane == 31) s_ex[w][32] = total;
+    __syncwarp();
     u32 tested = 0, accepted = 0;
-    for (int64_t q0 = plo; q0 <= phi; q0 += EV_CH) {
-        const int cn = (int)((phi - q0 + 1 < EV_CH) ? (phi - q0 + 1) : EV_CH);
-        __syncthreads();
-        for (int i = threadIdx.x; i <= cn; i += EV_BT) s_off[i] = off[q0 + i];
-        for (int i = threadIdx.x; i < cn; i += EV_BT) {
-            int64_t p = q0 + i;
-            PolyHdr H = hdr[p];
-            s_hdr[i] = H;
-            if (H.rows) {
-                Geo G;
-                if (p < mv.F) {
-                    const float *T = mv.soup + 9 * p, *N = mv.fn + 3 * p;
+    for (int base = 0; base < total; base += 32) {
+        const int r = base + lane;
+        if (r < total) {
+            int o = 0;                       // largest o with s_ex[o] <= r: the owner of row r
 #pragma unroll
-                    for (int c = 0; c < 9; c++) G.f[c] = T[c];
-                    G.f[9] = N[0]; G.f[10] = N[1]; G.f[11] = N[2];
-                    G.id = (int)p; G.type = 0;
-                } else if (p < (int64_t)mv.F + mv.E) {
-                    const EdgeRec &r = mv.erec[p - mv.F];
-#pragma unroll
-                    for (int c = 0; c < 3; c++) { G.f[c] = r.a[c]; G.f[3 + c] = r.b[c]; G.f[6 + c] = r.n1[c]; G.f[9 + c] = r.n2[c]; }
-                    G.id = r.tri; G.type = 1;
-                } else {
-                    int64_t q = p - mv.F - mv.E;
-                    const VertexRec &r = mv.vrec[q >> 1];
-                    float sg = (q & 1) ? -1.0f : 1.0f;
-#pragma unroll
-                    for (int c = 0; c < 3; c++) { G.f[c] = r.pos[c]; G.f[3 + c] = sg * r.axis[c]; }
-                    G.f[6] = r.cos_cone;
-                    G.id = mv.vmint[q >> 1]; G.type = 2;
-                }
-                G.pad0 = G.pad1 = 0;
-                s_geo[i] = G;
-            }
-        }
-        __syncthreads();
-        const u64 lo = s_off[0] > w0 ? s_off[0] : w0;
-        const u64 hi = s_off[cn] < w1 ? s_off[cn] : w1;
-        for (u64 w = lo + threadIdx.x; w < hi; w += EV_BT) {
-            int a = 0, b = cn;              // invariant: s_off[a] <= w < s_off[b]
-            while (b - a > 1) {
-                int mid = (a + b) >> 1;
-                if (s_off[mid] <= w) a = mid; else b = mid;
-            }
-            process_row(g, s_geo[a], s_hdr[a], (u32)(w - s_off[a]), table, scratch, tested, accepted);
+            for (int st = 16; st; st >>= 1)
+                if (s_ex[w][o + st] <= r) o += st;
+            process_row<1>(g, s_rec[w][o], (u32)(r - s_ex[w][o]), 0, table, scratch, tested, accepted);
         }
     }
-    atomicAdd(&s_stat[0], tested);
-    atomicAdd(&s_stat[1], accepted);
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        if (s_stat[0]) atomicAdd(&ctr[CTR_TESTED], (u64)s_stat[0]);
-        if (s_stat[1]) atomicAdd(&ctr[CTR_ACCEPTED], (u64)s_stat[1]);
+    add_stats(ctr, tested, accepted, (u32)rows);
+}
+
+// One block per big polyhedron (dynamic fetch): warps stride over its rows, lanes over x.
+#define EBIG_BT 256
+__global__ void __launch_bounds__(EBIG_BT) evaluate_big_kernel(MeshView mv, GridParams g,
+                                                               const PolyHdr *__restrict__ hdr,
+                                                               const u32 *__restrict__ big_list,
+                                                               const int *__restrict__ table,
+                                                               u64 *__restrict__ scratch, u64 *__restrict__ ctr) {
+    __shared__ float s_rec[PR_WORDS];
+    __shared__ u64 s_e;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const u64 nbig = ctr[CTR_BIG];
+    u32 tested = 0, accepted = 0, rows_done = 0;
+    while (true) {
+        __syncthreads();
+        if (threadIdx.x == 0) s_e = atomicAdd(&ctr[CTR_BIG_NEXT], 1ull);
+        __syncthreads();
+        const u64 e = s_e;
+        if (e >= nbig) break;
+        const int64_t p = (int64_t)big_list[e];
+        const PolyHdr H = hdr[p];
+        if (threadIdx.x == 0) build_record(mv, g, p, H, s_rec);
+        __syncthreads();
+        const u32 rows = H.rows & ~ROWS_BIG;
+        for (u32 r = (u32)w; r < rows; r += EBIG_BT / 32)
+            process_row<32>(g, s_rec, r, lane, table, scratch, tested, accepted);
+        if (threadIdx.x == 0) rows_done += rows;
     }
+    add_stats(ctr, tested, accepted, rows_done);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -580,10 +667,9 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
     mv.P = m->F + m->E + 2 * m->V;
     const int64_t P = mv.P;
     const int64_t nbricks = (int64_t)g.nbx * g.nby * g.nbz;
-    int64_t scan_n = P > nbricks ? P : nbricks;
     CKS(ensure(m, &m->hdr, &m->hdr_cap, (size_t)P, st));
-    CKS(ensure(m, &m->offsets, &m->offsets_cap, (size_t)P + 1, st));
-    CKS(ensure(m, &m->scan_ws, &m->scan_ws_cap, scan_ws_elems(scan_n), st));
+    CKS(ensure(m, &m->big_list, &m->big_list_cap, (size_t)P, st));
+    CKS(ensure(m, &m->scan_ws, &m->scan_ws_cap, scan_ws_elems(nbricks), st));
     CKS(ensure(m, &m->brick_flag, &m->brick_flag_cap, (size_t)nbricks, st));
     CKS(ensure(m, &m->brick_table, &m->brick_table_cap, (size_t)nbricks, st));
     CKS(ensure(m, &m->brick_list, &m->brick_list_cap, (size_t)nbricks, st));
@@ -611,35 +697,30 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
         CK(cudaEventRecord(m->ev_join, m->side));
     }
     CK(cudaMemsetAsync(m->brick_flag, 0, (size_t)nbricks, st));
-    CK(cudaMemsetAsync(m->d_ctr + CTR_POLY, 0, sizeof(u64) * (CTR_COUNT - CTR_POLY), st));
+    CK(cudaMemsetAsync(m->d_ctr + CTR_POLY, 0, sizeof(u64) * (CTR_TOTAL - CTR_POLY), st));
 
     // A5 + A6: clip, count rows, mark bricks; prefix sums
     stage_mark(m, SDF_T_CLIP_SCAN, 0, st);
-    KL; clip_count_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(mv, g, m->hdr, m->brick_flag);
-    KL; count_nonempty_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(m->hdr, P, m->d_ctr);
-    CKS(launch_scan(RowsIn{m->hdr}, RowsOut{m->offsets}, P, m->scan_ws, m->d_ctr + CTR_ITEMS, st));
-    KL; set_last_offset_kernel<<<1, 1, 0, st>>>(m->offsets, P, m->d_ctr + CTR_ITEMS);
+    KL; clip_count_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(mv, g, m->hdr, m->brick_flag, m->big_list, m->d_ctr);
     CKS(launch_scan(BrickIn{m->brick_flag}, BrickOut{m->brick_table, m->brick_list}, nbricks, m->scan_ws, m->d_ctr + CTR_BRICKS, st));
     CK(cudaGetLastError());
 
     // host crossing: totals size the launch and the scratch
-    u64 tot[2];
-    CK(cudaMemcpyAsync(tot, m->d_ctr + CTR_ITEMS, sizeof(tot), cudaMemcpyDeviceToHost, st));
+    u64 bricks = 0;
+    CK(cudaMemcpyAsync(&bricks, m->d_ctr + CTR_BRICKS, sizeof(bricks), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
-    const u64 items = tot[0], bricks = tot[1];
     stage_mark(m, SDF_T_CLIP_SCAN, 1, st);
     CKS(ensure(m, &m->scratch, &m->scratch_cap, (size_t)(bricks ? bricks : 1) * BRICK_CELLS, st));
     stage_mark(m, SDF_T_CLEAR, 0, st);
     if (bricks) CK(cudaMemsetAsync(m->scratch, 0xFF, (size_t)bricks * BRICK_CELLS * sizeof(u64), st));
     stage_mark(m, SDF_T_CLEAR, 1, st);
 
-    // A7
-    if (items) {
-        u64 nblk = (items + EV_IPB - 1) / EV_IPB;
-        if (nblk > 0x7FFFFFFFull) return SDF_EINVAL;
+    // A7: small polyhedra flattened per warp, big ones one block each (dynamic fetch)
+    if (bricks) {
         stage_mark(m, SDF_T_EVALUATE, 0, st);
-        KL; evaluate_kernel<<<(unsigned)nblk, EV_BT, 0, st>>>(mv, g, m->hdr, m->offsets, items, m->brick_table, m->scratch,
-                                                         m->d_ctr);
+        const int64_t nblk = (P + 32 * ES_WARPS - 1) / (32 * ES_WARPS);
+        KL; evaluate_small_kernel<<<(unsigned)nblk, 32 * ES_WARPS, 0, st>>>(mv, g, m->hdr, m->brick_table, m->scratch, m->d_ctr);
+        KL; evaluate_big_kernel<<<(unsigned)(sms * 4), EBIG_BT, 0, st>>>(mv, g, m->hdr, m->big_list, m->brick_table, m->scratch, m->d_ctr);
         stage_mark(m, SDF_T_EVALUATE, 1, st);
     }
     // A8b: join the fill, then overwrite the active bricks
@@ -651,7 +732,6 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
     }
     CK(cudaGetLastError());
     m->last_stream = st;
-    m->h_ctr[CTR_ITEMS] = items;
     m->h_ctr[CTR_BRICKS] = bricks;
     m->last_bricks_total = nbricks;
     return SDF_OK;

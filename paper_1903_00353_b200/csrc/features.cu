@@ -380,9 +380,9 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     CKS(dev_alloc(al, (void **)&m->fn, sizeof(float) * 3 * F, st));
     CKS(dev_alloc(al, (void **)&m->cvid, sizeof(int) * 3 * F, st));
     CKS(dev_alloc(al, (void **)&m->adj, sizeof(int) * 3 * F, st));
-    CKS(dev_alloc(al, (void **)&m->d_ctr, sizeof(u64) * CTR_COUNT, st));
+    CKS(dev_alloc(al, (void **)&m->d_ctr, sizeof(u64) * CTR_TOTAL, st));
     CKS(dev_alloc(al, (void **)&m->d_flags, sizeof(int) * 4, st));
-    CK(cudaMemsetAsync(m->d_ctr, 0, sizeof(u64) * CTR_COUNT, st));
+    CK(cudaMemsetAsync(m->d_ctr, 0, sizeof(u64) * CTR_TOTAL, st));
     CK(cudaMemsetAsync(m->d_flags, 0, sizeof(int) * 4, st));
     CK(cudaMemsetAsync(m->adj, 0xFF, sizeof(int) * 3 * F, st));
 
