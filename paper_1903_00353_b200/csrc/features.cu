@@ -17,12 +17,14 @@
 static inline unsigned blocks_for(int64_t n, int bt = FB) { return (unsigned)((n + bt - 1) / bt); }
 
 // ---------------------------------------------------------------------------------------
-// A0 ingest + A1 weld keys
+// A0 ingest + A1 weld: open-addressing hash table keyed by the exact coordinate bits
 // ---------------------------------------------------------------------------------------
+#define EMPTY32 0xFFFFFFFFu
+#define HE_MATCHED 0x80000000u
+
 __device__ __forceinline__ u32 mix32(u32 x, u32 y, u32 z) {
-    // 96 -> 32 bit avalanche hash of the exact coordinate bits.  Only has to make equal
-    // vertices adjacent after sorting ("the actual order does not matter");
-    // equality itself is decided on the exact bits.
+    // 96 -> 32 bit avalanche hash.  It only spreads the keys over the table
+    // ("the actual order does not matter"); equality is decided on the exact bits.
     u32 h = x * 0x9E3779B1u;
     h ^= h >> 15; h *= 0x85EBCA77u;
     h ^= y; h *= 0xC2B2AE3Du;
@@ -31,89 +33,61 @@ __device__ __forceinline__ u32 mix32(u32 x, u32 y, u32 z) {
     return h;
 }
 
-// one thread per corner (3 floats): reject non-finite input, canonicalise -0 -> +0, hash
-__global__ void __launch_bounds__(FB) ingest_kernel(const float *__restrict__ in, float *__restrict__ soup,
-                                                    int ncorner, u32 *__restrict__ keys, u32 *__restrict__ vals,
-                                                    int *__restrict__ flags) {
+__device__ __forceinline__ u32 canon_bits(float x) { return __float_as_uint(x + 0.0f); }   // -0 + +0 = +0
+
+// One thread per corner (3 floats): reject non-finite input, canonicalise -0 -> +0, then
+// find-or-insert the vertex in the weld table (linear probing).  A slot holds a corner index
+// of its vertex; identity is checked on the exact bits of that corner in the (immutable)
+// input, and the slot converges to the LOWEST corner index of the vertex (atomicMin), so the
+// representative does not depend on the insertion order.  slot[c] = table position of c.
+__global__ void __launch_bounds__(FB) ingest_weld_kernel(const float *__restrict__ in, float *__restrict__ soup,
+                                                         int ncorner, u32 *wtab, u32 mask, u32 *__restrict__ slot,
+                                                         int *__restrict__ flags) {
     int c = blockIdx.x * FB + threadIdx.x;
     if (c >= ncorner) return;
     float x = in[3 * (size_t)c], y = in[3 * (size_t)c + 1], z = in[3 * (size_t)c + 2];
     if (!(isfinite(x) && isfinite(y) && isfinite(z))) atomicOr(flags, ERRB_NONFINITE);
-    x += 0.0f; y += 0.0f; z += 0.0f;      // -0 + +0 = +0 (round to nearest)
+    x += 0.0f; y += 0.0f; z += 0.0f;
     soup[3 * (size_t)c] = x; soup[3 * (size_t)c + 1] = y; soup[3 * (size_t)c + 2] = z;
-    keys[c] = mix32(__float_as_uint(x), __float_as_uint(y), __float_as_uint(z));
-    vals[c] = (u32)c;
-}
-
-__device__ __forceinline__ bool same_vertex(const float *__restrict__ soup, u32 c0, u32 c1) {
-    const u32 *p = (const u32 *)(soup + 3 * (size_t)c0), *q = (const u32 *)(soup + 3 * (size_t)c1);
-    return p[0] == q[0] && p[1] == q[1] && p[2] == q[2];
-}
-
-// head[s] = 1 iff sorted corner s starts a new vertex (exact bits differ from s-1).
-// A new vertex inside an equal-hash run is a hash collision: counted, fixed by weld_fix.
-__global__ void __launch_bounds__(FB) weld_flags_kernel(const float *__restrict__ soup, const u32 *__restrict__ keys,
-                                                        const u32 *__restrict__ vals, int n,
-                                                        unsigned char *__restrict__ head, u64 *__restrict__ ctr) {
-    int s = blockIdx.x * FB + threadIdx.x;
-    if (s >= n) return;
-    bool h = true;
-    if (s > 0) {
-        h = !same_vertex(soup, vals[s], vals[s - 1]);
-        if (h && keys[s] == keys[s - 1]) atomicAdd(&ctr[CTR_WELD_BAD], 1ull);
+    const u32 bx = __float_as_uint(x), by = __float_as_uint(y), bz = __float_as_uint(z);
+    u32 h = mix32(bx, by, bz) & mask;
+    for (;;) {
+        u32 cur = *(volatile u32 *)(wtab + h);
+        if (cur == EMPTY32) {
+            cur = atomicCAS(wtab + h, EMPTY32, (u32)c);
+            if (cur == EMPTY32) break;
+        }
+        const float *q = in + 3 * (size_t)cur;
+        if (canon_bits(q[0]) == bx && canon_bits(q[1]) == by && canon_bits(q[2]) == bz) {
+            if ((u32)c < cur) atomicMin(wtab + h, (u32)c);     // the minimum only ever decreases
+            break;
+        }
+        h = (h + 1) & mask;
     }
-    head[s] = h ? 1 : 0;
+    slot[c] = h;
 }
 
-__device__ __forceinline__ bool corner_less(const float *__restrict__ soup, u32 c0, u32 c1) {
-    const u32 *p = (const u32 *)(soup + 3 * (size_t)c0), *q = (const u32 *)(soup + 3 * (size_t)c1);
-    if (p[0] != q[0]) return p[0] < q[0];
-    if (p[1] != q[1]) return p[1] < q[1];
-    if (p[2] != q[2]) return p[2] < q[2];
-    return c0 < c1;
-}
-
-// Only does work when a hash collision put distinct vertices in one equal-key run: the
-// thread at the head of such a run orders it by the exact bits (insertion sort, runs are
-// a few corners long) and recomputes its head flags.  This is the paper's per-group
-// regrouping, needed here only for the ~V^2/2^33 colliding pairs.
-__global__ void __launch_bounds__(FB) weld_fix_kernel(const float *__restrict__ soup, const u32 *__restrict__ keys,
-                                                      u32 *__restrict__ vals, int n, unsigned char *__restrict__ head,
-                                                      const u64 *__restrict__ ctr) {
-    if (ctr[CTR_WELD_BAD] == 0) return;
-    int s = blockIdx.x * FB + threadIdx.x;
-    if (s >= n) return;
-    if (s > 0 && keys[s] == keys[s - 1]) return;       // not the head of an equal-hash run
-    int e = s + 1;
-    bool mixed = false;
-    while (e < n && keys[e] == keys[s]) { mixed |= (head[e] != 0); e++; }
-    if (!mixed) return;
-    for (int i = s + 1; i < e; i++) {
-        u32 v = vals[i];
-        int j = i - 1;
-        while (j >= s && corner_less(soup, v, vals[j])) { vals[j + 1] = vals[j]; j--; }
-        vals[j + 1] = v;
-    }
-    for (int i = s + 1; i < e; i++) head[i] = same_vertex(soup, vals[i], vals[i - 1]) ? 0 : 1;
+// head[c] = 1 iff c is the lowest corner of its vertex; vertex ids are the ranks of the heads
+__global__ void __launch_bounds__(FB) weld_head_kernel(const u32 *__restrict__ wtab, const u32 *__restrict__ slot,
+                                                       int n, unsigned char *__restrict__ head) {
+    int c = blockIdx.x * FB + threadIdx.x;
+    if (c < n) head[c] = (wtab[slot[c]] == (u32)c) ? 1 : 0;
 }
 
 struct HeadIn {
     const unsigned char *head;
     __device__ u64 operator()(int64_t i) const { return head[i]; }
 };
-struct HeadOut {
-    const u32 *vals; int *cvid; int *vcorner;
+struct HeadOut {      // the head replaces the corner index in its slot by the vertex id
+    u32 *wtab; const u32 *slot; int *vcorner;
     __device__ void operator()(int64_t i, u64 ex, u64 v) const {
-        int vid = (int)(ex + v) - 1;          // inclusive count of heads - 1
-        u32 c = vals[i];
-        cvid[c] = vid;
-        if (v) vcorner[vid] = (int)c;
+        if (v) { wtab[slot[i]] = (u32)ex; vcorner[ex] = (int)i; }
     }
 };
 
 // ---------------------------------------------------------------------------------------
-// A3 triangle geometry: unit normal, corner angles, fixed-point pseudonormal accumulation,
-// half-edge keys for A2
+// A3 triangle geometry: corner -> vertex ids, unit normal, corner angles, fixed-point
+// pseudonormal accumulation, number of forward half-edges (for the edge ids of A2)
 // ---------------------------------------------------------------------------------------
 #define FIXSCALE 1099511627776.0   /* 2^40 */
 
@@ -138,14 +112,19 @@ __device__ __forceinline__ bool tri_normal64(const float *__restrict__ T, double
     return true;
 }
 
-__global__ void __launch_bounds__(FB) tri_geom_kernel(const float *__restrict__ soup, const int *__restrict__ cvid,
-                                                      int F, float *__restrict__ fn, u64 *__restrict__ vacc,
-                                                      u64 *__restrict__ ekeys, u32 *__restrict__ evals,
-                                                      int *__restrict__ flags) {
+__global__ void __launch_bounds__(FB) tri_geom_kernel(const float *__restrict__ soup, const u32 *__restrict__ wtab,
+                                                      const u32 *__restrict__ slot, int F, int *__restrict__ cvid,
+                                                      float *__restrict__ fn, u64 *__restrict__ vacc,
+                                                      unsigned char *__restrict__ fcnt, int *__restrict__ flags) {
     int t = blockIdx.x * FB + threadIdx.x;
     if (t >= F) return;
     const float *T = soup + 9 * (size_t)t;
-    int v[3] = {cvid[3 * (size_t)t], cvid[3 * (size_t)t + 1], cvid[3 * (size_t)t + 2]};
+    int v[3];
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        v[k] = (int)wtab[slot[3 * (size_t)t + k]];
+        cvid[3 * (size_t)t + k] = v[k];
+    }
     double n[3], p[3][3];
     bool ok = tri_normal64(T, n, p);
     if (!ok || v[0] == v[1] || v[1] == v[2] || v[2] == v[0]) {   // PAPER.md:137 "we disallow faces of zero area"
@@ -153,6 +132,7 @@ __global__ void __launch_bounds__(FB) tri_geom_kernel(const float *__restrict__ 
         n[0] = n[1] = 0.0; n[2] = 1.0;
     }
     fn[3 * (size_t)t] = (float)n[0]; fn[3 * (size_t)t + 1] = (float)n[1]; fn[3 * (size_t)t + 2] = (float)n[2];
+    int nf = 0;
 #pragma unroll
     for (int k = 0; k < 3; k++) {
         int k1 = (k + 1) % 3, k2 = (k + 2) % 3;
@@ -167,78 +147,145 @@ __global__ void __launch_bounds__(FB) tri_geom_kernel(const float *__restrict__ 
             for (int i = 0; i < 3; i++)
                 atomicAdd(&vacc[3 * (size_t)v[k] + i], (u64)(long long)llrint(alpha * n[i] * FIXSCALE));
         }
-        // half-edge 3t+k goes corner k -> k+1: key = (min vid, max vid)
-        u32 a = (u32)v[k], b = (u32)v[k1];
-        u32 lo = a < b ? a : b, hi = a < b ? b : a;
-        ekeys[3 * (size_t)t + k] = ((u64)lo << 32) | hi;
-        evals[3 * (size_t)t + k] = (u32)(3 * t + k);
+        nf += v[k] < v[k1];       // half-edge 3t+k goes corner k -> k+1; forward = ascending ids
+    }
+    fcnt[t] = (unsigned char)nf;
+}
+
+struct FcntIn {
+    const unsigned char *c;
+    __device__ u64 operator()(int64_t i) const { return c[i]; }
+};
+struct EbaseOut {
+    u32 *ebase;
+    __device__ void operator()(int64_t i, u64 ex, u64) const { ebase[i] = (u32)ex; }
+};
+
+// ---------------------------------------------------------------------------------------
+// A2 edge table: every undirected edge {u < w} of a closed, consistently oriented surface is
+// traversed once forward (u -> w) and once backward.  Forward half-edges
+// are inserted into a hash table keyed by (u,w) (the slot holds the half-edge index; its key
+// is read back from cvid); backward half-edges look their partner up and claim it.
+// The mesh is valid iff the number of claimed pairs equals 3F/2.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ u32 edge_hash(u32 u, u32 w) { return mix32(u, w, 0x51ED270Bu); }
+__device__ __forceinline__ int he_next(int he) { int k = he % 3; return he - k + (k == 2 ? 0 : k + 1); }
+
+__global__ void __launch_bounds__(FB) edge_insert_kernel(const int *__restrict__ cvid, int n, u32 *etab, u32 mask) {
+    int he = blockIdx.x * FB + threadIdx.x;
+    if (he >= n) return;
+    const u32 u = (u32)cvid[he], w = (u32)cvid[he_next(he)];
+    if (!(u < w)) return;
+    u32 h = edge_hash(u, w) & mask;
+    for (;;) {
+        u32 cur = *(volatile u32 *)(etab + h);
+        if (cur == EMPTY32) {
+            cur = atomicCAS(etab + h, EMPTY32, (u32)he);
+            if (cur == EMPTY32) return;
+        }
+        // same key already present: a second forward half-edge (invalid mesh; the pair count
+        // will fall short and the exact classification runs)
+        if ((u32)cvid[cur] == u && (u32)cvid[he_next((int)cur)] == w) return;
+        h = (h + 1) & mask;
     }
 }
 
-// ---------------------------------------------------------------------------------------
-// A2 edge table + A4 edge classes + wedge geometry: one thread per sorted half-edge
-// ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(FB) edge_pair_kernel(const u64 *__restrict__ keys, const u32 *__restrict__ vals,
-                                                       int n, const float *__restrict__ soup,
-                                                       const float *__restrict__ fn, const int *__restrict__ cvid,
-                                                       int *__restrict__ adj, EdgeRec *__restrict__ erec,
-                                                       int *__restrict__ flags, u64 *__restrict__ ctr) {
+// one thread per half-edge; backward ones claim their forward partner and write the edge
+__global__ void __launch_bounds__(FB) edge_pair_kernel(const int *__restrict__ cvid, int n, u32 *etab, u32 mask,
+                                                       const u32 *__restrict__ ebase, const float *__restrict__ soup,
+                                                       const float *__restrict__ fn, int *__restrict__ adj,
+                                                       EdgeRec *__restrict__ erec, u64 *__restrict__ ctr) {
     __shared__ u32 s_cnt[3];
     if (threadIdx.x < 3) s_cnt[threadIdx.x] = 0;
     __syncthreads();
-    int s = blockIdx.x * FB + threadIdx.x;
-    if (s < n) {
-        u64 k = keys[s];
-        bool same_prev = (s > 0) && keys[s - 1] == k;
-        bool same_next = (s + 1 < n) && keys[s + 1] == k;
-        bool even = (s & 1) == 0;
-        // closed manifold <=> every key occurs exactly twice <=> runs are aligned pairs
-        bool good = even ? (!same_prev && same_next) : (same_prev && !same_next);
-        if (!good) atomicOr(flags, ERRB_NOTCLOSED);
-        if (good && even) {
-            u32 he0 = vals[s], he1 = vals[s + 1];          // he0 < he1 (stable sort)
-            // opposite directions <=> the two half-edges start at different vertices
-            if (cvid[he0] == cvid[he1]) atomicOr(flags, ERRB_ORIENT);
-            adj[he0] = (int)he1;
-            adj[he1] = (int)he0;
-            int t0 = he0 / 3, k0 = he0 % 3, t1 = he1 / 3;
-            const float *A = soup + 9 * (size_t)t0 + 3 * k0, *B = soup + 9 * (size_t)t0 + 3 * ((k0 + 1) % 3);
-            {
-                // canonical direction a -> b = ascending exact position bits, so the record (and
-                // the fp32 rounding of every distance evaluated from it) does not depend on the
-                // order of the triangles in the soup; n1 stays the normal of the triangle that
-                // traverses a -> b
-                const u32 *pa = (const u32 *)A, *pb = (const u32 *)B;
-                bool swap = pa[0] != pb[0] ? pa[0] > pb[0] : (pa[1] != pb[1] ? pa[1] > pb[1] : pa[2] > pb[2]);
-                if (swap) {
-                    int k1 = he1 % 3;
-                    t0 = t1; t1 = he0 / 3; k0 = k1;
-                    A = soup + 9 * (size_t)t0 + 3 * k0; B = soup + 9 * (size_t)t0 + 3 * ((k0 + 1) % 3);
+    int he1 = blockIdx.x * FB + threadIdx.x;
+    if (he1 < n) {
+        const u32 w = (u32)cvid[he1], u = (u32)cvid[he_next(he1)];     // backward: w -> u with u < w
+        if (u < w) {
+            u32 h = edge_hash(u, w) & mask;
+            int he0 = -1;
+            for (;;) {
+                u32 cur = *(volatile u32 *)(etab + h);
+                if (cur == EMPTY32) break;                           // no forward partner
+                int cand = (int)(cur & ~HE_MATCHED);
+                if ((u32)cvid[cand] == u && (u32)cvid[he_next(cand)] == w) {
+                    u32 prev = atomicOr(etab + h, HE_MATCHED);
+                    if (!(prev & HE_MATCHED)) he0 = cand;            // else: a second backward half-edge
+                    break;
                 }
+                h = (h + 1) & mask;
             }
-            const float *N1 = fn + 3 * (size_t)t0, *N2 = fn + 3 * (size_t)t1;
-            EdgeRec r;
-            double u[3], n1[3], n2[3], x[3];
+            if (he0 >= 0) {
+                adj[he0] = he1;
+                adj[he1] = he0;
+                int t0 = he0 / 3, k0 = he0 % 3, t1 = he1 / 3;
+                // edge id: rank of he0 among the forward half-edges in soup order
+                const int c0 = cvid[3 * (size_t)t0], c1 = cvid[3 * (size_t)t0 + 1], c2 = cvid[3 * (size_t)t0 + 2];
+                int e = (int)ebase[t0] + (k0 > 0 ? (c0 < c1) : 0) + (k0 > 1 ? (c1 < c2) : 0);
+                const int tmin = t0 < t1 ? t0 : t1;
+                const float *A = soup + 9 * (size_t)t0 + 3 * k0, *B = soup + 9 * (size_t)t0 + 3 * ((k0 + 1) % 3);
+                {
+                    // canonical direction a -> b = ascending exact position bits, so the record (and
+                    // the fp32 rounding of every distance evaluated from it) does not depend on the
+                    // order of the triangles in the soup; n1 stays the normal of the triangle that
+                    // traverses a -> b
+                    const u32 *pa = (const u32 *)A, *pb = (const u32 *)B;
+                    bool swap = pa[0] != pb[0] ? pa[0] > pb[0] : (pa[1] != pb[1] ? pa[1] > pb[1] : pa[2] > pb[2]);
+                    if (swap) {
+                        int k1 = he1 % 3;
+                        t0 = t1; t1 = he0 / 3; k0 = k1;
+                        A = soup + 9 * (size_t)t0 + 3 * k0; B = soup + 9 * (size_t)t0 + 3 * ((k0 + 1) % 3);
+                    }
+                }
+                const float *N1 = fn + 3 * (size_t)t0, *N2 = fn + 3 * (size_t)t1;
+                EdgeRec r;
+                double ud[3], n1[3], n2[3], x[3];
 #pragma unroll
-            for (int i = 0; i < 3; i++) {
-                r.a[i] = A[i]; r.b[i] = B[i]; r.n1[i] = N1[i]; r.n2[i] = N2[i];
-                u[i] = (double)B[i] - (double)A[i]; n1[i] = N1[i]; n2[i] = N2[i];
+                for (int i = 0; i < 3; i++) {
+                    r.a[i] = A[i]; r.b[i] = B[i]; r.n1[i] = N1[i]; r.n2[i] = N2[i];
+                    ud[i] = (double)B[i] - (double)A[i]; n1[i] = N1[i]; n2[i] = N2[i];
+                }
+                double L = sqrt(ddot(ud, ud));
+                dcross(ud, n1, x);
+                double d = (L > 0.0) ? ddot(x, n2) / L : 0.0;       // PAPER.md:352 d = (ab x n1).n2, normalised
+                // flat: the wedge is thinner than 1e-6 * band and lies inside the eps-inflated
+                // neighbours (reading #5)
+                int cls = d > 1e-6 ? 1 : (d < -1e-6 ? -1 : 0);
+                r.tri = tmin;
+                r.cls = cls;
+                r.pad[0] = r.pad[1] = 0;
+                erec[e] = r;
+                atomicAdd(&s_cnt[cls > 0 ? 0 : (cls < 0 ? 1 : 2)], 1u);
             }
-            double L = sqrt(ddot(u, u));
-            dcross(u, n1, x);
-            double d = (L > 0.0) ? ddot(x, n2) / L : 0.0;       // PAPER.md:352 d = (ab x n1).n2, normalised
-            // flat: the wedge is thinner than 1e-6 * band and lies inside the eps-inflated
-            // neighbours (reading #5)
-            int cls = d > 1e-6 ? 1 : (d < -1e-6 ? -1 : 0);
-            r.tri = t0 < t1 ? t0 : t1;
-            r.cls = cls;
-            r.pad[0] = r.pad[1] = 0;
-            erec[s >> 1] = r;
-            atomicAdd(&s_cnt[cls > 0 ? 0 : (cls < 0 ? 1 : 2)], 1u);
         }
     }
     __syncthreads();
     if (threadIdx.x < 3 && s_cnt[threadIdx.x]) atomicAdd(&ctr[CTR_E_CONVEX + threadIdx.x], (u64)s_cnt[threadIdx.x]);
+}
+
+// ---- exact classification of an invalid edge table (error path only): sort the (min,max)
+// keys, a closed manifold has every key exactly twice (aligned pairs) in opposite directions
+__global__ void __launch_bounds__(FB) edge_keys_kernel(const int *__restrict__ cvid, int n, u64 *__restrict__ keys,
+                                                       u32 *__restrict__ vals) {
+    int he = blockIdx.x * FB + threadIdx.x;
+    if (he >= n) return;
+    u32 a = (u32)cvid[he], b = (u32)cvid[he_next(he)];
+    u32 lo = a < b ? a : b, hi = a < b ? b : a;
+    keys[he] = ((u64)lo << 32) | hi;
+    vals[he] = (u32)he;
+}
+__global__ void __launch_bounds__(FB) edge_validate_kernel(const u64 *__restrict__ keys, const u32 *__restrict__ vals,
+                                                           int n, const int *__restrict__ cvid, int *__restrict__ flags) {
+    int s = blockIdx.x * FB + threadIdx.x;
+    if (s >= n) return;
+    u64 k = keys[s];
+    bool same_prev = (s > 0) && keys[s - 1] == k;
+    bool same_next = (s + 1 < n) && keys[s + 1] == k;
+    bool even = (s & 1) == 0;
+    bool good = even ? (!same_prev && same_next) : (same_prev && !same_next);
+    if (!good) atomicOr(flags, ERRB_NOTCLOSED);
+    // opposite directions <=> the two half-edges start at different vertices
+    if (good && even && cvid[vals[s]] == cvid[vals[s + 1]]) atomicOr(flags, ERRB_ORIENT);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -370,6 +417,37 @@ static int status_from_flags(int f) {
     return SDF_OK;
 }
 
+static u32 pow2_at_least(u64 n) {
+    u64 c = 64;
+    while (c < n) c <<= 1;
+    return (u32)c;
+}
+
+// error path: which of NOTCLOSED / ORIENT does the invalid edge table amount to?
+static int classify_edge_errors(sdf_mesh *m, int nc, TmpPool &tmp, cudaStream_t st) {
+    if (nc & 1) {
+        int f = ERRB_NOTCLOSED;
+        CK(cudaMemcpyAsync(m->d_flags, &f, sizeof(int), cudaMemcpyHostToDevice, st));
+        return SDF_OK;
+    }
+    u64 *eka, *ekb, *scan_ws;
+    u32 *va, *vb, *hist;
+    CKS(tmp.get((void **)&eka, sizeof(u64) * nc));
+    CKS(tmp.get((void **)&ekb, sizeof(u64) * nc));
+    CKS(tmp.get((void **)&va, sizeof(u32) * nc));
+    CKS(tmp.get((void **)&vb, sizeof(u32) * nc));
+    CKS(tmp.get((void **)&hist, sizeof(u32) * radix_hist_elems(nc)));
+    CKS(tmp.get((void **)&scan_ws, sizeof(u64) * scan_ws_elems((int64_t)radix_hist_elems(nc))));
+    KL; edge_keys_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, eka, va);
+    int shifts[8];
+    for (int p = 0; p < 8; p++) shifts[p] = 8 * p;
+    bool first;
+    CKS(radix_sort_pairs<u64>(eka, va, ekb, vb, nc, shifts, 8, hist, scan_ws, st, &first));
+    KL; edge_validate_kernel<<<blocks_for(nc), FB, 0, st>>>(first ? eka : ekb, first ? va : vb, nc, m->cvid, m->d_flags);
+    CK(cudaGetLastError());
+    return SDF_OK;
+}
+
 int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st) {
     const int64_t F = m->F;
     const int nc = (int)(3 * F);
@@ -386,7 +464,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     CK(cudaMemsetAsync(m->d_flags, 0, sizeof(int) * 4, st));
     CK(cudaMemsetAsync(m->adj, 0xFF, sizeof(int) * 3 * F, st));
 
-    // ---- A0: ingest
+    // ---- A0 ingest + A1 weld (hash table on the exact coordinate bits)
     stage_mark(m, SDF_T_INGEST_WELD, 0, st);
     const float *src = tri;
     float *staging = nullptr;
@@ -395,33 +473,25 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
         CK(cudaMemcpyAsync(staging, tri, sizeof(float) * 9 * F, cudaMemcpyHostToDevice, st));
         src = staging;
     }
-    u32 *k32a, *k32b, *va, *vb, *hist;
+    const u32 capw = pow2_at_least((u64)nc + (u64)nc / 4 + 1);     // load <= 0.8 even if no vertex is shared
+    const u32 cape = pow2_at_least((u64)nc + 1);                   // <= 3F/2 forward half-edges: load <= 0.5
+    u32 *wtab, *slot, *etab, *ebase;
     u64 *scan_ws;
-    unsigned char *head;
+    unsigned char *head, *fcnt;
     int *vcorner;
-    CKS(tmp.get((void **)&k32a, sizeof(u32) * nc));
-    CKS(tmp.get((void **)&k32b, sizeof(u32) * nc));
-    CKS(tmp.get((void **)&va, sizeof(u32) * nc));
-    CKS(tmp.get((void **)&vb, sizeof(u32) * nc));
-    CKS(tmp.get((void **)&hist, sizeof(u32) * radix_hist_elems(nc)));
-    size_t ws_elems = scan_ws_elems((int64_t)nc > (int64_t)radix_hist_elems(nc) ? (int64_t)nc : (int64_t)radix_hist_elems(nc));
-    CKS(tmp.get((void **)&scan_ws, sizeof(u64) * ws_elems));
+    CKS(tmp.get((void **)&wtab, sizeof(u32) * (size_t)capw));
+    CKS(tmp.get((void **)&slot, sizeof(u32) * nc));
+    CKS(tmp.get((void **)&etab, sizeof(u32) * (size_t)cape));
+    CKS(tmp.get((void **)&ebase, sizeof(u32) * (size_t)F));
+    CKS(tmp.get((void **)&scan_ws, sizeof(u64) * scan_ws_elems((int64_t)nc)));
     CKS(tmp.get((void **)&head, (size_t)nc));
+    CKS(tmp.get((void **)&fcnt, (size_t)F));
     CKS(tmp.get((void **)&vcorner, sizeof(int) * nc));      // V <= 3F
-    KL; ingest_kernel<<<blocks_for(nc), FB, 0, st>>>(src, m->soup, nc, k32a, va, m->d_flags);
-
-    // ---- A1: weld (radix sort of the hashed keys, exact compare of neighbours)
-    {
-        const int shifts[4] = {0, 8, 16, 24};
-        bool first;
-        CKS(radix_sort_pairs<u32>(k32a, va, k32b, vb, nc, shifts, 4, hist, scan_ws, st, &first));
-        u32 *ks = first ? k32a : k32b, *vs = first ? va : vb;
-        KL; weld_flags_kernel<<<blocks_for(nc), FB, 0, st>>>(m->soup, ks, vs, nc, head, m->d_ctr);
-        KL; weld_fix_kernel<<<blocks_for(nc), FB, 0, st>>>(m->soup, ks, vs, nc, head, m->d_ctr);
-        HeadIn hin{head};
-        HeadOut hout{vs, m->cvid, vcorner};
-        CKS(launch_scan(hin, hout, (int64_t)nc, scan_ws, m->d_ctr + CTR_V, st));
-    }
+    CK(cudaMemsetAsync(wtab, 0xFF, sizeof(u32) * (size_t)capw, st));
+    CK(cudaMemsetAsync(etab, 0xFF, sizeof(u32) * (size_t)cape, st));
+    KL; ingest_weld_kernel<<<blocks_for(nc), FB, 0, st>>>(src, m->soup, nc, wtab, capw - 1, slot, m->d_flags);
+    KL; weld_head_kernel<<<blocks_for(nc), FB, 0, st>>>(wtab, slot, nc, head);
+    CKS(launch_scan(HeadIn{head}, HeadOut{wtab, slot, vcorner}, (int64_t)nc, scan_ws, m->d_ctr + CTR_V, st));
     stage_mark(m, SDF_T_INGEST_WELD, 1, st);
     // first host crossing: the vertex count sizes every per-vertex table
     CK(cudaMemcpyAsync(m->h_ctr, m->d_ctr, sizeof(u64) * CTR_COUNT, cudaMemcpyDeviceToHost, st));
@@ -429,35 +499,18 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     m->V = (int64_t)m->h_ctr[CTR_V];
     const int V = (int)m->V;
 
-    // ---- A3 (per triangle) + half-edge keys
+    // ---- A3 (per triangle), A2 edge table
     stage_mark(m, SDF_T_EDGES, 0, st);
-    u64 *vacc, *eka, *ekb;
+    u64 *vacc;
     CKS(tmp.get((void **)&vacc, sizeof(u64) * 3 * (size_t)V));
-    CKS(tmp.get((void **)&eka, sizeof(u64) * nc));
-    CKS(tmp.get((void **)&ekb, sizeof(u64) * nc));
     CK(cudaMemsetAsync(vacc, 0, sizeof(u64) * 3 * (size_t)V, st));
-    KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, m->cvid, (int)F, m->fn, vacc, eka, va, m->d_flags);
-
-    // ---- A2: edge table (radix sort of the (min,max) keys over their significant bits)
-    {
-        int bits = 1;
-        while (((int64_t)1 << bits) < (int64_t)V) bits++;          // vertex ids < V
-        int shifts[8], np = 0;
-        for (int b = 0; b < bits; b += 8) shifts[np++] = b;
-        for (int b = 0; b < bits; b += 8) shifts[np++] = 32 + b;
-        bool first;
-        CKS(radix_sort_pairs<u64>(eka, va, ekb, vb, nc, shifts, np, hist, scan_ws, st, &first));
-        u64 *ks = first ? eka : ekb;
-        u32 *vs = first ? va : vb;
-        if (nc & 1) {
-            int f = ERRB_NOTCLOSED;
-            CK(cudaMemcpyAsync(m->d_flags, &f, sizeof(int), cudaMemcpyHostToDevice, st));
-        }
-        m->E = nc / 2;
-        CKS(dev_alloc(al, (void **)&m->erec, sizeof(EdgeRec) * (size_t)(m->E > 0 ? m->E : 1), st));
-        KL; edge_pair_kernel<<<blocks_for(nc), FB, 0, st>>>(ks, vs, nc & ~1, m->soup, m->fn, m->cvid, m->adj, m->erec,
-                                                        m->d_flags, m->d_ctr);
-    }
+    KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wtab, slot, (int)F, m->cvid, m->fn, vacc, fcnt, m->d_flags);
+    CKS(launch_scan(FcntIn{fcnt}, EbaseOut{ebase}, F, scan_ws, (u64 *)nullptr, st));
+    m->E = nc / 2;
+    CKS(dev_alloc(al, (void **)&m->erec, sizeof(EdgeRec) * (size_t)(m->E > 0 ? m->E : 1), st));
+    KL; edge_insert_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, etab, cape - 1);
+    KL; edge_pair_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, etab, cape - 1, ebase, m->soup, m->fn, m->adj,
+                                                    m->erec, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_EDGES, 1, st);
 
@@ -483,6 +536,16 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     int hflags[4];
     CK(cudaMemcpyAsync(hflags, m->d_flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(m->h_ctr, m->d_ctr, sizeof(u64) * CTR_COUNT, cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));      // temporaries are released after this point
-    return status_from_flags(hflags[0]);
+    CK(cudaStreamSynchronize(st));
+    int status = status_from_flags(hflags[0]);
+    // closed + consistently oriented <=> every half-edge was claimed into a pair
+    const u64 pairs = m->h_ctr[CTR_E_CONVEX] + m->h_ctr[CTR_E_CONCAVE] + m->h_ctr[CTR_E_FLAT];
+    if (status == SDF_OK && 2 * pairs != (u64)nc) {
+        CKS(classify_edge_errors(m, nc, tmp, st));
+        CK(cudaMemcpyAsync(hflags, m->d_flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        status = status_from_flags(hflags[0]);
+        if (status == SDF_OK) status = SDF_ENOTCLOSED;
+    }
+    return status;      // temporaries are released here
 }
