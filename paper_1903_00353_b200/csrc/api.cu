@@ -91,7 +91,7 @@ void sdf_destroy(sdf_mesh *m) {
     if (m->side) { cudaStreamSynchronize(m->side); cudaStreamDestroy(m->side); }
     if (m->ev_fork) cudaEventDestroy(m->ev_fork);
     if (m->ev_join) cudaEventDestroy(m->ev_join);
-    void *ptrs[] = {m->soup, m->fn, m->cvid, m->adj, m->vmint, m->vrec, m->erec, m->d_ctr, m->d_flags, m->hdr,
+    void *ptrs[] = {m->soup, m->fn, m->cvid, m->adj, m->vmint, m->vrec, m->erec, m->d_ctr, m->d_flags,
                     m->scan_ws, m->brick_flag, m->brick_table, m->brick_list, m->big_list, m->scratch};
     for (size_t i = 0; i < sizeof(ptrs) / sizeof(ptrs[0]); i++) dev_free(&m->alloc, ptrs[i], st);
     for (int i = 0; i < SDF_T_COUNT; i++)
@@ -148,6 +148,12 @@ static int make_grid(const float origin[3], float h, int nx, int ny, int nz, flo
     g->rb = band + g->guard + g->eps;
     const char *dbg = getenv("SDF_AABB_MODE");
     g->aabb_mode = (dbg && dbg[0] == '1') ? 1 : 0;
+    const char *pf = getenv("SDF_FILL_MODE");
+    g->fill_mode = (pf && pf[0] >= '0' && pf[0] <= '4') ? pf[0] - '0' : 0;
+    const char *fd = getenv("SDF_FILL_DEPTH"), *fi = getenv("SDF_FILL_ISSUERS");
+    g->fill_depth = fd ? atoi(fd) : 8;
+    g->fill_issuers = fi ? atoi(fi) : 4;
+    if (g->fill_issuers < 1 || g->fill_issuers > 4) g->fill_issuers = 4;
     g->vec4 = (nx % 4 == 0) && (((uintptr_t)dist & 15) == 0) && (((uintptr_t)tri & 15) == 0);
     return SDF_OK;
 }

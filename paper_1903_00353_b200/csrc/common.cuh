@@ -95,6 +95,10 @@ struct GridParams {
     double dband;
     int aabb_mode;                  // debug: candidates = band-expanded triangle AABBs only
     int vec4;                       // 1: nx % 4 == 0 and outputs 16-B aligned -> 128-bit stores
+    int fill_mode;                  // 0: TMA fill on the side stream (default); debug: 1 plain stores on the
+                                    // side stream, 2 TMA fill on the main stream before the emit, 3 ... first,
+                                    // 4 forked after the mid-way host crossing
+    int fill_depth, fill_issuers;   // TMA fill: chunk pairs in flight per issuing lane, issuing lanes per SM
 };
 
 // ---------------------------------------------------------------------------------------
@@ -114,7 +118,6 @@ struct sdf_mesh {
     u64 *d_ctr;              // [CTR_COUNT]
     int *d_flags;            // [4]
     // persistent per-compute workspace (grown on demand)
-    PolyHdr *hdr;  size_t hdr_cap;         // [F + E + 2V]
     u64 *scan_ws;  size_t scan_ws_cap;
     unsigned char *brick_flag; size_t brick_flag_cap;
     int *brick_table; size_t brick_table_cap;

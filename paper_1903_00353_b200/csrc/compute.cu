@@ -99,17 +99,13 @@ __device__ __forceinline__ void cell_range(double mn, double mx, double o, doubl
     lo = (int)l; hi = (int)u;
 }
 
-__global__ void __launch_bounds__(256) clip_count_kernel(MeshView mv, GridParams g, PolyHdr *__restrict__ hdr,
-                                                         unsigned char *__restrict__ brick_flag,
-                                                         u32 *__restrict__ big_list, u64 *__restrict__ ctr) {
-    int64_t p = (int64_t)blockIdx.x * 256 + threadIdx.x;
-    const bool live = p < mv.P;
-    if (!live) p = 0;
+// A5: bounding volume of polyhedron p in cell indices, clipped to the grid.  Returns false if
+// the polyhedron is not emitted (flat edge, one-sided vertex, skipped cone) or misses the grid.
+__device__ __forceinline__ bool poly_aabv(const MeshView &mv, const GridParams &g, int64_t p, PolyHdr &h) {
     float mn[3], mx[3];
-    bool emit = live;
+    bool emit = true;
     const float rb = g.rb, eps = g.eps;
-    if (!live) {
-    } else if (p < mv.F) {
+    if (p < mv.F) {
         // face slab: triangle swept by +-rb along its normal
         const float *T = mv.soup + 9 * p, *N = mv.fn + 3 * p;
 #pragma unroll
@@ -164,33 +160,64 @@ __global__ void __launch_bounds__(256) clip_count_kernel(MeshView mv, GridParams
             }
         }
     }
-    PolyHdr h;
     h.i0 = h.j0 = h.k0 = 0; h.i1 = h.j1 = h.k1 = -1; h.rows = 0;
-    if (emit) {
-        int i0, i1, j0, j1, k0, k1;
-        double ih = 1.0 / g.dh;
-        cell_range(mn[0], mx[0], g.dox, ih, g.nx, i0, i1);
-        cell_range(mn[1], mx[1], g.doy, ih, g.ny, j0, j1);
-        cell_range(mn[2], mx[2], g.doz, ih, g.nz, k0, k1);
-        if (i0 <= i1 && j0 <= j1 && k0 <= k1) {
-            h.i0 = (short)i0; h.i1 = (short)i1; h.j0 = (short)j0; h.j1 = (short)j1; h.k0 = (short)k0; h.k1 = (short)k1;
-            h.rows = (u32)(j1 - j0 + 1) * (u32)(k1 - k0 + 1);
-            for (int bz = k0 >> 3; bz <= (k1 >> 3); bz++)
-                for (int by = j0 >> 3; by <= (j1 >> 3); by++)
-                    for (int bx = i0 >> 3; bx <= (i1 >> 3); bx++) {
-                        unsigned char *f = brick_flag + ((size_t)bz * g.nby + by) * g.nbx + bx;
-                        if (!*f) *f = 1;            // mostly already set: a cached read, not a write
-                    }
-            // big polyhedra (many rows or long rows) go to the block-per-polyhedron kernel
-            if (h.rows > BIG_ROWS || i1 - i0 >= BIG_NI) {
-                big_list[atomicAdd(&ctr[CTR_BIG], 1ull)] = (u32)p;
-                h.rows |= ROWS_BIG;
+    if (!emit) return false;
+    int i0, i1, j0, j1, k0, k1;
+    const double ih = 1.0 / g.dh;
+    cell_range(mn[0], mx[0], g.dox, ih, g.nx, i0, i1);
+    cell_range(mn[1], mx[1], g.doy, ih, g.ny, j0, j1);
+    cell_range(mn[2], mx[2], g.doz, ih, g.nz, k0, k1);
+    if (!(i0 <= i1 && j0 <= j1 && k0 <= k1)) return false;
+    h.i0 = (short)i0; h.i1 = (short)i1; h.j0 = (short)j0; h.j1 = (short)j1; h.k0 = (short)k0; h.k1 = (short)k1;
+    h.rows = (u32)(j1 - j0 + 1) * (u32)(k1 - k0 + 1);
+    return true;
+}
+
+// A6a: the 8x8x8-cell bricks that can receive a distance.  Every polyhedron of a triangle, of
+// its edges and of its vertices lies inside the triangle's slab box or inside the box of one
+// of its edges grown by the reach rb, so marking those four boxes per triangle (soup + normals
+// only) covers every cell the evaluation can touch.
+__device__ __forceinline__ void mark_box(const GridParams &g, const float *mn, const float *mx,
+                                         unsigned char *__restrict__ brick_flag) {
+    int i0, i1, j0, j1, k0, k1;
+    const double ih = 1.0 / g.dh;
+    cell_range(mn[0], mx[0], g.dox, ih, g.nx, i0, i1);
+    cell_range(mn[1], mx[1], g.doy, ih, g.ny, j0, j1);
+    cell_range(mn[2], mx[2], g.doz, ih, g.nz, k0, k1);
+    if (!(i0 <= i1 && j0 <= j1 && k0 <= k1)) return;
+    for (int bz = k0 >> 3; bz <= (k1 >> 3); bz++)
+        for (int by = j0 >> 3; by <= (j1 >> 3); by++)
+            for (int bx = i0 >> 3; bx <= (i1 >> 3); bx++) {
+                unsigned char *f = brick_flag + ((size_t)bz * g.nby + by) * g.nbx + bx;
+                if (!*f) *f = 1;            // mostly already set: a cached read, not a write
             }
-        }
+}
+
+__global__ void __launch_bounds__(256) brick_mark_kernel(MeshView mv, GridParams g,
+                                                         unsigned char *__restrict__ brick_flag) {
+    const int64_t t = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (t >= mv.F) return;
+    const float *T = mv.soup + 9 * t, *N = mv.fn + 3 * t;
+    const float rb = g.rb, eps = g.eps;
+    float mn[3], mx[3];
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+        float lo = fminf(T[i], fminf(T[3 + i], T[6 + i])), hi = fmaxf(T[i], fmaxf(T[3 + i], T[6 + i]));
+        float ext = g.aabb_mode ? rb : rb * fabsf(N[i]);
+        mn[i] = lo - ext - eps; mx[i] = hi + ext + eps;
     }
-    if (live) hdr[p] = h;
-    int c = __syncthreads_count(live && h.rows != 0);
-    if (threadIdx.x == 0 && c) atomicAdd(&ctr[CTR_SPREAD + (blockIdx.x & (CTR_SLOTS - 1)) * 8 + SP_POLY], (u64)c);
+    mark_box(g, mn, mx, brick_flag);
+    if (g.aabb_mode) return;
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const float *A = T + 3 * k, *B = T + 3 * (k == 2 ? 0 : k + 1);
+#pragma unroll
+        for (int i = 0; i < 3; i++) {
+            mn[i] = fminf(A[i], B[i]) - rb - eps;
+            mx[i] = fmaxf(A[i], B[i]) + rb + eps;
+        }
+        mark_box(g, mn, mx, brick_flag);
+    }
 }
 
 struct BrickIn {
@@ -216,7 +243,7 @@ struct BrickOut {
 // the lanes, and the warp then walks the flattened (polyhedron, row) list 32 rows at a time
 // -- the load balancing of PAPER.md:376-380 (dynamic parallelism) without child launches,
 // without a global work-item list and without a device-wide scan.  Polyhedra with many or
-// long rows are listed by clip_count_kernel and taken by evaluate_big_kernel, one block per
+// long rows are listed by evaluate_small_kernel and taken by evaluate_big_kernel, one block per
 // polyhedron with the lanes along x.
 // ---------------------------------------------------------------------------------------
 #define PR_GEO 20        // 13 geometry floats
@@ -308,6 +335,7 @@ __device__ __forceinline__ void build_record(const MeshView &mv, const GridParam
 __device__ __forceinline__ void put_min(const GridParams &g, const int *__restrict__ table, u64 *__restrict__ scratch,
                                         int i, int j, int k, float d, int id) {
     int slot = table[((size_t)(k >> 3) * g.nby + (j >> 3)) * g.nbx + (i >> 3)];
+    if (slot < 0) return;          // cannot happen: brick_mark_kernel covers every polyhedron
     u64 *cell = scratch + (size_t)slot * BRICK_CELLS + (((k & 7) * 8 + (j & 7)) * 8 + (i & 7));
     atomicMin(cell, ((u64)__float_as_uint(d) << 32) | (u32)id);
 }
@@ -419,7 +447,7 @@ __device__ __forceinline__ void add_stats(u64 *__restrict__ ctr, u32 tested, u32
 
 #define ES_WARPS 4
 __global__ void __launch_bounds__(32 * ES_WARPS) evaluate_small_kernel(MeshView mv, GridParams g,
-                                                                       const PolyHdr *__restrict__ hdr,
+                                                                       u32 *__restrict__ big_list,
                                                                        const int *__restrict__ table,
                                                                        u64 *__restrict__ scratch, u64 *__restrict__ ctr) {
     __shared__ float s_rec[ES_WARPS][32][PR_WORDS];
@@ -427,13 +455,23 @@ __global__ void __launch_bounds__(32 * ES_WARPS) evaluate_small_kernel(MeshView 
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int64_t p = ((int64_t)blockIdx.x * ES_WARPS + w) * 32 + lane;
     int rows = 0;
+    bool live = false;
     if (p < mv.P) {
-        const PolyHdr H = hdr[p];
-        if (H.rows != 0 && !(H.rows & ROWS_BIG)) {
-            rows = (int)H.rows;
-            build_record(mv, g, p, H, s_rec[w][lane]);
+        PolyHdr H;
+        live = poly_aabv(mv, g, p, H);
+        if (live) {
+            // big polyhedra (many rows or long rows) go to the block-per-polyhedron kernel
+            if (H.rows > BIG_ROWS || H.i1 - H.i0 >= BIG_NI) {
+                big_list[atomicAdd(&ctr[CTR_BIG], 1ull)] = (u32)p;
+            } else {
+                rows = (int)H.rows;
+                build_record(mv, g, p, H, s_rec[w][lane]);
+            }
         }
     }
+    const unsigned nlive = __popc(__ballot_sync(0xffffffffu, live));
+    if (lane == 0 && nlive)
+        atomicAdd(&ctr[CTR_SPREAD + ((blockIdx.x * ES_WARPS + w) & (CTR_SLOTS - 1)) * 8 + SP_POLY], (u64)nlive);
     int inc = rows;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -462,12 +500,12 @@ __global__ void __launch_bounds__(32 * ES_WARPS) evaluate_small_kernel(MeshView 
 // One block per big polyhedron (dynamic fetch): warps stride over its rows, lanes over x.
 #define EBIG_BT 256
 __global__ void __launch_bounds__(EBIG_BT) evaluate_big_kernel(MeshView mv, GridParams g,
-                                                               const PolyHdr *__restrict__ hdr,
                                                                const u32 *__restrict__ big_list,
                                                                const int *__restrict__ table,
                                                                u64 *__restrict__ scratch, u64 *__restrict__ ctr) {
     __shared__ float s_rec[PR_WORDS];
     __shared__ u64 s_e;
+    __shared__ u32 s_rows;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const u64 nbig = ctr[CTR_BIG];
     u32 tested = 0, accepted = 0, rows_done = 0;
@@ -477,11 +515,15 @@ __global__ void __launch_bounds__(EBIG_BT) evaluate_big_kernel(MeshView mv, Grid
         __syncthreads();
         const u64 e = s_e;
         if (e >= nbig) break;
-        const int64_t p = (int64_t)big_list[e];
-        const PolyHdr H = hdr[p];
-        if (threadIdx.x == 0) build_record(mv, g, p, H, s_rec);
+        if (threadIdx.x == 0) {
+            const int64_t p = (int64_t)big_list[e];
+            PolyHdr H;
+            poly_aabv(mv, g, p, H);
+            build_record(mv, g, p, H, s_rec);
+            s_rows = H.rows;
+        }
         __syncthreads();
-        const u32 rows = H.rows & ~ROWS_BIG;
+        const u32 rows = s_rows;
         for (u32 r = (u32)w; r < rows; r += EBIG_BT / 32)
             process_row<32>(g, s_rec, r, lane, table, scratch, tested, accepted);
         if (threadIdx.x == 0) rows_done += rows;
@@ -519,6 +561,47 @@ __global__ void __launch_bounds__(FILL_BT) fill_kernel(float *__restrict__ dist,
         for (int64_t i = (n4 << 2) + tid; i < n; i += nth) { dist[i] = INFINITY; tri[i] = -1; }
     } else {
         for (int64_t i = tid; i < n; i += nth) { dist[i] = INFINITY; tri[i] = -1; }
+    }
+}
+
+// TMA variant (the default): one CTA per SM keeps two 16 KiB sentinel tiles in shared memory and
+// one lane per warp streams them to HBM with bulk asynchronous copies (cp.async.bulk, SASS
+// UBLKCP), L2 evict-first.  It needs 4 warps and 32 KiB of shared memory per SM, so the kernels
+// of A5-A7 keep (almost) the whole SM while 8 B/cell stream out underneath them.
+#define FILL_TMA_BT 128
+#define FILL_TMA_CHUNK 16384
+template <int DEPTH>
+__global__ void __launch_bounds__(FILL_TMA_BT) fill_tma_kernel(float *__restrict__ dist, int *__restrict__ tri,
+                                                               int64_t n, int issuers) {
+    __shared__ __align__(128) u32 s_d[FILL_TMA_CHUNK / 4];
+    __shared__ __align__(128) u32 s_t[FILL_TMA_CHUNK / 4];
+    for (int i = threadIdx.x; i < FILL_TMA_CHUNK / 4; i += FILL_TMA_BT) { s_d[i] = 0x7F800000u; s_t[i] = 0xFFFFFFFFu; }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy writes -> async proxy reads
+    __syncthreads();
+    const int64_t per = FILL_TMA_CHUNK / 4;
+    const int64_t nchunks = n / per;
+    if ((threadIdx.x & 31) == 0 && (threadIdx.x >> 5) < issuers) {
+        u64 pol;
+        asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+        const u32 sd = (u32)__cvta_generic_to_shared(s_d), stt = (u32)__cvta_generic_to_shared(s_t);
+        const int64_t first = (int64_t)blockIdx.x * issuers + (threadIdx.x >> 5);
+        const int64_t stride = (int64_t)gridDim.x * issuers;
+        for (int64_t c = first; c < nchunks; c += stride) {
+            asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
+                         :: "l"(dist + c * per), "r"(sd), "r"(FILL_TMA_CHUNK), "l"(pol) : "memory");
+            asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
+                         :: "l"(tri + c * per), "r"(stt), "r"(FILL_TMA_CHUNK), "l"(pol) : "memory");
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            // at most DEPTH + 1 chunk pairs in flight per issuing lane: bounds the share of the
+            // memory queues the fill takes from the latency-bound kernels running beside it
+            asm volatile("cp.async.bulk.wait_group %0;" :: "n"(DEPTH) : "memory");
+        }
+        asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    }
+    // ragged tail (< one chunk) with plain stores
+    for (int64_t i = nchunks * per + (int64_t)blockIdx.x * FILL_TMA_BT + threadIdx.x; i < n;
+         i += (int64_t)gridDim.x * FILL_TMA_BT) {
+        dist[i] = INFINITY; tri[i] = -1;
     }
 }
 
@@ -667,7 +750,6 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
     mv.P = m->F + m->E + 2 * m->V;
     const int64_t P = mv.P;
     const int64_t nbricks = (int64_t)g.nbx * g.nby * g.nbz;
-    CKS(ensure(m, &m->hdr, &m->hdr_cap, (size_t)P, st));
     CKS(ensure(m, &m->big_list, &m->big_list_cap, (size_t)P, st));
     CKS(ensure(m, &m->scan_ws, &m->scan_ws_cap, scan_ws_elems(nbricks), st));
     CKS(ensure(m, &m->brick_flag, &m->brick_flag_cap, (size_t)nbricks, st));
@@ -680,28 +762,48 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     for (int i = SDF_T_CLIP_SCAN; i < SDF_T_COUNT; i++) m->ev_set[i] = false;
-    {
+    const int64_t N = (int64_t)g.nx * g.ny * g.nz;
+    const int vec = (((uintptr_t)dist & 15) == 0) && (((uintptr_t)tri & 15) == 0);
+    auto launch_fill = [&](cudaStream_t fs) -> int {
+        stage_mark(m, SDF_T_FILL, 0, fs);
+        if (vec && g.fill_mode != 1) {
+            const int iss = g.fill_issuers;
+            KL;
+            switch (g.fill_depth) {
+            case 0: fill_tma_kernel<0><<<(unsigned)sms, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss); break;
+            case 1: fill_tma_kernel<1><<<(unsigned)sms, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss); break;
+            case 2: fill_tma_kernel<2><<<(unsigned)sms, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss); break;
+            case 4: fill_tma_kernel<4><<<(unsigned)sms, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss); break;
+            default: fill_tma_kernel<8><<<(unsigned)sms, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss); break;
+            }
+        } else {
+            int64_t fb = (N / 4 + (int64_t)FILL_BT * FILL_UNROLL - 1) / ((int64_t)FILL_BT * FILL_UNROLL);
+            if (fb > (int64_t)sms * 2) fb = (int64_t)sms * 2;
+            if (fb < 1) fb = 1;
+            KL; fill_kernel<<<(unsigned)fb, FILL_BT, 0, fs>>>(dist, tri, N, vec);
+        }
+        stage_mark(m, SDF_T_FILL, 1, fs);
+        return SDF_OK;
+    };
+    const bool forked = g.fill_mode < 2 || g.fill_mode == 4;
+    auto fork_fill = [&]() -> int {
         if (!m->side) CK(cudaStreamCreateWithFlags(&m->side, cudaStreamNonBlocking));
         if (!m->ev_fork) CK(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
         if (!m->ev_join) CK(cudaEventCreateWithFlags(&m->ev_join, cudaEventDisableTiming));
         CK(cudaEventRecord(m->ev_fork, st));
         CK(cudaStreamWaitEvent(m->side, m->ev_fork, 0));
-        const int64_t N = (int64_t)g.nx * g.ny * g.nz;
-        int64_t fb = (N / 4 + (int64_t)FILL_BT * FILL_UNROLL - 1) / ((int64_t)FILL_BT * FILL_UNROLL);
-        if (fb > (int64_t)sms * 2) fb = (int64_t)sms * 2;
-        if (fb < 1) fb = 1;
-        const int vec = (((uintptr_t)dist & 15) == 0) && (((uintptr_t)tri & 15) == 0);
-        stage_mark(m, SDF_T_FILL, 0, m->side);
-        KL; fill_kernel<<<(unsigned)fb, FILL_BT, 0, m->side>>>(dist, tri, N, vec);
-        stage_mark(m, SDF_T_FILL, 1, m->side);
+        CKS(launch_fill(m->side));
         CK(cudaEventRecord(m->ev_join, m->side));
-    }
+        return SDF_OK;
+    };
+    if (g.fill_mode < 2) CKS(fork_fill());
+    else if (g.fill_mode == 3) CKS(launch_fill(st));
     CK(cudaMemsetAsync(m->brick_flag, 0, (size_t)nbricks, st));
     CK(cudaMemsetAsync(m->d_ctr + CTR_POLY, 0, sizeof(u64) * (CTR_TOTAL - CTR_POLY), st));
 
-    // A5 + A6: clip, count rows, mark bricks; prefix sums
+    // A6a: mark the bricks the band can reach; prefix sum -> brick table
     stage_mark(m, SDF_T_CLIP_SCAN, 0, st);
-    KL; clip_count_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(mv, g, m->hdr, m->brick_flag, m->big_list, m->d_ctr);
+    KL; brick_mark_kernel<<<(unsigned)((mv.F + 255) / 256), 256, 0, st>>>(mv, g, m->brick_flag);
     CKS(launch_scan(BrickIn{m->brick_flag}, BrickOut{m->brick_table, m->brick_list}, nbricks, m->scan_ws, m->d_ctr + CTR_BRICKS, st));
     CK(cudaGetLastError());
 
@@ -714,17 +816,20 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
     stage_mark(m, SDF_T_CLEAR, 0, st);
     if (bricks) CK(cudaMemsetAsync(m->scratch, 0xFF, (size_t)bricks * BRICK_CELLS * sizeof(u64), st));
     stage_mark(m, SDF_T_CLEAR, 1, st);
+    if (g.fill_mode == 4) CKS(fork_fill());
 
-    // A7: small polyhedra flattened per warp, big ones one block each (dynamic fetch)
+    // A5 + A6b + A7: clip every polyhedron, flatten the small ones per warp and evaluate them;
+    // big ones one block each (dynamic fetch)
     if (bricks) {
         stage_mark(m, SDF_T_EVALUATE, 0, st);
         const int64_t nblk = (P + 32 * ES_WARPS - 1) / (32 * ES_WARPS);
-        KL; evaluate_small_kernel<<<(unsigned)nblk, 32 * ES_WARPS, 0, st>>>(mv, g, m->hdr, m->brick_table, m->scratch, m->d_ctr);
-        KL; evaluate_big_kernel<<<(unsigned)(sms * 4), EBIG_BT, 0, st>>>(mv, g, m->hdr, m->big_list, m->brick_table, m->scratch, m->d_ctr);
+        KL; evaluate_small_kernel<<<(unsigned)nblk, 32 * ES_WARPS, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr);
+        KL; evaluate_big_kernel<<<(unsigned)(sms * 4), EBIG_BT, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr);
         stage_mark(m, SDF_T_EVALUATE, 1, st);
     }
     // A8b: join the fill, then overwrite the active bricks
-    CK(cudaStreamWaitEvent(st, m->ev_join, 0));
+    if (forked) CK(cudaStreamWaitEvent(st, m->ev_join, 0));
+    else if (g.fill_mode == 2) CKS(launch_fill(st));
     if (bricks) {
         stage_mark(m, SDF_T_EMIT, 0, st);
         KL; emit_bricks_kernel<<<(unsigned)bricks, EB_BT, 0, st>>>(mv, g, m->brick_list, m->scratch, dist, tri, m->d_ctr);

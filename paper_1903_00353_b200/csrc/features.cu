@@ -52,7 +52,7 @@ __global__ void __launch_bounds__(FB) ingest_weld_kernel(const float *__restrict
     const u32 bx = __float_as_uint(x), by = __float_as_uint(y), bz = __float_as_uint(z);
     u32 h = mix32(bx, by, bz) & mask;
     for (;;) {
-        u32 cur = *(volatile u32 *)(wtab + h);
+        u32 cur = __ldcg(wtab + h);
         if (cur == EMPTY32) {
             cur = atomicCAS(wtab + h, EMPTY32, (u32)c);
             if (cur == EMPTY32) break;
@@ -178,7 +178,7 @@ __global__ void __launch_bounds__(FB) edge_insert_kernel(const int *__restrict__
     if (!(u < w)) return;
     u32 h = edge_hash(u, w) & mask;
     for (;;) {
-        u32 cur = *(volatile u32 *)(etab + h);
+        u32 cur = __ldcg(etab + h);
         if (cur == EMPTY32) {
             cur = atomicCAS(etab + h, EMPTY32, (u32)he);
             if (cur == EMPTY32) return;
@@ -190,73 +190,76 @@ __global__ void __launch_bounds__(FB) edge_insert_kernel(const int *__restrict__
     }
 }
 
-// one thread per half-edge; backward ones claim their forward partner and write the edge
+// one thread per half-edge; backward ones claim their forward partner
 __global__ void __launch_bounds__(FB) edge_pair_kernel(const int *__restrict__ cvid, int n, u32 *etab, u32 mask,
-                                                       const u32 *__restrict__ ebase, const float *__restrict__ soup,
-                                                       const float *__restrict__ fn, int *__restrict__ adj,
-                                                       EdgeRec *__restrict__ erec, u64 *__restrict__ ctr) {
+                                                       int *__restrict__ adj) {
+    int he1 = blockIdx.x * FB + threadIdx.x;
+    if (he1 >= n) return;
+    const u32 w = (u32)cvid[he1], u = (u32)cvid[he_next(he1)];     // backward: w -> u with u < w
+    if (!(u < w)) return;
+    u32 h = edge_hash(u, w) & mask;
+    for (;;) {
+        u32 cur = __ldcg(etab + h);
+        if (cur == EMPTY32) return;                              // no forward partner
+        int cand = (int)(cur & ~HE_MATCHED);
+        if ((u32)cvid[cand] == u && (u32)cvid[he_next(cand)] == w) {
+            u32 prev = atomicOr(etab + h, HE_MATCHED);
+            if (!(prev & HE_MATCHED)) {                          // else: a second backward half-edge
+                adj[cand] = he1;
+                adj[he1] = cand;
+            }
+            return;
+        }
+        h = (h + 1) & mask;
+    }
+}
+
+// one thread per half-edge; the forward half-edge of every claimed pair writes the edge record
+// (A4 edge class + band-independent wedge geometry) at its rank among the forward half-edges
+__global__ void __launch_bounds__(FB) edge_record_kernel(const int *__restrict__ cvid, int n,
+                                                         const int *__restrict__ adj, const u32 *__restrict__ ebase,
+                                                         const float *__restrict__ soup, const float *__restrict__ fn,
+                                                         EdgeRec *__restrict__ erec, u64 *__restrict__ ctr) {
     __shared__ u32 s_cnt[3];
     if (threadIdx.x < 3) s_cnt[threadIdx.x] = 0;
     __syncthreads();
-    int he1 = blockIdx.x * FB + threadIdx.x;
-    if (he1 < n) {
-        const u32 w = (u32)cvid[he1], u = (u32)cvid[he_next(he1)];     // backward: w -> u with u < w
-        if (u < w) {
-            u32 h = edge_hash(u, w) & mask;
-            int he0 = -1;
-            for (;;) {
-                u32 cur = *(volatile u32 *)(etab + h);
-                if (cur == EMPTY32) break;                           // no forward partner
-                int cand = (int)(cur & ~HE_MATCHED);
-                if ((u32)cvid[cand] == u && (u32)cvid[he_next(cand)] == w) {
-                    u32 prev = atomicOr(etab + h, HE_MATCHED);
-                    if (!(prev & HE_MATCHED)) he0 = cand;            // else: a second backward half-edge
-                    break;
-                }
-                h = (h + 1) & mask;
+    int he0 = blockIdx.x * FB + threadIdx.x;
+    if (he0 < n) {
+        const int t0 = he0 / 3, k0 = he0 - 3 * t0;
+        const int c0 = cvid[3 * (size_t)t0], c1 = cvid[3 * (size_t)t0 + 1], c2 = cvid[3 * (size_t)t0 + 2];
+        const int u = k0 == 0 ? c0 : (k0 == 1 ? c1 : c2), w = k0 == 0 ? c1 : (k0 == 1 ? c2 : c0);
+        const int he1 = adj[he0];
+        if (u < w && he1 >= 0) {
+            const int t1 = he1 / 3;
+            const int e = (int)ebase[t0] + (k0 > 0 ? (c0 < c1) : 0) + (k0 > 1 ? (c1 < c2) : 0);
+            const float *A = soup + 9 * (size_t)t0 + 3 * k0, *B = soup + 9 * (size_t)t0 + 3 * (k0 == 2 ? 0 : k0 + 1);
+            const float *N1 = fn + 3 * (size_t)t0, *N2 = fn + 3 * (size_t)t1;
+            // canonical direction a -> b = ascending exact position bits, so the record (and the
+            // fp32 rounding of every distance evaluated from it) does not depend on the order of
+            // the triangles in the soup; n1 stays the normal of the triangle that traverses a -> b
+            const u32 *pa = (const u32 *)A, *pb = (const u32 *)B;
+            if (pa[0] != pb[0] ? pa[0] > pb[0] : (pa[1] != pb[1] ? pa[1] > pb[1] : pa[2] > pb[2])) {
+                const float *tp = A; A = B; B = tp;
+                tp = N1; N1 = N2; N2 = tp;
             }
-            if (he0 >= 0) {
-                adj[he0] = he1;
-                adj[he1] = he0;
-                int t0 = he0 / 3, k0 = he0 % 3, t1 = he1 / 3;
-                // edge id: rank of he0 among the forward half-edges in soup order
-                const int c0 = cvid[3 * (size_t)t0], c1 = cvid[3 * (size_t)t0 + 1], c2 = cvid[3 * (size_t)t0 + 2];
-                int e = (int)ebase[t0] + (k0 > 0 ? (c0 < c1) : 0) + (k0 > 1 ? (c1 < c2) : 0);
-                const int tmin = t0 < t1 ? t0 : t1;
-                const float *A = soup + 9 * (size_t)t0 + 3 * k0, *B = soup + 9 * (size_t)t0 + 3 * ((k0 + 1) % 3);
-                {
-                    // canonical direction a -> b = ascending exact position bits, so the record (and
-                    // the fp32 rounding of every distance evaluated from it) does not depend on the
-                    // order of the triangles in the soup; n1 stays the normal of the triangle that
-                    // traverses a -> b
-                    const u32 *pa = (const u32 *)A, *pb = (const u32 *)B;
-                    bool swap = pa[0] != pb[0] ? pa[0] > pb[0] : (pa[1] != pb[1] ? pa[1] > pb[1] : pa[2] > pb[2]);
-                    if (swap) {
-                        int k1 = he1 % 3;
-                        t0 = t1; t1 = he0 / 3; k0 = k1;
-                        A = soup + 9 * (size_t)t0 + 3 * k0; B = soup + 9 * (size_t)t0 + 3 * ((k0 + 1) % 3);
-                    }
-                }
-                const float *N1 = fn + 3 * (size_t)t0, *N2 = fn + 3 * (size_t)t1;
-                EdgeRec r;
-                double ud[3], n1[3], n2[3], x[3];
+            EdgeRec r;
+            double ud[3], n1[3], n2[3], x[3];
 #pragma unroll
-                for (int i = 0; i < 3; i++) {
-                    r.a[i] = A[i]; r.b[i] = B[i]; r.n1[i] = N1[i]; r.n2[i] = N2[i];
-                    ud[i] = (double)B[i] - (double)A[i]; n1[i] = N1[i]; n2[i] = N2[i];
-                }
-                double L = sqrt(ddot(ud, ud));
-                dcross(ud, n1, x);
-                double d = (L > 0.0) ? ddot(x, n2) / L : 0.0;       // PAPER.md:352 d = (ab x n1).n2, normalised
-                // flat: the wedge is thinner than 1e-6 * band and lies inside the eps-inflated
-                // neighbours (reading #5)
-                int cls = d > 1e-6 ? 1 : (d < -1e-6 ? -1 : 0);
-                r.tri = tmin;
-                r.cls = cls;
-                r.pad[0] = r.pad[1] = 0;
-                erec[e] = r;
-                atomicAdd(&s_cnt[cls > 0 ? 0 : (cls < 0 ? 1 : 2)], 1u);
+            for (int i = 0; i < 3; i++) {
+                r.a[i] = A[i]; r.b[i] = B[i]; r.n1[i] = N1[i]; r.n2[i] = N2[i];
+                ud[i] = (double)B[i] - (double)A[i]; n1[i] = N1[i]; n2[i] = N2[i];
             }
+            double L = sqrt(ddot(ud, ud));
+            dcross(ud, n1, x);
+            double d = (L > 0.0) ? ddot(x, n2) / L : 0.0;       // PAPER.md:352 d = (ab x n1).n2, normalised
+            // flat: the wedge is thinner than 1e-6 * band and lies inside the eps-inflated
+            // neighbours (reading #5)
+            int cls = d > 1e-6 ? 1 : (d < -1e-6 ? -1 : 0);
+            r.tri = t0 < t1 ? t0 : t1;
+            r.cls = cls;
+            r.pad[0] = r.pad[1] = 0;
+            erec[e] = r;
+            atomicAdd(&s_cnt[cls > 0 ? 0 : (cls < 0 ? 1 : 2)], 1u);
         }
     }
     __syncthreads();
@@ -509,8 +512,8 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     m->E = nc / 2;
     CKS(dev_alloc(al, (void **)&m->erec, sizeof(EdgeRec) * (size_t)(m->E > 0 ? m->E : 1), st));
     KL; edge_insert_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, etab, cape - 1);
-    KL; edge_pair_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, etab, cape - 1, ebase, m->soup, m->fn, m->adj,
-                                                    m->erec, m->d_ctr);
+    KL; edge_pair_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, etab, cape - 1, m->adj);
+    KL; edge_record_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, m->adj, ebase, m->soup, m->fn, m->erec, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_EDGES, 1, st);
 
