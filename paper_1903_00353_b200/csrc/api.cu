@@ -129,7 +129,7 @@ static int make_grid(const float origin[3], float h, int nx, int ny, int nz, flo
     if (nx <= 0 || ny <= 0 || nz <= 0 || nx > 32767 || ny > 32767 || nz > 32767) return SDF_EINVAL;
     if (!isfinite(origin[0]) || !isfinite(origin[1]) || !isfinite(origin[2])) return SDF_EINVAL;
     memset(g, 0, sizeof(*g));
-    g->ox = origin[0]; g->oy = origin[1]; g->oz = origin[2]; g->h = h;
+    g->ox = origin[0]; g->oy = origin[1]; g->oz = origin[2]; g->h = h; g->inv_h = 1.0f / h;
     g->dox = origin[0]; g->doy = origin[1]; g->doz = origin[2]; g->dh = h;
     g->nx = nx; g->ny = ny; g->nz = nz;
     g->nbx = (nx + BRICK - 1) / BRICK; g->nby = (ny + BRICK - 1) / BRICK; g->nbz = (nz + BRICK - 1) / BRICK;

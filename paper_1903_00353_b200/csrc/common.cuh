@@ -87,7 +87,7 @@ static_assert(sizeof(PolyHdr) == 16, "PolyHdr must be 16 B");
 #define PACK_EMPTY 0xFFFFFFFFFFFFFFFFull
 
 struct GridParams {
-    float ox, oy, oz, h;
+    float ox, oy, oz, h, inv_h;
     double dox, doy, doz, dh;       // same values promoted (fp64 re-check paths)
     int nx, ny, nz;
     int nbx, nby, nbz;              // bricks per axis

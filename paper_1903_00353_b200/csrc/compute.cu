@@ -27,6 +27,11 @@ template <typename T> __device__ __forceinline__ V3<T> cross(V3<T> a, V3<T> b) {
     return mk<T>(a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x);
 }
 __device__ __forceinline__ f3 ld3(const float *p) { return mk<float>(p[0], p[1], p[2]); }
+// dot product with a fixed association (no compiler contraction): the canonical form of every
+// distance that reaches the output, so a value does not depend on the kernel that produced it
+__device__ __forceinline__ float dot_rn(f3 a, f3 b) {
+    return __fmaf_rn(a.z, b.z, __fmaf_rn(a.y, b.y, __fmul_rn(a.x, b.x)));
+}
 __device__ __forceinline__ V3<double> ld3d(const float *p) { return mk<double>((double)p[0], (double)p[1], (double)p[2]); }
 
 enum { RG_FACE = 0, RG_E0 = 1, RG_E1 = 2, RG_E2 = 3, RG_V0 = 4, RG_V1 = 5, RG_V2 = 6 };
@@ -92,10 +97,14 @@ struct MeshView {
     int64_t P;
 };
 
-__device__ __forceinline__ void cell_range(double mn, double mx, double o, double inv_h, int n, int &lo, int &hi) {
-    double l = ceil((mn - o) * inv_h - 1e-4), u = floor((mx - o) * inv_h + 1e-4);
-    l = fmin(fmax(l, 0.0), (double)n);
-    u = fmax(fmin(u, (double)(n - 1)), -1.0);
+// Cell-index range of [mn, mx] along one axis, clipped to the grid.  fp32: the index estimate
+// (x - o) / h carries a rounding error below 32767 * 2^-22 < 8e-3 cells, covered by the slack
+// (a superset only costs candidate cells; every candidate gets the exact tests).
+#define CELL_SLACK 1e-2f
+__device__ __forceinline__ void cell_range(float mn, float mx, float o, float inv_h, int n, int &lo, int &hi) {
+    float l = ceilf((mn - o) * inv_h - CELL_SLACK), u = floorf((mx - o) * inv_h + CELL_SLACK);
+    l = fminf(fmaxf(l, 0.0f), (float)n);
+    u = fmaxf(fminf(u, (float)(n - 1)), -1.0f);
     lo = (int)l; hi = (int)u;
 }
 
@@ -163,10 +172,9 @@ __device__ __forceinline__ bool poly_aabv(const MeshView &mv, const GridParams &
     h.i0 = h.j0 = h.k0 = 0; h.i1 = h.j1 = h.k1 = -1; h.rows = 0;
     if (!emit) return false;
     int i0, i1, j0, j1, k0, k1;
-    const double ih = 1.0 / g.dh;
-    cell_range(mn[0], mx[0], g.dox, ih, g.nx, i0, i1);
-    cell_range(mn[1], mx[1], g.doy, ih, g.ny, j0, j1);
-    cell_range(mn[2], mx[2], g.doz, ih, g.nz, k0, k1);
+    cell_range(mn[0], mx[0], g.ox, g.inv_h, g.nx, i0, i1);
+    cell_range(mn[1], mx[1], g.oy, g.inv_h, g.ny, j0, j1);
+    cell_range(mn[2], mx[2], g.oz, g.inv_h, g.nz, k0, k1);
     if (!(i0 <= i1 && j0 <= j1 && k0 <= k1)) return false;
     h.i0 = (short)i0; h.i1 = (short)i1; h.j0 = (short)j0; h.j1 = (short)j1; h.k0 = (short)k0; h.k1 = (short)k1;
     h.rows = (u32)(j1 - j0 + 1) * (u32)(k1 - k0 + 1);
@@ -180,10 +188,9 @@ __device__ __forceinline__ bool poly_aabv(const MeshView &mv, const GridParams &
 __device__ __forceinline__ void mark_box(const GridParams &g, const float *mn, const float *mx,
                                          unsigned char *__restrict__ brick_flag) {
     int i0, i1, j0, j1, k0, k1;
-    const double ih = 1.0 / g.dh;
-    cell_range(mn[0], mx[0], g.dox, ih, g.nx, i0, i1);
-    cell_range(mn[1], mx[1], g.doy, ih, g.ny, j0, j1);
-    cell_range(mn[2], mx[2], g.doz, ih, g.nz, k0, k1);
+    cell_range(mn[0], mx[0], g.ox, g.inv_h, g.nx, i0, i1);
+    cell_range(mn[1], mx[1], g.oy, g.inv_h, g.ny, j0, j1);
+    cell_range(mn[2], mx[2], g.oz, g.inv_h, g.nz, k0, k1);
     if (!(i0 <= i1 && j0 <= j1 && k0 <= k1)) return;
     for (int bz = k0 >> 3; bz <= (k1 >> 3); bz++)
         for (int by = j0 >> 3; by <= (j1 >> 3); by++)
@@ -197,17 +204,29 @@ __global__ void __launch_bounds__(256) brick_mark_kernel(MeshView mv, GridParams
                                                          unsigned char *__restrict__ brick_flag) {
     const int64_t t = (int64_t)blockIdx.x * 256 + threadIdx.x;
     if (t >= mv.F) return;
-    const float *T = mv.soup + 9 * t, *N = mv.fn + 3 * t;
+    const float *T = mv.soup + 9 * t;
     const float rb = g.rb, eps = g.eps;
-    float mn[3], mx[3];
+    float lo[3], hi[3], mn[3], mx[3];
+    float ext_max = 0.0f;
 #pragma unroll
     for (int i = 0; i < 3; i++) {
-        float lo = fminf(T[i], fminf(T[3 + i], T[6 + i])), hi = fmaxf(T[i], fmaxf(T[3 + i], T[6 + i]));
-        float ext = g.aabb_mode ? rb : rb * fabsf(N[i]);
-        mn[i] = lo - ext - eps; mx[i] = hi + ext + eps;
+        lo[i] = fminf(T[i], fminf(T[3 + i], T[6 + i])); hi[i] = fmaxf(T[i], fmaxf(T[3 + i], T[6 + i]));
+        ext_max = fmaxf(ext_max, hi[i] - lo[i]);
+    }
+    if (g.aabb_mode || ext_max <= 4.0f * g.h) {
+        // small triangle: its box grown by the reach holds all four boxes and costs no extra brick
+#pragma unroll
+        for (int i = 0; i < 3; i++) { mn[i] = lo[i] - rb - eps; mx[i] = hi[i] + rb + eps; }
+        mark_box(g, mn, mx, brick_flag);
+        return;
+    }
+    const float *N = mv.fn + 3 * t;
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+        float ext = rb * fabsf(N[i]);
+        mn[i] = lo[i] - ext - eps; mx[i] = hi[i] + ext + eps;
     }
     mark_box(g, mn, mx, brick_flag);
-    if (g.aabb_mode) return;
 #pragma unroll
     for (int k = 0; k < 3; k++) {
         const float *A = T + 3 * k, *B = T + 3 * (k == 2 ? 0 : k + 1);
@@ -395,7 +414,7 @@ __device__ __forceinline__ void process_row(const GridParams &g, const float *re
             } else {
                 const float s0 = dot(m0, r), s1 = dot(m1, r - e0), s2 = dot(m2, r - ec);
                 if (s0 < -t0 || s1 < -t1 || s2 < -t2) continue;
-                if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f) d = fabsf(dot(n, r));
+                if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f) d = fabsf(dot_rn(n, r));
                 else { int rg; f3 q; d = tri_closest<float>(r, e0, ec, n, rg, q); }   // eps margin: exact clamped distance
             }
             if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id); }
@@ -409,9 +428,9 @@ __device__ __forceinline__ void process_row(const GridParams &g, const float *re
             tested++;
             const float t = dot(u, r);
             if (t < -eps || t > L + eps || dot(w1, r) < -eps || dot(w2, r) < -eps) continue;
-            const float tc = fminf(fmaxf(t, 0.0f), L);
-            const f3 q = r - tc * u;
-            const float d = sqrtf(dot(q, q));
+            const float tc = fminf(fmaxf(dot_rn(u, r), 0.0f), L);
+            const f3 q = mk<float>(__fmaf_rn(-tc, u.x, r.x), __fmaf_rn(-tc, u.y, r.y), __fmaf_rn(-tc, u.z, r.z));
+            const float d = __fsqrt_rn(dot_rn(q, q));
             if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id); }
         }
     } else {
@@ -421,7 +440,7 @@ __device__ __forceinline__ void process_row(const GridParams &g, const float *re
         for (int i = ia + lane0; i <= ib; i += STRIDE) {
             const f3 r = mk<float>(fmaf((float)i, h, g.ox) - v.x, ry, rz);
             tested++;
-            const float d = sqrtf(dot(r, r));
+            const float d = __fsqrt_rn(dot_rn(r, r));
             if (d >= reach || dot(A, r) < c * d - eps) continue;
             accepted++;
             put_min(g, table, scratch, i, j, k, d, id);
@@ -445,12 +464,171 @@ __device__ __forceinline__ void add_stats(u64 *__restrict__ ctr, u32 tested, u32
     }
 }
 
+// ---- small polyhedra: compact record + incremental scan conversion of a grid row.
+// Along a grid row every half-space test of PAPER.md:246-252 is linear in the cell index,
+// s(di) = base + di * g, so a row costs one set-up (the j,k terms) and one FMA + compare per
+// plane and cell; rows longer than ROW_CLIP_NI cells are first clipped analytically (a convex
+// body meets a line in one interval).  Cells that pass get the distance from the canonical
+// expressions (cell position by one fmaf, differences first, dot_rn), so a distance does not
+// depend on which path evaluated it.
+#define RR_ID 20
+#define RR_TYPE 21
+#define RR_I0 22
+#define RR_J0 23
+#define RR_K0 24
+#define RR_NI 25
+#define RR_NJ 26
+#define RR_INV_NJ 27     // float 1 / nj
+#define RR_WORDS 29      // odd stride: records of different owners fall in different banks
+#define ROW_CLIP_NI 8
+
+__device__ __forceinline__ void build_row_record(const MeshView &mv, const GridParams &g, int64_t p, const PolyHdr &H,
+                                                 float *rec) {
+    const float eps = g.eps;
+    int *ri = (int *)rec;
+    if (p < mv.F) {
+        // face slab: three inward side planes through the edges + the slab
+        const float *T = mv.soup + 9 * p, *N = mv.fn + 3 * p;
+        const f3 a = ld3(T), e0 = ld3(T + 3) - a, ec = ld3(T + 6) - a, n = ld3(N);
+        const f3 e1 = ec - e0;
+        const f3 m0 = cross(n, e0), m1 = cross(n, e1), m2 = cross(ec, n);          // inward, |m_i| = |edge_i|
+        rec[0] = a.x; rec[1] = a.y; rec[2] = a.z; rec[3] = n.x; rec[4] = n.y; rec[5] = n.z;
+        rec[6] = m0.x; rec[7] = m0.y; rec[8] = m0.z; rec[9] = m1.x; rec[10] = m1.y; rec[11] = m1.z;
+        rec[12] = m2.x; rec[13] = m2.y; rec[14] = m2.z;
+        rec[15] = dot(m1, e0); rec[16] = dot(m2, ec);
+        rec[17] = eps * sqrtf(dot(e0, e0)); rec[18] = eps * sqrtf(dot(e1, e1)); rec[19] = eps * sqrtf(dot(ec, ec));
+        ri[RR_ID] = (int)p; ri[RR_TYPE] = 0;
+    } else if (p < (int64_t)mv.F + mv.E) {
+        // edge wedge: beyond both faces' side planes, between the end caps
+        const EdgeRec &r = mv.erec[p - mv.F];
+        const f3 a = ld3(r.a), ab = ld3(r.b) - a, n1 = ld3(r.n1), n2 = ld3(r.n2);
+        const float L = sqrtf(dot(ab, ab));
+        const f3 u = (1.0f / L) * ab;
+        const f3 w1 = cross(u, n1), w2 = cross(n2, u);
+        rec[0] = a.x; rec[1] = a.y; rec[2] = a.z; rec[3] = u.x; rec[4] = u.y; rec[5] = u.z; rec[6] = L;
+        rec[7] = w1.x; rec[8] = w1.y; rec[9] = w1.z; rec[10] = w2.x; rec[11] = w2.y; rec[12] = w2.z;
+        ri[RR_ID] = r.tri; ri[RR_TYPE] = 1;
+    } else {
+        // vertex cone / hemisphere (eq.10, 362-364) inside the ball of radius reach
+        const int64_t q = p - mv.F - mv.E;
+        const VertexRec &r = mv.vrec[q >> 1];
+        const float sg = (q & 1) ? -1.0f : 1.0f;
+        rec[0] = r.pos[0]; rec[1] = r.pos[1]; rec[2] = r.pos[2];
+        rec[3] = sg * r.axis[0]; rec[4] = sg * r.axis[1]; rec[5] = sg * r.axis[2]; rec[6] = r.cos_cone;
+        ri[RR_ID] = mv.vmint[q >> 1]; ri[RR_TYPE] = 2;
+    }
+    const int nj = H.j1 - H.j0 + 1;
+    ri[RR_I0] = H.i0; ri[RR_J0] = H.j0; ri[RR_K0] = H.k0; ri[RR_NI] = H.i1 - H.i0 + 1; ri[RR_NJ] = nj;
+    rec[RR_INV_NJ] = 1.0f / (float)nj;
+}
+
+// clip the cell-index interval [lo, hi] of a row against base + di * g >= -tol
+__device__ __forceinline__ void clip_lin(float base, float gx, float tol, float &lo, float &hi) {
+    const float num = -tol - base;
+    if (gx > 0.0f) lo = fmaxf(lo, __fdividef(num, gx) - 1e-2f);
+    else if (gx < 0.0f) hi = fminf(hi, __fdividef(num, gx) + 1e-2f);
+    else if (num > 0.0f) hi = -1.0f;
+}
+
+__device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridParams &g, const float *rec, int row,
+                                                const int *__restrict__ table, u64 *__restrict__ scratch,
+                                                u32 &tested, u32 &accepted) {
+    const int *ri = (const int *)rec;
+    const int nj = ri[RR_NJ], ni = ri[RR_NI], i0 = ri[RR_I0], type = ri[RR_TYPE], id = ri[RR_ID];
+    const int dk = (int)(((float)row + 0.5f) * rec[RR_INV_NJ]);
+    const int j = ri[RR_J0] + row - dk * nj, k = ri[RR_K0] + dk;
+    const float h = g.h, eps = g.eps, reach = g.band + g.guard;      // accept d < reach; the emit pass decides exactly
+    const float ry = __fsub_rn(fmaf((float)j, h, g.oy), rec[1]), rz = __fsub_rn(fmaf((float)k, h, g.oz), rec[2]);
+    const float rx0 = fmaf((float)i0, h, g.ox) - rec[0];
+    int da = 0, db = ni - 1;
+    if (type == 0) {
+        const f3 n = ld3(rec + 3), m0 = ld3(rec + 6), m1 = ld3(rec + 9), m2 = ld3(rec + 12);
+        const float t0 = rec[17], t1 = rec[18], t2 = rec[19];
+        const float b0 = fmaf(m0.x, rx0, fmaf(m0.y, ry, m0.z * rz)), g0 = m0.x * h;
+        const float b1 = fmaf(m1.x, rx0, fmaf(m1.y, ry, m1.z * rz)) - rec[15], g1 = m1.x * h;
+        const float b2 = fmaf(m2.x, rx0, fmaf(m2.y, ry, m2.z * rz)) - rec[16], g2 = m2.x * h;
+        const float bn = fmaf(n.x, rx0, fmaf(n.y, ry, n.z * rz)), gn = n.x * h;
+        if (ni > ROW_CLIP_NI) {
+            float lo = 0.0f, hi = (float)db;
+            clip_lin(b0, g0, t0, lo, hi); clip_lin(b1, g1, t1, lo, hi); clip_lin(b2, g2, t2, lo, hi);
+            clip_lin(bn, gn, reach, lo, hi); clip_lin(-bn, -gn, reach, lo, hi);
+            if (!(lo <= hi)) return;
+            da = (int)ceilf(lo); db = (int)floorf(hi);
+        }
+        for (int di = da; di <= db; di++) {
+            const float fd = (float)di;
+            const float s0 = fmaf(fd, g0, b0), s1 = fmaf(fd, g1, b1), s2 = fmaf(fd, g2, b2), dn = fmaf(fd, gn, bn);
+            tested++;
+            if (s0 < -t0 || s1 < -t1 || s2 < -t2 || fabsf(dn) >= reach + eps) continue;
+            const int i = i0 + di;
+            const f3 r = mk<float>(__fsub_rn(fmaf((float)i, h, g.ox), rec[0]), ry, rz);
+            float d;
+            if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f) d = fabsf(dot_rn(n, r));
+            else {
+                // eps margin: exact clamped distance from the triangle itself
+                const float *T = mv.soup + 9 * (size_t)id;
+                const f3 a = ld3(T);
+                int rg; f3 qq;
+                d = tri_closest<float>(r, ld3(T + 3) - a, ld3(T + 6) - a, n, rg, qq);
+            }
+            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id); }
+        }
+    } else if (type == 1) {
+        const f3 u = ld3(rec + 3), w1 = ld3(rec + 7), w2 = ld3(rec + 10);
+        const float L = rec[6];
+        const float bt = fmaf(u.x, rx0, fmaf(u.y, ry, u.z * rz)), gt = u.x * h;
+        const float b1 = fmaf(w1.x, rx0, fmaf(w1.y, ry, w1.z * rz)), g1 = w1.x * h;
+        const float b2 = fmaf(w2.x, rx0, fmaf(w2.y, ry, w2.z * rz)), g2 = w2.x * h;
+        if (ni > ROW_CLIP_NI) {
+            float lo = 0.0f, hi = (float)db;
+            clip_lin(bt, gt, eps, lo, hi); clip_lin(L - bt, -gt, eps, lo, hi);
+            clip_lin(b1, g1, eps, lo, hi); clip_lin(b2, g2, eps, lo, hi);
+            if (!(lo <= hi)) return;
+            da = (int)ceilf(lo); db = (int)floorf(hi);
+        }
+        for (int di = da; di <= db; di++) {
+            const float fd = (float)di;
+            const float t = fmaf(fd, gt, bt);
+            tested++;
+            if (t < -eps || t > L + eps || fmaf(fd, g1, b1) < -eps || fmaf(fd, g2, b2) < -eps) continue;
+            const int i = i0 + di;
+            const f3 r = mk<float>(__fsub_rn(fmaf((float)i, h, g.ox), rec[0]), ry, rz);
+            const float tc = fminf(fmaxf(dot_rn(u, r), 0.0f), L);
+            const f3 q = mk<float>(__fmaf_rn(-tc, u.x, r.x), __fmaf_rn(-tc, u.y, r.y), __fmaf_rn(-tc, u.z, r.z));
+            const float d = __fsqrt_rn(dot_rn(q, q));
+            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id); }
+        }
+    } else {
+        const f3 A = ld3(rec + 3);
+        const float c = rec[6];
+        // ball of radius reach about the vertex: |rx| <= xr on this row
+        const float rem = reach * reach - ry * ry - rz * rz;
+        if (rem < 0.0f) return;
+        const float xr = sqrtf(rem);
+        float lo = fmaxf(0.0f, (-xr - rx0) * g.inv_h - 1e-2f), hi = fminf((float)db, (xr - rx0) * g.inv_h + 1e-2f);
+        // a cone of half angle <= 90 degrees lies in the half space A.r >= 0
+        const float ba = fmaf(A.x, rx0, fmaf(A.y, ry, A.z * rz)), ga = A.x * h;
+        if (c >= 0.0f) clip_lin(ba, ga, 2.0f * eps, lo, hi);
+        if (!(lo <= hi)) return;
+        da = (int)ceilf(lo); db = (int)floorf(hi);
+        for (int di = da; di <= db; di++) {
+            const int i = i0 + di;
+            const f3 r = mk<float>(__fsub_rn(fmaf((float)i, h, g.ox), rec[0]), ry, rz);
+            tested++;
+            const float d = __fsqrt_rn(dot_rn(r, r));
+            if (d >= reach || dot(A, r) < c * d - eps) continue;
+            accepted++;
+            put_min(g, table, scratch, i, j, k, d, id);
+        }
+    }
+}
+
 #define ES_WARPS 4
 __global__ void __launch_bounds__(32 * ES_WARPS) evaluate_small_kernel(MeshView mv, GridParams g,
                                                                        u32 *__restrict__ big_list,
                                                                        const int *__restrict__ table,
                                                                        u64 *__restrict__ scratch, u64 *__restrict__ ctr) {
-    __shared__ float s_rec[ES_WARPS][32][PR_WORDS];
+    __shared__ float s_rec[ES_WARPS][32][RR_WORDS];
     __shared__ int s_ex[ES_WARPS][33];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int64_t p = ((int64_t)blockIdx.x * ES_WARPS + w) * 32 + lane;
@@ -461,11 +639,11 @@ __global__ void __launch_bounds__(32 * ES_WARPS) evaluate_small_kernel(MeshView 
         live = poly_aabv(mv, g, p, H);
         if (live) {
             // big polyhedra (many rows or long rows) go to the block-per-polyhedron kernel
-            if (H.rows > BIG_ROWS || H.i1 - H.i0 >= BIG_NI) {
+            if (H.rows > BIG_ROWS || H.i1 - H.i0 >= BIG_NI || g.aabb_mode) {
                 big_list[atomicAdd(&ctr[CTR_BIG], 1ull)] = (u32)p;
             } else {
                 rows = (int)H.rows;
-                build_record(mv, g, p, H, s_rec[w][lane]);
+                build_row_record(mv, g, p, H, s_rec[w][lane]);
             }
         }
     }
@@ -491,7 +669,7 @@ __global__ void __launch_bounds__(32 * ES_WARPS) evaluate_small_kernel(MeshView 
 #pragma unroll
             for (int st = 16; st; st >>= 1)
                 if (s_ex[w][o + st] <= r) o += st;
-            process_row<1>(g, s_rec[w][o], (u32)(r - s_ex[w][o]), 0, table, scratch, tested, accepted);
+            process_row_inc(mv, g, s_rec[w][o], r - s_ex[w][o], table, scratch, tested, accepted);
         }
     }
     add_stats(ctr, tested, accepted, (u32)rows);
