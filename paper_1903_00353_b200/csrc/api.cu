@@ -149,7 +149,7 @@ static int make_grid(const float origin[3], float h, int nx, int ny, int nz, flo
     const char *dbg = getenv("SDF_AABB_MODE");
     g->aabb_mode = (dbg && dbg[0] == '1') ? 1 : 0;
     const char *pf = getenv("SDF_FILL_MODE");
-    g->fill_mode = (pf && pf[0] >= '0' && pf[0] <= '4') ? pf[0] - '0' : 0;
+    g->fill_mode = (pf && pf[0] >= '0' && pf[0] <= '4') ? pf[0] - '0' : 4;
     const char *fd = getenv("SDF_FILL_DEPTH"), *fi = getenv("SDF_FILL_ISSUERS");
     g->fill_depth = fd ? atoi(fd) : 8;
     g->fill_issuers = fi ? atoi(fi) : 4;

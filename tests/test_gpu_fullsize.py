@@ -1,0 +1,72 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times
+(device-resident soup, sdf_create + sdf_compute through the C ABI).
+
+C2 and C3 are compared with the oracle element by element over the whole grid.  C4 (1024^3) and
+C5 (2048x1024x1024, 2^31 cells: every linear index path is 64-bit) are compared element by
+element on z-slabs the oracle computes as crops of the same grid (first, middle, last slices:
+the slabs cross brick, tile and grid boundaries), and over the whole grid through properties
+that hold at any size: |d| < band on populated cells, sentinels elsewhere, ids in range, the
+populated count equals the library's own counter.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_1903_00353_b200 import workloads as W
+from gpu_util import f32_grid
+from helpers import compare_to_oracle
+
+pytestmark = pytest.mark.gpu
+
+KEYS = ("bad_sentinel", "bad_id_range", "bad_set", "bad_dist", "bad_sign", "bad_id")
+
+
+def _gpu(w):
+    from paper_1903_00353_b200 import binding as B
+    m, d, t = B.compute_workload(w)
+    torch.cuda.synchronize()
+    return m, d, t, B.sdf_stats(m)
+
+
+def _whole_grid_properties(w, d, t, stats):
+    pop = torch.isfinite(d)
+    n_pop = int(pop.sum().item())
+    assert n_pop == stats["band_cells"] and n_pop > 0
+    assert bool((torch.isposinf(d) | (torch.abs(d) < float(np.float32(w.band)))).all())
+    assert bool(((t >= 0) == pop).all())
+    assert int(t.max().item()) < w.ntri and int(t.min().item()) >= -1
+    return n_pop
+
+
+@pytest.mark.parametrize("name", ["C2", "C3"])
+def test_full_grid(oracle_mod, name):
+    w = f32_grid(W.config(name))
+    om = oracle_mod.Mesh(w.soup)
+    d_ref, t_ref = om.sdf(w.origin, w.h, w.dims, w.band)
+    m, d, t, stats = _gpu(w)
+    _whole_grid_properties(w, d, t, stats)
+    res = compare_to_oracle(d.cpu().numpy(), t.cpu().numpy(), d_ref, t_ref, w, om)
+    assert res["ok"] and all(res[k] == 0 for k in KEYS), {k: v for k, v in res.items()}
+    assert (stats["V"], stats["E"]) == (w.meta["V"], w.meta["E"])
+
+
+@pytest.mark.parametrize("name,slabs", [
+    ("C4", [(150, 24), (500, 24), (856, 24)]),
+    ("C5", [(40, 16), (505, 16), (1000, 16)]),
+])
+def test_full_size_slabs(oracle_mod, name, slabs):
+    w = f32_grid(W.config(name))
+    nx, ny, nz = w.dims
+    m, d, t, stats = _gpu(w)
+    assert d.shape == (nz, ny, nx)
+    _whole_grid_properties(w, d, t, stats)
+    assert (stats["F"], stats["V"], stats["E"]) == (w.ntri, w.meta["V"], w.meta["E"])
+    om = oracle_mod.Mesh(w.soup)
+    checked = 0
+    for k0, nk in slabs:
+        c = w.crop((0, 0, k0), (nx, ny, nk))
+        d_ref, t_ref = om.sdf(c.origin, c.h, c.dims, c.band)
+        res = compare_to_oracle(d[k0:k0 + nk].cpu().numpy(), t[k0:k0 + nk].cpu().numpy(), d_ref, t_ref, c, om)
+        assert res["ok"] and all(res[k] == 0 for k in KEYS), (k0, {k: v for k, v in res.items()})
+        checked += res["populated_ref"]
+    assert checked > 0
