@@ -91,8 +91,7 @@ void sdf_destroy(sdf_mesh *m) {
     if (m->side) { cudaStreamSynchronize(m->side); cudaStreamDestroy(m->side); }
     if (m->ev_fork) cudaEventDestroy(m->ev_fork);
     if (m->ev_join) cudaEventDestroy(m->ev_join);
-    void *ptrs[] = {m->soup, m->fn, m->cvid, m->adj, m->vmint, m->vrec, m->erec, m->d_ctr, m->d_flags,
-                    m->scan_ws, m->brick_flag, m->brick_table, m->brick_list, m->big_list, m->scratch};
+    void *ptrs[] = {m->slab_f, m->slab_v, m->slab_ws, m->scratch};
     for (size_t i = 0; i < sizeof(ptrs) / sizeof(ptrs[0]); i++) dev_free(&m->alloc, ptrs[i], st);
     for (int i = 0; i < SDF_T_COUNT; i++)
         for (int w = 0; w < 2; w++)

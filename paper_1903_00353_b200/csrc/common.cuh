@@ -107,7 +107,12 @@ struct GridParams {
 struct sdf_mesh {
     sdf_allocator alloc;     // copied; alloc.alloc == nullptr -> cudaMallocAsync
     int64_t F, E, V;
-    // feature tables (device)
+    // device memory comes in a few slabs carved into tables (one allocator call each: the
+    // caller's allocator may be a slow host callback)
+    void *slab_f;            // F-sized feature tables + counters
+    void *slab_v;            // V-sized feature tables
+    void *slab_ws; size_t slab_ws_cap;     // per-compute workspace (bytes), grown on demand
+    // feature tables (device, views into the slabs)
     float *soup;             // [F][9] canonicalised copy of the input
     float *fn;               // [F][3] unit face normals
     int *cvid;               // [3F]
@@ -118,11 +123,11 @@ struct sdf_mesh {
     u64 *d_ctr;              // [CTR_COUNT]
     int *d_flags;            // [4]
     // persistent per-compute workspace (grown on demand)
-    u64 *scan_ws;  size_t scan_ws_cap;
-    unsigned char *brick_flag; size_t brick_flag_cap;
-    int *brick_table; size_t brick_table_cap;
-    int *brick_list; size_t brick_list_cap;   // scratch slot -> brick index
-    u32 *big_list; size_t big_list_cap;       // polyhedra of evaluate_big_kernel
+    u64 *scan_ws;
+    unsigned char *brick_flag;
+    int *brick_table;
+    int *brick_list;                       // scratch slot -> brick index
+    u32 *big_list;                         // polyhedra of evaluate_big_kernel
     u64 *scratch;  size_t scratch_cap;     // bricks * 512 packed values
     u64 h_ctr[CTR_COUNT];
     cudaEvent_t ev[SDF_T_COUNT][2];   // stage begin / end events (created on first use)
@@ -131,6 +136,18 @@ struct sdf_mesh {
     cudaStream_t last_stream;
     cudaStream_t side;                // library-owned stream of the sentinel fill (A8a)
     cudaEvent_t ev_fork, ev_join;
+};
+
+// carve 256-byte aligned tables out of one slab; with base == nullptr it only adds up sizes
+struct Carver {
+    char *base; size_t off;
+    explicit Carver(void *b) : base((char *)b), off(0) {}
+    template <typename T> T *take(size_t n) {
+        off = (off + 255) & ~(size_t)255;
+        T *p = base ? (T *)(base + off) : nullptr;
+        off += n * sizeof(T);
+        return p;
+    }
 };
 
 // allocation through the handle's allocator

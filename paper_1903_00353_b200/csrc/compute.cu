@@ -928,11 +928,21 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
     mv.P = m->F + m->E + 2 * m->V;
     const int64_t P = mv.P;
     const int64_t nbricks = (int64_t)g.nbx * g.nby * g.nbz;
-    CKS(ensure(m, &m->big_list, &m->big_list_cap, (size_t)P, st));
-    CKS(ensure(m, &m->scan_ws, &m->scan_ws_cap, scan_ws_elems(nbricks), st));
-    CKS(ensure(m, &m->brick_flag, &m->brick_flag_cap, (size_t)nbricks, st));
-    CKS(ensure(m, &m->brick_table, &m->brick_table_cap, (size_t)nbricks, st));
-    CKS(ensure(m, &m->brick_list, &m->brick_list_cap, (size_t)nbricks, st));
+    // per-compute workspace: one slab, grown on demand
+    for (int pass = 0; pass < 2; pass++) {
+        Carver c(pass ? m->slab_ws : nullptr);
+        m->brick_flag = c.take<unsigned char>((size_t)nbricks);
+        m->brick_table = c.take<int>((size_t)nbricks);
+        m->brick_list = c.take<int>((size_t)nbricks);
+        m->scan_ws = c.take<u64>(scan_ws_elems(nbricks));
+        m->big_list = c.take<u32>((size_t)P);
+        if (pass == 0 && (c.off > m->slab_ws_cap || !m->slab_ws)) {
+            if (m->slab_ws) { dev_free(&m->alloc, m->slab_ws, st); m->slab_ws = nullptr; m->slab_ws_cap = 0; }
+            const size_t want = c.off + c.off / 8 + 256;
+            CKS(dev_alloc(&m->alloc, &m->slab_ws, want, st));
+            m->slab_ws_cap = want;
+        }
+    }
 
     // A8a: the sentinel fill depends on nothing: fork it onto the side stream so that it
     // streams to HBM underneath A5-A7 (which are latency / atomic bound)

@@ -389,15 +389,6 @@ __global__ void __launch_bounds__(FB) vertex_record_kernel(const float *__restri
     if (threadIdx.x < 5 && s_cnt[threadIdx.x]) atomicAdd(&ctr[CTR_V_POS + threadIdx.x], (u64)s_cnt[threadIdx.x]);
 }
 
-__global__ void fill_i32_kernel(int *p, int64_t n, int v) {
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) p[i] = v;
-}
-__global__ void fill_i64_kernel(long long *p, int64_t n, long long v) {
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) p[i] = v;
-}
-
 // ---------------------------------------------------------------------------------------
 // host driver
 // ---------------------------------------------------------------------------------------
@@ -456,42 +447,53 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     const int nc = (int)(3 * F);
     const sdf_allocator *al = &m->alloc;
     TmpPool tmp(al, st);
+    m->E = nc / 2;
 
-    CKS(dev_alloc(al, (void **)&m->soup, sizeof(float) * 9 * F, st));
-    CKS(dev_alloc(al, (void **)&m->fn, sizeof(float) * 3 * F, st));
-    CKS(dev_alloc(al, (void **)&m->cvid, sizeof(int) * 3 * F, st));
-    CKS(dev_alloc(al, (void **)&m->adj, sizeof(int) * 3 * F, st));
-    CKS(dev_alloc(al, (void **)&m->d_ctr, sizeof(u64) * CTR_TOTAL, st));
-    CKS(dev_alloc(al, (void **)&m->d_flags, sizeof(int) * 4, st));
+    // persistent F-sized tables: one slab
+    for (int pass = 0; pass < 2; pass++) {
+        Carver c(m->slab_f);
+        m->soup = c.take<float>(9 * (size_t)F);
+        m->fn = c.take<float>(3 * (size_t)F);
+        m->cvid = c.take<int>(3 * (size_t)F);
+        m->adj = c.take<int>(3 * (size_t)F);
+        m->erec = c.take<EdgeRec>((size_t)(m->E > 0 ? m->E : 1));
+        m->d_ctr = c.take<u64>(CTR_TOTAL);
+        m->d_flags = c.take<int>(4);
+        if (pass == 0) CKS(dev_alloc(al, &m->slab_f, c.off, st));
+    }
     CK(cudaMemsetAsync(m->d_ctr, 0, sizeof(u64) * CTR_TOTAL, st));
     CK(cudaMemsetAsync(m->d_flags, 0, sizeof(int) * 4, st));
     CK(cudaMemsetAsync(m->adj, 0xFF, sizeof(int) * 3 * F, st));
 
     // ---- A0 ingest + A1 weld (hash table on the exact coordinate bits)
     stage_mark(m, SDF_T_INGEST_WELD, 0, st);
-    const float *src = tri;
+    const u32 capw = pow2_at_least((u64)nc + (u64)nc / 4 + 1);     // load <= 0.8 even if no vertex is shared
+    const u32 cape = pow2_at_least((u64)nc + 1);                   // <= 3F/2 forward half-edges: load <= 0.5
     float *staging = nullptr;
+    u32 *wtab = nullptr, *slot = nullptr, *etab = nullptr, *ebase = nullptr;
+    u64 *scan_ws = nullptr;
+    unsigned char *head = nullptr, *fcnt = nullptr;
+    int *vcorner = nullptr;
+    void *tslab = nullptr;
+    for (int pass = 0; pass < 2; pass++) {
+        Carver c(tslab);
+        wtab = c.take<u32>((size_t)capw);           // wtab and etab adjacent: one memset
+        etab = c.take<u32>((size_t)cape);
+        slot = c.take<u32>((size_t)nc);
+        ebase = c.take<u32>((size_t)F);
+        scan_ws = c.take<u64>(scan_ws_elems((int64_t)nc));
+        head = c.take<unsigned char>((size_t)nc);
+        fcnt = c.take<unsigned char>((size_t)F);
+        vcorner = c.take<int>((size_t)nc);          // V <= 3F
+        if (!on_device) staging = c.take<float>(9 * (size_t)F);
+        if (pass == 0) CKS(tmp.get(&tslab, c.off));
+    }
+    const float *src = tri;
     if (!on_device) {
-        CKS(tmp.get((void **)&staging, sizeof(float) * 9 * F));
         CK(cudaMemcpyAsync(staging, tri, sizeof(float) * 9 * F, cudaMemcpyHostToDevice, st));
         src = staging;
     }
-    const u32 capw = pow2_at_least((u64)nc + (u64)nc / 4 + 1);     // load <= 0.8 even if no vertex is shared
-    const u32 cape = pow2_at_least((u64)nc + 1);                   // <= 3F/2 forward half-edges: load <= 0.5
-    u32 *wtab, *slot, *etab, *ebase;
-    u64 *scan_ws;
-    unsigned char *head, *fcnt;
-    int *vcorner;
-    CKS(tmp.get((void **)&wtab, sizeof(u32) * (size_t)capw));
-    CKS(tmp.get((void **)&slot, sizeof(u32) * nc));
-    CKS(tmp.get((void **)&etab, sizeof(u32) * (size_t)cape));
-    CKS(tmp.get((void **)&ebase, sizeof(u32) * (size_t)F));
-    CKS(tmp.get((void **)&scan_ws, sizeof(u64) * scan_ws_elems((int64_t)nc)));
-    CKS(tmp.get((void **)&head, (size_t)nc));
-    CKS(tmp.get((void **)&fcnt, (size_t)F));
-    CKS(tmp.get((void **)&vcorner, sizeof(int) * nc));      // V <= 3F
-    CK(cudaMemsetAsync(wtab, 0xFF, sizeof(u32) * (size_t)capw, st));
-    CK(cudaMemsetAsync(etab, 0xFF, sizeof(u32) * (size_t)cape, st));
+    CK(cudaMemsetAsync(wtab, 0xFF, (size_t)((char *)(etab + cape) - (char *)wtab), st));
     KL; ingest_weld_kernel<<<blocks_for(nc), FB, 0, st>>>(src, m->soup, nc, wtab, capw - 1, slot, m->d_flags);
     KL; weld_head_kernel<<<blocks_for(nc), FB, 0, st>>>(wtab, slot, nc, head);
     CKS(launch_scan(HeadIn{head}, HeadOut{wtab, slot, vcorner}, (int64_t)nc, scan_ws, m->d_ctr + CTR_V, st));
@@ -502,15 +504,32 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     m->V = (int64_t)m->h_ctr[CTR_V];
     const int V = (int)m->V;
 
+    // V-sized tables: one persistent slab, one temporary slab
+    for (int pass = 0; pass < 2; pass++) {
+        Carver c(m->slab_v);
+        m->vrec = c.take<VertexRec>((size_t)V);
+        m->vmint = c.take<int>((size_t)V);
+        if (pass == 0) CKS(dev_alloc(al, &m->slab_v, c.off, st));
+    }
+    u64 *vacc = nullptr;
+    double *vn64 = nullptr;
+    long long *vcosq = nullptr;
+    int *vside = nullptr;
+    void *vslab = nullptr;
+    for (int pass = 0; pass < 2; pass++) {
+        Carver c(vslab);
+        vacc = c.take<u64>(3 * (size_t)V);          // vacc and vside adjacent: one memset to 0
+        vside = c.take<int>((size_t)V);
+        vcosq = c.take<long long>((size_t)V);
+        vn64 = c.take<double>(3 * (size_t)V);
+        if (pass == 0) CKS(tmp.get(&vslab, c.off));
+    }
+
     // ---- A3 (per triangle), A2 edge table
     stage_mark(m, SDF_T_EDGES, 0, st);
-    u64 *vacc;
-    CKS(tmp.get((void **)&vacc, sizeof(u64) * 3 * (size_t)V));
-    CK(cudaMemsetAsync(vacc, 0, sizeof(u64) * 3 * (size_t)V, st));
+    CK(cudaMemsetAsync(vacc, 0, (size_t)((char *)(vside + V) - (char *)vacc), st));
     KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wtab, slot, (int)F, m->cvid, m->fn, vacc, fcnt, m->d_flags);
     CKS(launch_scan(FcntIn{fcnt}, EbaseOut{ebase}, F, scan_ws, (u64 *)nullptr, st));
-    m->E = nc / 2;
-    CKS(dev_alloc(al, (void **)&m->erec, sizeof(EdgeRec) * (size_t)(m->E > 0 ? m->E : 1), st));
     KL; edge_insert_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, etab, cape - 1);
     KL; edge_pair_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, etab, cape - 1, m->adj);
     KL; edge_record_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, m->adj, ebase, m->soup, m->fn, m->erec, m->d_ctr);
@@ -519,18 +538,10 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
 
     // ---- A3/A4 vertices (garbage-in on invalid input is harmless: ids stay in range)
     stage_mark(m, SDF_T_VERTICES, 0, st);
-    double *vn64;
-    long long *vcosq;
-    int *vside;
-    CKS(tmp.get((void **)&vn64, sizeof(double) * 3 * (size_t)V));
-    CKS(tmp.get((void **)&vcosq, sizeof(long long) * (size_t)V));
-    CKS(tmp.get((void **)&vside, sizeof(int) * (size_t)V));
-    CKS(dev_alloc(al, (void **)&m->vmint, sizeof(int) * (size_t)V, st));
-    CKS(dev_alloc(al, (void **)&m->vrec, sizeof(VertexRec) * (size_t)V, st));
+    // "larger than any value" initial states: 0x7F7F.. for the cone cosines and triangle ids
+    CK(cudaMemsetAsync(vcosq, 0x7F, sizeof(long long) * (size_t)V, st));
+    CK(cudaMemsetAsync(m->vmint, 0x7F, sizeof(int) * (size_t)V, st));
     KL; vertex_normal_kernel<<<blocks_for(V), FB, 0, st>>>(vacc, V, vn64);
-    KL; fill_i64_kernel<<<blocks_for(V), FB, 0, st>>>(vcosq, V, 0x7FFFFFFFFFFFFFFFll);
-    KL; fill_i32_kernel<<<blocks_for(V), FB, 0, st>>>(m->vmint, V, 0x7FFFFFFF);
-    CK(cudaMemsetAsync(vside, 0, sizeof(int) * (size_t)V, st));
     KL; vertex_cone_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, m->cvid, (int)F, vn64, vcosq, vside, m->vmint);
     KL; vertex_record_kernel<<<blocks_for(V), FB, 0, st>>>(m->soup, vcorner, vn64, vcosq, vside, V, m->vrec, m->d_ctr);
     CK(cudaGetLastError());
