@@ -235,7 +235,27 @@ int sdf_get_table(sdf_mesh *m, int which, void *dst, size_t bytes) {
     }
     if (bytes != need || !src) return SDF_EINVAL;
     CK(cudaStreamSynchronize(m->last_stream));
-    CK(cudaMemcpy(dst, src, need, cudaMemcpyDeviceToHost));
+    if (which > SDF_TABLE_FACE_NORMAL) {
+        CK(cudaMemcpy(dst, src, need, cudaMemcpyDeviceToHost));
+        return SDF_OK;
+    }
+    // per-triangle tables are stored in the internal (spatially binned) order: hand them out in
+    // the caller's soup order, half-edge indices included
+    const size_t F = (size_t)m->F;
+    int *perm = (int *)malloc(sizeof(int) * F);
+    int *tmp = (int *)malloc(need);
+    if (!perm || !tmp) { free(perm); free(tmp); return SDF_ENOMEM; }
+    cudaError_t e = cudaMemcpy(perm, m->perm, sizeof(int) * F, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(tmp, src, need, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) { free(perm); free(tmp); g_last_cuda_error = (int)e; (void)cudaGetLastError(); return SDF_ECUDA; }
+    int *out = (int *)dst;          // all three tables hold 3 four-byte words per triangle
+    for (size_t i = 0; i < F; i++)
+        for (int k = 0; k < 3; k++) {
+            int v = tmp[3 * i + k];
+            if (which == SDF_TABLE_HALFEDGE_ADJ && v >= 0) v = 3 * perm[v / 3] + v % 3;
+            out[3 * (size_t)perm[i] + k] = v;
+        }
+    free(perm); free(tmp);
     return SDF_OK;
 }
 

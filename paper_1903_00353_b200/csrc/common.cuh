@@ -115,6 +115,8 @@ struct sdf_mesh {
     // feature tables (device, views into the slabs)
     float *soup;             // [F][9] canonicalised copy of the input
     float *fn;               // [F][3] unit face normals
+    int *perm;               // [F] internal triangle index -> the caller's id (spatial binning)
+    int *inv_perm;           // [F] the caller's id -> internal index
     int *cvid;               // [3F]
     int *adj;                // [3F]
     int *vmint;              // [V]

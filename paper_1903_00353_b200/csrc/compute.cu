@@ -93,6 +93,7 @@ struct MeshView {
     const EdgeRec *erec;
     const VertexRec *vrec;
     const int *vmint, *cvid, *adj;
+    const int *perm, *inv_perm;     // internal triangle index <-> the caller's id
     int F, E, V;
     int64_t P;
 };
@@ -313,7 +314,7 @@ __device__ __forceinline__ void build_record(const MeshView &mv, const GridParam
         }
         G[0] = a.x; G[1] = a.y; G[2] = a.z; G[3] = e0.x; G[4] = e0.y; G[5] = e0.z;
         G[6] = ec.x; G[7] = ec.y; G[8] = ec.z; G[9] = n.x; G[10] = n.y; G[11] = n.z; G[12] = 0.0f;
-        ri[PR_ID] = (int)p; ri[PR_TYPE] = 0;
+        ri[PR_ID] = mv.perm[p]; ri[PR_TYPE] = 0;
     } else if (p < (int64_t)mv.F + mv.E) {
         // edge wedge: beyond both faces' side planes, between the end caps
         const EdgeRec &r = mv.erec[p - mv.F];
@@ -479,6 +480,7 @@ __device__ __forceinline__ void add_stats(u64 *__restrict__ ctr, u32 tested, u32
 #define RR_NI 25
 #define RR_NJ 26
 #define RR_INV_NJ 27     // float 1 / nj
+#define RR_TIDX 28       // faces: internal triangle index (the eps-margin path re-reads the corners)
 #define RR_WORDS 29      // odd stride: records of different owners fall in different banks
 #define ROW_CLIP_NI 8
 
@@ -497,7 +499,7 @@ __device__ __forceinline__ void build_row_record(const MeshView &mv, const GridP
         rec[12] = m2.x; rec[13] = m2.y; rec[14] = m2.z;
         rec[15] = dot(m1, e0); rec[16] = dot(m2, ec);
         rec[17] = eps * sqrtf(dot(e0, e0)); rec[18] = eps * sqrtf(dot(e1, e1)); rec[19] = eps * sqrtf(dot(ec, ec));
-        ri[RR_ID] = (int)p; ri[RR_TYPE] = 0;
+        ri[RR_ID] = mv.perm[p]; ri[RR_TYPE] = 0; ri[RR_TIDX] = (int)p;
     } else if (p < (int64_t)mv.F + mv.E) {
         // edge wedge: beyond both faces' side planes, between the end caps
         const EdgeRec &r = mv.erec[p - mv.F];
@@ -566,7 +568,7 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
             if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f) d = fabsf(dot_rn(n, r));
             else {
                 // eps margin: exact clamped distance from the triangle itself
-                const float *T = mv.soup + 9 * (size_t)id;
+                const float *T = mv.soup + 9 * (size_t)ri[RR_TIDX];
                 const f3 a = ld3(T);
                 int rg; f3 qq;
                 d = tri_closest<float>(r, ld3(T + 3) - a, ld3(T + 6) - a, n, rg, qq);
@@ -792,7 +794,8 @@ __device__ __forceinline__ CellOut finish_cell(const MeshView &mv, const GridPar
     CellOut o;
     o.d = INFINITY; o.t = -1;
     float d = __uint_as_float((u32)(pack >> 32));
-    int t = (int)(u32)pack;
+    const int xt = (int)(u32)pack;                 // the caller's id of the winning triangle
+    const int t = mv.inv_perm[xt];
     const float *T = mv.soup + 9 * (size_t)t, *N = mv.fn + 3 * (size_t)t;
     bool redo = !(d < g.band - g.guard);
     f3 a = ld3(T), e0 = ld3(T + 3) - a, ec = ld3(T + 6) - a, n = ld3(N);
@@ -825,7 +828,7 @@ __device__ __forceinline__ CellOut finish_cell(const MeshView &mv, const GridPar
         d = (float)D;
     }
     o.d = (neg && d != 0.0f) ? -d : d;
-    o.t = t;
+    o.t = xt;
     return o;
 }
 
@@ -923,7 +926,7 @@ static int ensure(sdf_mesh *m, T **p, size_t *cap, size_t need, cudaStream_t st)
 int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st) {
     MeshView mv;
     mv.soup = m->soup; mv.fn = m->fn; mv.erec = m->erec; mv.vrec = m->vrec; mv.vmint = m->vmint;
-    mv.cvid = m->cvid; mv.adj = m->adj;
+    mv.cvid = m->cvid; mv.adj = m->adj; mv.perm = m->perm; mv.inv_perm = m->inv_perm;
     mv.F = (int)m->F; mv.E = (int)m->E; mv.V = (int)m->V;
     mv.P = m->F + m->E + 2 * m->V;
     const int64_t P = mv.P;

@@ -11,6 +11,7 @@
 // regrouping.
 #include "primitives.cuh"
 #include <math.h>
+#include <stdlib.h>
 
 #define FB 256   // threads per block of the element-wise kernels
 
@@ -33,23 +34,95 @@ __device__ __forceinline__ u32 mix32(u32 x, u32 y, u32 z) {
     return h;
 }
 
-__device__ __forceinline__ u32 canon_bits(float x) { return __float_as_uint(x + 0.0f); }   // -0 + +0 = +0
+// ---- spatial binning (A0).  The soup arrives in arbitrary order; every later
+// step gathers and scatters by vertex / edge / cell, so the library works on a copy ordered
+// along a coarse Morton curve (the paper sorts by Morton code for the same reason,
+// PAPER.md:296-332).  The order is internal: ids written to the output are the caller's.
+__device__ __forceinline__ int f2ord(float f) {           // monotone float -> int
+    int i = __float_as_int(f);
+    return i >= 0 ? i : i ^ 0x7FFFFFFF;
+}
+__device__ __forceinline__ float ord2f(int i) { return __int_as_float(i >= 0 ? i : i ^ 0x7FFFFFFF); }
 
-// One thread per corner (3 floats): reject non-finite input, canonicalise -0 -> +0, then
-// find-or-insert the vertex in the weld table (linear probing).  A slot holds a corner index
-// of its vertex; identity is checked on the exact bits of that corner in the (immutable)
-// input, and the slot converges to the LOWEST corner index of the vertex (atomicMin), so the
-// representative does not depend on the insertion order.  slot[c] = table position of c.
-__global__ void __launch_bounds__(FB) ingest_weld_kernel(const float *__restrict__ in, float *__restrict__ soup,
-                                                         int ncorner, u32 *wtab, u32 mask, u32 *__restrict__ slot,
-                                                         int *__restrict__ flags) {
+// approximate bounding box from a strided sample of first corners (only steers the binning)
+__global__ void __launch_bounds__(FB) bbox_sample_kernel(const float *__restrict__ in, int F, int stride,
+                                                         int *__restrict__ bbox) {
+    int t = (blockIdx.x * FB + threadIdx.x) * stride;
+    int lo[3] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF}, hi[3] = {(int)0x80000000, (int)0x80000000, (int)0x80000000};
+    if (t < F) {
+        const float *p = in + 9 * (size_t)t;
+#pragma unroll
+        for (int i = 0; i < 3; i++)
+            if (isfinite(p[i])) { lo[i] = hi[i] = f2ord(p[i]); }
+    }
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+            lo[i] = min(lo[i], __shfl_xor_sync(0xffffffffu, lo[i], o));
+            hi[i] = max(hi[i], __shfl_xor_sync(0xffffffffu, hi[i], o));
+        }
+        if ((threadIdx.x & 31) == 0) { atomicMin(&bbox[i], lo[i]); atomicMax(&bbox[3 + i], hi[i]); }
+    }
+}
+
+__device__ __forceinline__ u32 spread3(u32 v) {           // 5 bits -> every third bit
+    v &= 31u;
+    v = (v | (v << 8)) & 0x100Fu;
+    v = (v | (v << 4)) & 0x10C3u;
+    v = (v | (v << 2)) & 0x1249u;
+    return v;
+}
+
+// 15-bit Morton key of the first corner (32 bins per axis over the sampled box)
+__global__ void __launch_bounds__(FB) bin_key_kernel(const float *__restrict__ in, int F, const int *__restrict__ bbox,
+                                                     u32 *__restrict__ keys, u32 *__restrict__ vals) {
+    int t = blockIdx.x * FB + threadIdx.x;
+    if (t >= F) return;
+    const float *p = in + 9 * (size_t)t;
+    u32 q[3];
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+        const float lo = ord2f(bbox[i]), hi = ord2f(bbox[3 + i]);
+        const float w = hi - lo;
+        float f = (w > 0.0f && isfinite(w)) ? (p[i] - lo) / w * 32.0f : 0.0f;
+        f = fminf(fmaxf(f, 0.0f), 31.0f);                 // NaN -> 0; outliers -> end bins
+        q[i] = (u32)f;
+    }
+    keys[t] = spread3(q[0]) | (spread3(q[1]) << 1) | (spread3(q[2]) << 2);
+    vals[t] = (u32)t;
+}
+
+__global__ void __launch_bounds__(FB) identity_perm_kernel(int F, u32 *__restrict__ perm) {
+    int t = blockIdx.x * FB + threadIdx.x;
+    if (t < F) perm[t] = (u32)t;
+}
+
+// one thread per float: gather the soup into the internal order, reject non-finite input,
+// canonicalise -0 -> +0; inv_perm[caller's id] = internal index
+__global__ void __launch_bounds__(FB) reorder_kernel(const float *__restrict__ in, const u32 *__restrict__ perm,
+                                                     int64_t n9, float *__restrict__ soup, int *__restrict__ inv_perm,
+                                                     int *__restrict__ flags) {
+    int64_t e = (int64_t)blockIdx.x * FB + threadIdx.x;
+    if (e >= n9) return;
+    const int i = (int)(e / 9), c = (int)(e - 9 * (int64_t)i);
+    const u32 t = perm[i];
+    float x = in[9 * (size_t)t + c];
+    if (!isfinite(x)) atomicOr(flags, ERRB_NONFINITE);
+    soup[e] = x + 0.0f;                                   // -0 + +0 = +0 (round to nearest)
+    if (c == 0) inv_perm[t] = i;
+}
+
+// One thread per corner (3 floats): find-or-insert the vertex in the weld table (linear
+// probing).  A slot holds a corner index of its vertex; identity is checked on the exact bits of
+// that corner, and the slot converges to the LOWEST corner index of the vertex (atomicMin), so
+// the representative does not depend on the insertion order.  slot[c] = table position of c.
+__global__ void __launch_bounds__(FB) weld_insert_kernel(const float *__restrict__ soup, int ncorner, u32 *wtab,
+                                                         u32 mask, u32 *__restrict__ slot) {
     int c = blockIdx.x * FB + threadIdx.x;
     if (c >= ncorner) return;
-    float x = in[3 * (size_t)c], y = in[3 * (size_t)c + 1], z = in[3 * (size_t)c + 2];
-    if (!(isfinite(x) && isfinite(y) && isfinite(z))) atomicOr(flags, ERRB_NONFINITE);
-    x += 0.0f; y += 0.0f; z += 0.0f;
-    soup[3 * (size_t)c] = x; soup[3 * (size_t)c + 1] = y; soup[3 * (size_t)c + 2] = z;
-    const u32 bx = __float_as_uint(x), by = __float_as_uint(y), bz = __float_as_uint(z);
+    const u32 *p = (const u32 *)(soup + 3 * (size_t)c);
+    const u32 bx = p[0], by = p[1], bz = p[2];
     u32 h = mix32(bx, by, bz) & mask;
     for (;;) {
         u32 cur = __ldcg(wtab + h);
@@ -57,8 +130,8 @@ __global__ void __launch_bounds__(FB) ingest_weld_kernel(const float *__restrict
             cur = atomicCAS(wtab + h, EMPTY32, (u32)c);
             if (cur == EMPTY32) break;
         }
-        const float *q = in + 3 * (size_t)cur;
-        if (canon_bits(q[0]) == bx && canon_bits(q[1]) == by && canon_bits(q[2]) == bz) {
+        const u32 *q = (const u32 *)(soup + 3 * (size_t)cur);
+        if (q[0] == bx && q[1] == by && q[2] == bz) {
             if ((u32)c < cur) atomicMin(wtab + h, (u32)c);     // the minimum only ever decreases
             break;
         }
@@ -219,6 +292,7 @@ __global__ void __launch_bounds__(FB) edge_pair_kernel(const int *__restrict__ c
 __global__ void __launch_bounds__(FB) edge_record_kernel(const int *__restrict__ cvid, int n,
                                                          const int *__restrict__ adj, const u32 *__restrict__ ebase,
                                                          const float *__restrict__ soup, const float *__restrict__ fn,
+                                                         const int *__restrict__ perm,
                                                          EdgeRec *__restrict__ erec, u64 *__restrict__ ctr) {
     __shared__ u32 s_cnt[3];
     if (threadIdx.x < 3) s_cnt[threadIdx.x] = 0;
@@ -255,7 +329,8 @@ __global__ void __launch_bounds__(FB) edge_record_kernel(const int *__restrict__
             // flat: the wedge is thinner than 1e-6 * band and lies inside the eps-inflated
             // neighbours (reading #5)
             int cls = d > 1e-6 ? 1 : (d < -1e-6 ? -1 : 0);
-            r.tri = t0 < t1 ? t0 : t1;
+            const int x0 = perm[t0], x1 = perm[t1];      // the caller's triangle ids
+            r.tri = x0 < x1 ? x0 : x1;
             r.cls = cls;
             r.pad[0] = r.pad[1] = 0;
             erec[e] = r;
@@ -315,11 +390,12 @@ __global__ void __launch_bounds__(FB) vertex_normal_kernel(const u64 *__restrict
 __global__ void __launch_bounds__(FB) vertex_cone_kernel(const float *__restrict__ soup, const int *__restrict__ cvid,
                                                          int F, const double *__restrict__ vn64,
                                                          long long *__restrict__ vcosq, int *__restrict__ vside,
-                                                         int *__restrict__ vmint) {
+                                                         const int *__restrict__ perm, int *__restrict__ vmint) {
     int t = blockIdx.x * FB + threadIdx.x;
     if (t >= F) return;
     double n[3], p[3][3];
     if (!tri_normal64(soup + 9 * (size_t)t, n, p)) return;
+    const int xt = perm[t];                               // the caller's triangle id
 #pragma unroll
     for (int k = 0; k < 3; k++) {
         int v = cvid[3 * (size_t)t + k];
@@ -335,7 +411,7 @@ __global__ void __launch_bounds__(FB) vertex_cone_kernel(const float *__restrict
             bits |= (s > 1e-9) ? 1 : ((s < -1e-9) ? 2 : 4);     // above / below / on the plane
         }
         if ((vside[v] & bits) != bits) atomicOr(&vside[v], bits);
-        if (vmint[v] > t) atomicMin(&vmint[v], t);
+        if (vmint[v] > xt) atomicMin(&vmint[v], xt);
     }
 }
 
@@ -457,6 +533,8 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
         m->cvid = c.take<int>(3 * (size_t)F);
         m->adj = c.take<int>(3 * (size_t)F);
         m->erec = c.take<EdgeRec>((size_t)(m->E > 0 ? m->E : 1));
+        m->perm = c.take<int>((size_t)F);
+        m->inv_perm = c.take<int>((size_t)F);
         m->d_ctr = c.take<u64>(CTR_TOTAL);
         m->d_flags = c.take<int>(4);
         if (pass == 0) CKS(dev_alloc(al, &m->slab_f, c.off, st));
@@ -470,6 +548,10 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     const u32 capw = pow2_at_least((u64)nc + (u64)nc / 4 + 1);     // load <= 0.8 even if no vertex is shared
     const u32 cape = pow2_at_least((u64)nc + 1);                   // <= 3F/2 forward half-edges: load <= 0.5
     float *staging = nullptr;
+    const char *nb = getenv("SDF_NO_BINNING");
+    const bool bin = !(nb && nb[0] == '1') && F >= 1024;       // tiny meshes live in L2 anyway
+    u32 *bkeys = nullptr, *bkeys2 = nullptr, *bvals2 = nullptr, *bhist = nullptr;
+    int *bbox = nullptr;
     u32 *wtab = nullptr, *slot = nullptr, *etab = nullptr, *ebase = nullptr;
     u64 *scan_ws = nullptr;
     unsigned char *head = nullptr, *fcnt = nullptr;
@@ -486,6 +568,11 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
         fcnt = c.take<unsigned char>((size_t)F);
         vcorner = c.take<int>((size_t)nc);          // V <= 3F
         if (!on_device) staging = c.take<float>(9 * (size_t)F);
+        if (bin) {
+            bkeys = c.take<u32>((size_t)F); bkeys2 = c.take<u32>((size_t)F); bvals2 = c.take<u32>((size_t)F);
+            bhist = c.take<u32>(radix_hist_elems((int)F));
+            bbox = c.take<int>(8);
+        }
         if (pass == 0) CKS(tmp.get(&tslab, c.off));
     }
     const float *src = tri;
@@ -494,7 +581,23 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
         src = staging;
     }
     CK(cudaMemsetAsync(wtab, 0xFF, (size_t)((char *)(etab + cape) - (char *)wtab), st));
-    KL; ingest_weld_kernel<<<blocks_for(nc), FB, 0, st>>>(src, m->soup, nc, wtab, capw - 1, slot, m->d_flags);
+    // A0: order the triangles along a coarse Morton curve, gather + canonicalise
+    u32 *perm = (u32 *)m->perm;
+    if (bin) {
+        const int lo_hi[8] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF, (int)0x80000000, (int)0x80000000, (int)0x80000000, 0, 0};
+        CK(cudaMemcpyAsync(bbox, lo_hi, sizeof(lo_hi), cudaMemcpyHostToDevice, st));
+        const int stride = F > (1 << 18) ? 16 : 1;
+        KL; bbox_sample_kernel<<<blocks_for((F + stride - 1) / stride), FB, 0, st>>>(src, (int)F, stride, bbox);
+        KL; bin_key_kernel<<<blocks_for(F), FB, 0, st>>>(src, (int)F, bbox, bkeys, perm);
+        const int shifts[2] = {0, 8};
+        bool first;
+        CKS(radix_sort_pairs<u32>(bkeys, perm, bkeys2, bvals2, (int)F, shifts, 2, bhist, scan_ws, st, &first));
+        if (!first) CK(cudaMemcpyAsync(perm, bvals2, sizeof(u32) * (size_t)F, cudaMemcpyDeviceToDevice, st));
+    } else {
+        KL; identity_perm_kernel<<<blocks_for(F), FB, 0, st>>>((int)F, perm);
+    }
+    KL; reorder_kernel<<<blocks_for(9 * F), FB, 0, st>>>(src, perm, 9 * F, m->soup, m->inv_perm, m->d_flags);
+    KL; weld_insert_kernel<<<blocks_for(nc), FB, 0, st>>>(m->soup, nc, wtab, capw - 1, slot);
     KL; weld_head_kernel<<<blocks_for(nc), FB, 0, st>>>(wtab, slot, nc, head);
     CKS(launch_scan(HeadIn{head}, HeadOut{wtab, slot, vcorner}, (int64_t)nc, scan_ws, m->d_ctr + CTR_V, st));
     stage_mark(m, SDF_T_INGEST_WELD, 1, st);
@@ -532,7 +635,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     CKS(launch_scan(FcntIn{fcnt}, EbaseOut{ebase}, F, scan_ws, (u64 *)nullptr, st));
     KL; edge_insert_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, etab, cape - 1);
     KL; edge_pair_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, etab, cape - 1, m->adj);
-    KL; edge_record_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, m->adj, ebase, m->soup, m->fn, m->erec, m->d_ctr);
+    KL; edge_record_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, m->adj, ebase, m->soup, m->fn, m->perm, m->erec, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_EDGES, 1, st);
 
@@ -542,7 +645,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     CK(cudaMemsetAsync(vcosq, 0x7F, sizeof(long long) * (size_t)V, st));
     CK(cudaMemsetAsync(m->vmint, 0x7F, sizeof(int) * (size_t)V, st));
     KL; vertex_normal_kernel<<<blocks_for(V), FB, 0, st>>>(vacc, V, vn64);
-    KL; vertex_cone_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, m->cvid, (int)F, vn64, vcosq, vside, m->vmint);
+    KL; vertex_cone_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, m->cvid, (int)F, vn64, vcosq, vside, m->perm, m->vmint);
     KL; vertex_record_kernel<<<blocks_for(V), FB, 0, st>>>(m->soup, vcorner, vn64, vcosq, vside, V, m->vrec, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_VERTICES, 1, st);

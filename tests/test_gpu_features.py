@@ -35,7 +35,10 @@ def test_feature_tables(name, scale):
     assert (s["F"], s["V"], s["E"]) == (F, V, 3 * F // 2)
     assert s["V"] - s["E"] + s["F"] == w.meta["V"] - w.meta["E"] + F          # Euler characteristic
     cvid = B.sdf_get_table(m, B.TABLE_CORNER_VID)
-    assert np.array_equal(cvid, cvid_ref)
+    # same partition of the corners (the numbering of the vertices is the library's own)
+    assert cvid.min() == 0 and cvid.max() == V - 1
+    pairs = np.unique(np.stack([cvid.reshape(-1), cvid_ref.reshape(-1)], axis=1), axis=0)
+    assert pairs.shape[0] == V
 
     # half-edge 3t+k runs corner k -> k+1; its opposite runs the same edge backwards
     adj = B.sdf_get_table(m, B.TABLE_HALFEDGE_ADJ).reshape(-1)
