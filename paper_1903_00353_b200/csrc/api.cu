@@ -150,6 +150,11 @@ static int make_grid(const float origin[3], float h, int nx, int ny, int nz, flo
     const char *pf = getenv("SDF_FILL_MODE");
     g->fill_mode = (pf && pf[0] >= '0' && pf[0] <= '4') ? pf[0] - '0' : 4;
     const char *fd = getenv("SDF_FILL_DEPTH"), *fi = getenv("SDF_FILL_ISSUERS");
+    const char *fp = getenv("SDF_FILL_PRIO");
+    g->fill_prio = fp ? (fp[0] == '1') : 1;
+    const char *fl = getenv("SDF_FILL_CTAS");
+    g->fill_ctas = fl ? atoi(fl) : 32;
+    if (g->fill_ctas < 1 || g->fill_ctas > 64) g->fill_ctas = 32;
     g->fill_depth = fd ? atoi(fd) : 8;
     g->fill_issuers = fi ? atoi(fi) : 4;
     if (g->fill_issuers < 1 || g->fill_issuers > 4) g->fill_issuers = 4;

@@ -44,7 +44,8 @@ enum {
     // statistics that every warp adds to are spread over CTR_SLOTS lines of 8 counters
     // (same-address atomics serialise in L2); sdf_stats sums the slots
     CTR_SPREAD = CTR_COUNT, CTR_SLOTS = 64,
-    CTR_TOTAL = CTR_SPREAD + CTR_SLOTS * 8
+    CTR_BIGCUR = CTR_SPREAD + CTR_SLOTS * 8,     // evaluate_big_kernel: one fetch cursor per row slice
+    CTR_TOTAL = CTR_BIGCUR + 8
 };
 enum { SP_POLY = 0, SP_TESTED, SP_ACCEPTED, SP_ROWS };
 
@@ -93,11 +94,14 @@ struct GridParams {
     int nbx, nby, nbz;              // bricks per axis
     float band, eps, guard, rb;     // rb = band + guard + eps : reach of every polyhedron
     double dband;
+    int big_rows, big_ni;           // polyhedra with more rows / longer rows go to evaluate_big_kernel
     int aabb_mode;                  // debug: candidates = band-expanded triangle AABBs only
     int vec4;                       // 1: nx % 4 == 0 and outputs 16-B aligned -> 128-bit stores
     int fill_mode;                  // 0: TMA fill on the side stream (default); debug: 1 plain stores on the
                                     // side stream, 2 TMA fill on the main stream before the emit, 3 ... first,
                                     // 4 forked after the mid-way host crossing
+    int fill_prio;                  // side stream at the highest priority
+    int fill_ctas;                  // TMA fill: CTAs launched per SM (one per SM survives)
     int fill_depth, fill_issuers;   // TMA fill: chunk pairs in flight per issuing lane, issuing lanes per SM
 };
 
@@ -130,6 +134,7 @@ struct sdf_mesh {
     int *brick_table;
     int *brick_list;                       // scratch slot -> brick index
     u32 *big_list;                         // polyhedra of evaluate_big_kernel
+    u32 *fill_state;                       // fill_tma_kernel: batch cursor + per-SM claims
     u64 *scratch;  size_t scratch_cap;     // bricks * 512 packed values
     u64 h_ctr[CTR_COUNT];
     cudaEvent_t ev[SDF_T_COUNT][2];   // stage begin / end events (created on first use)

@@ -641,7 +641,7 @@ __global__ void __launch_bounds__(32 * ES_WARPS) evaluate_small_kernel(MeshView 
         live = poly_aabv(mv, g, p, H);
         if (live) {
             // big polyhedra (many rows or long rows) go to the block-per-polyhedron kernel
-            if (H.rows > BIG_ROWS || H.i1 - H.i0 >= BIG_NI || g.aabb_mode) {
+            if (H.rows > (u32)g.big_rows || H.i1 - H.i0 >= g.big_ni || g.aabb_mode) {
                 big_list[atomicAdd(&ctr[CTR_BIG], 1ull)] = (u32)p;
             } else {
                 rows = (int)H.rows;
@@ -679,6 +679,7 @@ __global__ void __launch_bounds__(32 * ES_WARPS) evaluate_small_kernel(MeshView 
 
 // One block per big polyhedron (dynamic fetch): warps stride over its rows, lanes over x.
 #define EBIG_BT 256
+#define EBIG_SPLIT 8             // row slices per big polyhedron when the mesh has few polyhedra
 __global__ void __launch_bounds__(EBIG_BT) evaluate_big_kernel(MeshView mv, GridParams g,
                                                                const u32 *__restrict__ big_list,
                                                                const int *__restrict__ table,
@@ -691,7 +692,9 @@ __global__ void __launch_bounds__(EBIG_BT) evaluate_big_kernel(MeshView mv, Grid
     u32 tested = 0, accepted = 0, rows_done = 0;
     while (true) {
         __syncthreads();
-        if (threadIdx.x == 0) s_e = atomicAdd(&ctr[CTR_BIG_NEXT], 1ull);
+        // blockIdx.y = slice: every polyhedron is taken once per slice, and slice y does the
+        // row groups y, y + EBIG_SPLIT, ... (a few huge polyhedra, C1, still fill the GPU)
+        if (threadIdx.x == 0) s_e = atomicAdd(&ctr[CTR_BIGCUR + blockIdx.y], 1ull);
         __syncthreads();
         const u64 e = s_e;
         if (e >= nbig) break;
@@ -704,9 +707,9 @@ __global__ void __launch_bounds__(EBIG_BT) evaluate_big_kernel(MeshView mv, Grid
         }
         __syncthreads();
         const u32 rows = s_rows;
-        for (u32 r = (u32)w; r < rows; r += EBIG_BT / 32)
+        for (u32 r = blockIdx.y * (EBIG_BT / 32) + (u32)w; r < rows; r += gridDim.y * (EBIG_BT / 32))
             process_row<32>(g, s_rec, r, lane, table, scratch, tested, accepted);
-        if (threadIdx.x == 0) rows_done += rows;
+        if (threadIdx.x == 0 && blockIdx.y == 0) rows_done += rows;
     }
     add_stats(ctr, tested, accepted, rows_done);
 }
@@ -750,38 +753,53 @@ __global__ void __launch_bounds__(FILL_BT) fill_kernel(float *__restrict__ dist,
 // of A5-A7 keep (almost) the whole SM while 8 B/cell stream out underneath them.
 #define FILL_TMA_BT 128
 #define FILL_TMA_CHUNK 16384
+// fill_state: [0] = next batch (dynamic fetch), [1 + smid] = SM already has a fill CTA.  More
+// CTAs than SMs are launched and the first to arrive on an SM claims it; the others exit at
+// once.  (With one CTA per SM by count only, a busy GPU stacked several fill CTAs on the few
+// SMs that had room and the fill ran at a fraction of the HBM rate.)
+#define FILL_BATCH 64            // chunks per fetch: 1 MiB contiguous per array
+#define FILL_STATE_WORDS 1024
 template <int DEPTH>
 __global__ void __launch_bounds__(FILL_TMA_BT) fill_tma_kernel(float *__restrict__ dist, int *__restrict__ tri,
-                                                               int64_t n, int issuers) {
+                                                               int64_t n, int issuers, int batch, u32 *__restrict__ state) {
     __shared__ __align__(128) u32 s_d[FILL_TMA_CHUNK / 4];
     __shared__ __align__(128) u32 s_t[FILL_TMA_CHUNK / 4];
+    __shared__ int s_go;
+    const int64_t per = FILL_TMA_CHUNK / 4;
+    const int64_t nchunks = n / per;
+    if (threadIdx.x == 0) {
+        u32 smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        s_go = (smid < FILL_STATE_WORDS - 1) ? (atomicCAS(&state[1 + smid], 0u, 1u) == 0u) : 1;
+    }
+    // ragged tail (< one chunk) with plain stores
+    if (blockIdx.x == 0)
+        for (int64_t i = nchunks * per + threadIdx.x; i < n; i += FILL_TMA_BT) { dist[i] = INFINITY; tri[i] = -1; }
+    __syncthreads();
+    if (!s_go) return;
     for (int i = threadIdx.x; i < FILL_TMA_CHUNK / 4; i += FILL_TMA_BT) { s_d[i] = 0x7F800000u; s_t[i] = 0xFFFFFFFFu; }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy writes -> async proxy reads
     __syncthreads();
-    const int64_t per = FILL_TMA_CHUNK / 4;
-    const int64_t nchunks = n / per;
     if ((threadIdx.x & 31) == 0 && (threadIdx.x >> 5) < issuers) {
         u64 pol;
         asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
         const u32 sd = (u32)__cvta_generic_to_shared(s_d), stt = (u32)__cvta_generic_to_shared(s_t);
-        const int64_t first = (int64_t)blockIdx.x * issuers + (threadIdx.x >> 5);
-        const int64_t stride = (int64_t)gridDim.x * issuers;
-        for (int64_t c = first; c < nchunks; c += stride) {
-            asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
-                         :: "l"(dist + c * per), "r"(sd), "r"(FILL_TMA_CHUNK), "l"(pol) : "memory");
-            asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
-                         :: "l"(tri + c * per), "r"(stt), "r"(FILL_TMA_CHUNK), "l"(pol) : "memory");
-            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-            // at most DEPTH + 1 chunk pairs in flight per issuing lane: bounds the share of the
-            // memory queues the fill takes from the latency-bound kernels running beside it
-            asm volatile("cp.async.bulk.wait_group %0;" :: "n"(DEPTH) : "memory");
+        const int64_t nbatch = (nchunks + batch - 1) / batch;
+        for (;;) {
+            const int64_t bt = (int64_t)atomicAdd(&state[0], 1u);
+            if (bt >= nbatch) break;
+            const int64_t c0 = bt * batch, c1 = c0 + batch < nchunks ? c0 + batch : nchunks;
+            for (int64_t c = c0; c < c1; c++) {
+                asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
+                             :: "l"(dist + c * per), "r"(sd), "r"(FILL_TMA_CHUNK), "l"(pol) : "memory");
+                asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
+                             :: "l"(tri + c * per), "r"(stt), "r"(FILL_TMA_CHUNK), "l"(pol) : "memory");
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                // at most DEPTH + 1 chunk pairs in flight per issuing lane
+                asm volatile("cp.async.bulk.wait_group %0;" :: "n"(DEPTH) : "memory");
+            }
         }
         asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
-    }
-    // ragged tail (< one chunk) with plain stores
-    for (int64_t i = nchunks * per + (int64_t)blockIdx.x * FILL_TMA_BT + threadIdx.x; i < n;
-         i += (int64_t)gridDim.x * FILL_TMA_BT) {
-        dist[i] = INFINITY; tri[i] = -1;
     }
 }
 
@@ -923,7 +941,15 @@ static int ensure(sdf_mesh *m, T **p, size_t *cap, size_t need, cudaStream_t st)
     return SDF_OK;
 }
 
-int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st) {
+int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cudaStream_t st) {
+    GridParams g = g_in;
+    {
+        // a mesh with few polyhedra cannot fill the GPU with one lane per polyhedron: hand more
+        // of them to the block-per-polyhedron kernel
+        const int64_t P0 = m->F + m->E + 2 * m->V;
+        g.big_rows = P0 < 4096 ? 8 : (P0 < 65536 ? 64 : (int)BIG_ROWS);
+        g.big_ni = P0 < 4096 ? 4 : (P0 < 65536 ? 16 : BIG_NI);
+    }
     MeshView mv;
     mv.soup = m->soup; mv.fn = m->fn; mv.erec = m->erec; mv.vrec = m->vrec; mv.vmint = m->vmint;
     mv.cvid = m->cvid; mv.adj = m->adj; mv.perm = m->perm; mv.inv_perm = m->inv_perm;
@@ -939,6 +965,7 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
         m->brick_list = c.take<int>((size_t)nbricks);
         m->scan_ws = c.take<u64>(scan_ws_elems(nbricks));
         m->big_list = c.take<u32>((size_t)P);
+        m->fill_state = c.take<u32>(FILL_STATE_WORDS);
         if (pass == 0 && (c.off > m->slab_ws_cap || !m->slab_ws)) {
             if (m->slab_ws) { dev_free(&m->alloc, m->slab_ws, st); m->slab_ws = nullptr; m->slab_ws_cap = 0; }
             const size_t want = c.off + c.off / 8 + 256;
@@ -959,13 +986,19 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
         stage_mark(m, SDF_T_FILL, 0, fs);
         if (vec && g.fill_mode != 1) {
             const int iss = g.fill_issuers;
+            CK(cudaMemsetAsync(m->fill_state, 0, sizeof(u32) * FILL_STATE_WORDS, fs));
+            const unsigned nb = (unsigned)(sms * g.fill_ctas);
+            // batch of chunks per fetch: 1 MiB per array on large grids, smaller when the grid has
+            // fewer than ~8 batches per issuing lane
+            int64_t bq = (N / (FILL_TMA_CHUNK / 4)) / ((int64_t)sms * iss * 8);
+            const int batch = (int)(bq < 1 ? 1 : (bq > FILL_BATCH ? FILL_BATCH : bq));
             KL;
             switch (g.fill_depth) {
-            case 0: fill_tma_kernel<0><<<(unsigned)sms, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss); break;
-            case 1: fill_tma_kernel<1><<<(unsigned)sms, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss); break;
-            case 2: fill_tma_kernel<2><<<(unsigned)sms, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss); break;
-            case 4: fill_tma_kernel<4><<<(unsigned)sms, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss); break;
-            default: fill_tma_kernel<8><<<(unsigned)sms, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss); break;
+            case 0: fill_tma_kernel<0><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state); break;
+            case 1: fill_tma_kernel<1><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state); break;
+            case 2: fill_tma_kernel<2><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state); break;
+            case 4: fill_tma_kernel<4><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state); break;
+            default: fill_tma_kernel<8><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state); break;
             }
         } else {
             int64_t fb = (N / 4 + (int64_t)FILL_BT * FILL_UNROLL - 1) / ((int64_t)FILL_BT * FILL_UNROLL);
@@ -978,7 +1011,12 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
     };
     const bool forked = g.fill_mode < 2 || g.fill_mode == 4;
     auto fork_fill = [&]() -> int {
-        if (!m->side) CK(cudaStreamCreateWithFlags(&m->side, cudaStreamNonBlocking));
+        if (!m->side) {
+            // highest priority: the (few, tiny) fill CTAs are placed before the evaluate blocks
+            int plo = 0, phi = 0;
+            cudaDeviceGetStreamPriorityRange(&plo, &phi);
+            CK(cudaStreamCreateWithPriority(&m->side, cudaStreamNonBlocking, g.fill_prio ? phi : plo));
+        }
         if (!m->ev_fork) CK(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
         if (!m->ev_join) CK(cudaEventCreateWithFlags(&m->ev_join, cudaEventDisableTiming));
         CK(cudaEventRecord(m->ev_fork, st));
@@ -1014,8 +1052,9 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
     if (bricks) {
         stage_mark(m, SDF_T_EVALUATE, 0, st);
         const int64_t nblk = (P + 32 * ES_WARPS - 1) / (32 * ES_WARPS);
+        const unsigned split = P < 65536 ? EBIG_SPLIT : (P < (1 << 20) ? 2 : 1);
         KL; evaluate_small_kernel<<<(unsigned)nblk, 32 * ES_WARPS, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr);
-        KL; evaluate_big_kernel<<<(unsigned)(sms * 4), EBIG_BT, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr);
+        KL; evaluate_big_kernel<<<dim3((unsigned)(sms * 4 / split), split), EBIG_BT, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr);
         stage_mark(m, SDF_T_EVALUATE, 1, st);
     }
     // A8b: join the fill, then overwrite the active bricks

@@ -98,31 +98,30 @@ __global__ void __launch_bounds__(FB) identity_perm_kernel(int F, u32 *__restric
     if (t < F) perm[t] = (u32)t;
 }
 
-// one thread per float: gather the soup into the internal order, reject non-finite input,
-// canonicalise -0 -> +0; inv_perm[caller's id] = internal index
-__global__ void __launch_bounds__(FB) reorder_kernel(const float *__restrict__ in, const u32 *__restrict__ perm,
-                                                     int64_t n9, float *__restrict__ soup, int *__restrict__ inv_perm,
-                                                     int *__restrict__ flags) {
-    int64_t e = (int64_t)blockIdx.x * FB + threadIdx.x;
-    if (e >= n9) return;
-    const int i = (int)(e / 9), c = (int)(e - 9 * (int64_t)i);
-    const u32 t = perm[i];
-    float x = in[9 * (size_t)t + c];
-    if (!isfinite(x)) atomicOr(flags, ERRB_NONFINITE);
-    soup[e] = x + 0.0f;                                   // -0 + +0 = +0 (round to nearest)
-    if (c == 0) inv_perm[t] = i;
-}
+__device__ __forceinline__ u32 canon_bits(float x) { return __float_as_uint(x + 0.0f); }   // -0 + +0 = +0
 
-// One thread per corner (3 floats): find-or-insert the vertex in the weld table (linear
-// probing).  A slot holds a corner index of its vertex; identity is checked on the exact bits of
-// that corner, and the slot converges to the LOWEST corner index of the vertex (atomicMin), so
-// the representative does not depend on the insertion order.  slot[c] = table position of c.
-__global__ void __launch_bounds__(FB) weld_insert_kernel(const float *__restrict__ soup, int ncorner, u32 *wtab,
-                                                         u32 mask, u32 *__restrict__ slot) {
+// One thread per corner of the internal order: gather the corner from the caller's soup
+// (reject non-finite input, canonicalise -0 -> +0, write the internal copy), then find-or-insert
+// its vertex in the weld table (linear probing).  A slot holds a corner index of its vertex;
+// identity is checked on the exact bits of that corner in the immutable input (its sector was
+// just read by the thread that owns it, so the check hits L2), and the slot converges to the
+// LOWEST corner index of the vertex (atomicMin): the representative does not depend on the
+// insertion order.  slot[c] = table position of c.
+__global__ void __launch_bounds__(FB) ingest_weld_kernel(const float *__restrict__ in, const int *__restrict__ perm,
+                                                         int ncorner, float *__restrict__ soup,
+                                                         int *__restrict__ inv_perm, u32 *wtab, u32 mask,
+                                                         u32 *__restrict__ slot, int *__restrict__ flags) {
     int c = blockIdx.x * FB + threadIdx.x;
     if (c >= ncorner) return;
-    const u32 *p = (const u32 *)(soup + 3 * (size_t)c);
-    const u32 bx = p[0], by = p[1], bz = p[2];
+    const int i = c / 3, k = c - 3 * i;
+    const int t = perm[i];
+    const float *p = in + 9 * (size_t)t + 3 * k;
+    float x = p[0], y = p[1], z = p[2];
+    if (!(isfinite(x) && isfinite(y) && isfinite(z))) atomicOr(flags, ERRB_NONFINITE);
+    x += 0.0f; y += 0.0f; z += 0.0f;
+    soup[3 * (size_t)c] = x; soup[3 * (size_t)c + 1] = y; soup[3 * (size_t)c + 2] = z;
+    if (k == 0) inv_perm[t] = i;
+    const u32 bx = __float_as_uint(x), by = __float_as_uint(y), bz = __float_as_uint(z);
     u32 h = mix32(bx, by, bz) & mask;
     for (;;) {
         u32 cur = __ldcg(wtab + h);
@@ -130,8 +129,9 @@ __global__ void __launch_bounds__(FB) weld_insert_kernel(const float *__restrict
             cur = atomicCAS(wtab + h, EMPTY32, (u32)c);
             if (cur == EMPTY32) break;
         }
-        const u32 *q = (const u32 *)(soup + 3 * (size_t)cur);
-        if (q[0] == bx && q[1] == by && q[2] == bz) {
+        const int ci = (int)cur / 3, ck = (int)cur - 3 * ci;
+        const float *q = in + 9 * (size_t)perm[ci] + 3 * ck;
+        if (canon_bits(q[0]) == bx && canon_bits(q[1]) == by && canon_bits(q[2]) == bz) {
             if ((u32)c < cur) atomicMin(wtab + h, (u32)c);     // the minimum only ever decreases
             break;
         }
@@ -586,7 +586,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     if (bin) {
         const int lo_hi[8] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF, (int)0x80000000, (int)0x80000000, (int)0x80000000, 0, 0};
         CK(cudaMemcpyAsync(bbox, lo_hi, sizeof(lo_hi), cudaMemcpyHostToDevice, st));
-        const int stride = F > (1 << 18) ? 16 : 1;
+        const int stride = F > (1 << 20) ? 64 : (F > (1 << 16) ? 8 : 1);
         KL; bbox_sample_kernel<<<blocks_for((F + stride - 1) / stride), FB, 0, st>>>(src, (int)F, stride, bbox);
         KL; bin_key_kernel<<<blocks_for(F), FB, 0, st>>>(src, (int)F, bbox, bkeys, perm);
         const int shifts[2] = {0, 8};
@@ -596,8 +596,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     } else {
         KL; identity_perm_kernel<<<blocks_for(F), FB, 0, st>>>((int)F, perm);
     }
-    KL; reorder_kernel<<<blocks_for(9 * F), FB, 0, st>>>(src, perm, 9 * F, m->soup, m->inv_perm, m->d_flags);
-    KL; weld_insert_kernel<<<blocks_for(nc), FB, 0, st>>>(m->soup, nc, wtab, capw - 1, slot);
+    KL; ingest_weld_kernel<<<blocks_for(nc), FB, 0, st>>>(src, m->perm, nc, m->soup, m->inv_perm, wtab, capw - 1, slot, m->d_flags);
     KL; weld_head_kernel<<<blocks_for(nc), FB, 0, st>>>(wtab, slot, nc, head);
     CKS(launch_scan(HeadIn{head}, HeadOut{wtab, slot, vcorner}, (int64_t)nc, scan_ws, m->d_ctr + CTR_V, st));
     stage_mark(m, SDF_T_INGEST_WELD, 1, st);
