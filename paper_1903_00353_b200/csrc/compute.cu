@@ -266,6 +266,16 @@ struct BrickOut {
 // long rows are listed by evaluate_small_kernel and taken by evaluate_big_kernel, one block per
 // polyhedron with the lanes along x.
 // ---------------------------------------------------------------------------------------
+// Sign carried with the candidate (the polarity of the winning extrusion).  A face
+// prism knows the side from n.r, a wedge from its class, a cone from its side; FL_SURE says the
+// emit pass may take that sign as is.  Candidates from the eps margin of a prism, from the end
+// cap of a wedge, near the dividing plane of a cone / hemisphere or from a knife edge leave it
+// clear and the emit pass decides from the pseudonormal of the closest feature.
+#define FL_NEG 1u
+#define FL_SURE 2u
+#define TY_NEG 16        // record type word: bit 4 = interior side, bit 5 = never sure
+#define TY_UNSURE 32
+
 #define PR_GEO 20        // 13 geometry floats
 #define PR_ID 33
 #define PR_TYPE 34
@@ -274,7 +284,8 @@ struct BrickOut {
 #define PR_J0 37
 #define PR_NJ 38         // j1 - j0 + 1
 #define PR_K0 39
-#define PR_WORDS 41      // odd stride: records of different owners fall in different banks
+#define PR_NB 40         // wedges: unit bisector of n1, n2 (3 floats)
+#define PR_WORDS 45      // odd stride: records of different owners fall in different banks
 
 __device__ __forceinline__ void set_con(float *rec, int c, f3 m, f3 r0, float lim, float h) {
     const float gx = h * m.x;
@@ -330,7 +341,13 @@ __device__ __forceinline__ void build_record(const MeshView &mv, const GridParam
         no_con(rec, 4);
         G[0] = a.x; G[1] = a.y; G[2] = a.z; G[3] = u.x; G[4] = u.y; G[5] = u.z; G[6] = L;
         G[7] = w1.x; G[8] = w1.y; G[9] = w1.z; G[10] = w2.x; G[11] = w2.y; G[12] = w2.z;
-        ri[PR_ID] = r.tri; ri[PR_TYPE] = 1;
+        ri[PR_ID] = r.tri;
+        ri[PR_TYPE] = 1 | (r.cls < 0 ? TY_NEG : 0) | (dot(n1, n2) < -0.99f ? TY_UNSURE : 0);
+        {
+            const f3 nb = n1 + n2;
+            const float il = rsqrtf(fmaxf(dot(nb, nb), 1e-30f));
+            rec[PR_NB] = il * nb.x; rec[PR_NB + 1] = il * nb.y; rec[PR_NB + 2] = il * nb.z;
+        }
     } else {
         // vertex cone / hemisphere (eq.10, 362-364) inside the ball of radius reach
         const int64_t q = p - mv.F - mv.E;
@@ -345,19 +362,24 @@ __device__ __forceinline__ void build_record(const MeshView &mv, const GridParam
         G[0] = v.x; G[1] = v.y; G[2] = v.z; G[3] = A.x; G[4] = A.y; G[5] = A.z; G[6] = c;
 #pragma unroll
         for (int k = 7; k < 13; k++) G[k] = 0.0f;
-        ri[PR_ID] = mv.vmint[q >> 1]; ri[PR_TYPE] = 2;
+        ri[PR_ID] = mv.vmint[q >> 1];
+        ri[PR_TYPE] = 2 | ((q & 1) ? TY_NEG : 0) | (c <= -1.0f ? TY_UNSURE : 0);
     }
     ri[PR_I0] = H.i0; ri[PR_NI] = H.i1 - H.i0;
     ri[PR_J0] = H.j0; ri[PR_NJ] = H.j1 - H.j0 + 1;
     ri[PR_K0] = H.k0;
 }
 
+// a distance this small against the operands it was differenced from has no reliable sign in fp32
+__device__ __forceinline__ bool tiny_vs(float d, f3 r) { return d <= 1e-5f * (fabsf(r.x) + fabsf(r.y) + fabsf(r.z)); }
+
 __device__ __forceinline__ void put_min(const GridParams &g, const int *__restrict__ table, u64 *__restrict__ scratch,
-                                        int i, int j, int k, float d, int id) {
+                                        int i, int j, int k, float d, int id, u32 fl) {
     int slot = table[((size_t)(k >> 3) * g.nby + (j >> 3)) * g.nbx + (i >> 3)];
     if (slot < 0) return;          // cannot happen: brick_mark_kernel covers every polyhedron
     u64 *cell = scratch + (size_t)slot * BRICK_CELLS + (((k & 7) * 8 + (j & 7)) * 8 + (i & 7));
-    atomicMin(cell, ((u64)__float_as_uint(d) << 32) | (u32)id);
+    // low word: id, then FL_SURE, then FL_NEG -- among equal (d, id) an unsure entry wins
+    atomicMin(cell, ((u64)__float_as_uint(d) << 32) | ((u32)id << 2) | fl);
 }
 
 // One grid row (j,k) of one polyhedron: clip the x-span, then test and evaluate its cells
@@ -369,7 +391,8 @@ __device__ __forceinline__ void process_row(const GridParams &g, const float *re
     const int *ri = (const int *)rec;
     const int nj = ri[PR_NJ];
     const int dk = (int)(row / (u32)nj), dj = (int)(row - (u32)dk * (u32)nj);
-    const int i0 = ri[PR_I0], type = ri[PR_TYPE];
+    const int i0 = ri[PR_I0], tyw = ri[PR_TYPE], type = tyw & 15;
+    const u32 fl_rec = ((tyw & TY_NEG) ? FL_NEG : 0u) | ((tyw & TY_UNSURE) ? 0u : FL_SURE);
     const float fj = (float)dj, fk = (float)dk;
     float tlo = 0.0f, thi = (float)ri[PR_NI];
     bool empty = false;
@@ -409,19 +432,23 @@ __device__ __forceinline__ void process_row(const GridParams &g, const float *re
             const f3 r = mk<float>(fmaf((float)i, h, g.ox) - a.x, ry, rz);
             tested++;
             float d;
+            u32 fl = 0;
             if (g.aabb_mode) {
                 int rg; f3 q;
                 d = tri_closest<float>(r, e0, ec, n, rg, q);
             } else {
                 const float s0 = dot(m0, r), s1 = dot(m1, r - e0), s2 = dot(m2, r - ec);
                 if (s0 < -t0 || s1 < -t1 || s2 < -t2) continue;
-                if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f) d = fabsf(dot_rn(n, r));
-                else { int rg; f3 q; d = tri_closest<float>(r, e0, ec, n, rg, q); }   // eps margin: exact clamped distance
+                if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f) {
+                    const float dn = dot_rn(n, r);
+                    d = fabsf(dn);
+                    fl = (tiny_vs(d, r) ? 0u : FL_SURE) | (dn < 0.0f ? FL_NEG : 0u);
+                } else { int rg; f3 q; d = tri_closest<float>(r, e0, ec, n, rg, q); }   // eps margin: exact clamped distance
             }
-            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id); }
+            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id, fl); }
         }
     } else if (type == 1) {
-        const f3 a = ld3(G), u = ld3(G + 3), w1 = ld3(G + 7), w2 = ld3(G + 10);
+        const f3 a = ld3(G), u = ld3(G + 3), w1 = ld3(G + 7), w2 = ld3(G + 10), nbis = ld3(rec + PR_NB);
         const float L = G[6];
         const float ry = y - a.y, rz = z - a.z;
         for (int i = ia + lane0; i <= ib; i += STRIDE) {
@@ -429,10 +456,14 @@ __device__ __forceinline__ void process_row(const GridParams &g, const float *re
             tested++;
             const float t = dot(u, r);
             if (t < -eps || t > L + eps || dot(w1, r) < -eps || dot(w2, r) < -eps) continue;
-            const float tc = fminf(fmaxf(dot_rn(u, r), 0.0f), L);
+            const float tu = dot_rn(u, r), tc = fminf(fmaxf(tu, 0.0f), L);
             const f3 q = mk<float>(__fmaf_rn(-tc, u.x, r.x), __fmaf_rn(-tc, u.y, r.y), __fmaf_rn(-tc, u.z, r.z));
             const float d = __fsqrt_rn(dot_rn(q, q));
-            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id); }
+            // the end caps belong to the end vertices, and the eps slack of a nearly flat wedge
+            // reaches through the surface: the class gives the sign only where the bisector agrees
+            const float sb = (fl_rec & FL_NEG) ? -dot(nbis, q) : dot(nbis, q);
+            const u32 fl = (tu > 0.0f && tu < L && sb > 1e-2f * d && !tiny_vs(d, r)) ? fl_rec : (fl_rec & FL_NEG);
+            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id, fl); }
         }
     } else {
         const f3 v = ld3(G), A = ld3(G + 3);
@@ -441,10 +472,11 @@ __device__ __forceinline__ void process_row(const GridParams &g, const float *re
         for (int i = ia + lane0; i <= ib; i += STRIDE) {
             const f3 r = mk<float>(fmaf((float)i, h, g.ox) - v.x, ry, rz);
             tested++;
-            const float d = __fsqrt_rn(dot_rn(r, r));
-            if (d >= reach || dot(A, r) < c * d - eps) continue;
+            const float d = __fsqrt_rn(dot_rn(r, r)), ar = dot(A, r);
+            if (d >= reach || ar < c * d - eps) continue;
             accepted++;
-            put_min(g, table, scratch, i, j, k, d, id);
+            // near the plane through the vertex normal to the axis the side is not decided here
+            put_min(g, table, scratch, i, j, k, d, id, ar > 1e-2f * d ? fl_rec : (fl_rec & FL_NEG));
         }
     }
 }
@@ -509,7 +541,13 @@ __device__ __forceinline__ void build_row_record(const MeshView &mv, const GridP
         const f3 w1 = cross(u, n1), w2 = cross(n2, u);
         rec[0] = a.x; rec[1] = a.y; rec[2] = a.z; rec[3] = u.x; rec[4] = u.y; rec[5] = u.z; rec[6] = L;
         rec[7] = w1.x; rec[8] = w1.y; rec[9] = w1.z; rec[10] = w2.x; rec[11] = w2.y; rec[12] = w2.z;
-        ri[RR_ID] = r.tri; ri[RR_TYPE] = 1;
+        ri[RR_ID] = r.tri;
+        ri[RR_TYPE] = 1 | (r.cls < 0 ? TY_NEG : 0) | (dot(n1, n2) < -0.99f ? TY_UNSURE : 0);
+        {
+            const f3 nb = n1 + n2;
+            const float il = rsqrtf(fmaxf(dot(nb, nb), 1e-30f));
+            rec[13] = il * nb.x; rec[14] = il * nb.y; rec[15] = il * nb.z;
+        }
     } else {
         // vertex cone / hemisphere (eq.10, 362-364) inside the ball of radius reach
         const int64_t q = p - mv.F - mv.E;
@@ -517,7 +555,8 @@ __device__ __forceinline__ void build_row_record(const MeshView &mv, const GridP
         const float sg = (q & 1) ? -1.0f : 1.0f;
         rec[0] = r.pos[0]; rec[1] = r.pos[1]; rec[2] = r.pos[2];
         rec[3] = sg * r.axis[0]; rec[4] = sg * r.axis[1]; rec[5] = sg * r.axis[2]; rec[6] = r.cos_cone;
-        ri[RR_ID] = mv.vmint[q >> 1]; ri[RR_TYPE] = 2;
+        ri[RR_ID] = mv.vmint[q >> 1];
+        ri[RR_TYPE] = 2 | ((q & 1) ? TY_NEG : 0) | (r.cos_cone <= -1.0f ? TY_UNSURE : 0);
     }
     const int nj = H.j1 - H.j0 + 1;
     ri[RR_I0] = H.i0; ri[RR_J0] = H.j0; ri[RR_K0] = H.k0; ri[RR_NI] = H.i1 - H.i0 + 1; ri[RR_NJ] = nj;
@@ -536,7 +575,8 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
                                                 const int *__restrict__ table, u64 *__restrict__ scratch,
                                                 u32 &tested, u32 &accepted) {
     const int *ri = (const int *)rec;
-    const int nj = ri[RR_NJ], ni = ri[RR_NI], i0 = ri[RR_I0], type = ri[RR_TYPE], id = ri[RR_ID];
+    const int nj = ri[RR_NJ], ni = ri[RR_NI], i0 = ri[RR_I0], tyw = ri[RR_TYPE], type = tyw & 15, id = ri[RR_ID];
+    const u32 fl_rec = ((tyw & TY_NEG) ? FL_NEG : 0u) | ((tyw & TY_UNSURE) ? 0u : FL_SURE);
     const int dk = (int)(((float)row + 0.5f) * rec[RR_INV_NJ]);
     const int j = ri[RR_J0] + row - dk * nj, k = ri[RR_K0] + dk;
     const float h = g.h, eps = g.eps, reach = g.band + g.guard;      // accept d < reach; the emit pass decides exactly
@@ -565,18 +605,22 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
             const int i = i0 + di;
             const f3 r = mk<float>(__fsub_rn(fmaf((float)i, h, g.ox), rec[0]), ry, rz);
             float d;
-            if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f) d = fabsf(dot_rn(n, r));
-            else {
+            u32 fl = 0;
+            if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f) {
+                const float dnc = dot_rn(n, r);
+                d = fabsf(dnc);
+                fl = (tiny_vs(d, r) ? 0u : FL_SURE) | (dnc < 0.0f ? FL_NEG : 0u);
+            } else {
                 // eps margin: exact clamped distance from the triangle itself
                 const float *T = mv.soup + 9 * (size_t)ri[RR_TIDX];
                 const f3 a = ld3(T);
                 int rg; f3 qq;
                 d = tri_closest<float>(r, ld3(T + 3) - a, ld3(T + 6) - a, n, rg, qq);
             }
-            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id); }
+            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id, fl); }
         }
     } else if (type == 1) {
-        const f3 u = ld3(rec + 3), w1 = ld3(rec + 7), w2 = ld3(rec + 10);
+        const f3 u = ld3(rec + 3), w1 = ld3(rec + 7), w2 = ld3(rec + 10), nbis = ld3(rec + 13);
         const float L = rec[6];
         const float bt = fmaf(u.x, rx0, fmaf(u.y, ry, u.z * rz)), gt = u.x * h;
         const float b1 = fmaf(w1.x, rx0, fmaf(w1.y, ry, w1.z * rz)), g1 = w1.x * h;
@@ -595,10 +639,14 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
             if (t < -eps || t > L + eps || fmaf(fd, g1, b1) < -eps || fmaf(fd, g2, b2) < -eps) continue;
             const int i = i0 + di;
             const f3 r = mk<float>(__fsub_rn(fmaf((float)i, h, g.ox), rec[0]), ry, rz);
-            const float tc = fminf(fmaxf(dot_rn(u, r), 0.0f), L);
+            const float tu = dot_rn(u, r), tc = fminf(fmaxf(tu, 0.0f), L);
             const f3 q = mk<float>(__fmaf_rn(-tc, u.x, r.x), __fmaf_rn(-tc, u.y, r.y), __fmaf_rn(-tc, u.z, r.z));
             const float d = __fsqrt_rn(dot_rn(q, q));
-            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id); }
+            // the end caps belong to the end vertices, and the eps slack of a nearly flat wedge
+            // reaches through the surface: the class gives the sign only where the bisector agrees
+            const float sb = (fl_rec & FL_NEG) ? -dot(nbis, q) : dot(nbis, q);
+            const u32 fl = (tu > 0.0f && tu < L && sb > 1e-2f * d && !tiny_vs(d, r)) ? fl_rec : (fl_rec & FL_NEG);
+            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id, fl); }
         }
     } else {
         const f3 A = ld3(rec + 3);
@@ -617,10 +665,11 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
             const int i = i0 + di;
             const f3 r = mk<float>(__fsub_rn(fmaf((float)i, h, g.ox), rec[0]), ry, rz);
             tested++;
-            const float d = __fsqrt_rn(dot_rn(r, r));
-            if (d >= reach || dot(A, r) < c * d - eps) continue;
+            const float d = __fsqrt_rn(dot_rn(r, r)), ar = dot(A, r);
+            if (d >= reach || ar < c * d - eps) continue;
             accepted++;
-            put_min(g, table, scratch, i, j, k, d, id);
+            // near the plane through the vertex normal to the axis the side is not decided here
+            put_min(g, table, scratch, i, j, k, d, id, ar > 1e-2f * d ? fl_rec : (fl_rec & FL_NEG));
         }
     }
 }
@@ -812,7 +861,13 @@ __device__ __forceinline__ CellOut finish_cell(const MeshView &mv, const GridPar
     CellOut o;
     o.d = INFINITY; o.t = -1;
     float d = __uint_as_float((u32)(pack >> 32));
-    const int xt = (int)(u32)pack;                 // the caller's id of the winning triangle
+    const int xt = (int)((u32)pack >> 2);          // the caller's id of the winning triangle
+    if (((u32)pack & FL_SURE) && d < g.band - g.guard) {
+        // the winning extrusion already told the side and the band test is clear
+        o.d = (((u32)pack & FL_NEG) && d != 0.0f) ? -d : d;
+        o.t = xt;
+        return o;
+    }
     const int t = mv.inv_perm[xt];
     const float *T = mv.soup + 9 * (size_t)t, *N = mv.fn + 3 * (size_t)t;
     bool redo = !(d < g.band - g.guard);
@@ -827,7 +882,7 @@ __device__ __forceinline__ CellOut finish_cell(const MeshView &mv, const GridPar
     f3 dv = (x - a) - q;
     float s = dot(pn, dv);
     bool neg = s < 0.0f;
-    if (fabsf(s) <= 1e-3f * sqrtf(dot(pn, pn) * dot(dv, dv))) redo = true;
+    if (fabsf(s) <= 1e-3f * sqrtf(dot(pn, pn) * dot(dv, dv)) || tiny_vs(d, x - a)) redo = true;
     if (redo) {
         // fp64 on the same winning triangle: exact cell position, distance, region, sign
         recheck++;

@@ -549,7 +549,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     const u32 cape = pow2_at_least((u64)nc + 1);                   // <= 3F/2 forward half-edges: load <= 0.5
     float *staging = nullptr;
     const char *nb = getenv("SDF_NO_BINNING");
-    const bool bin = !(nb && nb[0] == '1') && F >= 1024;       // tiny meshes live in L2 anyway
+    const bool bin = !(nb && nb[0] == '1') && F >= 131072;     // smaller meshes live in L2 anyway
     u32 *bkeys = nullptr, *bkeys2 = nullptr, *bvals2 = nullptr, *bhist = nullptr;
     int *bbox = nullptr;
     u32 *wtab = nullptr, *slot = nullptr, *etab = nullptr, *ebase = nullptr;
