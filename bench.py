@@ -37,6 +37,8 @@ from paper_1903_00353_b200 import workloads as W  # noqa: E402
 METRIC = "narrow_band_sdf_cells_per_s"
 UNIT = "band cells/s"
 L2_BYTES = 126 * 1024 * 1024
+# dram__bytes_read.sum + dram__bytes_write.sum of fill_tma_kernel at C4 (profiles/r1x_ncu_full.md)
+NCU_FILL_TRAFFIC_C4 = 0.010752e6 + 8.529632e9
 
 
 # --------------------------------------------------------------------------------------- #
@@ -65,7 +67,7 @@ class ClockSampler:
     def start(self):
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                       "--format=csv,noheader,nounits", "-lms", "50"],
+                                       "--format=csv,noheader,nounits", "-lms", "10"],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
@@ -289,7 +291,8 @@ def run_ours(args):
     fill_ms = stage_ms.get("fill") or 0.0
     fill_gbs = 8.0 * N / (fill_ms * 1e-3) / 1e9 if fill_ms else 0.0
     roofline = {"bound": "hbm", "kernel": "fill_tma_kernel (A8a dense write of both grids, cp.async.bulk shared->global)",
-                "achieved": fill_gbs, "peak": peak, "unit": "GB/s", "frac": fill_gbs / peak, "traffic": args.traffic,
+                "achieved": fill_gbs, "peak": peak, "unit": "GB/s", "frac": fill_gbs / peak,
+                "traffic": args.traffic if args.traffic is not None else (NCU_FILL_TRAFFIC_C4 if w.name == "C4" else None),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": 8.0 * N,
                 "ms_per_launch": fill_ms, "dominant_stage": dom}
     step_bytes = 8.0 * N + 36.0 * w.ntri
@@ -327,7 +330,8 @@ def main():
     ap.add_argument("--cpu-slices", type=int, default=256, help="z-slices of the oracle sample (cpu_baseline)")
     ap.add_argument("--ref-slices", type=int, default=64, help="z-slices per step of --impl reference")
     ap.add_argument("--traffic", type=float, default=None,
-                    help="dram bytes per emit launch from the committed ncu --set full capture (profiles/)")
+                    help="dram bytes (read + write) per launch of the dominant kernel from the committed "
+                         "ncu --set full capture; default: the C4 figure of profiles/r1x_ncu_full.md")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

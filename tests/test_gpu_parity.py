@@ -82,6 +82,19 @@ def test_ragged_grid_and_offsets(oracle_mod):
     _assert_ok(check_parity(w2, oracle_mod))
 
 
+def test_cells_on_the_surface(oracle_mod):
+    """Box whose faces, edges and corners pass (to fp32 rounding) through cell centres: distances of
+    +-1e-8, zero-area of doubt for the sign carried with a candidate -- those cells must fall back to
+    the fp64 pseudonormal decision and agree with the oracle."""
+    v, t = W.box_mesh((0.525, 0.325, 0.225))
+    soup = W.soup_from_indexed(v, t, np.random.default_rng(21))
+    origin, h, dims = W.grid_over((-1.0,) * 3, (1.0,) * 3, (40,) * 3)
+    w = W.Workload("onsurf", soup, origin, h, dims, 3 * h)
+    res = check_parity(w, oracle_mod)
+    _assert_ok(res)
+    assert res["stats"]["fp64_rechecks"] > 0
+
+
 def test_grid_misses_mesh():
     """Degenerate case: the band does not reach the grid -> all sentinels."""
     v, t = W.box_mesh((0.1, 0.1, 0.1))
