@@ -61,15 +61,16 @@ typedef struct sdf_stats_t {
     int64_t edges_convex, edges_concave, edges_flat;      /* PAPER.md:352 discriminant         */
     int64_t verts_pos_only, verts_neg_only, verts_both, verts_skipped; /* cone sides emitted   */
     int64_t verts_hemisphere;             /* "ruff" vertices: cos_cone <= 0 */
-    int64_t weld_collisions;              /* hash-equal runs that held distinct vertices        */
+    int64_t weld_collisions;              /* reserved (always 0: the weld table probes, it has no runs) */
     /* last sdf_compute */
     int64_t polyhedra;                    /* extrusions with a non-empty clipped bounding volume */
-    int64_t work_items;                   /* (polyhedron, grid row) items after the prefix sum  */
-    int64_t pairs_tested;                 /* (cell, polyhedron) pairs inside a clipped row span */
+    int64_t work_items;                   /* (polyhedron, grid row) items scan-converted        */
+    int64_t pairs_tested;                 /* (cell, polyhedron) pairs a row loop looked at      */
     int64_t pairs_accepted;               /* of those: inside the polyhedron and d < band       */
     int64_t bricks_active, bricks_total;  /* 8x8x8-cell bricks holding packed scratch           */
     int64_t band_cells;                   /* populated output cells                             */
     int64_t fp64_rechecks;                /* cells whose band / sign decision was redone in fp64 */
+                                          /* (cells without a certain sign from their candidate) */
 } sdf_stats_t;
 
 /*
@@ -84,10 +85,12 @@ typedef struct sdf_stats_t {
  *             cudaMemcpyAsync), DEVICE pointer when on_device == 1.  Borrowed for the
  *             duration of the call only.  Vertices are identical iff their three fp32
  *             values are bit-identical (-0 == +0).
- *   ntri      1 .. 2^30-1
+ *   ntri      1 .. 2^29
  *   a         device allocator, or NULL
  *   stream    cudaStream_t (0 = legacy default stream).  The call synchronises the stream
- *             once before returning (validation flags and the vertex count).
+ *             twice (the vertex count mid-way, the validation flags before returning).
+ * The library works on a spatially binned copy of the soup (coarse Morton order); every
+ * triangle id it reports is the caller's.
  *   out       receives the handle on SDF_OK; set to NULL otherwise.
  * Errors: SDF_EINVAL, SDF_ENOTCLOSED, SDF_EORIENT, SDF_EDEGENERATE, SDF_ENOMEM, SDF_ECUDA.
  */
@@ -96,11 +99,11 @@ int sdf_create(const float *tri_xyz, int64_t ntri, int on_device,
 
 /*
  * sdf_compute -- clip every characteristic polyhedron to the band and the grid
- * (PAPER.md:344-364), scan-convert it into (polyhedron, grid-row) work items
- * (sec.5, replacing the schedulers of PAPER.md:366-380), evaluate the
- * exact feature distance for every cell inside and min-combine (PAPER.md:63-77, 374,
- * 386-392), then sign every populated cell from the pseudonormal of its closest feature
- * and write both grids.
+ * (PAPER.md:344-364), scan-convert it row by row (sec.5, replacing the
+ * schedulers of PAPER.md:366-380), evaluate the exact feature distance for every cell
+ * inside and min-combine, then sign every populated cell --
+ * from the polarity of the winning extrusion where that is certain, else
+ * from the pseudonormal of its closest feature -- and write both grids.
  *
  *   origin    HOST pointer to 3 floats: position of sample (0,0,0).  Sample (i,j,k) sits at
  *             origin + (i,j,k)*h (cell centres).
@@ -113,7 +116,9 @@ int sdf_create(const float *tri_xyz, int64_t ntri, int on_device,
  *             the closest triangle, -1 outside the band.  Where several triangles are
  *             equally close (closest point on a shared edge / vertex) the lowest index.
  *   stream    cudaStream_t.  Work is enqueued on it; the call synchronises it once
- *             mid-way (work-item and brick totals) and leaves the final kernels enqueued.
+ *             mid-way (active-brick total) and leaves the final kernels enqueued.  The
+ *             dense sentinel write runs on a library-owned stream that is forked from and
+ *             joined back into `stream` with events (stream-ordered for the caller).
  * May be called repeatedly on one handle with different grids / bands.
  * Errors: SDF_EINVAL, SDF_ENOMEM, SDF_ECUDA.
  */
@@ -156,15 +161,15 @@ int sdf_get_table(sdf_mesh *m, int which, void *dst, size_t bytes);
  * that did not run reports 0.
  */
 enum {
-    SDF_T_INGEST_WELD = 0,  /* A0+A1: copy/canonicalise, hash keys, radix sort, weld ids        */
-    SDF_T_EDGES       = 1,  /* A2+A3: triangle geometry, half-edge sort, pairing, edge classes  */
-    SDF_T_VERTICES    = 2,  /* A3+A4: pseudonormals, cone angles, vertex classes                */
-    SDF_T_CLIP_SCAN   = 3,  /* A5+A6: clip polyhedra, row counts, prefix sums, brick table      */
-    SDF_T_CLEAR       = 4,  /* scratch bricks reset to "empty"                                  */
-    SDF_T_EVALUATE    = 5,  /* A7: work items -> distances -> packed atomicMin                  */
-    SDF_T_EMIT        = 6,  /* A8b: sign pass over the active bricks, written into both grids   */
+    SDF_T_INGEST_WELD = 0,  /* A0+A1: spatial binning, gather/canonicalise, weld table, vertex ids */
+    SDF_T_EDGES       = 1,  /* A2+A3: triangle geometry, half-edge table, pairing, edge classes   */
+    SDF_T_VERTICES    = 2,  /* A3+A4: pseudonormals, cone angles, vertex classes                  */
+    SDF_T_CLIP_SCAN   = 3,  /* A6a: brick marks, prefix sum, brick table, the host crossing       */
+    SDF_T_CLEAR       = 4,  /* scratch bricks reset to "empty"                                    */
+    SDF_T_EVALUATE    = 5,  /* A5-A7: clip, scan-convert, distances, packed atomicMin             */
+    SDF_T_EMIT        = 6,  /* A8b: sign pass over the active bricks, written into both grids     */
     SDF_T_FILL        = 7,  /* A8a: dense sentinel fill of both grids (library-owned side stream,
-                               concurrent with stages 3-5)                                     */
+                               concurrent with stage 5)                                         */
     SDF_T_COUNT       = 8
 };
 int sdf_enable_timing(int on);
