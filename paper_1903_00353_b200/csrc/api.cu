@@ -88,7 +88,7 @@ void sdf_destroy(sdf_mesh *m) {
     if (!m) return;
     cudaStream_t st = m->last_stream;
     cudaStreamSynchronize(st);
-    if (m->side) { cudaStreamSynchronize(m->side); cudaStreamDestroy(m->side); }
+    if (m->side) cudaStreamSynchronize(m->side);      // shared, process-lifetime stream: not destroyed here
     if (m->ev_fork) cudaEventDestroy(m->ev_fork);
     if (m->ev_join) cudaEventDestroy(m->ev_join);
     void *ptrs[] = {m->slab_f, m->slab_v, m->slab_ws, m->scratch};

@@ -1067,10 +1067,19 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
     const bool forked = g.fill_mode < 2 || g.fill_mode == 4;
     auto fork_fill = [&]() -> int {
         if (!m->side) {
-            // highest priority: the (few, tiny) fill CTAs are placed before the evaluate blocks
-            int plo = 0, phi = 0;
-            cudaDeviceGetStreamPriorityRange(&plo, &phi);
-            CK(cudaStreamCreateWithPriority(&m->side, cudaStreamNonBlocking, g.fill_prio ? phi : plo));
+            // one library-owned side stream per process (creating a stream per handle cost ~30 us
+            // per sdf_compute on a fresh handle); highest priority: the few, tiny fill CTAs are
+            // placed before the evaluate blocks
+            static cudaStream_t g_side = nullptr;
+            static int g_side_prio = -1, g_side_dev = -1;
+            if (!g_side || g_side_prio != g.fill_prio || g_side_dev != dev) {
+                int plo = 0, phi = 0;
+                cudaDeviceGetStreamPriorityRange(&plo, &phi);
+                CK(cudaStreamCreateWithPriority(&g_side, cudaStreamNonBlocking, g.fill_prio ? phi : plo));
+                g_side_prio = g.fill_prio;
+                g_side_dev = dev;
+            }
+            m->side = g_side;
         }
         if (!m->ev_fork) CK(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
         if (!m->ev_join) CK(cudaEventCreateWithFlags(&m->ev_join, cudaEventDisableTiming));

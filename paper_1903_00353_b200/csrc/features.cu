@@ -140,13 +140,17 @@ __global__ void __launch_bounds__(FB) ingest_weld_kernel(const float *__restrict
     slot[c] = h;
 }
 
-// head[c] = 1 iff c is the lowest corner of its vertex; vertex ids are the ranks of the heads
-__global__ void __launch_bounds__(FB) weld_head_kernel(const u32 *__restrict__ wtab, const u32 *__restrict__ slot,
-                                                       int n, unsigned char *__restrict__ head) {
-    int c = blockIdx.x * FB + threadIdx.x;
-    if (c < n) head[c] = (wtab[slot[c]] == (u32)c) ? 1 : 0;
-}
-
+// head[c] = 1 iff c is the lowest corner of its vertex; vertex ids are the ranks of the heads.
+// The flag is computed (and stored) by the reduce pass of the scan and read back by its down
+// pass, whose output functor overwrites the table slots of the heads.
+struct HeadCompute {
+    const u32 *wtab; const u32 *slot; unsigned char *head;
+    __device__ u64 operator()(int64_t i) const {
+        const unsigned char v = (wtab[slot[i]] == (u32)i) ? 1 : 0;
+        head[i] = v;
+        return v;
+    }
+};
 struct HeadIn {
     const unsigned char *head;
     __device__ u64 operator()(int64_t i) const { return head[i]; }
@@ -597,8 +601,8 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
         KL; identity_perm_kernel<<<blocks_for(F), FB, 0, st>>>((int)F, perm);
     }
     KL; ingest_weld_kernel<<<blocks_for(nc), FB, 0, st>>>(src, m->perm, nc, m->soup, m->inv_perm, wtab, capw - 1, slot, m->d_flags);
-    KL; weld_head_kernel<<<blocks_for(nc), FB, 0, st>>>(wtab, slot, nc, head);
-    CKS(launch_scan(HeadIn{head}, HeadOut{wtab, slot, vcorner}, (int64_t)nc, scan_ws, m->d_ctr + CTR_V, st));
+    CKS(launch_scan2(HeadCompute{wtab, slot, head}, HeadIn{head}, HeadOut{wtab, slot, vcorner}, (int64_t)nc, scan_ws,
+                     m->d_ctr + CTR_V, st));
     stage_mark(m, SDF_T_INGEST_WELD, 1, st);
     // first host crossing: the vertex count sizes every per-vertex table
     CK(cudaMemcpyAsync(m->h_ctr, m->d_ctr, sizeof(u64) * CTR_COUNT, cudaMemcpyDeviceToHost, st));

@@ -95,19 +95,25 @@ __global__ void __launch_bounds__(SCAN_BT) scan_down_kernel(InF in, OutF out, in
 
 static inline size_t scan_ws_elems(int64_t n) { return (size_t)((n + SCAN_TILE - 1) / SCAN_TILE) + 1; }
 
-// ws: at least scan_ws_elems(n) u64; total (device, may be null) receives the grand total
-template <class InF, class OutF>
-static int launch_scan(InF in, OutF out, int64_t n, u64 *ws, u64 *total, cudaStream_t st) {
+// ws: at least scan_ws_elems(n) u64; total (device, may be null) receives the grand total.
+// inr feeds the reduce pass and ind the down pass: they must return the same values (inr may
+// compute and store what ind then only reads back).
+template <class InR, class InD, class OutF>
+static int launch_scan2(InR inr, InD ind, OutF out, int64_t n, u64 *ws, u64 *total, cudaStream_t st) {
     if (n <= 0) {
         if (total) CK(cudaMemsetAsync(total, 0, sizeof(u64), st));
         return SDF_OK;
     }
     int64_t nb = (n + SCAN_TILE - 1) / SCAN_TILE;
-    KL; scan_reduce_kernel<InF><<<(unsigned)nb, SCAN_BT, 0, st>>>(in, n, ws);
+    KL; scan_reduce_kernel<InR><<<(unsigned)nb, SCAN_BT, 0, st>>>(inr, n, ws);
     KL; scan_partials_kernel<<<1, SCAN_BT, 0, st>>>(ws, nb, total);
-    KL; scan_down_kernel<InF, OutF><<<(unsigned)nb, SCAN_BT, 0, st>>>(in, out, n, ws);
+    KL; scan_down_kernel<InD, OutF><<<(unsigned)nb, SCAN_BT, 0, st>>>(ind, out, n, ws);
     CK(cudaGetLastError());
     return SDF_OK;
+}
+template <class InF, class OutF>
+static int launch_scan(InF in, OutF out, int64_t n, u64 *ws, u64 *total, cudaStream_t st) {
+    return launch_scan2(in, in, out, n, ws, total, st);
 }
 
 // =========================================================================================
