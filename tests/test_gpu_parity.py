@@ -82,6 +82,34 @@ def test_ragged_grid_and_offsets(oracle_mod):
     _assert_ok(check_parity(w2, oracle_mod))
 
 
+def _rotated(vt, seed):
+    v, t = vt
+    return v @ W.random_rotation(np.random.default_rng(seed)).T, t
+
+
+def _shell(r_out=0.7, r_in=0.45, sub=3):
+    """Hollow ball: outer sphere outward-oriented, inner sphere oriented into the void (two
+    components, one inside the other)."""
+    vo, to = W.icosphere_mesh(sub, r_out)
+    vi, ti = W.icosphere_mesh(sub, r_in)
+    return np.concatenate([vo, vi], 0), np.concatenate([to, ti[:, ::-1] + vo.shape[0]], 0)
+
+
+@pytest.mark.parametrize("maker,seed,n,band", [
+    (lambda: W.icosphere_mesh(2, 0.5), 31, 64, 20),                      # band >> triangle: big polyhedra only
+    (lambda: _rotated(W.box_mesh((0.55, 0.4, 0.3)), 32), 32, 96, 6),     # 12 huge oblique triangles (analytic row clips)
+    (lambda: _rotated(W.box_mesh((0.85, 0.004, 0.003)), 33), 33, 80, 4), # needle thinner than a cell in two directions
+    (lambda: _shell(), 34, 72, 5),                                       # nested components, concave inner shell
+    (lambda: _rotated(W.torus_mesh(0.5, 0.2, 48, 24), 35), 35, 96, 9),   # medium polyhedra (row-flattened path), saddles
+])
+def test_regimes(oracle_mod, maker, seed, n, band):
+    """Band / triangle / cell size ratios the five configs do not span, each exercising another
+    path of the scan converter (block-per-polyhedron, flattened rows, analytic clipping)."""
+    w = _small(maker(), seed, n=n, band_cells=band)
+    res = check_parity(w, oracle_mod)
+    _assert_ok(res)
+
+
 def test_cells_on_the_surface(oracle_mod):
     """Box whose faces, edges and corners pass (to fp32 rounding) through cell centres: distances of
     +-1e-8, zero-area of doubt for the sign carried with a candidate -- those cells must fall back to
