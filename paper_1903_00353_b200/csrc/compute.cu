@@ -675,7 +675,10 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
 }
 
 #define ES_WARPS 4
-__global__ void __launch_bounds__(32 * ES_WARPS) evaluate_small_kernel(MeshView mv, GridParams g,
+#ifndef ES_MINB
+#define ES_MINB 9
+#endif
+__global__ void __launch_bounds__(32 * ES_WARPS, ES_MINB) evaluate_small_kernel(MeshView mv, GridParams g,
                                                                        u32 *__restrict__ big_list,
                                                                        const int *__restrict__ table,
                                                                        u64 *__restrict__ scratch, u64 *__restrict__ ctr) {

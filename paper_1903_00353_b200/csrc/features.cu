@@ -168,6 +168,9 @@ struct HeadOut {      // the head replaces the corner index in its slot by the v
 // ---------------------------------------------------------------------------------------
 #define FIXSCALE 1099511627776.0   /* 2^40 */
 
+__device__ __forceinline__ u32 edge_hash(u32 u, u32 w) { return mix32(u, w, 0x51ED270Bu); }
+__device__ __forceinline__ int he_next(int he) { int k = he % 3; return he - k + (k == 2 ? 0 : k + 1); }
+
 __device__ __forceinline__ void dcross(const double *a, const double *b, double *r) {
     r[0] = a[1] * b[2] - a[2] * b[1]; r[1] = a[2] * b[0] - a[0] * b[2]; r[2] = a[0] * b[1] - a[1] * b[0];
 }
@@ -192,7 +195,8 @@ __device__ __forceinline__ bool tri_normal64(const float *__restrict__ T, double
 __global__ void __launch_bounds__(FB) tri_geom_kernel(const float *__restrict__ soup, const u32 *__restrict__ wtab,
                                                       const u32 *__restrict__ slot, int F, int *__restrict__ cvid,
                                                       float *__restrict__ fn, u64 *__restrict__ vacc,
-                                                      unsigned char *__restrict__ fcnt, int *__restrict__ flags) {
+                                                      unsigned char *__restrict__ fcnt, u32 *etab, u32 emask,
+                                                      int *__restrict__ flags) {
     int t = blockIdx.x * FB + threadIdx.x;
     if (t >= F) return;
     const float *T = soup + 9 * (size_t)t;
@@ -224,7 +228,16 @@ __global__ void __launch_bounds__(FB) tri_geom_kernel(const float *__restrict__ 
             for (int i = 0; i < 3; i++)
                 atomicAdd(&vacc[3 * (size_t)v[k] + i], (u64)(long long)llrint(alpha * n[i] * FIXSCALE));
         }
-        nf += v[k] < v[k1];       // half-edge 3t+k goes corner k -> k+1; forward = ascending ids
+        // half-edge 3t+k goes corner k -> k+1; forward = ascending ids.  Forward
+        // half-edges take the first empty slot of the edge table on their probe sequence (no key
+        // check: a valid mesh has one forward half-edge per key, and a duplicate just leaves an
+        // entry nobody claims, which the pair count exposes)
+        if (v[k] < v[k1]) {
+            nf++;
+            u32 h = edge_hash((u32)v[k], (u32)v[k1]) & emask;
+            while (__ldcg(etab + h) != EMPTY32 || atomicCAS(etab + h, EMPTY32, (u32)(3 * t + k)) != EMPTY32)
+                h = (h + 1) & emask;
+        }
     }
     fcnt[t] = (unsigned char)nf;
 }
@@ -245,49 +258,51 @@ struct EbaseOut {
 // is read back from cvid); backward half-edges look their partner up and claim it.
 // The mesh is valid iff the number of claimed pairs equals 3F/2.
 // ---------------------------------------------------------------------------------------
-__device__ __forceinline__ u32 edge_hash(u32 u, u32 w) { return mix32(u, w, 0x51ED270Bu); }
-__device__ __forceinline__ int he_next(int he) { int k = he % 3; return he - k + (k == 2 ? 0 : k + 1); }
 
-__global__ void __launch_bounds__(FB) edge_insert_kernel(const int *__restrict__ cvid, int n, u32 *etab, u32 mask) {
-    int he = blockIdx.x * FB + threadIdx.x;
-    if (he >= n) return;
-    const u32 u = (u32)cvid[he], w = (u32)cvid[he_next(he)];
-    if (!(u < w)) return;
-    u32 h = edge_hash(u, w) & mask;
-    for (;;) {
-        u32 cur = __ldcg(etab + h);
-        if (cur == EMPTY32) {
-            cur = atomicCAS(etab + h, EMPTY32, (u32)he);
-            if (cur == EMPTY32) return;
-        }
-        // same key already present: a second forward half-edge (invalid mesh; the pair count
-        // will fall short and the exact classification runs)
-        if ((u32)cvid[cur] == u && (u32)cvid[he_next((int)cur)] == w) return;
-        h = (h + 1) & mask;
-    }
-}
-
-// one thread per half-edge; backward ones claim their forward partner
-__global__ void __launch_bounds__(FB) edge_pair_kernel(const int *__restrict__ cvid, int n, u32 *etab, u32 mask,
+// one thread per triangle; its backward half-edges claim their forward partners.  The three
+// probe chains of a thread are independent, which is what hides the L2 latency here.
+__global__ void __launch_bounds__(FB) edge_pair_kernel(const int *__restrict__ cvid, int F, u32 *etab, u32 mask,
                                                        int *__restrict__ adj) {
-    int he1 = blockIdx.x * FB + threadIdx.x;
-    if (he1 >= n) return;
-    const u32 w = (u32)cvid[he1], u = (u32)cvid[he_next(he1)];     // backward: w -> u with u < w
-    if (!(u < w)) return;
-    u32 h = edge_hash(u, w) & mask;
-    for (;;) {
-        u32 cur = __ldcg(etab + h);
-        if (cur == EMPTY32) return;                              // no forward partner
-        int cand = (int)(cur & ~HE_MATCHED);
-        if ((u32)cvid[cand] == u && (u32)cvid[he_next(cand)] == w) {
-            u32 prev = atomicOr(etab + h, HE_MATCHED);
-            if (!(prev & HE_MATCHED)) {                          // else: a second backward half-edge
-                adj[cand] = he1;
-                adj[he1] = cand;
+    int t = blockIdx.x * FB + threadIdx.x;
+    if (t >= F) return;
+    const u32 c[3] = {(u32)cvid[3 * (size_t)t], (u32)cvid[3 * (size_t)t + 1], (u32)cvid[3 * (size_t)t + 2]};
+    u32 h[3];
+    bool act[3];
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const u32 w = c[k], u = c[k == 2 ? 0 : k + 1];         // backward: w -> u with u < w
+        act[k] = u < w;
+        h[k] = edge_hash(u, w) & mask;
+    }
+    while (act[0] || act[1] || act[2]) {
+        u32 cur[3];
+#pragma unroll
+        for (int k = 0; k < 3; k++) cur[k] = act[k] ? __ldcg(etab + h[k]) : EMPTY32;
+        u32 ku[3], kw[3];
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            if (act[k] && cur[k] == EMPTY32) act[k] = false;             // no forward partner
+            if (act[k]) {
+                const int cand = (int)(cur[k] & ~HE_MATCHED);
+                ku[k] = (u32)cvid[cand]; kw[k] = (u32)cvid[he_next(cand)];
             }
-            return;
         }
-        h = (h + 1) & mask;
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            if (!act[k]) continue;
+            const u32 w = c[k], u = c[k == 2 ? 0 : k + 1];
+            if (ku[k] == u && kw[k] == w) {
+                const u32 prev = atomicOr(etab + h[k], HE_MATCHED);
+                if (!(prev & HE_MATCHED)) {                              // else: a second backward half-edge
+                    const int cand = (int)(cur[k] & ~HE_MATCHED);
+                    adj[cand] = 3 * t + k;
+                    adj[3 * t + k] = cand;
+                }
+                act[k] = false;
+            } else {
+                h[k] = (h[k] + 1) & mask;
+            }
+        }
     }
 }
 
@@ -634,10 +649,9 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     // ---- A3 (per triangle), A2 edge table
     stage_mark(m, SDF_T_EDGES, 0, st);
     CK(cudaMemsetAsync(vacc, 0, (size_t)((char *)(vside + V) - (char *)vacc), st));
-    KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wtab, slot, (int)F, m->cvid, m->fn, vacc, fcnt, m->d_flags);
+    KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wtab, slot, (int)F, m->cvid, m->fn, vacc, fcnt, etab, cape - 1, m->d_flags);
     CKS(launch_scan(FcntIn{fcnt}, EbaseOut{ebase}, F, scan_ws, (u64 *)nullptr, st));
-    KL; edge_insert_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, etab, cape - 1);
-    KL; edge_pair_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, etab, cape - 1, m->adj);
+    KL; edge_pair_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, etab, cape - 1, m->adj);
     KL; edge_record_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, m->adj, ebase, m->soup, m->fn, m->perm, m->erec, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_EDGES, 1, st);
