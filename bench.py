@@ -147,7 +147,7 @@ def run_reference(args):
     rank, _lr, world = dist_env()
     if rank != 0:
         return
-    w = W.config(args.config)
+    w = load_workload(args)
     r = time_oracle(w, args.ref_slices, args.steps, args.warmup)
     line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["s_per_step"] * 1e3,
@@ -157,6 +157,16 @@ def run_reference(args):
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+def load_workload(args):
+    """BASELINE.json config, optionally with another band width (exploration only: the headline
+    numbers are the configs as BASELINE.json states them)."""
+    import dataclasses
+    w = W.config(args.config)
+    if args.band_cells:
+        w = dataclasses.replace(w, band=float(args.band_cells) * w.h)
+    return w
 
 
 def workload_config(w, args):
@@ -185,7 +195,7 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    w = W.config(args.config)
+    w = load_workload(args)
     nx, ny, nz = w.dims
     N = w.ncells
     soup_host = torch.from_numpy(np.ascontiguousarray(w.soup)).pin_memory()
@@ -324,6 +334,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C4", choices=list(W.CONFIG_NAMES))
+    ap.add_argument("--band-cells", type=float, default=0.0, help="override the band width (cells); 0 = the config's")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
