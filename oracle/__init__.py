@@ -65,6 +65,8 @@ def _load():
     lib.oracle_query.restype = C.c_int
     lib.oracle_dist_to_triangles.argtypes = [C.c_void_p, dp, ip, C.c_int64, dp]
     lib.oracle_dist_to_triangles.restype = C.c_int
+    lib.oracle_fill_interior.argtypes = [fp, C.c_int, C.c_int, C.c_int, C.c_float]
+    lib.oracle_fill_interior.restype = C.c_int
     lib.oracle_point_triangle.argtypes = [dp, fp, dp, C.POINTER(C.c_int)]
     lib.oracle_point_triangle.restype = C.c_double
     _lib = lib
@@ -180,6 +182,17 @@ class Mesh:
         if st != 0:
             raise OracleError(st)
         return d
+
+
+def fill_interior(dist, band):
+    """PAPER.md:493 axis sweeps on a narrow-band grid [nz,ny,nx] (a filled copy is returned)."""
+    _load()
+    out = np.ascontiguousarray(dist, dtype=np.float32).copy()
+    nz, ny, nx = out.shape
+    st = _lib.oracle_fill_interior(_p(out, C.c_float), nx, ny, nz, float(np.float32(band)))
+    if st != 0:
+        raise OracleError(st)
+    return out
 
 
 def sdf(workload, nthreads=None):

@@ -433,3 +433,39 @@ int oracle_dist_to_triangles(const oracle_mesh *m, const double *pts, const int3
     }
     return ORACLE_OK;
 }
+
+/*
+ * oracle_fill_interior -- SURVEY.md 8(f) NEXT-1.  PAPER.md:493 (sec.11.3): the narrow band
+ * "lead[s] to a secondary zero crossing between the negative limit of the SDF and the interior
+ * of the surface beyond the maximum distance.  This can be easily fixed by sweeping along each of
+ * the coordinate axes and filling in unset values in the interior of the geometry."
+ *
+ * Written out as stated: for the axes x, y, z in turn, every grid line is walked forward and then
+ * backward, in place.  Walking a line keeps the sign of the last set cell seen (nothing before
+ * the first); an unset cell (+inf) met while that sign is negative lies in the interior and is set
+ * to -band, the negative limit of the narrow-band SDF.  Cells set by an earlier walk count as set
+ * for the later ones.  Exterior cells stay +inf.
+ */
+static void fill_line(float *d, int64_t n, int64_t stride, float fillv) {
+    for (int dir = 0; dir < 2; dir++) {
+        int state = 0;
+        for (int64_t q = 0; q < n; q++) {
+            float *c = d + (dir ? (n - 1 - q) : q) * stride;
+            if (isfinite(*c)) state = (*c < 0.0f) ? -1 : 1;
+            else if (state < 0) *c = fillv;
+        }
+    }
+}
+
+int oracle_fill_interior(float *dist, int nx, int ny, int nz, float band) {
+    if (!dist || nx <= 0 || ny <= 0 || nz <= 0 || !(band > 0.0f)) return ORACLE_EINVAL;
+    const float fillv = -band;
+    const int64_t sx = 1, sy = nx, sz = (int64_t)nx * ny;
+    for (int k = 0; k < nz; k++)
+        for (int j = 0; j < ny; j++) fill_line(dist + k * sz + j * sy, nx, sx, fillv);
+    for (int k = 0; k < nz; k++)
+        for (int i = 0; i < nx; i++) fill_line(dist + k * sz + i * sx, ny, sy, fillv);
+    for (int j = 0; j < ny; j++)
+        for (int i = 0; i < nx; i++) fill_line(dist + j * sy + i * sx, nz, sz, fillv);
+    return ORACLE_OK;
+}
