@@ -285,6 +285,27 @@ def run_ours(args):
                "h2d_bytes_per_step": int(soup_host.numel() * 4), "d2h_bytes_per_step": int(8 * N)}
         del dist_host, tri_host
 
+    # ---- SURVEY.md 8(f) NEXT-1 (not part of the step): interior fill by axis sweeps on the last result
+    fill_int = None
+    if args.fill_interior and rank == 0:
+        keep = dist_out.clone()
+        tms = []
+        for _ in range(3):
+            dist_out.copy_(keep)
+            torch.cuda.synchronize()
+            f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            f0.record(stream)
+            B.sdf_fill_interior(dist_out, w.band, stream=stream)
+            f1.record(stream)
+            torch.cuda.synchronize()
+            tms.append(f0.elapsed_time(f1))
+        filled = int((torch.isfinite(dist_out) & ~torch.isfinite(keep)).sum())
+        fb = 4.0 * N + 4.0 * filled                       # read every cell once, write the interior once
+        fill_int = {"ms": min(tms), "cells_filled": filled, "algorithmic_bytes": fb,
+                    "achieved_gbs": fb / (min(tms) * 1e-3) / 1e9, "bound": "hbm",
+                    "note": "three in-place sweeps: x reads the grid once, y and z twice"}
+        del keep
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -319,7 +340,7 @@ def run_ours(args):
             "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(w, args),
             "band_cells": band_cells, "stage_ms": stage_ms, "step_ms_min": min(step_ms), "wall_ms_per_step":
             t_wall * 1e3 / args.steps, "roofline": roofline, "roofline_step": roofline_step, "cpu_baseline": cpu,
-            "e2e": e2e, "gpu_launches": int(launches), "clocks": clk,
+            "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "fill_interior": fill_int,
             "stats": {k: stats[k] for k in ("polyhedra", "work_items", "pairs_tested", "pairs_accepted",
                                             "bricks_active", "fp64_rechecks")}}
     print(json.dumps(line), flush=True)
@@ -335,6 +356,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C4", choices=list(W.CONFIG_NAMES))
     ap.add_argument("--band-cells", type=float, default=0.0, help="override the band width (cells); 0 = the config's")
+    ap.add_argument("--fill-interior", action="store_true", help="also time sdf_fill_interior (NEXT-1) on the result")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")

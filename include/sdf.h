@@ -133,6 +133,22 @@ int sdf_compute(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int
 int sdf_compute_host(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz,
                      float band, float *dist_out_host, int32_t *tri_out_host, void *stream);
 
+/*
+ * sdf_fill_interior -- PAPER.md:493 (sec.11.3): the narrow band leaves "a secondary zero crossing
+ * between the negative limit of the SDF and the interior of the surface beyond the maximum
+ * distance", fixed "by sweeping along each of the coordinate axes and filling in unset values in
+ * the interior of the geometry".  Operates in place on a dist grid written by sdf_compute: for the
+ * axes x, y, z in turn every grid line is walked forward and then backward; a walk keeps the sign
+ * of the last set (finite) cell, and an unset (+INFINITY) cell met while that sign is negative is
+ * set to -band.  Cells outside the solid stay +INFINITY; the band itself and tri_out are not touched.
+ *
+ *   dist      DEVICE, nx*ny*nz floats, layout of sdf_compute (x fastest)
+ *   band      the band width sdf_compute was called with (the value written is -band)
+ *   stream    cudaStream_t; the three sweeps are enqueued on it, nothing is synchronised
+ * Errors: SDF_EINVAL, SDF_ECUDA.
+ */
+int sdf_fill_interior(float *dist, int nx, int ny, int nz, float band, void *stream);
+
 /* Counters (host struct filled from the handle; synchronises `the last stream used` if a
  * compute is still in flight). */
 int sdf_stats(sdf_mesh *m, sdf_stats_t *out);

@@ -22,7 +22,7 @@ SDF_OK, SDF_EINVAL, SDF_ENOTCLOSED, SDF_EORIENT, SDF_EDEGENERATE, SDF_ENOMEM, SD
 TABLE_CORNER_VID, TABLE_HALFEDGE_ADJ, TABLE_FACE_NORMAL, TABLE_VERTEX_REC, TABLE_EDGE_REC, \
     TABLE_VERTEX_MINTRI = range(6)
 
-EXPORTS = ("sdf_create", "sdf_compute", "sdf_compute_host", "sdf_stats", "sdf_get_table",
+EXPORTS = ("sdf_create", "sdf_compute", "sdf_compute_host", "sdf_fill_interior", "sdf_stats", "sdf_get_table",
            "sdf_destroy", "sdf_strerror", "sdf_last_cuda_error", "sdf_version",
            "sdf_enable_timing", "sdf_get_timings", "sdf_launch_count")
 
@@ -90,6 +90,8 @@ def lib():
     L.sdf_compute.restype = C.c_int
     L.sdf_compute_host.argtypes = L.sdf_compute.argtypes
     L.sdf_compute_host.restype = C.c_int
+    L.sdf_fill_interior.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_float, vp]
+    L.sdf_fill_interior.restype = C.c_int
     L.sdf_stats.argtypes = [vp, C.POINTER(Stats)]
     L.sdf_stats.restype = C.c_int
     L.sdf_get_table.argtypes = [vp, C.c_int, vp, C.c_size_t]
@@ -245,6 +247,16 @@ def sdf_compute_host(mesh: Mesh, origin, h, dims, band, dist_out=None, tri_out=N
     if st != SDF_OK:
         raise SdfError(st, "sdf_compute_host")
     return dist_out, tri_out
+
+
+def sdf_fill_interior(dist, band, stream=None):
+    """PAPER.md:493 axis sweeps, in place on a device dist tensor [nz,ny,nx] written by sdf_compute."""
+    assert dist.is_cuda and dist.is_contiguous() and dist.dim() == 3
+    nz, ny, nx = (int(v) for v in dist.shape)
+    st = lib().sdf_fill_interior(C.c_void_p(dist.data_ptr()), nx, ny, nz, float(band), C.c_void_p(_stream_ptr(stream)))
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_fill_interior")
+    return dist
 
 
 def sdf_stats(mesh: Mesh) -> dict:
