@@ -107,7 +107,8 @@ int sdf_create(const float *tri_xyz, int64_t ntri, int on_device,
  *
  *   origin    HOST pointer to 3 floats: position of sample (0,0,0).  Sample (i,j,k) sits at
  *             origin + (i,j,k)*h (cell centres).
- *   h         grid spacing > 0;  nx,ny,nz: 1 .. 32767 each;  band > 0 in length units.
+ *   h         grid spacing > 0;  nx,ny,nz: 1 .. 32767 each;  band in length units,
+ *             0 < band <= 250 * h (the paper's bands are 5 .. 62 cells).
  *   dist_out  DEVICE, caller-owned, nx*ny*nz floats, linear index ((int64)k*ny + j)*nx + i
  *             (x fastest).  Signed distance, negative inside, written iff
  *             |d| < band; +INFINITY elsewhere.  Every element is

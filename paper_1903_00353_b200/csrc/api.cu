@@ -126,6 +126,9 @@ static int make_grid(const float origin[3], float h, int nx, int ny, int nz, flo
                      const int32_t *tri, GridParams *g) {
     if (!origin || !(h > 0.0f) || !(band > 0.0f) || !isfinite(h) || !isfinite(band)) return SDF_EINVAL;
     if (nx <= 0 || ny <= 0 || nz <= 0 || nx > 32767 || ny > 32767 || nz > 32767) return SDF_EINVAL;
+    // features flatter than 1e-6 rad are dropped (reading #5): the sliver they would cover,
+    // 1e-6 * band thick, must stay inside the eps = 1e-3 * h inflation of their neighbours
+    if (band > 250.0f * h) return SDF_EINVAL;
     if (!isfinite(origin[0]) || !isfinite(origin[1]) || !isfinite(origin[2])) return SDF_EINVAL;
     memset(g, 0, sizeof(*g));
     g->ox = origin[0]; g->oy = origin[1]; g->oz = origin[2]; g->h = h; g->inv_h = 1.0f / h;

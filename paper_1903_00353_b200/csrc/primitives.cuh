@@ -55,20 +55,29 @@ __global__ void __launch_bounds__(SCAN_BT) scan_reduce_kernel(InF in, int64_t n,
     if (threadIdx.x == 0) partial[blockIdx.x] = tot;
 }
 
-// one block: exclusive scan of partial[0..np) in place, grand total to *total
+// one block: exclusive scan of partial[0..np) in place, grand total to *total; a thread takes
+// SCAN_IPT consecutive values per round
 static __global__ void __launch_bounds__(SCAN_BT) scan_partials_kernel(u64 *partial, int64_t np, u64 *total) {
     __shared__ u64 s_run;
     if (threadIdx.x == 0) s_run = 0;
     __syncthreads();
-    for (int64_t base = 0; base < np; base += SCAN_BT) {
-        int64_t i = base + threadIdx.x;
-        u64 v = (i < np) ? partial[i] : 0;
+    for (int64_t base = 0; base < np; base += SCAN_TILE) {
+        const int64_t i0 = base + (int64_t)threadIdx.x * SCAN_IPT;
+        u64 v[SCAN_IPT], s = 0;
+#pragma unroll
+        for (int k = 0; k < SCAN_IPT; k++) {
+            v[k] = (i0 + k < np) ? partial[i0 + k] : 0;
+            s += v[k];
+        }
         u64 tot;
-        u64 ex = block_excl_scan(v, &tot);
-        u64 run = s_run;
-        if (i < np) partial[i] = run + ex;
+        u64 ex = block_excl_scan(s, &tot) + s_run;
+#pragma unroll
+        for (int k = 0; k < SCAN_IPT; k++) {
+            if (i0 + k < np) partial[i0 + k] = ex;
+            ex += v[k];
+        }
         __syncthreads();
-        if (threadIdx.x == 0) s_run = run + tot;
+        if (threadIdx.x == 0) s_run += tot;
         __syncthreads();
     }
     if (threadIdx.x == 0 && total) *total = s_run;

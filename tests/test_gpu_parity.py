@@ -197,3 +197,6 @@ def test_error_statuses():
     with pytest.raises(B.SdfError) as e:
         B.sdf_compute(m, (0, 0, 0), -1.0, (8, 8, 8), 0.1)
     assert e.value.status == B.SDF_EINVAL
+    with pytest.raises(B.SdfError) as e:
+        B.sdf_compute(m, (0, 0, 0), 0.01, (8, 8, 8), 2.6)       # band > 250 h
+    assert e.value.status == B.SDF_EINVAL
