@@ -219,7 +219,7 @@ int sdf_stats(sdf_mesh *m, sdf_stats_t *o) {
     o->verts_pos_only = (int64_t)c[CTR_V_POS]; o->verts_neg_only = (int64_t)c[CTR_V_NEG];
     o->verts_both = (int64_t)c[CTR_V_BOTH]; o->verts_skipped = (int64_t)c[CTR_V_SKIP];
     o->verts_hemisphere = (int64_t)c[CTR_V_HEMI];
-    o->weld_collisions = (int64_t)c[CTR_WELD_BAD];
+    o->weld_collisions = 0;
     o->polyhedra = (int64_t)c[CTR_POLY]; o->work_items = (int64_t)c[CTR_ITEMS];
     o->pairs_tested = (int64_t)c[CTR_TESTED]; o->pairs_accepted = (int64_t)c[CTR_ACCEPTED];
     o->bricks_active = (int64_t)c[CTR_BRICKS];

@@ -36,10 +36,10 @@ enum { ERRB_NONFINITE = 1, ERRB_NOTCLOSED = 2, ERRB_ORIENT = 4, ERRB_DEGENERATE 
 
 // device counters (sdf_mesh::d_ctr), 64-bit each
 enum {
-    CTR_V = 0, CTR_WELD_BAD, CTR_E_CONVEX, CTR_E_CONCAVE, CTR_E_FLAT,
+    CTR_V = 0, CTR_RESERVED1, CTR_E_CONVEX, CTR_E_CONCAVE, CTR_E_FLAT,
     CTR_V_POS, CTR_V_NEG, CTR_V_BOTH, CTR_V_SKIP, CTR_V_HEMI,
     CTR_POLY, CTR_ITEMS, CTR_BRICKS, CTR_TESTED, CTR_ACCEPTED, CTR_BAND, CTR_RECHECK,
-    CTR_BIG, CTR_BIG_NEXT,       // big-polyhedron list: length, dynamic fetch cursor
+    CTR_BIG, CTR_RESERVED2,      // big-polyhedron list: length (the fetch cursors are CTR_BIGCUR)
     CTR_COUNT = 24,
     // statistics that every warp adds to are spread over CTR_SLOTS lines of 8 counters
     // (same-address atomics serialise in L2); sdf_stats sums the slots
@@ -71,15 +71,14 @@ struct __align__(16) VertexRec {
 };
 static_assert(sizeof(VertexRec) == 32, "VertexRec must be 32 B");
 
-// Band- and grid-dependent header of one polyhedron: its bounding volume in cell indices
-// clipped to the grid and the number of grid rows (j,k) it covers.
+// Band- and grid-dependent bounding volume of one polyhedron in cell indices, clipped to the grid
+// (PAPER.md:348, 364, 370), and the number of grid rows (j,k) it covers.  Lives in registers only.
 struct __align__(16) PolyHdr {
     short i0, i1, j0, j1, k0, k1;
     u32 rows;
 };
 static_assert(sizeof(PolyHdr) == 16, "PolyHdr must be 16 B");
 
-#define ROWS_BIG 0x80000000u         // PolyHdr::rows flag: taken by evaluate_big_kernel
 #define BIG_ROWS 256u                // ... when it has more rows than this
 #define BIG_NI 32                    // ... or rows at least this long
 

@@ -767,7 +767,7 @@ __global__ void __launch_bounds__(EBIG_BT) evaluate_big_kernel(MeshView mv, Grid
 }
 
 // ---------------------------------------------------------------------------------------
-// A8: sign + emit.  Two kernels: (1) fill_kernel streams the sentinels (+inf, -1;
+// A8: sign + emit.  Two kernels: (1) fill_tma_kernel (fill_kernel for unaligned outputs) streams the sentinels (+inf, -1;
 // PAPER.md:66) over both dense grids at HBM write speed -- it depends on nothing, so it
 // runs on a side stream underneath A5-A7; (2) emit_bricks_kernel then overwrites the cells
 // of the active bricks: sign from the pseudonormal of the closest feature.

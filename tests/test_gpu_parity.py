@@ -154,6 +154,31 @@ def test_host_pointer_and_repeat_compute(oracle_mod):
     assert np.array_equal(dh.numpy(), d1) and np.array_equal(th.numpy(), t1)
 
 
+def test_unaligned_outputs_and_user_stream():
+    """Output pointers that are only 4-byte aligned take the plain-store fill and the scalar emit;
+    a caller's non-default stream; results identical to the aligned default-stream run."""
+    import torch
+    from paper_1903_00353_b200 import binding as B
+    w = f32_grid(W.config("C2", 0.5))
+    nx, ny, nz = w.dims
+    n = nx * ny * nz
+    m = B.sdf_create(w.soup)
+    d0, t0 = B.sdf_compute(m, w.origin, w.h, w.dims, w.band)
+    torch.cuda.synchronize()
+    db = torch.full((n + 3,), 7.0, dtype=torch.float32, device="cuda")
+    tb = torch.full((n + 3,), 7, dtype=torch.int32, device="cuda")
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        d1, t1 = B.sdf_compute(m, w.origin, w.h, w.dims, w.band, db[1:n + 1].view(nz, ny, nx), tb[3:n + 3].view(nz, ny, nx),
+                               stream=st)
+    st.synchronize()
+    assert d1.data_ptr() % 16 != 0 and t1.data_ptr() % 16 != 0
+    assert torch.equal(d1, d0) and torch.equal(t1, t0)
+    # nothing outside the two grids was written
+    assert float(db[0]) == 7.0 and float(db[n + 1]) == 7.0 and float(db[n + 2]) == 7.0
+    assert int(tb[0]) == 7 and int(tb[1]) == 7 and int(tb[2]) == 7
+
+
 def test_permutation_invariance():
     """Shuffling the soup permutes ids and leaves distances / signs bit-identical (the packed
     atomicMin is order independent)."""
