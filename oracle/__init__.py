@@ -65,6 +65,8 @@ def _load():
     lib.oracle_query.restype = C.c_int
     lib.oracle_dist_to_triangles.argtypes = [C.c_void_p, dp, ip, C.c_int64, dp]
     lib.oracle_dist_to_triangles.restype = C.c_int
+    lib.oracle_closest_points.argtypes = [C.c_void_p, dp, C.c_double, C.c_int, C.c_int, C.c_int, ip, fp]
+    lib.oracle_closest_points.restype = C.c_int
     lib.oracle_fill_interior.argtypes = [fp, C.c_int, C.c_int, C.c_int, C.c_float]
     lib.oracle_fill_interior.restype = C.c_int
     lib.oracle_point_triangle.argtypes = [dp, fp, dp, C.POINTER(C.c_int)]
@@ -161,6 +163,18 @@ class Mesh:
         if st != 0:
             raise OracleError(st)
         return dist, tri
+
+    def closest_points(self, origin, h, dims, tri):
+        """Closest point on triangle tri[cell] for every cell with tri >= 0: float32 [nz,ny,nx,3], +inf elsewhere."""
+        nx, ny, nz = (int(v) for v in dims)
+        o = np.ascontiguousarray(origin, dtype=np.float64)
+        t = np.ascontiguousarray(tri, dtype=np.int32).reshape(-1)
+        out = np.empty((nz, ny, nx, 3), dtype=np.float32)
+        st = _lib.oracle_closest_points(self._h, _p(o, C.c_double), float(h), nx, ny, nz, _p(t, C.c_int32),
+                                        _p(out, C.c_float))
+        if st != 0:
+            raise OracleError(st)
+        return out
 
     def query(self, pts, nthreads=None):
         """Brute-force signed fp64 distance + closest triangle id for arbitrary points."""

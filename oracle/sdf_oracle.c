@@ -469,3 +469,30 @@ int oracle_fill_interior(float *dist, int nx, int ny, int nz, float band) {
         for (int i = 0; i < nx; i++) fill_line(dist + j * sy + i * sx, nz, sz, fillv);
     return ORACLE_OK;
 }
+
+/*
+ * oracle_closest_points -- SURVEY.md 8(f) NEXT-2: the closest point transform proper
+ * ("the closest point transform ... computes the closest point on the surface" beside
+ * the distance).  Plain definition: for every cell with a closest-triangle id t >= 0 the point of
+ * triangle t nearest to the cell centre x = origin + (i,j,k)*h (same seven-region routine as the
+ * distance, fp64); +inf in the three components elsewhere.
+ */
+int oracle_closest_points(const oracle_mesh *m, const double *origin, double h, int nx, int ny, int nz,
+                          const int32_t *tri, float *cp_out) {
+    if (!m || !origin || !tri || !cp_out || nx <= 0 || ny <= 0 || nz <= 0) return ORACLE_EINVAL;
+    for (int k = 0; k < nz; k++)
+        for (int j = 0; j < ny; j++)
+            for (int i = 0; i < nx; i++) {
+                const int64_t c = ((int64_t)k * ny + j) * nx + i;
+                float *o = cp_out + 3 * c;
+                const int32_t t = tri[c];
+                if (t < 0 || t >= m->F) { o[0] = o[1] = o[2] = INFINITY; continue; }
+                const double p[3] = {origin[0] + i * h, origin[1] + j * h, origin[2] + k * h};
+                const double *T = m->pos + 9 * (int64_t)t;
+                double q[3];
+                int region;
+                closest_point_triangle(p, T, T + 3, T + 6, q, &region);
+                o[0] = (float)q[0]; o[1] = (float)q[1]; o[2] = (float)q[2];
+            }
+    return ORACLE_OK;
+}
