@@ -306,6 +306,25 @@ def run_ours(args):
                     "note": "three in-place sweeps: x reads the grid once, y and z twice"}
         del keep
 
+    # ---- SURVEY.md 8(f) NEXT-2 (not part of the step): closest points of the last result
+    cpt = None
+    if args.closest_points and rank == 0:
+        m = step_device()
+        cp_out = torch.empty((nz, ny, nx, 3), dtype=torch.float32, device=dev)
+        tms = []
+        for _ in range(3):
+            torch.cuda.synchronize()
+            f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            f0.record(stream)
+            B.sdf_closest_points(m, w.origin, w.h, w.dims, tri_out, cp_out, stream=stream)
+            f1.record(stream)
+            torch.cuda.synchronize()
+            tms.append(f0.elapsed_time(f1))
+        m.destroy()
+        cb = 16.0 * N                                      # 4 B of id read + 12 B of point written per cell
+        cpt = {"ms": min(tms), "algorithmic_bytes": cb, "achieved_gbs": cb / (min(tms) * 1e-3) / 1e9, "bound": "hbm"}
+        del cp_out
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -340,7 +359,7 @@ def run_ours(args):
             "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(w, args),
             "band_cells": band_cells, "stage_ms": stage_ms, "step_ms_min": min(step_ms), "wall_ms_per_step":
             t_wall * 1e3 / args.steps, "roofline": roofline, "roofline_step": roofline_step, "cpu_baseline": cpu,
-            "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "fill_interior": fill_int,
+            "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "fill_interior": fill_int, "closest_points": cpt,
             "stats": {k: stats[k] for k in ("polyhedra", "work_items", "pairs_tested", "pairs_accepted",
                                             "bricks_active", "fp64_rechecks")}}
     print(json.dumps(line), flush=True)
@@ -357,6 +376,7 @@ def main():
     ap.add_argument("--config", default="C4", choices=list(W.CONFIG_NAMES))
     ap.add_argument("--band-cells", type=float, default=0.0, help="override the band width (cells); 0 = the config's")
     ap.add_argument("--fill-interior", action="store_true", help="also time sdf_fill_interior (NEXT-1) on the result")
+    ap.add_argument("--closest-points", action="store_true", help="also time sdf_closest_points (NEXT-2) on the result")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -135,6 +135,20 @@ int sdf_compute_host(sdf_mesh *m, const float origin[3], float h, int nx, int ny
                      float band, float *dist_out_host, int32_t *tri_out_host, void *stream);
 
 /*
+ * sdf_closest_points -- the closest point transform proper: for every cell whose
+ * closest-triangle id (as written by sdf_compute on the same grid) is >= 0, the point of that
+ * triangle nearest to the cell centre; +INFINITY in all three components elsewhere.
+ *
+ *   origin, h, nx, ny, nz   the grid sdf_compute was called with
+ *   tri_in    DEVICE, nx*ny*nz int32, the tri_out of sdf_compute
+ *   cp_out    DEVICE, caller-owned, nx*ny*nz*3 floats, [cell][x,y,z], cells in the order of dist_out
+ *   stream    cudaStream_t; one kernel is enqueued, nothing is synchronised
+ * Errors: SDF_EINVAL, SDF_ECUDA.
+ */
+int sdf_closest_points(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz,
+                       const int32_t *tri_in, float *cp_out, void *stream);
+
+/*
  * sdf_fill_interior -- PAPER.md:493 (sec.11.3): the narrow band leaves "a secondary zero crossing
  * between the negative limit of the SDF and the interior of the surface beyond the maximum
  * distance", fixed "by sweeping along each of the coordinate axes and filling in unset values in

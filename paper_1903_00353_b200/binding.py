@@ -22,7 +22,7 @@ SDF_OK, SDF_EINVAL, SDF_ENOTCLOSED, SDF_EORIENT, SDF_EDEGENERATE, SDF_ENOMEM, SD
 TABLE_CORNER_VID, TABLE_HALFEDGE_ADJ, TABLE_FACE_NORMAL, TABLE_VERTEX_REC, TABLE_EDGE_REC, \
     TABLE_VERTEX_MINTRI = range(6)
 
-EXPORTS = ("sdf_create", "sdf_compute", "sdf_compute_host", "sdf_fill_interior", "sdf_stats", "sdf_get_table",
+EXPORTS = ("sdf_create", "sdf_compute", "sdf_compute_host", "sdf_fill_interior", "sdf_closest_points", "sdf_stats", "sdf_get_table",
            "sdf_destroy", "sdf_strerror", "sdf_last_cuda_error", "sdf_version",
            "sdf_enable_timing", "sdf_get_timings", "sdf_launch_count")
 
@@ -90,6 +90,8 @@ def lib():
     L.sdf_compute.restype = C.c_int
     L.sdf_compute_host.argtypes = L.sdf_compute.argtypes
     L.sdf_compute_host.restype = C.c_int
+    L.sdf_closest_points.argtypes = [vp, C.POINTER(C.c_float), C.c_float, C.c_int, C.c_int, C.c_int, vp, vp, vp]
+    L.sdf_closest_points.restype = C.c_int
     L.sdf_fill_interior.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_float, vp]
     L.sdf_fill_interior.restype = C.c_int
     L.sdf_stats.argtypes = [vp, C.POINTER(Stats)]
@@ -247,6 +249,21 @@ def sdf_compute_host(mesh: Mesh, origin, h, dims, band, dist_out=None, tri_out=N
     if st != SDF_OK:
         raise SdfError(st, "sdf_compute_host")
     return dist_out, tri_out
+
+
+def sdf_closest_points(mesh: Mesh, origin, h, dims, tri, cp_out=None, stream=None):
+    """Closest point on the winning triangle for every band cell: float32 [nz,ny,nx,3] CUDA tensor."""
+    torch = _torch()
+    nx, ny, nz = (int(v) for v in dims)
+    assert tri.is_cuda and tri.is_contiguous() and tri.dtype == torch.int32 and tri.numel() == nx * ny * nz
+    if cp_out is None:
+        cp_out = torch.empty((nz, ny, nx, 3), dtype=torch.float32, device="cuda")
+    assert cp_out.is_cuda and cp_out.is_contiguous() and cp_out.numel() == 3 * nx * ny * nz
+    st = lib().sdf_closest_points(mesh.handle, _origin3(origin), float(h), nx, ny, nz, C.c_void_p(tri.data_ptr()),
+                                  C.c_void_p(cp_out.data_ptr()), C.c_void_p(_stream_ptr(stream)))
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_closest_points")
+    return cp_out
 
 
 def sdf_fill_interior(dist, band, stream=None):

@@ -175,6 +175,14 @@ int sdf_compute(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int
     return s;
 }
 
+int sdf_closest_points(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz, const int32_t *tri_in,
+                       float *cp_out, void *stream) {
+    if (!m || !tri_in || !cp_out) return SDF_EINVAL;
+    GridParams g;
+    CKS(make_grid(origin, h, nx, ny, nz, h, nullptr, nullptr, &g));      // the band plays no part here
+    return run_closest_points(m, g, tri_in, cp_out, (cudaStream_t)stream);
+}
+
 int sdf_compute_host(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz, float band,
                      float *dist_out_host, int32_t *tri_out_host, void *stream) {
     if (!m || !dist_out_host || !tri_out_host) return SDF_EINVAL;

@@ -166,3 +166,4 @@ void stage_mark(sdf_mesh *m, int stage, int which, cudaStream_t st);
 // stages (features.cu / compute.cu)
 int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st);
 int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st);
+int run_closest_points(sdf_mesh *m, const GridParams &g, const int *tri, float *cp, cudaStream_t st);

@@ -1138,3 +1138,68 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
     m->last_bricks_total = nbricks;
     return SDF_OK;
 }
+
+// ---------------------------------------------------------------------------------------
+// closest points (the closest point transform proper).
+// One thread per cell: the point of the winning triangle nearest to the cell centre, +inf outside
+// the band.  HBM-bound: 4 B read + 12 B written per cell; the triangle gathers stay in L2 (the band
+// is walked in grid order and the soup is spatially binned).
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ void closest_point_of(const MeshView &mv, const GridParams &g, int xt, int64_t c, float *o) {
+    o[0] = o[1] = o[2] = INFINITY;
+    if (xt >= 0 && xt < mv.F) {
+        const int i = (int)(c % g.nx), j = (int)((c / g.nx) % g.ny), k = (int)(c / ((int64_t)g.nx * g.ny));
+        const int t = mv.inv_perm[xt];
+        const float *T = mv.soup + 9 * (size_t)t;
+        const f3 a = ld3(T), x = mk<float>(fmaf((float)i, g.h, g.ox), fmaf((float)j, g.h, g.oy), fmaf((float)k, g.h, g.oz));
+        int rg; f3 q;
+        tri_closest<float>(x - a, ld3(T + 3) - a, ld3(T + 6) - a, ld3(mv.fn + 3 * (size_t)t), rg, q);
+        o[0] = a.x + q.x; o[1] = a.y + q.y; o[2] = a.z + q.z;
+    }
+}
+
+// VEC = 4: a thread takes four consecutive cells (one 128-bit load of ids, three 128-bit streaming
+// stores of points); VEC = 1 for unaligned buffers and the ragged tail
+template <int VEC>
+__global__ void __launch_bounds__(256) closest_points_kernel(MeshView mv, GridParams g, const int *__restrict__ tri,
+                                                             float *__restrict__ cp, int64_t first, int64_t n) {
+    const int64_t c = first + ((int64_t)blockIdx.x * 256 + threadIdx.x) * VEC;
+    if (c >= n) return;
+    if (VEC == 4) {
+        const int4 t4 = *(const int4 *)(tri + c);
+        const int xt[4] = {t4.x, t4.y, t4.z, t4.w};
+        float o[12];
+        if ((xt[0] & xt[1] & xt[2] & xt[3]) < 0 && xt[0] < 0 && xt[1] < 0 && xt[2] < 0 && xt[3] < 0) {
+#pragma unroll
+            for (int u = 0; u < 12; u++) o[u] = INFINITY;
+        } else {
+#pragma unroll
+            for (int u = 0; u < 4; u++) closest_point_of(mv, g, xt[u], c + u, o + 3 * u);
+        }
+        float4 *dst = (float4 *)(cp + 3 * c);
+        __stcs(dst, make_float4(o[0], o[1], o[2], o[3]));
+        __stcs(dst + 1, make_float4(o[4], o[5], o[6], o[7]));
+        __stcs(dst + 2, make_float4(o[8], o[9], o[10], o[11]));
+    } else {
+        float o[3];
+        closest_point_of(mv, g, tri[c], c, o);
+        cp[3 * c] = o[0]; cp[3 * c + 1] = o[1]; cp[3 * c + 2] = o[2];
+    }
+}
+
+int run_closest_points(sdf_mesh *m, const GridParams &g, const int *tri, float *cp, cudaStream_t st) {
+    MeshView mv;
+    mv.soup = m->soup; mv.fn = m->fn; mv.erec = m->erec; mv.vrec = m->vrec; mv.vmint = m->vmint;
+    mv.cvid = m->cvid; mv.adj = m->adj; mv.perm = m->perm; mv.inv_perm = m->inv_perm;
+    mv.F = (int)m->F; mv.E = (int)m->E; mv.V = (int)m->V;
+    mv.P = m->F + m->E + 2 * m->V;
+    const int64_t n = (int64_t)g.nx * g.ny * g.nz;
+    const bool vec = (((uintptr_t)tri & 15) == 0) && (((uintptr_t)cp & 15) == 0);
+    const int64_t n4 = vec ? (n & ~(int64_t)3) : 0;
+    if (n4) { KL; closest_points_kernel<4><<<(unsigned)((n4 / 4 + 255) / 256), 256, 0, st>>>(mv, g, tri, cp, 0, n4); }
+    if (n > n4) { KL; closest_points_kernel<1><<<(unsigned)((n - n4 + 255) / 256), 256, 0, st>>>(mv, g, tri, cp, n4, n); }
+    CK(cudaGetLastError());
+    m->last_stream = st;
+    return SDF_OK;
+}
+
