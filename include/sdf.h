@@ -37,7 +37,8 @@ enum {
     SDF_EORIENT     = 3,  /* an edge traversed in the same direction by both triangles */
     SDF_EDEGENERATE = 4,  /* zero-area triangle or repeated vertex in a triangle */
     SDF_ENOMEM      = 5,  /* device (or host staging) allocation failed */
-    SDF_ECUDA       = 6   /* CUDA runtime error / no device; see sdf_last_cuda_error() */
+    SDF_ECUDA       = 6,  /* CUDA runtime error / no device; see sdf_last_cuda_error() */
+    SDF_EIO         = 7   /* file cannot be opened / read / written, or is not a valid STL file */
 };
 
 /* Opaque handle: device-resident feature tables of one mesh.  Owned by the library,
@@ -163,6 +164,26 @@ int sdf_closest_points(sdf_mesh *m, const float origin[3], float h, int nx, int 
  * Errors: SDF_EINVAL, SDF_ECUDA.
  */
 int sdf_fill_interior(float *dist, int nx, int ny, int nz, float band, void *stream);
+
+/*
+ * STL and grid files (host code; "takes as input a stereolithography (STL) file and
+ * outputs a file that lists the SDF values in a 3D grid"; ASCII facet layout PAPER.md:278-288).
+ *
+ * sdf_read_stl   binary or ASCII (detected), -> HOST array [ntri][3 vertices][xyz] allocated by the
+ *                library (release with sdf_free_host), in file order, ready for sdf_create with
+ *                on_device = 0.  The facet normals of the file are ignored: orientation is the
+ *                counter-clockwise vertex order.
+ * sdf_write_stl  ascii != 0: ASCII with 9 significant digits (fp32 round-trips), else binary.
+ * sdf_write_grid the library's own layout (the paper gives none): "SDFGRID1", int32 nx, ny, nz,
+ *                has_tri, float origin[3], h, band, nx*ny*nz floats (x fastest), then, if tri_host is
+ *                not NULL, nx*ny*nz int32.  dist_host / tri_host are HOST buffers.
+ * Errors: SDF_EINVAL, SDF_EIO, SDF_ENOMEM.
+ */
+int  sdf_read_stl(const char *path, float **tri_xyz_out, int64_t *ntri_out);
+void sdf_free_host(void *p);
+int  sdf_write_stl(const char *path, const float *tri_xyz, int64_t ntri, int ascii);
+int  sdf_write_grid(const char *path, const float *dist_host, const int32_t *tri_host,
+                    const float origin[3], float h, int nx, int ny, int nz, float band);
 
 /* Counters (host struct filled from the handle; synchronises `the last stream used` if a
  * compute is still in flight). */

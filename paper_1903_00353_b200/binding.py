@@ -16,15 +16,16 @@ import numpy as np
 from . import build as _build
 
 STATUS_NAMES = {0: "SDF_OK", 1: "SDF_EINVAL", 2: "SDF_ENOTCLOSED", 3: "SDF_EORIENT",
-                4: "SDF_EDEGENERATE", 5: "SDF_ENOMEM", 6: "SDF_ECUDA"}
-SDF_OK, SDF_EINVAL, SDF_ENOTCLOSED, SDF_EORIENT, SDF_EDEGENERATE, SDF_ENOMEM, SDF_ECUDA = range(7)
+                4: "SDF_EDEGENERATE", 5: "SDF_ENOMEM", 6: "SDF_ECUDA", 7: "SDF_EIO"}
+SDF_OK, SDF_EINVAL, SDF_ENOTCLOSED, SDF_EORIENT, SDF_EDEGENERATE, SDF_ENOMEM, SDF_ECUDA, SDF_EIO = range(8)
 
 TABLE_CORNER_VID, TABLE_HALFEDGE_ADJ, TABLE_FACE_NORMAL, TABLE_VERTEX_REC, TABLE_EDGE_REC, \
     TABLE_VERTEX_MINTRI = range(6)
 
 EXPORTS = ("sdf_create", "sdf_compute", "sdf_compute_host", "sdf_fill_interior", "sdf_closest_points", "sdf_stats", "sdf_get_table",
            "sdf_destroy", "sdf_strerror", "sdf_last_cuda_error", "sdf_version",
-           "sdf_enable_timing", "sdf_get_timings", "sdf_launch_count")
+           "sdf_enable_timing", "sdf_get_timings", "sdf_launch_count",
+           "sdf_read_stl", "sdf_free_host", "sdf_write_stl", "sdf_write_grid")
 
 TIMING_STAGES = ("ingest_weld", "edges", "vertices", "clip_scan", "clear", "evaluate", "emit", "fill")
 
@@ -92,6 +93,14 @@ def lib():
     L.sdf_compute_host.restype = C.c_int
     L.sdf_closest_points.argtypes = [vp, C.POINTER(C.c_float), C.c_float, C.c_int, C.c_int, C.c_int, vp, vp, vp]
     L.sdf_closest_points.restype = C.c_int
+    L.sdf_read_stl.argtypes = [C.c_char_p, C.POINTER(C.POINTER(C.c_float)), C.POINTER(C.c_int64)]
+    L.sdf_read_stl.restype = C.c_int
+    L.sdf_free_host.argtypes = [vp]
+    L.sdf_free_host.restype = None
+    L.sdf_write_stl.argtypes = [C.c_char_p, vp, C.c_int64, C.c_int]
+    L.sdf_write_stl.restype = C.c_int
+    L.sdf_write_grid.argtypes = [C.c_char_p, vp, vp, C.POINTER(C.c_float), C.c_float, C.c_int, C.c_int, C.c_int, C.c_float]
+    L.sdf_write_grid.restype = C.c_int
     L.sdf_fill_interior.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_float, vp]
     L.sdf_fill_interior.restype = C.c_int
     L.sdf_stats.argtypes = [vp, C.POINTER(Stats)]
@@ -274,6 +283,37 @@ def sdf_fill_interior(dist, band, stream=None):
     if st != SDF_OK:
         raise SdfError(st, "sdf_fill_interior")
     return dist
+
+
+def sdf_read_stl(path) -> np.ndarray:
+    """Binary or ASCII STL file -> soup float32 [ntri,3,3] (a copy; the library's buffer is released)."""
+    p = C.POINTER(C.c_float)()
+    n = C.c_int64(0)
+    st = lib().sdf_read_stl(str(path).encode(), C.byref(p), C.byref(n))
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_read_stl")
+    try:
+        return np.ctypeslib.as_array(p, shape=(n.value, 3, 3)).copy()
+    finally:
+        lib().sdf_free_host(p)
+
+
+def sdf_write_stl(path, soup, ascii=False):
+    s = np.ascontiguousarray(soup, dtype=np.float32)
+    st = lib().sdf_write_stl(str(path).encode(), C.c_void_p(s.ctypes.data), s.shape[0], 1 if ascii else 0)
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_write_stl")
+
+
+def sdf_write_grid(path, dist, tri, origin, h, band):
+    """dist / tri: HOST arrays [nz,ny,nx] (tri may be None)."""
+    d = np.ascontiguousarray(dist, dtype=np.float32)
+    t = None if tri is None else np.ascontiguousarray(tri, dtype=np.int32)
+    nz, ny, nx = d.shape
+    st = lib().sdf_write_grid(str(path).encode(), C.c_void_p(d.ctypes.data), C.c_void_p(t.ctypes.data if t is not None else None),
+                              _origin3(origin), float(h), nx, ny, nz, float(band))
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_write_grid")
 
 
 def sdf_stats(mesh: Mesh) -> dict:

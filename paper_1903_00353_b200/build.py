@@ -14,7 +14,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libsdf_b200.so")
-SOURCES = ["api.cu", "features.cu", "compute.cu", "fill.cu"]
+SOURCES = ["api.cu", "features.cu", "compute.cu", "fill.cu", "stl_io.cu"]
 HEADERS = ["common.cuh", "primitives.cuh", os.path.join("..", "..", "include", "sdf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--cudart", "static"]

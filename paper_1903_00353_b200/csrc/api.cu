@@ -80,6 +80,7 @@ const char *sdf_strerror(int s) {
     case SDF_EDEGENERATE: return "degenerate triangle (zero area or repeated vertex)";
     case SDF_ENOMEM: return "out of memory";
     case SDF_ECUDA: return "CUDA error or no CUDA device";
+    case SDF_EIO: return "file cannot be opened, read or written, or is not a valid STL file";
     default: return "unknown status";
     }
 }

@@ -179,6 +179,24 @@ def test_unaligned_outputs_and_user_stream():
     assert int(tb[0]) == 7 and int(tb[1]) == 7 and int(tb[2]) == 7
 
 
+def test_stl_file_to_grid_file(tmp_path):
+    """The paper's outer shell: STL file in, grid file out, through the library's own
+    reader and writer; same grids as from the soup in memory."""
+    import torch
+    from paper_1903_00353_b200 import binding as B
+    w = f32_grid(W.config("C2", 0.25))
+    B.sdf_write_stl(tmp_path / "m.stl", w.soup, ascii=True)
+    soup = B.sdf_read_stl(tmp_path / "m.stl")
+    assert np.array_equal(soup, w.soup)
+    d0, t0 = B.sdf_compute(B.sdf_create(w.soup), w.origin, w.h, w.dims, w.band)
+    d1, t1 = B.sdf_compute(B.sdf_create(soup), w.origin, w.h, w.dims, w.band)
+    assert torch.equal(d0, d1) and torch.equal(t0, t1)
+    B.sdf_write_grid(tmp_path / "g.bin", d1.cpu().numpy(), t1.cpu().numpy(), w.origin, w.h, w.band)
+    raw = open(tmp_path / "g.bin", "rb").read()
+    n = d1.numel()
+    assert np.array_equal(np.frombuffer(raw[44:44 + 4 * n], dtype=np.float32), d1.cpu().numpy().reshape(-1))
+
+
 def test_permutation_invariance():
     """Shuffling the soup permutes ids and leaves distances / signs bit-identical (the packed
     atomicMin is order independent)."""
