@@ -154,6 +154,8 @@ static int make_grid(const float origin[3], float h, int nx, int ny, int nz, flo
     const char *pf = getenv("SDF_FILL_MODE");
     g->fill_mode = (pf && pf[0] >= '0' && pf[0] <= '4') ? pf[0] - '0' : 4;
     const char *fd = getenv("SDF_FILL_DEPTH"), *fi = getenv("SDF_FILL_ISSUERS");
+    const char *sc = getenv("SDF_SCHEDULER");
+    g->serial_loop = (sc && !strcmp(sc, "serial")) ? 1 : 0;
     const char *fp = getenv("SDF_FILL_PRIO");
     g->fill_prio = fp ? (fp[0] == '1') : 1;
     const char *fl = getenv("SDF_FILL_CTAS");

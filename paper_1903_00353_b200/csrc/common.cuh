@@ -94,6 +94,7 @@ struct GridParams {
     float band, eps, guard, rb;     // rb = band + guard + eps : reach of every polyhedron
     double dband;
     int big_rows, big_ni;           // polyhedra with more rows / longer rows go to evaluate_big_kernel
+    int serial_loop;                // ablation: the paper's thread-per-extrusion serial loop
     int aabb_mode;                  // debug: candidates = band-expanded triangle AABBs only
     int vec4;                       // 1: nx % 4 == 0 and outputs 16-B aligned -> 128-bit stores
     int fill_mode;                  // 0: TMA fill on the side stream (default); debug: 1 plain stores on the

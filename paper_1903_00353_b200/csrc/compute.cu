@@ -674,11 +674,123 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
     }
 }
 
+// ---- ABLATION, off by default: the paper's first scheduler, "a single
+// thread per extrusion that loops over the cells of its bounding volume" (Table 4).
+// The lane that owns the polyhedron walks its bounding volume itself, plane coefficients in
+// registers: no record, no search, two FMAs per plane and row, one per plane and cell -- and the
+// divergent trip counts of 32 different polyhedra per warp.  SDF_SCHEDULER=serial selects it for
+// every polyhedron the block-per-polyhedron kernel does not take; DESIGN.md sec.12 has the numbers.
+__device__ __forceinline__ void process_direct(const MeshView &mv, const GridParams &g, int64_t p, const PolyHdr &H,
+                                               const int *__restrict__ table, u64 *__restrict__ scratch,
+                                               u32 &tested, u32 &accepted) {
+    const float h = g.h, eps = g.eps, reach = g.band + g.guard;
+    const int i0 = H.i0, j0 = H.j0, k0 = H.k0, ni = H.i1 - H.i0 + 1, nj = H.j1 - H.j0 + 1, nk = H.k1 - H.k0 + 1;
+    if (p < mv.F) {
+        const float *T = mv.soup + 9 * p, *N = mv.fn + 3 * p;
+        const f3 a = ld3(T), e0 = ld3(T + 3) - a, ec = ld3(T + 6) - a, n = ld3(N);
+        const f3 e1 = ec - e0;
+        const f3 m0 = cross(n, e0), m1 = cross(n, e1), m2 = cross(ec, n);          // inward, |m_i| = |edge_i|
+        const float t0 = eps * sqrtf(dot(e0, e0)), t1 = eps * sqrtf(dot(e1, e1)), t2 = eps * sqrtf(dot(ec, ec));
+        const int id = mv.perm[p];
+        const f3 r0 = mk<float>(fmaf((float)i0, h, g.ox) - a.x, fmaf((float)j0, h, g.oy) - a.y, fmaf((float)k0, h, g.oz) - a.z);
+        const float c0 = dot(m0, r0), c1 = dot(m1, r0) - dot(m1, e0), c2 = dot(m2, r0) - dot(m2, ec), cn = dot(n, r0);
+        for (int dk = 0; dk < nk; dk++) {
+            const float fk = (float)dk * h;
+            const float rz = __fsub_rn(fmaf((float)(k0 + dk), h, g.oz), a.z);
+            for (int dj = 0; dj < nj; dj++) {
+                const float fj = (float)dj * h;
+                const float ry = __fsub_rn(fmaf((float)(j0 + dj), h, g.oy), a.y);
+                const float b0 = fmaf(m0.z, fk, fmaf(m0.y, fj, c0)), b1 = fmaf(m1.z, fk, fmaf(m1.y, fj, c1));
+                const float b2 = fmaf(m2.z, fk, fmaf(m2.y, fj, c2)), bn = fmaf(n.z, fk, fmaf(n.y, fj, cn));
+                for (int di = 0; di < ni; di++) {
+                    const float fi = (float)di * h;
+                    const float s0 = fmaf(m0.x, fi, b0), s1 = fmaf(m1.x, fi, b1), s2 = fmaf(m2.x, fi, b2);
+                    const float dn = fmaf(n.x, fi, bn);
+                    if (s0 < -t0 || s1 < -t1 || s2 < -t2 || fabsf(dn) >= reach + eps) continue;
+                    const int i = i0 + di;
+                    const f3 r = mk<float>(__fsub_rn(fmaf((float)i, h, g.ox), a.x), ry, rz);
+                    float d;
+                    u32 fl = 0;
+                    if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f) {
+                        const float dnc = dot_rn(n, r);
+                        d = fabsf(dnc);
+                        fl = (tiny_vs(d, r) ? 0u : FL_SURE) | (dnc < 0.0f ? FL_NEG : 0u);
+                    } else {
+                        int rg; f3 qq;                // eps margin: exact clamped distance
+                        d = tri_closest<float>(r, e0, ec, n, rg, qq);
+                    }
+                    if (d < reach) { accepted++; put_min(g, table, scratch, i, j0 + dj, k0 + dk, d, id, fl); }
+                }
+            }
+        }
+    } else if (p < (int64_t)mv.F + mv.E) {
+        const EdgeRec &er = mv.erec[p - mv.F];
+        const f3 a = ld3(er.a), ab = ld3(er.b) - a, n1 = ld3(er.n1), n2 = ld3(er.n2);
+        const float L = sqrtf(dot(ab, ab));
+        const f3 u = (1.0f / L) * ab;
+        const f3 w1 = cross(u, n1), w2 = cross(n2, u);
+        f3 nbis = n1 + n2;
+        nbis = rsqrtf(fmaxf(dot(nbis, nbis), 1e-30f)) * nbis;
+        const int id = er.tri;
+        const u32 fl_rec = (er.cls < 0 ? FL_NEG : 0u) | (dot(n1, n2) < -0.99f ? 0u : FL_SURE);
+        const f3 r0 = mk<float>(fmaf((float)i0, h, g.ox) - a.x, fmaf((float)j0, h, g.oy) - a.y, fmaf((float)k0, h, g.oz) - a.z);
+        const float ct = dot(u, r0), c1 = dot(w1, r0), c2 = dot(w2, r0);
+        for (int dk = 0; dk < nk; dk++) {
+            const float fk = (float)dk * h;
+            const float rz = __fsub_rn(fmaf((float)(k0 + dk), h, g.oz), a.z);
+            for (int dj = 0; dj < nj; dj++) {
+                const float fj = (float)dj * h;
+                const float ry = __fsub_rn(fmaf((float)(j0 + dj), h, g.oy), a.y);
+                const float bt = fmaf(u.z, fk, fmaf(u.y, fj, ct)), b1 = fmaf(w1.z, fk, fmaf(w1.y, fj, c1));
+                const float b2 = fmaf(w2.z, fk, fmaf(w2.y, fj, c2));
+                for (int di = 0; di < ni; di++) {
+                    const float fi = (float)di * h;
+                    const float t = fmaf(u.x, fi, bt);
+                    if (t < -eps || t > L + eps || fmaf(w1.x, fi, b1) < -eps || fmaf(w2.x, fi, b2) < -eps) continue;
+                    const int i = i0 + di;
+                    const f3 r = mk<float>(__fsub_rn(fmaf((float)i, h, g.ox), a.x), ry, rz);
+                    const float tu = dot_rn(u, r), tc = fminf(fmaxf(tu, 0.0f), L);
+                    const f3 q = mk<float>(__fmaf_rn(-tc, u.x, r.x), __fmaf_rn(-tc, u.y, r.y), __fmaf_rn(-tc, u.z, r.z));
+                    const float d = __fsqrt_rn(dot_rn(q, q));
+                    const float sb = (fl_rec & FL_NEG) ? -dot(nbis, q) : dot(nbis, q);
+                    const u32 fl = (tu > 0.0f && tu < L && sb > 1e-2f * d && !tiny_vs(d, r)) ? fl_rec : (fl_rec & FL_NEG);
+                    if (d < reach) { accepted++; put_min(g, table, scratch, i, j0 + dj, k0 + dk, d, id, fl); }
+                }
+            }
+        }
+    } else {
+        const int64_t q = p - mv.F - mv.E;
+        const VertexRec &vr = mv.vrec[q >> 1];
+        const float sg = (q & 1) ? -1.0f : 1.0f;
+        const f3 v = ld3(vr.pos), A = sg * ld3(vr.axis);
+        const float c = vr.cos_cone;
+        const int id = mv.vmint[q >> 1];
+        const u32 fl_rec = ((q & 1) ? FL_NEG : 0u) | (c <= -1.0f ? 0u : FL_SURE);
+        for (int dk = 0; dk < nk; dk++) {
+            const float rz = __fsub_rn(fmaf((float)(k0 + dk), h, g.oz), v.z);
+            for (int dj = 0; dj < nj; dj++) {
+                const float ry = __fsub_rn(fmaf((float)(j0 + dj), h, g.oy), v.y);
+                if (ry * ry + rz * rz >= reach * reach) continue;
+                for (int di = 0; di < ni; di++) {
+                    const int i = i0 + di;
+                    const f3 r = mk<float>(__fsub_rn(fmaf((float)i, h, g.ox), v.x), ry, rz);
+                    const float d = __fsqrt_rn(dot_rn(r, r)), ar = dot(A, r);
+                    if (d >= reach || ar < c * d - eps) continue;
+                    accepted++;
+                    put_min(g, table, scratch, i, j0 + dj, k0 + dk, d, id, ar > 1e-2f * d ? fl_rec : (fl_rec & FL_NEG));
+                }
+            }
+        }
+    }
+    tested += (u32)(ni * nj * nk);
+}
+
 #define ES_WARPS 4
 #ifndef ES_MINB
 #define ES_MINB 9
 #endif
-__global__ void __launch_bounds__(32 * ES_WARPS, ES_MINB) evaluate_small_kernel(MeshView mv, GridParams g,
+template <bool SERIAL>
+__global__ void __launch_bounds__(32 * ES_WARPS, SERIAL ? 1 : ES_MINB) evaluate_small_kernel(MeshView mv, GridParams g,
                                                                        u32 *__restrict__ big_list,
                                                                        const int *__restrict__ table,
                                                                        u64 *__restrict__ scratch, u64 *__restrict__ ctr) {
@@ -687,7 +799,8 @@ __global__ void __launch_bounds__(32 * ES_WARPS, ES_MINB) evaluate_small_kernel(
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int64_t p = ((int64_t)blockIdx.x * ES_WARPS + w) * 32 + lane;
     int rows = 0;
-    bool live = false;
+    bool live = false, direct = false;
+    PolyHdr Hd;
     if (p < mv.P) {
         PolyHdr H;
         live = poly_aabv(mv, g, p, H);
@@ -695,12 +808,17 @@ __global__ void __launch_bounds__(32 * ES_WARPS, ES_MINB) evaluate_small_kernel(
             // big polyhedra (many rows or long rows) go to the block-per-polyhedron kernel
             if (H.rows > (u32)g.big_rows || H.i1 - H.i0 >= g.big_ni || g.aabb_mode) {
                 big_list[atomicAdd(&ctr[CTR_BIG], 1ull)] = (u32)p;
+            } else if (SERIAL) {
+                direct = true;
+                Hd = H;
             } else {
                 rows = (int)H.rows;
                 build_row_record(mv, g, p, H, s_rec[w][lane]);
             }
         }
     }
+    u32 tested = 0, accepted = 0, rows_direct = 0;
+    if (SERIAL && direct) { process_direct(mv, g, p, Hd, table, scratch, tested, accepted); rows_direct = Hd.rows; }
     const unsigned nlive = __popc(__ballot_sync(0xffffffffu, live));
     if (lane == 0 && nlive)
         atomicAdd(&ctr[CTR_SPREAD + ((blockIdx.x * ES_WARPS + w) & (CTR_SLOTS - 1)) * 8 + SP_POLY], (u64)nlive);
@@ -711,11 +829,9 @@ __global__ void __launch_bounds__(32 * ES_WARPS, ES_MINB) evaluate_small_kernel(
         if (lane >= o) inc += v;
     }
     const int total = __shfl_sync(0xffffffffu, inc, 31);
-    if (total == 0) return;
     s_ex[w][lane] = inc - rows;
     if (lane == 31) s_ex[w][32] = total;
     __syncwarp();
-    u32 tested = 0, accepted = 0;
     for (int base = 0; base < total; base += 32) {
         const int r = base + lane;
         if (r < total) {
@@ -726,7 +842,7 @@ __global__ void __launch_bounds__(32 * ES_WARPS, ES_MINB) evaluate_small_kernel(
             process_row_inc(mv, g, s_rec[w][o], r - s_ex[w][o], table, scratch, tested, accepted);
         }
     }
-    add_stats(ctr, tested, accepted, (u32)rows);
+    add_stats(ctr, tested, accepted, (u32)rows + rows_direct);
 }
 
 // One block per big polyhedron (dynamic fetch): warps stride over its rows, lanes over x.
@@ -1120,7 +1236,9 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
         stage_mark(m, SDF_T_EVALUATE, 0, st);
         const int64_t nblk = (P + 32 * ES_WARPS - 1) / (32 * ES_WARPS);
         const unsigned split = P < 65536 ? EBIG_SPLIT : (P < (1 << 20) ? 2 : 1);
-        KL; evaluate_small_kernel<<<(unsigned)nblk, 32 * ES_WARPS, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr);
+        KL;
+        if (g.serial_loop) evaluate_small_kernel<true><<<(unsigned)nblk, 32 * ES_WARPS, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr);
+        else evaluate_small_kernel<false><<<(unsigned)nblk, 32 * ES_WARPS, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr);
         KL; evaluate_big_kernel<<<dim3((unsigned)(sms * 4 / split), split), EBIG_BT, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr);
         stage_mark(m, SDF_T_EVALUATE, 1, st);
     }

@@ -197,6 +197,27 @@ def test_stl_file_to_grid_file(tmp_path):
     assert np.array_equal(np.frombuffer(raw[44:44 + 4 * n], dtype=np.float32), d1.cpu().numpy().reshape(-1))
 
 
+def test_serial_scheduler_ablation(oracle_mod, monkeypatch):
+    """SDF_SCHEDULER=serial (the paper's thread-per-extrusion loop, kept as an ablation)
+    meets the same four parity clauses, and agrees with the flattened scan converter to the last
+    bit except at cells on a prism's side plane (where the two walks may take the interior or the
+    eps-margin expression of the same distance)."""
+    import torch
+    from paper_1903_00353_b200 import binding as B
+    for w in (f32_grid(W.config("C2", 0.5)), f32_grid(_small(W.torus_mesh(0.5, 0.2, 48, 24), 35, n=96, band_cells=9)),
+              f32_grid(_small(W.ruff_mesh(), 16, n=44, band_cells=5))):
+        m = B.sdf_create(w.soup)
+        d0, t0 = B.sdf_compute(m, w.origin, w.h, w.dims, w.band)
+        monkeypatch.setenv("SDF_SCHEDULER", "serial")
+        _assert_ok(check_parity(w, oracle_mod))
+        d1, t1 = B.sdf_compute(m, w.origin, w.h, w.dims, w.band)
+        monkeypatch.delenv("SDF_SCHEDULER")
+        pop = torch.isfinite(d0)
+        assert torch.equal(pop, torch.isfinite(d1))
+        assert float((d0[pop] - d1[pop]).abs().max()) <= 1e-7
+        assert float((d0[pop] == d1[pop]).float().mean()) > 0.999
+
+
 def test_permutation_invariance():
     """Shuffling the soup permutes ids and leaves distances / signs bit-identical (the packed
     atomicMin is order independent)."""
