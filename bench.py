@@ -67,7 +67,7 @@ class ClockSampler:
     def start(self):
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                       "--format=csv,noheader,nounits", "-lms", "10"],
+                                       "--format=csv,noheader,nounits", "-lms", os.environ.get("BENCH_SMI_MS", "20")],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
@@ -357,7 +357,7 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(w, args),
-            "band_cells": band_cells, "stage_ms": stage_ms, "step_ms_min": min(step_ms), "wall_ms_per_step":
+            "band_cells": band_cells, "stage_ms": stage_ms, "step_ms_min": min(step_ms), "step_ms_max": max(step_ms), "wall_ms_per_step":
             t_wall * 1e3 / args.steps, "roofline": roofline, "roofline_step": roofline_step, "cpu_baseline": cpu,
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "fill_interior": fill_int, "closest_points": cpt,
             "stats": {k: stats[k] for k in ("polyhedra", "work_items", "pairs_tested", "pairs_accepted",
