@@ -12,6 +12,7 @@
 #include "primitives.cuh"
 #include <math.h>
 #include <stdlib.h>
+#include <string.h>
 
 #define FB 256   // threads per block of the element-wise kernels
 
@@ -409,7 +410,8 @@ __global__ void __launch_bounds__(FB) vertex_normal_kernel(const u64 *__restrict
 __global__ void __launch_bounds__(FB) vertex_cone_kernel(const float *__restrict__ soup, const int *__restrict__ cvid,
                                                          int F, const double *__restrict__ vn64,
                                                          long long *__restrict__ vcosq, int *__restrict__ vside,
-                                                         const int *__restrict__ perm, int *__restrict__ vmint) {
+                                                         const int *__restrict__ perm, int *__restrict__ vmint,
+                                                         long long *__restrict__ vcospos) {
     int t = blockIdx.x * FB + threadIdx.x;
     if (t >= F) return;
     double n[3], p[3][3];
@@ -421,6 +423,8 @@ __global__ void __launch_bounds__(FB) vertex_cone_kernel(const float *__restrict
         const double *N = vn64 + 3 * (size_t)v;
         double c = ddot(n, N);
         atomicMin(&vcosq[v], (long long)floor(c * COSSCALE));
+        // ablation: the cone over the positive-pointing normals only
+        if (vcospos && c > 0.0) atomicMin(&vcospos[v], (long long)floor(c * COSSCALE));
         int bits = 0;
 #pragma unroll
         for (int q = 1; q <= 2; q++) {
@@ -439,6 +443,7 @@ __global__ void __launch_bounds__(FB) vertex_record_kernel(const float *__restri
                                                            const double *__restrict__ vn64,
                                                            const long long *__restrict__ vcosq,
                                                            const int *__restrict__ vside, int V,
+                                                           const long long *__restrict__ vcospos,
                                                            VertexRec *__restrict__ vrec, u64 *__restrict__ ctr) {
     __shared__ u32 s_cnt[5];
     if (threadIdx.x < 5) s_cnt[threadIdx.x] = 0;
@@ -460,7 +465,13 @@ __global__ void __launch_bounds__(FB) vertex_record_kernel(const float *__restri
         bool hemi = !(c > 0.0) || noaxis;     // ruff: normals span a half space or more
         float cf;
         if (noaxis) cf = -1.0f;               // whole sphere
-        else if (hemi) cf = 0.0f;             // hemisphere about the pseudonormal
+        else if (hemi && vcospos && vcospos[v] != 0x7F7F7F7F7F7F7F7Fll) {
+            // ablation: "a cone of positive pointing normals is sufficient in practice"
+            const double cp = (double)vcospos[v] * (1.0 / COSSCALE);
+            cf = (float)cp;
+            if ((double)cf > cp) cf = nextafterf(cf, -2.0f);
+            cf -= 2e-7f;
+        } else if (hemi) cf = 0.0f;           // hemisphere about the pseudonormal
         else {
             cf = (float)c;
             if ((double)cf > c) cf = nextafterf(cf, -2.0f);
@@ -634,7 +645,9 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     }
     u64 *vacc = nullptr;
     double *vn64 = nullptr;
-    long long *vcosq = nullptr;
+    long long *vcosq = nullptr, *vcospos = nullptr;
+    const char *rc = getenv("SDF_RUFF");
+    const bool ruff_cone = rc && !strcmp(rc, "cone");
     int *vside = nullptr;
     void *vslab = nullptr;
     for (int pass = 0; pass < 2; pass++) {
@@ -642,6 +655,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
         vacc = c.take<u64>(3 * (size_t)V);          // vacc and vside adjacent: one memset to 0
         vside = c.take<int>((size_t)V);
         vcosq = c.take<long long>((size_t)V);
+        if (ruff_cone) vcospos = c.take<long long>((size_t)V);     // right behind vcosq: one memset
         vn64 = c.take<double>(3 * (size_t)V);
         if (pass == 0) CKS(tmp.get(&vslab, c.off));
     }
@@ -660,10 +674,11 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     stage_mark(m, SDF_T_VERTICES, 0, st);
     // "larger than any value" initial states: 0x7F7F.. for the cone cosines and triangle ids
     CK(cudaMemsetAsync(vcosq, 0x7F, sizeof(long long) * (size_t)V, st));
+    if (vcospos) CK(cudaMemsetAsync(vcospos, 0x7F, sizeof(long long) * (size_t)V, st));
     CK(cudaMemsetAsync(m->vmint, 0x7F, sizeof(int) * (size_t)V, st));
     KL; vertex_normal_kernel<<<blocks_for(V), FB, 0, st>>>(vacc, V, vn64);
-    KL; vertex_cone_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, m->cvid, (int)F, vn64, vcosq, vside, m->perm, m->vmint);
-    KL; vertex_record_kernel<<<blocks_for(V), FB, 0, st>>>(m->soup, vcorner, vn64, vcosq, vside, V, m->vrec, m->d_ctr);
+    KL; vertex_cone_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, m->cvid, (int)F, vn64, vcosq, vside, m->perm, m->vmint, vcospos);
+    KL; vertex_record_kernel<<<blocks_for(V), FB, 0, st>>>(m->soup, vcorner, vn64, vcosq, vside, V, vcospos, m->vrec, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_VERTICES, 1, st);
     // second host crossing: validation flags + class counters

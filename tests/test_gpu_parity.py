@@ -63,6 +63,7 @@ def test_configs_reduced(oracle_mod, name, scale):
     (lambda: W.icosphere_mesh(2, 0.6), 18, 6),
     (lambda: W.torus_mesh(0.55, 0.25, 24, 12), 19, 4),
     (lambda: W.box_mesh((0.6, 0.5, 0.02)), 20, 4),        # plate thinner than the band
+    (lambda: W.spike_mesh(lean=1.2, height=0.3), 21, 5),  # two ruff vertices (cos_cone <= 0): hemispheres
 ])
 def test_unit_meshes(oracle_mod, maker, seed, band):
     """Convex / concave / saddle / ruff / pathological vertices, thin plate."""
@@ -195,6 +196,29 @@ def test_stl_file_to_grid_file(tmp_path):
     raw = open(tmp_path / "g.bin", "rb").read()
     n = d1.numel()
     assert np.array_equal(np.frombuffer(raw[44:44 + 4 * n], dtype=np.float32), d1.cpu().numpy().reshape(-1))
+
+
+def test_ruff_vertices_hemisphere_and_cone_variant(oracle_mod, monkeypatch):
+    """Ruff vertices (an incident normal at 90 degrees or more from the pseudonormal):
+    the default extrusion is the hemisphere; SDF_RUFF=cone selects the paper's
+    other choice, the cone over the positive-pointing normals ("sufficient in practice",
+    PAPER.md:410) -- on these meshes it leaves no gap and evaluates fewer pairs."""
+    from paper_1903_00353_b200 import binding as B
+    for lean, height, n, band in ((1.2, 0.3, 64, 8), (1.4, 0.25, 96, 12)):
+        w = _small(W.spike_mesh(lean=lean, height=height), 19, n=n, band_cells=band)
+        res = check_parity(w, oracle_mod)
+        _assert_ok(res)
+        assert res["stats"]["verts_hemisphere"] == 2
+        m = B.sdf_create(w.soup)
+        assert np.all(B.sdf_get_table(m, B.TABLE_VERTEX_REC)["cos_cone"][B.sdf_get_table(m, B.TABLE_VERTEX_REC)["info"] & 4 != 0] == 0.0)
+        monkeypatch.setenv("SDF_RUFF", "cone")
+        res_c = check_parity(w, oracle_mod)
+        m = B.sdf_create(w.soup)
+        vr = B.sdf_get_table(m, B.TABLE_VERTEX_REC)
+        monkeypatch.delenv("SDF_RUFF")
+        _assert_ok(res_c)
+        assert np.all(vr["cos_cone"][vr["info"] & 4 != 0] > 0.5)
+        assert res_c["stats"]["pairs_accepted"] < res["stats"]["pairs_accepted"]
 
 
 def test_serial_scheduler_ablation(oracle_mod, monkeypatch):

@@ -121,6 +121,7 @@ _TINY = {
     "saddle8": lambda: W.monkey_saddle_mesh(8, 0.5, 0.3, -0.5, 2),
     "ruff": lambda: W.ruff_mesh(),
     "spike": lambda: W.spike_mesh(),
+    "leanspike": lambda: W.spike_mesh(lean=1.2, height=0.3),    # two ruff vertices: cos_cone <= 0
     "plate": lambda: W.box_mesh((0.6, 0.5, 0.02)),          # thinner than the band
 }
 
@@ -331,6 +332,9 @@ def test_feature_counts_known_topology(oracle_mod):
     _, vclass, vcos = ruff.classes()
     apex = ruff.corner_vid()[np.all(ruff.soup == np.float32([0, 0, 0.3]), axis=2)][0]
     assert vclass[apex] == 1                                  # classified convex
+    v, t = W.spike_mesh(lean=1.2, height=0.3)
+    _, _, vcos = oracle_mod.Mesh(W.soup_from_indexed(v, t, None)).classes()
+    assert int((vcos <= 0).sum()) == 2                        # normals at 90 degrees or more from N_v
     v, t = W.config("C4", 0.05).soup, None
     star = oracle_mod.Mesh(v).counts
     assert star["V"] - star["E"] + star["F"] == 2
