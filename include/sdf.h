@@ -59,7 +59,8 @@ typedef struct sdf_allocator {
 /* Counters of the feature builder and of the last sdf_compute (host values). */
 typedef struct sdf_stats_t {
     int64_t F, V, E;                      /* triangles, welded vertices, undirected edges      */
-    int64_t edges_convex, edges_concave, edges_flat;      /* PAPER.md:352 discriminant         */
+    int64_t edges_convex, edges_concave, edges_flat;      /* PAPER.md:352 discriminant; knife   */
+                                          /* edges (n1 = -n2) count as convex                   */
     int64_t verts_pos_only, verts_neg_only, verts_both, verts_skipped; /* cone sides emitted   */
     int64_t verts_hemisphere;             /* "ruff" vertices: cos_cone <= 0 */
     int64_t weld_collisions;              /* reserved (always 0: the weld table probes, it has no runs) */

@@ -57,7 +57,7 @@ enum { SP_POLY = 0, SP_TESTED, SP_ACCEPTED, SP_ROWS };
 struct __align__(16) EdgeRec {
     float a[3], b[3], n1[3], n2[3];
     int tri;     // min(t0, t1): the id written for cells closest to this edge
-    int cls;     // +1 convex, -1 concave, 0 flat (no wedge)
+    int cls;     // +1 convex, -1 concave, 0 flat (no wedge), 2 knife (faces folded back: whole cylinder)
     int pad[2];
 };
 static_assert(sizeof(EdgeRec) == 64, "EdgeRec must be 64 B");

@@ -128,7 +128,14 @@ __device__ __forceinline__ bool poly_aabv(const MeshView &mv, const GridParams &
         // edge wedge: segment swept by the arc between n1 and n2, radius rb
         const EdgeRec &r = mv.erec[p - mv.F];
         emit = (r.cls != 0) && !g.aabb_mode;
-        if (emit) {
+        if (emit && r.cls == 2) {
+            // knife edge: the cylinder of radius rb about the segment
+#pragma unroll
+            for (int i = 0; i < 3; i++) {
+                mn[i] = fminf(r.a[i], r.b[i]) - rb - eps;
+                mx[i] = fmaxf(r.a[i], r.b[i]) + rb + eps;
+            }
+        } else if (emit) {
             // the wedge spans the arc n1 -> n2 on the outside of a convex edge and the arc
             // -n1 -> -n2 on the inside of a concave one
             const float sg = r.cls > 0 ? 1.0f : -1.0f;
@@ -332,7 +339,8 @@ __device__ __forceinline__ void build_record(const MeshView &mv, const GridParam
         const f3 a = ld3(r.a), ab = ld3(r.b) - a, n1 = ld3(r.n1), n2 = ld3(r.n2);
         const float L = sqrtf(dot(ab, ab));
         const f3 u = (1.0f / L) * ab;
-        const f3 w1 = cross(u, n1), w2 = cross(n2, u);
+        f3 w1 = cross(u, n1), w2 = cross(n2, u);
+        if (r.cls == 2) w1 = w2 = mk<float>(0.0f, 0.0f, 0.0f);        // knife edge: no side planes
         const f3 r0 = x0 - a;
         set_con(rec, 0, u, r0, -2.0f * eps, h);
         set_con(rec, 1, mk<float>(-u.x, -u.y, -u.z), r0, -(L + 2.0f * eps), h);
@@ -342,7 +350,7 @@ __device__ __forceinline__ void build_record(const MeshView &mv, const GridParam
         G[0] = a.x; G[1] = a.y; G[2] = a.z; G[3] = u.x; G[4] = u.y; G[5] = u.z; G[6] = L;
         G[7] = w1.x; G[8] = w1.y; G[9] = w1.z; G[10] = w2.x; G[11] = w2.y; G[12] = w2.z;
         ri[PR_ID] = r.tri;
-        ri[PR_TYPE] = 1 | (r.cls < 0 ? TY_NEG : 0) | (dot(n1, n2) < -0.99f ? TY_UNSURE : 0);
+        ri[PR_TYPE] = 1 | (r.cls < 0 ? TY_NEG : 0) | ((dot(n1, n2) < -0.99f || r.cls == 2) ? TY_UNSURE : 0);
         {
             const f3 nb = n1 + n2;
             const float il = rsqrtf(fmaxf(dot(nb, nb), 1e-30f));
@@ -538,11 +546,12 @@ __device__ __forceinline__ void build_row_record(const MeshView &mv, const GridP
         const f3 a = ld3(r.a), ab = ld3(r.b) - a, n1 = ld3(r.n1), n2 = ld3(r.n2);
         const float L = sqrtf(dot(ab, ab));
         const f3 u = (1.0f / L) * ab;
-        const f3 w1 = cross(u, n1), w2 = cross(n2, u);
+        f3 w1 = cross(u, n1), w2 = cross(n2, u);
+        if (r.cls == 2) w1 = w2 = mk<float>(0.0f, 0.0f, 0.0f);        // knife edge: no side planes
         rec[0] = a.x; rec[1] = a.y; rec[2] = a.z; rec[3] = u.x; rec[4] = u.y; rec[5] = u.z; rec[6] = L;
         rec[7] = w1.x; rec[8] = w1.y; rec[9] = w1.z; rec[10] = w2.x; rec[11] = w2.y; rec[12] = w2.z;
         ri[RR_ID] = r.tri;
-        ri[RR_TYPE] = 1 | (r.cls < 0 ? TY_NEG : 0) | (dot(n1, n2) < -0.99f ? TY_UNSURE : 0);
+        ri[RR_TYPE] = 1 | (r.cls < 0 ? TY_NEG : 0) | ((dot(n1, n2) < -0.99f || r.cls == 2) ? TY_UNSURE : 0);
         {
             const f3 nb = n1 + n2;
             const float il = rsqrtf(fmaxf(dot(nb, nb), 1e-30f));
@@ -728,11 +737,12 @@ __device__ __forceinline__ void process_direct(const MeshView &mv, const GridPar
         const f3 a = ld3(er.a), ab = ld3(er.b) - a, n1 = ld3(er.n1), n2 = ld3(er.n2);
         const float L = sqrtf(dot(ab, ab));
         const f3 u = (1.0f / L) * ab;
-        const f3 w1 = cross(u, n1), w2 = cross(n2, u);
+        f3 w1 = cross(u, n1), w2 = cross(n2, u);
+        if (er.cls == 2) w1 = w2 = mk<float>(0.0f, 0.0f, 0.0f);       // knife edge: no side planes
         f3 nbis = n1 + n2;
         nbis = rsqrtf(fmaxf(dot(nbis, nbis), 1e-30f)) * nbis;
         const int id = er.tri;
-        const u32 fl_rec = (er.cls < 0 ? FL_NEG : 0u) | (dot(n1, n2) < -0.99f ? 0u : FL_SURE);
+        const u32 fl_rec = (er.cls < 0 ? FL_NEG : 0u) | ((dot(n1, n2) < -0.99f || er.cls == 2) ? 0u : FL_SURE);
         const f3 r0 = mk<float>(fmaf((float)i0, h, g.ox) - a.x, fmaf((float)j0, h, g.oy) - a.y, fmaf((float)k0, h, g.oz) - a.z);
         const float ct = dot(u, r0), c1 = dot(w1, r0), c2 = dot(w2, r0);
         for (int dk = 0; dk < nk; dk++) {

@@ -349,12 +349,17 @@ __global__ void __launch_bounds__(FB) edge_record_kernel(const int *__restrict__
             // flat: the wedge is thinner than 1e-6 * band and lies inside the eps-inflated
             // neighbours (reading #5)
             int cls = d > 1e-6 ? 1 : (d < -1e-6 ? -1 : 0);
+            // sin(dihedral) also vanishes when the faces fold back onto each other (n1 = -n2: a
+            // blade or a slit).  That edge is as far from flat as an edge gets, and which side its
+            // wedge is on cannot be told from a vanishing discriminant: class 2, "knife", whose
+            // extrusion is the whole cylinder about the edge
+            if (cls == 0 && ddot(n1, n2) <= 0.0) cls = 2;
             const int x0 = perm[t0], x1 = perm[t1];      // the caller's triangle ids
             r.tri = x0 < x1 ? x0 : x1;
             r.cls = cls;
             r.pad[0] = r.pad[1] = 0;
             erec[e] = r;
-            atomicAdd(&s_cnt[cls > 0 ? 0 : (cls < 0 ? 1 : 2)], 1u);
+            atomicAdd(&s_cnt[cls > 0 ? 0 : (cls < 0 ? 1 : 2)], 1u);      // knife edges count as convex
         }
     }
     __syncthreads();

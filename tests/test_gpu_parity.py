@@ -221,6 +221,34 @@ def test_ruff_vertices_hemisphere_and_cone_variant(oracle_mod, monkeypatch):
         assert res_c["stats"]["pairs_accepted"] < res["stats"]["pairs_accepted"]
 
 
+def test_knife_edges(oracle_mod):
+    """Edges whose faces fold back onto each other (n1 = -n2): sin(dihedral) vanishes as it does for a
+    flat edge, but the edge needs the widest extrusion there is.  A two-triangle "pillow" (zero volume,
+    every edge a knife) and a blade (prism with an apex angle of 2.5e-8 rad).  The solids are thinner than
+    fp32 can resolve, so the sign is not defined; the populated set and |d| are, and must match."""
+    from paper_1903_00353_b200 import binding as B
+    tri = np.array([[0.1, 0.05, 0.02], [0.7, 0.1, 0.3], [0.2, 0.6, -0.1]], dtype=np.float32)
+    pillow = np.stack([tri, tri[::-1]]).astype(np.float32)
+    t_ = 1e-8
+    xs = np.array([[-0.4, 0.0], [0.4, t_], [0.4, -t_]])
+    v = np.array([[x, y, z] for z in (-0.3, 0.3) for x, y in xs])
+    tr = np.array([[0, 2, 1], [3, 4, 5], [0, 1, 4], [0, 4, 3], [1, 2, 5], [1, 5, 4], [2, 0, 3], [2, 3, 5]])
+    blade = W.soup_from_indexed(v, tr, np.random.default_rng(1))
+    origin, h, dims = W.grid_over((-1.0,) * 3, (1.0,) * 3, (48,) * 3)
+    for soup, knives in ((pillow, 3), (blade, 1)):
+        w = f32_grid(W.Workload("knife", soup, origin, h, dims, 4 * h))
+        om = oracle_mod.Mesh(w.soup)
+        d_ref, t_ref = om.sdf(w.origin, w.h, w.dims, w.band)
+        m, d, t, stats = run_gpu(w)
+        er = B.sdf_get_table(m, B.TABLE_EDGE_REC)
+        assert int((er["cls"] == 2).sum()) == knives
+        pop = np.isfinite(d)
+        assert np.array_equal(pop, np.isfinite(d_ref)) and pop.sum() > 1000
+        tol = 1e-5 * w.h + 1e-6 * w.diag
+        assert np.max(np.abs(np.abs(d[pop]).astype(np.float64) - np.abs(d_ref[pop]))) <= tol
+        assert np.all(t[pop] >= 0) and np.all(t[~pop] == -1)
+
+
 def test_serial_scheduler_ablation(oracle_mod, monkeypatch):
     """SDF_SCHEDULER=serial (the paper's thread-per-extrusion loop, kept as an ablation)
     meets the same four parity clauses, and agrees with the flattened scan converter to the last
