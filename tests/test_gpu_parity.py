@@ -221,6 +221,32 @@ def test_ruff_vertices_hemisphere_and_cone_variant(oracle_mod, monkeypatch):
         assert res_c["stats"]["pairs_accepted"] < res["stats"]["pairs_accepted"]
 
 
+def test_degenerate_shapes_and_grids(oracle_mod):
+    """Slivers of aspect 1e6, 1500 tiny tetrahedra (as many vertices as faces), a band of a twentieth
+    of a cell, grids of one slice, one row and one cell."""
+    rng = np.random.default_rng(7)
+    g48 = W.grid_over((-1.0,) * 3, (1.0,) * 3, (48,) * 3)
+    v, t = W.icosphere_mesh(2, 0.6)
+    nb = t[np.any(t == 0, axis=1)][0]
+    other = [x for x in nb if x != 0][0]
+    v2 = v.copy()
+    v2[0] = v2[other] + (v2[0] - v2[other]) * 1e-6 / np.linalg.norm(v2[0] - v2[other])
+    cases = [W.Workload("sliver", W.soup_from_indexed(v2, t, rng), *g48, 4 * g48[1])]
+    tv, tt = W.tetrahedron_mesh(0.03)
+    vs = [tv @ W.random_rotation(rng).T + rng.uniform(-0.9, 0.9, 3) for _ in range(1500)]
+    ts = [tt + 4 * k for k in range(1500)]
+    cases.append(W.Workload("tets", W.soup_from_indexed(np.concatenate(vs), np.concatenate(ts), rng),
+                            *W.grid_over((-1.0,) * 3, (1.0,) * 3, (96,) * 3), 3 * (2 / 96)))
+    ico = W.soup_from_indexed(v, t, rng)
+    cases.append(W.Workload("thinband", W.soup_from_indexed(*W.torus_mesh(0.5, 0.2, 24, 12), rng), *g48, 0.05 * g48[1]))
+    cases.append(W.Workload("slice_x", ico, (0.013, -1 + 1 / 48, -1 + 1 / 48), 2 / 48, (1, 48, 48), 0.2))
+    cases.append(W.Workload("slice_z", ico, (-1 + 1 / 48, -1 + 1 / 48, 0.21), 2 / 48, (48, 48, 1), 0.2))
+    cases.append(W.Workload("row", ico, (-1 + 1 / 48, 0.1, 0.05), 2 / 48, (48, 1, 1), 0.2))
+    cases.append(W.Workload("cell", ico, (0.55, 0.1, 0.05), 2 / 48, (1, 1, 1), 0.2))
+    for w in cases:
+        _assert_ok(check_parity(w, oracle_mod))
+
+
 def test_knife_edges(oracle_mod):
     """Edges whose faces fold back onto each other (n1 = -n2): sin(dihedral) vanishes as it does for a
     flat edge, but the edge needs the widest extrusion there is.  A two-triangle "pillow" (zero volume,
