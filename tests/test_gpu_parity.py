@@ -243,6 +243,17 @@ def test_degenerate_shapes_and_grids(oracle_mod):
     cases.append(W.Workload("slice_z", ico, (-1 + 1 / 48, -1 + 1 / 48, 0.21), 2 / 48, (48, 48, 1), 0.2))
     cases.append(W.Workload("row", ico, (-1 + 1 / 48, 0.1, 0.05), 2 / 48, (48, 1, 1), 0.2))
     cases.append(W.Workload("cell", ico, (0.55, 0.1, 0.05), 2 / 48, (1, 1, 1), 0.2))
+    # crumpled sphere: hundreds of saddle, concave and ruff vertices
+    g64 = W.grid_over((-1.0,) * 3, (1.0,) * 3, (64,) * 3)
+    v3, t3 = W.icosphere_mesh(3, 0.6)
+    cases.append(W.Workload("crumpled", W.soup_from_indexed(v3 * (1 + 0.2 * rng.standard_normal(len(v3)))[:, None], t3, rng),
+                            *g64, 6 * g64[1]))
+    # funnel: a concave vertex of valence 500
+    n = 500
+    phi = 2 * np.pi * np.arange(n) / n
+    vf = np.concatenate([np.stack([0.6 * np.cos(phi), 0.6 * np.sin(phi), np.zeros(n)], 1), [[0, 0, -0.2]], [[0, 0, -0.6]]])
+    tf = np.array([[k, (k + 1) % n, n] for k in range(n)] + [[(k + 1) % n, k, n + 1] for k in range(n)])
+    cases.append(W.Workload("funnel", W.soup_from_indexed(vf, tf, rng), *g64, 5 * g64[1]))
     for w in cases:
         _assert_ok(check_parity(w, oracle_mod))
 
