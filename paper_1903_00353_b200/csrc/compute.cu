@@ -262,16 +262,16 @@ struct BrickOut {
 // ---------------------------------------------------------------------------------------
 // A6 + A7: scan conversion and evaluation.
 //
-// A polyhedron is turned into a 40-word record in shared memory: five row-clip constraints
-// (a convex body meets a grid row in one interval, so each half-space s(i,j,k) = A + gx*di +
-// gy*dj + gz*dk >= 0 clips the row's x-span analytically), the geometry the
-// per-cell tests and distances need, the triangle id and the AABV.  Work is flattened
-// WITHIN A WARP: lane l owns polyhedron 32*warp + l, the row counts are prefix-summed across
-// the lanes, and the warp then walks the flattened (polyhedron, row) list 32 rows at a time
-// -- the load balancing of PAPER.md:376-380 (dynamic parallelism) without child launches,
-// without a global work-item list and without a device-wide scan.  Polyhedra with many or
-// long rows are listed by evaluate_small_kernel and taken by evaluate_big_kernel, one block per
-// polyhedron with the lanes along x.
+// A polyhedron is turned into a 29-word record in shared memory: its planes in the form the row
+// walk needs (a convex body meets a grid row in one interval, and along the row every half-space
+// test s = base + di * g is linear in the cell index), the triangle id, the sign
+// flags and the AABV.  Work is flattened WITHIN A WARP: lane l owns polyhedron 32*warp + l, the
+// row counts are prefix-summed across the lanes, and the warp then walks the flattened
+// (polyhedron, row) list 32 rows at a time -- the load balancing of PAPER.md:376-380 (dynamic
+// parallelism) without child launches, without a global work-item list and without a device-wide
+// scan.  Polyhedra with many or long rows are listed by evaluate_small_kernel and taken by
+// evaluate_big_kernel, one block per polyhedron: a thread per row when there are many rows, a
+// warp per row with the lanes along x when there are few long ones.
 // ---------------------------------------------------------------------------------------
 // Sign carried with the candidate (the polarity of the winning extrusion).  A face
 // prism knows the side from n.r, a wedge from its class, a cone from its side; FL_SURE says the
@@ -283,101 +283,6 @@ struct BrickOut {
 #define TY_NEG 16        // record type word: bit 4 = interior side, bit 5 = never sure
 #define TY_UNSURE 32
 
-#define PR_GEO 20        // 13 geometry floats
-#define PR_ID 33
-#define PR_TYPE 34
-#define PR_I0 35
-#define PR_NI 36         // i1 - i0
-#define PR_J0 37
-#define PR_NJ 38         // j1 - j0 + 1
-#define PR_K0 39
-#define PR_NB 40         // wedges: unit bisector of n1, n2 (3 floats)
-#define PR_WORDS 45      // odd stride: records of different owners fall in different banks
-
-__device__ __forceinline__ void set_con(float *rec, int c, f3 m, f3 r0, float lim, float h) {
-    const float gx = h * m.x;
-    rec[4 * c + 0] = dot(m, r0) - lim;                 // s >= lim at the AABV corner cell
-    rec[4 * c + 1] = h * m.y;
-    rec[4 * c + 2] = h * m.z;
-    rec[4 * c + 3] = gx != 0.0f ? 1.0f / gx : 0.0f;    // 0: the constraint does not depend on x
-}
-__device__ __forceinline__ void no_con(float *rec, int c) {
-    rec[4 * c + 0] = 1.0f; rec[4 * c + 1] = 0.0f; rec[4 * c + 2] = 0.0f; rec[4 * c + 3] = 0.0f;
-}
-
-// A5: the polyhedron of feature p, clipped to the band, as a record
-__device__ __forceinline__ void build_record(const MeshView &mv, const GridParams &g, int64_t p, const PolyHdr &H,
-                                             float *rec) {
-    const float h = g.h, eps = g.eps, reach = g.band + g.guard;
-    const f3 x0 = mk<float>(fmaf((float)H.i0, h, g.ox), fmaf((float)H.j0, h, g.oy), fmaf((float)H.k0, h, g.oz));
-    int *ri = (int *)rec;
-    float *G = rec + PR_GEO;
-    if (p < mv.F) {
-        // face slab: three inward side planes through the edges + the slab
-        const float *T = mv.soup + 9 * p, *N = mv.fn + 3 * p;
-        const f3 a = ld3(T), e0 = ld3(T + 3) - a, ec = ld3(T + 6) - a, n = ld3(N);
-        const f3 r0 = x0 - a;
-        if (!g.aabb_mode) {
-            const f3 e1 = ec - e0;
-            const f3 m0 = cross(n, e0), m1 = cross(n, e1), m2 = cross(ec, n);          // inward, |m_i| = |edge_i|
-            const float t0 = eps * sqrtf(dot(e0, e0)), t1 = eps * sqrtf(dot(e1, e1)), t2 = eps * sqrtf(dot(ec, ec));
-            set_con(rec, 0, m0, r0, -2.0f * t0, h);
-            set_con(rec, 1, m1, r0 - e0, -2.0f * t1, h);
-            set_con(rec, 2, m2, r0 - ec, -2.0f * t2, h);
-            set_con(rec, 3, n, r0, -(reach + eps), h);
-            set_con(rec, 4, mk<float>(-n.x, -n.y, -n.z), r0, -(reach + eps), h);
-        } else {
-#pragma unroll
-            for (int c = 0; c < 5; c++) no_con(rec, c);
-        }
-        G[0] = a.x; G[1] = a.y; G[2] = a.z; G[3] = e0.x; G[4] = e0.y; G[5] = e0.z;
-        G[6] = ec.x; G[7] = ec.y; G[8] = ec.z; G[9] = n.x; G[10] = n.y; G[11] = n.z; G[12] = 0.0f;
-        ri[PR_ID] = mv.perm[p]; ri[PR_TYPE] = 0;
-    } else if (p < (int64_t)mv.F + mv.E) {
-        // edge wedge: beyond both faces' side planes, between the end caps
-        const EdgeRec &r = mv.erec[p - mv.F];
-        const f3 a = ld3(r.a), ab = ld3(r.b) - a, n1 = ld3(r.n1), n2 = ld3(r.n2);
-        const float L = sqrtf(dot(ab, ab));
-        const f3 u = (1.0f / L) * ab;
-        f3 w1 = cross(u, n1), w2 = cross(n2, u);
-        if (r.cls == 2) w1 = w2 = mk<float>(0.0f, 0.0f, 0.0f);        // knife edge: no side planes
-        const f3 r0 = x0 - a;
-        set_con(rec, 0, u, r0, -2.0f * eps, h);
-        set_con(rec, 1, mk<float>(-u.x, -u.y, -u.z), r0, -(L + 2.0f * eps), h);
-        set_con(rec, 2, w1, r0, -2.0f * eps, h);
-        set_con(rec, 3, w2, r0, -2.0f * eps, h);
-        no_con(rec, 4);
-        G[0] = a.x; G[1] = a.y; G[2] = a.z; G[3] = u.x; G[4] = u.y; G[5] = u.z; G[6] = L;
-        G[7] = w1.x; G[8] = w1.y; G[9] = w1.z; G[10] = w2.x; G[11] = w2.y; G[12] = w2.z;
-        ri[PR_ID] = r.tri;
-        ri[PR_TYPE] = 1 | (r.cls < 0 ? TY_NEG : 0) | ((dot(n1, n2) < -0.99f || r.cls == 2) ? TY_UNSURE : 0);
-        {
-            const f3 nb = n1 + n2;
-            const float il = rsqrtf(fmaxf(dot(nb, nb), 1e-30f));
-            rec[PR_NB] = il * nb.x; rec[PR_NB + 1] = il * nb.y; rec[PR_NB + 2] = il * nb.z;
-        }
-    } else {
-        // vertex cone / hemisphere (eq.10, 362-364) inside the ball of radius reach
-        const int64_t q = p - mv.F - mv.E;
-        const VertexRec &r = mv.vrec[q >> 1];
-        const float sg = (q & 1) ? -1.0f : 1.0f;
-        const f3 v = ld3(r.pos), A = sg * ld3(r.axis);
-        const float c = r.cos_cone;
-        // a cone of half angle <= 90 degrees lies in the half space A.(x - v) >= 0
-        if (c >= 0.0f) set_con(rec, 0, A, x0 - v, -2.0f * eps, h); else no_con(rec, 0);
-#pragma unroll
-        for (int k = 1; k < 5; k++) no_con(rec, k);
-        G[0] = v.x; G[1] = v.y; G[2] = v.z; G[3] = A.x; G[4] = A.y; G[5] = A.z; G[6] = c;
-#pragma unroll
-        for (int k = 7; k < 13; k++) G[k] = 0.0f;
-        ri[PR_ID] = mv.vmint[q >> 1];
-        ri[PR_TYPE] = 2 | ((q & 1) ? TY_NEG : 0) | (c <= -1.0f ? TY_UNSURE : 0);
-    }
-    ri[PR_I0] = H.i0; ri[PR_NI] = H.i1 - H.i0;
-    ri[PR_J0] = H.j0; ri[PR_NJ] = H.j1 - H.j0 + 1;
-    ri[PR_K0] = H.k0;
-}
-
 // a distance this small against the operands it was differenced from has no reliable sign in fp32
 __device__ __forceinline__ bool tiny_vs(float d, f3 r) { return d <= 1e-5f * (fabsf(r.x) + fabsf(r.y) + fabsf(r.z)); }
 
@@ -388,105 +293,6 @@ __device__ __forceinline__ void put_min(const GridParams &g, const int *__restri
     u64 *cell = scratch + (size_t)slot * BRICK_CELLS + (((k & 7) * 8 + (j & 7)) * 8 + (i & 7));
     // low word: id, then FL_SURE, then FL_NEG -- among equal (d, id) an unsure entry wins
     atomicMin(cell, ((u64)__float_as_uint(d) << 32) | ((u32)id << 2) | fl);
-}
-
-// One grid row (j,k) of one polyhedron: clip the x-span, then test and evaluate its cells
-// i = ia + lane0, ia + lane0 + STRIDE, ...  (STRIDE 1: a lane owns the row; 32: a warp does).
-template <int STRIDE>
-__device__ __forceinline__ void process_row(const GridParams &g, const float *rec, u32 row, int lane0,
-                                            const int *__restrict__ table, u64 *__restrict__ scratch, u32 &tested,
-                                            u32 &accepted) {
-    const int *ri = (const int *)rec;
-    const int nj = ri[PR_NJ];
-    const int dk = (int)(row / (u32)nj), dj = (int)(row - (u32)dk * (u32)nj);
-    const int i0 = ri[PR_I0], tyw = ri[PR_TYPE], type = tyw & 15;
-    const u32 fl_rec = ((tyw & TY_NEG) ? FL_NEG : 0u) | ((tyw & TY_UNSURE) ? 0u : FL_SURE);
-    const float fj = (float)dj, fk = (float)dk;
-    float tlo = 0.0f, thi = (float)ri[PR_NI];
-    bool empty = false;
-#pragma unroll
-    for (int c = 0; c < 5; c++) {
-        const float s = fmaf(rec[4 * c + 2], fk, fmaf(rec[4 * c + 1], fj, rec[4 * c]));
-        const float inv = rec[4 * c + 3], t = -s * inv;
-        if (inv > 0.0f) tlo = fmaxf(tlo, t);
-        else if (inv < 0.0f) thi = fminf(thi, t);
-        else if (s < 0.0f) empty = true;
-    }
-    const int j = ri[PR_J0] + dj, k = ri[PR_K0] + dk;
-    const float h = g.h, eps = g.eps;
-    const float y = fmaf((float)j, h, g.oy), z = fmaf((float)k, h, g.oz);
-    const float reach = g.band + g.guard;          // accept d < reach; the emit pass decides exactly
-    const float *G = rec + PR_GEO;
-    if (type == 2) {
-        // ball of radius reach about the vertex
-        const float ry = y - G[1], rz = z - G[2];
-        const float rem = reach * reach - ry * ry - rz * rz;
-        if (rem < 0.0f) return;
-        const float xr = sqrtf(rem), inv_h = 1.0f / h, x0 = fmaf((float)i0, h, g.ox);
-        tlo = fmaxf(tlo, (G[0] - xr - x0) * inv_h - 1e-2f);
-        thi = fminf(thi, (G[0] + xr - x0) * inv_h + 1e-2f);
-    }
-    if (empty || !(tlo <= thi)) return;
-    const int ia = i0 + (int)ceilf(tlo), ib = i0 + (int)floorf(thi);
-    if (ia + lane0 > ib) return;
-    const int id = ri[PR_ID];
-    if (type == 0) {
-        const f3 a = ld3(G), e0 = ld3(G + 3), ec = ld3(G + 6), n = ld3(G + 9);
-        const f3 e1 = ec - e0;
-        const f3 m0 = cross(n, e0), m1 = cross(n, e1), m2 = cross(ec, n);
-        const float t0 = eps * sqrtf(dot(e0, e0)), t1 = eps * sqrtf(dot(e1, e1)), t2 = eps * sqrtf(dot(ec, ec));
-        const float ry = y - a.y, rz = z - a.z;
-        for (int i = ia + lane0; i <= ib; i += STRIDE) {
-            const f3 r = mk<float>(fmaf((float)i, h, g.ox) - a.x, ry, rz);
-            tested++;
-            float d;
-            u32 fl = 0;
-            if (g.aabb_mode) {
-                int rg; f3 q;
-                d = tri_closest<float>(r, e0, ec, n, rg, q);
-            } else {
-                const float s0 = dot(m0, r), s1 = dot(m1, r - e0), s2 = dot(m2, r - ec);
-                if (s0 < -t0 || s1 < -t1 || s2 < -t2) continue;
-                if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f) {
-                    const float dn = dot_rn(n, r);
-                    d = fabsf(dn);
-                    fl = (tiny_vs(d, r) ? 0u : FL_SURE) | (dn < 0.0f ? FL_NEG : 0u);
-                } else { int rg; f3 q; d = tri_closest<float>(r, e0, ec, n, rg, q); }   // eps margin: exact clamped distance
-            }
-            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id, fl); }
-        }
-    } else if (type == 1) {
-        const f3 a = ld3(G), u = ld3(G + 3), w1 = ld3(G + 7), w2 = ld3(G + 10), nbis = ld3(rec + PR_NB);
-        const float L = G[6];
-        const float ry = y - a.y, rz = z - a.z;
-        for (int i = ia + lane0; i <= ib; i += STRIDE) {
-            const f3 r = mk<float>(fmaf((float)i, h, g.ox) - a.x, ry, rz);
-            tested++;
-            const float t = dot(u, r);
-            if (t < -eps || t > L + eps || dot(w1, r) < -eps || dot(w2, r) < -eps) continue;
-            const float tu = dot_rn(u, r), tc = fminf(fmaxf(tu, 0.0f), L);
-            const f3 q = mk<float>(__fmaf_rn(-tc, u.x, r.x), __fmaf_rn(-tc, u.y, r.y), __fmaf_rn(-tc, u.z, r.z));
-            const float d = __fsqrt_rn(dot_rn(q, q));
-            // the end caps belong to the end vertices, and the eps slack of a nearly flat wedge
-            // reaches through the surface: the class gives the sign only where the bisector agrees
-            const float sb = (fl_rec & FL_NEG) ? -dot(nbis, q) : dot(nbis, q);
-            const u32 fl = (tu > 0.0f && tu < L && sb > 1e-2f * d && !tiny_vs(d, r)) ? fl_rec : (fl_rec & FL_NEG);
-            if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id, fl); }
-        }
-    } else {
-        const f3 v = ld3(G), A = ld3(G + 3);
-        const float c = G[6];
-        const float ry = y - v.y, rz = z - v.z;
-        for (int i = ia + lane0; i <= ib; i += STRIDE) {
-            const f3 r = mk<float>(fmaf((float)i, h, g.ox) - v.x, ry, rz);
-            tested++;
-            const float d = __fsqrt_rn(dot_rn(r, r)), ar = dot(A, r);
-            if (d >= reach || ar < c * d - eps) continue;
-            accepted++;
-            // near the plane through the vertex normal to the axis the side is not decided here
-            put_min(g, table, scratch, i, j, k, d, id, ar > 1e-2f * d ? fl_rec : (fl_rec & FL_NEG));
-        }
-    }
 }
 
 __device__ __forceinline__ void add_stats(u64 *__restrict__ ctr, u32 tested, u32 accepted, u32 rows) {
@@ -580,13 +386,16 @@ __device__ __forceinline__ void clip_lin(float base, float gx, float tol, float 
     else if (num > 0.0f) hi = -1.0f;
 }
 
+// STRIDE 1: a lane owns the row (small polyhedra); STRIDE 32: a warp does, lane0 = its lane (big ones)
+template <int STRIDE, bool EXACT_DIV>
 __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridParams &g, const float *rec, int row,
-                                                const int *__restrict__ table, u64 *__restrict__ scratch,
+                                                int lane0, const int *__restrict__ table, u64 *__restrict__ scratch,
                                                 u32 &tested, u32 &accepted) {
     const int *ri = (const int *)rec;
     const int nj = ri[RR_NJ], ni = ri[RR_NI], i0 = ri[RR_I0], tyw = ri[RR_TYPE], type = tyw & 15, id = ri[RR_ID];
     const u32 fl_rec = ((tyw & TY_NEG) ? FL_NEG : 0u) | ((tyw & TY_UNSURE) ? 0u : FL_SURE);
-    const int dk = (int)(((float)row + 0.5f) * rec[RR_INV_NJ]);
+    // rows of a small polyhedron (<= 256) divide exactly through the fp32 reciprocal
+    const int dk = EXACT_DIV ? row / nj : (int)(((float)row + 0.5f) * rec[RR_INV_NJ]);
     const int j = ri[RR_J0] + row - dk * nj, k = ri[RR_K0] + dk;
     const float h = g.h, eps = g.eps, reach = g.band + g.guard;      // accept d < reach; the emit pass decides exactly
     const float ry = __fsub_rn(fmaf((float)j, h, g.oy), rec[1]), rz = __fsub_rn(fmaf((float)k, h, g.oz), rec[2]);
@@ -599,23 +408,24 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
         const float b1 = fmaf(m1.x, rx0, fmaf(m1.y, ry, m1.z * rz)) - rec[15], g1 = m1.x * h;
         const float b2 = fmaf(m2.x, rx0, fmaf(m2.y, ry, m2.z * rz)) - rec[16], g2 = m2.x * h;
         const float bn = fmaf(n.x, rx0, fmaf(n.y, ry, n.z * rz)), gn = n.x * h;
-        if (ni > ROW_CLIP_NI) {
+        if (ni > ROW_CLIP_NI && !g.aabb_mode) {
             float lo = 0.0f, hi = (float)db;
             clip_lin(b0, g0, t0, lo, hi); clip_lin(b1, g1, t1, lo, hi); clip_lin(b2, g2, t2, lo, hi);
             clip_lin(bn, gn, reach, lo, hi); clip_lin(-bn, -gn, reach, lo, hi);
             if (!(lo <= hi)) return;
             da = (int)ceilf(lo); db = (int)floorf(hi);
         }
-        for (int di = da; di <= db; di++) {
+        for (int di = da + lane0; di <= db; di += STRIDE) {
             const float fd = (float)di;
             const float s0 = fmaf(fd, g0, b0), s1 = fmaf(fd, g1, b1), s2 = fmaf(fd, g2, b2), dn = fmaf(fd, gn, bn);
             tested++;
-            if (s0 < -t0 || s1 < -t1 || s2 < -t2 || fabsf(dn) >= reach + eps) continue;
+            // debug mode "AABB candidates": every cell of the band-expanded box gets the clamped distance
+            if (!g.aabb_mode && (s0 < -t0 || s1 < -t1 || s2 < -t2 || fabsf(dn) >= reach + eps)) continue;
             const int i = i0 + di;
             const f3 r = mk<float>(__fsub_rn(fmaf((float)i, h, g.ox), rec[0]), ry, rz);
             float d;
             u32 fl = 0;
-            if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f) {
+            if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f && !g.aabb_mode) {
                 const float dnc = dot_rn(n, r);
                 d = fabsf(dnc);
                 fl = (tiny_vs(d, r) ? 0u : FL_SURE) | (dnc < 0.0f ? FL_NEG : 0u);
@@ -641,7 +451,7 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
             if (!(lo <= hi)) return;
             da = (int)ceilf(lo); db = (int)floorf(hi);
         }
-        for (int di = da; di <= db; di++) {
+        for (int di = da + lane0; di <= db; di += STRIDE) {
             const float fd = (float)di;
             const float t = fmaf(fd, gt, bt);
             tested++;
@@ -670,7 +480,7 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
         if (c >= 0.0f) clip_lin(ba, ga, 2.0f * eps, lo, hi);
         if (!(lo <= hi)) return;
         da = (int)ceilf(lo); db = (int)floorf(hi);
-        for (int di = da; di <= db; di++) {
+        for (int di = da + lane0; di <= db; di += STRIDE) {
             const int i = i0 + di;
             const f3 r = mk<float>(__fsub_rn(fmaf((float)i, h, g.ox), rec[0]), ry, rz);
             tested++;
@@ -849,7 +659,7 @@ __global__ void __launch_bounds__(32 * ES_WARPS, SERIAL ? 1 : ES_MINB) evaluate_
 #pragma unroll
             for (int st = 16; st; st >>= 1)
                 if (s_ex[w][o + st] <= r) o += st;
-            process_row_inc(mv, g, s_rec[w][o], r - s_ex[w][o], table, scratch, tested, accepted);
+            process_row_inc<1, false>(mv, g, s_rec[w][o], r - s_ex[w][o], 0, table, scratch, tested, accepted);
         }
     }
     add_stats(ctr, tested, accepted, (u32)rows + rows_direct);
@@ -857,12 +667,13 @@ __global__ void __launch_bounds__(32 * ES_WARPS, SERIAL ? 1 : ES_MINB) evaluate_
 
 // One block per big polyhedron (dynamic fetch): warps stride over its rows, lanes over x.
 #define EBIG_BT 256
+#define EBIG_THREAD_ROWS 128      // a big polyhedron with at least this many rows is walked a thread per row
 #define EBIG_SPLIT 8             // row slices per big polyhedron when the mesh has few polyhedra
 __global__ void __launch_bounds__(EBIG_BT) evaluate_big_kernel(MeshView mv, GridParams g,
                                                                const u32 *__restrict__ big_list,
                                                                const int *__restrict__ table,
                                                                u64 *__restrict__ scratch, u64 *__restrict__ ctr) {
-    __shared__ float s_rec[PR_WORDS];
+    __shared__ float s_rec[RR_WORDS];
     __shared__ u64 s_e;
     __shared__ u32 s_rows;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -880,13 +691,20 @@ __global__ void __launch_bounds__(EBIG_BT) evaluate_big_kernel(MeshView mv, Grid
             const int64_t p = (int64_t)big_list[e];
             PolyHdr H;
             poly_aabv(mv, g, p, H);
-            build_record(mv, g, p, H, s_rec);
+            build_row_record(mv, g, p, H, s_rec);
             s_rows = H.rows;
         }
         __syncthreads();
         const u32 rows = s_rows;
-        for (u32 r = blockIdx.y * (EBIG_BT / 32) + (u32)w; r < rows; r += gridDim.y * (EBIG_BT / 32))
-            process_row<32>(g, s_rec, r, lane, table, scratch, tested, accepted);
+        if (rows >= EBIG_THREAD_ROWS) {
+            // many rows: a thread per row (the row set-up is paid once per row, not once per lane)
+            for (u32 r = blockIdx.y * EBIG_BT + threadIdx.x; r < rows; r += gridDim.y * EBIG_BT)
+                process_row_inc<1, true>(mv, g, s_rec, (int)r, 0, table, scratch, tested, accepted);
+        } else {
+            // few, long rows: a warp per row, lanes along x
+            for (u32 r = blockIdx.y * (EBIG_BT / 32) + (u32)w; r < rows; r += gridDim.y * (EBIG_BT / 32))
+                process_row_inc<32, true>(mv, g, s_rec, (int)r, lane, table, scratch, tested, accepted);
+        }
         if (threadIdx.x == 0 && blockIdx.y == 0) rows_done += rows;
     }
     add_stats(ctr, tested, accepted, rows_done);
@@ -1234,11 +1052,13 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
     CK(cudaMemcpyAsync(&bricks, m->d_ctr + CTR_BRICKS, sizeof(bricks), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     stage_mark(m, SDF_T_CLIP_SCAN, 1, st);
+    // fork the fill first: its CTAs claim their SMs while the GPU is still empty (the scratch
+    // allocation and its clear come next), before the evaluate blocks flood it
+    if (g.fill_mode == 4) CKS(fork_fill());
     CKS(ensure(m, &m->scratch, &m->scratch_cap, (size_t)(bricks ? bricks : 1) * BRICK_CELLS, st));
     stage_mark(m, SDF_T_CLEAR, 0, st);
     if (bricks) CK(cudaMemsetAsync(m->scratch, 0xFF, (size_t)bricks * BRICK_CELLS * sizeof(u64), st));
     stage_mark(m, SDF_T_CLEAR, 1, st);
-    if (g.fill_mode == 4) CKS(fork_fill());
 
     // A5 + A6b + A7: clip every polyhedron, flatten the small ones per warp and evaluate them;
     // big ones one block each (dynamic fetch)
