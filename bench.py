@@ -37,8 +37,8 @@ from paper_1903_00353_b200 import workloads as W  # noqa: E402
 METRIC = "narrow_band_sdf_cells_per_s"
 UNIT = "band cells/s"
 L2_BYTES = 126 * 1024 * 1024
-# dram__bytes_read.sum + dram__bytes_write.sum of fill_tma_kernel at C4 (profiles/r1z_ncu_full.md)
-NCU_FILL_TRAFFIC_C4 = 0.012288e6 + 8.529719e9
+# dram__bytes_read.sum + dram__bytes_write.sum of fill_tma_kernel at C4 (profiles/r1_final_ncu_full.md)
+NCU_FILL_TRAFFIC_C4 = 0.024320e6 + 8.530644e9
 
 
 # --------------------------------------------------------------------------------------- #
@@ -384,7 +384,7 @@ def main():
     ap.add_argument("--ref-slices", type=int, default=64, help="z-slices per step of --impl reference")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes (read + write) per launch of the dominant kernel from the committed "
-                         "ncu --set full capture; default: the C4 figure of profiles/r1z_ncu_full.md")
+                         "ncu --set full capture; default: the C4 figure of profiles/r1_final_ncu_full.md")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
