@@ -254,6 +254,21 @@ def test_degenerate_shapes_and_grids(oracle_mod):
     vf = np.concatenate([np.stack([0.6 * np.cos(phi), 0.6 * np.sin(phi), np.zeros(n)], 1), [[0, 0, -0.2]], [[0, 0, -0.6]]])
     tf = np.array([[k, (k + 1) % n, n] for k in range(n)] + [[(k + 1) % n, k, n + 1] for k in range(n)])
     cases.append(W.Workload("funnel", W.soup_from_indexed(vf, tf, rng), *g64, 5 * g64[1]))
+    # hourglass: two pyramids apex to apex (a pinched, non-manifold vertex; every edge still manifold)
+    def pyramid(base_z, s):
+        b = np.array([[-s, -s, base_z], [s, -s, base_z], [s, s, base_z], [-s, s, base_z], [0.0, 0.0, 0.0]])
+        tt_ = np.array([[k, (k + 1) % 4, 4] for k in range(4)] + [[0, 2, 1], [0, 3, 2]])
+        return b, (tt_ if base_z < 0 else tt_[:, ::-1])
+    (va, ta), (vb, tb) = pyramid(-0.6, 0.5), pyramid(0.6, 0.4)
+    cases.append(W.Workload("hourglass", W.soup_from_indexed(np.concatenate([va, vb]), np.concatenate([ta, tb + 5]), rng),
+                            *g64, 5 * g64[1]))
+    # inside-out box: a cavity in an infinite solid (all edges and vertices concave)
+    vbx, tbx = W.box_mesh((0.5, 0.4, 0.3))
+    cases.append(W.Workload("insideout", W.soup_from_indexed(vbx, tbx[:, ::-1], rng), *g64, 5 * g64[1]))
+    # sea urchin: twenty vertices of a small icosphere pulled far out
+    vu, tu = W.icosphere_mesh(2, 0.3)
+    vu[rng.choice(len(vu), 20, replace=False)] *= 2.8
+    cases.append(W.Workload("urchin", W.soup_from_indexed(vu, tu, rng), *g64, 6 * g64[1]))
     for w in cases:
         _assert_ok(check_parity(w, oracle_mod))
 
