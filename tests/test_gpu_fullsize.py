@@ -70,3 +70,25 @@ def test_full_size_slabs(oracle_mod, name, slabs):
         assert res["ok"] and all(res[k] == 0 for k in KEYS), (k0, {k: v for k, v in res.items()})
         checked += res["populated_ref"]
     assert checked > 0
+
+
+def test_scale_36m_triangles():
+    """Nine times C4's triangle count (the same star surface on a 6000 x 3000 UV mesh, 1.3 GB of soup):
+    index arithmetic and table sizing beyond the configs.  No oracle at this size: generator-known
+    topology, whole-grid properties, and the band itself -- the surface is C4's, so is the band."""
+    from paper_1903_00353_b200 import binding as B
+    rng = np.random.default_rng(1004)
+    v, t = W.uv_star_mesh(nphi=6000, ntheta=3000, rng=rng)
+    soup = W.soup_from_indexed(v, t, rng)
+    F = soup.shape[0]
+    assert F == 35_988_000
+    origin, h, dims = W.grid_over((-1.0,) * 3, (1.0,) * 3, (1024,) * 3)
+    w = f32_grid(W.Workload("star36m", soup, origin, h, dims, 2 * h))
+    m = B.sdf_create(torch.from_numpy(soup).cuda())
+    d, tr = B.sdf_compute(m, w.origin, w.h, w.dims, w.band)
+    torch.cuda.synchronize()
+    st = B.sdf_stats(m)
+    assert (st["F"], st["V"], st["E"]) == (F, v.shape[0], 3 * F // 2) and st["V"] - st["E"] + st["F"] == 2
+    assert st["edges_convex"] + st["edges_concave"] + st["edges_flat"] == st["E"]
+    _whole_grid_properties(w, d, tr, st)
+    assert abs(st["band_cells"] - 5_186_000) < 2_000          # C4's surface, C4's band
