@@ -19,6 +19,12 @@
  * Every function returns an int status (0 = SDF_OK); none throws, aborts or prints.
  * The library never falls back to a CPU implementation: without a CUDA device every
  * compute entry point returns SDF_ECUDA.
+ * Threading: calls on one handle must not overlap, and neither may calls that create library-wide
+ * state for the first time (the first sdf_compute of a process creates the side stream of the
+ * sentinel fill); distinct handles on distinct streams are otherwise independent.
+ * Debug / ablation switches (environment, read per call): SDF_AABB_MODE=1 (candidates = band-expanded
+ * triangle boxes only), SDF_FILL_MODE=0..4, SDF_SCHEDULER=serial, SDF_RUFF=cone, SDF_NO_BINNING=1;
+ * see DESIGN.md.
  */
 #ifndef PAPER_1903_00353_SDF_H
 #define PAPER_1903_00353_SDF_H
