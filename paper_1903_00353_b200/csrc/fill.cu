@@ -25,13 +25,18 @@ __device__ __forceinline__ int state_from_right(unsigned set, unsigned neg, int 
 }
 
 #define SX_BATCH 8       // chunks of 32 cells loaded before they are resolved (memory-level parallelism)
+// One walk per row (see sweep_line_kernel for why one is enough).  A chunk of 32 cells is resolved
+// with two ballots: an unset cell is filled if the nearest set cell to its left (in the chunk, else
+// the carry) or to its right IN THE CHUNK is negative; unset cells with no set cell to their right
+// in the chunk join the pending run, which the first set cell of a later chunk resolves (the warp
+// then fills the earlier chunks' part of the run with coalesced stores).
 __global__ void __launch_bounds__(256) sweep_x_kernel(float *__restrict__ dist, int nx, int64_t nrows, float fillv) {
     const int lane = threadIdx.x & 31;
     const int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
     if (row >= nrows) return;
     float *d = dist + row * nx;
-    int carry = 0;
-    for (int base = 0; base < nx; base += 32 * SX_BATCH) {                   // forward
+    int carry = 0, run = -1;
+    for (int base = 0; base < nx; base += 32 * SX_BATCH) {
         float v[SX_BATCH];
 #pragma unroll
         for (int u = 0; u < SX_BATCH; u++) {
@@ -40,35 +45,34 @@ __global__ void __launch_bounds__(256) sweep_x_kernel(float *__restrict__ dist, 
         }
 #pragma unroll
         for (int u = 0; u < SX_BATCH; u++) {
-            const int i = base + 32 * u + lane;
+            const int cb = base + 32 * u, i = cb + lane;
+            if (cb >= nx) break;
             const bool set = i < nx && isfinite(v[u]);
             const unsigned ms = __ballot_sync(0xffffffffu, set), mn = __ballot_sync(0xffffffffu, set && v[u] < 0.0f);
-            if (i < nx && !set && state_from_left(ms, mn, lane, carry) < 0) d[i] = fillv;
+            const int sl = state_from_left(ms, mn, lane, carry), sr = state_from_right(ms, mn, lane, 0);
+            if (i < nx && !set && (sl < 0 || sr < 0)) d[i] = fillv;
+            if (ms) {
+                // the first set cell of the chunk decides the run pending from earlier chunks
+                if (run >= 0 && ((mn >> (__ffs(ms) - 1)) & 1u))
+                    for (int x = run + lane; x < cb; x += 32) d[x] = fillv;
+                run = -1;
+            }
             carry = state_from_left(ms, mn, 31, carry);
-        }
-    }
-    __syncwarp();
-    carry = 0;
-    const int nchunk = (nx + 31) / 32;
-    for (int cb = ((nchunk - 1) / SX_BATCH) * SX_BATCH; cb >= 0; cb -= SX_BATCH) {   // backward (the row is in L1/L2 now)
-        float v[SX_BATCH];
-#pragma unroll
-        for (int u = 0; u < SX_BATCH; u++) {
-            const int i = (cb + u) * 32 + lane;
-            v[u] = i < nx ? d[i] : INFINITY;
-        }
-#pragma unroll
-        for (int u = SX_BATCH - 1; u >= 0; u--) {
-            const int i = (cb + u) * 32 + lane;
-            const bool set = i < nx && isfinite(v[u]);
-            const unsigned ms = __ballot_sync(0xffffffffu, set), mn = __ballot_sync(0xffffffffu, set && v[u] < 0.0f);
-            if (i < nx && !set && state_from_right(ms, mn, lane, carry) < 0) d[i] = fillv;
-            carry = state_from_right(ms, mn, 0, carry);
+            if (carry >= 0 && run < 0) {
+                const int start = cb + (ms ? 32 - __clz(ms) : 0);       // first cell after the last set one
+                if (start < min(nx, cb + 32)) run = start;
+            }
         }
     }
 }
 
-// ---- y and z: one thread per line, lines of a warp adjacent in x (coalesced); n cells, stride s
+// ---- y and z: one thread per line, lines of a warp adjacent in x (coalesced); n cells, stride s.
+// ONE walk does the work of the forward and the backward walk.  Within a sweep the two commute: a
+// cell is filled iff the nearest set cell on either side is negative in the data at the start of the
+// sweep (a forward fill never sits between an unset cell and its nearest set cell to the right
+// unless that cell was filled by the same forward walk).  So the walk fills an unset cell at once
+// when the last set cell was negative, and otherwise remembers where the unset run began and fills
+// it when the next set cell turns out to be negative -- writes only, no second read of the line.
 #define SL_BATCH 8
 __global__ void __launch_bounds__(256) sweep_line_kernel(float *__restrict__ dist, int nx, int64_t nlines_outer,
                                                          int64_t outer_stride, int n, int64_t stride, float fillv) {
@@ -76,28 +80,25 @@ __global__ void __launch_bounds__(256) sweep_line_kernel(float *__restrict__ dis
     const int64_t o = blockIdx.y;
     if (i >= nx || o >= nlines_outer) return;
     float *d = dist + o * outer_stride + i;
-    int state = 0;
+    int state = 0, run = -1;                 // run: first cell of the pending unset run, -1 = none
     for (int q0 = 0; q0 < n; q0 += SL_BATCH) {
-        float v[SL_BATCH];
-#pragma unroll
-        for (int u = 0; u < SL_BATCH; u++) v[u] = (q0 + u < n) ? d[(int64_t)(q0 + u) * stride] : 0.0f;
-#pragma unroll
-        for (int u = 0; u < SL_BATCH; u++) {
-            if (q0 + u >= n) break;
-            if (isfinite(v[u])) state = v[u] < 0.0f ? -1 : 1;
-            else if (state < 0) d[(int64_t)(q0 + u) * stride] = fillv;
-        }
-    }
-    state = 0;
-    for (int q0 = ((n - 1) / SL_BATCH) * SL_BATCH; q0 >= 0; q0 -= SL_BATCH) {
         float v[SL_BATCH];
 #pragma unroll
         for (int u = 0; u < SL_BATCH; u++) v[u] = (q0 + u < n) ? d[(int64_t)(q0 + u) * stride] : INFINITY;
 #pragma unroll
-        for (int u = SL_BATCH - 1; u >= 0; u--) {
-            if (q0 + u >= n) continue;
-            if (isfinite(v[u])) state = v[u] < 0.0f ? -1 : 1;
-            else if (state < 0) d[(int64_t)(q0 + u) * stride] = fillv;
+        for (int u = 0; u < SL_BATCH; u++) {
+            const int q = q0 + u;
+            if (q >= n) break;
+            if (isfinite(v[u])) {
+                state = v[u] < 0.0f ? -1 : 1;
+                if (state < 0 && run >= 0)
+                    for (int r = run; r < q; r++) d[(int64_t)r * stride] = fillv;
+                run = -1;
+            } else if (state < 0) {
+                d[(int64_t)q * stride] = fillv;
+            } else if (run < 0) {
+                run = q;
+            }
         }
     }
 }

@@ -36,16 +36,18 @@ def test_fill_matches_oracle(oracle_mod, name, scale):
     assert np.all(t.cpu().numpy()[filled] == -1)
 
 
-@pytest.mark.parametrize("dims", [(37, 29, 43), (1, 1, 70), (65, 1, 3), (33, 64, 1), (200, 7, 5)])
+@pytest.mark.parametrize("dims", [(37, 29, 43), (1, 1, 70), (65, 1, 3), (33, 64, 1), (200, 7, 5), (700, 3, 2), (31, 300, 2), (5, 2, 290)])
 def test_fill_arbitrary_grids(oracle_mod, dims):
     """Random sparse grids (not SDFs): ragged sizes, lines of length 1, runs that start and end unset."""
     nx, ny, nz = dims
     rng = np.random.default_rng(nx * 1000 + ny * 10 + nz)
     d = np.full((nz, ny, nx), np.inf, dtype=np.float32)
-    sel = rng.random(d.shape) < 0.08
-    d[sel] = rng.standard_normal(int(sel.sum())).astype(np.float32)
-    ref = oracle_mod.fill_interior(d, 0.75)
-    assert np.array_equal(_gpu_fill(d, 0.75), ref)
+    for density in (0.002, 0.08, 0.5):
+        d[:] = np.inf
+        sel = rng.random(d.shape) < density
+        d[sel] = rng.standard_normal(int(sel.sum())).astype(np.float32)
+        ref = oracle_mod.fill_interior(d, 0.75)
+        assert np.array_equal(_gpu_fill(d, 0.75), ref)
 
 
 def test_fill_full_size_c3(oracle_mod):
