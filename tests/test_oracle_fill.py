@@ -78,3 +78,43 @@ def test_fill_is_idempotent_and_axis_order_free_on_valid_input(oracle_mod):
     # sweeping the transposed grid (z, y, x order of the axes) fills the same cells
     ft = oracle_mod.fill_interior(np.ascontiguousarray(d.transpose(2, 1, 0)), w.band).transpose(2, 1, 0)
     assert np.array_equal(ft, f)
+
+
+def _sweep_axis_commuted(d, axis, fillv):
+    """One axis, written the other way round: a cell is filled iff the nearest set cell on either side
+    is negative in the data at the START of the sweep (no in-place forward-then-backward walk)."""
+    a = np.moveaxis(d, axis, -1)
+    out = a.copy()
+    n = a.shape[-1]
+    for idx in np.ndindex(a.shape[:-1]):
+        line = a[idx]
+        setm = np.isfinite(line)
+        left = np.zeros(n, dtype=np.int8)
+        right = np.zeros(n, dtype=np.int8)
+        s = 0
+        for q in range(n):
+            if setm[q]:
+                s = -1 if line[q] < 0 else 1
+            left[q] = s
+        s = 0
+        for q in range(n - 1, -1, -1):
+            if setm[q]:
+                s = -1 if line[q] < 0 else 1
+            right[q] = s
+        fill = ~setm & ((left < 0) | (right < 0))
+        out[idx][fill] = fillv
+    return np.moveaxis(out, -1, axis)
+
+
+def test_forward_and_backward_walks_commute_within_a_sweep(oracle_mod):
+    """The property the one-walk GPU sweeps rely on, on grids that are not SDFs."""
+    rng = np.random.default_rng(11)
+    for dims, density in (((9, 7, 11), 0.1), ((16, 5, 3), 0.4), ((4, 4, 30), 0.02), ((12, 12, 12), 0.2)):
+        d = np.full(dims, np.inf, dtype=np.float32)
+        sel = rng.random(dims) < density
+        d[sel] = rng.standard_normal(int(sel.sum())).astype(np.float32)
+        ref = oracle_mod.fill_interior(d, 0.5)
+        got = d.copy()
+        for axis in (2, 1, 0):              # x, y, z of a [nz, ny, nx] array
+            got = _sweep_axis_commuted(got, axis, np.float32(-0.5))
+        assert np.array_equal(got, ref)
