@@ -92,7 +92,7 @@ void sdf_destroy(sdf_mesh *m) {
     if (m->side) cudaStreamSynchronize(m->side);      // shared, process-lifetime stream: not destroyed here
     if (m->ev_fork) cudaEventDestroy(m->ev_fork);
     if (m->ev_join) cudaEventDestroy(m->ev_join);
-    void *ptrs[] = {m->slab_f, m->slab_v, m->slab_ws, m->scratch};
+    void *ptrs[] = {m->slab_f, m->slab_v, m->slab_ws, m->scratch, m->cp_state};
     for (size_t i = 0; i < sizeof(ptrs) / sizeof(ptrs[0]); i++) dev_free(&m->alloc, ptrs[i], st);
     for (int i = 0; i < SDF_T_COUNT; i++)
         for (int w = 0; w < 2; w++)
@@ -154,6 +154,8 @@ static int make_grid(const float origin[3], float h, int nx, int ny, int nz, flo
     const char *pf = getenv("SDF_FILL_MODE");
     g->fill_mode = (pf && pf[0] >= '0' && pf[0] <= '4') ? pf[0] - '0' : 4;
     const char *fd = getenv("SDF_FILL_DEPTH"), *fi = getenv("SDF_FILL_ISSUERS");
+    const char *pc = getenv("SDF_CPT_PLAIN");
+    g->plain_cpt = (pc && pc[0] == '1') ? 1 : 0;
     const char *sc = getenv("SDF_SCHEDULER");
     g->serial_loop = (sc && !strcmp(sc, "serial")) ? 1 : 0;
     const char *fp = getenv("SDF_FILL_PRIO");

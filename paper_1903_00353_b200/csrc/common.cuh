@@ -94,6 +94,7 @@ struct GridParams {
     float band, eps, guard, rb;     // rb = band + guard + eps : reach of every polyhedron
     double dband;
     int big_rows, big_ni;           // polyhedra with more rows / longer rows go to evaluate_big_kernel
+    int plain_cpt;                  // debug: closest points with the dense one-pass kernel only
     int serial_loop;                // ablation: the paper's thread-per-extrusion serial loop
     int aabb_mode;                  // debug: candidates = band-expanded triangle AABBs only
     int vec4;                       // 1: nx % 4 == 0 and outputs 16-B aligned -> 128-bit stores
@@ -135,6 +136,7 @@ struct sdf_mesh {
     int *brick_list;                       // scratch slot -> brick index
     u32 *big_list;                         // polyhedra of evaluate_big_kernel
     u32 *fill_state;                       // fill_tma_kernel: batch cursor + per-SM claims
+    u32 *cp_state;                         // same, for the +inf fill of sdf_closest_points (own allocation)
     u64 *scratch;  size_t scratch_cap;     // bricks * 512 packed values
     u64 h_ctr[CTR_COUNT];
     cudaEvent_t ev[SDF_T_COUNT][2];   // stage begin / end events (created on first use)

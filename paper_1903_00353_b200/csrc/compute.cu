@@ -757,7 +757,8 @@ __global__ void __launch_bounds__(FILL_BT) fill_kernel(float *__restrict__ dist,
 #define FILL_STATE_WORDS 1024
 template <int DEPTH>
 __global__ void __launch_bounds__(FILL_TMA_BT) fill_tma_kernel(float *__restrict__ dist, int *__restrict__ tri,
-                                                               int64_t n, int issuers, int batch, u32 *__restrict__ state) {
+                                                               int64_t n, int issuers, int batch, u32 *__restrict__ state,
+                                                               u32 pat_d, u32 pat_t) {
     __shared__ __align__(128) u32 s_d[FILL_TMA_CHUNK / 4];
     __shared__ __align__(128) u32 s_t[FILL_TMA_CHUNK / 4];
     __shared__ int s_go;
@@ -770,10 +771,12 @@ __global__ void __launch_bounds__(FILL_TMA_BT) fill_tma_kernel(float *__restrict
     }
     // ragged tail (< one chunk) with plain stores
     if (blockIdx.x == 0)
-        for (int64_t i = nchunks * per + threadIdx.x; i < n; i += FILL_TMA_BT) { dist[i] = INFINITY; tri[i] = -1; }
+        for (int64_t i = nchunks * per + threadIdx.x; i < n; i += FILL_TMA_BT) {
+            dist[i] = __uint_as_float(pat_d); tri[i] = (int)pat_t;
+        }
     __syncthreads();
     if (!s_go) return;
-    for (int i = threadIdx.x; i < FILL_TMA_CHUNK / 4; i += FILL_TMA_BT) { s_d[i] = 0x7F800000u; s_t[i] = 0xFFFFFFFFu; }
+    for (int i = threadIdx.x; i < FILL_TMA_CHUNK / 4; i += FILL_TMA_BT) { s_d[i] = pat_d; s_t[i] = pat_t; }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy writes -> async proxy reads
     __syncthreads();
     if ((threadIdx.x & 31) == 0 && (threadIdx.x >> 5) < issuers) {
@@ -996,11 +999,11 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
             const int batch = (int)(bq < 1 ? 1 : (bq > FILL_BATCH ? FILL_BATCH : bq));
             KL;
             switch (g.fill_depth) {
-            case 0: fill_tma_kernel<0><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state); break;
-            case 1: fill_tma_kernel<1><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state); break;
-            case 2: fill_tma_kernel<2><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state); break;
-            case 4: fill_tma_kernel<4><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state); break;
-            default: fill_tma_kernel<8><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state); break;
+            case 0: fill_tma_kernel<0><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state, 0x7F800000u, 0xFFFFFFFFu); break;
+            case 1: fill_tma_kernel<1><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state, 0x7F800000u, 0xFFFFFFFFu); break;
+            case 2: fill_tma_kernel<2><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state, 0x7F800000u, 0xFFFFFFFFu); break;
+            case 4: fill_tma_kernel<4><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state, 0x7F800000u, 0xFFFFFFFFu); break;
+            default: fill_tma_kernel<8><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state, 0x7F800000u, 0xFFFFFFFFu); break;
             }
         } else {
             int64_t fb = (N / 4 + (int64_t)FILL_BT * FILL_UNROLL - 1) / ((int64_t)FILL_BT * FILL_UNROLL);
@@ -1135,6 +1138,35 @@ __global__ void __launch_bounds__(256) closest_points_kernel(MeshView mv, GridPa
     }
 }
 
+// After a TMA fill of the whole output with +inf: only the cells of the band are visited for real.
+// A block streams CPS_LOADS * 256 int4 of ids (all loads issued before any is looked at); the few
+// quads that hold a band cell are handled in a rolled loop so the streaming part stays small.
+#define CPS_LOADS 4
+__global__ void __launch_bounds__(256) closest_points_sparse_kernel(MeshView mv, GridParams g, const int *__restrict__ tri,
+                                                                    float *__restrict__ cp, int64_t n4) {
+    const int64_t q0 = (int64_t)blockIdx.x * (256 * CPS_LOADS) + threadIdx.x;      // in units of int4
+    const int64_t nq = n4 >> 2;
+    int4 t4[CPS_LOADS];
+#pragma unroll
+    for (int u = 0; u < CPS_LOADS; u++) {
+        const int64_t q = q0 + (int64_t)u * 256;
+        t4[u] = q < nq ? __ldcs((const int4 *)tri + q) : make_int4(-1, -1, -1, -1);
+    }
+#pragma unroll 1
+    for (int u = 0; u < CPS_LOADS; u++) {
+        if ((t4[u].x & t4[u].y & t4[u].z & t4[u].w) < 0 && t4[u].x < 0 && t4[u].y < 0 && t4[u].z < 0 && t4[u].w < 0) continue;
+        const int64_t c = (q0 + (int64_t)u * 256) * 4;
+        const int xt[4] = {t4[u].x, t4[u].y, t4[u].z, t4[u].w};
+#pragma unroll 1
+        for (int e = 0; e < 4; e++)
+            if (xt[e] >= 0) {
+                float o[3];
+                closest_point_of(mv, g, xt[e], c + e, o);
+                cp[3 * (c + e)] = o[0]; cp[3 * (c + e) + 1] = o[1]; cp[3 * (c + e) + 2] = o[2];
+            }
+    }
+}
+
 int run_closest_points(sdf_mesh *m, const GridParams &g, const int *tri, float *cp, cudaStream_t st) {
     MeshView mv;
     mv.soup = m->soup; mv.fn = m->fn; mv.erec = m->erec; mv.vrec = m->vrec; mv.vmint = m->vmint;
@@ -1143,6 +1175,24 @@ int run_closest_points(sdf_mesh *m, const GridParams &g, const int *tri, float *
     mv.P = m->F + m->E + 2 * m->V;
     const int64_t n = (int64_t)g.nx * g.ny * g.nz;
     const bool vec = (((uintptr_t)tri & 15) == 0) && (((uintptr_t)cp & 15) == 0);
+    if (vec && n % 8 == 0 && n >= (1 << 20) && !g.plain_cpt) {
+        // large aligned grids: +inf over everything with TMA bulk stores (the two halves of cp play
+        // the two arrays of the sentinel fill), then the band only
+        int dev = 0, sms = 148;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (!m->cp_state) CKS(dev_alloc(&m->alloc, (void **)&m->cp_state, sizeof(u32) * FILL_STATE_WORDS, st));
+        CK(cudaMemsetAsync(m->cp_state, 0, sizeof(u32) * FILL_STATE_WORDS, st));
+        const int64_t half = 3 * n / 2;
+        int64_t bq = (half / (FILL_TMA_CHUNK / 4)) / ((int64_t)sms * 4 * 8);
+        const int batch = (int)(bq < 1 ? 1 : (bq > FILL_BATCH ? FILL_BATCH : bq));
+        KL; fill_tma_kernel<8><<<(unsigned)(sms * 4), FILL_TMA_BT, 0, st>>>(cp, (int *)(cp + half), half, 4, batch, m->cp_state,
+                                                                         0x7F800000u, 0x7F800000u);
+        KL; closest_points_sparse_kernel<<<(unsigned)((n / 4 + 256 * CPS_LOADS - 1) / (256 * CPS_LOADS)), 256, 0, st>>>(mv, g, tri, cp, n);
+        CK(cudaGetLastError());
+        m->last_stream = st;
+        return SDF_OK;
+    }
     const int64_t n4 = vec ? (n & ~(int64_t)3) : 0;
     if (n4) { KL; closest_points_kernel<4><<<(unsigned)((n4 / 4 + 255) / 256), 256, 0, st>>>(mv, g, tri, cp, 0, n4); }
     if (n > n4) { KL; closest_points_kernel<1><<<(unsigned)((n - n4 + 255) / 256), 256, 0, st>>>(mv, g, tri, cp, n4, n); }
