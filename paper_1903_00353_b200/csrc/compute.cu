@@ -860,7 +860,7 @@ __device__ __forceinline__ CellOut finish_cell(const MeshView &mv, const GridPar
 // the threads (the sign pass is the expensive, divergent part); phase 3 writes the brick's
 // 64 row segments (8 cells = one 32-B sector each) into both grids.
 #define EB_BT 128
-__global__ void __launch_bounds__(EB_BT) emit_bricks_kernel(MeshView mv, GridParams g, const int *__restrict__ list,
+__global__ void __launch_bounds__(EB_BT, 12) emit_bricks_kernel(MeshView mv, GridParams g, const int *__restrict__ list,
                                                             const u64 *__restrict__ scratch,
                                                             float *__restrict__ dist, int *__restrict__ tri,
                                                             u64 *__restrict__ ctr) {
