@@ -15,6 +15,9 @@
 #include <string.h>
 
 #define FB 256   // threads per block of the element-wise kernels
+#ifndef TG_MINB
+#define TG_MINB 5 // resident blocks per SM asked of the fp64-heavy per-triangle kernels (latency bound)
+#endif
 
 static inline unsigned blocks_for(int64_t n, int bt = FB) { return (unsigned)((n + bt - 1) / bt); }
 
@@ -193,7 +196,7 @@ __device__ __forceinline__ bool tri_normal64(const float *__restrict__ T, double
     return true;
 }
 
-__global__ void __launch_bounds__(FB) tri_geom_kernel(const float *__restrict__ soup, const u32 *__restrict__ wtab,
+__global__ void __launch_bounds__(FB, TG_MINB) tri_geom_kernel(const float *__restrict__ soup, const u32 *__restrict__ wtab,
                                                       const u32 *__restrict__ slot, int F, int *__restrict__ cvid,
                                                       float *__restrict__ fn, u64 *__restrict__ vacc,
                                                       unsigned char *__restrict__ fcnt, u32 *etab, u32 emask,
@@ -412,7 +415,7 @@ __global__ void __launch_bounds__(FB) vertex_normal_kernel(const u64 *__restrict
 // one thread per triangle: for each corner, cos of the angle between the face normal and the
 // vertex axis (eq.9), which side of the pseudonormal plane the two
 // neighbours lie on, lowest incident triangle id
-__global__ void __launch_bounds__(FB) vertex_cone_kernel(const float *__restrict__ soup, const int *__restrict__ cvid,
+__global__ void __launch_bounds__(FB, TG_MINB) vertex_cone_kernel(const float *__restrict__ soup, const int *__restrict__ cvid,
                                                          int F, const double *__restrict__ vn64,
                                                          long long *__restrict__ vcosq, int *__restrict__ vside,
                                                          const int *__restrict__ perm, int *__restrict__ vmint,
