@@ -743,17 +743,19 @@ __global__ void __launch_bounds__(FILL_BT) fill_kernel(float *__restrict__ dist,
     }
 }
 
-// TMA variant (the default): one CTA per SM keeps two 16 KiB sentinel tiles in shared memory and
+// TMA variant (the default): one CTA per SM keeps two 4 KiB sentinel tiles in shared memory and
 // one lane per warp streams them to HBM with bulk asynchronous copies (cp.async.bulk, SASS
-// UBLKCP), L2 evict-first.  It needs 4 warps and 32 KiB of shared memory per SM, so the kernels
+// UBLKCP), L2 evict-first.  It needs 4 warps and 8 KiB of shared memory per SM, so the kernels
 // of A5-A7 keep (almost) the whole SM while 8 B/cell stream out underneath them.
 #define FILL_TMA_BT 128
-#define FILL_TMA_CHUNK 16384
+#define FILL_TMA_CHUNK 4096      // bytes per bulk copy.  The size sets the balance with the kernels running beside
+                                 // the fill: 2 KiB starves them (evaluate 1.46 -> 1.96 ms at C4), 16 KiB yields to them
+                                 // (fill 1.55 ms); alone the fill does 7.3 TB/s at 4 KiB
 // fill_state: [0] = next batch (dynamic fetch), [1 + smid] = SM already has a fill CTA.  More
 // CTAs than SMs are launched and the first to arrive on an SM claims it; the others exit at
 // once.  (With one CTA per SM by count only, a busy GPU stacked several fill CTAs on the few
 // SMs that had room and the fill ran at a fraction of the HBM rate.)
-#define FILL_BATCH 64            // chunks per fetch: 1 MiB contiguous per array
+#define FILL_BATCH (1048576 / FILL_TMA_CHUNK)   // chunks per fetch: 1 MiB contiguous per array
 #define FILL_STATE_WORDS 1024
 template <int DEPTH>
 __global__ void __launch_bounds__(FILL_TMA_BT) fill_tma_kernel(float *__restrict__ dist, int *__restrict__ tri,
