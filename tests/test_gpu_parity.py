@@ -273,6 +273,24 @@ def test_degenerate_shapes_and_grids(oracle_mod):
         _assert_ok(check_parity(w, oracle_mod))
 
 
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_maximum_grid_dimension(oracle_mod, axis):
+    """32767 cells (the largest dimension the 16-bit bounding volumes allow) along one axis, the mesh at
+    its far end, coordinates around 1000."""
+    v, t = W.icosphere_mesh(2, 0.6)
+    h = 2.0 / 64
+    dims = [5, 5, 5]
+    dims[axis] = 32767
+    c = np.zeros(3)
+    c[axis] = (32767 - 40) * h
+    origin = [-2 * h] * 3
+    origin[axis] = 0.0
+    w = W.Workload("long", W.soup_from_indexed(v + c, t, np.random.default_rng(axis)), tuple(origin), h, tuple(dims), 3 * h)
+    res = check_parity(w, oracle_mod)
+    _assert_ok(res)
+    assert res["populated_gpu"] == 312
+
+
 def test_knife_edges(oracle_mod):
     """Edges whose faces fold back onto each other (n1 = -n2): sin(dihedral) vanishes as it does for a
     flat edge, but the edge needs the widest extrusion there is.  A two-triangle "pillow" (zero volume,
