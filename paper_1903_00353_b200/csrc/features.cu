@@ -310,9 +310,9 @@ __global__ void __launch_bounds__(FB) edge_pair_kernel(const int *__restrict__ c
     }
 }
 
-// one thread per half-edge; the forward half-edge of every claimed pair writes the edge record
+// one thread per triangle; the forward half-edge of every claimed pair writes the edge record
 // (A4 edge class + band-independent wedge geometry) at its rank among the forward half-edges
-__global__ void __launch_bounds__(FB) edge_record_kernel(const int *__restrict__ cvid, int n,
+__global__ void __launch_bounds__(FB) edge_record_kernel(const int *__restrict__ cvid, int F,
                                                          const int *__restrict__ adj, const u32 *__restrict__ ebase,
                                                          const float *__restrict__ soup, const float *__restrict__ fn,
                                                          const int *__restrict__ perm,
@@ -320,15 +320,19 @@ __global__ void __launch_bounds__(FB) edge_record_kernel(const int *__restrict__
     __shared__ u32 s_cnt[3];
     if (threadIdx.x < 3) s_cnt[threadIdx.x] = 0;
     __syncthreads();
-    int he0 = blockIdx.x * FB + threadIdx.x;
-    if (he0 < n) {
-        const int t0 = he0 / 3, k0 = he0 - 3 * t0;
-        const int c0 = cvid[3 * (size_t)t0], c1 = cvid[3 * (size_t)t0 + 1], c2 = cvid[3 * (size_t)t0 + 2];
-        const int u = k0 == 0 ? c0 : (k0 == 1 ? c1 : c2), w = k0 == 0 ? c1 : (k0 == 1 ? c2 : c0);
-        const int he1 = adj[he0];
-        if (u < w && he1 >= 0) {
-            const int t1 = he1 / 3;
-            const int e = (int)ebase[t0] + (k0 > 0 ? (c0 < c1) : 0) + (k0 > 1 ? (c1 < c2) : 0);
+    const int t0 = blockIdx.x * FB + threadIdx.x;
+    if (t0 < F) {
+        const int c[3] = {cvid[3 * (size_t)t0], cvid[3 * (size_t)t0 + 1], cvid[3 * (size_t)t0 + 2]};
+        const int he1[3] = {adj[3 * (size_t)t0], adj[3 * (size_t)t0 + 1], adj[3 * (size_t)t0 + 2]};
+        int e = (int)ebase[t0];
+        int x0 = -1;
+#pragma unroll
+        for (int k0 = 0; k0 < 3; k0++) {
+            const int u = c[k0], w = c[k0 == 2 ? 0 : k0 + 1];
+            if (!(u < w)) continue;
+            const int erank = e++;                       // rank among the forward half-edges in soup order
+            if (he1[k0] < 0) continue;
+            const int t1 = he1[k0] / 3;
             const float *A = soup + 9 * (size_t)t0 + 3 * k0, *B = soup + 9 * (size_t)t0 + 3 * (k0 == 2 ? 0 : k0 + 1);
             const float *N1 = fn + 3 * (size_t)t0, *N2 = fn + 3 * (size_t)t1;
             // canonical direction a -> b = ascending exact position bits, so the record (and the
@@ -357,11 +361,12 @@ __global__ void __launch_bounds__(FB) edge_record_kernel(const int *__restrict__
             // wedge is on cannot be told from a vanishing discriminant: class 2, "knife", whose
             // extrusion is the whole cylinder about the edge
             if (cls == 0 && ddot(n1, n2) <= 0.0) cls = 2;
-            const int x0 = perm[t0], x1 = perm[t1];      // the caller's triangle ids
+            if (x0 < 0) x0 = perm[t0];                   // the caller's triangle ids
+            const int x1 = perm[t1];
             r.tri = x0 < x1 ? x0 : x1;
             r.cls = cls;
             r.pad[0] = r.pad[1] = 0;
-            erec[e] = r;
+            erec[erank] = r;
             atomicAdd(&s_cnt[cls > 0 ? 0 : (cls < 0 ? 1 : 2)], 1u);      // knife edges count as convex
         }
     }
@@ -674,7 +679,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wtab, slot, (int)F, m->cvid, m->fn, vacc, fcnt, etab, cape - 1, m->d_flags);
     CKS(launch_scan(FcntIn{fcnt}, EbaseOut{ebase}, F, scan_ws, (u64 *)nullptr, st));
     KL; edge_pair_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, etab, cape - 1, m->adj);
-    KL; edge_record_kernel<<<blocks_for(nc), FB, 0, st>>>(m->cvid, nc, m->adj, ebase, m->soup, m->fn, m->perm, m->erec, m->d_ctr);
+    KL; edge_record_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, m->adj, ebase, m->soup, m->fn, m->perm, m->erec, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_EDGES, 1, st);
 
