@@ -613,15 +613,18 @@ template <bool SERIAL>
 __global__ void __launch_bounds__(32 * ES_WARPS, SERIAL ? 1 : ES_MINB) evaluate_small_kernel(MeshView mv, GridParams g,
                                                                        u32 *__restrict__ big_list,
                                                                        const int *__restrict__ table,
-                                                                       u64 *__restrict__ scratch, u64 *__restrict__ ctr) {
+                                                                       u64 *__restrict__ scratch, u64 *__restrict__ ctr,
+                                                                       int ppw) {
+    // ppw = polyhedra per warp: 32, or fewer when the mesh has few polyhedra (more warps for the
+    // same rows: a mesh of 1e5 medium polyhedra otherwise leaves each scheduler 5 long-running warps)
     __shared__ float s_rec[ES_WARPS][32][RR_WORDS];
     __shared__ int s_ex[ES_WARPS][33];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int64_t p = ((int64_t)blockIdx.x * ES_WARPS + w) * 32 + lane;
+    const int64_t p = ((int64_t)blockIdx.x * ES_WARPS + w) * ppw + lane;
     int rows = 0;
     bool live = false, direct = false;
     PolyHdr Hd;
-    if (p < mv.P) {
+    if (lane < ppw && p < mv.P) {
         PolyHdr H;
         live = poly_aabv(mv, g, p, H);
         if (live) {
@@ -1069,11 +1072,12 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
     // big ones one block each (dynamic fetch)
     if (bricks) {
         stage_mark(m, SDF_T_EVALUATE, 0, st);
-        const int64_t nblk = (P + 32 * ES_WARPS - 1) / (32 * ES_WARPS);
+        const int ppw = P < (1 << 17) ? 4 : (P < (1 << 20) ? 8 : 32);
+        const int64_t nblk = (P + (int64_t)ppw * ES_WARPS - 1) / ((int64_t)ppw * ES_WARPS);
         const unsigned split = P < 65536 ? EBIG_SPLIT : (P < (1 << 20) ? 2 : 1);
         KL;
-        if (g.serial_loop) evaluate_small_kernel<true><<<(unsigned)nblk, 32 * ES_WARPS, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr);
-        else evaluate_small_kernel<false><<<(unsigned)nblk, 32 * ES_WARPS, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr);
+        if (g.serial_loop) evaluate_small_kernel<true><<<(unsigned)nblk, 32 * ES_WARPS, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr, ppw);
+        else evaluate_small_kernel<false><<<(unsigned)nblk, 32 * ES_WARPS, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr, ppw);
         KL; evaluate_big_kernel<<<dim3((unsigned)(sms * 4 / split), split), EBIG_BT, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr);
         stage_mark(m, SDF_T_EVALUATE, 1, st);
     }
