@@ -144,15 +144,26 @@ def torch_allocator():
     if _torch_allocator is None:
         torch = _torch()
 
+        # the raw entry points of torch's caching allocator (what torch.cuda.caching_allocator_alloc
+        # ends up calling, without its device-context manager: these callbacks sit on the critical
+        # path of every sdf_create / sdf_compute); the public functions if a build lacks them
+        raw_alloc = getattr(torch._C, "_cuda_cudaCachingAllocator_raw_alloc", None)
+        raw_delete = getattr(torch._C, "_cuda_cudaCachingAllocator_raw_delete", None)
+
         def _alloc(nbytes, stream, user):
             try:
+                if raw_alloc is not None:
+                    return raw_alloc(int(nbytes), int(stream or 0))
                 return torch.cuda.caching_allocator_alloc(int(nbytes), stream=int(stream or 0))
             except Exception:
                 return None
 
         def _free(ptr, user):
             if ptr:
-                torch.cuda.caching_allocator_delete(int(ptr))
+                if raw_delete is not None:
+                    raw_delete(int(ptr))
+                else:
+                    torch.cuda.caching_allocator_delete(int(ptr))
 
         a = _Allocator(_ALLOC_FN(_alloc), _FREE_FN(_free), None)
         _torch_allocator = a
