@@ -20,10 +20,11 @@
  * The library never falls back to a CPU implementation: without a CUDA device every
  * compute entry point returns SDF_ECUDA.
  * Threading: calls on one handle must not overlap, and neither may calls that create library-wide
- * state for the first time (the first sdf_compute of a process creates the side stream of the
- * sentinel fill); distinct handles on distinct streams are otherwise independent.
+ * state for the first time (the first sdf_create / sdf_compute of a process create the library's
+ * side streams: vertex stage, sentinel fill); distinct handles on distinct streams are otherwise independent.
  * Debug / ablation switches (environment, read per call): SDF_AABB_MODE=1 (candidates = band-expanded
- * triangle boxes only), SDF_FILL_MODE=0..4, SDF_SCHEDULER=serial, SDF_RUFF=cone, SDF_NO_BINNING=1;
+ * triangle boxes only), SDF_FILL_MODE=0..4, SDF_SCHEDULER=serial, SDF_RUFF=cone, SDF_NO_BINNING=1,
+ * SDF_CREATE_FORK=0 (vertex stage on the caller's stream);
  * see DESIGN.md.
  */
 #ifndef PAPER_1903_00353_SDF_H
@@ -222,7 +223,8 @@ int sdf_get_table(sdf_mesh *m, int which, void *dst, size_t bytes);
 enum {
     SDF_T_INGEST_WELD = 0,  /* A0+A1: spatial binning, gather/canonicalise, weld table, vertex ids */
     SDF_T_EDGES       = 1,  /* A2+A3: triangle geometry, half-edge table, pairing, edge classes   */
-    SDF_T_VERTICES    = 2,  /* A3+A4: pseudonormals, cone angles, vertex classes                  */
+    SDF_T_VERTICES    = 2,  /* A3+A4: pseudonormals, cone angles, vertex classes (library-owned
+                               second stream, concurrent with the pairing part of stage 1)       */
     SDF_T_CLIP_SCAN   = 3,  /* A6a: brick marks, prefix sum, brick table, the host crossing       */
     SDF_T_CLEAR       = 4,  /* scratch bricks reset to "empty"                                    */
     SDF_T_EVALUATE    = 5,  /* A5-A7: clip, scan-convert, distances, packed atomicMin             */

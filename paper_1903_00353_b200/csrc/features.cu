@@ -677,6 +677,26 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     stage_mark(m, SDF_T_EDGES, 0, st);
     CK(cudaMemsetAsync(vacc, 0, (size_t)((char *)(vside + V) - (char *)vacc), st));
     KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wtab, slot, (int)F, m->cvid, m->fn, vacc, fcnt, etab, cape - 1, m->d_flags);
+    // the vertex stage needs only what tri_geom wrote: it runs on a second stream beside the edge stage
+    cudaStream_t vs = st;
+    {
+        const char *cf = getenv("SDF_CREATE_FORK");
+        if (!(cf && cf[0] == '0')) {
+            static cudaStream_t g_vs = nullptr;
+            static int g_vs_dev = -1;
+            int dev = 0;
+            CK(cudaGetDevice(&dev));
+            if (!g_vs || g_vs_dev != dev) {
+                CK(cudaStreamCreateWithFlags(&g_vs, cudaStreamNonBlocking));
+                g_vs_dev = dev;
+            }
+            vs = g_vs;
+            if (!m->ev_fork) CK(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
+            if (!m->ev_join) CK(cudaEventCreateWithFlags(&m->ev_join, cudaEventDisableTiming));
+            CK(cudaEventRecord(m->ev_fork, st));
+            CK(cudaStreamWaitEvent(vs, m->ev_fork, 0));
+        }
+    }
     CKS(launch_scan(FcntIn{fcnt}, EbaseOut{ebase}, F, scan_ws, (u64 *)nullptr, st));
     KL; edge_pair_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, etab, cape - 1, m->adj);
     KL; edge_record_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, m->adj, ebase, m->soup, m->fn, m->perm, m->erec, m->d_ctr);
@@ -684,16 +704,20 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     stage_mark(m, SDF_T_EDGES, 1, st);
 
     // ---- A3/A4 vertices (garbage-in on invalid input is harmless: ids stay in range)
-    stage_mark(m, SDF_T_VERTICES, 0, st);
+    stage_mark(m, SDF_T_VERTICES, 0, vs);
     // "larger than any value" initial states: 0x7F7F.. for the cone cosines and triangle ids
-    CK(cudaMemsetAsync(vcosq, 0x7F, sizeof(long long) * (size_t)V, st));
-    if (vcospos) CK(cudaMemsetAsync(vcospos, 0x7F, sizeof(long long) * (size_t)V, st));
-    CK(cudaMemsetAsync(m->vmint, 0x7F, sizeof(int) * (size_t)V, st));
-    KL; vertex_normal_kernel<<<blocks_for(V), FB, 0, st>>>(vacc, V, vn64);
-    KL; vertex_cone_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, m->cvid, (int)F, vn64, vcosq, vside, m->perm, m->vmint, vcospos);
-    KL; vertex_record_kernel<<<blocks_for(V), FB, 0, st>>>(m->soup, vcorner, vn64, vcosq, vside, V, vcospos, m->vrec, m->d_ctr);
+    CK(cudaMemsetAsync(vcosq, 0x7F, sizeof(long long) * (size_t)V, vs));
+    if (vcospos) CK(cudaMemsetAsync(vcospos, 0x7F, sizeof(long long) * (size_t)V, vs));
+    CK(cudaMemsetAsync(m->vmint, 0x7F, sizeof(int) * (size_t)V, vs));
+    KL; vertex_normal_kernel<<<blocks_for(V), FB, 0, vs>>>(vacc, V, vn64);
+    KL; vertex_cone_kernel<<<blocks_for(F), FB, 0, vs>>>(m->soup, m->cvid, (int)F, vn64, vcosq, vside, m->perm, m->vmint, vcospos);
+    KL; vertex_record_kernel<<<blocks_for(V), FB, 0, vs>>>(m->soup, vcorner, vn64, vcosq, vside, V, vcospos, m->vrec, m->d_ctr);
     CK(cudaGetLastError());
-    stage_mark(m, SDF_T_VERTICES, 1, st);
+    stage_mark(m, SDF_T_VERTICES, 1, vs);
+    if (vs != st) {
+        CK(cudaEventRecord(m->ev_join, vs));
+        CK(cudaStreamWaitEvent(st, m->ev_join, 0));
+    }
     // second host crossing: validation flags + class counters
     int hflags[4];
     CK(cudaMemcpyAsync(hflags, m->d_flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
