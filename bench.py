@@ -174,7 +174,9 @@ def workload_config(w, args):
     return {"workload": "%s: %d triangles, grid %dx%dx%d, h=%g, band %gh (BASELINE.json configs[%d])"
                         % (w.name, w.ntri, nx, ny, nz, w.h, w.band / w.h, W.CONFIG_NAMES.index(w.name)),
             "triangles": w.ntri, "grid": [nx, ny, nz], "band_cells": w.band / w.h,
-            "parallelism": "replicas only (the path does not shard)" if args.gpus > 1 else "1 GPU",
+            "parallelism": ("z-slabs: every rank builds the mesh and computes 1/%d of the grid, no exchange"
+                            % (args.zslab_parts or args.gpus)) if (args.zslab or args.zslab_parts) else
+                           "replicas only (the path does not shard)" if args.gpus > 1 else "1 GPU",
             "l2": "no flush needed: each step streams %.2f GB of output > %d MB L2"
                   % (8.0 * w.ncells / 1e9, L2_BYTES >> 20)}
 
@@ -197,6 +199,22 @@ def run_ours(args):
 
     w = load_workload(args)
     nx, ny, nz = w.dims
+    # --zslab: every rank builds the whole mesh and computes one
+    # z-slab of the grid (strong scaling, no data-path collective); --zslab-parts / --zslab-part time
+    # one slab of a P-way split on a single GPU
+    zslab = None
+    if args.zslab or args.zslab_parts:
+        parts = args.zslab_parts or world
+        part = args.zslab_part if args.zslab_parts else rank
+        k0, nk = B.sdf_zslab(nz, part, parts)
+        if nk == 0:
+            raise SystemExit("z-slab %d of %d of %d slices is empty" % (part, parts, nz))
+        zslab = {"part": part, "parts": parts, "k0": k0, "nk": nk}
+        full_dims, full_origin = w.dims, w.origin
+        # the slab as a grid of its own (include/sdf.h, sdf_compute_zslab: origin_z + k0*h in double, rounded once)
+        oz = float(np.float32(np.float64(np.float32(w.origin[2])) + k0 * np.float64(np.float32(w.h))))
+        w = W.Workload(w.name, w.soup, (w.origin[0], w.origin[1], oz), w.h, (nx, ny, nk), w.band, dict(w.meta))
+        nx, ny, nz = w.dims
     N = w.ncells
     soup_host = torch.from_numpy(np.ascontiguousarray(w.soup)).pin_memory()
     soup_dev = soup_host.to(dev)
@@ -208,7 +226,11 @@ def run_ours(args):
 
     def step_device():
         m = B.sdf_create(soup_dev, stream=stream)
-        B.sdf_compute(m, w.origin, w.h, w.dims, w.band, dist_out, tri_out, stream=stream)
+        if zslab:
+            B.sdf_compute_zslab(m, full_origin, w.h, full_dims, w.band, zslab["part"], zslab["parts"], dist_out, tri_out,
+                                stream=stream)
+        else:
+            B.sdf_compute(m, w.origin, w.h, w.dims, w.band, dist_out, tri_out, stream=stream)
         return m
 
     def barrier():
@@ -252,7 +274,12 @@ def run_ours(args):
         total_ms = float(t.item())
     ms_per_step = total_ms / args.steps
     band_cells = int(stats["band_cells"])
-    value = world * band_cells / (ms_per_step * 1e-3)
+    total_cells = world * band_cells
+    if zslab and world > 1:                       # the slabs differ: sum what the ranks computed
+        t = torch.tensor([band_cells], dtype=torch.int64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        total_cells = int(t.item())
+    value = total_cells / (ms_per_step * 1e-3)
 
     # ---- end to end: HOST buffers through the C ABI (H2D of the soup, D2H of both grids)
     e2e = None
@@ -281,7 +308,7 @@ def run_ours(args):
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             e_ms = float(t.item())
         assert int(torch.isfinite(dist_host).sum()) == band_cells
-        e2e = {"value": world * band_cells / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": e_ms, "steps": ne,
+        e2e = {"value": total_cells / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": e_ms, "steps": ne,
                "h2d_bytes_per_step": int(soup_host.numel() * 4), "d2h_bytes_per_step": int(8 * N)}
         del dist_host, tri_host
 
@@ -342,7 +369,7 @@ def run_ours(args):
     fill_gbs = 8.0 * N / (fill_ms * 1e-3) / 1e9 if fill_ms else 0.0
     roofline = {"bound": "hbm", "kernel": "fill_tma_kernel (A8a dense write of both grids, cp.async.bulk shared->global)",
                 "achieved": fill_gbs, "peak": peak, "unit": "GB/s", "frac": fill_gbs / peak,
-                "traffic": args.traffic if args.traffic is not None else (NCU_FILL_TRAFFIC_C4 if w.name == "C4" else None),
+                "traffic": args.traffic if args.traffic is not None else (NCU_FILL_TRAFFIC_C4 if w.name == "C4" and not zslab else None),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": 8.0 * N,
                 "ms_per_launch": fill_ms, "dominant_stage": dom}
     step_bytes = 8.0 * N + 36.0 * w.ntri
@@ -355,11 +382,11 @@ def run_ours(args):
         cpu = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if zslab and world > 1 else "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(w, args),
             "band_cells": band_cells, "stage_ms": stage_ms, "step_ms_min": min(step_ms), "step_ms_max": max(step_ms), "wall_ms_per_step":
             t_wall * 1e3 / args.steps, "roofline": roofline, "roofline_step": roofline_step, "cpu_baseline": cpu,
-            "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "fill_interior": fill_int, "closest_points": cpt,
+            "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "zslab": zslab, "fill_interior": fill_int, "closest_points": cpt,
             "stats": {k: stats[k] for k in ("polyhedra", "work_items", "pairs_tested", "pairs_accepted",
                                             "bricks_active", "fp64_rechecks")}}
     print(json.dumps(line), flush=True)
@@ -377,6 +404,9 @@ def main():
     ap.add_argument("--band-cells", type=float, default=0.0, help="override the band width (cells); 0 = the config's")
     ap.add_argument("--fill-interior", action="store_true", help="also time sdf_fill_interior (NEXT-1) on the result")
     ap.add_argument("--closest-points", action="store_true", help="also time sdf_closest_points (NEXT-2) on the result")
+    ap.add_argument("--zslab", action="store_true", help="strong scaling: rank r computes z-slab r of WORLD_SIZE (NEXT-4)")
+    ap.add_argument("--zslab-parts", type=int, default=0, help="time one slab of a P-way z split on this GPU")
+    ap.add_argument("--zslab-part", type=int, default=0)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")

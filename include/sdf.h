@@ -136,6 +136,32 @@ int sdf_compute(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int
                 float band, float *dist_out, int32_t *tri_out, void *stream);
 
 /*
+ * sdf_zslab / sdf_compute_zslab -- the paper's multi-card outlook (a domain
+ * "distributed across multiple cards"): the grid is cut into `parts` slabs of whole z-slices and
+ * every process computes one of them from the complete feature tables of its own handle.  No cell
+ * of a slab needs anything from another slab (every polyhedron that reaches it is evaluated
+ * locally), so there is no halo and no exchange: the slabs are independent sdf_compute calls.
+ *
+ * sdf_zslab (host only, no CUDA): slab `part` of `parts` of a grid of nz slices is
+ * [*k0, *k0 + *nk); boundaries fall on multiples of 8 slices (the brick height), the slabs are
+ * disjoint, ordered, cover [0, nz), and differ by at most 8 slices; *nk may be 0 when
+ * parts > ceil(nz / 8).  Errors: SDF_EINVAL (nz < 1, parts < 1, part outside [0, parts), NULL).
+ *
+ * sdf_compute_zslab: sdf_compute on the grid (nx, ny, *nk) whose sample (0,0,0) sits at
+ * origin + (0, 0, k0 * h), the z component evaluated in double and rounded once to float (that
+ * float IS the slab's origin: sample k of the slab sits at fmaf(k, h, origin_z'), which equals
+ * the whole grid's fmaf(k0 + k, h, origin_z) whenever both are exact, e.g. for power-of-two h,
+ * and differs from it by at most one rounding otherwise).  dist_out / tri_out: DEVICE,
+ * nx*ny*(*nk) elements, slab-local linear index.  k0_out / nk_out (HOST, may be NULL) receive
+ * the range.  An empty slab returns SDF_OK without touching the outputs.
+ * Errors: those of sdf_zslab and sdf_compute.
+ */
+int sdf_zslab(int nz, int part, int parts, int *k0, int *nk);
+int sdf_compute_zslab(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz,
+                      float band, int part, int parts, float *dist_out, int32_t *tri_out,
+                      void *stream, int *k0_out, int *nk_out);
+
+/*
  * sdf_compute_host -- same as sdf_compute but dist_out / tri_out are HOST buffers
  * (pinned memory recommended): device grids are taken from the allocator, computed,
  * copied back with cudaMemcpyAsync and the stream is synchronised before returning.

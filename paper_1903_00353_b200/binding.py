@@ -22,7 +22,7 @@ SDF_OK, SDF_EINVAL, SDF_ENOTCLOSED, SDF_EORIENT, SDF_EDEGENERATE, SDF_ENOMEM, SD
 TABLE_CORNER_VID, TABLE_HALFEDGE_ADJ, TABLE_FACE_NORMAL, TABLE_VERTEX_REC, TABLE_EDGE_REC, \
     TABLE_VERTEX_MINTRI = range(6)
 
-EXPORTS = ("sdf_create", "sdf_compute", "sdf_compute_host", "sdf_fill_interior", "sdf_closest_points", "sdf_stats", "sdf_get_table",
+EXPORTS = ("sdf_create", "sdf_compute", "sdf_compute_host", "sdf_zslab", "sdf_compute_zslab", "sdf_fill_interior", "sdf_closest_points", "sdf_stats", "sdf_get_table",
            "sdf_destroy", "sdf_strerror", "sdf_last_cuda_error", "sdf_version",
            "sdf_enable_timing", "sdf_get_timings", "sdf_launch_count",
            "sdf_read_stl", "sdf_free_host", "sdf_write_stl", "sdf_write_grid")
@@ -90,6 +90,11 @@ def lib():
     L.sdf_compute.argtypes = [vp, C.POINTER(C.c_float), C.c_float, C.c_int, C.c_int, C.c_int, C.c_float, vp, vp, vp]
     L.sdf_compute.restype = C.c_int
     L.sdf_compute_host.argtypes = L.sdf_compute.argtypes
+    L.sdf_zslab.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]
+    L.sdf_zslab.restype = C.c_int
+    L.sdf_compute_zslab.argtypes = [vp, C.POINTER(C.c_float), C.c_float, C.c_int, C.c_int, C.c_int, C.c_float, C.c_int, C.c_int,
+                                    vp, vp, vp, C.POINTER(C.c_int), C.POINTER(C.c_int)]
+    L.sdf_compute_zslab.restype = C.c_int
     L.sdf_compute_host.restype = C.c_int
     L.sdf_closest_points.argtypes = [vp, C.POINTER(C.c_float), C.c_float, C.c_int, C.c_int, C.c_int, vp, vp, vp]
     L.sdf_closest_points.restype = C.c_int
@@ -269,6 +274,35 @@ def sdf_compute_host(mesh: Mesh, origin, h, dims, band, dist_out=None, tri_out=N
     if st != SDF_OK:
         raise SdfError(st, "sdf_compute_host")
     return dist_out, tri_out
+
+
+def sdf_zslab(nz, part, parts):
+    """(k0, nk): z-slab `part` of `parts` of a grid of nz slices (host only, no CUDA)."""
+    k0, nk = C.c_int(0), C.c_int(0)
+    st = lib().sdf_zslab(int(nz), int(part), int(parts), C.byref(k0), C.byref(nk))
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_zslab")
+    return k0.value, nk.value
+
+
+def sdf_compute_zslab(mesh: Mesh, origin, h, dims, band, part, parts, dist_out=None, tri_out=None, stream=None):
+    """Slab `part` of `parts` of the grid: returns (k0, dist [nk,ny,nx], tri [nk,ny,nx]) CUDA tensors."""
+    torch = _torch()
+    nx, ny, nz = (int(v) for v in dims)
+    k0, nk = sdf_zslab(nz, part, parts)
+    if dist_out is None:
+        dist_out = torch.empty((nk, ny, nx), dtype=torch.float32, device="cuda")
+    if tri_out is None:
+        tri_out = torch.empty((nk, ny, nx), dtype=torch.int32, device="cuda")
+    assert dist_out.is_cuda and tri_out.is_cuda and dist_out.is_contiguous() and tri_out.is_contiguous()
+    assert dist_out.numel() == nx * ny * nk and tri_out.numel() == nx * ny * nk
+    assert dist_out.dtype == torch.float32 and tri_out.dtype == torch.int32
+    st = lib().sdf_compute_zslab(mesh.handle, _origin3(origin), float(h), nx, ny, nz, float(band), int(part), int(parts),
+                                 C.c_void_p(dist_out.data_ptr()), C.c_void_p(tri_out.data_ptr()),
+                                 C.c_void_p(_stream_ptr(stream)), None, None)
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_compute_zslab")
+    return k0, dist_out, tri_out
 
 
 def sdf_closest_points(mesh: Mesh, origin, h, dims, tri, cp_out=None, stream=None):

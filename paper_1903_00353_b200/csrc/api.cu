@@ -180,6 +180,29 @@ int sdf_compute(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int
     return s;
 }
 
+int sdf_zslab(int nz, int part, int parts, int *k0, int *nk) {
+    if (!k0 || !nk || nz < 1 || parts < 1 || part < 0 || part >= parts) return SDF_EINVAL;
+    const int64_t nb = ((int64_t)nz + BRICK - 1) / BRICK;          // slabs are whole bricks high
+    int64_t a = nb * part / parts * BRICK, b = nb * ((int64_t)part + 1) / parts * BRICK;
+    if (a > nz) a = nz;
+    if (b > nz) b = nz;
+    *k0 = (int)a;
+    *nk = (int)(b - a);
+    return SDF_OK;
+}
+
+int sdf_compute_zslab(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz, float band, int part,
+                      int parts, float *dist_out, int32_t *tri_out, void *stream, int *k0_out, int *nk_out) {
+    if (!m || !origin) return SDF_EINVAL;
+    int k0 = 0, nk = 0;
+    CKS(sdf_zslab(nz, part, parts, &k0, &nk));
+    if (k0_out) *k0_out = k0;
+    if (nk_out) *nk_out = nk;
+    if (nk == 0) return SDF_OK;
+    const float o[3] = {origin[0], origin[1], (float)((double)origin[2] + (double)k0 * (double)h)};
+    return sdf_compute(m, o, h, nx, ny, nk, band, dist_out, tri_out, stream);
+}
+
 int sdf_closest_points(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz, const int32_t *tri_in,
                        float *cp_out, void *stream) {
     if (!m || !tri_in || !cp_out) return SDF_EINVAL;
