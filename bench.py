@@ -388,7 +388,7 @@ def run_ours(args):
             t_wall * 1e3 / args.steps, "roofline": roofline, "roofline_step": roofline_step, "cpu_baseline": cpu,
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "zslab": zslab, "fill_interior": fill_int, "closest_points": cpt,
             "stats": {k: stats[k] for k in ("polyhedra", "work_items", "pairs_tested", "pairs_accepted",
-                                            "bricks_active", "fp64_rechecks")}}
+                                            "bricks_active", "fp64_rechecks", "cdp_fallbacks")}}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -23,7 +23,7 @@
  * state for the first time (the first sdf_create / sdf_compute of a process create the library's
  * side streams: vertex stage, sentinel fill); distinct handles on distinct streams are otherwise independent.
  * Debug / ablation switches (environment, read per call): SDF_AABB_MODE=1 (candidates = band-expanded
- * triangle boxes only), SDF_FILL_MODE=0..4, SDF_SCHEDULER=serial, SDF_RUFF=cone, SDF_NO_BINNING=1,
+ * triangle boxes only), SDF_FILL_MODE=0..4, SDF_SCHEDULER=serial | dynamic[:N], SDF_RUFF=cone, SDF_NO_BINNING=1,
  * SDF_CREATE_FORK=0 (vertex stage on the caller's stream);
  * see DESIGN.md.
  */
@@ -80,6 +80,8 @@ typedef struct sdf_stats_t {
     int64_t band_cells;                   /* populated output cells                             */
     int64_t fp64_rechecks;                /* cells whose band / sign decision was redone in fp64 */
                                           /* (cells without a certain sign from their candidate) */
+    int64_t cdp_fallbacks;                /* SDF_SCHEDULER=dynamic only: child launches the device    */
+                                          /* runtime refused (their volumes were walked serially)     */
 } sdf_stats_t;
 
 /*

@@ -60,7 +60,7 @@ class Stats(C.Structure):
         "F", "V", "E", "edges_convex", "edges_concave", "edges_flat",
         "verts_pos_only", "verts_neg_only", "verts_both", "verts_skipped", "verts_hemisphere",
         "weld_collisions", "polyhedra", "work_items", "pairs_tested", "pairs_accepted",
-        "bricks_active", "bricks_total", "band_cells", "fp64_rechecks")]
+        "bricks_active", "bricks_total", "band_cells", "fp64_rechecks", "cdp_fallbacks")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}

@@ -15,9 +15,11 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libsdf_b200.so")
 SOURCES = ["api.cu", "features.cu", "compute.cu", "fill.cu", "stl_io.cu"]
-HEADERS = ["common.cuh", "primitives.cuh", os.path.join("..", "..", "include", "sdf.h")]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared", "--cudart", "static"]
+RDC_SOURCES = ["cdp.cu"]          # device-side launches (the dynamic-parallelism ablation): relocatable device code
+HEADERS = ["common.cuh", "primitives.cuh", "evaluate.cuh", os.path.join("..", "..", "include", "sdf.h")]
+ARCH_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a"]
+NVCC_FLAGS = ARCH_FLAGS + ["-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
+LINK_FLAGS = ARCH_FLAGS + ["-shared", "-Xcompiler", "-fPIC", "--cudart", "static", "-lcudadevrt"]
 
 
 def _nvcc() -> str:
@@ -32,8 +34,8 @@ def source_hash() -> str:
     snapshot copy to the GPU box)."""
     import hashlib
     h = hashlib.sha256()
-    h.update(" ".join(NVCC_FLAGS).encode())
-    for s in SOURCES + HEADERS:
+    h.update(" ".join(NVCC_FLAGS + LINK_FLAGS).encode())
+    for s in SOURCES + RDC_SOURCES + HEADERS:
         with open(os.path.join(CSRC, s), "rb") as f:
             h.update(f.read())
     return h.hexdigest()
@@ -49,9 +51,21 @@ def needs_build() -> bool:
 def build_library(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return LIB
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-          ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
-    subprocess.check_call(cmd)
+    # one object per source (compiled side by side), cdp.cu alone as relocatable device code; the
+    # final nvcc link runs the device link for it and leaves the other objects as they are
+    import tempfile
+    extra = ["-Xptxas", "-v"] if verbose else []
+    with tempfile.TemporaryDirectory(prefix="sdf_b200_build_") as tmp:
+        jobs, objs = [], []
+        for s in SOURCES + RDC_SOURCES:
+            obj = os.path.join(tmp, os.path.splitext(s)[0] + ".o")
+            rdc = ["-rdc=true"] if s in RDC_SOURCES else []
+            jobs.append(subprocess.Popen([_nvcc()] + NVCC_FLAGS + rdc + extra + ["-c", os.path.join(CSRC, s), "-o", obj]))
+            objs.append(obj)
+        rcs = [j.wait() for j in jobs]
+        if any(rcs):
+            raise subprocess.CalledProcessError(max(rcs), "nvcc -c")
+        subprocess.check_call([_nvcc()] + LINK_FLAGS + ["-o", LIB] + objs)
     with open(LIB + ".hash", "w") as f:
         f.write(source_hash())
     return LIB

@@ -158,6 +158,9 @@ static int make_grid(const float origin[3], float h, int nx, int ny, int nz, flo
     g->plain_cpt = (pc && pc[0] == '1') ? 1 : 0;
     const char *sc = getenv("SDF_SCHEDULER");
     g->serial_loop = (sc && !strcmp(sc, "serial")) ? 1 : 0;
+    g->cdp = (sc && !strncmp(sc, "dynamic", 7) && (sc[7] == 0 || sc[7] == ':')) ? 1 : 0;
+    g->cdp_serial_below = (g->cdp && sc[7] == ':') ? atoi(sc + 8) : 0;
+    if (g->cdp_serial_below < 0) g->cdp_serial_below = 0;
     const char *fp = getenv("SDF_FILL_PRIO");
     g->fill_prio = fp ? (fp[0] == '1') : 1;
     const char *fl = getenv("SDF_FILL_CTAS");
@@ -261,6 +264,7 @@ int sdf_stats(sdf_mesh *m, sdf_stats_t *o) {
     o->bricks_active = (int64_t)c[CTR_BRICKS];
     o->bricks_total = m->last_bricks_total;
     o->band_cells = (int64_t)c[CTR_BAND]; o->fp64_rechecks = (int64_t)c[CTR_RECHECK];
+    o->cdp_fallbacks = (int64_t)c[CTR_CDP_FALLBACK];
     return SDF_OK;
 }
 

@@ -39,7 +39,7 @@ enum {
     CTR_V = 0, CTR_RESERVED1, CTR_E_CONVEX, CTR_E_CONCAVE, CTR_E_FLAT,
     CTR_V_POS, CTR_V_NEG, CTR_V_BOTH, CTR_V_SKIP, CTR_V_HEMI,
     CTR_POLY, CTR_ITEMS, CTR_BRICKS, CTR_TESTED, CTR_ACCEPTED, CTR_BAND, CTR_RECHECK,
-    CTR_BIG, CTR_RESERVED2,      // big-polyhedron list: length (the fetch cursors are CTR_BIGCUR)
+    CTR_BIG, CTR_CDP_FALLBACK,   // big-polyhedron list length (fetch cursors: CTR_BIGCUR); refused child launches (cdp.cu)
     CTR_COUNT = 24,
     // statistics that every warp adds to are spread over CTR_SLOTS lines of 8 counters
     // (same-address atomics serialise in L2); sdf_stats sums the slots
@@ -96,6 +96,7 @@ struct GridParams {
     int big_rows, big_ni;           // polyhedra with more rows / longer rows go to evaluate_big_kernel
     int plain_cpt;                  // debug: closest points with the dense one-pass kernel only
     int serial_loop;                // ablation: the paper's thread-per-extrusion serial loop
+    int cdp, cdp_serial_below;      // ablation: the paper's dynamic-parallelism scheduler (cdp.cu)
     int aabb_mode;                  // debug: candidates = band-expanded triangle AABBs only
     int vec4;                       // 1: nx % 4 == 0 and outputs 16-B aligned -> 128-bit stores
     int fill_mode;                  // 0: TMA fill on the side stream (default); debug: 1 plain stores on the

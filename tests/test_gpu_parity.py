@@ -340,6 +340,27 @@ def test_serial_scheduler_ablation(oracle_mod, monkeypatch):
         assert float((d0[pop] == d1[pop]).float().mean()) > 0.999
 
 
+@pytest.mark.parametrize("mode", ["dynamic", "dynamic:64"])
+def test_dynamic_parallelism_ablation(oracle_mod, monkeypatch, mode):
+    """SDF_SCHEDULER=dynamic[:N] (the paper's device-side child grids, one thread per bounding-volume cell,
+    PAPER.md:376-380; N = hybrid threshold) meets the same four parity clauses and agrees
+    with the flattened scan converter as the serial ablation does."""
+    import torch
+    from paper_1903_00353_b200 import binding as B
+    for w in (f32_grid(W.config("C1")), f32_grid(W.config("C2", 0.5)),
+              f32_grid(_small(W.ruff_mesh(), 16, n=44, band_cells=5))):
+        m = B.sdf_create(w.soup)
+        d0, t0 = B.sdf_compute(m, w.origin, w.h, w.dims, w.band)
+        monkeypatch.setenv("SDF_SCHEDULER", mode)
+        _assert_ok(check_parity(w, oracle_mod))
+        d1, t1 = B.sdf_compute(m, w.origin, w.h, w.dims, w.band)
+        monkeypatch.delenv("SDF_SCHEDULER")
+        pop = torch.isfinite(d0)
+        assert torch.equal(pop, torch.isfinite(d1))
+        assert float((d0[pop] - d1[pop]).abs().max()) <= 1e-7
+        assert float((d0[pop] == d1[pop]).float().mean()) > 0.999
+
+
 def test_permutation_invariance():
     """Shuffling the soup permutes ids and leaves distances / signs bit-identical (the packed
     atomicMin is order independent)."""
