@@ -330,7 +330,7 @@ def run_ours(args):
         fb = 4.0 * N + 4.0 * filled                       # read every cell once, write the interior once
         fill_int = {"ms": min(tms), "cells_filled": filled, "algorithmic_bytes": fb,
                     "achieved_gbs": fb / (min(tms) * 1e-3) / 1e9, "bound": "hbm",
-                    "note": "three in-place sweeps: x reads the grid once, y and z twice"}
+                    "note": "three in-place sweeps: x reads the grid, y and z skip the 32-cell segments x left blank"}
         del keep
 
     # ---- SURVEY.md 8(f) NEXT-2 (not part of the step): closest points of the last result

@@ -24,7 +24,7 @@
  * side streams: vertex stage, sentinel fill); distinct handles on distinct streams are otherwise independent.
  * Debug / ablation switches (environment, read per call): SDF_AABB_MODE=1 (candidates = band-expanded
  * triangle boxes only), SDF_FILL_MODE=0..4, SDF_SCHEDULER=serial | dynamic[:N], SDF_RUFF=cone, SDF_NO_BINNING=1,
- * SDF_CREATE_FORK=0 (vertex stage on the caller's stream);
+ * SDF_CREATE_FORK=0 (vertex stage on the caller's stream), SDF_FILLINT_PLAIN=1 (interior fill without the blank map);
  * see DESIGN.md.
  */
 #ifndef PAPER_1903_00353_SDF_H
@@ -197,7 +197,10 @@ int sdf_closest_points(sdf_mesh *m, const float origin[3], float h, int nx, int 
  *   dist      DEVICE, nx*ny*nz floats, layout of sdf_compute (x fastest)
  *   band      the band width sdf_compute was called with (the value written is -band)
  *   stream    cudaStream_t; the three sweeps are enqueued on it, nothing is synchronised
- * Errors: SDF_EINVAL, SDF_ECUDA.
+ * Scratch: nx*ny*nz/128 bytes (one bit per 32-cell row segment, twice) from the device's default
+ * memory pool with cudaMallocAsync / cudaFreeAsync on `stream`; the pool's release threshold is
+ * raised to that size if it is lower (the one process-wide setting the library changes).
+ * Errors: SDF_EINVAL, SDF_ENOMEM, SDF_ECUDA.
  */
 int sdf_fill_interior(float *dist, int nx, int ny, int nz, float band, void *stream);
 

@@ -9,6 +9,7 @@
 // HBM-bound: 4 B per cell read per sweep, the interior written once.
 #include "common.cuh"
 #include <math.h>
+#include <stdlib.h>
 
 // ---- x: one warp per row; a chunk of 32 cells is resolved with two ballots
 __device__ __forceinline__ int state_from_left(unsigned set, unsigned neg, int lane, int carry) {
@@ -24,18 +25,31 @@ __device__ __forceinline__ int state_from_right(unsigned set, unsigned neg, int 
     return ((neg >> b) & 1u) ? -1 : 1;
 }
 
-#define SX_BATCH 8       // chunks of 32 cells loaded before they are resolved (memory-level parallelism)
+#define SX_BATCH 4       // chunks of 32 cells loaded before they are resolved (memory-level parallelism)
 // One walk per row (see sweep_line_kernel for why one is enough).  A chunk of 32 cells is resolved
 // with two ballots: an unset cell is filled if the nearest set cell to its left (in the chunk, else
 // the carry) or to its right IN THE CHUNK is negative; unset cells with no set cell to their right
 // in the chunk join the pending run, which the first set cell of a later chunk resolves (the warp
 // then fills the earlier chunks' part of the run with coalesced stores).
-__global__ void __launch_bounds__(256) sweep_x_kernel(float *__restrict__ dist, int nx, int64_t nrows, float fillv) {
+//
+// Blank map: the walk also records which 32-cell segments of its row are still entirely unset when it
+// is done (bit s of word w of the row = segment 32 w + s), once in the order of the y walk and once in
+// the order of the z walk.  Most of a grid is such segments -- everything
+// outside the band on the outside -- and the y and z walks need not read them (sweep_line_kernel).
+__device__ __forceinline__ unsigned chunk_mask(int lane, int a, int b) {      // bits of chunks [a, b) in word `lane`
+    const int lo = max(a, 32 * lane), hi = min(b, 32 * lane + 32);
+    return lo < hi ? (0xFFFFFFFFu >> (32 - (hi - lo))) << (lo - 32 * lane) : 0u;
+}
+
+__global__ void __launch_bounds__(256, 8) sweep_x_kernel(float *__restrict__ dist, int nx, int64_t nrows, float fillv,
+                                                      unsigned *__restrict__ blank_y, unsigned *__restrict__ blank_z,
+                                                      int nwords, int ny, int nz) {
     const int lane = threadIdx.x & 31;
     const int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
     if (row >= nrows) return;
     float *d = dist + row * nx;
     int carry = 0, run = -1;
+    unsigned bits = 0;           // lane l: word l of the row's blank map
     for (int base = 0; base < nx; base += 32 * SX_BATCH) {
         float v[SX_BATCH];
 #pragma unroll
@@ -48,21 +62,39 @@ __global__ void __launch_bounds__(256) sweep_x_kernel(float *__restrict__ dist, 
             const int cb = base + 32 * u, i = cb + lane;
             if (cb >= nx) break;
             const bool set = i < nx && isfinite(v[u]);
-            const unsigned ms = __ballot_sync(0xffffffffu, set), mn = __ballot_sync(0xffffffffu, set && v[u] < 0.0f);
+            const unsigned ms = __ballot_sync(0xffffffffu, set);
+            const int c = cb >> 5;
+            if (!ms) {
+                // no set cell in the chunk (most of a grid): filled at once when the walk is inside,
+                // else part of the pending run and, so far, blank
+                if (carry < 0) {
+                    if (i < nx) d[i] = fillv;
+                } else {
+                    if (run < 0) run = cb;
+                    if (lane == (c >> 5)) bits |= 1u << (c & 31);
+                }
+                continue;
+            }
+            const unsigned mn = __ballot_sync(0xffffffffu, set && v[u] < 0.0f);
             const int sl = state_from_left(ms, mn, lane, carry), sr = state_from_right(ms, mn, lane, 0);
             if (i < nx && !set && (sl < 0 || sr < 0)) d[i] = fillv;
-            if (ms) {
-                // the first set cell of the chunk decides the run pending from earlier chunks
-                if (run >= 0 && ((mn >> (__ffs(ms) - 1)) & 1u))
-                    for (int x = run + lane; x < cb; x += 32) d[x] = fillv;
-                run = -1;
+            // the first set cell of the chunk decides the run pending from earlier chunks
+            if (run >= 0 && ((mn >> (__ffs(ms) - 1)) & 1u)) {
+                for (int x = run + lane; x < cb; x += 32) d[x] = fillv;
+                bits &= ~chunk_mask(lane, run >> 5, c);                   // the pending chunks were filled after all
             }
-            carry = state_from_left(ms, mn, 31, carry);
-            if (carry >= 0 && run < 0) {
-                const int start = cb + (ms ? 32 - __clz(ms) : 0);       // first cell after the last set one
+            run = -1;
+            carry = ((mn >> (31 - __clz(ms))) & 1u) ? -1 : 1;             // the last set cell of the chunk
+            if (carry >= 0) {
+                const int start = cb + 32 - __clz(ms);                    // first cell after the last set one
                 if (start < min(nx, cb + 32)) run = start;
             }
         }
+    }
+    if (blank_y && lane < nwords) {
+        const int64_t k = row / ny, j = row - k * ny;
+        blank_y[(k * nwords + lane) * ny + j] = bits;        // along y for the y walk
+        blank_z[(j * nwords + lane) * nz + k] = bits;        // along z for the z walk
     }
 }
 
@@ -73,31 +105,68 @@ __global__ void __launch_bounds__(256) sweep_x_kernel(float *__restrict__ dist, 
 // unless that cell was filled by the same forward walk).  So the walk fills an unset cell at once
 // when the last set cell was negative, and otherwise remembers where the unset run began and fills
 // it when the next set cell turns out to be negative -- writes only, no second read of the line.
+//
+// The 32 lines of a warp share their 32-cell segment of every row, so the blank map says per (warp, row)
+// whether the 32 cells are all unset: then they are not read (the walk of an unset cell needs no data).
+// `mine` is the map laid out along this sweep's walk (word q of the line's run), fetched 32 rows at a
+// time -- lane l takes row q0 + l, one ballot turns the 32 words into the skip mask of the warp.  A lane
+// that fills a cell of a blank segment clears the bit in `next`, the map of the following sweep; that
+// never happens on a well-resolved surface, where the x walk has already filled the whole interior.
 #define SL_BATCH 8
-__global__ void __launch_bounds__(256) sweep_line_kernel(float *__restrict__ dist, int nx, int64_t nlines_outer,
-                                                         int64_t outer_stride, int n, int64_t stride, float fillv) {
-    const int i = blockIdx.x * 256 + threadIdx.x;
+__global__ void __launch_bounds__(256, 8) sweep_line_kernel(float *__restrict__ dist, int nx, int64_t outer_stride, int n,
+                                                            int64_t stride, float fillv, int nwords,
+                                                            const unsigned *__restrict__ mine,
+                                                            unsigned *__restrict__ next, int64_t next_stride) {
+    const int i = blockIdx.x * 256 + threadIdx.x, lane = threadIdx.x & 31;
     const int64_t o = blockIdx.y;
-    if (i >= nx || o >= nlines_outer) return;
+    const bool valid = i < nx;                  // lanes past the row end walk along, unset and silent
     float *d = dist + o * outer_stride + i;
+    const int w = i >> 10;
+    const unsigned bbit = 1u << ((i >> 5) & 31);
+    if (mine) mine += (o * nwords + w) * (int64_t)n;
+    if (next) next += (int64_t)w * (next_stride / nwords) + o;       // word of row (o, q): next[q * next_stride]
     int state = 0, run = -1;                 // run: first cell of the pending unset run, -1 = none
-    for (int q0 = 0; q0 < n; q0 += SL_BATCH) {
-        float v[SL_BATCH];
+    unsigned ahead = (mine && lane < n) ? mine[lane] : 0u;
+    for (int q32 = 0; q32 < n; q32 += 32) {
+        const unsigned skipmask = __ballot_sync(0xffffffffu, (ahead & bbit) != 0u);
+        ahead = (mine && q32 + 32 + lane < n) ? mine[q32 + 32 + lane] : 0u;
+        const int qe = min(n, q32 + 32);
+        if (skipmask == 0xffffffffu >> (32 - (qe - q32))) {
+            // 32 blank rows: nothing to read, and (unless the walk is inside) nothing to write
+            if (valid && state < 0) {
+                for (int r = q32; r < qe; r++) {
+                    d[(int64_t)r * stride] = fillv;
+                    if (next) atomicAnd(&next[r * next_stride], ~bbit);
+                }
+            } else if (valid && run < 0) {
+                run = q32;
+            }
+            continue;
+        }
+        for (int q0 = q32; q0 < qe; q0 += SL_BATCH) {
+            float v[SL_BATCH];
 #pragma unroll
-        for (int u = 0; u < SL_BATCH; u++) v[u] = (q0 + u < n) ? d[(int64_t)(q0 + u) * stride] : INFINITY;
+            for (int u = 0; u < SL_BATCH; u++)
+                v[u] = (valid && q0 + u < qe && !((skipmask >> (q0 + u - q32)) & 1u)) ? d[(int64_t)(q0 + u) * stride] : INFINITY;
 #pragma unroll
-        for (int u = 0; u < SL_BATCH; u++) {
-            const int q = q0 + u;
-            if (q >= n) break;
-            if (isfinite(v[u])) {
-                state = v[u] < 0.0f ? -1 : 1;
-                if (state < 0 && run >= 0)
-                    for (int r = run; r < q; r++) d[(int64_t)r * stride] = fillv;
-                run = -1;
-            } else if (state < 0) {
-                d[(int64_t)q * stride] = fillv;
-            } else if (run < 0) {
-                run = q;
+            for (int u = 0; u < SL_BATCH; u++) {
+                const int q = q0 + u;
+                if (q >= qe) break;
+                if (isfinite(v[u])) {
+                    state = v[u] < 0.0f ? -1 : 1;
+                    if (state < 0 && run >= 0)
+                        for (int r = run; r < q; r++) {
+                            d[(int64_t)r * stride] = fillv;
+                            if (next && (next[r * next_stride] & bbit)) atomicAnd(&next[r * next_stride], ~bbit);
+                        }
+                    run = -1;
+                } else if (!valid) {
+                } else if (state < 0) {
+                    d[(int64_t)q * stride] = fillv;
+                    if (next && ((skipmask >> (q - q32)) & 1u)) atomicAnd(&next[q * next_stride], ~bbit);
+                } else if (run < 0) {
+                    run = q;
+                }
             }
         }
     }
@@ -111,12 +180,39 @@ extern "C" int sdf_fill_interior(float *dist, int nx, int ny, int nz, float band
     cudaStream_t st = (cudaStream_t)stream;
     const float fillv = -band;
     const int64_t nrows = (int64_t)ny * nz;
-    KL; sweep_x_kernel<<<(unsigned)((nrows + 7) / 8), 256, 0, st>>>(dist, nx, nrows, fillv);
-    // y: lines (i, k), cells nx apart;  z: lines (i, j), cells nx*ny apart
+    // blank maps: one bit per 32-cell segment, in y order and in z order (2/1024 of the grid),
+    // stream-ordered scratch
+    const int nwords = ((nx + 31) / 32 + 31) / 32;
+    const size_t mapw = (size_t)nrows * nwords;
+    unsigned *blank = nullptr;
+    const char *pl = getenv("SDF_FILLINT_PLAIN");            // debug: every walk reads every cell
+    if (!(pl && pl[0] == '1')) {
+        // the maps come from the device's default memory pool; by default that pool hands everything back
+        // to the driver at the next synchronisation and the allocation alone would cost more than the
+        // sweeps: let it keep as much as the maps need (the one process-wide setting this call touches)
+        const size_t need = sizeof(unsigned) * 2 * mapw;
+        int dev = 0;
+        cudaMemPool_t pool;
+        CK(cudaGetDevice(&dev));
+        CK(cudaDeviceGetDefaultMemPool(&pool, dev));
+        unsigned long long keep = 0;
+        CK(cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+        if (keep < need) {
+            keep = need;
+            CK(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+        }
+        CK(cudaMallocAsync((void **)&blank, need, st));
+    }
+    unsigned *by = blank, *bz = blank ? blank + mapw : nullptr;
+    KL; sweep_x_kernel<<<(unsigned)((nrows + 7) / 8), 256, 0, st>>>(dist, nx, nrows, fillv, by, bz, nwords, ny, nz);
+    // y: lines (i, k), cells nx apart;  z: lines (i, j), cells nx*ny apart.  A cell (j, k) filled by
+    // the y walk clears word (j * nwords + w) * nz + k of the z map
     KL; sweep_line_kernel<<<dim3((unsigned)((nx + 255) / 256), (unsigned)nz), 256, 0, st>>>(
-        dist, nx, nz, (int64_t)nx * ny, ny, nx, fillv);
+        dist, nx, (int64_t)nx * ny, ny, nx, fillv, nwords, by, bz, (int64_t)nwords * nz);
     KL; sweep_line_kernel<<<dim3((unsigned)((nx + 255) / 256), (unsigned)ny), 256, 0, st>>>(
-        dist, nx, ny, nx, nz, (int64_t)nx * ny, fillv);
-    CK(cudaGetLastError());
+        dist, nx, nx, nz, (int64_t)nx * ny, fillv, nwords, bz, nullptr, 0);
+    cudaError_t e = cudaGetLastError();
+    if (blank) cudaFreeAsync(blank, st);
+    CK(e);
     return SDF_OK;
 }

@@ -36,18 +36,24 @@ def test_fill_matches_oracle(oracle_mod, name, scale):
     assert np.all(t.cpu().numpy()[filled] == -1)
 
 
-@pytest.mark.parametrize("dims", [(37, 29, 43), (1, 1, 70), (65, 1, 3), (33, 64, 1), (200, 7, 5), (700, 3, 2), (31, 300, 2), (5, 2, 290)])
-def test_fill_arbitrary_grids(oracle_mod, dims):
-    """Random sparse grids (not SDFs): ragged sizes, lines of length 1, runs that start and end unset."""
+@pytest.mark.parametrize("dims", [(37, 29, 43), (1, 1, 70), (65, 1, 3), (33, 64, 1), (200, 7, 5), (700, 3, 2), (31, 300, 2), (5, 2, 290),
+                                  (1100, 5, 40), (2100, 3, 35), (70, 45, 100), (40, 100, 37), (96, 64, 64)])
+def test_fill_arbitrary_grids(oracle_mod, monkeypatch, dims):
+    """Random sparse grids (not SDFs): ragged sizes, lines of length 1, runs that start and end unset; rows wider
+    than one word of the blank map (1024 cells), lines longer than one 32-row block of it, and densities so low
+    that the y and z walks fill whole blank segments (the map of the next sweep must follow)."""
     nx, ny, nz = dims
     rng = np.random.default_rng(nx * 1000 + ny * 10 + nz)
     d = np.full((nz, ny, nx), np.inf, dtype=np.float32)
-    for density in (0.002, 0.08, 0.5):
+    for density in (0.0002, 0.002, 0.08, 0.5):
         d[:] = np.inf
         sel = rng.random(d.shape) < density
         d[sel] = rng.standard_normal(int(sel.sum())).astype(np.float32)
         ref = oracle_mod.fill_interior(d, 0.75)
         assert np.array_equal(_gpu_fill(d, 0.75), ref)
+        monkeypatch.setenv("SDF_FILLINT_PLAIN", "1")              # every walk reads every cell: same result
+        assert np.array_equal(_gpu_fill(d, 0.75), ref)
+        monkeypatch.delenv("SDF_FILLINT_PLAIN")
 
 
 def test_fill_full_size_c3(oracle_mod):
