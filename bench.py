@@ -38,7 +38,7 @@ METRIC = "narrow_band_sdf_cells_per_s"
 UNIT = "band cells/s"
 L2_BYTES = 126 * 1024 * 1024
 # dram__bytes_read.sum + dram__bytes_write.sum of fill_tma_kernel at C4 (profiles/r1_final_ncu_full.md)
-NCU_FILL_TRAFFIC_C4 = 0.070912e6 + 8.530324e9
+NCU_FILL_TRAFFIC_C4 = 0.185088e6 + 8.531763e9
 
 
 # --------------------------------------------------------------------------------------- #
