@@ -199,7 +199,8 @@ int sdf_closest_points(sdf_mesh *m, const float origin[3], float h, int nx, int 
  *   stream    cudaStream_t; the three sweeps are enqueued on it, nothing is synchronised
  * Scratch: nx*ny*nz/128 bytes (one bit per 32-cell row segment, twice) from the device's default
  * memory pool with cudaMallocAsync / cudaFreeAsync on `stream`; the pool's release threshold is
- * raised to that size if it is lower (the one process-wide setting the library changes).
+ * raised to twice that size plus 64 MiB if it is lower (the one process-wide setting the library
+ * changes; the pool reserves in chunks and would otherwise hand them back at every synchronisation).
  * Errors: SDF_EINVAL, SDF_ENOMEM, SDF_ECUDA.
  */
 int sdf_fill_interior(float *dist, int nx, int ny, int nz, float band, void *stream);

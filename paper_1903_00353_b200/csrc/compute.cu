@@ -825,31 +825,46 @@ __global__ void __launch_bounds__(256) closest_points_kernel(MeshView mv, GridPa
 }
 
 // After a TMA fill of the whole output with +inf: only the cells of the band are visited for real.
-// A block streams CPS_LOADS * 256 int4 of ids (all loads issued before any is looked at); the few
-// quads that hold a band cell are handled in a rolled loop so the streaming part stays small.
+// A block streams CPS_LOADS * 256 int4 of ids (all loads issued before any is looked at) and queues the
+// band cells it meets (0.5 % of a grid, in clusters) in shared memory; the queue is then worked off a
+// thread per entry, so the expensive part -- gathers and the seven-region routine -- runs on full warps
+// instead of on the odd lane of a streaming warp.
 #define CPS_LOADS 4
+#define CPS_CELLS (256 * CPS_LOADS * 4)
 __global__ void __launch_bounds__(256) closest_points_sparse_kernel(MeshView mv, GridParams g, const int *__restrict__ tri,
                                                                     float *__restrict__ cp, int64_t n4) {
-    const int64_t q0 = (int64_t)blockIdx.x * (256 * CPS_LOADS) + threadIdx.x;      // in units of int4
+    __shared__ int s_n;
+    __shared__ unsigned short s_cell[CPS_CELLS];       // cell index within the block's range
+    __shared__ int s_tri[CPS_CELLS];
+    if (threadIdx.x == 0) s_n = 0;
+    const int64_t qb = (int64_t)blockIdx.x * (256 * CPS_LOADS);       // in units of int4
     const int64_t nq = n4 >> 2;
     int4 t4[CPS_LOADS];
 #pragma unroll
     for (int u = 0; u < CPS_LOADS; u++) {
-        const int64_t q = q0 + (int64_t)u * 256;
+        const int64_t q = qb + u * 256 + threadIdx.x;
         t4[u] = q < nq ? __ldcs((const int4 *)tri + q) : make_int4(-1, -1, -1, -1);
     }
-#pragma unroll 1
+    __syncthreads();
+#pragma unroll
     for (int u = 0; u < CPS_LOADS; u++) {
-        if ((t4[u].x & t4[u].y & t4[u].z & t4[u].w) < 0 && t4[u].x < 0 && t4[u].y < 0 && t4[u].z < 0 && t4[u].w < 0) continue;
-        const int64_t c = (q0 + (int64_t)u * 256) * 4;
         const int xt[4] = {t4[u].x, t4[u].y, t4[u].z, t4[u].w};
-#pragma unroll 1
+        if ((xt[0] & xt[1] & xt[2] & xt[3]) < 0) continue;            // all four negative: no band cell
+#pragma unroll
         for (int e = 0; e < 4; e++)
             if (xt[e] >= 0) {
-                float o[3];
-                closest_point_of(mv, g, xt[e], c + e, o);
-                cp[3 * (c + e)] = o[0]; cp[3 * (c + e) + 1] = o[1]; cp[3 * (c + e) + 2] = o[2];
+                const int k = atomicAdd(&s_n, 1);
+                s_cell[k] = (unsigned short)((u * 256 + threadIdx.x) * 4 + e);
+                s_tri[k] = xt[e];
             }
+    }
+    __syncthreads();
+    const int nk = s_n;
+    for (int k = threadIdx.x; k < nk; k += 256) {
+        const int64_t c = qb * 4 + s_cell[k];
+        float o[3];
+        closest_point_of(mv, g, s_tri[k], c, o);
+        cp[3 * c] = o[0]; cp[3 * c + 1] = o[1]; cp[3 * c + 2] = o[2];
     }
 }
 

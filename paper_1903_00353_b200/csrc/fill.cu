@@ -50,12 +50,45 @@ __global__ void __launch_bounds__(256, 8) sweep_x_kernel(float *__restrict__ dis
     float *d = dist + row * nx;
     int carry = 0, run = -1;
     unsigned bits = 0;           // lane l: word l of the row's blank map
+    const bool vec = (nx & 3) == 0 && (((size_t)dist) & 15) == 0;      // every row starts on 16 bytes
     for (int base = 0; base < nx; base += 32 * SX_BATCH) {
+        if (vec && base + 32 * SX_BATCH <= nx) {
+            // a whole batch without a set cell (most of a grid) is settled from one 128-bit load per lane;
+            // otherwise the cells are loaded again the way the chunk logic wants them (from L1)
+            static_assert(SX_BATCH == 4, "one float4 per lane covers the batch");
+            float4 *qp = reinterpret_cast<float4 *>(d + base) + lane;
+            const float4 q = *qp;
+            const bool any = isfinite(q.x) || isfinite(q.y) || isfinite(q.z) || isfinite(q.w);
+            if (!__any_sync(0xffffffffu, any)) {
+                if (carry < 0) {
+                    *qp = make_float4(fillv, fillv, fillv, fillv);
+                } else {
+                    if (run < 0) run = base;
+                    if (lane == (base >> 10)) bits |= 0xFu << ((base >> 5) & 31);
+                }
+                continue;
+            }
+        }
         float v[SX_BATCH];
 #pragma unroll
         for (int u = 0; u < SX_BATCH; u++) {
             const int i = base + 32 * u + lane;
             v[u] = i < nx ? d[i] : INFINITY;
+        }
+        // a whole batch without a set cell (most of a grid) is settled at once
+        bool any = false;
+#pragma unroll
+        for (int u = 0; u < SX_BATCH; u++) any |= isfinite(v[u]);
+        if (!__any_sync(0xffffffffu, any)) {
+            const int nch = min(SX_BATCH, (nx - base + 31) >> 5), c0 = base >> 5;      // c0 is a multiple of SX_BATCH
+            if (carry < 0) {
+                for (int u = 0; u < nch; u++)
+                    if (base + 32 * u + lane < nx) d[base + 32 * u + lane] = fillv;
+            } else {
+                if (run < 0) run = base;
+                if (lane == (c0 >> 5)) bits |= ((1u << nch) - 1u) << (c0 & 31);
+            }
+            continue;
         }
 #pragma unroll
         for (int u = 0; u < SX_BATCH; u++) {
@@ -197,8 +230,8 @@ extern "C" int sdf_fill_interior(float *dist, int nx, int ny, int nz, float band
         CK(cudaDeviceGetDefaultMemPool(&pool, dev));
         unsigned long long keep = 0;
         CK(cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
-        if (keep < need) {
-            keep = need;
+        if (keep < 2 * need + (64ull << 20)) {           // the pool reserves in chunks larger than the request
+            keep = 2 * need + (64ull << 20);
             CK(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
         }
         CK(cudaMallocAsync((void **)&blank, need, st));
