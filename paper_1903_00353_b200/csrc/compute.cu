@@ -782,6 +782,33 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
 // the band.  HBM-bound: 4 B read + 12 B written per cell; the triangle gathers stay in L2 (the band
 // is walked in grid order and the soup is spatially binned).
 // ---------------------------------------------------------------------------------------
+// Closest point of the triangle (0, e0, ec) to r.  Not tri_closest: that one ranks the candidate edges by their
+// squared distances, which is right for the distance but leaves the POINT undecided within d * sqrt(2 eps) -- far
+// from the triangle a vertex and a point 1e-4 along an edge are equally far in fp32.  Here the edge whose foot point
+// is interior wins outright: a point outside an edge's half-plane whose foot lies inside the segment has that foot
+// as the closest point of the whole half-plane, hence of the triangle; only end points are ranked by distance.
+__device__ __forceinline__ void edge_candidate(f3 r, f3 o, f3 e, float &best, bool &interior, f3 &q) {
+    const f3 ro = r - o;
+    float t = dot(ro, e) / dot(e, e);
+    const bool in = t > 0.0f && t < 1.0f;
+    t = fminf(fmaxf(t, 0.0f), 1.0f);
+    const f3 c = o + t * e, d = r - c;
+    const float d2 = dot(d, d);
+    if ((in && !interior) || (in == interior && d2 < best)) { best = d2; q = c; interior = in; }
+}
+__device__ __forceinline__ f3 tri_closest_point(f3 r, f3 e0, f3 ec, f3 n) {
+    const f3 e1 = ec - e0;
+    const float s0 = dot(cross(n, e0), r), s1 = dot(cross(n, e1), r - e0), s2 = -dot(cross(n, ec), r - ec);
+    if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f) return r - dot(n, r) * n;
+    float best = INFINITY;
+    bool interior = false;
+    f3 q = mk<float>(0.0f, 0.0f, 0.0f);
+    if (s0 < 0.0f) edge_candidate(r, q, e0, best, interior, q);
+    if (s1 < 0.0f) edge_candidate(r, e0, e1, best, interior, q);
+    if (s2 < 0.0f) edge_candidate(r, mk<float>(0.0f, 0.0f, 0.0f), ec, best, interior, q);
+    return q;
+}
+
 __device__ __forceinline__ void closest_point_of(const MeshView &mv, const GridParams &g, int xt, int64_t c, float *o) {
     o[0] = o[1] = o[2] = INFINITY;
     if (xt >= 0 && xt < mv.F) {
@@ -789,8 +816,7 @@ __device__ __forceinline__ void closest_point_of(const MeshView &mv, const GridP
         const int t = mv.inv_perm[xt];
         const float *T = mv.soup + 9 * (size_t)t;
         const f3 a = ld3(T), x = mk<float>(fmaf((float)i, g.h, g.ox), fmaf((float)j, g.h, g.oy), fmaf((float)k, g.h, g.oz));
-        int rg; f3 q;
-        tri_closest<float>(x - a, ld3(T + 3) - a, ld3(T + 6) - a, ld3(mv.fn + 3 * (size_t)t), rg, q);
+        const f3 q = tri_closest_point(x - a, ld3(T + 3) - a, ld3(T + 6) - a, ld3(mv.fn + 3 * (size_t)t));
         o[0] = a.x + q.x; o[1] = a.y + q.y; o[2] = a.z + q.z;
     }
 }

@@ -3,7 +3,8 @@ than a cell, cavities, monkey saddles, ruffs, leaning spikes, tetrahedra, cube f
 and shifted, on random ragged grids (5..150 cells per axis, spacing and origin not exact in binary) with random
 bands (0.6..12 cells).  Every case must meet the four north_star clauses, and sdf_fill_interior on its result
 must equal the oracle's sweeps bit for bit.  (10,800 such cases were run once with zero failures, also under the
-ablation switches; the suite keeps 400 of them.)"""
+ablation switches, and 11,000 more with multi-body meshes, bands up to 80 cells, grids that only partly meet the
+mesh and the closest-point call; the suite keeps 700 of them.)"""
 import numpy as np
 import pytest
 import torch
@@ -26,15 +27,23 @@ MAKERS = [
     lambda r: W.spike_mesh(nfan=int(r.integers(3, 9)), lean=float(r.uniform(0.0, 1.4)), height=float(r.uniform(0.15, 0.6))),
     lambda r: W.tetrahedron_mesh(float(r.uniform(0.1, 0.7))),
     lambda r: W.cube_fan_mesh((int(r.integers(0, 4)), int(r.integers(0, 6)), int(r.integers(0, 8)))),
+    lambda r: W.multibody_mesh(r, counts=(int(r.integers(1, 6)), int(r.integers(1, 6)), int(r.integers(0, 4)), int(r.integers(0, 3))),
+                               lattice=(4, 2, 2), pitch=0.5, ico_subdiv=int(r.integers(0, 3)),
+                               torus_res=(int(r.integers(6, 24)), int(r.integers(4, 12)))),
 ]
 
 
-def _case(r):
+def _case(r, wide=False):
     v, t = MAKERS[int(r.integers(0, len(MAKERS)))](r)
     if r.random() < 0.7:
         v = v @ W.random_rotation(r).T
     v = v * float(r.uniform(0.5, 1.3)) + r.uniform(-0.15, 0.15, 3)
     soup = W.soup_from_indexed(v, t, r)
+    if wide:        # small grids (down to one cell per axis), bands of 0.05 .. 80 cells, grids that only partly meet the mesh
+        dims = tuple(int(x) for x in r.integers(1, 48, 3))
+        h = float(r.uniform(1.0, 4.0) / max(max(dims), 8))
+        origin = tuple(float(x) for x in (-0.5 * np.array(dims) * h + r.uniform(-0.9, 0.9, 3)))
+        return f32_grid(W.Workload("fuzz", soup, origin, h, dims, float(r.uniform(0.05, 80.0)) * h))
     dims = tuple(int(x) for x in r.integers(5, 150, 3))
     h = float(r.uniform(1.6, 2.6) / max(dims))
     origin = tuple(float(x) for x in (-0.5 * np.array(dims) * h + r.uniform(-0.2, 0.2, 3)))
@@ -58,5 +67,30 @@ def test_fuzz_parity_and_fill(oracle_mod, seed):
         B.sdf_fill_interior(d, w.band)
         torch.cuda.synchronize()
         assert np.array_equal(d.cpu().numpy(), oracle_mod.fill_interior(d_np, w.band)), (seed, c, w.dims)
+        B.sdf_destroy(m)
+    assert populated > 100000
+
+
+@pytest.mark.parametrize("seed", [201, 202])
+def test_fuzz_wide_bands_partial_overlap_closest_points(oracle_mod, seed):
+    from paper_1903_00353_b200 import binding as B
+    populated = 0
+    for c in range(150):
+        w = _case(np.random.default_rng(seed * 100003 + c), wide=True)
+        om = oracle_mod.Mesh(w.soup)
+        d_ref, t_ref = om.sdf(w.origin, w.h, w.dims, w.band)
+        m = B.sdf_create(np.ascontiguousarray(w.soup))
+        d, tr = B.sdf_compute(m, w.origin, w.h, w.dims, w.band)
+        t_np = tr.cpu().numpy()
+        res = compare_to_oracle(d.cpu().numpy(), t_np, d_ref, t_ref, w, om)
+        assert res["ok"] and all(res[k] == 0 for k in KEYS), (seed, c, w.dims, w.band / w.h, {k: res[k] for k in KEYS})
+        populated += res["populated_gpu"]
+        # closest points on the GPU's own ids against the oracle's routine on the same ids
+        cp = B.sdf_closest_points(m, w.origin, w.h, w.dims, tr).cpu().numpy()
+        ref = om.closest_points(w.origin, w.h, w.dims, t_np)
+        pop = t_np >= 0
+        assert np.all(np.isposinf(cp[~pop]))
+        if pop.any():
+            assert np.max(np.abs(cp[pop].astype(np.float64) - ref[pop])) <= 1e-5 * w.h + 1e-6 * w.diag, (seed, c)
         B.sdf_destroy(m)
     assert populated > 100000
