@@ -94,3 +94,46 @@ def test_fuzz_wide_bands_partial_overlap_closest_points(oracle_mod, seed):
             assert np.max(np.abs(cp[pop].astype(np.float64) - ref[pop])) <= 1e-5 * w.h + 1e-6 * w.diag, (seed, c)
         B.sdf_destroy(m)
     assert populated > 100000
+
+
+def test_fuzz_defective_input_statuses(oracle_mod):
+    """One random defect per mesh (hole, flipped triangle, duplicated triangle, repeated corner, NaN / Inf, a corner
+    moved by one ulp, a collapsed triangle -- or a harmless corner rotation): sdf_create must return the status the
+    oracle returns for the same soup (1,500 such cases were run once: no mismatch)."""
+    from paper_1903_00353_b200 import binding as B
+    seen = set()
+    for c in range(300):
+        r = np.random.default_rng(7919 * 3 + c)
+        v, t = MAKERS[int(r.integers(0, len(MAKERS)))](r)
+        soup = W.soup_from_indexed(v, t, r).copy()
+        n = soup.shape[0]
+        kind, k = int(r.integers(0, 8)), int(r.integers(0, n))
+        if kind == 0:
+            soup = np.delete(soup, r.choice(n, size=int(r.integers(1, 4)), replace=False), axis=0)
+        elif kind == 1:
+            soup[k] = soup[k][::-1].copy()
+        elif kind == 2:
+            soup = np.concatenate([soup, soup[k:k + 1]])
+        elif kind == 3:
+            soup[k, 1] = soup[k, 0]
+        elif kind == 4:
+            soup[k, int(r.integers(0, 3)), int(r.integers(0, 3))] = [np.nan, np.inf, -np.inf][int(r.integers(0, 3))]
+        elif kind == 5:
+            soup[k, 0, 0] = np.nextafter(soup[k, 0, 0], np.float32(9))
+        elif kind == 6:
+            soup[k] = soup[k][[1, 2, 0]]
+        else:
+            soup[k, 2] = (soup[k, 0] + soup[k, 1]) * np.float32(0.5)
+        soup = np.ascontiguousarray(soup, dtype=np.float32)
+        so = sg = 0
+        try:
+            oracle_mod.Mesh(soup)
+        except oracle_mod.OracleError as e:
+            so = e.status
+        try:
+            B.sdf_destroy(B.sdf_create(soup))
+        except B.SdfError as e:
+            sg = e.status
+        assert so == sg, (c, kind, so, sg)
+        seen.add((kind, sg))
+    assert {s for _, s in seen} >= {0, 1, 2, 3, 4}
