@@ -138,6 +138,30 @@ int sdf_compute(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int
                 float band, float *dist_out, int32_t *tri_out, void *stream);
 
 /*
+ * sdf_transform -- one pass of the whole hot path A0-A8 on one mesh and one grid: sdf_create
+ * followed by sdf_compute, with identical results (bit for bit), arguments, layouts and error
+ * behaviour; every argument is checked before any work is enqueued.  Knowing the grid before the
+ * feature construction lets the dense sentinel write of both grids (A8a:
+ * +INFINITY / -1 outside the band), which depends on nothing but the output
+ * pointers, start earlier: environment SDF_PREFILL_AT = 1 (before A0), 2 (before the edge table),
+ * 3 (before edge pairing), 4 (default: where sdf_compute forks it, beside A5-A7).  On a B200 the
+ * early starts LOSE (the feature kernels stall under the fill's write stream), so
+ * they are an ablation, not the default.
+ *
+ *   tri_xyz, ntri, on_device, a      as for sdf_create
+ *   origin, h, nx, ny, nz, band      as for sdf_compute
+ *   dist_out, tri_out                DEVICE, caller-owned, as for sdf_compute; overwritten entirely
+ *   stream                           cudaStream_t; synchronised three times (sdf_create's two, sdf_compute's one)
+ *   out                              receives the handle (for sdf_stats, further sdf_compute calls ...) on
+ *                                    SDF_OK; NULL otherwise, and then the output grids hold unspecified values
+ *                                    (the fill has been waited for: nothing is left in flight).
+ * Errors: those of sdf_create and sdf_compute; arguments are checked before any work is enqueued.
+ */
+int sdf_transform(const float *tri_xyz, int64_t ntri, int on_device, const sdf_allocator *a,
+                  const float origin[3], float h, int nx, int ny, int nz, float band,
+                  float *dist_out, int32_t *tri_out, void *stream, sdf_mesh **out);
+
+/*
  * sdf_zslab / sdf_compute_zslab -- the paper's multi-card outlook (a domain
  * "distributed across multiple cards"): the grid is cut into `parts` slabs of whole z-slices and
  * every process computes one of them from the complete feature tables of its own handle.  No cell

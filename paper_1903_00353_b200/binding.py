@@ -22,7 +22,7 @@ SDF_OK, SDF_EINVAL, SDF_ENOTCLOSED, SDF_EORIENT, SDF_EDEGENERATE, SDF_ENOMEM, SD
 TABLE_CORNER_VID, TABLE_HALFEDGE_ADJ, TABLE_FACE_NORMAL, TABLE_VERTEX_REC, TABLE_EDGE_REC, \
     TABLE_VERTEX_MINTRI = range(6)
 
-EXPORTS = ("sdf_create", "sdf_compute", "sdf_compute_host", "sdf_zslab", "sdf_compute_zslab", "sdf_fill_interior", "sdf_closest_points", "sdf_stats", "sdf_get_table",
+EXPORTS = ("sdf_create", "sdf_transform", "sdf_compute", "sdf_compute_host", "sdf_zslab", "sdf_compute_zslab", "sdf_fill_interior", "sdf_closest_points", "sdf_stats", "sdf_get_table",
            "sdf_destroy", "sdf_strerror", "sdf_last_cuda_error", "sdf_version",
            "sdf_enable_timing", "sdf_get_timings", "sdf_launch_count",
            "sdf_read_stl", "sdf_free_host", "sdf_write_stl", "sdf_write_grid")
@@ -90,6 +90,9 @@ def lib():
     L.sdf_compute.argtypes = [vp, C.POINTER(C.c_float), C.c_float, C.c_int, C.c_int, C.c_int, C.c_float, vp, vp, vp]
     L.sdf_compute.restype = C.c_int
     L.sdf_compute_host.argtypes = L.sdf_compute.argtypes
+    L.sdf_transform.argtypes = [vp, C.c_int64, C.c_int, C.POINTER(_Allocator), C.POINTER(C.c_float), C.c_float, C.c_int, C.c_int,
+                                C.c_int, C.c_float, vp, vp, vp, C.POINTER(vp)]
+    L.sdf_transform.restype = C.c_int
     L.sdf_zslab.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.sdf_zslab.restype = C.c_int
     L.sdf_compute_zslab.argtypes = [vp, C.POINTER(C.c_float), C.c_float, C.c_int, C.c_int, C.c_int, C.c_float, C.c_int, C.c_int,
@@ -230,6 +233,45 @@ def sdf_create(tri_xyz, stream=None, use_torch_allocator=True) -> Mesh:
     if st != SDF_OK:
         raise SdfError(st, "sdf_create")
     return Mesh(out, ntri)
+
+
+def _soup_ptr(tri_xyz):
+    torch = _torch()
+    if isinstance(tri_xyz, torch.Tensor):
+        t = tri_xyz.detach()
+        if t.dtype != torch.float32:
+            raise TypeError("tri_xyz must be float32")
+        t = t.contiguous()
+        return t.data_ptr(), int(t.is_cuda), t.numel() // 9, t.numel(), t
+    a = np.ascontiguousarray(tri_xyz, dtype=np.float32)
+    return a.ctypes.data, 0, a.size // 9, a.size, a
+
+
+def sdf_transform(tri_xyz, origin, h, dims, band, dist_out=None, tri_out=None, stream=None, use_torch_allocator=True):
+    """sdf_create + sdf_compute in one call (include/sdf.h: the sentinel fill starts before the
+    feature construction).  Returns (Mesh, dist float32 [nz,ny,nx], tri int32 [nz,ny,nx])."""
+    L = lib()
+    torch = _torch()
+    ptr, on_dev, ntri, nel, keep = _soup_ptr(tri_xyz)
+    if nel != 9 * ntri:
+        raise ValueError("tri_xyz must hold 9 floats per triangle")
+    nx, ny, nz = (int(v) for v in dims)
+    if dist_out is None:
+        dist_out = torch.empty((nz, ny, nx), dtype=torch.float32, device="cuda")
+    if tri_out is None:
+        tri_out = torch.empty((nz, ny, nx), dtype=torch.int32, device="cuda")
+    assert dist_out.is_cuda and tri_out.is_cuda and dist_out.is_contiguous() and tri_out.is_contiguous()
+    assert dist_out.numel() == nx * ny * nz and tri_out.numel() == nx * ny * nz
+    assert dist_out.dtype == torch.float32 and tri_out.dtype == torch.int32
+    out = C.c_void_p()
+    alloc = C.byref(torch_allocator()) if use_torch_allocator else None
+    st = L.sdf_transform(C.c_void_p(ptr), ntri, on_dev, alloc, _origin3(origin), float(h), nx, ny, nz, float(band),
+                         C.c_void_p(dist_out.data_ptr()), C.c_void_p(tri_out.data_ptr()),
+                         C.c_void_p(_stream_ptr(stream)), C.byref(out))
+    del keep
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_transform")
+    return Mesh(out, ntri), dist_out, tri_out
 
 
 def _origin3(origin):

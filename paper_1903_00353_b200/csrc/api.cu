@@ -92,7 +92,7 @@ void sdf_destroy(sdf_mesh *m) {
     if (m->side) cudaStreamSynchronize(m->side);      // shared, process-lifetime stream: not destroyed here
     if (m->ev_fork) cudaEventDestroy(m->ev_fork);
     if (m->ev_join) cudaEventDestroy(m->ev_join);
-    void *ptrs[] = {m->slab_f, m->slab_v, m->slab_ws, m->scratch, m->cp_state};
+    void *ptrs[] = {m->slab_f, m->slab_v, m->slab_ws, m->scratch, m->cp_state, m->fill_state};
     for (size_t i = 0; i < sizeof(ptrs) / sizeof(ptrs[0]); i++) dev_free(&m->alloc, ptrs[i], st);
     for (int i = 0; i < SDF_T_COUNT; i++)
         for (int w = 0; w < 2; w++)
@@ -101,12 +101,7 @@ void sdf_destroy(sdf_mesh *m) {
     free(m);
 }
 
-int sdf_create(const float *tri_xyz, int64_t ntri, int on_device, const sdf_allocator *a, void *stream,
-               sdf_mesh **out) {
-    if (out) *out = nullptr;
-    if (!tri_xyz || !out || ntri <= 0 || ntri > ((int64_t)1 << 29)) return SDF_EINVAL;
-    if (a && (!a->alloc || !a->free)) return SDF_EINVAL;
-    if (!have_device()) return SDF_ECUDA;
+static int new_mesh(int64_t ntri, const sdf_allocator *a, void *stream, sdf_mesh **out) {
     void *mem = calloc(1, sizeof(sdf_mesh));
     if (!mem) return SDF_ENOMEM;
     sdf_mesh *m = new (mem) sdf_mesh;
@@ -114,6 +109,18 @@ int sdf_create(const float *tri_xyz, int64_t ntri, int on_device, const sdf_allo
     if (a) m->alloc = *a;
     m->F = ntri;
     m->last_stream = (cudaStream_t)stream;
+    *out = m;
+    return SDF_OK;
+}
+
+int sdf_create(const float *tri_xyz, int64_t ntri, int on_device, const sdf_allocator *a, void *stream,
+               sdf_mesh **out) {
+    if (out) *out = nullptr;
+    if (!tri_xyz || !out || ntri <= 0 || ntri > ((int64_t)1 << 29)) return SDF_EINVAL;
+    if (a && (!a->alloc || !a->free)) return SDF_EINVAL;
+    if (!have_device()) return SDF_ECUDA;
+    sdf_mesh *m = nullptr;
+    CKS(new_mesh(ntri, a, stream, &m));
     int s = build_features(m, tri_xyz, on_device, (cudaStream_t)stream);
     if (s != SDF_OK) {
         sdf_destroy(m);
@@ -181,6 +188,42 @@ int sdf_compute(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int
     int s = run_compute(m, g, dist_out, tri_out, (cudaStream_t)stream);
     if (s != SDF_OK && m->side) cudaStreamSynchronize(m->side);   // never leave the fill in flight on failure
     return s;
+}
+
+int sdf_transform(const float *tri_xyz, int64_t ntri, int on_device, const sdf_allocator *a, const float origin[3],
+                  float h, int nx, int ny, int nz, float band, float *dist_out, int32_t *tri_out, void *stream,
+                  sdf_mesh **out) {
+    if (out) *out = nullptr;
+    if (!tri_xyz || !out || ntri <= 0 || ntri > ((int64_t)1 << 29)) return SDF_EINVAL;
+    if (a && (!a->alloc || !a->free)) return SDF_EINVAL;
+    if (!dist_out || !tri_out) return SDF_EINVAL;
+    GridParams g;
+    CKS(make_grid(origin, h, nx, ny, nz, band, dist_out, tri_out, &g));
+    if (!have_device()) return SDF_ECUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    sdf_mesh *m = nullptr;
+    CKS(new_mesh(ntri, a, stream, &m));
+    // the sentinel fill (A8a) needs only the output pointers, so it could start under A0-A4: build_features
+    // starts it at the stage boundary SDF_PREFILL_AT (1 before A0, 2 before the edge table, 3 before edge
+    // pairing).  Measured: the feature kernels are DRAM-latency bound and stall under the fill's
+    // write stream -- the step gets 0.7 ms longer at C4 -- so the default is 4: run_compute forks it beside A5-A7.
+    const bool pre = g.fill_mode < 2 || g.fill_mode == 4;
+    const char *pa = getenv("SDF_PREFILL_AT");
+    m->pre_at = (pa && pa[0] >= '1' && pa[0] <= '4') ? pa[0] - '0' : 4;
+    m->pre_g = pre ? &g : nullptr;
+    m->pre_dist = dist_out;
+    m->pre_tri = tri_out;
+    int s = build_features(m, tri_xyz, on_device, st);
+    const bool started = pre && !m->pre_g;
+    m->pre_g = nullptr;
+    if (s == SDF_OK) s = run_compute(m, g, dist_out, tri_out, st, started);
+    if (s != SDF_OK) {
+        if (m->side) cudaStreamSynchronize(m->side);   // never leave the fill in flight on failure
+        sdf_destroy(m);
+        return s;
+    }
+    *out = m;
+    return SDF_OK;
 }
 
 int sdf_zslab(int nz, int part, int parts, int *k0, int *nk) {

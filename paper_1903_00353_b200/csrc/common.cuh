@@ -146,6 +146,8 @@ struct sdf_mesh {
     cudaStream_t last_stream;
     cudaStream_t side;                // library-owned stream of the sentinel fill (A8a)
     cudaEvent_t ev_fork, ev_join;
+    // sdf_transform: sentinel fill still to be started at stage boundary pre_at of build_features (0 = none pending)
+    const GridParams *pre_g; float *pre_dist; int *pre_tri; int pre_at;
 };
 
 // carve 256-byte aligned tables out of one slab; with base == nullptr it only adds up sizes
@@ -169,5 +171,7 @@ void stage_mark(sdf_mesh *m, int stage, int which, cudaStream_t st);
 
 // stages (features.cu / compute.cu)
 int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st);
-int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st);
+int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st, bool prefilled = false);
+int start_prefill(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st);
+int maybe_prefill(sdf_mesh *m, int point, cudaStream_t st);
 int run_closest_points(sdf_mesh *m, const GridParams &g, const int *tri, float *cp, cudaStream_t st);

@@ -627,47 +627,16 @@ static int ensure(sdf_mesh *m, T **p, size_t *cap, size_t need, cudaStream_t st)
     return SDF_OK;
 }
 
-int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cudaStream_t st) {
-    GridParams g = g_in;
-    {
-        // a mesh with few polyhedra cannot fill the GPU with one lane per polyhedron: hand more
-        // of them to the block-per-polyhedron kernel
-        const int64_t P0 = m->F + m->E + 2 * m->V;
-        g.big_rows = P0 < 4096 ? 8 : (P0 < 65536 ? 64 : (int)BIG_ROWS);
-        g.big_ni = P0 < 4096 ? 4 : (P0 < 65536 ? 16 : BIG_NI);
-    }
-    MeshView mv;
-    mv.soup = m->soup; mv.fn = m->fn; mv.erec = m->erec; mv.vrec = m->vrec; mv.vmint = m->vmint;
-    mv.cvid = m->cvid; mv.adj = m->adj; mv.perm = m->perm; mv.inv_perm = m->inv_perm;
-    mv.F = (int)m->F; mv.E = (int)m->E; mv.V = (int)m->V;
-    mv.P = m->F + m->E + 2 * m->V;
-    const int64_t P = mv.P;
-    const int64_t nbricks = (int64_t)g.nbx * g.nby * g.nbz;
-    // per-compute workspace: one slab, grown on demand
-    for (int pass = 0; pass < 2; pass++) {
-        Carver c(pass ? m->slab_ws : nullptr);
-        m->brick_flag = c.take<unsigned char>((size_t)nbricks);
-        m->brick_table = c.take<int>((size_t)nbricks);
-        m->brick_list = c.take<int>((size_t)nbricks);
-        m->scan_ws = c.take<u64>(scan_ws_elems(nbricks));
-        m->big_list = c.take<u32>((size_t)P);
-        m->fill_state = c.take<u32>(FILL_STATE_WORDS);
-        if (pass == 0 && (c.off > m->slab_ws_cap || !m->slab_ws)) {
-            if (m->slab_ws) { dev_free(&m->alloc, m->slab_ws, st); m->slab_ws = nullptr; m->slab_ws_cap = 0; }
-            const size_t want = c.off + c.off / 8 + 256;
-            CKS(dev_alloc(&m->alloc, &m->slab_ws, want, st));
-            m->slab_ws_cap = want;
-        }
-    }
-
-    // A8a: the sentinel fill depends on nothing: fork it onto the side stream so that it
-    // streams to HBM underneath A5-A7 (which are latency / atomic bound)
+// A8a: the sentinel fill depends on nothing but the output pointers.  Forked onto the side stream it
+// streams to HBM underneath whatever runs on `st` next: A5-A7 inside sdf_compute, or -- when
+// sdf_transform starts it first -- the whole feature construction A0-A4 as well.
+static int fork_sentinel_fill(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st, bool fork) {
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    for (int i = SDF_T_CLIP_SCAN; i < SDF_T_COUNT; i++) m->ev_set[i] = false;
     const int64_t N = (int64_t)g.nx * g.ny * g.nz;
     const int vec = (((uintptr_t)dist & 15) == 0) && (((uintptr_t)tri & 15) == 0);
+    if (!m->fill_state) CKS(dev_alloc(&m->alloc, (void **)&m->fill_state, sizeof(u32) * FILL_STATE_WORDS, st));
     auto launch_fill = [&](cudaStream_t fs) -> int {
         stage_mark(m, SDF_T_FILL, 0, fs);
         if (vec && g.fill_mode != 1) {
@@ -695,32 +664,89 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
         stage_mark(m, SDF_T_FILL, 1, fs);
         return SDF_OK;
     };
-    const bool forked = g.fill_mode < 2 || g.fill_mode == 4;
-    auto fork_fill = [&]() -> int {
-        if (!m->side) {
-            // one library-owned side stream per process (creating a stream per handle cost ~30 us
-            // per sdf_compute on a fresh handle); highest priority: the few, tiny fill CTAs are
-            // placed before the evaluate blocks
-            static cudaStream_t g_side = nullptr;
-            static int g_side_prio = -1, g_side_dev = -1;
-            if (!g_side || g_side_prio != g.fill_prio || g_side_dev != dev) {
-                int plo = 0, phi = 0;
-                cudaDeviceGetStreamPriorityRange(&plo, &phi);
-                CK(cudaStreamCreateWithPriority(&g_side, cudaStreamNonBlocking, g.fill_prio ? phi : plo));
-                g_side_prio = g.fill_prio;
-                g_side_dev = dev;
-            }
-            m->side = g_side;
+    if (!fork) return launch_fill(st);
+    if (!m->side) {
+        // one library-owned side stream per process (creating a stream per handle cost ~30 us
+        // per sdf_compute on a fresh handle); highest priority: the few, tiny fill CTAs are
+        // placed before the evaluate blocks
+        static cudaStream_t g_side = nullptr;
+        static int g_side_prio = -1, g_side_dev = -1;
+        if (!g_side || g_side_prio != g.fill_prio || g_side_dev != dev) {
+            int plo = 0, phi = 0;
+            cudaDeviceGetStreamPriorityRange(&plo, &phi);
+            CK(cudaStreamCreateWithPriority(&g_side, cudaStreamNonBlocking, g.fill_prio ? phi : plo));
+            g_side_prio = g.fill_prio;
+            g_side_dev = dev;
         }
-        if (!m->ev_fork) CK(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
-        if (!m->ev_join) CK(cudaEventCreateWithFlags(&m->ev_join, cudaEventDisableTiming));
-        CK(cudaEventRecord(m->ev_fork, st));
-        CK(cudaStreamWaitEvent(m->side, m->ev_fork, 0));
-        CKS(launch_fill(m->side));
-        CK(cudaEventRecord(m->ev_join, m->side));
-        return SDF_OK;
-    };
-    if (g.fill_mode < 2) CKS(fork_fill());
+        m->side = g_side;
+    }
+    if (!m->ev_fork) CK(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
+    if (!m->ev_join) CK(cudaEventCreateWithFlags(&m->ev_join, cudaEventDisableTiming));
+    CK(cudaEventRecord(m->ev_fork, st));
+    CK(cudaStreamWaitEvent(m->side, m->ev_fork, 0));
+    CKS(launch_fill(m->side));
+    CK(cudaEventRecord(m->ev_join, m->side));
+    return SDF_OK;
+}
+
+// sdf_transform: start the sentinel fill of the outputs before the feature tables exist
+int start_prefill(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st) {
+    m->ev_set[SDF_T_FILL] = false;
+    return fork_sentinel_fill(m, g, dist, tri, st, true);
+}
+
+// stage boundary `point` of build_features: start the pending fill if this is where it was asked for
+int maybe_prefill(sdf_mesh *m, int point, cudaStream_t st) {
+    if (!m->pre_g || m->pre_at != point) return SDF_OK;
+    const GridParams *g = m->pre_g;
+    m->pre_g = nullptr;
+    return start_prefill(m, *g, m->pre_dist, m->pre_tri, st);
+}
+
+int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cudaStream_t st, bool prefilled) {
+    GridParams g = g_in;
+    {
+        // a mesh with few polyhedra cannot fill the GPU with one lane per polyhedron: hand more
+        // of them to the block-per-polyhedron kernel
+        const int64_t P0 = m->F + m->E + 2 * m->V;
+        g.big_rows = P0 < 4096 ? 8 : (P0 < 65536 ? 64 : (int)BIG_ROWS);
+        g.big_ni = P0 < 4096 ? 4 : (P0 < 65536 ? 16 : BIG_NI);
+    }
+    MeshView mv;
+    mv.soup = m->soup; mv.fn = m->fn; mv.erec = m->erec; mv.vrec = m->vrec; mv.vmint = m->vmint;
+    mv.cvid = m->cvid; mv.adj = m->adj; mv.perm = m->perm; mv.inv_perm = m->inv_perm;
+    mv.F = (int)m->F; mv.E = (int)m->E; mv.V = (int)m->V;
+    mv.P = m->F + m->E + 2 * m->V;
+    const int64_t P = mv.P;
+    const int64_t nbricks = (int64_t)g.nbx * g.nby * g.nbz;
+    // per-compute workspace: one slab, grown on demand
+    for (int pass = 0; pass < 2; pass++) {
+        Carver c(pass ? m->slab_ws : nullptr);
+        m->brick_flag = c.take<unsigned char>((size_t)nbricks);
+        m->brick_table = c.take<int>((size_t)nbricks);
+        m->brick_list = c.take<int>((size_t)nbricks);
+        m->scan_ws = c.take<u64>(scan_ws_elems(nbricks));
+        m->big_list = c.take<u32>((size_t)P);
+        if (pass == 0 && (c.off > m->slab_ws_cap || !m->slab_ws)) {
+            if (m->slab_ws) { dev_free(&m->alloc, m->slab_ws, st); m->slab_ws = nullptr; m->slab_ws_cap = 0; }
+            const size_t want = c.off + c.off / 8 + 256;
+            CKS(dev_alloc(&m->alloc, &m->slab_ws, want, st));
+            m->slab_ws_cap = want;
+        }
+    }
+
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    for (int i = SDF_T_CLIP_SCAN; i < SDF_T_COUNT; i++)
+        if (!(prefilled && i == SDF_T_FILL)) m->ev_set[i] = false;
+    // the fill is forked here (or, fill_mode 4, after the host crossing below) unless sdf_transform
+    // already started it ahead of the feature construction
+    const bool forked = prefilled || g.fill_mode < 2 || g.fill_mode == 4;
+    auto fork_fill = [&]() -> int { return fork_sentinel_fill(m, g, dist, tri, st, true); };
+    auto launch_fill = [&](cudaStream_t fs) -> int { return fork_sentinel_fill(m, g, dist, tri, fs, false); };
+    if (prefilled) {}
+    else if (g.fill_mode < 2) CKS(fork_fill());
     else if (g.fill_mode == 3) CKS(launch_fill(st));
     CK(cudaMemsetAsync(m->brick_flag, 0, (size_t)nbricks, st));
     CK(cudaMemsetAsync(m->d_ctr + CTR_POLY, 0, sizeof(u64) * (CTR_TOTAL - CTR_POLY), st));
@@ -738,7 +764,7 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
     stage_mark(m, SDF_T_CLIP_SCAN, 1, st);
     // fork the fill first: its CTAs claim their SMs while the GPU is still empty (the scratch
     // allocation and its clear come next), before the evaluate blocks flood it
-    if (g.fill_mode == 4) CKS(fork_fill());
+    if (g.fill_mode == 4 && !prefilled) CKS(fork_fill());
     CKS(ensure(m, &m->scratch, &m->scratch_cap, (size_t)(bricks ? bricks : 1) * BRICK_CELLS, st));
     stage_mark(m, SDF_T_CLEAR, 0, st);
     if (bricks) CK(cudaMemsetAsync(m->scratch, 0xFF, (size_t)bricks * BRICK_CELLS * sizeof(u64), st));

@@ -587,6 +587,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     CK(cudaMemsetAsync(m->adj, 0xFF, sizeof(int) * 3 * F, st));
 
     // ---- A0 ingest + A1 weld (hash table on the exact coordinate bits)
+    CKS(maybe_prefill(m, 1, st));
     stage_mark(m, SDF_T_INGEST_WELD, 0, st);
     const u32 capw = pow2_at_least((u64)nc + (u64)nc / 4 + 1);     // load <= 0.8 even if no vertex is shared
     const u32 cape = pow2_at_least((u64)nc + 1);                   // <= 3F/2 forward half-edges: load <= 0.5
@@ -674,6 +675,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     }
 
     // ---- A3 (per triangle), A2 edge table
+    CKS(maybe_prefill(m, 2, st));
     stage_mark(m, SDF_T_EDGES, 0, st);
     CK(cudaMemsetAsync(vacc, 0, (size_t)((char *)(vside + V) - (char *)vacc), st));
     KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wtab, slot, (int)F, m->cvid, m->fn, vacc, fcnt, etab, cape - 1, m->d_flags);
@@ -698,6 +700,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
         }
     }
     CKS(launch_scan(FcntIn{fcnt}, EbaseOut{ebase}, F, scan_ws, (u64 *)nullptr, st));
+    CKS(maybe_prefill(m, 3, st));
     KL; edge_pair_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, etab, cape - 1, m->adj);
     KL; edge_record_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, m->adj, ebase, m->soup, m->fn, m->perm, m->erec, m->d_ctr);
     CK(cudaGetLastError());
