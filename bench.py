@@ -178,7 +178,7 @@ def workload_config(w, args):
                             % (args.zslab_parts or args.gpus)) if (args.zslab or args.zslab_parts) else
                            "replicas only (the path does not shard)" if args.gpus > 1 else "1 GPU",
             "call": "sdf_transform (= sdf_create + sdf_compute in one call)"
-                    if (getattr(args, "transform", False) and not (args.zslab or args.zslab_parts)) else "sdf_create + sdf_compute",
+                    if not (getattr(args, "split_calls", False) or args.zslab or args.zslab_parts) else "sdf_create + sdf_compute",
             "l2": "no flush needed: each step streams %.2f GB of output > %d MB L2"
                   % (8.0 * w.ncells / 1e9, L2_BYTES >> 20)}
 
@@ -227,7 +227,7 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
 
     def step_device():
-        if not zslab and args.transform:
+        if not zslab and not args.split_calls:
             # one call for the whole path (SDF_PREFILL_AT picks where the sentinel fill starts: DESIGN.md 9b)
             return B.sdf_transform(soup_dev, w.origin, w.h, w.dims, w.band, dist_out, tri_out, stream=stream)[0]
         m = B.sdf_create(soup_dev, stream=stream)
@@ -412,8 +412,8 @@ def main():
     ap.add_argument("--zslab", action="store_true", help="strong scaling: rank r computes z-slab r of WORLD_SIZE (NEXT-4)")
     ap.add_argument("--zslab-parts", type=int, default=0, help="time one slab of a P-way z split on this GPU")
     ap.add_argument("--zslab-part", type=int, default=0)
-    ap.add_argument("--transform", action="store_true",
-                    help="step = sdf_transform (the same path in one call) instead of sdf_create + sdf_compute")
+    ap.add_argument("--split-calls", action="store_true",
+                    help="step = sdf_create + sdf_compute (two calls) instead of sdf_transform (the same path in one call)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -146,12 +146,15 @@ int sdf_compute(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int
  * pointers, start earlier: environment SDF_PREFILL_AT = 1 (before A0), 2 (before the edge table),
  * 3 (before edge pairing), 4 (default: where sdf_compute forks it, beside A5-A7).  On a B200 the
  * early starts LOSE (the feature kernels stall under the fill's write stream), so
- * they are an ablation, not the default.
+ * they are an ablation, not the default.  What the single call does gain: the brick marking and
+ * its prefix sum (A6a) run on the vertex stream beside the edge stage and their total returns with
+ * the validation flags -- one stream synchronisation fewer than the two calls (
+ * SDF_HOIST_BRICKS=0 switches that off).
  *
  *   tri_xyz, ntri, on_device, a      as for sdf_create
  *   origin, h, nx, ny, nz, band      as for sdf_compute
  *   dist_out, tri_out                DEVICE, caller-owned, as for sdf_compute; overwritten entirely
- *   stream                           cudaStream_t; synchronised three times (sdf_create's two, sdf_compute's one)
+ *   stream                           cudaStream_t; synchronised twice (sdf_create's two crossings)
  *   out                              receives the handle (for sdf_stats, further sdf_compute calls ...) on
  *                                    SDF_OK; NULL otherwise, and then the output grids hold unspecified values
  *                                    (the fill has been waited for: nothing is left in flight).

@@ -92,6 +92,8 @@ void sdf_destroy(sdf_mesh *m) {
     if (m->side) cudaStreamSynchronize(m->side);      // shared, process-lifetime stream: not destroyed here
     if (m->ev_fork) cudaEventDestroy(m->ev_fork);
     if (m->ev_join) cudaEventDestroy(m->ev_join);
+    if (m->ev_ffork) cudaEventDestroy(m->ev_ffork);
+    if (m->ev_fjoin) cudaEventDestroy(m->ev_fjoin);
     void *ptrs[] = {m->slab_f, m->slab_v, m->slab_ws, m->scratch, m->cp_state, m->fill_state};
     for (size_t i = 0; i < sizeof(ptrs) / sizeof(ptrs[0]); i++) dev_free(&m->alloc, ptrs[i], st);
     for (int i = 0; i < SDF_T_COUNT; i++)
@@ -213,9 +215,15 @@ int sdf_transform(const float *tri_xyz, int64_t ntri, int on_device, const sdf_a
     m->pre_g = pre ? &g : nullptr;
     m->pre_dist = dist_out;
     m->pre_tri = tri_out;
+    // A6a (brick marks + scan, 0.2 ms at C4) needs the soup, the face normals and the grid, not the edge table:
+    // build_features runs it on the vertex stream beside the edge stage, and its total comes back with the
+    // validation flags -- one host crossing fewer (SDF_HOIST_BRICKS=0: leave it to run_compute)
+    const char *hb = getenv("SDF_HOIST_BRICKS");
+    m->hoist_g = (hb && hb[0] == '0') ? nullptr : &g;
     int s = build_features(m, tri_xyz, on_device, st);
     const bool started = pre && !m->pre_g;
     m->pre_g = nullptr;
+    m->hoist_g = nullptr;
     if (s == SDF_OK) s = run_compute(m, g, dist_out, tri_out, st, started);
     if (s != SDF_OK) {
         if (m->side) cudaStreamSynchronize(m->side);   // never leave the fill in flight on failure

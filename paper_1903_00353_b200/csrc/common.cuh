@@ -148,6 +148,9 @@ struct sdf_mesh {
     cudaEvent_t ev_fork, ev_join;
     // sdf_transform: sentinel fill still to be started at stage boundary pre_at of build_features (0 = none pending)
     const GridParams *pre_g; float *pre_dist; int *pre_tri; int pre_at;
+    // sdf_transform: A6a (brick marks + scan) still to be run by build_features / already run for the next run_compute
+    const GridParams *hoist_g; bool bricks_ready;
+    cudaEvent_t ev_ffork, ev_fjoin;   // fork / join of the sentinel fill (ev_fork / ev_join: the vertex stream)
 };
 
 // carve 256-byte aligned tables out of one slab; with base == nullptr it only adds up sizes
@@ -174,4 +177,5 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
 int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st, bool prefilled = false);
 int start_prefill(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st);
 int maybe_prefill(sdf_mesh *m, int point, cudaStream_t st);
+int maybe_prepare_bricks(sdf_mesh *m, cudaStream_t st, cudaStream_t vs);
 int run_closest_points(sdf_mesh *m, const GridParams &g, const int *tri, float *cp, cudaStream_t st);

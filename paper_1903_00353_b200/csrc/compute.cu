@@ -680,12 +680,12 @@ static int fork_sentinel_fill(sdf_mesh *m, const GridParams &g, float *dist, int
         }
         m->side = g_side;
     }
-    if (!m->ev_fork) CK(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
-    if (!m->ev_join) CK(cudaEventCreateWithFlags(&m->ev_join, cudaEventDisableTiming));
-    CK(cudaEventRecord(m->ev_fork, st));
-    CK(cudaStreamWaitEvent(m->side, m->ev_fork, 0));
+    if (!m->ev_ffork) CK(cudaEventCreateWithFlags(&m->ev_ffork, cudaEventDisableTiming));
+    if (!m->ev_fjoin) CK(cudaEventCreateWithFlags(&m->ev_fjoin, cudaEventDisableTiming));
+    CK(cudaEventRecord(m->ev_ffork, st));
+    CK(cudaStreamWaitEvent(m->side, m->ev_ffork, 0));
     CKS(launch_fill(m->side));
-    CK(cudaEventRecord(m->ev_join, m->side));
+    CK(cudaEventRecord(m->ev_fjoin, m->side));
     return SDF_OK;
 }
 
@@ -703,6 +703,57 @@ int maybe_prefill(sdf_mesh *m, int point, cudaStream_t st) {
     return start_prefill(m, *g, m->pre_dist, m->pre_tri, st);
 }
 
+static MeshView make_view(const sdf_mesh *m) {
+    MeshView mv;
+    mv.soup = m->soup; mv.fn = m->fn; mv.erec = m->erec; mv.vrec = m->vrec; mv.vmint = m->vmint;
+    mv.cvid = m->cvid; mv.adj = m->adj; mv.perm = m->perm; mv.inv_perm = m->inv_perm;
+    mv.F = (int)m->F; mv.E = (int)m->E; mv.V = (int)m->V;
+    mv.P = m->F + m->E + 2 * m->V;
+    return mv;
+}
+
+// A6a: per-compute workspace (allocated in the order of stream `as`), then on stream `ps`: mark the bricks
+// the band can reach, prefix sum -> brick table, list and the total in d_ctr[CTR_BRICKS].  Needs the soup,
+// the face normals and V; sdf_transform runs it on the vertex stream beside the edge stage.
+int prepare_bricks(sdf_mesh *m, const GridParams &g, cudaStream_t as, cudaStream_t ps) {
+    const MeshView mv = make_view(m);
+    const int64_t P = mv.P;
+    const int64_t nbricks = (int64_t)g.nbx * g.nby * g.nbz;
+    for (int pass = 0; pass < 2; pass++) {
+        Carver c(pass ? m->slab_ws : nullptr);
+        m->brick_flag = c.take<unsigned char>((size_t)nbricks);
+        m->brick_table = c.take<int>((size_t)nbricks);
+        m->brick_list = c.take<int>((size_t)nbricks);
+        m->scan_ws = c.take<u64>(scan_ws_elems(nbricks));
+        m->big_list = c.take<u32>((size_t)P);
+        if (pass == 0 && (c.off > m->slab_ws_cap || !m->slab_ws)) {
+            if (m->slab_ws) { dev_free(&m->alloc, m->slab_ws, as); m->slab_ws = nullptr; m->slab_ws_cap = 0; }
+            const size_t want = c.off + c.off / 8 + 256;
+            CKS(dev_alloc(&m->alloc, &m->slab_ws, want, as));
+            m->slab_ws_cap = want;
+        }
+    }
+    m->ev_set[SDF_T_CLIP_SCAN] = false;
+    CK(cudaMemsetAsync(m->brick_flag, 0, (size_t)nbricks, ps));
+    CK(cudaMemsetAsync(m->d_ctr + CTR_POLY, 0, sizeof(u64) * (CTR_TOTAL - CTR_POLY), ps));
+    stage_mark(m, SDF_T_CLIP_SCAN, 0, ps);
+    KL; brick_mark_kernel<<<(unsigned)((mv.F + 255) / 256), 256, 0, ps>>>(mv, g, m->brick_flag);
+    CKS(launch_scan(BrickIn{m->brick_flag}, BrickOut{m->brick_table, m->brick_list}, nbricks, m->scan_ws, m->d_ctr + CTR_BRICKS, ps));
+    CK(cudaGetLastError());
+    return SDF_OK;
+}
+
+// sdf_transform: stage boundary of build_features after the vertex kernels (stream vs, forked from st)
+int maybe_prepare_bricks(sdf_mesh *m, cudaStream_t st, cudaStream_t vs) {
+    if (!m->hoist_g) return SDF_OK;
+    const GridParams *g = m->hoist_g;
+    m->hoist_g = nullptr;
+    CKS(prepare_bricks(m, *g, st, vs));
+    stage_mark(m, SDF_T_CLIP_SCAN, 1, vs);
+    m->bricks_ready = true;        // the total travels with the validation flags (second host crossing)
+    return SDF_OK;
+}
+
 int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cudaStream_t st, bool prefilled) {
     GridParams g = g_in;
     {
@@ -712,33 +763,16 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
         g.big_rows = P0 < 4096 ? 8 : (P0 < 65536 ? 64 : (int)BIG_ROWS);
         g.big_ni = P0 < 4096 ? 4 : (P0 < 65536 ? 16 : BIG_NI);
     }
-    MeshView mv;
-    mv.soup = m->soup; mv.fn = m->fn; mv.erec = m->erec; mv.vrec = m->vrec; mv.vmint = m->vmint;
-    mv.cvid = m->cvid; mv.adj = m->adj; mv.perm = m->perm; mv.inv_perm = m->inv_perm;
-    mv.F = (int)m->F; mv.E = (int)m->E; mv.V = (int)m->V;
-    mv.P = m->F + m->E + 2 * m->V;
+    const MeshView mv = make_view(m);
     const int64_t P = mv.P;
     const int64_t nbricks = (int64_t)g.nbx * g.nby * g.nbz;
-    // per-compute workspace: one slab, grown on demand
-    for (int pass = 0; pass < 2; pass++) {
-        Carver c(pass ? m->slab_ws : nullptr);
-        m->brick_flag = c.take<unsigned char>((size_t)nbricks);
-        m->brick_table = c.take<int>((size_t)nbricks);
-        m->brick_list = c.take<int>((size_t)nbricks);
-        m->scan_ws = c.take<u64>(scan_ws_elems(nbricks));
-        m->big_list = c.take<u32>((size_t)P);
-        if (pass == 0 && (c.off > m->slab_ws_cap || !m->slab_ws)) {
-            if (m->slab_ws) { dev_free(&m->alloc, m->slab_ws, st); m->slab_ws = nullptr; m->slab_ws_cap = 0; }
-            const size_t want = c.off + c.off / 8 + 256;
-            CKS(dev_alloc(&m->alloc, &m->slab_ws, want, st));
-            m->slab_ws_cap = want;
-        }
-    }
+    const bool hoisted = m->bricks_ready;
+    m->bricks_ready = false;
 
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    for (int i = SDF_T_CLIP_SCAN; i < SDF_T_COUNT; i++)
+    for (int i = SDF_T_CLEAR; i < SDF_T_COUNT; i++)
         if (!(prefilled && i == SDF_T_FILL)) m->ev_set[i] = false;
     // the fill is forked here (or, fill_mode 4, after the host crossing below) unless sdf_transform
     // already started it ahead of the feature construction
@@ -748,20 +782,18 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
     if (prefilled) {}
     else if (g.fill_mode < 2) CKS(fork_fill());
     else if (g.fill_mode == 3) CKS(launch_fill(st));
-    CK(cudaMemsetAsync(m->brick_flag, 0, (size_t)nbricks, st));
-    CK(cudaMemsetAsync(m->d_ctr + CTR_POLY, 0, sizeof(u64) * (CTR_TOTAL - CTR_POLY), st));
 
-    // A6a: mark the bricks the band can reach; prefix sum -> brick table
-    stage_mark(m, SDF_T_CLIP_SCAN, 0, st);
-    KL; brick_mark_kernel<<<(unsigned)((mv.F + 255) / 256), 256, 0, st>>>(mv, g, m->brick_flag);
-    CKS(launch_scan(BrickIn{m->brick_flag}, BrickOut{m->brick_table, m->brick_list}, nbricks, m->scan_ws, m->d_ctr + CTR_BRICKS, st));
-    CK(cudaGetLastError());
-
-    // host crossing: totals size the launch and the scratch
+    // A6a: brick table and its total (host crossing: the total sizes the launch and the scratch), unless
+    // sdf_transform already ran it beside the edge stage and fetched the total with the validation flags
     u64 bricks = 0;
-    CK(cudaMemcpyAsync(&bricks, m->d_ctr + CTR_BRICKS, sizeof(bricks), cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
-    stage_mark(m, SDF_T_CLIP_SCAN, 1, st);
+    if (hoisted) {
+        bricks = m->h_ctr[CTR_BRICKS];
+    } else {
+        CKS(prepare_bricks(m, g, st, st));
+        CK(cudaMemcpyAsync(&bricks, m->d_ctr + CTR_BRICKS, sizeof(bricks), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        stage_mark(m, SDF_T_CLIP_SCAN, 1, st);
+    }
     // fork the fill first: its CTAs claim their SMs while the GPU is still empty (the scratch
     // allocation and its clear come next), before the evaluate blocks flood it
     if (g.fill_mode == 4 && !prefilled) CKS(fork_fill());
@@ -788,7 +820,7 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
         stage_mark(m, SDF_T_EVALUATE, 1, st);
     }
     // A8b: join the fill, then overwrite the active bricks
-    if (forked) CK(cudaStreamWaitEvent(st, m->ev_join, 0));
+    if (forked) CK(cudaStreamWaitEvent(st, m->ev_fjoin, 0));
     else if (g.fill_mode == 2) CKS(launch_fill(st));
     if (bricks) {
         stage_mark(m, SDF_T_EMIT, 0, st);

@@ -717,6 +717,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     KL; vertex_record_kernel<<<blocks_for(V), FB, 0, vs>>>(m->soup, vcorner, vn64, vcosq, vside, V, vcospos, m->vrec, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_VERTICES, 1, vs);
+    CKS(maybe_prepare_bricks(m, st, vs));
     if (vs != st) {
         CK(cudaEventRecord(m->ev_join, vs));
         CK(cudaStreamWaitEvent(st, m->ev_join, 0));

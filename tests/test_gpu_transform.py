@@ -34,6 +34,27 @@ def test_transform_equals_two_calls(name, scale):
     m1.destroy(); m2.destroy()
 
 
+@pytest.mark.parametrize("name", ["C4", "C5"])
+def test_transform_equals_two_calls_full_size(name):
+    """BASELINE.json's full sizes, the call bench.py times: identical to sdf_create + sdf_compute, whose
+    results tests/test_gpu_fullsize.py checks against the oracle."""
+    w = W.config(name)
+    (m1, d1, t1), (m2, d2, t2) = _both(w)
+    assert torch.equal(t1, t2)
+    assert torch.equal(d1.view(torch.int32), d2.view(torch.int32))
+    assert B.sdf_stats(m1)["band_cells"] == B.sdf_stats(m2)["band_cells"] == int((t2 >= 0).sum())
+    m1.destroy(); m2.destroy()
+
+
+@pytest.mark.parametrize("hoist", ["0", "1"])
+def test_transform_brick_hoist_switch(hoist, monkeypatch):
+    monkeypatch.setenv("SDF_HOIST_BRICKS", hoist)
+    w = W.config("C2", 0.5)
+    (m1, d1, t1), (m2, d2, t2) = _both(w)
+    assert torch.equal(t1, t2) and torch.equal(d1.view(torch.int32), d2.view(torch.int32))
+    m1.destroy(); m2.destroy()
+
+
 @pytest.mark.parametrize("at", ["1", "2", "3", "4"])
 def test_transform_fill_start_points(at, monkeypatch):
     """SDF_PREFILL_AT ablation: wherever the sentinel fill starts, the result is the two-call one, bit for bit."""
