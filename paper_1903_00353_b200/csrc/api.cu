@@ -292,7 +292,7 @@ int sdf_compute_host(sdf_mesh *m, const float origin[3], float h, int nx, int ny
 int sdf_stats(sdf_mesh *m, sdf_stats_t *o) {
     if (!m || !o) return SDF_EINVAL;
     CK(cudaStreamSynchronize(m->last_stream));
-    static u64 all[CTR_TOTAL];
+    u64 all[CTR_TOTAL];            // on the stack: calls on distinct handles may run concurrently
     CK(cudaMemcpy(all, m->d_ctr, sizeof(u64) * CTR_TOTAL, cudaMemcpyDeviceToHost));
     memcpy(m->h_ctr, all, sizeof(u64) * CTR_COUNT);
     u64 *c = m->h_ctr;

@@ -177,5 +177,6 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
 int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st, bool prefilled = false);
 int start_prefill(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st);
 int maybe_prefill(sdf_mesh *m, int point, cudaStream_t st);
+int maybe_alloc_brick_ws(sdf_mesh *m, cudaStream_t st);
 int maybe_prepare_bricks(sdf_mesh *m, cudaStream_t st, cudaStream_t vs);
 int run_closest_points(sdf_mesh *m, const GridParams &g, const int *tri, float *cp, cudaStream_t st);

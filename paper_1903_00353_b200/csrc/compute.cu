@@ -712,12 +712,10 @@ static MeshView make_view(const sdf_mesh *m) {
     return mv;
 }
 
-// A6a: per-compute workspace (allocated in the order of stream `as`), then on stream `ps`: mark the bricks
-// the band can reach, prefix sum -> brick table, list and the total in d_ctr[CTR_BRICKS].  Needs the soup,
-// the face normals and V; sdf_transform runs it on the vertex stream beside the edge stage.
-int prepare_bricks(sdf_mesh *m, const GridParams &g, cudaStream_t as, cudaStream_t ps) {
-    const MeshView mv = make_view(m);
-    const int64_t P = mv.P;
+// A6a workspace: brick flags / table / list, scan partials, big-polyhedron list -- one slab, grown on demand,
+// taken in the order of stream `as`
+static int alloc_brick_ws(sdf_mesh *m, const GridParams &g, cudaStream_t as) {
+    const int64_t P = m->F + m->E + 2 * m->V;
     const int64_t nbricks = (int64_t)g.nbx * g.nby * g.nbz;
     for (int pass = 0; pass < 2; pass++) {
         Carver c(pass ? m->slab_ws : nullptr);
@@ -733,6 +731,15 @@ int prepare_bricks(sdf_mesh *m, const GridParams &g, cudaStream_t as, cudaStream
             m->slab_ws_cap = want;
         }
     }
+    return SDF_OK;
+}
+
+// A6a on stream `ps` (workspace already carved): mark the bricks the band can reach, prefix sum -> brick table,
+// list and the total in d_ctr[CTR_BRICKS].  Needs the soup, the face normals and V; sdf_transform runs it on the
+// vertex stream beside the edge stage.
+static int mark_bricks(sdf_mesh *m, const GridParams &g, cudaStream_t ps) {
+    const MeshView mv = make_view(m);
+    const int64_t nbricks = (int64_t)g.nbx * g.nby * g.nbz;
     m->ev_set[SDF_T_CLIP_SCAN] = false;
     CK(cudaMemsetAsync(m->brick_flag, 0, (size_t)nbricks, ps));
     CK(cudaMemsetAsync(m->d_ctr + CTR_POLY, 0, sizeof(u64) * (CTR_TOTAL - CTR_POLY), ps));
@@ -743,12 +750,18 @@ int prepare_bricks(sdf_mesh *m, const GridParams &g, cudaStream_t as, cudaStream
     return SDF_OK;
 }
 
+// sdf_transform, before build_features forks the vertex stream
+int maybe_alloc_brick_ws(sdf_mesh *m, cudaStream_t st) {
+    return m->hoist_g ? alloc_brick_ws(m, *m->hoist_g, st) : SDF_OK;
+}
+
 // sdf_transform: stage boundary of build_features after the vertex kernels (stream vs, forked from st)
 int maybe_prepare_bricks(sdf_mesh *m, cudaStream_t st, cudaStream_t vs) {
     if (!m->hoist_g) return SDF_OK;
     const GridParams *g = m->hoist_g;
     m->hoist_g = nullptr;
-    CKS(prepare_bricks(m, *g, st, vs));
+    (void)st;
+    CKS(mark_bricks(m, *g, vs));
     stage_mark(m, SDF_T_CLIP_SCAN, 1, vs);
     m->bricks_ready = true;        // the total travels with the validation flags (second host crossing)
     return SDF_OK;
@@ -789,7 +802,8 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
     if (hoisted) {
         bricks = m->h_ctr[CTR_BRICKS];
     } else {
-        CKS(prepare_bricks(m, g, st, st));
+        CKS(alloc_brick_ws(m, g, st));
+        CKS(mark_bricks(m, g, st));
         CK(cudaMemcpyAsync(&bricks, m->d_ctr + CTR_BRICKS, sizeof(bricks), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
         stage_mark(m, SDF_T_CLIP_SCAN, 1, st);

@@ -316,7 +316,7 @@ __global__ void __launch_bounds__(FB) edge_record_kernel(const int *__restrict__
                                                          const int *__restrict__ adj, const u32 *__restrict__ ebase,
                                                          const float *__restrict__ soup, const float *__restrict__ fn,
                                                          const int *__restrict__ perm,
-                                                         EdgeRec *__restrict__ erec, u64 *__restrict__ ctr) {
+                                                         EdgeRec *__restrict__ erec, int E, u64 *__restrict__ ctr) {
     __shared__ u32 s_cnt[3];
     if (threadIdx.x < 3) s_cnt[threadIdx.x] = 0;
     __syncthreads();
@@ -366,7 +366,10 @@ __global__ void __launch_bounds__(FB) edge_record_kernel(const int *__restrict__
             r.tri = x0 < x1 ? x0 : x1;
             r.cls = cls;
             r.pad[0] = r.pad[1] = 0;
-            erec[erank] = r;
+            // erec holds E = 3F/2 records: exactly the forward half-edges of a closed, oriented mesh.  A
+            // mis-oriented or open soup can have up to 2F of them; those ranks are dropped (the pair count
+            // below still exposes the mesh as invalid)
+            if (erank < E) erec[erank] = r;
             atomicAdd(&s_cnt[cls > 0 ? 0 : (cls < 0 ? 1 : 2)], 1u);      // knife edges count as convex
         }
     }
@@ -511,6 +514,15 @@ __global__ void __launch_bounds__(FB) vertex_record_kernel(const float *__restri
 // ---------------------------------------------------------------------------------------
 // host driver
 // ---------------------------------------------------------------------------------------
+// Work forked onto the vertex stream must not outlive an early (error) return: the temporaries it reads are
+// released on `st` by TmpPool, and sdf_destroy never sees that stream.  Declared AFTER the TmpPool it protects,
+// so it is destroyed (and the stream drained) first.
+struct StreamDrain {
+    cudaStream_t s; bool armed;
+    StreamDrain() : s(nullptr), armed(false) {}
+    ~StreamDrain() { if (armed) cudaStreamSynchronize(s); }
+};
+
 struct TmpPool {     // temporaries of sdf_create, released together
     const sdf_allocator *a; cudaStream_t st; void *p[24]; int n;
     TmpPool(const sdf_allocator *a_, cudaStream_t s) : a(a_), st(s), n(0) {}
@@ -566,6 +578,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     const int nc = (int)(3 * F);
     const sdf_allocator *al = &m->alloc;
     TmpPool tmp(al, st);
+    StreamDrain drain;
     m->E = nc / 2;
 
     // persistent F-sized tables: one slab
@@ -645,8 +658,12 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
                      m->d_ctr + CTR_V, st));
     stage_mark(m, SDF_T_INGEST_WELD, 1, st);
     // first host crossing: the vertex count sizes every per-vertex table
+    int hflags[4] = {0, 0, 0, 0};
     CK(cudaMemcpyAsync(m->h_ctr, m->d_ctr, sizeof(u64) * CTR_COUNT, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(hflags, m->d_flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    // non-finite input is rejected here: Inf / NaN coordinates would turn into whole-axis cell ranges downstream
+    if (hflags[0] & ERRB_NONFINITE) return SDF_EINVAL;
     m->V = (int64_t)m->h_ctr[CTR_V];
     const int V = (int)m->V;
 
@@ -679,6 +696,9 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     stage_mark(m, SDF_T_EDGES, 0, st);
     CK(cudaMemsetAsync(vacc, 0, (size_t)((char *)(vside + V) - (char *)vacc), st));
     KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wtab, slot, (int)F, m->cvid, m->fn, vacc, fcnt, etab, cape - 1, m->d_flags);
+    // sdf_transform: the per-compute workspace of A6a is taken in the order of `st` BEFORE the fork, so that the
+    // vertex stream (which first touches it) is ordered after the allocation
+    CKS(maybe_alloc_brick_ws(m, st));
     // the vertex stage needs only what tri_geom wrote: it runs on a second stream beside the edge stage
     cudaStream_t vs = st;
     {
@@ -697,12 +717,13 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
             if (!m->ev_join) CK(cudaEventCreateWithFlags(&m->ev_join, cudaEventDisableTiming));
             CK(cudaEventRecord(m->ev_fork, st));
             CK(cudaStreamWaitEvent(vs, m->ev_fork, 0));
+            drain.s = vs; drain.armed = true;
         }
     }
     CKS(launch_scan(FcntIn{fcnt}, EbaseOut{ebase}, F, scan_ws, (u64 *)nullptr, st));
     CKS(maybe_prefill(m, 3, st));
     KL; edge_pair_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, etab, cape - 1, m->adj);
-    KL; edge_record_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, m->adj, ebase, m->soup, m->fn, m->perm, m->erec, m->d_ctr);
+    KL; edge_record_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, m->adj, ebase, m->soup, m->fn, m->perm, m->erec, (int)m->E, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_EDGES, 1, st);
 
@@ -721,9 +742,9 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     if (vs != st) {
         CK(cudaEventRecord(m->ev_join, vs));
         CK(cudaStreamWaitEvent(st, m->ev_join, 0));
+        drain.armed = false;           // joined: `st` now carries the dependency
     }
     // second host crossing: validation flags + class counters
-    int hflags[4];
     CK(cudaMemcpyAsync(hflags, m->d_flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(m->h_ctr, m->d_ctr, sizeof(u64) * CTR_COUNT, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));

@@ -137,3 +137,48 @@ def test_fuzz_defective_input_statuses(oracle_mod):
         assert so == sg, (c, kind, so, sg)
         seen.add((kind, sg))
     assert {s for _, s in seen} >= {0, 1, 2, 3, 4}
+
+
+@pytest.mark.parametrize("name,scale", [("C2", 1.0), ("C3", 0.5)])
+def test_mass_defects_stay_in_bounds(oracle_mod, name, scale):
+    """Many defects at once (features.cu edge records): a soup whose every second triangle is flipped, and
+    one whose corners are all sorted, have far more than 3F/2 forward half-edges -- the edge-record table holds 3F/2.
+    Both calls must return the oracle's status, and a valid mesh built right afterwards must still be bit-identical
+    to one built before (nothing was scribbled over)."""
+    from paper_1903_00353_b200 import binding as B
+    w = f32_grid(W.config(name, scale) if scale < 1.0 else W.config(name))
+    good = np.ascontiguousarray(w.soup)
+    m0, d0, t0 = B.compute_workload(w)
+    torch.cuda.synchronize()
+    r = np.random.default_rng(4242)
+    variants = []
+    s = good.copy(); s[::2] = s[::2, ::-1]; variants.append(s)                       # every second triangle flipped
+    s = good.copy(); idx = r.random(len(s)) < 0.3; s[idx] = s[idx][:, ::-1]; variants.append(s)   # 30 % flipped
+    s = good.copy()                                                                # corners sorted lexicographically
+    for i in range(len(s)):
+        s[i] = s[i][np.lexsort((s[i][:, 2], s[i][:, 1], s[i][:, 0]))]
+    variants.append(s)
+    s = np.delete(good, r.choice(len(good), size=len(good) // 3, replace=False), axis=0); variants.append(s)   # a third missing
+    for vi, s in enumerate(variants):
+        s = np.ascontiguousarray(s, dtype=np.float32)
+        so = 0
+        try:
+            oracle_mod.Mesh(s)
+        except oracle_mod.OracleError as e:
+            so = e.status
+        assert so in (2, 3)
+        for call in ("create", "transform"):
+            sg = 0
+            try:
+                if call == "create":
+                    B.sdf_destroy(B.sdf_create(torch.from_numpy(s).cuda()))
+                else:
+                    B.sdf_transform(torch.from_numpy(s).cuda(), w.origin, w.h, w.dims, w.band)[0].destroy()
+            except B.SdfError as e:
+                sg = e.status
+            assert sg == so, (vi, call, so, sg)
+        m1, d1, t1 = B.compute_workload(w)
+        torch.cuda.synchronize()
+        assert torch.equal(t0, t1) and torch.equal(d0.view(torch.int32), d1.view(torch.int32)), vi
+        m1.destroy()
+    m0.destroy()
