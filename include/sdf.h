@@ -23,7 +23,8 @@
  * state for the first time (the first sdf_create / sdf_compute of a process create the library's
  * side streams: vertex stage, sentinel fill); distinct handles on distinct streams are otherwise independent.
  * Debug / ablation switches (environment, read per call): SDF_AABB_MODE=1 (candidates = band-expanded
- * triangle boxes only), SDF_FILL_MODE=0..4, SDF_SCHEDULER=serial | dynamic[:N], SDF_RUFF=cone, SDF_NO_BINNING=1,
+ * triangle boxes only), SDF_DISABLE=faces|wedges|cones (leave an extrusion class out: the parity harness must notice),
+ * SDF_FILL_MODE=0..4, SDF_SCHEDULER=serial | dynamic[:N], SDF_RUFF=cone, SDF_NO_BINNING=1,
  * SDF_CREATE_FORK=0 (vertex stage on the caller's stream), SDF_FILLINT_PLAIN=1 (interior fill without the blank map);
  * see DESIGN.md.
  */

@@ -160,6 +160,9 @@ static int make_grid(const float origin[3], float h, int nx, int ny, int nz, flo
     g->rb = band + g->guard + g->eps;
     const char *dbg = getenv("SDF_AABB_MODE");
     g->aabb_mode = (dbg && dbg[0] == '1') ? 1 : 0;
+    // harness self-test: leave an extrusion class out and watch parity break
+    const char *dis = getenv("SDF_DISABLE");
+    g->disable = !dis ? 0 : ((strstr(dis, "faces") ? 1 : 0) | (strstr(dis, "wedges") ? 2 : 0) | (strstr(dis, "cones") ? 4 : 0));
     const char *pf = getenv("SDF_FILL_MODE");
     g->fill_mode = (pf && pf[0] >= '0' && pf[0] <= '4') ? pf[0] - '0' : 4;
     const char *fd = getenv("SDF_FILL_DEPTH"), *fi = getenv("SDF_FILL_ISSUERS");

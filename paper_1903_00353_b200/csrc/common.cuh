@@ -98,6 +98,7 @@ struct GridParams {
     int serial_loop;                // ablation: the paper's thread-per-extrusion serial loop
     int cdp, cdp_serial_below;      // ablation: the paper's dynamic-parallelism scheduler (cdp.cu)
     int aabb_mode;                  // debug: candidates = band-expanded triangle AABBs only
+    int disable;                    // debug (harness self-test): extrusion classes left out, bit0 face slabs, bit1 edge wedges, bit2 vertex cones
     int vec4;                       // 1: nx % 4 == 0 and outputs 16-B aligned -> 128-bit stores
     int fill_mode;                  // 0: TMA fill on the side stream (default); debug: 1 plain stores on the
                                     // side stream, 2 TMA fill on the main stream before the emit, 3 ... first,

@@ -112,6 +112,7 @@ __device__ __forceinline__ bool poly_aabv(const MeshView &mv, const GridParams &
     if (p < mv.F) {
         // face slab: triangle swept by +-rb along its normal
         const float *T = mv.soup + 9 * p, *N = mv.fn + 3 * p;
+        emit = !(g.disable & 1);
 #pragma unroll
         for (int i = 0; i < 3; i++) {
             float lo = fminf(T[i], fminf(T[3 + i], T[6 + i])), hi = fmaxf(T[i], fmaxf(T[3 + i], T[6 + i]));
@@ -121,7 +122,7 @@ __device__ __forceinline__ bool poly_aabv(const MeshView &mv, const GridParams &
     } else if (p < (int64_t)mv.F + mv.E) {
         // edge wedge: segment swept by the arc between n1 and n2, radius rb
         const EdgeRec &r = mv.erec[p - mv.F];
-        emit = (r.cls != 0) && !g.aabb_mode;
+        emit = (r.cls != 0) && !g.aabb_mode && !(g.disable & 2);
         if (emit && r.cls == 2) {
             // knife edge: the cylinder of radius rb about the segment
 #pragma unroll
@@ -157,7 +158,7 @@ __device__ __forceinline__ bool poly_aabv(const MeshView &mv, const GridParams &
         int64_t q = p - mv.F - mv.E;
         const VertexRec &r = mv.vrec[q >> 1];
         int side = (int)(q & 1);
-        emit = ((r.info >> side) & 1) && !g.aabb_mode && !(side == 1 && r.cos_cone <= -1.0f);
+        emit = ((r.info >> side) & 1) && !g.aabb_mode && !(side == 1 && r.cos_cone <= -1.0f) && !(g.disable & 4);
         if (emit) {
             float sg = side ? -1.0f : 1.0f;
             float c = r.cos_cone, sn = sqrtf(fmaxf(0.0f, 1.0f - c * c));

@@ -48,6 +48,14 @@ def test_full_grid(oracle_mod, name):
     res = compare_to_oracle(d.cpu().numpy(), t.cpu().numpy(), d_ref, t_ref, w, om)
     assert res["ok"] and all(res[k] == 0 for k in KEYS), {k: v for k, v in res.items()}
     assert (stats["V"], stats["E"]) == (w.meta["V"], w.meta["E"])
+    # ids (clause 4): how many differ from the oracle's, and how.  "Ties" = the closest point lies on a shared edge /
+    # vertex and the GPU's triangle is as close as the oracle's to the rounding of the oracle's fp32 output (several
+    # ids are correct); "near" = accepted by the tolerance without being such a tie.  The near share
+    # is bounded: a kernel that ignored the lowest-id rule, or named a neighbouring triangle, would show up here.
+    print("ids %s: populated %d, id mismatches %d (share %.4f): ties %d, near %d (share %.2e), bad %d"
+          % (name, res["populated_ref"], res["id_mismatch_total"], res["id_mismatch_share"], res["id_mismatch_ties"],
+             res["id_mismatch_near"], res["id_near_share"], res["bad_id"]))
+    assert res["id_near_share"] <= 2e-3, res
 
 
 @pytest.mark.parametrize("name,slabs", [

@@ -407,3 +407,45 @@ def test_error_statuses():
     with pytest.raises(B.SdfError) as e:
         B.sdf_compute(m, (0, 0, 0), 0.01, (8, 8, 8), 2.6)       # band > 250 h
     assert e.value.status == B.SDF_EINVAL
+
+
+@pytest.mark.parametrize("what,expect_cells", [("cones", 20), ("wedges", 100), ("faces", 1000)])
+def test_harness_detects_a_missing_extrusion_class(oracle_mod, monkeypatch, what, expect_cells):
+    """SURVEY.md sec.4 / PAPER.md:402, 427: leave one extrusion class out of the scan conversion (SDF_DISABLE) on the
+    rotated torus and on a box: the comparison harness must report the coverage gap (distances too large, cells
+    missing at the rim of the band) -- never a sign or sentinel problem -- and the same call without the switch passes."""
+    ws = [f32_grid(W.config("C3", 0.25)), f32_grid(W.config("C1"))]
+    for w in ws:
+        _assert_ok(check_parity(w, oracle_mod))
+        monkeypatch.setenv("SDF_DISABLE", what)
+        res = check_parity(w, oracle_mod)
+        monkeypatch.delenv("SDF_DISABLE")
+        assert not res["ok"]
+        assert res["bad_dist"] + res["bad_set"] >= expect_cells, {k: res[k] for k in res if k != "stats"}
+        assert res["bad_sentinel"] == 0 and res["bad_id_range"] == 0
+        # a gap only ever makes a distance larger or a cell vanish (SURVEY.md 8(c): never too small)
+        assert res["populated_gpu"] <= res["populated_ref"]
+        _assert_ok(check_parity(w, oracle_mod))
+
+
+@pytest.mark.parametrize("name,scale", [("C1", 1.0), ("C2", 0.25), ("C3", 0.25), ("C5", 0.02)])
+def test_aabb_candidates_mode_meets_the_four_clauses(oracle_mod, monkeypatch, name, scale):
+    """with SDF_AABB_MODE=1 the candidates are the band-expanded triangle boxes (the oracle's
+    own loop on the GPU) instead of the characteristic polyhedra: parity must not change, only the pair count."""
+    from paper_1903_00353_b200 import binding as B
+    import torch
+    w = f32_grid(W.config(name, scale) if scale < 1.0 else W.config(name))
+    res0 = check_parity(w, oracle_mod)
+    _assert_ok(res0)
+    m0, d0, t0 = B.compute_workload(w)
+    monkeypatch.setenv("SDF_AABB_MODE", "1")
+    res1 = check_parity(w, oracle_mod)
+    m1, d1, t1 = B.compute_workload(w)
+    monkeypatch.delenv("SDF_AABB_MODE")
+    _assert_ok(res1)
+    assert res1["populated_gpu"] == res0["populated_gpu"]
+    assert res1["stats"]["pairs_tested"] > res0["stats"]["pairs_tested"]
+    # same cells, same signs, distances within an ulp of the coordinates (polyhedra only cull)
+    pop = torch.isfinite(d0)
+    assert torch.equal(pop, torch.isfinite(d1)) and torch.equal(torch.signbit(d0[pop]), torch.signbit(d1[pop]))
+    assert float((d0[pop] - d1[pop]).abs().max()) <= 2e-7

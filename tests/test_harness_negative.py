@@ -1,0 +1,206 @@
+"""The comparison harness must be able to FAIL (a missing extrusion shows as
+"pyramid" artefacts -- a harness that cannot see one proves nothing).  No GPU here: an oracle result stands in for
+the GPU output and is corrupted one thing at a time; each corruption must raise exactly the counter of the clause
+it violates (BASELINE.json north_star: populated set, distance, sign, id), and the untouched result must pass."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+from paper_1903_00353_b200 import workloads as W
+from helpers import compare_to_oracle
+
+KEYS = ("bad_sentinel", "bad_id_range", "bad_set", "bad_dist", "bad_sign", "bad_id")
+
+
+@pytest.fixture(scope="module")
+def case(oracle_mod):
+    w = W.config("C3", 0.12)                      # rotated torus, 61^3, band 3h: convex, concave and saddle parts
+    w = dataclasses.replace(w, origin=tuple(float(np.float32(v)) for v in w.origin), h=float(np.float32(w.h)),
+                            band=float(np.float32(w.band)))
+    om = oracle_mod.Mesh(w.soup)
+    d, t = om.sdf(w.origin, w.h, w.dims, w.band)
+    return w, om, d, t
+
+
+def _cmp(case, d, t):
+    w, om, d_ref, t_ref = case
+    return compare_to_oracle(d, t, d_ref, t_ref, w, om)
+
+
+def _only(res, key):
+    assert not res["ok"], res
+    assert res[key] > 0, (key, {k: res[k] for k in KEYS})
+    assert all(res[k] == 0 for k in KEYS if k != key), (key, {k: res[k] for k in KEYS})
+
+
+def _deep_cells(case, n=3):
+    """populated cells well inside the band (not within the band-edge exemption), spread over the grid"""
+    w, om, d, t = case
+    flat = np.flatnonzero(np.isfinite(d.reshape(-1)) & (np.abs(d.reshape(-1)) < 0.5 * w.band) & (np.abs(d.reshape(-1)) > 0.2 * w.h))
+    assert flat.size > 100
+    return flat[np.linspace(0, flat.size - 1, n).astype(int)]
+
+
+def test_untouched_result_passes(case):
+    w, om, d, t = case
+    res = _cmp(case, d.copy(), t.copy())
+    assert res["ok"] and res["populated_gpu"] == res["populated_ref"] > 1000 and res["id_mismatch_total"] == 0
+
+
+def test_dropped_cell_is_a_set_violation(case):
+    w, om, d, t = case
+    for c in _deep_cells(case):
+        d2, t2 = d.copy().reshape(-1), t.copy().reshape(-1)
+        d2[c], t2[c] = np.inf, -1
+        _only(_cmp(case, d2, t2), "bad_set")
+
+
+def test_cell_beyond_the_band_is_a_set_violation(case):
+    w, om, d, t = case
+    far = np.flatnonzero(~np.isfinite(d.reshape(-1)))
+    d_true, i_true = om.query(np.stack([np.asarray(w.origin)[a] + (far // s % n) * w.h for a, s, n in
+                                        ((0, 1, w.dims[0]), (1, w.dims[0], w.dims[1]), (2, w.dims[0] * w.dims[1], w.dims[2]))], axis=1))
+    pick = far[np.abs(d_true) > 1.5 * w.band][:3]
+    assert pick.size == 3
+    for c in pick:
+        d2, t2 = d.copy().reshape(-1), t.copy().reshape(-1)
+        d2[c], t2[c] = np.float32(0.9 * w.band), 0           # looks like a band value, but the cell is far outside
+        _only(_cmp(case, d2, t2), "bad_set")
+
+
+def test_cell_at_the_band_edge_is_exempt(case):
+    """clause 1's own exemption: a cell whose true |d| is within 1e-5 h of the band may be in either set"""
+    w, om, d, t = case
+    # move the band instead of hunting for such a cell: compare against an oracle run whose band ends 0.5e-5 h past a cell's |d|
+    flat = np.flatnonzero(np.isfinite(d.reshape(-1)))
+    c = flat[np.argmax(np.abs(d.reshape(-1)[flat]))]
+    d_true = abs(float(om.query(_xyz(w, np.array([c])))[0][0]))
+    w2 = dataclasses.replace(w, band=d_true + 0.5e-5 * w.h)
+    d_ref, t_ref = om.sdf(w2.origin, w2.h, w2.dims, w2.band)
+    assert np.isfinite(d_ref.reshape(-1)[c])
+    d2, t2 = d_ref.copy().reshape(-1), t_ref.copy().reshape(-1)
+    d2[c], t2[c] = np.inf, -1                                 # dropping THIS cell is allowed ...
+    res = compare_to_oracle(d2, t2, d_ref, t_ref, w2, om)
+    assert res["ok"] and res["set_diff_total"] == 1 and res["bad_set"] == 0
+    w3 = dataclasses.replace(w, band=d_true + 3e-5 * w.h)     # ... but not with the band 3e-5 h away
+    d_ref, t_ref = om.sdf(w3.origin, w3.h, w3.dims, w3.band)
+    d2, t2 = d_ref.copy().reshape(-1), t_ref.copy().reshape(-1)
+    d2[c], t2[c] = np.inf, -1
+    _only(compare_to_oracle(d2, t2, d_ref, t_ref, w3, om), "bad_set")
+
+
+def _xyz(w, idx):
+    nx, ny, nz = w.dims
+    o = np.asarray(w.origin, dtype=np.float64)
+    return np.stack([o[0] + (idx % nx) * w.h, o[1] + (idx // nx % ny) * w.h, o[2] + (idx // (nx * ny)) * w.h], axis=1)
+
+
+def test_shifted_distance_is_a_distance_violation(case):
+    w, om, d, t = case
+    tol = 1e-5 * w.h + 1e-6 * w.diag
+    for c in _deep_cells(case):
+        for shift in (2.0 * tol, -2.0 * tol):
+            d2 = d.copy().reshape(-1)
+            d2[c] = np.float32(d2[c] + np.copysign(shift, d2[c]) if shift > 0 else d2[c] - np.copysign(-shift, d2[c]))
+            _only(_cmp(case, d2, t.copy()), "bad_dist")
+        d2 = d.copy().reshape(-1)
+        d2[c] = np.float32(d2[c] + 0.4 * tol)                  # inside the tolerance: accepted
+        assert _cmp(case, d2, t.copy())["ok"]
+
+
+def test_flipped_sign_is_a_sign_violation(case):
+    w, om, d, t = case
+    for c in _deep_cells(case):
+        d2 = d.copy().reshape(-1)
+        if abs(d2[c]) <= 0.5 * (1e-5 * w.h + 1e-6 * w.diag):
+            continue
+        d2[c] = -d2[c]
+        res = _cmp(case, d2, t.copy())
+        assert not res["ok"] and res["bad_sign"] > 0           # (a flipped sign is also a distance error of 2|d|)
+        assert all(res[k] == 0 for k in KEYS if k not in ("bad_sign", "bad_dist"))
+
+
+def test_wrong_id_is_an_id_violation_but_a_tying_id_is_not(case):
+    w, om, d, t = case
+    F = w.ntri
+    for c in _deep_cells(case):
+        t2 = t.copy().reshape(-1)
+        t2[c] = (t2[c] + F // 2) % F                          # a triangle on the other side of the torus
+        res = _cmp(case, d.copy(), t2)
+        _only(res, "bad_id")
+        assert res["id_mismatch_total"] == 1 and res["id_mismatch_ties"] == 0
+    # a cell whose closest point is on an edge: the other triangle of that edge ties exactly and must be accepted
+    flat = np.flatnonzero(np.isfinite(d.reshape(-1)))
+    found = 0
+    adj = _edge_neighbours(w.soup)
+    for c in flat[:: max(1, flat.size // 4000)]:
+        tc = int(t.reshape(-1)[c])
+        for tn in adj[tc]:
+            d_alt = om.dist_to_triangles(_xyz(w, np.array([c])), np.array([tn], dtype=np.int32))[0]
+            if abs(d_alt - abs(float(om.query(_xyz(w, np.array([c])))[0][0]))) <= 1e-13:
+                t2 = t.copy().reshape(-1)
+                t2[c] = tn
+                res = _cmp(case, d.copy(), t2)
+                assert res["ok"] and res["id_mismatch_total"] == 1 and res["id_mismatch_ties"] == 1, res
+                found += 1
+                break
+        if found >= 3:
+            break
+    assert found >= 3
+
+
+def _edge_neighbours(soup):
+    """triangles sharing an edge with each triangle (exact vertex bits), numpy only"""
+    F = soup.shape[0]
+    _, vid = np.unique(soup.reshape(-1, 3).view([("", soup.dtype)] * 3), return_inverse=True)
+    vid = vid.reshape(F, 3)
+    owners = {}
+    for tix in range(F):
+        for k in range(3):
+            e = tuple(sorted((int(vid[tix, k]), int(vid[tix, (k + 1) % 3]))))
+            owners.setdefault(e, []).append(tix)
+    adj = [[] for _ in range(F)]
+    for e, ts in owners.items():
+        if len(ts) == 2:
+            adj[ts[0]].append(ts[1]); adj[ts[1]].append(ts[0])
+    return adj
+
+
+def test_bad_sentinels_and_id_range(case):
+    w, om, d, t = case
+    out = np.flatnonzero(~np.isfinite(d.reshape(-1)))[:1]
+    for dv, tv in ((np.inf, 5), (-np.inf, -1), (np.nan, -1)):
+        d2, t2 = d.copy().reshape(-1), t.copy().reshape(-1)
+        d2[out], t2[out] = dv, tv
+        _only(_cmp(case, d2, t2), "bad_sentinel")
+    c = _deep_cells(case)[:1]
+    for tv in (-1, -7, w.ntri, 2 ** 31 - 1):
+        t2 = t.copy().reshape(-1)
+        t2[c] = tv
+        res = _cmp(case, d.copy(), t2)
+        assert not res["ok"] and res["bad_id_range"] > 0
+
+
+def test_missing_extrusion_class_shows(case, oracle_mod):
+    """What a missing extrusion class does to the result: with the vertex cones left out, cells
+    whose closest feature is a vertex get the distance of the nearest face or edge instead -- too large, or, at the
+    rim of the band, missing.  Emulated here with the oracle: a cell closest to a vertex gets the distance to the
+    clamped second-best feature; the harness must call it a distance violation (and a set violation where the
+    larger value leaves the band)."""
+    w, om, d, t = case
+    flat = np.flatnonzero(np.isfinite(d.reshape(-1)))
+    x = _xyz(w, flat)
+    # cells strictly closest to a mesh vertex: distance to the nearest vertex equals the distance to the surface
+    verts = np.unique(w.soup.reshape(-1, 3).astype(np.float64), axis=0)
+    dv = np.min(np.linalg.norm(x[:, None, :] - verts[None, :, :], axis=2), axis=1)
+    at_vertex = flat[np.abs(dv - np.abs(d.reshape(-1)[flat].astype(np.float64))) < 1e-6 * w.h]
+    assert at_vertex.size > 50                 # the outer half of the torus is convex: its vertices own cone cells
+    d2, t2 = d.copy().reshape(-1), t.copy().reshape(-1)
+    grew = np.float32(1.0 + 1e-3)              # what the edge / face next to the vertex would give: a larger value
+    d2[at_vertex] = d2[at_vertex] * grew
+    gone = np.abs(d2[at_vertex]) >= np.float32(w.band)
+    d2[at_vertex[gone]], t2[at_vertex[gone]] = np.inf, -1
+    res = _cmp(case, d2, t2)
+    assert not res["ok"] and res["bad_dist"] > 0
+    assert res["bad_dist"] + res["bad_set"] >= 0.5 * at_vertex.size

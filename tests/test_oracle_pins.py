@@ -366,3 +366,48 @@ def test_status_codes(oracle_mod):
     z2 = z.copy()
     z2[0][z2[0] == 0] = -0.0
     assert oracle_mod.Mesh(z2).counts == oracle_mod.Mesh(z).counts
+
+
+def test_dist_to_triangles_pinned(oracle_mod):
+    """oracle_dist_to_triangles decides clause 4 of the comparison harness (an id mismatch is accepted only if the
+    GPU's triangle is as close as the oracle's within the tolerance), so it gets its own pin: against the independent
+    numpy formulation (projection + three clamped segments) on random (point, id) pairs -- near and far points, every
+    Voronoi region of slivers and fat triangles alike -- against hand-derived closed forms, and out-of-range ids -> inf."""
+    r = np.random.default_rng(77)
+    v, t = W.torus_mesh(0.6, 0.25, 24, 12)
+    soup = W.soup_from_indexed(v, t, r)
+    om = oracle_mod.Mesh(soup)
+    F = soup.shape[0]
+    n = 20000
+    ids = r.integers(0, F, n).astype(np.int32)
+    # points around the named triangle (all seven regions) and far from it
+    bary = r.dirichlet((0.6, 0.6, 0.6), n) * 2.0 - 0.5                  # in- and outside the triangle
+    on = np.einsum("nk,nkc->nc", bary, soup[ids].astype(np.float64))
+    pts = on + r.normal(0.0, 1.0, (n, 3)) * r.choice([1e-6, 1e-3, 0.05, 1.0], n)[:, None]
+    d = om.dist_to_triangles(pts, ids)
+    ref = point_triangle_dist(pts, soup[ids])
+    assert np.max(np.abs(d - ref)) <= 1e-12
+    assert np.all(d >= 0)
+    # it is the distance to THAT triangle: never below the distance to the whole mesh, equal for the closest id
+    dq, iq = om.query(pts[:2000])
+    assert np.all(d[:2000] >= np.abs(dq) - 1e-12)
+    assert np.max(np.abs(om.dist_to_triangles(pts[:2000], iq) - np.abs(dq))) <= 1e-12
+    # a transposed operand / wrong id would show here: the triangle with the next id is (almost always) farther or nearer
+    d_next = om.dist_to_triangles(pts, (ids + 1) % F)
+    assert np.mean(np.abs(d_next - d) > 1e-9) > 0.9
+    # closed forms on triangle 0 of a tetrahedron
+    tet = W.soup_from_indexed(*W.tetrahedron_mesh(0.5), np.random.default_rng(1))
+    o1, tri = oracle_mod.Mesh(tet), tet[:1]
+    a, b, c = (tri[0, k].astype(np.float64) for k in range(3))
+    nrm = np.cross(b - a, c - a); nrm /= np.linalg.norm(nrm)
+    cen = (a + b + c) / 3
+    q = np.stack([cen + 0.3 * nrm,                       # above the centroid: plane distance
+                  a + 2.0 * (a - cen),                   # beyond vertex a on the ray from the centroid: |p - a|
+                  0.5 * (a + b) + 0.7 * np.cross(b - a, nrm) / np.linalg.norm(b - a)])   # beside edge ab, in plane
+    dd = o1.dist_to_triangles(q, np.zeros(3, dtype=np.int32))
+    assert abs(dd[0] - 0.3) <= 1e-12
+    assert abs(dd[1] - 2.0 * np.linalg.norm(a - cen)) <= 1e-12
+    assert abs(dd[2] - 0.7) <= 1e-12
+    # ids outside [0, F) -> +inf, never a crash or a wrapped index
+    bad = om.dist_to_triangles(pts[:4], np.array([-1, F, F + 7, -2 ** 31], dtype=np.int32))
+    assert np.all(np.isposinf(bad))
