@@ -37,8 +37,22 @@ from paper_1903_00353_b200 import workloads as W  # noqa: E402
 METRIC = "narrow_band_sdf_cells_per_s"
 UNIT = "band cells/s"
 L2_BYTES = 126 * 1024 * 1024
-# dram__bytes_read.sum + dram__bytes_write.sum of fill_tma_kernel at C4 (profiles/r1_final_ncu_full.md)
-NCU_FILL_TRAFFIC_C4 = 0.185088e6 + 8.531763e9
+# dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed `ncu --set full` captures:
+# rows "config,kernel,dram_bytes_read,dram_bytes_write,source" (profiles/kernel_traffic.md names the commands)
+TRAFFIC_CSV = os.path.join("profiles", "kernel_traffic.csv")
+FLOP_PER_PAIR = 40.0          # <= 5 half-plane tests + one feature distance per (cell, polyhedron) pair
+
+# stage -> (the kernel that dominates it, what its algorithmic bytes are); F triangles, N cells, E edges, V vertices
+STAGE_KERNEL = {
+    "fill": ("fill_tma_kernel", "A8a dense write of both grids, cp.async.bulk shared->global: 8 B per cell"),
+    "evaluate": ("evaluate_small_kernel", "A5-A7: every feature record read once (36 B per face, 64 B per edge, 32 B per vertex)"),
+    "emit": ("emit_bricks_kernel", "A8b: 8 B of packed scratch read + 8 B written per cell of an active brick"),
+    "ingest_weld": ("ingest_weld_kernel", "A0/A1: the soup read once and written once in the internal order, 72 B per triangle"),
+    "edges": ("tri_geom_kernel", "A2/A3: the soup read once, 36 B per triangle"),
+    "vertices": ("vertex_cone_kernel", "A3/A4: the soup read once, 36 B per triangle"),
+    "clip_scan": ("brick_mark_kernel", "A6a: the soup read once, 36 B per triangle"),
+    "clear": ("cudaMemsetAsync", "scratch reset: 8 B per cell of an active brick"),
+}
 
 
 # --------------------------------------------------------------------------------------- #
@@ -106,25 +120,45 @@ class ClockSampler:
         return out
 
 
+def kernel_traffic(config, kernel):
+    """(dram bytes per launch, where from) out of the committed ncu summary, or (None, None)."""
+    path = os.path.join(ROOT, TRAFFIC_CSV)
+    if not os.path.exists(path):
+        return None, None
+    with open(path) as f:
+        for line in f:
+            r = [c.strip() for c in line.split(",")]
+            if len(r) >= 5 and r[0] == config and r[1] == kernel:
+                try:
+                    return float(r[2]) + float(r[3]), "%s (%s)" % (TRAFFIC_CSV, r[4])
+                except ValueError:
+                    continue
+    return None, None
+
+
 def dist_env():
     return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
 
 
 def sample_slab(w, nslices):
-    """Bounded sample of the workload for the oracle: the central z-slab of `nslices` slices."""
+    """Bounded sample of the workload for the oracle: `nslices` z-slices starting one brick below the lowest slice
+    the band reaches -- at C4 that slab holds the south pole (a valence-2000 fan of slivers, the expensive part for
+    the oracle) and the surface up to the equator's neighbourhood, not just the easy middle of the mesh."""
     nx, ny, nz = w.dims
     ns = min(nslices, nz)
-    k0 = (nz - ns) // 2
-    return w.crop((0, 0, k0), (nx, ny, ns)), "central z-slab k in [%d,%d) of %d slices, full mesh" % (k0, k0 + ns, nz)
+    zmin = float(w.soup[:, :, 2].min())
+    k0 = int(np.floor((zmin - w.band - w.origin[2]) / w.h)) - 8
+    k0 = max(0, min(k0, nz - ns))
+    return w.crop((0, 0, k0), (nx, ny, ns)), "z-slab k in [%d,%d) of %d slices (from the lowest slice of the band upwards), full mesh" % (k0, k0 + ns, nz)
 
 
 # --------------------------------------------------------------------------------------- #
 # reference arm: the CPU oracle, as it stands, on the host cores
 # --------------------------------------------------------------------------------------- #
-def time_oracle(w, nslices, steps, warmup):
+def time_oracle(w, nslices, steps, warmup, threads=None):
     import oracle
     oracle.build()
-    cores = oracle.default_threads()
+    cores = threads or oracle.default_threads()
     t0 = time.perf_counter()
     om = oracle.Mesh(w.soup)
     build_s = time.perf_counter() - t0
@@ -247,9 +281,11 @@ def run_ours(args):
     for _ in range(max(args.warmup, 0)):
         step_device().destroy()
     # ---- timed: K steps, device-resident inputs and outputs
-    B.sdf_enable_timing(True)
+    # only the dense writer (the kernel `roofline` is quoted on) is instrumented inside the timed steps: two event
+    # records on the library's side stream; the full stage breakdown comes from a separate pass below
+    B.sdf_enable_timing(2)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    stage_sum, stats = {}, None
+    fill_sum, stats = 0.0, None
     clocks = ClockSampler(torch.cuda.current_device())
     barrier()
     clocks.start()
@@ -261,8 +297,7 @@ def run_ours(args):
         ev[i][0].record(stream)
         m = step_device()
         ev[i][1].record(stream)
-        for k, v in B.sdf_get_timings(m).items():        # synchronises the stream
-            stage_sum[k] = stage_sum.get(k, 0.0) + v
+        fill_sum += B.sdf_get_timings(m)["fill"]         # synchronises the stream
         if i == args.steps - 1:
             stats = B.sdf_stats(m)
         m.destroy()
@@ -270,7 +305,17 @@ def run_ours(args):
     t_wall = time.perf_counter() - t_wall
     launches = B.sdf_launch_count() - l0
     clk = clocks.stop()
-    B.sdf_enable_timing(False)
+    # ---- stage breakdown (not part of the timed region): a few more steps with every stage instrumented
+    B.sdf_enable_timing(1)
+    stage_sum, nbr = {}, max(1, min(args.steps, args.breakdown_steps))
+    for _ in range(nbr):
+        if flush_buf is not None:
+            flush_buf.zero_()
+        m = step_device()
+        for k, v in B.sdf_get_timings(m).items():
+            stage_sum[k] = stage_sum.get(k, 0.0) + v
+        m.destroy()
+    B.sdf_enable_timing(0)
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = float(sum(step_ms))
     if world > 1:
@@ -362,34 +407,58 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (stage durations from CUDA events on the launch stream)
+    # ---- roofline of the dominant kernel
     peak, peak_src = measured_peaks()
-    stage_ms = {k: v / args.steps for k, v in stage_sum.items()}
+    stage_ms = {k: v / nbr for k, v in stage_sum.items()}
     dom = max(stage_ms, key=stage_ms.get)
-    # dominant kernel = the dense writer of both grids (fill_tma_kernel, A8a): 8 B per cell,
-    # written once; timed by CUDA events on the library's side stream, where it
-    # runs concurrently with the evaluate kernels (A5-A7) of the same step -- so this is the
-    # in-step (contended) figure; profiles/ holds the same kernel timed alone
-    fill_ms = stage_ms.get("fill") or 0.0
-    fill_gbs = 8.0 * N / (fill_ms * 1e-3) / 1e9 if fill_ms else 0.0
-    roofline = {"bound": "hbm", "kernel": "fill_tma_kernel (A8a dense write of both grids, cp.async.bulk shared->global)",
-                "achieved": fill_gbs, "peak": peak, "unit": "GB/s", "frac": fill_gbs / peak,
-                "traffic": args.traffic if args.traffic is not None else (NCU_FILL_TRAFFIC_C4 if w.name == "C4" and not zslab else None),
-                "peak_source": peak_src, "algorithmic_bytes_per_launch": 8.0 * N,
-                "ms_per_launch": fill_ms, "dominant_stage": dom}
+    F_, E_, V_ = w.ntri, 3 * w.ntri // 2, int(stats["V"])
+    bricks = int(stats["bricks_active"])
+    alg_bytes = {"fill": 8.0 * N, "evaluate": 36.0 * F_ + 64.0 * E_ + 32.0 * V_, "emit": 16.0 * 512 * bricks,
+                 "ingest_weld": 72.0 * F_, "edges": 36.0 * F_, "vertices": 36.0 * F_, "clip_scan": 36.0 * F_,
+                 "clear": 8.0 * 512 * bricks}
+    kern, what = STAGE_KERNEL[dom]
+    # the dense writer is timed live in every timed step (CUDA events on the library's side stream, where it runs
+    # beside the evaluate kernels: the in-step, contended figure); any other stage by the breakdown pass
+    dom_ms = (fill_sum / args.steps) if dom == "fill" else stage_ms[dom]
+    dom_gbs = alg_bytes[dom] / (dom_ms * 1e-3) / 1e9 if dom_ms else 0.0
+    traffic, traffic_src = kernel_traffic(w.name, kern) if not zslab else (None, None)
+    if args.traffic is not None:
+        traffic, traffic_src = args.traffic, "--traffic"
+    roofline = {"bound": "hbm", "kernel": "%s (%s)" % (kern, what), "achieved": dom_gbs, "peak": peak, "unit": "GB/s",
+                "frac": dom_gbs / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg_bytes[dom], "ms_per_launch": dom_ms, "dominant_stage": dom,
+                "timed": "live in the %d timed steps" % args.steps if dom == "fill" else "breakdown pass of %d steps" % nbr}
+    if dom != "fill" and stage_ms.get("fill"):
+        fg = 8.0 * N / (fill_sum / args.steps * 1e-3) / 1e9
+        roofline["dense_writer"] = {"kernel": "fill_tma_kernel", "achieved": fg, "frac": fg / peak,
+                                    "ms_per_launch": fill_sum / args.steps, "algorithmic_bytes_per_launch": 8.0 * N}
+    # north_star: the slower of (grid + feature bytes at HBM peak) and (pair evaluations at FP32 peak)
+    fp32_tf, sms = B.sdf_measure_fp32_peak(stream=stream)
     step_bytes = 8.0 * N + 36.0 * w.ntri
-    roofline_step = {"bound": "hbm", "algorithmic_bytes": step_bytes, "ideal_ms": step_bytes / (peak * 1e9) * 1e3,
-                     "frac": step_bytes / (peak * 1e9) * 1e3 / ms_per_step}
+    hbm_ms = step_bytes / (peak * 1e9) * 1e3
+    fp32_ms = float(stats["pairs_accepted"]) * FLOP_PER_PAIR / (fp32_tf * 1e12) * 1e3
+    ideal_ms = max(hbm_ms, fp32_ms)
+    roofline_step = {"bound": "hbm" if hbm_ms >= fp32_ms else "fp32", "algorithmic_bytes": step_bytes, "hbm_ms": hbm_ms,
+                     "fp32_peak_tflops": fp32_tf, "fp32_peak_source": "measured: sdf_measure_fp32_peak, FMA loop on %d SMs" % sms,
+                     "algorithmic_flop": float(stats["pairs_accepted"]) * FLOP_PER_PAIR, "fp32_ms": fp32_ms,
+                     "ideal_ms": ideal_ms, "frac": ideal_ms / ms_per_step}
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         r = time_oracle(w, args.cpu_slices, 1, 0)
         cpu = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        # "plus a 1-thread time on C1-C3" -- bounded samples of each, one thread
+        one = {}
+        for cn, sl in (("C1", 64), ("C2", 24), ("C3", 12)):
+            r1 = time_oracle(W.config(cn), sl, 1, 0, threads=1)
+            one[cn] = {"value": r1["value"], "s": r1["s_per_step"], "band_cells": r1["band_cells"], "sample": r1["sample"].split(";")[0]}
+        cpu["one_thread"] = one
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if zslab and world > 1 else "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(w, args),
-            "band_cells": band_cells, "stage_ms": stage_ms, "step_ms_min": min(step_ms), "step_ms_max": max(step_ms), "wall_ms_per_step":
+            "band_cells": band_cells, "stage_ms": stage_ms, "step_ms_min": min(step_ms), "step_ms_median": float(np.median(step_ms)),
+            "step_ms_max": max(step_ms), "wall_ms_per_step":
             t_wall * 1e3 / args.steps, "roofline": roofline, "roofline_step": roofline_step, "cpu_baseline": cpu,
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clk, "zslab": zslab, "fill_interior": fill_int, "closest_points": cpt,
             "stats": {k: stats[k] for k in ("polyhedra", "work_items", "pairs_tested", "pairs_accepted",
@@ -414,14 +483,15 @@ def main():
     ap.add_argument("--zslab-part", type=int, default=0)
     ap.add_argument("--split-calls", action="store_true",
                     help="step = sdf_create + sdf_compute (two calls) instead of sdf_transform (the same path in one call)")
+    ap.add_argument("--breakdown-steps", type=int, default=3, help="extra untimed steps with every stage instrumented (stage_ms)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-slices", type=int, default=256, help="z-slices of the oracle sample (cpu_baseline)")
     ap.add_argument("--ref-slices", type=int, default=64, help="z-slices per step of --impl reference")
     ap.add_argument("--traffic", type=float, default=None,
-                    help="dram bytes (read + write) per launch of the dominant kernel from the committed "
-                         "ncu --set full capture; default: the C4 figure of profiles/r1_final_ncu_full.md")
+                    help="dram bytes (read + write) per launch of the dominant kernel; default: read from "
+                         "profiles/kernel_traffic.csv (the committed ncu --set full captures)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -275,7 +275,9 @@ int sdf_get_table(sdf_mesh *m, int which, void *dst, size_t bytes);
 /*
  * Stage timing (measurement support).  sdf_enable_timing(1) makes every
  * later sdf_create / sdf_compute record CUDA events around its stages ON THE STREAM IT WAS
- * GIVEN (no extra synchronisation); sdf_get_timings synchronises that stream and returns
+ * GIVEN (no extra synchronisation); sdf_enable_timing(2) records only the two events around the
+ * dense sentinel write (SDF_T_FILL, the kernel the roofline is quoted on), so that a timed step
+ * carries next to no instrumentation; 0 switches it off.  sdf_get_timings synchronises that stream and returns
  * the durations, in milliseconds, of the stages of the handle's sdf_create and of its last
  * sdf_compute.  ms: HOST array of SDF_T_COUNT floats (n must equal SDF_T_COUNT); a stage
  * that did not run reports 0.
@@ -295,6 +297,16 @@ enum {
 };
 int sdf_enable_timing(int on);
 int sdf_get_timings(sdf_mesh *m, float *ms, int n);
+
+/*
+ * sdf_measure_fp32_peak -- measurement support for the FP32 leg of the roofline (BASELINE.json north_star: "the
+ * candidate cell x feature distance evaluations at FP32 peak"): runs a register-resident FMA loop
+ * (16 independent chains per thread, 2048 threads per SM) six times on `stream`, synchronises, and returns the best
+ * rate in TFLOP/s (2 flop per FMA) in *tflops_out (HOST); *sm_count_out (HOST, may be NULL) receives the SM count.
+ * Nominal on a B200: 148 SMs x 128 FMA lanes x 2 x 1.965 GHz = 74.4 TFLOP/s.
+ * Errors: SDF_EINVAL, SDF_ENOMEM, SDF_ECUDA.
+ */
+int sdf_measure_fp32_peak(double *tflops_out, int *sm_count_out, void *stream);
 
 /* Number of CUDA kernels this library has launched in this process so far. */
 int64_t sdf_launch_count(void);

@@ -24,7 +24,7 @@ TABLE_CORNER_VID, TABLE_HALFEDGE_ADJ, TABLE_FACE_NORMAL, TABLE_VERTEX_REC, TABLE
 
 EXPORTS = ("sdf_create", "sdf_transform", "sdf_compute", "sdf_compute_host", "sdf_zslab", "sdf_compute_zslab", "sdf_fill_interior", "sdf_closest_points", "sdf_stats", "sdf_get_table",
            "sdf_destroy", "sdf_strerror", "sdf_last_cuda_error", "sdf_version",
-           "sdf_enable_timing", "sdf_get_timings", "sdf_launch_count",
+           "sdf_enable_timing", "sdf_get_timings", "sdf_launch_count", "sdf_measure_fp32_peak",
            "sdf_read_stl", "sdf_free_host", "sdf_write_stl", "sdf_write_grid")
 
 TIMING_STAGES = ("ingest_weld", "edges", "vertices", "clip_scan", "clear", "evaluate", "emit", "fill")
@@ -127,6 +127,8 @@ def lib():
     L.sdf_enable_timing.restype = C.c_int
     L.sdf_get_timings.argtypes = [vp, C.POINTER(C.c_float), C.c_int]
     L.sdf_get_timings.restype = C.c_int
+    L.sdf_measure_fp32_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_int), vp]
+    L.sdf_measure_fp32_peak.restype = C.c_int
     L.sdf_launch_count.argtypes = []
     L.sdf_launch_count.restype = C.c_int64
     _lib = L
@@ -425,8 +427,19 @@ def sdf_get_table(mesh: Mesh, which: int) -> np.ndarray:
     return out
 
 
-def sdf_enable_timing(on: bool):
-    lib().sdf_enable_timing(1 if on else 0)
+def sdf_measure_fp32_peak(stream=None):
+    """(TFLOP/s of an FMA loop on every SM, SM count): the FP32 leg of the roofline (measurement support)."""
+    _torch()
+    tf, sms = C.c_double(0.0), C.c_int(0)
+    st = lib().sdf_measure_fp32_peak(C.byref(tf), C.byref(sms), C.c_void_p(_stream_ptr(stream)))
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_measure_fp32_peak")
+    return float(tf.value), int(sms.value)
+
+
+def sdf_enable_timing(on):
+    """0 / False: off; 1 / True: every stage; 2: only the dense sentinel write (SDF_T_FILL)."""
+    lib().sdf_enable_timing(int(on))
 
 
 def sdf_get_timings(mesh: Mesh) -> dict:

@@ -14,7 +14,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libsdf_b200.so")
-SOURCES = ["api.cu", "features.cu", "compute.cu", "fill.cu", "stl_io.cu"]
+SOURCES = ["api.cu", "features.cu", "compute.cu", "fill.cu", "stl_io.cu", "peaks.cu"]
 RDC_SOURCES = ["cdp.cu"]          # device-side launches (the dynamic-parallelism ablation): relocatable device code
 HEADERS = ["common.cuh", "primitives.cuh", "evaluate.cuh", os.path.join("..", "..", "include", "sdf.h")]
 ARCH_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a"]

@@ -10,7 +10,7 @@ int g_timing = 0;
 long long g_launch_count = 0;
 
 void stage_mark(sdf_mesh *m, int stage, int which, cudaStream_t st) {
-    if (!g_timing) return;
+    if (!g_timing || (g_timing == 2 && stage != SDF_T_FILL)) return;
     if (!m->ev[stage][which] && cudaEventCreate(&m->ev[stage][which]) != cudaSuccess) {
         m->ev[stage][which] = nullptr;
         (void)cudaGetLastError();
@@ -58,7 +58,7 @@ extern "C" {
 
 int sdf_version(void) { return 100; }
 int64_t sdf_launch_count(void) { return (int64_t)g_launch_count; }
-int sdf_enable_timing(int on) { g_timing = on ? 1 : 0; return SDF_OK; }
+int sdf_enable_timing(int on) { g_timing = on == 2 ? 2 : (on ? 1 : 0); return SDF_OK; }
 
 int sdf_get_timings(sdf_mesh *m, float *ms, int n) {
     if (!m || !ms || n != SDF_T_COUNT) return SDF_EINVAL;
