@@ -25,7 +25,8 @@
  * Debug / ablation switches (environment, read per call): SDF_AABB_MODE=1 (candidates = band-expanded
  * triangle boxes only), SDF_DISABLE=faces|wedges|cones (leave an extrusion class out: the parity harness must notice),
  * SDF_FILL_MODE=0..4, SDF_SCHEDULER=serial | dynamic[:N], SDF_RUFF=cone, SDF_NO_BINNING=1,
- * SDF_CREATE_FORK=0 (vertex stage on the caller's stream), SDF_FILLINT_PLAIN=1 (interior fill without the blank map);
+ * SDF_CREATE_FORK=0 (vertex stage on the caller's stream), SDF_SMOOTH_SIN=x (edges / vertices whose normals span less
+ * than asin(x) get no wedge / cone of their own, their faces' prisms are widened instead; default 1/32, 0 = off), SDF_FILLINT_PLAIN=1 (interior fill without the blank map);
  * see DESIGN.md.
  */
 #ifndef PAPER_1903_00353_SDF_H
@@ -68,8 +69,10 @@ typedef struct sdf_allocator {
 typedef struct sdf_stats_t {
     int64_t F, V, E;                      /* triangles, welded vertices, undirected edges      */
     int64_t edges_convex, edges_concave, edges_flat;      /* PAPER.md:352 discriminant; knife   */
-                                          /* edges (n1 = -n2) count as convex                   */
-    int64_t verts_pos_only, verts_neg_only, verts_both, verts_skipped; /* cone sides emitted   */
+                                          /* edges (n1 = -n2) count as convex; edges_flat also  */
+                                          /* counts the smooth edges absorbed by their faces    */
+    int64_t verts_pos_only, verts_neg_only, verts_both, verts_skipped; /* cone sides emitted;  */
+                                          /* skipped = smooth vertices absorbed by their faces  */
     int64_t verts_hemisphere;             /* "ruff" vertices: cos_cone <= 0 */
     int64_t weld_collisions;              /* reserved (always 0: the weld table probes, it has no runs) */
     /* last sdf_compute */
@@ -266,8 +269,12 @@ enum {
     SDF_TABLE_CORNER_VID   = 0,  /* int32 [3F]   corner -> welded vertex id                      */
     SDF_TABLE_HALFEDGE_ADJ = 1,  /* int32 [3F]   half-edge 3t+k (corner k -> k+1) -> its opposite */
     SDF_TABLE_FACE_NORMAL  = 2,  /* float [F][3] unit face normals                               */
-    SDF_TABLE_VERTEX_REC   = 3,  /* 32 B  [V]    {float pos[3], axis[3], cos_cone; int32 info}   */
-    SDF_TABLE_EDGE_REC     = 4,  /* 64 B  [E]    {float a[3], b[3], n1[3], n2[3]; int32 tri, cls, pad[2]} */
+    SDF_TABLE_VERTEX_REC   = 3,  /* 32 B  [V]    {float pos[3], axis[3], cos_cone; int32 info}; info bit0 / bit1: cone on
+                                    the + / - side of the axis, bit2: hemisphere (ruff), bit3: smooth vertex (no cone
+                                    of its own: its region is covered by the widened prisms of its faces)           */
+    SDF_TABLE_EDGE_REC     = 4,  /* 64 B  [edges_convex + edges_concave]  {float a[3], b[3], n1[3], n2[3]; int32 tri, cls,
+                                    pad[2]}: one record per edge that has a wedge, in no particular order; flat and
+                                    smooth edges (counted in edges_flat) have none                                   */
     SDF_TABLE_VERTEX_MINTRI= 5   /* int32 [V]    lowest incident triangle id                     */
 };
 int sdf_get_table(sdf_mesh *m, int which, void *dst, size_t bytes);

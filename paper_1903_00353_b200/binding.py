@@ -419,7 +419,7 @@ def sdf_get_table(mesh: Mesh, which: int) -> np.ndarray:
     shape_dtype = {
         TABLE_CORNER_VID: ((F, 3), np.int32), TABLE_HALFEDGE_ADJ: ((F, 3), np.int32),
         TABLE_FACE_NORMAL: ((F, 3), np.float32), TABLE_VERTEX_REC: ((V,), VERTEX_REC_DTYPE),
-        TABLE_EDGE_REC: ((E,), EDGE_REC_DTYPE), TABLE_VERTEX_MINTRI: ((V,), np.int32)}[which]
+        TABLE_EDGE_REC: ((s["edges_convex"] + s["edges_concave"],), EDGE_REC_DTYPE), TABLE_VERTEX_MINTRI: ((V,), np.int32)}[which]
     out = np.empty(shape_dtype[0], dtype=shape_dtype[1])
     st = lib().sdf_get_table(mesh.handle, which, C.c_void_p(out.ctypes.data), out.nbytes)
     if st != SDF_OK:

@@ -331,7 +331,7 @@ int sdf_get_table(sdf_mesh *m, int which, void *dst, size_t bytes) {
     case SDF_TABLE_HALFEDGE_ADJ: src = m->adj; need = sizeof(int) * 3 * (size_t)m->F; break;
     case SDF_TABLE_FACE_NORMAL: src = m->fn; need = sizeof(float) * 3 * (size_t)m->F; break;
     case SDF_TABLE_VERTEX_REC: src = m->vrec; need = sizeof(VertexRec) * (size_t)m->V; break;
-    case SDF_TABLE_EDGE_REC: src = m->erec; need = sizeof(EdgeRec) * (size_t)m->E; break;
+    case SDF_TABLE_EDGE_REC: src = m->erec; need = sizeof(EdgeRec) * (size_t)m->Elive; break;
     case SDF_TABLE_VERTEX_MINTRI: src = m->vmint; need = sizeof(int) * (size_t)m->V; break;
     default: return SDF_EINVAL;
     }

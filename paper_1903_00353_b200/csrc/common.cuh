@@ -36,8 +36,8 @@ enum { ERRB_NONFINITE = 1, ERRB_NOTCLOSED = 2, ERRB_ORIENT = 4, ERRB_DEGENERATE 
 
 // device counters (sdf_mesh::d_ctr), 64-bit each
 enum {
-    CTR_V = 0, CTR_RESERVED1, CTR_E_CONVEX, CTR_E_CONCAVE, CTR_E_FLAT,
-    CTR_V_POS, CTR_V_NEG, CTR_V_BOTH, CTR_V_SKIP, CTR_V_HEMI,
+    CTR_V = 0, CTR_ELIVE, CTR_E_CONVEX, CTR_E_CONCAVE, CTR_E_FLAT,      // ELIVE: edge records written (wedges that exist)
+    CTR_V_POS, CTR_V_NEG, CTR_V_BOTH, CTR_V_SKIP, CTR_V_HEMI, CTR_NCONE,   // NCONE: entries of the cone list
     CTR_POLY, CTR_ITEMS, CTR_BRICKS, CTR_TESTED, CTR_ACCEPTED, CTR_BAND, CTR_RECHECK,
     CTR_BIG, CTR_CDP_FALLBACK,   // big-polyhedron list length (fetch cursors: CTR_BIGCUR); refused child launches (cdp.cu)
     CTR_COUNT = 24,
@@ -67,9 +67,24 @@ static_assert(sizeof(EdgeRec) == 64, "EdgeRec must be 64 B");
 struct __align__(16) VertexRec {
     float pos[3], axis[3];
     float cos_cone;
-    int info;    // bit0: emit +axis side, bit1: emit -axis side, bit2: hemisphere (ruff)
+    int info;    // bit0: emit +axis side, bit1: emit -axis side, bit2: hemisphere (ruff),
+                 // bit3: smooth vertex, no cone of its own: absorbed by the margins of its faces
 };
 static_assert(sizeof(VertexRec) == 32, "VertexRec must be 32 B");
+
+// Smooth features: an edge whose two face normals, or a vertex whose cone of normals,
+// spans less than asin(SMOOTH_SIN) gets no polyhedron of its own.  Its characteristic region (the wedge of PAPER.md:352,
+// the cone of eq.9) lies within reach * sin(angle) of the side planes of every incident face's prism -- a
+// point p + r d with p on the face and d at angle a from the face normal projects r sin(a) away from p -- so each
+// incident face widens its prism sideways by that much and evaluates the clamped point-triangle distance there, which is
+// the distance to the edge / vertex.  (At C4 the dihedral angles are ~3e-3: 5.9 M wedges and 2-4 M cones, 99 % of them
+// without a single cell centre inside, become a 0.6 % wider face prism.)
+#define SMOOTH_SIN_DEFAULT 0.03125f
+// sine of twice the half angle of a vertex cone from its (already widened) stored cosine, rounded up
+__device__ __forceinline__ float cone_sin2(float c) {
+    if (!(c > 0.9f)) return INFINITY;
+    return 2.0f * c * sqrtf(fmaxf(0.0f, 1.0f - c * c)) * 1.00001f + 1e-7f;
+}
 
 // Band- and grid-dependent bounding volume of one polyhedron in cell indices, clipped to the grid
 // (PAPER.md:348, 364, 370), and the number of grid rows (j,k) it covers.  Lives in registers only.
@@ -128,7 +143,11 @@ struct sdf_mesh {
     int *adj;                // [3F]
     int *vmint;              // [V]
     VertexRec *vrec;         // [V]
-    EdgeRec *erec;           // [E]
+    EdgeRec *erec;           // [E] capacity; Elive records written: the wedges that exist (not flat, not absorbed)
+    float *fsm;              // [F] face margin factor: max sine of the normal-cone angle over the smooth edges /
+                             //     vertices the face absorbs; its prism is widened sideways by reach * fsm
+    u32 *cone_list;          // [2V] capacity; NC entries (vertex id << 1 | side): the vertex cones that exist
+    int64_t Elive, NC;
     u64 *d_ctr;              // [CTR_COUNT]
     int *d_flags;            // [4]
     // persistent per-compute workspace (grown on demand)

@@ -132,7 +132,8 @@ __device__ __forceinline__ void build_row_record(const MeshView &mv, const GridP
         rec[6] = m0.x; rec[7] = m0.y; rec[8] = m0.z; rec[9] = m1.x; rec[10] = m1.y; rec[11] = m1.z;
         rec[12] = m2.x; rec[13] = m2.y; rec[14] = m2.z;
         rec[15] = dot(m1, e0); rec[16] = dot(m2, ec);
-        rec[17] = eps * sqrtf(dot(e0, e0)); rec[18] = eps * sqrtf(dot(e1, e1)); rec[19] = eps * sqrtf(dot(ec, ec));
+        const float em = eps + g.rb * mv.fsm[p];       // eps + the margin for absorbed smooth features
+        rec[17] = em * sqrtf(dot(e0, e0)); rec[18] = em * sqrtf(dot(e1, e1)); rec[19] = em * sqrtf(dot(ec, ec));
         ri[RR_ID] = mv.perm[p]; ri[RR_TYPE] = 0; ri[RR_TIDX] = (int)p;
     } else if (p < (int64_t)mv.F + mv.E) {
         // edge wedge: beyond both faces' side planes, between the end caps
@@ -153,7 +154,7 @@ __device__ __forceinline__ void build_row_record(const MeshView &mv, const GridP
         }
     } else {
         // vertex cone / hemisphere (eq.10, 362-364) inside the ball of radius reach
-        const int64_t q = p - mv.F - mv.E;
+        const u32 q = mv.cone_list[p - mv.F - mv.E];
         const VertexRec &r = mv.vrec[q >> 1];
         const float sg = (q & 1) ? -1.0f : 1.0f;
         rec[0] = r.pos[0]; rec[1] = r.pos[1]; rec[2] = r.pos[2];
@@ -705,10 +706,11 @@ int maybe_prefill(sdf_mesh *m, int point, cudaStream_t st) {
 
 static MeshView make_view(const sdf_mesh *m) {
     MeshView mv;
-    mv.soup = m->soup; mv.fn = m->fn; mv.erec = m->erec; mv.vrec = m->vrec; mv.vmint = m->vmint;
+    mv.soup = m->soup; mv.fn = m->fn; mv.fsm = m->fsm; mv.erec = m->erec; mv.vrec = m->vrec; mv.vmint = m->vmint;
+    mv.cone_list = m->cone_list;
     mv.cvid = m->cvid; mv.adj = m->adj; mv.perm = m->perm; mv.inv_perm = m->inv_perm;
-    mv.F = (int)m->F; mv.E = (int)m->E; mv.V = (int)m->V;
-    mv.P = m->F + m->E + 2 * m->V;
+    mv.F = (int)m->F; mv.E = (int)m->Elive; mv.V = (int)m->V; mv.NC = (int)m->NC;
+    mv.P = m->F + m->Elive + m->NC;
     return mv;
 }
 
@@ -772,7 +774,7 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
     {
         // a mesh with few polyhedra cannot fill the GPU with one lane per polyhedron: hand more
         // of them to the block-per-polyhedron kernel
-        const int64_t P0 = m->F + m->E + 2 * m->V;
+        const int64_t P0 = m->F + m->Elive + m->NC;
         g.big_rows = P0 < 4096 ? 8 : (P0 < 65536 ? 64 : (int)BIG_ROWS);
         g.big_ni = P0 < 4096 ? 4 : (P0 < 65536 ? 16 : BIG_NI);
     }
@@ -967,11 +969,7 @@ __global__ void __launch_bounds__(256) closest_points_sparse_kernel(MeshView mv,
 }
 
 int run_closest_points(sdf_mesh *m, const GridParams &g, const int *tri, float *cp, cudaStream_t st) {
-    MeshView mv;
-    mv.soup = m->soup; mv.fn = m->fn; mv.erec = m->erec; mv.vrec = m->vrec; mv.vmint = m->vmint;
-    mv.cvid = m->cvid; mv.adj = m->adj; mv.perm = m->perm; mv.inv_perm = m->inv_perm;
-    mv.F = (int)m->F; mv.E = (int)m->E; mv.V = (int)m->V;
-    mv.P = m->F + m->E + 2 * m->V;
+    const MeshView mv = make_view(m);
     const int64_t n = (int64_t)g.nx * g.ny * g.nz;
     const bool vec = (((uintptr_t)tri & 15) == 0) && (((uintptr_t)cp & 15) == 0);
     if (vec && n % 8 == 0 && n >= (1 << 20) && !g.plain_cpt) {

@@ -83,14 +83,17 @@ __device__ __forceinline__ T tri_closest(V3<T> r, V3<T> e0, V3<T> ec, V3<T> n, i
 //   [0,F) face slabs | [F,F+E) edge wedges | [F+E, F+E+2V) vertex cones (+axis, -axis)
 // ---------------------------------------------------------------------------------------
 struct MeshView {
-    const float *soup, *fn;
+    const float *soup, *fn, *fsm;
     const EdgeRec *erec;
     const VertexRec *vrec;
+    const u32 *cone_list;
     const int *vmint, *cvid, *adj;
     const int *perm, *inv_perm;     // internal triangle index <-> the caller's id
-    int F, E, V;
-    int64_t P;
+    int F, E, V;                    // E = edge records (live wedges), not 3F/2
+    int NC;                         // entries of cone_list
+    int64_t P;                      // F + E + NC
 };
+
 
 // Cell-index range of [mn, mx] along one axis, clipped to the grid.  fp32: the index estimate
 // (x - o) / h carries a rounding error below 32767 * 2^-22 < 8e-3 cells, covered by the slack
@@ -113,16 +116,17 @@ __device__ __forceinline__ bool poly_aabv(const MeshView &mv, const GridParams &
         // face slab: triangle swept by +-rb along its normal
         const float *T = mv.soup + 9 * p, *N = mv.fn + 3 * p;
         emit = !(g.disable & 1);
+        const float dl = rb * mv.fsm[p];            // sideways margin for the smooth edges / vertices it absorbs
 #pragma unroll
         for (int i = 0; i < 3; i++) {
             float lo = fminf(T[i], fminf(T[3 + i], T[6 + i])), hi = fmaxf(T[i], fmaxf(T[3 + i], T[6 + i]));
-            float ext = g.aabb_mode ? rb : rb * fabsf(N[i]);
+            float ext = g.aabb_mode ? rb : rb * fabsf(N[i]) + dl;
             mn[i] = lo - ext - eps; mx[i] = hi + ext + eps;
         }
     } else if (p < (int64_t)mv.F + mv.E) {
         // edge wedge: segment swept by the arc between n1 and n2, radius rb
         const EdgeRec &r = mv.erec[p - mv.F];
-        emit = (r.cls != 0) && !g.aabb_mode && !(g.disable & 2);
+        emit = !g.aabb_mode && !(g.disable & 2);          // every record is a wedge that exists
         if (emit && r.cls == 2) {
             // knife edge: the cylinder of radius rb about the segment
 #pragma unroll
@@ -155,10 +159,10 @@ __device__ __forceinline__ bool poly_aabv(const MeshView &mv, const GridParams &
     } else {
         // vertex cone about +-pseudonormal intersected with the ball of radius rb
         // (cone AABV intersected with the sphere AABV)
-        int64_t q = p - mv.F - mv.E;
+        const u32 q = mv.cone_list[p - mv.F - mv.E];
         const VertexRec &r = mv.vrec[q >> 1];
         int side = (int)(q & 1);
-        emit = ((r.info >> side) & 1) && !g.aabb_mode && !(side == 1 && r.cos_cone <= -1.0f) && !(g.disable & 4);
+        emit = !g.aabb_mode && !(g.disable & 4);          // every entry is a cone that exists
         if (emit) {
             float sg = side ? -1.0f : 1.0f;
             float c = r.cos_cone, sn = sqrtf(fmaxf(0.0f, 1.0f - c * c));
@@ -238,7 +242,8 @@ __device__ __forceinline__ void process_direct(const MeshView &mv, const GridPar
         const f3 a = ld3(T), e0 = ld3(T + 3) - a, ec = ld3(T + 6) - a, n = ld3(N);
         const f3 e1 = ec - e0;
         const f3 m0 = cross(n, e0), m1 = cross(n, e1), m2 = cross(ec, n);          // inward, |m_i| = |edge_i|
-        const float t0 = eps * sqrtf(dot(e0, e0)), t1 = eps * sqrtf(dot(e1, e1)), t2 = eps * sqrtf(dot(ec, ec));
+        const float em = eps + g.rb * mv.fsm[p];
+        const float t0 = em * sqrtf(dot(e0, e0)), t1 = em * sqrtf(dot(e1, e1)), t2 = em * sqrtf(dot(ec, ec));
         const int id = mv.perm[p];
         const f3 r0 = mk<float>(fmaf((float)i0, h, g.ox) - a.x, fmaf((float)j0, h, g.oy) - a.y, fmaf((float)k0, h, g.oz) - a.z);
         const float c0 = dot(m0, r0), c1 = dot(m1, r0) - dot(m1, e0), c2 = dot(m2, r0) - dot(m2, ec), cn = dot(n, r0);
@@ -308,7 +313,7 @@ __device__ __forceinline__ void process_direct(const MeshView &mv, const GridPar
             }
         }
     } else {
-        const int64_t q = p - mv.F - mv.E;
+        const u32 q = mv.cone_list[p - mv.F - mv.E];
         const VertexRec &vr = mv.vrec[q >> 1];
         const float sg = (q & 1) ? -1.0f : 1.0f;
         const f3 v = ld3(vr.pos), A = sg * ld3(vr.axis);

@@ -199,8 +199,7 @@ __device__ __forceinline__ bool tri_normal64(const float *__restrict__ T, double
 __global__ void __launch_bounds__(FB, TG_MINB) tri_geom_kernel(const float *__restrict__ soup, const u32 *__restrict__ wtab,
                                                       const u32 *__restrict__ slot, int F, int *__restrict__ cvid,
                                                       float *__restrict__ fn, u64 *__restrict__ vacc,
-                                                      unsigned char *__restrict__ fcnt, u32 *etab, u32 emask,
-                                                      int *__restrict__ flags) {
+                                                      u32 *etab, u32 emask, int *__restrict__ flags) {
     int t = blockIdx.x * FB + threadIdx.x;
     if (t >= F) return;
     const float *T = soup + 9 * (size_t)t;
@@ -217,7 +216,6 @@ __global__ void __launch_bounds__(FB, TG_MINB) tri_geom_kernel(const float *__re
         n[0] = n[1] = 0.0; n[2] = 1.0;
     }
     fn[3 * (size_t)t] = (float)n[0]; fn[3 * (size_t)t + 1] = (float)n[1]; fn[3 * (size_t)t + 2] = (float)n[2];
-    int nf = 0;
 #pragma unroll
     for (int k = 0; k < 3; k++) {
         int k1 = (k + 1) % 3, k2 = (k + 2) % 3;
@@ -237,23 +235,12 @@ __global__ void __launch_bounds__(FB, TG_MINB) tri_geom_kernel(const float *__re
         // check: a valid mesh has one forward half-edge per key, and a duplicate just leaves an
         // entry nobody claims, which the pair count exposes)
         if (v[k] < v[k1]) {
-            nf++;
             u32 h = edge_hash((u32)v[k], (u32)v[k1]) & emask;
             while (__ldcg(etab + h) != EMPTY32 || atomicCAS(etab + h, EMPTY32, (u32)(3 * t + k)) != EMPTY32)
                 h = (h + 1) & emask;
         }
     }
-    fcnt[t] = (unsigned char)nf;
 }
-
-struct FcntIn {
-    const unsigned char *c;
-    __device__ u64 operator()(int64_t i) const { return c[i]; }
-};
-struct EbaseOut {
-    u32 *ebase;
-    __device__ void operator()(int64_t i, u64 ex, u64) const { ebase[i] = (u32)ex; }
-};
 
 // ---------------------------------------------------------------------------------------
 // A2 edge table: every undirected edge {u < w} of a closed, consistently oriented surface is
@@ -310,70 +297,100 @@ __global__ void __launch_bounds__(FB) edge_pair_kernel(const int *__restrict__ c
     }
 }
 
-// one thread per triangle; the forward half-edge of every claimed pair writes the edge record
-// (A4 edge class + band-independent wedge geometry) at its rank among the forward half-edges
+// one thread per triangle; the forward half-edge of every claimed pair classifies its edge (A4) and, if the edge
+// gets a wedge, writes the band-independent wedge geometry.  Records are compact: a block counts its wedges, takes
+// a range of the table with one atomicAdd and its threads write at their ranks (the order of the records is not
+// defined and nothing depends on it).  Smooth edges are absorbed by their two faces (evaluate.cuh, SMOOTH_SIN).
+struct EdgeGeom { const float *A, *B, *N1, *N2; int t1; };
+__device__ __forceinline__ EdgeGeom edge_geom(const float *__restrict__ soup, const float *__restrict__ fn, int t0, int k0,
+                                              int he1) {
+    EdgeGeom g;
+    g.t1 = he1 / 3;
+    g.A = soup + 9 * (size_t)t0 + 3 * k0; g.B = soup + 9 * (size_t)t0 + 3 * (k0 == 2 ? 0 : k0 + 1);
+    g.N1 = fn + 3 * (size_t)t0; g.N2 = fn + 3 * (size_t)g.t1;
+    // canonical direction a -> b = ascending exact position bits, so the record (and the fp32 rounding of every
+    // distance evaluated from it) does not depend on the order of the triangles in the soup; n1 stays the normal
+    // of the triangle that traverses a -> b
+    const u32 *pa = (const u32 *)g.A, *pb = (const u32 *)g.B;
+    if (pa[0] != pb[0] ? pa[0] > pb[0] : (pa[1] != pb[1] ? pa[1] > pb[1] : pa[2] > pb[2])) {
+        const float *tp = g.A; g.A = g.B; g.B = tp;
+        tp = g.N1; g.N1 = g.N2; g.N2 = tp;
+    }
+    return g;
+}
+
 __global__ void __launch_bounds__(FB) edge_record_kernel(const int *__restrict__ cvid, int F,
-                                                         const int *__restrict__ adj, const u32 *__restrict__ ebase,
+                                                         const int *__restrict__ adj,
                                                          const float *__restrict__ soup, const float *__restrict__ fn,
-                                                         const int *__restrict__ perm,
-                                                         EdgeRec *__restrict__ erec, int E, u64 *__restrict__ ctr) {
-    __shared__ u32 s_cnt[3];
+                                                         const int *__restrict__ perm, float smooth_sin,
+                                                         EdgeRec *__restrict__ erec, int E, int *__restrict__ fsm_bits,
+                                                         u64 *__restrict__ ctr) {
+    __shared__ u32 s_cnt[3], s_live, s_base;
     if (threadIdx.x < 3) s_cnt[threadIdx.x] = 0;
+    if (threadIdx.x == 3) s_live = 0;
     __syncthreads();
     const int t0 = blockIdx.x * FB + threadIdx.x;
+    int cls[3] = {0, 0, 0}, rank[3] = {-1, -1, -1}, he1[3] = {-1, -1, -1};
     if (t0 < F) {
         const int c[3] = {cvid[3 * (size_t)t0], cvid[3 * (size_t)t0 + 1], cvid[3 * (size_t)t0 + 2]};
-        const int he1[3] = {adj[3 * (size_t)t0], adj[3 * (size_t)t0 + 1], adj[3 * (size_t)t0 + 2]};
-        int e = (int)ebase[t0];
-        int x0 = -1;
 #pragma unroll
         for (int k0 = 0; k0 < 3; k0++) {
             const int u = c[k0], w = c[k0 == 2 ? 0 : k0 + 1];
-            if (!(u < w)) continue;
-            const int erank = e++;                       // rank among the forward half-edges in soup order
-            if (he1[k0] < 0) continue;
-            const int t1 = he1[k0] / 3;
-            const float *A = soup + 9 * (size_t)t0 + 3 * k0, *B = soup + 9 * (size_t)t0 + 3 * (k0 == 2 ? 0 : k0 + 1);
-            const float *N1 = fn + 3 * (size_t)t0, *N2 = fn + 3 * (size_t)t1;
-            // canonical direction a -> b = ascending exact position bits, so the record (and the
-            // fp32 rounding of every distance evaluated from it) does not depend on the order of
-            // the triangles in the soup; n1 stays the normal of the triangle that traverses a -> b
-            const u32 *pa = (const u32 *)A, *pb = (const u32 *)B;
-            if (pa[0] != pb[0] ? pa[0] > pb[0] : (pa[1] != pb[1] ? pa[1] > pb[1] : pa[2] > pb[2])) {
-                const float *tp = A; A = B; B = tp;
-                tp = N1; N1 = N2; N2 = tp;
-            }
-            EdgeRec r;
+            if (!(u < w)) continue;                      // forward half-edges only
+            he1[k0] = adj[3 * (size_t)t0 + k0];
+            if (he1[k0] < 0) continue;                   // unpaired
+            const EdgeGeom g = edge_geom(soup, fn, t0, k0, he1[k0]);
             double ud[3], n1[3], n2[3], x[3];
 #pragma unroll
-            for (int i = 0; i < 3; i++) {
-                r.a[i] = A[i]; r.b[i] = B[i]; r.n1[i] = N1[i]; r.n2[i] = N2[i];
-                ud[i] = (double)B[i] - (double)A[i]; n1[i] = N1[i]; n2[i] = N2[i];
-            }
-            double L = sqrt(ddot(ud, ud));
+            for (int i = 0; i < 3; i++) { ud[i] = (double)g.B[i] - (double)g.A[i]; n1[i] = g.N1[i]; n2[i] = g.N2[i]; }
+            const double L = sqrt(ddot(ud, ud));
             dcross(ud, n1, x);
-            double d = (L > 0.0) ? ddot(x, n2) / L : 0.0;       // PAPER.md:352 d = (ab x n1).n2, normalised
+            const double d = (L > 0.0) ? ddot(x, n2) / L : 0.0;       // PAPER.md:352 d = (ab x n1).n2, normalised
+            const double c12 = ddot(n1, n2);
             // flat: the wedge is thinner than 1e-6 * band and lies inside the eps-inflated
             // neighbours (reading #5)
-            int cls = d > 1e-6 ? 1 : (d < -1e-6 ? -1 : 0);
+            int cl = d > 1e-6 ? 1 : (d < -1e-6 ? -1 : 0);
             // sin(dihedral) also vanishes when the faces fold back onto each other (n1 = -n2: a
             // blade or a slit).  That edge is as far from flat as an edge gets, and which side its
             // wedge is on cannot be told from a vanishing discriminant: class 2, "knife", whose
             // extrusion is the whole cylinder about the edge
-            if (cls == 0 && ddot(n1, n2) <= 0.0) cls = 2;
-            if (x0 < 0) x0 = perm[t0];                   // the caller's triangle ids
-            const int x1 = perm[t1];
-            r.tri = x0 < x1 ? x0 : x1;
-            r.cls = cls;
-            r.pad[0] = r.pad[1] = 0;
-            // erec holds E = 3F/2 records: exactly the forward half-edges of a closed, oriented mesh.  A
-            // mis-oriented or open soup can have up to 2F of them; those ranks are dropped (the pair count
-            // below still exposes the mesh as invalid)
-            if (erank < E) erec[erank] = r;
-            atomicAdd(&s_cnt[cls > 0 ? 0 : (cls < 0 ? 1 : 2)], 1u);      // knife edges count as convex
+            if (cl == 0 && c12 <= 0.0) cl = 2;
+            // smooth: |sin| of the angle between the two normals below the threshold (and the angle acute).  No wedge;
+            // both faces widen their prisms by reach * sin instead
+            if (c12 > 0.0 && fabs(d) <= (double)smooth_sin) {
+                const int sb = __float_as_int(__double2float_ru(fabs(d) * 1.000001 + 1e-9));
+                if (fsm_bits[t0] < sb) atomicMax(&fsm_bits[t0], sb);
+                if (fsm_bits[g.t1] < sb) atomicMax(&fsm_bits[g.t1], sb);
+                cl = 0;
+            }
+            cls[k0] = cl;
+            atomicAdd(&s_cnt[cl > 0 ? 0 : (cl < 0 ? 1 : 2)], 1u);      // knife edges count as convex
+            if (cl != 0) rank[k0] = (int)atomicAdd(&s_live, 1u);
         }
     }
     __syncthreads();
+    if (threadIdx.x == 0 && s_live) s_base = (u32)atomicAdd(&ctr[CTR_ELIVE], (u64)s_live);
+    __syncthreads();
+    if (t0 < F) {
+        int x0 = -1;
+#pragma unroll
+        for (int k0 = 0; k0 < 3; k0++) {
+            if (rank[k0] < 0) continue;
+            const u32 slot = s_base + (u32)rank[k0];
+            // the table holds 3F/2 records: pairs never outnumber that (two distinct half-edges each)
+            if (slot >= (u32)E) continue;
+            const EdgeGeom g = edge_geom(soup, fn, t0, k0, he1[k0]);
+            EdgeRec r;
+#pragma unroll
+            for (int i = 0; i < 3; i++) { r.a[i] = g.A[i]; r.b[i] = g.B[i]; r.n1[i] = g.N1[i]; r.n2[i] = g.N2[i]; }
+            if (x0 < 0) x0 = perm[t0];                   // the caller's triangle ids
+            const int x1 = perm[g.t1];
+            r.tri = x0 < x1 ? x0 : x1;
+            r.cls = cls[k0];
+            r.pad[0] = r.pad[1] = 0;
+            erec[slot] = r;
+        }
+    }
     if (threadIdx.x < 3 && s_cnt[threadIdx.x]) atomicAdd(&ctr[CTR_E_CONVEX + threadIdx.x], (u64)s_cnt[threadIdx.x]);
 }
 
@@ -459,12 +476,15 @@ __global__ void __launch_bounds__(FB) vertex_record_kernel(const float *__restri
                                                            const double *__restrict__ vn64,
                                                            const long long *__restrict__ vcosq,
                                                            const int *__restrict__ vside, int V,
-                                                           const long long *__restrict__ vcospos,
-                                                           VertexRec *__restrict__ vrec, u64 *__restrict__ ctr) {
-    __shared__ u32 s_cnt[5];
+                                                           const long long *__restrict__ vcospos, float smooth_sin,
+                                                           VertexRec *__restrict__ vrec, u32 *__restrict__ cone_list,
+                                                           u64 *__restrict__ ctr) {
+    __shared__ u32 s_cnt[5], s_live, s_base;
     if (threadIdx.x < 5) s_cnt[threadIdx.x] = 0;
+    if (threadIdx.x == 5) s_live = 0;
     __syncthreads();
     int v = blockIdx.x * FB + threadIdx.x;
+    int sides = 0, rank = 0;
     if (v < V) {
         const float *P = soup + 3 * (size_t)vcorner[v];
         const double *N = vn64 + 3 * (size_t)v;
@@ -496,7 +516,10 @@ __global__ void __launch_bounds__(FB) vertex_record_kernel(const float *__restri
         if (hemi) info |= 4;
         // a cone thinner than 1e-6 rad is covered by the eps-inflated neighbours
         bool skip = !hemi && (1.0 - c) < 5e-13;
-        if (skip) info = 0;
+        // smooth: the whole cone of normals within asin(smooth_sin) / 2 of the axis.  No cone; the incident faces
+        // widen their prisms by reach * sin(2 theta) instead (face_margin_kernel reads it back from cos_cone)
+        if (!hemi && !noaxis && cone_sin2(cf) <= smooth_sin) skip = true;
+        if (skip) info = 8;
         VertexRec r;
 #pragma unroll
         for (int i = 0; i < 3; i++) { r.pos[i] = P[i]; r.axis[i] = (float)N[i]; }
@@ -506,9 +529,34 @@ __global__ void __launch_bounds__(FB) vertex_record_kernel(const float *__restri
         int slot = skip ? 3 : ((info & 3) == 1 ? 0 : ((info & 3) == 2 ? 1 : 2));
         atomicAdd(&s_cnt[slot], 1u);
         if (hemi && !skip) atomicAdd(&s_cnt[4], 1u);
+        // the cones that exist: one entry per emitted side (a vertex without axis is one whole ball: + side only)
+        sides = skip ? 0 : (cf <= -1.0f ? 1 : (info & 3));
+        if (sides) rank = (int)atomicAdd(&s_live, (u32)__popc(sides));
     }
     __syncthreads();
+    if (threadIdx.x == 0 && s_live) s_base = (u32)atomicAdd(&ctr[CTR_NCONE], (u64)s_live);
+    __syncthreads();
+    if (sides) {
+        u32 o = s_base + (u32)rank;
+        if (sides & 1) cone_list[o++] = ((u32)v << 1);
+        if (sides & 2) cone_list[o] = ((u32)v << 1) | 1u;
+    }
     if (threadIdx.x < 5 && s_cnt[threadIdx.x]) atomicAdd(&ctr[CTR_V_POS + threadIdx.x], (u64)s_cnt[threadIdx.x]);
+}
+
+// one thread per triangle: its prism is widened for the smooth vertices it touches (the smooth edges already raised
+// fsm in edge_record_kernel; this runs after both streams have joined)
+__global__ void __launch_bounds__(FB) face_margin_kernel(const int *__restrict__ cvid, int F,
+                                                         const VertexRec *__restrict__ vrec, float *__restrict__ fsm) {
+    int t = blockIdx.x * FB + threadIdx.x;
+    if (t >= F) return;
+    float s = fsm[t];
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const VertexRec &r = vrec[cvid[3 * (size_t)t + k]];
+        if (r.info & 8) s = fmaxf(s, cone_sin2(r.cos_cone));
+    }
+    fsm[t] = s;
 }
 
 // ---------------------------------------------------------------------------------------
@@ -589,6 +637,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
         m->cvid = c.take<int>(3 * (size_t)F);
         m->adj = c.take<int>(3 * (size_t)F);
         m->erec = c.take<EdgeRec>((size_t)(m->E > 0 ? m->E : 1));
+        m->fsm = c.take<float>((size_t)F);
         m->perm = c.take<int>((size_t)F);
         m->inv_perm = c.take<int>((size_t)F);
         m->d_ctr = c.take<u64>(CTR_TOTAL);
@@ -609,9 +658,9 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     const bool bin = !(nb && nb[0] == '1') && F >= 131072;     // smaller meshes live in L2 anyway
     u32 *bkeys = nullptr, *bkeys2 = nullptr, *bvals2 = nullptr, *bhist = nullptr;
     int *bbox = nullptr;
-    u32 *wtab = nullptr, *slot = nullptr, *etab = nullptr, *ebase = nullptr;
+    u32 *wtab = nullptr, *slot = nullptr, *etab = nullptr;
     u64 *scan_ws = nullptr;
-    unsigned char *head = nullptr, *fcnt = nullptr;
+    unsigned char *head = nullptr;
     int *vcorner = nullptr;
     void *tslab = nullptr;
     for (int pass = 0; pass < 2; pass++) {
@@ -619,10 +668,8 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
         wtab = c.take<u32>((size_t)capw);           // wtab and etab adjacent: one memset
         etab = c.take<u32>((size_t)cape);
         slot = c.take<u32>((size_t)nc);
-        ebase = c.take<u32>((size_t)F);
         scan_ws = c.take<u64>(scan_ws_elems((int64_t)nc));
         head = c.take<unsigned char>((size_t)nc);
-        fcnt = c.take<unsigned char>((size_t)F);
         vcorner = c.take<int>((size_t)nc);          // V <= 3F
         if (!on_device) staging = c.take<float>(9 * (size_t)F);
         if (bin) {
@@ -672,11 +719,15 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
         Carver c(m->slab_v);
         m->vrec = c.take<VertexRec>((size_t)V);
         m->vmint = c.take<int>((size_t)V);
+        m->cone_list = c.take<u32>(2 * (size_t)V);
         if (pass == 0) CKS(dev_alloc(al, &m->slab_v, c.off, st));
     }
     u64 *vacc = nullptr;
     double *vn64 = nullptr;
     long long *vcosq = nullptr, *vcospos = nullptr;
+    // smooth features get no polyhedron of their own (common.cuh, SMOOTH_SIN_DEFAULT); SDF_SMOOTH_SIN=0 switches that off
+    float smooth_sin = SMOOTH_SIN_DEFAULT;
+    if (const char *ss = getenv("SDF_SMOOTH_SIN")) { smooth_sin = (float)atof(ss); if (!(smooth_sin >= 0.0f && smooth_sin <= 0.25f)) smooth_sin = SMOOTH_SIN_DEFAULT; }
     const char *rc = getenv("SDF_RUFF");
     const bool ruff_cone = rc && !strcmp(rc, "cone");
     int *vside = nullptr;
@@ -695,7 +746,8 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     CKS(maybe_prefill(m, 2, st));
     stage_mark(m, SDF_T_EDGES, 0, st);
     CK(cudaMemsetAsync(vacc, 0, (size_t)((char *)(vside + V) - (char *)vacc), st));
-    KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wtab, slot, (int)F, m->cvid, m->fn, vacc, fcnt, etab, cape - 1, m->d_flags);
+    CK(cudaMemsetAsync(m->fsm, 0, sizeof(float) * (size_t)F, st));
+    KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wtab, slot, (int)F, m->cvid, m->fn, vacc, etab, cape - 1, m->d_flags);
     // sdf_transform: the per-compute workspace of A6a is taken in the order of `st` BEFORE the fork, so that the
     // vertex stream (which first touches it) is ordered after the allocation
     CKS(maybe_alloc_brick_ws(m, st));
@@ -720,10 +772,9 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
             drain.s = vs; drain.armed = true;
         }
     }
-    CKS(launch_scan(FcntIn{fcnt}, EbaseOut{ebase}, F, scan_ws, (u64 *)nullptr, st));
     CKS(maybe_prefill(m, 3, st));
     KL; edge_pair_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, etab, cape - 1, m->adj);
-    KL; edge_record_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, m->adj, ebase, m->soup, m->fn, m->perm, m->erec, (int)m->E, m->d_ctr);
+    KL; edge_record_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, m->adj, m->soup, m->fn, m->perm, smooth_sin, m->erec, (int)m->E, (int *)m->fsm, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_EDGES, 1, st);
 
@@ -735,7 +786,7 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     CK(cudaMemsetAsync(m->vmint, 0x7F, sizeof(int) * (size_t)V, vs));
     KL; vertex_normal_kernel<<<blocks_for(V), FB, 0, vs>>>(vacc, V, vn64);
     KL; vertex_cone_kernel<<<blocks_for(F), FB, 0, vs>>>(m->soup, m->cvid, (int)F, vn64, vcosq, vside, m->perm, m->vmint, vcospos);
-    KL; vertex_record_kernel<<<blocks_for(V), FB, 0, vs>>>(m->soup, vcorner, vn64, vcosq, vside, V, vcospos, m->vrec, m->d_ctr);
+    KL; vertex_record_kernel<<<blocks_for(V), FB, 0, vs>>>(m->soup, vcorner, vn64, vcosq, vside, V, vcospos, smooth_sin, m->vrec, m->cone_list, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_VERTICES, 1, vs);
     CKS(maybe_prepare_bricks(m, st, vs));
@@ -744,11 +795,15 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
         CK(cudaStreamWaitEvent(st, m->ev_join, 0));
         drain.armed = false;           // joined: `st` now carries the dependency
     }
+    KL; face_margin_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, m->vrec, m->fsm);
+    CK(cudaGetLastError());
     // second host crossing: validation flags + class counters
     CK(cudaMemcpyAsync(hflags, m->d_flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(m->h_ctr, m->d_ctr, sizeof(u64) * CTR_COUNT, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     int status = status_from_flags(hflags[0]);
+    m->Elive = (int64_t)m->h_ctr[CTR_ELIVE];
+    m->NC = (int64_t)m->h_ctr[CTR_NCONE];
     // closed + consistently oriented <=> every half-edge was claimed into a pair
     const u64 pairs = m->h_ctr[CTR_E_CONVEX] + m->h_ctr[CTR_E_CONCAVE] + m->h_ctr[CTR_E_FLAT];
     if (status == SDF_OK && 2 * pairs != (u64)nc) {

@@ -59,14 +59,16 @@ def test_feature_tables(name, scale):
     # edge records: one per undirected edge, end points = the edge's two vertices, n1 / n2 = the
     # normals of its two triangles, tri = the lower triangle id
     er = B.sdf_get_table(m, B.TABLE_EDGE_REC)
-    assert er.shape[0] == 3 * F // 2
+    # one record per edge that has a wedge (flat and smooth edges have none), in no particular order
+    assert er.shape[0] == s["edges_convex"] + s["edges_concave"] and s["edges_flat"] == 3 * F // 2 - er.shape[0]
+    assert er.shape[0] > 0 and np.all(er["cls"] != 0)
     pos_to_vid = {}
     flat = (soup.reshape(-1, 3) + np.float32(0.0))
     for c in (np.unique(src, return_index=True)[1]):
         pos_to_vid[flat[c].tobytes()] = src[c]
     fwd = np.nonzero(src < dst)[0]
     edge_of = {(int(src[h]), int(dst[h])): h for h in fwd}
-    assert len(edge_of) == er.shape[0]
+    assert len(edge_of) == 3 * F // 2
     seen = set()
     step = max(1, er.shape[0] // 4000)
     for e in range(0, er.shape[0], step):
@@ -82,7 +84,7 @@ def test_feature_tables(name, scale):
         ta = t0 if (a, b) == (int(src[h0]), int(dst[h0])) else t1
         tb = t1 if ta == t0 else t0
         assert np.array_equal(er["n1"][e], fn[ta]) and np.array_equal(er["n2"][e], fn[tb])
-    assert s["edges_convex"] + s["edges_concave"] + s["edges_flat"] == er.shape[0]
+    assert s["edges_convex"] + s["edges_concave"] + s["edges_flat"] == 3 * F // 2
     assert np.count_nonzero(er["cls"] > 0) == s["edges_convex"]
     assert np.count_nonzero(er["cls"] < 0) == s["edges_concave"]
 
