@@ -102,20 +102,71 @@ __global__ void __launch_bounds__(FB) identity_perm_kernel(int F, u32 *__restric
     if (t < F) perm[t] = (u32)t;
 }
 
+// ---- tile builder: ONE-pass counting sort by a fine Morton bin (up to 7 bits per axis).  Only a 4-byte index moves
+// (the triangles themselves are gathered by tile_weld_kernel), so a bin's slot is handed out by an atomic ticket and
+// the bin offsets come from one scan over the bins.  Inside a bin the order is the order of arrival -- it differs from
+// run to run and nothing that reaches the output depends on it.
+__device__ __forceinline__ u32 spread3_10(u32 v) {         // 10 bits -> every third bit
+    v &= 0x3FFu;
+    v = (v | (v << 16)) & 0x030000FFu;
+    v = (v | (v << 8)) & 0x0300F00Fu;
+    v = (v | (v << 4)) & 0x030C30C3u;
+    v = (v | (v << 2)) & 0x09249249u;
+    return v;
+}
+__global__ void __launch_bounds__(FB) fine_bin_kernel(const float *__restrict__ in, int F, const int *__restrict__ bbox,
+                                                      int bits, u32 *cnt, u32 *__restrict__ key, u32 *__restrict__ ticket) {
+    int t = blockIdx.x * FB + threadIdx.x;
+    if (t >= F) return;
+    const float *p = in + 9 * (size_t)t;
+    const float nb = (float)(1 << bits);
+    u32 q[3];
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+        const float lo = ord2f(bbox[i]), hi = ord2f(bbox[3 + i]);
+        const float w = hi - lo;
+        float f = (w > 0.0f && isfinite(w)) ? (p[i] - lo) / w * nb : 0.0f;
+        f = fminf(fmaxf(f, 0.0f), nb - 1.0f);                 // NaN -> 0; outliers -> end bins
+        q[i] = (u32)f;
+    }
+    const u32 k = spread3_10(q[0]) | (spread3_10(q[1]) << 1) | (spread3_10(q[2]) << 2);
+    key[t] = k;
+    ticket[t] = atomicAdd(&cnt[k], 1u);
+}
+struct BinIn {
+    const u32 *c;
+    __device__ u64 operator()(int64_t i) const { return c[i]; }
+};
+struct BinOut {
+    u32 *c;
+    __device__ void operator()(int64_t i, u64 ex, u64) const { c[i] = (u32)ex; }
+};
+__global__ void __launch_bounds__(FB) fine_scatter_kernel(int F, const u32 *__restrict__ base, const u32 *__restrict__ key,
+                                                          const u32 *__restrict__ ticket, u32 *__restrict__ perm) {
+    int t = blockIdx.x * FB + threadIdx.x;
+    if (t < F) perm[base[key[t]] + ticket[t]] = (u32)t;
+}
+
 __device__ __forceinline__ u32 canon_bits(float x) { return __float_as_uint(x + 0.0f); }   // -0 + +0 = +0
 
 // One thread per corner of the internal order: gather the corner from the caller's soup
 // (reject non-finite input, canonicalise -0 -> +0, write the internal copy), then find-or-insert
 // its vertex in the weld table (linear probing).  A slot holds a corner index of its vertex;
 // identity is checked on the exact bits of that corner in the immutable input (its sector was
-// just read by the thread that owns it, so the check hits L2), and the slot converges to the
-// LOWEST corner index of the vertex (atomicMin): the representative does not depend on the
-// insertion order.  slot[c] = table position of c.
+// just read by the thread that owns it, so the check hits L2).  The corner that inserts a vertex
+// takes its id from a counter (one atomicAdd per warp), resets the vertex' accumulators and leaves
+// the id in wvid[slot]; slot[c] = table position of c, resolved to ids by tri_geom_kernel.  (The ids
+// depend on the order in which warps run; nothing that reaches the output does.)
 __global__ void __launch_bounds__(FB) ingest_weld_kernel(const float *__restrict__ in, const int *__restrict__ perm,
                                                          int ncorner, float *__restrict__ soup,
                                                          int *__restrict__ inv_perm, u32 *wtab, u32 mask,
-                                                         u32 *__restrict__ slot, int *__restrict__ flags) {
+                                                         u32 *__restrict__ slot, u32 *__restrict__ wvid,
+                                                         int *__restrict__ vcorner, u64 *__restrict__ vacc,
+                                                         long long *__restrict__ vcosq, long long *__restrict__ vcospos,
+                                                         int *__restrict__ vside, int *__restrict__ vmint, int vcap,
+                                                         u64 *ctr, int *__restrict__ flags) {
     int c = blockIdx.x * FB + threadIdx.x;
+    const unsigned act = __ballot_sync(0xffffffffu, c < ncorner);
     if (c >= ncorner) return;
     const int i = c / 3, k = c - 3 * i;
     const int t = perm[i];
@@ -127,50 +178,48 @@ __global__ void __launch_bounds__(FB) ingest_weld_kernel(const float *__restrict
     if (k == 0) inv_perm[t] = i;
     const u32 bx = __float_as_uint(x), by = __float_as_uint(y), bz = __float_as_uint(z);
     u32 h = mix32(bx, by, bz) & mask;
+    bool inserted = false;
     for (;;) {
         u32 cur = __ldcg(wtab + h);
         if (cur == EMPTY32) {
             cur = atomicCAS(wtab + h, EMPTY32, (u32)c);
-            if (cur == EMPTY32) break;
+            if (cur == EMPTY32) { inserted = true; break; }
         }
         const int ci = (int)cur / 3, ck = (int)cur - 3 * ci;
         const float *q = in + 9 * (size_t)perm[ci] + 3 * ck;
-        if (canon_bits(q[0]) == bx && canon_bits(q[1]) == by && canon_bits(q[2]) == bz) {
-            if ((u32)c < cur) atomicMin(wtab + h, (u32)c);     // the minimum only ever decreases
-            break;
-        }
+        if (canon_bits(q[0]) == bx && canon_bits(q[1]) == by && canon_bits(q[2]) == bz) break;
         h = (h + 1) & mask;
     }
     slot[c] = h;
+    const unsigned ins = __ballot_sync(act, inserted);
+    if (inserted) {
+        const int lane = threadIdx.x & 31, leader = __ffs(ins) - 1;
+        u32 base = 0;
+        if (lane == leader) base = (u32)atomicAdd(&ctr[CTR_V], (u64)__popc(ins));
+        base = __shfl_sync(ins, base, leader);
+        const u32 vid = base + (u32)__popc(ins & ((1u << lane) - 1u));
+        if (vid >= (u32)vcap) {
+            // more vertices than a closed surface of F triangles can have (V <= 3F/2): the tables are not that large
+            atomicOr(flags, ERRB_NOTCLOSED);
+            wvid[h] = (u32)(vcap - 1);
+        } else {
+            wvid[h] = vid;
+            vcorner[vid] = c;
+            vacc[3 * (size_t)vid] = 0ull; vacc[3 * (size_t)vid + 1] = 0ull; vacc[3 * (size_t)vid + 2] = 0ull;
+            vcosq[vid] = 0x7F7F7F7F7F7F7F7Fll;
+            if (vcospos) vcospos[vid] = 0x7F7F7F7F7F7F7F7Fll;
+            vside[vid] = 0;
+            vmint[vid] = 0x7F7F7F7F;
+        }
+    }
 }
-
-// head[c] = 1 iff c is the lowest corner of its vertex; vertex ids are the ranks of the heads.
-// The flag is computed (and stored) by the reduce pass of the scan and read back by its down
-// pass, whose output functor overwrites the table slots of the heads.
-struct HeadCompute {
-    const u32 *wtab; const u32 *slot; unsigned char *head;
-    __device__ u64 operator()(int64_t i) const {
-        const unsigned char v = (wtab[slot[i]] == (u32)i) ? 1 : 0;
-        head[i] = v;
-        return v;
-    }
-};
-struct HeadIn {
-    const unsigned char *head;
-    __device__ u64 operator()(int64_t i) const { return head[i]; }
-};
-struct HeadOut {      // the head replaces the corner index in its slot by the vertex id
-    u32 *wtab; const u32 *slot; int *vcorner;
-    __device__ void operator()(int64_t i, u64 ex, u64 v) const {
-        if (v) { wtab[slot[i]] = (u32)ex; vcorner[ex] = (int)i; }
-    }
-};
 
 // ---------------------------------------------------------------------------------------
 // A3 triangle geometry: corner -> vertex ids, unit normal, corner angles, fixed-point
 // pseudonormal accumulation, number of forward half-edges (for the edge ids of A2)
 // ---------------------------------------------------------------------------------------
 #define FIXSCALE 1099511627776.0   /* 2^40 */
+#define COSSCALE 4503599627370496.0   /* 2^52 */
 
 __device__ __forceinline__ u32 edge_hash(u32 u, u32 w) { return mix32(u, w, 0x51ED270Bu); }
 __device__ __forceinline__ int he_next(int he) { int k = he % 3; return he - k + (k == 2 ? 0 : k + 1); }
@@ -196,7 +245,12 @@ __device__ __forceinline__ bool tri_normal64(const float *__restrict__ T, double
     return true;
 }
 
-__global__ void __launch_bounds__(FB, TG_MINB) tri_geom_kernel(const float *__restrict__ soup, const u32 *__restrict__ wtab,
+#include "tile_features.cuh"
+
+// ===================================================================================================
+// the global-table builder (default): every corner / half-edge through hash tables in global memory
+// ===================================================================================================
+__global__ void __launch_bounds__(FB, TG_MINB) tri_geom_kernel(const float *__restrict__ soup, const u32 *__restrict__ wvid,
                                                       const u32 *__restrict__ slot, int F, int *__restrict__ cvid,
                                                       float *__restrict__ fn, u64 *__restrict__ vacc,
                                                       u32 *etab, u32 emask, int *__restrict__ flags) {
@@ -206,7 +260,7 @@ __global__ void __launch_bounds__(FB, TG_MINB) tri_geom_kernel(const float *__re
     int v[3];
 #pragma unroll
     for (int k = 0; k < 3; k++) {
-        v[k] = (int)wtab[slot[3 * (size_t)t + k]];
+        v[k] = (int)wvid[slot[3 * (size_t)t + k]];
         cvid[3 * (size_t)t + k] = v[k];
     }
     double n[3], p[3][3];
@@ -301,24 +355,6 @@ __global__ void __launch_bounds__(FB) edge_pair_kernel(const int *__restrict__ c
 // gets a wedge, writes the band-independent wedge geometry.  Records are compact: a block counts its wedges, takes
 // a range of the table with one atomicAdd and its threads write at their ranks (the order of the records is not
 // defined and nothing depends on it).  Smooth edges are absorbed by their two faces (evaluate.cuh, SMOOTH_SIN).
-struct EdgeGeom { const float *A, *B, *N1, *N2; int t1; };
-__device__ __forceinline__ EdgeGeom edge_geom(const float *__restrict__ soup, const float *__restrict__ fn, int t0, int k0,
-                                              int he1) {
-    EdgeGeom g;
-    g.t1 = he1 / 3;
-    g.A = soup + 9 * (size_t)t0 + 3 * k0; g.B = soup + 9 * (size_t)t0 + 3 * (k0 == 2 ? 0 : k0 + 1);
-    g.N1 = fn + 3 * (size_t)t0; g.N2 = fn + 3 * (size_t)g.t1;
-    // canonical direction a -> b = ascending exact position bits, so the record (and the fp32 rounding of every
-    // distance evaluated from it) does not depend on the order of the triangles in the soup; n1 stays the normal
-    // of the triangle that traverses a -> b
-    const u32 *pa = (const u32 *)g.A, *pb = (const u32 *)g.B;
-    if (pa[0] != pb[0] ? pa[0] > pb[0] : (pa[1] != pb[1] ? pa[1] > pb[1] : pa[2] > pb[2])) {
-        const float *tp = g.A; g.A = g.B; g.B = tp;
-        tp = g.N1; g.N1 = g.N2; g.N2 = tp;
-    }
-    return g;
-}
-
 __global__ void __launch_bounds__(FB) edge_record_kernel(const int *__restrict__ cvid, int F,
                                                          const int *__restrict__ adj,
                                                          const float *__restrict__ soup, const float *__restrict__ fn,
@@ -339,29 +375,14 @@ __global__ void __launch_bounds__(FB) edge_record_kernel(const int *__restrict__
             if (!(u < w)) continue;                      // forward half-edges only
             he1[k0] = adj[3 * (size_t)t0 + k0];
             if (he1[k0] < 0) continue;                   // unpaired
-            const EdgeGeom g = edge_geom(soup, fn, t0, k0, he1[k0]);
-            double ud[3], n1[3], n2[3], x[3];
-#pragma unroll
-            for (int i = 0; i < 3; i++) { ud[i] = (double)g.B[i] - (double)g.A[i]; n1[i] = g.N1[i]; n2[i] = g.N2[i]; }
-            const double L = sqrt(ddot(ud, ud));
-            dcross(ud, n1, x);
-            const double d = (L > 0.0) ? ddot(x, n2) / L : 0.0;       // PAPER.md:352 d = (ab x n1).n2, normalised
-            const double c12 = ddot(n1, n2);
-            // flat: the wedge is thinner than 1e-6 * band and lies inside the eps-inflated
-            // neighbours (reading #5)
-            int cl = d > 1e-6 ? 1 : (d < -1e-6 ? -1 : 0);
-            // sin(dihedral) also vanishes when the faces fold back onto each other (n1 = -n2: a
-            // blade or a slit).  That edge is as far from flat as an edge gets, and which side its
-            // wedge is on cannot be told from a vanishing discriminant: class 2, "knife", whose
-            // extrusion is the whole cylinder about the edge
-            if (cl == 0 && c12 <= 0.0) cl = 2;
-            // smooth: |sin| of the angle between the two normals below the threshold (and the angle acute).  No wedge;
-            // both faces widen their prisms by reach * sin instead
-            if (c12 > 0.0 && fabs(d) <= (double)smooth_sin) {
-                const int sb = __float_as_int(__double2float_ru(fabs(d) * 1.000001 + 1e-9));
+            const int t1 = he1[k0] / 3;
+            const EdgeGeom g = edge_geom_of(soup + 9 * (size_t)t0 + 3 * k0, soup + 9 * (size_t)t0 + 3 * (k0 == 2 ? 0 : k0 + 1),
+                                            fn + 3 * (size_t)t0, fn + 3 * (size_t)t1);
+            int sb;
+            const int cl = edge_class_of(g, smooth_sin, &sb);
+            if (sb) {
                 if (fsm_bits[t0] < sb) atomicMax(&fsm_bits[t0], sb);
-                if (fsm_bits[g.t1] < sb) atomicMax(&fsm_bits[g.t1], sb);
-                cl = 0;
+                if (fsm_bits[t1] < sb) atomicMax(&fsm_bits[t1], sb);
             }
             cls[k0] = cl;
             atomicAdd(&s_cnt[cl > 0 ? 0 : (cl < 0 ? 1 : 2)], 1u);      // knife edges count as convex
@@ -372,23 +393,17 @@ __global__ void __launch_bounds__(FB) edge_record_kernel(const int *__restrict__
     if (threadIdx.x == 0 && s_live) s_base = (u32)atomicAdd(&ctr[CTR_ELIVE], (u64)s_live);
     __syncthreads();
     if (t0 < F) {
-        int x0 = -1;
 #pragma unroll
         for (int k0 = 0; k0 < 3; k0++) {
             if (rank[k0] < 0) continue;
             const u32 slot = s_base + (u32)rank[k0];
             // the table holds 3F/2 records: pairs never outnumber that (two distinct half-edges each)
             if (slot >= (u32)E) continue;
-            const EdgeGeom g = edge_geom(soup, fn, t0, k0, he1[k0]);
-            EdgeRec r;
-#pragma unroll
-            for (int i = 0; i < 3; i++) { r.a[i] = g.A[i]; r.b[i] = g.B[i]; r.n1[i] = g.N1[i]; r.n2[i] = g.N2[i]; }
-            if (x0 < 0) x0 = perm[t0];                   // the caller's triangle ids
-            const int x1 = perm[g.t1];
-            r.tri = x0 < x1 ? x0 : x1;
-            r.cls = cls[k0];
-            r.pad[0] = r.pad[1] = 0;
-            erec[slot] = r;
+            const int t1 = he1[k0] / 3;
+            const EdgeGeom g = edge_geom_of(soup + 9 * (size_t)t0 + 3 * k0, soup + 9 * (size_t)t0 + 3 * (k0 == 2 ? 0 : k0 + 1),
+                                            fn + 3 * (size_t)t0, fn + 3 * (size_t)t1);
+            const int x0 = perm[t0], x1 = perm[t1];
+            edge_record_write(erec + slot, g, x0 < x1 ? x0 : x1, cls[k0]);
         }
     }
     if (threadIdx.x < 3 && s_cnt[threadIdx.x]) atomicAdd(&ctr[CTR_E_CONVEX + threadIdx.x], (u64)s_cnt[threadIdx.x]);
@@ -422,9 +437,10 @@ __global__ void __launch_bounds__(FB) edge_validate_kernel(const u64 *__restrict
 // ---------------------------------------------------------------------------------------
 // A3/A4 vertices: pseudonormal, cone angle, class
 // ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(FB) vertex_normal_kernel(const u64 *__restrict__ vacc, int V,
+__global__ void __launch_bounds__(FB) vertex_normal_kernel(const u64 *__restrict__ vacc, int V, const u64 *__restrict__ vcount,
                                                            double *__restrict__ vn64) {
     int v = blockIdx.x * FB + threadIdx.x;
+    if (vcount) V = min(V, (int)*vcount);
     if (v >= V) return;
     double N[3];
 #pragma unroll
@@ -434,8 +450,6 @@ __global__ void __launch_bounds__(FB) vertex_normal_kernel(const u64 *__restrict
     else { N[0] = 0.0; N[1] = 0.0; N[2] = 0.0; }      // no usable axis: full sphere on both sides
     vn64[3 * (size_t)v] = N[0]; vn64[3 * (size_t)v + 1] = N[1]; vn64[3 * (size_t)v + 2] = N[2];
 }
-
-#define COSSCALE 4503599627370496.0   /* 2^52 */
 
 // one thread per triangle: for each corner, cos of the angle between the face normal and the
 // vertex axis (eq.9), which side of the pseudonormal plane the two
@@ -471,9 +485,12 @@ __global__ void __launch_bounds__(FB, TG_MINB) vertex_cone_kernel(const float *_
     }
 }
 
+// vn64 == nullptr: the axis is normalised here from the fixed-point sums vacc; vcount != nullptr: the number of
+// vertices is read on the device (the tile builder launches for the capacity of the tables)
 __global__ void __launch_bounds__(FB) vertex_record_kernel(const float *__restrict__ soup,
                                                            const int *__restrict__ vcorner,
-                                                           const double *__restrict__ vn64,
+                                                           const double *__restrict__ vn64, const u64 *__restrict__ vacc,
+                                                           const u64 *__restrict__ vcount,
                                                            const long long *__restrict__ vcosq,
                                                            const int *__restrict__ vside, int V,
                                                            const long long *__restrict__ vcospos, float smooth_sin,
@@ -485,9 +502,13 @@ __global__ void __launch_bounds__(FB) vertex_record_kernel(const float *__restri
     __syncthreads();
     int v = blockIdx.x * FB + threadIdx.x;
     int sides = 0, rank = 0;
+    if (vcount) V = min(V, (int)*vcount);
     if (v < V) {
         const float *P = soup + 3 * (size_t)vcorner[v];
-        const double *N = vn64 + 3 * (size_t)v;
+        double Nl[3];
+        const double *N = Nl;
+        if (vn64) N = vn64 + 3 * (size_t)v;
+        else vertex_axis64(vacc, (size_t)v, Nl);
         double c = (double)vcosq[v] * (1.0 / COSSCALE);
         int side = vside[v];
         bool noaxis = (N[0] == 0.0 && N[1] == 0.0 && N[2] == 0.0);
@@ -621,15 +642,103 @@ static int classify_edge_errors(sdf_mesh *m, int nc, TmpPool &tmp, cudaStream_t 
     return SDF_OK;
 }
 
-int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st) {
+// the library's second stream (vertex stage beside the edge stage): forked from st, drained on early returns
+static int fork_vertex_stream(sdf_mesh *m, cudaStream_t st, cudaStream_t *vs_out, StreamDrain &drain) {
+    *vs_out = st;
+    const char *cf = getenv("SDF_CREATE_FORK");
+    if (cf && cf[0] == '0') return SDF_OK;
+    static cudaStream_t g_vs = nullptr;
+    static int g_vs_dev = -1;
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    if (!g_vs || g_vs_dev != dev) {
+        CK(cudaStreamCreateWithFlags(&g_vs, cudaStreamNonBlocking));
+        g_vs_dev = dev;
+    }
+    if (!m->ev_fork) CK(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
+    if (!m->ev_join) CK(cudaEventCreateWithFlags(&m->ev_join, cudaEventDisableTiming));
+    CK(cudaEventRecord(m->ev_fork, st));
+    CK(cudaStreamWaitEvent(g_vs, m->ev_fork, 0));
+    drain.s = g_vs; drain.armed = true;
+    *vs_out = g_vs;
+    return SDF_OK;
+}
+
+// the one host crossing of sdf_create: validation flags, vertex / wedge / cone counts, class counters (and, inside
+// sdf_transform, the brick total of the hoisted A6a)
+static int finish_features(sdf_mesh *m, int nc, int vcap, TmpPool &tmp, cudaStream_t st) {
+    int hflags[4] = {0, 0, 0, 0};
+    CK(cudaMemcpyAsync(hflags, m->d_flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(m->h_ctr, m->d_ctr, sizeof(u64) * CTR_COUNT, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    int status = status_from_flags(hflags[0]);
+    m->V = (int64_t)(m->h_ctr[CTR_V] < (u64)vcap ? m->h_ctr[CTR_V] : (u64)vcap);
+    m->Elive = (int64_t)m->h_ctr[CTR_ELIVE];
+    m->NC = (int64_t)m->h_ctr[CTR_NCONE];
+    // closed + consistently oriented <=> every half-edge was claimed into a pair
+    const u64 pairs = m->h_ctr[CTR_E_CONVEX] + m->h_ctr[CTR_E_CONCAVE] + m->h_ctr[CTR_E_FLAT];
+    if ((status == SDF_OK || status == SDF_ENOTCLOSED) && 2 * pairs != (u64)nc) {
+        // which of "not closed" / "mis-oriented" it is: the exact (sorted-key) classifier
+        CKS(classify_edge_errors(m, nc, tmp, st));
+        CK(cudaMemcpyAsync(hflags, m->d_flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        status = status_from_flags(hflags[0]);
+        if (status == SDF_OK) status = SDF_ENOTCLOSED;
+    }
+    return status;
+}
+
+// A0: order the triangles along a Morton curve, fine enough that consecutive triangles share vertices and edges
+// (every later gather / scatter then stays L2-local; the paper sorts by Morton code for the same reason,
+// PAPER.md:296-332): bins per axis ~ sqrt(F / 192) -- a surface occupies ~6 n^2 of the n^3 bins, ~32 triangles each.
+// One-pass counting sort (fine_bin_kernel).  The order is internal: ids written to the output are the caller's.
+struct OrderWs { u32 *cnt, *key, *ticket; u64 *scan_ws; int *bbox; int bits; int64_t nbins; bool on; };
+static void order_plan(int64_t F, int64_t min_f, OrderWs *w) {
+    const char *nb = getenv("SDF_NO_BINNING");
+    w->on = !(nb && nb[0] == '1') && F >= min_f;
+    int bits = 2;
+    while (bits < 7 && (int64_t)192 * (1 << (2 * bits)) < F) bits++;
+    if (const char *bb = getenv("SDF_BIN_BITS")) { const int v = atoi(bb); if (v >= 1 && v <= 8) bits = v; }
+    w->bits = bits;
+    w->nbins = (int64_t)1 << (3 * bits);
+}
+static void order_carve(Carver &c, int64_t F, OrderWs *w) {
+    if (!w->on) return;
+    w->cnt = c.take<u32>((size_t)w->nbins);
+    w->scan_ws = c.take<u64>(scan_ws_elems(w->nbins));
+    w->key = c.take<u32>((size_t)F); w->ticket = c.take<u32>((size_t)F);
+    w->bbox = c.take<int>(8);
+}
+static int order_triangles(const float *src, int64_t F, const OrderWs &w, u32 *perm, cudaStream_t st) {
+    if (!w.on) {
+        KL; identity_perm_kernel<<<blocks_for(F), FB, 0, st>>>((int)F, perm);
+        return SDF_OK;
+    }
+    const int lo_hi[8] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF, (int)0x80000000, (int)0x80000000, (int)0x80000000, 0, 0};
+    CK(cudaMemcpyAsync(w.bbox, lo_hi, sizeof(lo_hi), cudaMemcpyHostToDevice, st));
+    CK(cudaMemsetAsync(w.cnt, 0, sizeof(u32) * (size_t)w.nbins, st));
+    const int stride = F > (1 << 20) ? 64 : (F > (1 << 16) ? 8 : 1);
+    KL; bbox_sample_kernel<<<blocks_for((F + stride - 1) / stride), FB, 0, st>>>(src, (int)F, stride, w.bbox);
+    KL; fine_bin_kernel<<<blocks_for(F), FB, 0, st>>>(src, (int)F, w.bbox, w.bits, w.cnt, w.key, w.ticket);
+    CKS(launch_scan(BinIn{w.cnt}, BinOut{w.cnt}, w.nbins, w.scan_ws, (u64 *)nullptr, st));
+    KL; fine_scatter_kernel<<<blocks_for(F), FB, 0, st>>>((int)F, w.cnt, w.key, w.ticket, perm);
+    CK(cudaGetLastError());
+    return SDF_OK;
+}
+
+static int build_features_global(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st) {
     const int64_t F = m->F;
     const int nc = (int)(3 * F);
     const sdf_allocator *al = &m->alloc;
     TmpPool tmp(al, st);
     StreamDrain drain;
     m->E = nc / 2;
+    // every vertex of a closed surface has at least two corners, so V <= 3F/2; the per-vertex tables are sized by that
+    // bound (no host crossing for the count) and a soup with more vertices is flagged not closed by ingest_weld_kernel
+    const int vcap = (int)((3 * F < 3 * F / 2 + 64) ? 3 * F : 3 * F / 2 + 64);
+    m->V = vcap;                                   // provisional: the count comes back with the validation flags
 
-    // persistent F-sized tables: one slab
+    // persistent tables: one slab
     for (int pass = 0; pass < 2; pass++) {
         Carver c(m->slab_f);
         m->soup = c.take<float>(9 * (size_t)F);
@@ -640,6 +749,9 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
         m->fsm = c.take<float>((size_t)F);
         m->perm = c.take<int>((size_t)F);
         m->inv_perm = c.take<int>((size_t)F);
+        m->vrec = c.take<VertexRec>((size_t)vcap);
+        m->vmint = c.take<int>((size_t)vcap);
+        m->cone_list = c.take<u32>(2 * (size_t)vcap);
         m->d_ctr = c.take<u64>(CTR_TOTAL);
         m->d_flags = c.take<int>(4);
         if (pass == 0) CKS(dev_alloc(al, &m->slab_f, c.off, st));
@@ -647,6 +759,13 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     CK(cudaMemsetAsync(m->d_ctr, 0, sizeof(u64) * CTR_TOTAL, st));
     CK(cudaMemsetAsync(m->d_flags, 0, sizeof(int) * 4, st));
     CK(cudaMemsetAsync(m->adj, 0xFF, sizeof(int) * 3 * F, st));
+    CK(cudaMemsetAsync(m->fsm, 0, sizeof(float) * (size_t)F, st));
+
+    // smooth features get no polyhedron of their own (common.cuh, SMOOTH_SIN_DEFAULT); SDF_SMOOTH_SIN=0 switches that off
+    float smooth_sin = SMOOTH_SIN_DEFAULT;
+    if (const char *ss = getenv("SDF_SMOOTH_SIN")) { smooth_sin = (float)atof(ss); if (!(smooth_sin >= 0.0f && smooth_sin <= 0.25f)) smooth_sin = SMOOTH_SIN_DEFAULT; }
+    const char *rc = getenv("SDF_RUFF");
+    const bool ruff_cone = rc && !strcmp(rc, "cone");
 
     // ---- A0 ingest + A1 weld (hash table on the exact coordinate bits)
     CKS(maybe_prefill(m, 1, st));
@@ -654,29 +773,28 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     const u32 capw = pow2_at_least((u64)nc + (u64)nc / 4 + 1);     // load <= 0.8 even if no vertex is shared
     const u32 cape = pow2_at_least((u64)nc + 1);                   // <= 3F/2 forward half-edges: load <= 0.5
     float *staging = nullptr;
-    const char *nb = getenv("SDF_NO_BINNING");
-    const bool bin = !(nb && nb[0] == '1') && F >= 131072;     // smaller meshes live in L2 anyway
-    u32 *bkeys = nullptr, *bkeys2 = nullptr, *bvals2 = nullptr, *bhist = nullptr;
-    int *bbox = nullptr;
-    u32 *wtab = nullptr, *slot = nullptr, *etab = nullptr;
-    u64 *scan_ws = nullptr;
-    unsigned char *head = nullptr;
-    int *vcorner = nullptr;
+    OrderWs ow = {};
+    order_plan(F, 131072, &ow);                     // smaller meshes live in L2 anyway
+    u32 *wtab = nullptr, *slot = nullptr, *etab = nullptr, *wvid = nullptr;
+    int *vcorner = nullptr, *vside = nullptr;
+    u64 *vacc = nullptr;
+    double *vn64 = nullptr;
+    long long *vcosq = nullptr, *vcospos = nullptr;
     void *tslab = nullptr;
     for (int pass = 0; pass < 2; pass++) {
         Carver c(tslab);
         wtab = c.take<u32>((size_t)capw);           // wtab and etab adjacent: one memset
         etab = c.take<u32>((size_t)cape);
+        wvid = c.take<u32>((size_t)capw);           // slot -> vertex id, written by the inserter (no reset needed)
         slot = c.take<u32>((size_t)nc);
-        scan_ws = c.take<u64>(scan_ws_elems((int64_t)nc));
-        head = c.take<unsigned char>((size_t)nc);
-        vcorner = c.take<int>((size_t)nc);          // V <= 3F
+        vcorner = c.take<int>((size_t)vcap);
+        vacc = c.take<u64>(3 * (size_t)vcap);
+        vside = c.take<int>((size_t)vcap);
+        vcosq = c.take<long long>((size_t)vcap);
+        if (ruff_cone) vcospos = c.take<long long>((size_t)vcap);
+        vn64 = c.take<double>(3 * (size_t)vcap);
         if (!on_device) staging = c.take<float>(9 * (size_t)F);
-        if (bin) {
-            bkeys = c.take<u32>((size_t)F); bkeys2 = c.take<u32>((size_t)F); bvals2 = c.take<u32>((size_t)F);
-            bhist = c.take<u32>(radix_hist_elems((int)F));
-            bbox = c.take<int>(8);
-        }
+        order_carve(c, F, &ow);
         if (pass == 0) CKS(tmp.get(&tslab, c.off));
     }
     const float *src = tri;
@@ -685,108 +803,34 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
         src = staging;
     }
     CK(cudaMemsetAsync(wtab, 0xFF, (size_t)((char *)(etab + cape) - (char *)wtab), st));
-    // A0: order the triangles along a coarse Morton curve, gather + canonicalise
-    u32 *perm = (u32 *)m->perm;
-    if (bin) {
-        const int lo_hi[8] = {0x7FFFFFFF, 0x7FFFFFFF, 0x7FFFFFFF, (int)0x80000000, (int)0x80000000, (int)0x80000000, 0, 0};
-        CK(cudaMemcpyAsync(bbox, lo_hi, sizeof(lo_hi), cudaMemcpyHostToDevice, st));
-        const int stride = F > (1 << 20) ? 64 : (F > (1 << 16) ? 8 : 1);
-        KL; bbox_sample_kernel<<<blocks_for((F + stride - 1) / stride), FB, 0, st>>>(src, (int)F, stride, bbox);
-        KL; bin_key_kernel<<<blocks_for(F), FB, 0, st>>>(src, (int)F, bbox, bkeys, perm);
-        const int shifts[2] = {0, 8};
-        bool first;
-        CKS(radix_sort_pairs<u32>(bkeys, perm, bkeys2, bvals2, (int)F, shifts, 2, bhist, scan_ws, st, &first));
-        if (!first) CK(cudaMemcpyAsync(perm, bvals2, sizeof(u32) * (size_t)F, cudaMemcpyDeviceToDevice, st));
-    } else {
-        KL; identity_perm_kernel<<<blocks_for(F), FB, 0, st>>>((int)F, perm);
-    }
-    KL; ingest_weld_kernel<<<blocks_for(nc), FB, 0, st>>>(src, m->perm, nc, m->soup, m->inv_perm, wtab, capw - 1, slot, m->d_flags);
-    CKS(launch_scan2(HeadCompute{wtab, slot, head}, HeadIn{head}, HeadOut{wtab, slot, vcorner}, (int64_t)nc, scan_ws,
-                     m->d_ctr + CTR_V, st));
+    CKS(order_triangles(src, F, ow, (u32 *)m->perm, st));
+    KL; ingest_weld_kernel<<<blocks_for(nc), FB, 0, st>>>(src, m->perm, nc, m->soup, m->inv_perm, wtab, capw - 1, slot, wvid, vcorner,
+                                                        vacc, vcosq, vcospos, vside, m->vmint, vcap, m->d_ctr, m->d_flags);
     stage_mark(m, SDF_T_INGEST_WELD, 1, st);
-    // first host crossing: the vertex count sizes every per-vertex table
-    int hflags[4] = {0, 0, 0, 0};
-    CK(cudaMemcpyAsync(m->h_ctr, m->d_ctr, sizeof(u64) * CTR_COUNT, cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(hflags, m->d_flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
-    // non-finite input is rejected here: Inf / NaN coordinates would turn into whole-axis cell ranges downstream
-    if (hflags[0] & ERRB_NONFINITE) return SDF_EINVAL;
-    m->V = (int64_t)m->h_ctr[CTR_V];
-    const int V = (int)m->V;
-
-    // V-sized tables: one persistent slab, one temporary slab
-    for (int pass = 0; pass < 2; pass++) {
-        Carver c(m->slab_v);
-        m->vrec = c.take<VertexRec>((size_t)V);
-        m->vmint = c.take<int>((size_t)V);
-        m->cone_list = c.take<u32>(2 * (size_t)V);
-        if (pass == 0) CKS(dev_alloc(al, &m->slab_v, c.off, st));
-    }
-    u64 *vacc = nullptr;
-    double *vn64 = nullptr;
-    long long *vcosq = nullptr, *vcospos = nullptr;
-    // smooth features get no polyhedron of their own (common.cuh, SMOOTH_SIN_DEFAULT); SDF_SMOOTH_SIN=0 switches that off
-    float smooth_sin = SMOOTH_SIN_DEFAULT;
-    if (const char *ss = getenv("SDF_SMOOTH_SIN")) { smooth_sin = (float)atof(ss); if (!(smooth_sin >= 0.0f && smooth_sin <= 0.25f)) smooth_sin = SMOOTH_SIN_DEFAULT; }
-    const char *rc = getenv("SDF_RUFF");
-    const bool ruff_cone = rc && !strcmp(rc, "cone");
-    int *vside = nullptr;
-    void *vslab = nullptr;
-    for (int pass = 0; pass < 2; pass++) {
-        Carver c(vslab);
-        vacc = c.take<u64>(3 * (size_t)V);          // vacc and vside adjacent: one memset to 0
-        vside = c.take<int>((size_t)V);
-        vcosq = c.take<long long>((size_t)V);
-        if (ruff_cone) vcospos = c.take<long long>((size_t)V);     // right behind vcosq: one memset
-        vn64 = c.take<double>(3 * (size_t)V);
-        if (pass == 0) CKS(tmp.get(&vslab, c.off));
-    }
 
     // ---- A3 (per triangle), A2 edge table
     CKS(maybe_prefill(m, 2, st));
     stage_mark(m, SDF_T_EDGES, 0, st);
-    CK(cudaMemsetAsync(vacc, 0, (size_t)((char *)(vside + V) - (char *)vacc), st));
-    CK(cudaMemsetAsync(m->fsm, 0, sizeof(float) * (size_t)F, st));
-    KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wtab, slot, (int)F, m->cvid, m->fn, vacc, etab, cape - 1, m->d_flags);
+    KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wvid, slot, (int)F, m->cvid, m->fn, vacc, etab, cape - 1, m->d_flags);
     // sdf_transform: the per-compute workspace of A6a is taken in the order of `st` BEFORE the fork, so that the
     // vertex stream (which first touches it) is ordered after the allocation
     CKS(maybe_alloc_brick_ws(m, st));
     // the vertex stage needs only what tri_geom wrote: it runs on a second stream beside the edge stage
     cudaStream_t vs = st;
-    {
-        const char *cf = getenv("SDF_CREATE_FORK");
-        if (!(cf && cf[0] == '0')) {
-            static cudaStream_t g_vs = nullptr;
-            static int g_vs_dev = -1;
-            int dev = 0;
-            CK(cudaGetDevice(&dev));
-            if (!g_vs || g_vs_dev != dev) {
-                CK(cudaStreamCreateWithFlags(&g_vs, cudaStreamNonBlocking));
-                g_vs_dev = dev;
-            }
-            vs = g_vs;
-            if (!m->ev_fork) CK(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
-            if (!m->ev_join) CK(cudaEventCreateWithFlags(&m->ev_join, cudaEventDisableTiming));
-            CK(cudaEventRecord(m->ev_fork, st));
-            CK(cudaStreamWaitEvent(vs, m->ev_fork, 0));
-            drain.s = vs; drain.armed = true;
-        }
-    }
+    CKS(fork_vertex_stream(m, st, &vs, drain));
     CKS(maybe_prefill(m, 3, st));
-    KL; edge_pair_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, etab, cape - 1, m->adj);
-    KL; edge_record_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, m->adj, m->soup, m->fn, m->perm, smooth_sin, m->erec, (int)m->E, (int *)m->fsm, m->d_ctr);
+    // pairing, classes and wedge records in one pass
+    KL; edge_pair_record_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, etab, cape - 1, m->adj, m->soup, m->fn, m->perm,
+                                                            smooth_sin, m->erec, (int)m->E, (int *)m->fsm, m->d_ctr, m->d_flags);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_EDGES, 1, st);
 
     // ---- A3/A4 vertices (garbage-in on invalid input is harmless: ids stay in range)
     stage_mark(m, SDF_T_VERTICES, 0, vs);
-    // "larger than any value" initial states: 0x7F7F.. for the cone cosines and triangle ids
-    CK(cudaMemsetAsync(vcosq, 0x7F, sizeof(long long) * (size_t)V, vs));
-    if (vcospos) CK(cudaMemsetAsync(vcospos, 0x7F, sizeof(long long) * (size_t)V, vs));
-    CK(cudaMemsetAsync(m->vmint, 0x7F, sizeof(int) * (size_t)V, vs));
-    KL; vertex_normal_kernel<<<blocks_for(V), FB, 0, vs>>>(vacc, V, vn64);
+    KL; vertex_normal_kernel<<<blocks_for(vcap), FB, 0, vs>>>(vacc, vcap, m->d_ctr + CTR_V, vn64);
     KL; vertex_cone_kernel<<<blocks_for(F), FB, 0, vs>>>(m->soup, m->cvid, (int)F, vn64, vcosq, vside, m->perm, m->vmint, vcospos);
-    KL; vertex_record_kernel<<<blocks_for(V), FB, 0, vs>>>(m->soup, vcorner, vn64, vcosq, vside, V, vcospos, smooth_sin, m->vrec, m->cone_list, m->d_ctr);
+    KL; vertex_record_kernel<<<blocks_for(vcap), FB, 0, vs>>>(m->soup, vcorner, vn64, nullptr, m->d_ctr + CTR_V, vcosq, vside, vcap,
+                                                           vcospos, smooth_sin, m->vrec, m->cone_list, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_VERTICES, 1, vs);
     CKS(maybe_prepare_bricks(m, st, vs));
@@ -797,21 +841,137 @@ int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st
     }
     KL; face_margin_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, m->vrec, m->fsm);
     CK(cudaGetLastError());
-    // second host crossing: validation flags + class counters
-    CK(cudaMemcpyAsync(hflags, m->d_flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(m->h_ctr, m->d_ctr, sizeof(u64) * CTR_COUNT, cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
-    int status = status_from_flags(hflags[0]);
-    m->Elive = (int64_t)m->h_ctr[CTR_ELIVE];
-    m->NC = (int64_t)m->h_ctr[CTR_NCONE];
-    // closed + consistently oriented <=> every half-edge was claimed into a pair
-    const u64 pairs = m->h_ctr[CTR_E_CONVEX] + m->h_ctr[CTR_E_CONCAVE] + m->h_ctr[CTR_E_FLAT];
-    if (status == SDF_OK && 2 * pairs != (u64)nc) {
-        CKS(classify_edge_errors(m, nc, tmp, st));
-        CK(cudaMemcpyAsync(hflags, m->d_flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
-        CK(cudaStreamSynchronize(st));
-        status = status_from_flags(hflags[0]);
-        if (status == SDF_OK) status = SDF_ENOTCLOSED;
+    return finish_features(m, nc, vcap, tmp, st);
+}
+
+// ===================================================================================================
+// the tile-local builder (default; tile_features.cuh)
+// ===================================================================================================
+static int build_features_tile(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st) {
+    const int64_t F = m->F;
+    const int nc = (int)(3 * F);
+    const sdf_allocator *al = &m->alloc;
+    TmpPool tmp(al, st);
+    StreamDrain drain;
+    m->E = nc / 2;
+    // every vertex of a closed surface has at least two corners, so V <= 3F/2; the per-vertex tables are sized by that
+    // bound (no host crossing for the count) and a soup with more vertices is flagged not closed by tile_weld_kernel
+    const int vcap = (int)((3 * F < 3 * F / 2 + 64) ? 3 * F : 3 * F / 2 + 64);
+    m->V = vcap;                                   // provisional: the count comes back with the validation flags
+    const int ntiles = (int)((F + TT - 1) / TT);
+
+    for (int pass = 0; pass < 2; pass++) {
+        Carver c(m->slab_f);
+        m->soup = c.take<float>(9 * (size_t)F);
+        m->fn = c.take<float>(3 * (size_t)F);
+        m->cvid = c.take<int>(3 * (size_t)F);
+        m->adj = c.take<int>(3 * (size_t)F);
+        m->erec = c.take<EdgeRec>((size_t)(m->E > 0 ? m->E : 1));
+        m->fsm = c.take<float>((size_t)F);
+        m->perm = c.take<int>((size_t)F);
+        m->inv_perm = c.take<int>((size_t)F);
+        m->vrec = c.take<VertexRec>((size_t)vcap);
+        m->vmint = c.take<int>((size_t)vcap);
+        m->cone_list = c.take<u32>(2 * (size_t)vcap);
+        m->d_ctr = c.take<u64>(CTR_TOTAL);
+        m->d_flags = c.take<int>(4);
+        if (pass == 0) CKS(dev_alloc(al, &m->slab_f, c.off, st));
     }
-    return status;      // temporaries are released here
+    CK(cudaMemsetAsync(m->d_ctr, 0, sizeof(u64) * CTR_TOTAL, st));
+    CK(cudaMemsetAsync(m->d_flags, 0, sizeof(int) * 4, st));
+
+    float smooth_sin = SMOOTH_SIN_DEFAULT;
+    if (const char *ss = getenv("SDF_SMOOTH_SIN")) { smooth_sin = (float)atof(ss); if (!(smooth_sin >= 0.0f && smooth_sin <= 0.25f)) smooth_sin = SMOOTH_SIN_DEFAULT; }
+    const char *rc = getenv("SDF_RUFF");
+    const bool ruff_cone = rc && !strcmp(rc, "cone");
+
+    CKS(maybe_prefill(m, 1, st));
+    stage_mark(m, SDF_T_INGEST_WELD, 0, st);
+    // global tables: only the unique vertices of each tile and the half-edges without a partner in their tile go
+    // through them, but a hostile soup can still send every corner there: sized for that, so no probe loop can fill one
+    const u32 capw = pow2_at_least((u64)nc + (u64)nc / 4 + 1);
+    const u32 cape = pow2_at_least((u64)nc + 1);
+    float *staging = nullptr;
+    OrderWs ow = {};
+    order_plan(F, 4 * TT, &ow);                     // a few tiles need no order
+    u32 *wtab = nullptr, *etab = nullptr;
+    int *vcorner = nullptr, *vside = nullptr;
+    u64 *vacc = nullptr;
+    long long *vcosq = nullptr, *vcospos = nullptr;
+    TileTables tt = {nullptr, nullptr, nullptr, nullptr};
+    void *tslab = nullptr;
+    for (int pass = 0; pass < 2; pass++) {
+        Carver c(tslab);
+        wtab = c.take<u32>((size_t)capw);           // wtab and etab adjacent: one memset
+        etab = c.take<u32>((size_t)cape);
+        tt.wvid = c.take<u32>((size_t)capw);
+        tt.clv = c.take<unsigned short>((size_t)nc);
+        tt.tvid = c.take<u32>((size_t)nc);
+        tt.tnlv = c.take<int>((size_t)ntiles);
+        vcorner = c.take<int>((size_t)vcap);
+        vacc = c.take<u64>(3 * (size_t)vcap);
+        vside = c.take<int>((size_t)vcap);
+        vcosq = c.take<long long>((size_t)vcap);
+        if (ruff_cone) vcospos = c.take<long long>((size_t)vcap);
+        if (!on_device) staging = c.take<float>(9 * (size_t)F);
+        order_carve(c, F, &ow);
+        if (pass == 0) CKS(tmp.get(&tslab, c.off));
+    }
+    const float *src = tri;
+    if (!on_device) {
+        CK(cudaMemcpyAsync(staging, tri, sizeof(float) * 9 * F, cudaMemcpyHostToDevice, st));
+        src = staging;
+    }
+    CK(cudaMemsetAsync(wtab, 0xFF, (size_t)((char *)(etab + cape) - (char *)wtab), st));
+    CKS(order_triangles(src, F, ow, (u32 *)m->perm, st));
+    static bool attr_set = false;
+    if (!attr_set) {
+        CK(cudaFuncSetAttribute(tile_geom_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileGeomSmem)));
+        CK(cudaFuncSetAttribute(tile_cone_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileConeSmem)));
+        attr_set = true;
+    }
+    // A1: weld inside the tiles, the tiles' unique vertices through the global table
+    KL; tile_weld_kernel<<<ntiles, TB, 0, st>>>(src, m->perm, (int)F, m->soup, m->inv_perm, wtab, capw - 1, tt, vcorner, vacc,
+                                              vcosq, vcospos, vside, m->vmint, vcap, m->d_ctr, m->d_flags);
+    stage_mark(m, SDF_T_INGEST_WELD, 1, st);
+    // A2 + A3: ids, normals, angle-weighted sums, edges inside the tiles
+    CKS(maybe_prefill(m, 2, st));
+    stage_mark(m, SDF_T_EDGES, 0, st);
+    KL; tile_geom_kernel<<<ntiles, TB, sizeof(TileGeomSmem), st>>>(m->soup, (int)F, m->perm, tt, wtab, m->cvid, m->fn, vacc, m->adj,
+                                                                 etab, cape - 1, smooth_sin, m->erec, (int)m->E, m->fsm,
+                                                                 m->d_ctr, m->d_flags);
+    CK(cudaGetLastError());
+    // sdf_transform: the workspace of A6a is taken in the order of `st` BEFORE the fork (the vertex stream touches it first)
+    CKS(maybe_alloc_brick_ws(m, st));
+    cudaStream_t vs = st;
+    CKS(fork_vertex_stream(m, st, &vs, drain));
+    CKS(maybe_prefill(m, 3, st));
+    // edges across tile boundaries
+    KL; edge_pair_record_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, etab, cape - 1, m->adj, m->soup, m->fn, m->perm,
+                                                            smooth_sin, m->erec, (int)m->E, (int *)m->fsm, m->d_ctr, m->d_flags);
+    CK(cudaGetLastError());
+    stage_mark(m, SDF_T_EDGES, 1, st);
+    // A3/A4 vertices: cone angles, sides, lowest triangle ids per tile; then the records
+    stage_mark(m, SDF_T_VERTICES, 0, vs);
+    KL; tile_cone_kernel<<<ntiles, TB, sizeof(TileConeSmem), vs>>>(m->soup, (int)F, m->perm, tt, vacc, vcosq, vside, m->vmint, vcospos);
+    KL; vertex_record_kernel<<<blocks_for(vcap), FB, 0, vs>>>(m->soup, vcorner, nullptr, vacc, m->d_ctr + CTR_V, vcosq, vside, vcap,
+                                                           vcospos, smooth_sin, m->vrec, m->cone_list, m->d_ctr);
+    CK(cudaGetLastError());
+    stage_mark(m, SDF_T_VERTICES, 1, vs);
+    CKS(maybe_prepare_bricks(m, st, vs));
+    if (vs != st) {
+        CK(cudaEventRecord(m->ev_join, vs));
+        CK(cudaStreamWaitEvent(st, m->ev_join, 0));
+        drain.armed = false;           // joined: `st` now carries the dependency
+    }
+    KL; face_margin_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, m->vrec, m->fsm);
+    CK(cudaGetLastError());
+    return finish_features(m, nc, vcap, tmp, st);
+}
+
+int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st) {
+    // SDF_BUILDER=tile: the tile-local builder (tile_features.cuh), measured slower on a B200: an ablation
+    const char *b = getenv("SDF_BUILDER");
+    if (b && !strcmp(b, "tile")) return build_features_tile(m, tri, on_device, st);
+    return build_features_global(m, tri, on_device, st);
 }

@@ -120,3 +120,35 @@ def test_edge_error_classification():
         B.sdf_create(np.ascontiguousarray(np.concatenate([soup, fin])))
     assert e.value.status == B.SDF_ENOTCLOSED
     B.sdf_destroy(B.sdf_create(soup))
+
+
+@pytest.mark.parametrize("name,scale", [("C1", 1.0), ("C2", 1.0), ("C3", 0.5), ("C4", 0.12), ("C5", 0.05)])
+def test_tile_builder_equals_global_builder(monkeypatch, name, scale):
+    """The tile-local feature builder (default: weld, pair and accumulate inside spatial tiles in shared memory, only
+    tile-boundary features through the global tables) against the first builder (SDF_BUILDER=global: every corner and
+    half-edge through the global tables): same topology, same class counts, same pseudonormal data and bit-identical
+    grids -- the two differ in how the data moves, not in any arithmetic that reaches the output."""
+    import torch
+    from paper_1903_00353_b200 import binding as B
+    from gpu_util import f32_grid
+    w = f32_grid(W.config(name, scale) if scale < 1.0 else W.config(name))
+    keys = ("F", "V", "E", "edges_convex", "edges_concave", "edges_flat", "verts_pos_only", "verts_neg_only", "verts_both",
+            "verts_skipped", "verts_hemisphere", "band_cells", "polyhedra")
+    m1, d1, t1 = B.compute_workload(w)
+    s1 = B.sdf_stats(m1)
+    monkeypatch.setenv("SDF_BUILDER", "tile")
+    m0, d0, t0 = B.compute_workload(w)
+    s0 = B.sdf_stats(m0)
+    monkeypatch.delenv("SDF_BUILDER")
+    assert {k: s1[k] for k in keys} == {k: s0[k] for k in keys}
+    assert torch.equal(t0, t1) and torch.equal(d0.view(torch.int32), d1.view(torch.int32))
+    # per-vertex data, matched through the corner -> vertex tables (the numbering of the vertices differs)
+    c0, c1 = (B.sdf_get_table(m, B.TABLE_CORNER_VID).reshape(-1) for m in (m0, m1))
+    v0, v1 = (B.sdf_get_table(m, B.TABLE_VERTEX_REC) for m in (m0, m1))
+    for f in ("pos", "axis", "cos_cone", "info"):
+        assert np.array_equal(np.asarray(v0[f])[c0], np.asarray(v1[f])[c1]), f
+    assert np.array_equal(B.sdf_get_table(m0, B.TABLE_VERTEX_MINTRI)[c0], B.sdf_get_table(m1, B.TABLE_VERTEX_MINTRI)[c1])
+    assert np.array_equal(B.sdf_get_table(m0, B.TABLE_HALFEDGE_ADJ), B.sdf_get_table(m1, B.TABLE_HALFEDGE_ADJ))
+    assert np.array_equal(B.sdf_get_table(m0, B.TABLE_FACE_NORMAL), B.sdf_get_table(m1, B.TABLE_FACE_NORMAL))
+    e0, e1 = (np.sort(B.sdf_get_table(m, B.TABLE_EDGE_REC).view(np.uint8).reshape(-1, 64).view("V64").reshape(-1)) for m in (m0, m1))
+    assert np.array_equal(e0, e1)
