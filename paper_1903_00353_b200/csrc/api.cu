@@ -181,6 +181,12 @@ static int make_grid(const float origin[3], float h, int nx, int ny, int nz, flo
     g->fill_depth = fd ? atoi(fd) : 8;
     g->fill_issuers = fi ? atoi(fi) : 4;
     if (g->fill_issuers < 1 || g->fill_issuers > 4) g->fill_issuers = 4;
+    const char *fck = getenv("SDF_FILL_CHUNK_LOG2");
+    g->fill_chunk_log2 = fck ? atoi(fck) : 12;
+    if (g->fill_chunk_log2 < 11 || g->fill_chunk_log2 > 14) g->fill_chunk_log2 = 12;
+    const char *fsh = getenv("SDF_FILL_SM_SHARE");
+    g->fill_sm_share = fsh ? atoi(fsh) : 8;
+    if (g->fill_sm_share < 1 || g->fill_sm_share > 8) g->fill_sm_share = 8;
     g->vec4 = (nx % 4 == 0) && (((uintptr_t)dist & 15) == 0) && (((uintptr_t)tri & 15) == 0);
     return SDF_OK;
 }
@@ -208,13 +214,15 @@ int sdf_transform(const float *tri_xyz, int64_t ntri, int on_device, const sdf_a
     cudaStream_t st = (cudaStream_t)stream;
     sdf_mesh *m = nullptr;
     CKS(new_mesh(ntri, a, stream, &m));
-    // the sentinel fill (A8a) needs only the output pointers, so it could start under A0-A4: build_features
-    // starts it at the stage boundary SDF_PREFILL_AT (1 before A0, 2 before the edge table, 3 before edge
-    // pairing).  Measured: the feature kernels are DRAM-latency bound and stall under the fill's
-    // write stream -- the step gets 0.7 ms longer at C4 -- so the default is 4: run_compute forks it beside A5-A7.
+    // the sentinel fill (A8a) needs only the output pointers: build_features starts it at the stage boundary
+    // SDF_PREFILL_AT (1 before A0, 2 before the edge table, 3 before edge pairing, 4 = default: behind the last feature
+    // kernel, i.e. under the host crossing; 5: run_compute forks it after the crossing, as the two calls do).
+    // Measured: the feature kernels are bound by the same memory pipe as the fill -- beside it each is
+    // stretched by what the fill moves meanwhile, whatever the fill's rate -- so 1..3 lose; only the instruction-bound
+    // evaluate kernels hide it.
     const bool pre = g.fill_mode < 2 || g.fill_mode == 4;
     const char *pa = getenv("SDF_PREFILL_AT");
-    m->pre_at = (pa && pa[0] >= '1' && pa[0] <= '4') ? pa[0] - '0' : 4;
+    m->pre_at = (pa && pa[0] >= '1' && pa[0] <= '5') ? pa[0] - '0' : 4;
     m->pre_g = pre ? &g : nullptr;
     m->pre_dist = dist_out;
     m->pre_tri = tri_out;

@@ -121,6 +121,8 @@ struct GridParams {
     int fill_prio;                  // side stream at the highest priority
     int fill_ctas;                  // TMA fill: CTAs launched per SM (one per SM survives)
     int fill_depth, fill_issuers;   // TMA fill: chunk pairs in flight per issuing lane, issuing lanes per SM
+    int fill_chunk_log2;            // TMA fill: log2 of the bytes per bulk copy (11..14)
+    int fill_sm_share;              // TMA fill: SMs out of every 8 that stream (8 = all; fewer = throttled, ablation)
 };
 
 // ---------------------------------------------------------------------------------------

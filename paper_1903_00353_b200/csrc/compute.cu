@@ -428,29 +428,34 @@ __global__ void __launch_bounds__(FILL_BT) fill_kernel(float *__restrict__ dist,
 // UBLKCP), L2 evict-first.  It needs 4 warps and 8 KiB of shared memory per SM, so the kernels
 // of A5-A7 keep (almost) the whole SM while 8 B/cell stream out underneath them.
 #define FILL_TMA_BT 128
-#define FILL_TMA_CHUNK 4096      // bytes per bulk copy.  The size sets the balance with the kernels running beside
+#define FILL_TMA_CHUNK 4096      // default bytes per bulk copy (runtime: bits 16.. of the `issuers` argument hold log2).  The size sets the balance with the kernels running beside
                                  // the fill: 2 KiB starves them (evaluate 1.46 -> 1.96 ms at C4), 16 KiB yields to them
                                  // (fill 1.55 ms); alone the fill does 7.3 TB/s at 4 KiB
 // fill_state: [0] = next batch (dynamic fetch), [1 + smid] = SM already has a fill CTA.  More
 // CTAs than SMs are launched and the first to arrive on an SM claims it; the others exit at
 // once.  (With one CTA per SM by count only, a busy GPU stacked several fill CTAs on the few
 // SMs that had room and the fill ran at a fraction of the HBM rate.)
-#define FILL_BATCH (1048576 / FILL_TMA_CHUNK)   // chunks per fetch: 1 MiB contiguous per array
+#define FILL_TMA_MAX 16384
+#define FILL_BATCH_BYTES 1048576                // bytes per fetch: 1 MiB contiguous per array
 #define FILL_STATE_WORDS 1024
 template <int DEPTH>
 __global__ void __launch_bounds__(FILL_TMA_BT) fill_tma_kernel(float *__restrict__ dist, int *__restrict__ tri,
                                                                int64_t n, int issuers, int batch, u32 *__restrict__ state,
                                                                u32 pat_d, u32 pat_t) {
-    __shared__ __align__(128) u32 s_d[FILL_TMA_CHUNK / 4];
-    __shared__ __align__(128) u32 s_t[FILL_TMA_CHUNK / 4];
+    __shared__ __align__(128) u32 s_d[FILL_TMA_MAX / 4];
+    __shared__ __align__(128) u32 s_t[FILL_TMA_MAX / 4];
+    const int chunk = 1 << ((issuers >> 16) & 31);
     __shared__ int s_go;
-    const int64_t per = FILL_TMA_CHUNK / 4;
+    const int64_t per = chunk / 4;
     const int64_t nchunks = n / per;
     if (threadIdx.x == 0) {
         u32 smid;
         asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
         s_go = (smid < FILL_STATE_WORDS - 1) ? (atomicCAS(&state[1 + smid], 0u, 1u) == 0u) : 1;
+        // throttle (ablation): only sm_share of every 8 SMs stream
+        if ((int)(smid & 7u) >= ((issuers >> 8) & 255)) s_go = 0;
     }
+    issuers &= 255;
     // ragged tail (< one chunk) with plain stores
     if (blockIdx.x == 0)
         for (int64_t i = nchunks * per + threadIdx.x; i < n; i += FILL_TMA_BT) {
@@ -458,7 +463,7 @@ __global__ void __launch_bounds__(FILL_TMA_BT) fill_tma_kernel(float *__restrict
         }
     __syncthreads();
     if (!s_go) return;
-    for (int i = threadIdx.x; i < FILL_TMA_CHUNK / 4; i += FILL_TMA_BT) { s_d[i] = pat_d; s_t[i] = pat_t; }
+    for (int i = threadIdx.x; i < chunk / 4; i += FILL_TMA_BT) { s_d[i] = pat_d; s_t[i] = pat_t; }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy writes -> async proxy reads
     __syncthreads();
     if ((threadIdx.x & 31) == 0 && (threadIdx.x >> 5) < issuers) {
@@ -472,9 +477,9 @@ __global__ void __launch_bounds__(FILL_TMA_BT) fill_tma_kernel(float *__restrict
             const int64_t c0 = bt * batch, c1 = c0 + batch < nchunks ? c0 + batch : nchunks;
             for (int64_t c = c0; c < c1; c++) {
                 asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
-                             :: "l"(dist + c * per), "r"(sd), "r"(FILL_TMA_CHUNK), "l"(pol) : "memory");
+                             :: "l"(dist + c * per), "r"(sd), "r"(chunk), "l"(pol) : "memory");
                 asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
-                             :: "l"(tri + c * per), "r"(stt), "r"(FILL_TMA_CHUNK), "l"(pol) : "memory");
+                             :: "l"(tri + c * per), "r"(stt), "r"(chunk), "l"(pol) : "memory");
                 asm volatile("cp.async.bulk.commit_group;" ::: "memory");
                 // at most DEPTH + 1 chunk pairs in flight per issuing lane
                 asm volatile("cp.async.bulk.wait_group %0;" :: "n"(DEPTH) : "memory");
@@ -537,19 +542,18 @@ __device__ __forceinline__ CellOut finish_cell(const MeshView &mv, const GridPar
     return o;
 }
 
-// One block per active brick (8x8x8 cells, 4 KiB of packed scratch).  Phase 1 loads the
-// brick and compacts its populated cells into a shared list; phase 2 spreads the list over
-// the threads (the sign pass is the expensive, divergent part); phase 3 writes the brick's
-// 64 row segments (8 cells = one 32-B sector each) into both grids.
+// One block per active brick (8x8x8 cells, 4 KiB of packed scratch).  A thread loads four cells (half of an 8-cell
+// row segment = one 32-B sector of each grid).  A cell whose winning extrusion already told the side and whose band
+// test is clear is unpacked on the spot; the others (a few per cent) are queued in shared memory and spread over the
+// threads afterwards -- the sign pass is the expensive, divergent part.  Only row segments that hold a populated
+// cell are written: the sentinel fill has been there before.
 #define EB_BT 128
 __global__ void __launch_bounds__(EB_BT, 12) emit_bricks_kernel(MeshView mv, GridParams g, const int *__restrict__ list,
                                                             const u64 *__restrict__ scratch,
                                                             float *__restrict__ dist, int *__restrict__ tri,
                                                             u64 *__restrict__ ctr) {
-    __shared__ __align__(16) u64 s_pack[BRICK_CELLS];
-    __shared__ __align__(16) float s_d[BRICK_CELLS];
-    __shared__ __align__(16) int s_t[BRICK_CELLS];
-    __shared__ unsigned short s_list[BRICK_CELLS];
+    __shared__ u64 s_pack[BRICK_CELLS];
+    __shared__ unsigned short s_cell[BRICK_CELLS];
     __shared__ u32 s_n, s_stat[2];
     const int tid = threadIdx.x;
     if (tid == 0) { s_n = 0; s_stat[0] = s_stat[1] = 0; }
@@ -557,53 +561,59 @@ __global__ void __launch_bounds__(EB_BT, 12) emit_bricks_kernel(MeshView mv, Gri
     const int slot = blockIdx.x;
     const int b = list[slot];
     const int bx = b % g.nbx, by = (b / g.nbx) % g.nby, bz = b / (g.nbx * g.nby);
+    u32 band = 0, recheck = 0;
     {
         const ulonglong2 *src = (const ulonglong2 *)(scratch + (size_t)slot * BRICK_CELLS) + 2 * tid;
-        ulonglong2 p01 = src[0], p23 = src[1];
+        const ulonglong2 p01 = __ldcs(src), p23 = __ldcs(src + 1);
         const u64 p[4] = {p01.x, p01.y, p23.x, p23.y};
         const int c0 = 4 * tid;
-        // warp-aggregated append of the populated cells
-        int cnt = (p[0] != PACK_EMPTY) + (p[1] != PACK_EMPTY) + (p[2] != PACK_EMPTY) + (p[3] != PACK_EMPTY);
-        const int lane = tid & 31;
-        int inc = cnt;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            int v = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += v;
-        }
-        int base = 0;
-        if (lane == 31 && inc) base = (int)atomicAdd(&s_n, (u32)inc);
-        base = __shfl_sync(0xffffffffu, base, 31) + inc - cnt;
+        float od[4];
+        int ot[4];
+        bool any = false;
+        const float clear = g.band - g.guard;
 #pragma unroll
         for (int c = 0; c < 4; c++) {
-            s_d[c0 + c] = INFINITY; s_t[c0 + c] = -1;
-            if (p[c] != PACK_EMPTY) { s_pack[c0 + c] = p[c]; s_list[base++] = (unsigned short)(c0 + c); }
+            od[c] = INFINITY; ot[c] = -1;
+            if (p[c] == PACK_EMPTY) continue;
+            const float d = __uint_as_float((u32)(p[c] >> 32));
+            if (((u32)p[c] & FL_SURE) && d < clear) {
+                // the winning extrusion already told the side and the band test is clear
+                od[c] = (((u32)p[c] & FL_NEG) && d != 0.0f) ? -d : d;
+                ot[c] = (int)((u32)p[c] >> 2);
+                any = true;
+                band++;
+            } else {
+                const u32 q = atomicAdd(&s_n, 1u);
+                s_pack[q] = p[c];
+                s_cell[q] = (unsigned short)(c0 + c);
+            }
         }
-    }
-    __syncthreads();
-    const int n = (int)s_n;
-    u32 band = 0, recheck = 0;
-    for (int q = tid; q < n; q += EB_BT) {
-        const int c = s_list[q];
-        const int i = bx * 8 + (c & 7), j = by * 8 + ((c >> 3) & 7), k = bz * 8 + (c >> 6);
-        CellOut o = finish_cell(mv, g, i, j, k, s_pack[c], recheck);
-        s_d[c] = o.d; s_t[c] = o.t;
-        band += o.t >= 0;
-    }
-    __syncthreads();
-    {
-        const int c0 = 4 * tid;
+        // the two halves of a row segment go out together (full 32-B sectors)
+        const bool other = __shfl_xor_sync(0xffffffffu, any ? 1 : 0, 1) != 0;     // (every lane takes part: no short circuit)
+        const bool seg = any || other;
         const int i = bx * 8 + (c0 & 7), j = by * 8 + ((c0 >> 3) & 7), k = bz * 8 + (c0 >> 6);
-        if (j < g.ny && k < g.nz) {
+        if (seg && j < g.ny && k < g.nz) {
             const size_t o = ((size_t)k * g.ny + j) * g.nx + i;
             if (g.vec4 && i + 3 < g.nx) {
-                *(float4 *)(dist + o) = *(const float4 *)(s_d + c0);
-                *(int4 *)(tri + o) = *(const int4 *)(s_t + c0);
+                *(float4 *)(dist + o) = make_float4(od[0], od[1], od[2], od[3]);
+                *(int4 *)(tri + o) = make_int4(ot[0], ot[1], ot[2], ot[3]);
             } else {
 #pragma unroll
                 for (int c = 0; c < 4; c++)
-                    if (i + c < g.nx) { dist[o + c] = s_d[c0 + c]; tri[o + c] = s_t[c0 + c]; }
+                    if (i + c < g.nx && ot[c] >= 0) { dist[o + c] = od[c]; tri[o + c] = ot[c]; }
             }
+        }
+    }
+    __syncthreads();        // the segment stores above come before the single-cell stores below
+    const int n = (int)s_n;
+    for (int q = tid; q < n; q += EB_BT) {
+        const int c = s_cell[q];
+        const int i = bx * 8 + (c & 7), j = by * 8 + ((c >> 3) & 7), k = bz * 8 + (c >> 6);
+        const CellOut o = finish_cell(mv, g, i, j, k, s_pack[q], recheck);
+        if (o.t >= 0) {
+            const size_t idx = ((size_t)k * g.ny + j) * g.nx + i;
+            dist[idx] = o.d; tri[idx] = o.t;
+            band++;
         }
     }
     if (band) atomicAdd(&s_stat[0], band);
@@ -641,13 +651,14 @@ static int fork_sentinel_fill(sdf_mesh *m, const GridParams &g, float *dist, int
     auto launch_fill = [&](cudaStream_t fs) -> int {
         stage_mark(m, SDF_T_FILL, 0, fs);
         if (vec && g.fill_mode != 1) {
-            const int iss = g.fill_issuers;
+            const int iss = g.fill_issuers | (g.fill_sm_share << 8) | (g.fill_chunk_log2 << 16);
+            const int chunk = 1 << g.fill_chunk_log2;
             CK(cudaMemsetAsync(m->fill_state, 0, sizeof(u32) * FILL_STATE_WORDS, fs));
             const unsigned nb = (unsigned)(sms * g.fill_ctas);
             // batch of chunks per fetch: 1 MiB per array on large grids, smaller when the grid has
             // fewer than ~8 batches per issuing lane
-            int64_t bq = (N / (FILL_TMA_CHUNK / 4)) / ((int64_t)sms * iss * 8);
-            const int batch = (int)(bq < 1 ? 1 : (bq > FILL_BATCH ? FILL_BATCH : bq));
+            int64_t bq = (N / (chunk / 4)) / ((int64_t)sms * g.fill_issuers * 8);
+            const int batch = (int)(bq < 1 ? 1 : (bq > FILL_BATCH_BYTES / chunk ? FILL_BATCH_BYTES / chunk : bq));
             KL;
             switch (g.fill_depth) {
             case 0: fill_tma_kernel<0><<<nb, FILL_TMA_BT, 0, fs>>>(dist, tri, N, iss, batch, m->fill_state, 0x7F800000u, 0xFFFFFFFFu); break;
@@ -982,8 +993,8 @@ int run_closest_points(sdf_mesh *m, const GridParams &g, const int *tri, float *
         CK(cudaMemsetAsync(m->cp_state, 0, sizeof(u32) * FILL_STATE_WORDS, st));
         const int64_t half = 3 * n / 2;
         int64_t bq = (half / (FILL_TMA_CHUNK / 4)) / ((int64_t)sms * 4 * 8);
-        const int batch = (int)(bq < 1 ? 1 : (bq > FILL_BATCH ? FILL_BATCH : bq));
-        KL; fill_tma_kernel<8><<<(unsigned)(sms * 4), FILL_TMA_BT, 0, st>>>(cp, (int *)(cp + half), half, 4, batch, m->cp_state,
+        const int batch = (int)(bq < 1 ? 1 : (bq > FILL_BATCH_BYTES / FILL_TMA_CHUNK ? FILL_BATCH_BYTES / FILL_TMA_CHUNK : bq));
+        KL; fill_tma_kernel<8><<<(unsigned)(sms * 4), FILL_TMA_BT, 0, st>>>(cp, (int *)(cp + half), half, 4 | (8 << 8) | (12 << 16), batch, m->cp_state,
                                                                          0x7F800000u, 0x7F800000u);
         KL; closest_points_sparse_kernel<<<(unsigned)((n / 4 + 256 * CPS_LOADS - 1) / (256 * CPS_LOADS)), 256, 0, st>>>(mv, g, tri, cp, n);
         CK(cudaGetLastError());
