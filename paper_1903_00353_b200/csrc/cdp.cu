@@ -39,6 +39,7 @@ __global__ void __launch_bounds__(CDP_BT) cdp_child_kernel(const CdpParams *__re
     one.j0 = one.j1 = (short)(H.j0 + (int)((c / ni) % nj));
     one.k0 = one.k1 = (short)(H.k0 + (int)(c / ((int64_t)ni * nj)));
     one.rows = 1;
+    one.msin = H.msin;
     u32 tested = 0, accepted = 0;
     process_direct(P->mv, P->g, p, one, P->table, P->scratch, tested, accepted);
 }

@@ -81,6 +81,7 @@ static_assert(sizeof(VertexRec) == 32, "VertexRec must be 32 B");
 // without a single cell centre inside, become a 0.6 % wider face prism.)
 #define SMOOTH_SIN_DEFAULT 0.03125f
 // sine of twice the half angle of a vertex cone from its (already widened) stored cosine, rounded up
+#define VSM_SCALE 8192.0f           // byte code of a smooth vertex' margin sine (SMOOTH_SIN_DEFAULT * VSM_SCALE = 256)
 __device__ __forceinline__ float cone_sin2(float c) {
     if (!(c > 0.9f)) return INFINITY;
     return 2.0f * c * sqrtf(fmaxf(0.0f, 1.0f - c * c)) * 1.00001f + 1e-7f;
@@ -88,11 +89,11 @@ __device__ __forceinline__ float cone_sin2(float c) {
 
 // Band- and grid-dependent bounding volume of one polyhedron in cell indices, clipped to the grid
 // (PAPER.md:348, 364, 370), and the number of grid rows (j,k) it covers.  Lives in registers only.
-struct __align__(16) PolyHdr {
+struct PolyHdr {
     short i0, i1, j0, j1, k0, k1;
     u32 rows;
+    float msin;                      // face slabs: sine of the sideways margin for the smooth features it absorbs
 };
-static_assert(sizeof(PolyHdr) == 16, "PolyHdr must be 16 B");
 
 #define BIG_ROWS 256u                // ... when it has more rows than this
 #define BIG_NI 32                    // ... or rows at least this long
@@ -146,8 +147,11 @@ struct sdf_mesh {
     int *vmint;              // [V]
     VertexRec *vrec;         // [V]
     EdgeRec *erec;           // [E] capacity; Elive records written: the wedges that exist (not flat, not absorbed)
-    float *fsm;              // [F] face margin factor: max sine of the normal-cone angle over the smooth edges /
-                             //     vertices the face absorbs; its prism is widened sideways by reach * fsm
+    float *fsm;              // [F] face margin factor: max sine of the angle between the normals over the smooth EDGES the
+                             //     face absorbs (its smooth vertices are looked up by the evaluation: evaluate.cuh
+                             //     face_margin_sin); the prism is widened sideways by reach * that sine
+    unsigned char *vsm;      // [V] smooth vertices: ceil(8192 * sine of the full cone angle) (1..255), 0 = not smooth.  What the
+                             //     evaluation looks up per face corner: a table small enough to stay in L2
     u32 *cone_list;          // [2V] capacity; NC entries (vertex id << 1 | side): the vertex cones that exist
     int64_t Elive, NC;
     u64 *d_ctr;              // [CTR_COUNT]
@@ -172,6 +176,7 @@ struct sdf_mesh {
     const GridParams *pre_g; float *pre_dist; int *pre_tri; int pre_at;
     // sdf_transform: A6a (brick marks + scan) still to be run by build_features / already run for the next run_compute
     const GridParams *hoist_g; bool bricks_ready;
+    GridParams *hoist_g_dev;          // device copy of the grid for kernels of sdf_create that mark bricks (sdf_transform)
     cudaEvent_t ev_ffork, ev_fjoin;   // fork / join of the sentinel fill (ev_fork / ev_join: the vertex stream)
 };
 
@@ -200,5 +205,6 @@ int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStr
 int start_prefill(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st);
 int maybe_prefill(sdf_mesh *m, int point, cudaStream_t st);
 int maybe_alloc_brick_ws(sdf_mesh *m, cudaStream_t st);
-int maybe_prepare_bricks(sdf_mesh *m, cudaStream_t st, cudaStream_t vs);
+int maybe_begin_bricks(sdf_mesh *m, cudaStream_t st, const GridParams **g_dev, unsigned char **flag);
+int maybe_prepare_bricks(sdf_mesh *m, cudaStream_t st, cudaStream_t vs, bool marked);
 int run_closest_points(sdf_mesh *m, const GridParams &g, const int *tri, float *cp, cudaStream_t st);

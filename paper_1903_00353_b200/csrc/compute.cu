@@ -15,62 +15,12 @@
 
 #include "evaluate.cuh"
 
-// A6a: the 8x8x8-cell bricks that can receive a distance.  Every polyhedron of a triangle, of
-// its edges and of its vertices lies inside the triangle's slab box or inside the box of one
-// of its edges grown by the reach rb, so marking those four boxes per triangle (soup + normals
-// only) covers every cell the evaluation can touch.
-__device__ __forceinline__ void mark_box(const GridParams &g, const float *mn, const float *mx,
-                                         unsigned char *__restrict__ brick_flag) {
-    int i0, i1, j0, j1, k0, k1;
-    cell_range(mn[0], mx[0], g.ox, g.inv_h, g.nx, i0, i1);
-    cell_range(mn[1], mx[1], g.oy, g.inv_h, g.ny, j0, j1);
-    cell_range(mn[2], mx[2], g.oz, g.inv_h, g.nz, k0, k1);
-    if (!(i0 <= i1 && j0 <= j1 && k0 <= k1)) return;
-    for (int bz = k0 >> 3; bz <= (k1 >> 3); bz++)
-        for (int by = j0 >> 3; by <= (j1 >> 3); by++)
-            for (int bx = i0 >> 3; bx <= (i1 >> 3); bx++) {
-                unsigned char *f = brick_flag + ((size_t)bz * g.nby + by) * g.nbx + bx;
-                if (!*f) *f = 1;            // mostly already set: a cached read, not a write
-            }
-}
-
+// A6a (evaluate.cuh mark_triangle_bricks): one thread per triangle
 __global__ void __launch_bounds__(256) brick_mark_kernel(MeshView mv, GridParams g,
                                                          unsigned char *__restrict__ brick_flag) {
     const int64_t t = (int64_t)blockIdx.x * 256 + threadIdx.x;
     if (t >= mv.F) return;
-    const float *T = mv.soup + 9 * t;
-    const float rb = g.rb, eps = g.eps;
-    float lo[3], hi[3], mn[3], mx[3];
-    float ext_max = 0.0f;
-#pragma unroll
-    for (int i = 0; i < 3; i++) {
-        lo[i] = fminf(T[i], fminf(T[3 + i], T[6 + i])); hi[i] = fmaxf(T[i], fmaxf(T[3 + i], T[6 + i]));
-        ext_max = fmaxf(ext_max, hi[i] - lo[i]);
-    }
-    if (g.aabb_mode || ext_max <= 4.0f * g.h) {
-        // small triangle: its box grown by the reach holds all four boxes and costs no extra brick
-#pragma unroll
-        for (int i = 0; i < 3; i++) { mn[i] = lo[i] - rb - eps; mx[i] = hi[i] + rb + eps; }
-        mark_box(g, mn, mx, brick_flag);
-        return;
-    }
-    const float *N = mv.fn + 3 * t;
-#pragma unroll
-    for (int i = 0; i < 3; i++) {
-        float ext = rb * fabsf(N[i]);
-        mn[i] = lo[i] - ext - eps; mx[i] = hi[i] + ext + eps;
-    }
-    mark_box(g, mn, mx, brick_flag);
-#pragma unroll
-    for (int k = 0; k < 3; k++) {
-        const float *A = T + 3 * k, *B = T + 3 * (k == 2 ? 0 : k + 1);
-#pragma unroll
-        for (int i = 0; i < 3; i++) {
-            mn[i] = fminf(A[i], B[i]) - rb - eps;
-            mx[i] = fmaxf(A[i], B[i]) + rb + eps;
-        }
-        mark_box(g, mn, mx, brick_flag);
-    }
+    mark_triangle_bricks(g, mv.soup + 9 * t, mv.fn + 3 * t, brick_flag);
 }
 
 struct BrickIn {
@@ -132,7 +82,7 @@ __device__ __forceinline__ void build_row_record(const MeshView &mv, const GridP
         rec[6] = m0.x; rec[7] = m0.y; rec[8] = m0.z; rec[9] = m1.x; rec[10] = m1.y; rec[11] = m1.z;
         rec[12] = m2.x; rec[13] = m2.y; rec[14] = m2.z;
         rec[15] = dot(m1, e0); rec[16] = dot(m2, ec);
-        const float em = eps + g.rb * mv.fsm[p];       // eps + the margin for absorbed smooth features
+        const float em = eps + g.rb * H.msin;          // eps + the margin for absorbed smooth features
         rec[17] = em * sqrtf(dot(e0, e0)); rec[18] = em * sqrtf(dot(e1, e1)); rec[19] = em * sqrtf(dot(ec, ec));
         ri[RR_ID] = mv.perm[p]; ri[RR_TYPE] = 0; ri[RR_TIDX] = (int)p;
     } else if (p < (int64_t)mv.F + mv.E) {
@@ -718,7 +668,7 @@ int maybe_prefill(sdf_mesh *m, int point, cudaStream_t st) {
 static MeshView make_view(const sdf_mesh *m) {
     MeshView mv;
     mv.soup = m->soup; mv.fn = m->fn; mv.fsm = m->fsm; mv.erec = m->erec; mv.vrec = m->vrec; mv.vmint = m->vmint;
-    mv.cone_list = m->cone_list;
+    mv.cone_list = m->cone_list; mv.vsm = m->vsm;
     mv.cvid = m->cvid; mv.adj = m->adj; mv.perm = m->perm; mv.inv_perm = m->inv_perm;
     mv.F = (int)m->F; mv.E = (int)m->Elive; mv.V = (int)m->V; mv.NC = (int)m->NC;
     mv.P = m->F + m->Elive + m->NC;
@@ -747,36 +697,58 @@ static int alloc_brick_ws(sdf_mesh *m, const GridParams &g, cudaStream_t as) {
     return SDF_OK;
 }
 
-// A6a on stream `ps` (workspace already carved): mark the bricks the band can reach, prefix sum -> brick table,
-// list and the total in d_ctr[CTR_BRICKS].  Needs the soup, the face normals and V; sdf_transform runs it on the
-// vertex stream beside the edge stage.
-static int mark_bricks(sdf_mesh *m, const GridParams &g, cudaStream_t ps) {
-    const MeshView mv = make_view(m);
+// A6a on stream `ps` (workspace already carved): reset the flags and the per-compute counters; mark the bricks the band
+// can reach (unless a kernel of sdf_create did: `marked`); prefix sum -> brick table, list and the total in
+// d_ctr[CTR_BRICKS].  Needs the soup, the face normals and V; sdf_transform runs it beside the edge stage.
+static int reset_bricks(sdf_mesh *m, const GridParams &g, cudaStream_t ps) {
     const int64_t nbricks = (int64_t)g.nbx * g.nby * g.nbz;
     m->ev_set[SDF_T_CLIP_SCAN] = false;
     CK(cudaMemsetAsync(m->brick_flag, 0, (size_t)nbricks, ps));
     CK(cudaMemsetAsync(m->d_ctr + CTR_POLY, 0, sizeof(u64) * (CTR_TOTAL - CTR_POLY), ps));
+    return SDF_OK;
+}
+static int scan_bricks(sdf_mesh *m, const GridParams &g, cudaStream_t ps, bool marked) {
+    const int64_t nbricks = (int64_t)g.nbx * g.nby * g.nbz;
     stage_mark(m, SDF_T_CLIP_SCAN, 0, ps);
-    KL; brick_mark_kernel<<<(unsigned)((mv.F + 255) / 256), 256, 0, ps>>>(mv, g, m->brick_flag);
+    if (!marked) {
+        const MeshView mv = make_view(m);
+        KL; brick_mark_kernel<<<(unsigned)((mv.F + 255) / 256), 256, 0, ps>>>(mv, g, m->brick_flag);
+    }
     CKS(launch_scan(BrickIn{m->brick_flag}, BrickOut{m->brick_table, m->brick_list}, nbricks, m->scan_ws, m->d_ctr + CTR_BRICKS, ps));
     CK(cudaGetLastError());
     return SDF_OK;
 }
 
-// sdf_transform, before build_features forks the vertex stream
+// sdf_transform, before build_features forks the vertex stream (tile builder: the marking kernel runs later)
 int maybe_alloc_brick_ws(sdf_mesh *m, cudaStream_t st) {
-    return m->hoist_g ? alloc_brick_ws(m, *m->hoist_g, st) : SDF_OK;
+    if (!m->hoist_g) return SDF_OK;
+    CKS(alloc_brick_ws(m, *m->hoist_g, st));
+    return reset_bricks(m, *m->hoist_g, st);
+}
+
+// sdf_transform, global builder: workspace + reset on `st`, and a device copy of the grid for tri_geom_kernel, which
+// marks the bricks itself
+int maybe_begin_bricks(sdf_mesh *m, cudaStream_t st, const GridParams **g_dev, unsigned char **flag) {
+    *g_dev = nullptr; *flag = nullptr;
+    if (!m->hoist_g) return SDF_OK;
+    CKS(alloc_brick_ws(m, *m->hoist_g, st));
+    CKS(reset_bricks(m, *m->hoist_g, st));
+    if (!m->hoist_g_dev) CKS(dev_alloc(&m->alloc, (void **)&m->hoist_g_dev, sizeof(GridParams), st));
+    CK(cudaMemcpyAsync(m->hoist_g_dev, m->hoist_g, sizeof(GridParams), cudaMemcpyHostToDevice, st));
+    *g_dev = m->hoist_g_dev;
+    *flag = m->brick_flag;
+    return SDF_OK;
 }
 
 // sdf_transform: stage boundary of build_features after the vertex kernels (stream vs, forked from st)
-int maybe_prepare_bricks(sdf_mesh *m, cudaStream_t st, cudaStream_t vs) {
+int maybe_prepare_bricks(sdf_mesh *m, cudaStream_t st, cudaStream_t vs, bool marked) {
     if (!m->hoist_g) return SDF_OK;
     const GridParams *g = m->hoist_g;
     m->hoist_g = nullptr;
     (void)st;
-    CKS(mark_bricks(m, *g, vs));
+    CKS(scan_bricks(m, *g, vs, marked));
     stage_mark(m, SDF_T_CLIP_SCAN, 1, vs);
-    m->bricks_ready = true;        // the total travels with the validation flags (second host crossing)
+    m->bricks_ready = true;        // the total travels with the validation flags (the host crossing)
     return SDF_OK;
 }
 
@@ -816,7 +788,8 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
         bricks = m->h_ctr[CTR_BRICKS];
     } else {
         CKS(alloc_brick_ws(m, g, st));
-        CKS(mark_bricks(m, g, st));
+        CKS(reset_bricks(m, g, st));
+        CKS(scan_bricks(m, g, st, false));
         CK(cudaMemcpyAsync(&bricks, m->d_ctr + CTR_BRICKS, sizeof(bricks), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
         stage_mark(m, SDF_T_CLIP_SCAN, 1, st);

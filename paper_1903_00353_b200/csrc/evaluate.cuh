@@ -84,6 +84,7 @@ __device__ __forceinline__ T tri_closest(V3<T> r, V3<T> e0, V3<T> ec, V3<T> n, i
 // ---------------------------------------------------------------------------------------
 struct MeshView {
     const float *soup, *fn, *fsm;
+    const unsigned char *vsm;
     const EdgeRec *erec;
     const VertexRec *vrec;
     const u32 *cone_list;
@@ -106,6 +107,68 @@ __device__ __forceinline__ void cell_range(float mn, float mx, float o, float in
     lo = (int)l; hi = (int)u;
 }
 
+// A6a: the 8x8x8-cell bricks that can receive a distance.  Every polyhedron of a triangle, of its edges and of its
+// vertices lies inside the triangle's slab box or inside the box of one of its edges grown by the reach rb, so marking
+// those four boxes per triangle (corners + normal only) covers every cell the evaluation can touch.
+__device__ __forceinline__ void mark_box(const GridParams &g, const float *mn, const float *mx,
+                                         unsigned char *__restrict__ brick_flag) {
+    int i0, i1, j0, j1, k0, k1;
+    cell_range(mn[0], mx[0], g.ox, g.inv_h, g.nx, i0, i1);
+    cell_range(mn[1], mx[1], g.oy, g.inv_h, g.ny, j0, j1);
+    cell_range(mn[2], mx[2], g.oz, g.inv_h, g.nz, k0, k1);
+    if (!(i0 <= i1 && j0 <= j1 && k0 <= k1)) return;
+    for (int bz = k0 >> 3; bz <= (k1 >> 3); bz++)
+        for (int by = j0 >> 3; by <= (j1 >> 3); by++)
+            for (int bx = i0 >> 3; bx <= (i1 >> 3); bx++) {
+                unsigned char *f = brick_flag + ((size_t)bz * g.nby + by) * g.nbx + bx;
+                if (!*f) *f = 1;            // mostly already set: a cached read, not a write
+            }
+}
+__device__ __forceinline__ void mark_triangle_bricks(const GridParams &g, const float *T, const float *N,
+                                                     unsigned char *__restrict__ brick_flag) {
+    const float rb = g.rb, eps = g.eps;
+    float lo[3], hi[3], mn[3], mx[3];
+    float ext_max = 0.0f;
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+        lo[i] = fminf(T[i], fminf(T[3 + i], T[6 + i])); hi[i] = fmaxf(T[i], fmaxf(T[3 + i], T[6 + i]));
+        ext_max = fmaxf(ext_max, hi[i] - lo[i]);
+    }
+    if (g.aabb_mode || ext_max <= 4.0f * g.h) {
+        // small triangle: its box grown by the reach holds all four boxes and costs no extra brick
+#pragma unroll
+        for (int i = 0; i < 3; i++) { mn[i] = lo[i] - rb - eps; mx[i] = hi[i] + rb + eps; }
+        mark_box(g, mn, mx, brick_flag);
+        return;
+    }
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+        float ext = rb * fabsf(N[i]);
+        mn[i] = lo[i] - ext - eps; mx[i] = hi[i] + ext + eps;
+    }
+    mark_box(g, mn, mx, brick_flag);
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const float *A = T + 3 * k, *B = T + 3 * (k == 2 ? 0 : k + 1);
+#pragma unroll
+        for (int i = 0; i < 3; i++) {
+            mn[i] = fminf(A[i], B[i]) - rb - eps;
+            mx[i] = fmaxf(A[i], B[i]) + rb + eps;
+        }
+        mark_box(g, mn, mx, brick_flag);
+    }
+}
+
+// Face slab p: sine of its sideways margin = the widest smooth edge (fsm, from the edge pass) or smooth vertex (vsm: one
+// byte per vertex, rounded up) it absorbs.  Three byte gathers per face, inside the instruction-bound evaluate kernels.
+__device__ __forceinline__ float face_margin_sin(const MeshView &mv, int64_t p) {
+    float s = mv.fsm[p];
+    u32 code = 0;
+#pragma unroll
+    for (int k = 0; k < 3; k++) code = max(code, (u32)mv.vsm[mv.cvid[3 * p + k]]);
+    return fmaxf(s, (float)code * (1.0f / VSM_SCALE));
+}
+
 // A5: bounding volume of polyhedron p in cell indices, clipped to the grid.  Returns false if
 // the polyhedron is not emitted (flat edge, one-sided vertex, skipped cone) or misses the grid.
 __device__ __forceinline__ bool poly_aabv(const MeshView &mv, const GridParams &g, int64_t p, PolyHdr &h) {
@@ -116,7 +179,8 @@ __device__ __forceinline__ bool poly_aabv(const MeshView &mv, const GridParams &
         // face slab: triangle swept by +-rb along its normal
         const float *T = mv.soup + 9 * p, *N = mv.fn + 3 * p;
         emit = !(g.disable & 1);
-        const float dl = rb * mv.fsm[p];            // sideways margin for the smooth edges / vertices it absorbs
+        h.msin = emit ? face_margin_sin(mv, p) : 0.0f;
+        const float dl = rb * h.msin;               // sideways margin for the smooth edges / vertices it absorbs
 #pragma unroll
         for (int i = 0; i < 3; i++) {
             float lo = fminf(T[i], fminf(T[3 + i], T[6 + i])), hi = fmaxf(T[i], fmaxf(T[3 + i], T[6 + i]));
@@ -177,6 +241,7 @@ __device__ __forceinline__ bool poly_aabv(const MeshView &mv, const GridParams &
         }
     }
     h.i0 = h.j0 = h.k0 = 0; h.i1 = h.j1 = h.k1 = -1; h.rows = 0;
+    if (p >= mv.F) h.msin = 0.0f;
     if (!emit) return false;
     int i0, i1, j0, j1, k0, k1;
     cell_range(mn[0], mx[0], g.ox, g.inv_h, g.nx, i0, i1);
@@ -242,7 +307,7 @@ __device__ __forceinline__ void process_direct(const MeshView &mv, const GridPar
         const f3 a = ld3(T), e0 = ld3(T + 3) - a, ec = ld3(T + 6) - a, n = ld3(N);
         const f3 e1 = ec - e0;
         const f3 m0 = cross(n, e0), m1 = cross(n, e1), m2 = cross(ec, n);          // inward, |m_i| = |edge_i|
-        const float em = eps + g.rb * mv.fsm[p];
+        const float em = eps + g.rb * H.msin;
         const float t0 = em * sqrtf(dot(e0, e0)), t1 = em * sqrtf(dot(e1, e1)), t2 = em * sqrtf(dot(ec, ec));
         const int id = mv.perm[p];
         const f3 r0 = mk<float>(fmaf((float)i0, h, g.ox) - a.x, fmaf((float)j0, h, g.oy) - a.y, fmaf((float)k0, h, g.oz) - a.z);

@@ -10,6 +10,7 @@
 // (PAPER.md:336), order-independent fixed-point atomics instead of the per-group serial
 // regrouping.
 #include "primitives.cuh"
+#include "evaluate.cuh"
 #include <math.h>
 #include <stdlib.h>
 #include <string.h>
@@ -262,7 +263,9 @@ __device__ __forceinline__ bool tri_normal64(const float *__restrict__ T, double
 __global__ void __launch_bounds__(FB, TG_MINB) tri_geom_kernel(const float *__restrict__ soup, const u32 *__restrict__ wvid,
                                                       const u32 *__restrict__ slot, int F, int *__restrict__ cvid,
                                                       float *__restrict__ fn, u64 *__restrict__ vacc,
-                                                      u32 *etab, u32 emask, int *__restrict__ flags) {
+                                                      u32 *etab, u32 emask, int *__restrict__ flags,
+                                                      const GridParams *__restrict__ mark_g,
+                                                      unsigned char *__restrict__ brick_flag) {
     int t = blockIdx.x * FB + threadIdx.x;
     if (t >= F) return;
     const float *T = soup + 9 * (size_t)t;
@@ -278,7 +281,10 @@ __global__ void __launch_bounds__(FB, TG_MINB) tri_geom_kernel(const float *__re
         atomicOr(flags, ERRB_DEGENERATE);
         n[0] = n[1] = 0.0; n[2] = 1.0;
     }
-    fn[3 * (size_t)t] = (float)n[0]; fn[3 * (size_t)t + 1] = (float)n[1]; fn[3 * (size_t)t + 2] = (float)n[2];
+    const float nf[3] = {(float)n[0], (float)n[1], (float)n[2]};
+    fn[3 * (size_t)t] = nf[0]; fn[3 * (size_t)t + 1] = nf[1]; fn[3 * (size_t)t + 2] = nf[2];
+    // sdf_transform (the grid is known already): A6a's brick marks while the corners and the normal are in registers
+    if (mark_g) mark_triangle_bricks(*mark_g, T, nf, brick_flag);
 #pragma unroll
     for (int k = 0; k < 3; k++) {
         int k1 = (k + 1) % 3, k2 = (k + 2) % 3;
@@ -503,8 +509,8 @@ __global__ void __launch_bounds__(FB) vertex_record_kernel(const float *__restri
                                                            const long long *__restrict__ vcosq,
                                                            const int *__restrict__ vside, int V,
                                                            const long long *__restrict__ vcospos, float smooth_sin,
-                                                           VertexRec *__restrict__ vrec, u32 *__restrict__ cone_list,
-                                                           u64 *__restrict__ ctr) {
+                                                           VertexRec *__restrict__ vrec, unsigned char *__restrict__ vsm,
+                                                           u32 *__restrict__ cone_list, u64 *__restrict__ ctr) {
     __shared__ u32 s_cnt[5], s_live, s_base;
     if (threadIdx.x < 5) s_cnt[threadIdx.x] = 0;
     if (threadIdx.x == 5) s_live = 0;
@@ -547,9 +553,12 @@ __global__ void __launch_bounds__(FB) vertex_record_kernel(const float *__restri
         // a cone thinner than 1e-6 rad is covered by the eps-inflated neighbours
         bool skip = !hemi && (1.0 - c) < 5e-13;
         // smooth: the whole cone of normals within asin(smooth_sin) / 2 of the axis.  No cone; the incident faces
-        // widen their prisms by reach * sin(2 theta) instead (face_margin_kernel reads it back from cos_cone)
-        if (!hemi && !noaxis && cone_sin2(cf) <= smooth_sin) skip = true;
+        // widen their prisms by reach * sin(2 theta) instead (evaluate.cuh face_margin_sin reads it back from cos_cone)
+        // (also the cones thinner than 1e-6 rad, skipped above: their margin is the smallest the byte code holds)
+        const float s2 = (hemi || noaxis) ? INFINITY : cone_sin2(cf);
+        if (s2 <= smooth_sin && s2 * VSM_SCALE <= 255.0f) skip = true;       // (the byte code must hold it, rounded up)
         if (skip) info = 8;
+        vsm[v] = skip ? (unsigned char)min(255, max(1, (int)ceilf(s2 * VSM_SCALE))) : (unsigned char)0;
         VertexRec r;
 #pragma unroll
         for (int i = 0; i < 3; i++) { r.pos[i] = P[i]; r.axis[i] = (float)N[i]; }
@@ -572,21 +581,6 @@ __global__ void __launch_bounds__(FB) vertex_record_kernel(const float *__restri
         if (sides & 2) cone_list[o] = ((u32)v << 1) | 1u;
     }
     if (threadIdx.x < 5 && s_cnt[threadIdx.x]) atomicAdd(&ctr[CTR_V_POS + threadIdx.x], (u64)s_cnt[threadIdx.x]);
-}
-
-// one thread per triangle: its prism is widened for the smooth vertices it touches (the smooth edges already raised
-// fsm in edge_record_kernel; this runs after both streams have joined)
-__global__ void __launch_bounds__(FB) face_margin_kernel(const int *__restrict__ cvid, int F,
-                                                         const VertexRec *__restrict__ vrec, float *__restrict__ fsm) {
-    int t = blockIdx.x * FB + threadIdx.x;
-    if (t >= F) return;
-    float s = fsm[t];
-#pragma unroll
-    for (int k = 0; k < 3; k++) {
-        const VertexRec &r = vrec[cvid[3 * (size_t)t + k]];
-        if (r.info & 8) s = fmaxf(s, cone_sin2(r.cos_cone));
-    }
-    fsm[t] = s;
 }
 
 // ---------------------------------------------------------------------------------------
@@ -761,6 +755,7 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
         m->vrec = c.take<VertexRec>((size_t)vcap);
         m->vmint = c.take<int>((size_t)vcap);
         m->cone_list = c.take<u32>(2 * (size_t)vcap);
+        m->vsm = c.take<unsigned char>((size_t)vcap);
         m->d_ctr = c.take<u64>(CTR_TOTAL);
         m->d_flags = c.take<int>(4);
         if (pass == 0) CKS(dev_alloc(al, &m->slab_f, c.off, st));
@@ -772,7 +767,7 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
 
     // smooth features get no polyhedron of their own (common.cuh, SMOOTH_SIN_DEFAULT); SDF_SMOOTH_SIN=0 switches that off
     float smooth_sin = SMOOTH_SIN_DEFAULT;
-    if (const char *ss = getenv("SDF_SMOOTH_SIN")) { smooth_sin = (float)atof(ss); if (!(smooth_sin >= 0.0f && smooth_sin <= 0.25f)) smooth_sin = SMOOTH_SIN_DEFAULT; }
+    if (const char *ss = getenv("SDF_SMOOTH_SIN")) { smooth_sin = (float)atof(ss); if (!(smooth_sin >= 0.0f && smooth_sin <= SMOOTH_SIN_DEFAULT)) smooth_sin = SMOOTH_SIN_DEFAULT; }
     const char *rc = getenv("SDF_RUFF");
     const bool ruff_cone = rc && !strcmp(rc, "cone");
 
@@ -820,10 +815,14 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
     // ---- A3 (per triangle), A2 edge table
     CKS(maybe_prefill(m, 2, st));
     stage_mark(m, SDF_T_EDGES, 0, st);
-    KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wvid, slot, (int)F, m->cvid, m->fn, vacc, etab, cape - 1, m->d_flags);
-    // sdf_transform: the per-compute workspace of A6a is taken in the order of `st` BEFORE the fork, so that the
-    // vertex stream (which first touches it) is ordered after the allocation
-    CKS(maybe_alloc_brick_ws(m, st));
+    // sdf_transform: A6a's workspace is taken in the order of `st` before anything touches it; tri_geom_kernel then marks
+    // the bricks as it goes and the vertex stream only runs the scan
+    const GridParams *mark_g = nullptr;
+    unsigned char *mark_flag = nullptr;
+    if (F >= ((int64_t)1 << 21)) CKS(maybe_begin_bricks(m, st, &mark_g, &mark_flag));   // (big triangles mark hundreds of bricks per thread: C5 loses 0.14 ms)
+    else CKS(maybe_alloc_brick_ws(m, st));
+    KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wvid, slot, (int)F, m->cvid, m->fn, vacc, etab, cape - 1, m->d_flags,
+                                                    mark_g, mark_flag);
     // the vertex stage needs only what tri_geom wrote: it runs on a second stream beside the edge stage
     cudaStream_t vs = st;
     CKS(fork_vertex_stream(m, st, &vs, drain));
@@ -839,17 +838,15 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
     KL; vertex_normal_kernel<<<blocks_for(vcap), FB, 0, vs>>>(vacc, vcap, m->d_ctr + CTR_V, vn64);
     KL; vertex_cone_kernel<<<blocks_for(F), FB, 0, vs>>>(m->soup, m->cvid, (int)F, vn64, vcosq, vside, m->perm, m->vmint, vcospos);
     KL; vertex_record_kernel<<<blocks_for(vcap), FB, 0, vs>>>(m->soup, vcorner, vn64, nullptr, m->d_ctr + CTR_V, vcosq, vside, vcap,
-                                                           vcospos, smooth_sin, m->vrec, m->cone_list, m->d_ctr);
+                                                           vcospos, smooth_sin, m->vrec, m->vsm, m->cone_list, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_VERTICES, 1, vs);
-    CKS(maybe_prepare_bricks(m, st, vs));
+    CKS(maybe_prepare_bricks(m, st, vs, mark_g != nullptr));
     if (vs != st) {
         CK(cudaEventRecord(m->ev_join, vs));
         CK(cudaStreamWaitEvent(st, m->ev_join, 0));
         drain.armed = false;           // joined: `st` now carries the dependency
     }
-    KL; face_margin_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, m->vrec, m->fsm);
-    CK(cudaGetLastError());
     // sdf_transform: the sentinel fill starts as soon as the feature kernels have drained, under the host crossing
     CKS(maybe_prefill(m, 4, st));
     return finish_features(m, nc, vcap, tmp, st);
@@ -884,6 +881,7 @@ static int build_features_tile(sdf_mesh *m, const float *tri, int on_device, cud
         m->vrec = c.take<VertexRec>((size_t)vcap);
         m->vmint = c.take<int>((size_t)vcap);
         m->cone_list = c.take<u32>(2 * (size_t)vcap);
+        m->vsm = c.take<unsigned char>((size_t)vcap);
         m->d_ctr = c.take<u64>(CTR_TOTAL);
         m->d_flags = c.take<int>(4);
         if (pass == 0) CKS(dev_alloc(al, &m->slab_f, c.off, st));
@@ -892,7 +890,7 @@ static int build_features_tile(sdf_mesh *m, const float *tri, int on_device, cud
     CK(cudaMemsetAsync(m->d_flags, 0, sizeof(int) * 4, st));
 
     float smooth_sin = SMOOTH_SIN_DEFAULT;
-    if (const char *ss = getenv("SDF_SMOOTH_SIN")) { smooth_sin = (float)atof(ss); if (!(smooth_sin >= 0.0f && smooth_sin <= 0.25f)) smooth_sin = SMOOTH_SIN_DEFAULT; }
+    if (const char *ss = getenv("SDF_SMOOTH_SIN")) { smooth_sin = (float)atof(ss); if (!(smooth_sin >= 0.0f && smooth_sin <= SMOOTH_SIN_DEFAULT)) smooth_sin = SMOOTH_SIN_DEFAULT; }
     const char *rc = getenv("SDF_RUFF");
     const bool ruff_cone = rc && !strcmp(rc, "cone");
 
@@ -966,17 +964,15 @@ static int build_features_tile(sdf_mesh *m, const float *tri, int on_device, cud
     stage_mark(m, SDF_T_VERTICES, 0, vs);
     KL; tile_cone_kernel<<<ntiles, TB, sizeof(TileConeSmem), vs>>>(m->soup, (int)F, m->perm, tt, vacc, vcosq, vside, m->vmint, vcospos);
     KL; vertex_record_kernel<<<blocks_for(vcap), FB, 0, vs>>>(m->soup, vcorner, nullptr, vacc, m->d_ctr + CTR_V, vcosq, vside, vcap,
-                                                           vcospos, smooth_sin, m->vrec, m->cone_list, m->d_ctr);
+                                                           vcospos, smooth_sin, m->vrec, m->vsm, m->cone_list, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_VERTICES, 1, vs);
-    CKS(maybe_prepare_bricks(m, st, vs));
+    CKS(maybe_prepare_bricks(m, st, vs, false));
     if (vs != st) {
         CK(cudaEventRecord(m->ev_join, vs));
         CK(cudaStreamWaitEvent(st, m->ev_join, 0));
         drain.armed = false;           // joined: `st` now carries the dependency
     }
-    KL; face_margin_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, m->vrec, m->fsm);
-    CK(cudaGetLastError());
     // sdf_transform: the sentinel fill starts as soon as the feature kernels have drained, under the host crossing
     CKS(maybe_prefill(m, 4, st));
     return finish_features(m, nc, vcap, tmp, st);
