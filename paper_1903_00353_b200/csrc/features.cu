@@ -115,12 +115,10 @@ __device__ __forceinline__ u32 spread3_10(u32 v) {         // 10 bits -> every t
     v = (v | (v << 2)) & 0x09249249u;
     return v;
 }
-__global__ void __launch_bounds__(FB) fine_bin_kernel(const float *__restrict__ in, int F, const int *__restrict__ bbox,
-                                                      int bits, u32 *cnt, u32 *__restrict__ key, u32 *__restrict__ ticket) {
-    int t = blockIdx.x * FB + threadIdx.x;
-    if (t >= F) return;
-    const float *p = in + 9 * (size_t)t;
+// Morton bin of a position: `bits` bits per axis over the sampled box (a function of the position alone)
+__device__ __forceinline__ u32 fine_bin_of(float x, float y, float z, const int *__restrict__ bbox, int bits) {
     const float nb = (float)(1 << bits);
+    const float p[3] = {x, y, z};
     u32 q[3];
 #pragma unroll
     for (int i = 0; i < 3; i++) {
@@ -130,7 +128,14 @@ __global__ void __launch_bounds__(FB) fine_bin_kernel(const float *__restrict__ 
         f = fminf(fmaxf(f, 0.0f), nb - 1.0f);                 // NaN -> 0; outliers -> end bins
         q[i] = (u32)f;
     }
-    const u32 k = spread3_10(q[0]) | (spread3_10(q[1]) << 1) | (spread3_10(q[2]) << 2);
+    return spread3_10(q[0]) | (spread3_10(q[1]) << 1) | (spread3_10(q[2]) << 2);
+}
+__global__ void __launch_bounds__(FB) fine_bin_kernel(const float *__restrict__ in, int F, const int *__restrict__ bbox,
+                                                      int bits, u32 *cnt, u32 *__restrict__ key, u32 *__restrict__ ticket) {
+    int t = blockIdx.x * FB + threadIdx.x;
+    if (t >= F) return;
+    const float *p = in + 9 * (size_t)t;
+    const u32 k = fine_bin_of(p[0], p[1], p[2], bbox, bits);
     key[t] = k;
     ticket[t] = atomicAdd(&cnt[k], 1u);
 }
@@ -150,6 +155,28 @@ __global__ void __launch_bounds__(FB) fine_scatter_kernel(int F, const u32 *__re
 
 __device__ __forceinline__ u32 canon_bits(float x) { return __float_as_uint(x + 0.0f); }   // -0 + +0 = +0
 
+// The global weld table, laid out along the sorted order of the triangles: the home slot of a position is the start of
+// its Morton bin in that order (the exclusive bin counts of the counting sort) scaled to the table, plus a hash over the bin's share of the table.
+// The corners of a bin, welded at about the same time, then probe one small region of the table (L2 hits instead of
+// DRAM round trips); after WTAB_LOCAL probes without success the sequence continues at the uniformly hashed position.
+struct WeldTab { u32 *tab; u32 mask; u32 scale; const u32 *base; const int *bbox; int bits; u32 nf; };
+#define WTAB_LOCAL 64
+__device__ __forceinline__ u32 wtab_home(const WeldTab &w, float x, float y, float z, u32 bx, u32 by, u32 bz) {
+    const u32 hs = mix32(bx, by, bz);
+    if (!w.scale) return hs & w.mask;
+    // the bin's region: [base[b], base[b+1]) triangles scaled to the table (~4 slots per triangle, two vertices per
+    // four triangles: load 1/8 everywhere, also in the bins at the poles of a UV mesh that hold thousands of vertices)
+    const u32 b = fine_bin_of(x, y, z, w.bbox, w.bits);
+    const u32 b0 = w.base[b], b1 = (b + 1u < (1u << (3 * w.bits))) ? w.base[b + 1u] : w.nf;
+    const u32 lo = (u32)(((u64)b0 * w.scale) >> 12), len = (u32)(((u64)(b1 - b0) * w.scale) >> 12) + 16u;
+    return (lo + (u32)(((u64)hs * len) >> 32)) & w.mask;
+}
+__device__ __forceinline__ void wtab_next(const WeldTab &w, u32 bx, u32 by, u32 bz, u32 &h, int &n) {
+    n++;
+    if (w.scale && n == WTAB_LOCAL) h = mix32(bx, by, bz) & w.mask;
+    else h = (h + 1) & w.mask;
+}
+
 // One thread per corner of the internal order: gather the corner from the caller's soup
 // (reject non-finite input, canonicalise -0 -> +0, write the internal copy), then find-or-insert
 // its vertex in the weld table (linear probing).  A slot holds a corner index of its vertex;
@@ -160,7 +187,7 @@ __device__ __forceinline__ u32 canon_bits(float x) { return __float_as_uint(x + 
 // depend on the order in which warps run; nothing that reaches the output does.)
 __global__ void __launch_bounds__(FB) ingest_weld_kernel(const float *__restrict__ in, const int *__restrict__ perm,
                                                          int ncorner, float *__restrict__ soup,
-                                                         int *__restrict__ inv_perm, u32 *wtab, u32 mask,
+                                                         int *__restrict__ inv_perm, WeldTab wt,
                                                          u32 *__restrict__ slot, u32 *__restrict__ wvid,
                                                          int *__restrict__ vcorner, u64 *__restrict__ vacc,
                                                          long long *__restrict__ vcosq, long long *__restrict__ vcospos,
@@ -182,17 +209,18 @@ __global__ void __launch_bounds__(FB) ingest_weld_kernel(const float *__restrict
         soup[3 * (size_t)c] = x; soup[3 * (size_t)c + 1] = y; soup[3 * (size_t)c + 2] = z;
         if (k == 0) inv_perm[t] = i;
         const u32 bx = __float_as_uint(x), by = __float_as_uint(y), bz = __float_as_uint(z);
-        h = mix32(bx, by, bz) & mask;
+        h = wtab_home(wt, x, y, z, bx, by, bz);
+        int np = 0;
         for (;;) {
-            u32 cur = __ldcg(wtab + h);
+            u32 cur = __ldcg(wt.tab + h);
             if (cur == EMPTY32) {
-                cur = atomicCAS(wtab + h, EMPTY32, (u32)c);
+                cur = atomicCAS(wt.tab + h, EMPTY32, (u32)c);
                 if (cur == EMPTY32) { inserted = true; break; }
             }
             const int ci = (int)cur / 3, ck = (int)cur - 3 * ci;
             const float *q = in + 9 * (size_t)perm[ci] + 3 * ck;
             if (canon_bits(q[0]) == bx && canon_bits(q[1]) == by && canon_bits(q[2]) == bz) break;
-            h = (h + 1) & mask;
+            wtab_next(wt, bx, by, bz, h, np);
         }
         slot[c] = h;
     }
@@ -232,6 +260,7 @@ __global__ void __launch_bounds__(FB) ingest_weld_kernel(const float *__restrict
 #define COSSCALE 4503599627370496.0   /* 2^52 */
 
 __device__ __forceinline__ u32 edge_hash(u32 u, u32 w) { return mix32(u, w, 0x51ED270Bu); }
+
 __device__ __forceinline__ int he_next(int he) { int k = he % 3; return he - k + (k == 2 ? 0 : k + 1); }
 
 __device__ __forceinline__ void dcross(const double *a, const double *b, double *r) {
@@ -304,124 +333,14 @@ __global__ void __launch_bounds__(FB, TG_MINB) tri_geom_kernel(const float *__re
         // check: a valid mesh has one forward half-edge per key, and a duplicate just leaves an
         // entry nobody claims, which the pair count exposes)
         if (v[k] < v[k1]) {
+            // (a table laid out along the vertex ids, so that the probes of an edge's two triangles hit L2, was measured:
+            // it halves the DRAM reads of the two edge kernels and makes them slower -- their stalls are the round
+            // trips of the L2 atomics themselves, and clustered homes lengthen the probe sequences)
             u32 h = edge_hash((u32)v[k], (u32)v[k1]) & emask;
             while (__ldcg(etab + h) != EMPTY32 || atomicCAS(etab + h, EMPTY32, (u32)(3 * t + k)) != EMPTY32)
                 h = (h + 1) & emask;
         }
     }
-}
-
-// ---------------------------------------------------------------------------------------
-// A2 edge table: every undirected edge {u < w} of a closed, consistently oriented surface is
-// traversed once forward (u -> w) and once backward.  Forward half-edges
-// are inserted into a hash table keyed by (u,w) (the slot holds the half-edge index; its key
-// is read back from cvid); backward half-edges look their partner up and claim it.
-// The mesh is valid iff the number of claimed pairs equals 3F/2.
-// ---------------------------------------------------------------------------------------
-
-// one thread per triangle; its backward half-edges claim their forward partners.  The three
-// probe chains of a thread are independent, which is what hides the L2 latency here.
-__global__ void __launch_bounds__(FB) edge_pair_kernel(const int *__restrict__ cvid, int F, u32 *etab, u32 mask,
-                                                       int *__restrict__ adj) {
-    int t = blockIdx.x * FB + threadIdx.x;
-    if (t >= F) return;
-    const u32 c[3] = {(u32)cvid[3 * (size_t)t], (u32)cvid[3 * (size_t)t + 1], (u32)cvid[3 * (size_t)t + 2]};
-    u32 h[3];
-    bool act[3];
-#pragma unroll
-    for (int k = 0; k < 3; k++) {
-        const u32 w = c[k], u = c[k == 2 ? 0 : k + 1];         // backward: w -> u with u < w
-        act[k] = u < w;
-        h[k] = edge_hash(u, w) & mask;
-    }
-    while (act[0] || act[1] || act[2]) {
-        u32 cur[3];
-#pragma unroll
-        for (int k = 0; k < 3; k++) cur[k] = act[k] ? __ldcg(etab + h[k]) : EMPTY32;
-        u32 ku[3], kw[3];
-#pragma unroll
-        for (int k = 0; k < 3; k++) {
-            if (act[k] && cur[k] == EMPTY32) act[k] = false;             // no forward partner
-            if (act[k]) {
-                const int cand = (int)(cur[k] & ~HE_MATCHED);
-                ku[k] = (u32)cvid[cand]; kw[k] = (u32)cvid[he_next(cand)];
-            }
-        }
-#pragma unroll
-        for (int k = 0; k < 3; k++) {
-            if (!act[k]) continue;
-            const u32 w = c[k], u = c[k == 2 ? 0 : k + 1];
-            if (ku[k] == u && kw[k] == w) {
-                const u32 prev = atomicOr(etab + h[k], HE_MATCHED);
-                if (!(prev & HE_MATCHED)) {                              // else: a second backward half-edge
-                    const int cand = (int)(cur[k] & ~HE_MATCHED);
-                    adj[cand] = 3 * t + k;
-                    adj[3 * t + k] = cand;
-                }
-                act[k] = false;
-            } else {
-                h[k] = (h[k] + 1) & mask;
-            }
-        }
-    }
-}
-
-// one thread per triangle; the forward half-edge of every claimed pair classifies its edge (A4) and, if the edge
-// gets a wedge, writes the band-independent wedge geometry.  Records are compact: a block counts its wedges, takes
-// a range of the table with one atomicAdd and its threads write at their ranks (the order of the records is not
-// defined and nothing depends on it).  Smooth edges are absorbed by their two faces (evaluate.cuh, SMOOTH_SIN).
-__global__ void __launch_bounds__(FB) edge_record_kernel(const int *__restrict__ cvid, int F,
-                                                         const int *__restrict__ adj,
-                                                         const float *__restrict__ soup, const float *__restrict__ fn,
-                                                         const int *__restrict__ perm, float smooth_sin,
-                                                         EdgeRec *__restrict__ erec, int E, int *__restrict__ fsm_bits,
-                                                         u64 *__restrict__ ctr) {
-    __shared__ u32 s_cnt[3], s_live, s_base;
-    if (threadIdx.x < 3) s_cnt[threadIdx.x] = 0;
-    if (threadIdx.x == 3) s_live = 0;
-    __syncthreads();
-    const int t0 = blockIdx.x * FB + threadIdx.x;
-    int cls[3] = {0, 0, 0}, rank[3] = {-1, -1, -1}, he1[3] = {-1, -1, -1};
-    if (t0 < F) {
-        const int c[3] = {cvid[3 * (size_t)t0], cvid[3 * (size_t)t0 + 1], cvid[3 * (size_t)t0 + 2]};
-#pragma unroll
-        for (int k0 = 0; k0 < 3; k0++) {
-            const int u = c[k0], w = c[k0 == 2 ? 0 : k0 + 1];
-            if (!(u < w)) continue;                      // forward half-edges only
-            he1[k0] = adj[3 * (size_t)t0 + k0];
-            if (he1[k0] < 0) continue;                   // unpaired
-            const int t1 = he1[k0] / 3;
-            const EdgeGeom g = edge_geom_of(soup + 9 * (size_t)t0 + 3 * k0, soup + 9 * (size_t)t0 + 3 * (k0 == 2 ? 0 : k0 + 1),
-                                            fn + 3 * (size_t)t0, fn + 3 * (size_t)t1);
-            int sb;
-            const int cl = edge_class_of(g, smooth_sin, &sb);
-            if (sb) {
-                if (fsm_bits[t0] < sb) atomicMax(&fsm_bits[t0], sb);
-                if (fsm_bits[t1] < sb) atomicMax(&fsm_bits[t1], sb);
-            }
-            cls[k0] = cl;
-            atomicAdd(&s_cnt[cl > 0 ? 0 : (cl < 0 ? 1 : 2)], 1u);      // knife edges count as convex
-            if (cl != 0) rank[k0] = (int)atomicAdd(&s_live, 1u);
-        }
-    }
-    __syncthreads();
-    if (threadIdx.x == 0 && s_live) s_base = (u32)atomicAdd(&ctr[CTR_ELIVE], (u64)s_live);
-    __syncthreads();
-    if (t0 < F) {
-#pragma unroll
-        for (int k0 = 0; k0 < 3; k0++) {
-            if (rank[k0] < 0) continue;
-            const u32 slot = s_base + (u32)rank[k0];
-            // the table holds 3F/2 records: pairs never outnumber that (two distinct half-edges each)
-            if (slot >= (u32)E) continue;
-            const int t1 = he1[k0] / 3;
-            const EdgeGeom g = edge_geom_of(soup + 9 * (size_t)t0 + 3 * k0, soup + 9 * (size_t)t0 + 3 * (k0 == 2 ? 0 : k0 + 1),
-                                            fn + 3 * (size_t)t0, fn + 3 * (size_t)t1);
-            const int x0 = perm[t0], x1 = perm[t1];
-            edge_record_write(erec + slot, g, x0 < x1 ? x0 : x1, cls[k0]);
-        }
-    }
-    if (threadIdx.x < 3 && s_cnt[threadIdx.x]) atomicAdd(&ctr[CTR_E_CONVEX + threadIdx.x], (u64)s_cnt[threadIdx.x]);
 }
 
 // ---- exact classification of an invalid edge table (error path only): sort the (min,max)
@@ -808,7 +727,12 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
     }
     CK(cudaMemsetAsync(wtab, 0xFF, (size_t)((char *)(etab + cape) - (char *)wtab), st));
     CKS(order_triangles(src, F, ow, (u32 *)m->perm, st));
-    KL; ingest_weld_kernel<<<blocks_for(nc), FB, 0, st>>>(src, m->perm, nc, m->soup, m->inv_perm, wtab, capw - 1, slot, wvid, vcorner,
+    WeldTab wt = {wtab, capw - 1, 0u, ow.cnt, ow.bbox, ow.bits, (u32)F};
+    {
+        const char *ul = getenv("SDF_UNIFORM_TABLES");
+        if (ow.on && !(ul && ul[0] == '1') && capw >= 4096) wt.scale = (u32)((((u64)capw - 1024) << 12) / (u64)F);
+    }
+    KL; ingest_weld_kernel<<<blocks_for(nc), FB, 0, st>>>(src, m->perm, nc, m->soup, m->inv_perm, wt, slot, wvid, vcorner,
                                                         vacc, vcosq, vcospos, vside, m->vmint, vcap, m->d_ctr, m->d_flags);
     stage_mark(m, SDF_T_INGEST_WELD, 1, st);
 
