@@ -306,7 +306,9 @@ __global__ void __launch_bounds__(FB, TG_MINB) tri_geom_kernel(const float *__re
     }
     double n[3], p[3][3];
     bool ok = tri_normal64(T, n, p);
-    if (!ok || v[0] == v[1] || v[1] == v[2] || v[2] == v[0]) {   // PAPER.md:137 "we disallow faces of zero area"
+    // PAPER.md:137 "we disallow faces of zero area".  (A repeated vertex IS a zero area, exactly: equal corners give a zero
+    // cross product.  The ids are not consulted: past the capacity of the vertex tables they are clamped.)
+    if (!ok) {
         atomicOr(flags, ERRB_DEGENERATE);
         n[0] = n[1] = 0.0; n[2] = 1.0;
     }

@@ -300,7 +300,7 @@ __global__ void __launch_bounds__(TB, 3) tile_geom_kernel(const float *__restric
         const int lv3[3] = {S.lv[3 * i], S.lv[3 * i + 1], S.lv[3 * i + 2]};
         double n[3], p[3][3];
         bool ok = tri_normal64(&S.pos[9 * i], n, p);
-        if (!ok || lv3[0] == lv3[1] || lv3[1] == lv3[2] || lv3[2] == lv3[0]) {      // PAPER.md:137 "we disallow faces of zero area"
+        if (!ok) {      // PAPER.md:137 "we disallow faces of zero area" (a repeated vertex is one, exactly)
             atomicOr(flags, ERRB_DEGENERATE);
             n[0] = n[1] = 0.0; n[2] = 1.0;
         }

@@ -90,3 +90,16 @@ def test_binding_fails_loudly_without_cuda():
     from paper_1903_00353_b200 import binding as B
     with pytest.raises(RuntimeError):
         B.sdf_create(np.zeros((4, 3, 3), dtype=np.float32))
+
+
+def test_bench_reads_kernel_traffic_from_profiles():
+    """bench.py takes roofline.traffic from the committed ncu summary (profiles/kernel_traffic.csv), not from a
+    literal: the file must exist, parse, and hold the dense writer at the headline config."""
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("bench_mod", os.path.join(ROOT, "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    t, src = bench.kernel_traffic("C4", "fill_tma_kernel")
+    assert t is not None and 8.4e9 < t < 9.0e9 and src.startswith("profiles/kernel_traffic.csv")
+    assert bench.kernel_traffic("C4", "no_such_kernel") == (None, None)
+    assert set(bench.STAGE_KERNEL) == {"ingest_weld", "edges", "vertices", "clip_scan", "clear", "evaluate", "emit", "fill"}

@@ -449,3 +449,66 @@ def test_aabb_candidates_mode_meets_the_four_clauses(oracle_mod, monkeypatch, na
     pop = torch.isfinite(d0)
     assert torch.equal(pop, torch.isfinite(d1)) and torch.equal(torch.signbit(d0[pop]), torch.signbit(d1[pop]))
     assert float((d0[pop] - d1[pop]).abs().max()) <= 2e-7
+
+
+@pytest.mark.parametrize("name,scale", [("C4", 0.12), ("C2", 0.5), ("C3", 0.25)])
+def test_smooth_features_absorbed_by_their_faces(oracle_mod, monkeypatch, name, scale):
+    """Edges / vertices whose normals span less than asin(1/32) get no wedge / cone of their own: the incident face
+    prisms are widened by reach * sin(angle) and evaluate the clamped triangle distance there (DESIGN.md "smooth
+    features").  With the switch off (SDF_SMOOTH_SIN=0) every non-flat feature has its polyhedron as in the paper
+    (PAPER.md:352-364).  Both must meet the four clauses; the populated sets, signs and ids-up-to-ties are those of the
+    oracle either way, and on a smooth mesh the absorbed variant scan-converts far fewer polyhedra."""
+    import torch
+    from paper_1903_00353_b200 import binding as B
+    w = f32_grid(W.config(name, scale))
+    res1 = check_parity(w, oracle_mod)
+    _assert_ok(res1)
+    m1, d1, t1 = B.compute_workload(w)
+    monkeypatch.setenv("SDF_SMOOTH_SIN", "0")
+    res0 = check_parity(w, oracle_mod)
+    m0, d0, t0 = B.compute_workload(w)
+    monkeypatch.delenv("SDF_SMOOTH_SIN")
+    _assert_ok(res0)
+    s0, s1 = res0["stats"], res1["stats"]
+    assert res0["populated_gpu"] == res1["populated_gpu"]
+    assert s1["polyhedra"] <= s0["polyhedra"] and s1["edges_flat"] >= s0["edges_flat"] and s1["verts_skipped"] >= s0["verts_skipped"]
+    if name == "C4":
+        assert s1["polyhedra"] < 0.85 * s0["polyhedra"]         # (at full size the star surface is smooth almost everywhere: 3.9 M of 9.5 M)
+    pop = torch.isfinite(d0)
+    assert torch.equal(pop, torch.isfinite(d1)) and torch.equal(torch.signbit(d0[pop]), torch.signbit(d1[pop]))
+    assert float((d0[pop] - d1[pop]).abs().max()) <= 2e-7       # same distances to an ulp of the coordinates
+
+
+def test_more_vertices_than_a_closed_surface_can_have(oracle_mod):
+    """The per-vertex tables are sized by V <= 3F/2 (every vertex of a closed surface has at least two corners), so
+    sdf_create needs no host crossing for the count.  A soup that breaks the bound -- disjoint triangles: V = 3F -- must
+    come back SDF_ENOTCLOSED (the oracle's status) without touching memory it does not own, through both builders."""
+    import os
+    import torch
+    from paper_1903_00353_b200 import binding as B
+    r = np.random.default_rng(99)
+    for F in (7, 300, 5000, 200000):
+        base = r.uniform(-0.8, 0.8, (F, 1, 3))
+        soup = np.ascontiguousarray((base + r.uniform(-0.01, 0.01, (F, 3, 3))).astype(np.float32))
+        if F <= 5000:
+            with pytest.raises(oracle_mod.OracleError) as eo:
+                oracle_mod.Mesh(soup)
+            assert eo.value.status == 2
+        for builder in ("", "tile"):
+            os.environ["SDF_BUILDER"] = builder
+            try:
+                with pytest.raises(B.SdfError) as e:
+                    B.sdf_create(torch.from_numpy(soup).cuda())
+                assert e.value.status == B.SDF_ENOTCLOSED, (F, builder)
+            finally:
+                del os.environ["SDF_BUILDER"]
+    # the library is intact afterwards
+    _assert_ok(check_parity(f32_grid(W.config("C1")), oracle_mod))
+
+
+def test_fp32_peak_microbenchmark():
+    """sdf_measure_fp32_peak (the FP32 leg of north_star's roofline): a B200 does 148 SMs x 128 FMA x 2 x 1.965 GHz =
+    74.4 TFLOP/s nominally; the FMA loop must land in that neighbourhood (clocks may sit a little lower)."""
+    from paper_1903_00353_b200 import binding as B
+    tf, sms = B.sdf_measure_fp32_peak()
+    assert sms > 0 and 0.5 * sms * 128 * 2 * 1.0e9 / 1e12 < tf < sms * 128 * 2 * 2.3e9 / 1e12, (tf, sms)
