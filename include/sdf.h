@@ -203,6 +203,34 @@ int sdf_compute_host(sdf_mesh *m, const float origin[3], float h, int nx, int ny
                      float band, float *dist_out_host, int32_t *tri_out_host, void *stream);
 
 /*
+ * sdf_compute_sparse / sdf_compute_sparse_host -- the same narrow band in band-sparse storage: only the 8x8x8-cell
+ * bricks the band can reach are stored (at C4: 43,350 of 2,097,152 bricks, 178 MB instead of 8.6 GB), the way level-set
+ * codes keep a band (PAPER.md:392 writes a distance only inside the band; PAPER.md:493 names the dense grid as the limit
+ * of the method's reach).  Identical values to sdf_compute, cell for cell (tests/test_gpu_sparse.py); no dense grid is
+ * allocated, filled or copied.
+ *
+ *   origin, h, nx, ny, nz, band   as for sdf_compute
+ *   brick_cap     capacity of the three outputs, in bricks (0 is allowed: the call then only counts)
+ *   brick_ids     int32 [brick_cap]: linear index (bz * nby + by) * nbx + bx of each stored brick, ascending, with
+ *                 nbx = ceil(nx / 8) etc.; brick (bx,by,bz) holds the cells 8*bx .. 8*bx+7 (clipped to the grid) etc.
+ *   dist_bricks   float [brick_cap][512]: cell (i,j,k) of its brick at [(k & 7) * 64 + (j & 7) * 8 + (i & 7)]; signed
+ *                 distance, +INFINITY where |d| >= band or the cell lies outside the grid; 16-byte aligned
+ *   tri_bricks    int32 [brick_cap][512]: closest triangle id, -1 where dist is +INFINITY; 16-byte aligned
+ *   nbricks_out   HOST: the number of bricks the band reaches.  If it exceeds brick_cap nothing is written and the call
+ *                 returns SDF_ENOMEM: call again with at least that capacity (the count costs A6a only, not the evaluation)
+ *   stream        cudaStream_t; synchronised once mid-way (the brick count), like sdf_compute
+ * sdf_compute_sparse: outputs in DEVICE memory, left enqueued on `stream`.  sdf_compute_sparse_host: outputs in HOST
+ * memory (pinned recommended): staged on the device through the allocator, copied back (only *nbricks_out bricks) and
+ * the stream synchronised before returning.
+ * Errors: SDF_EINVAL, SDF_ENOMEM (also: brick_cap too small), SDF_ECUDA.
+ */
+int sdf_compute_sparse(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz, float band, int64_t brick_cap,
+                       int32_t *brick_ids, float *dist_bricks, int32_t *tri_bricks, int64_t *nbricks_out, void *stream);
+int sdf_compute_sparse_host(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz, float band,
+                            int64_t brick_cap, int32_t *brick_ids_host, float *dist_bricks_host, int32_t *tri_bricks_host,
+                            int64_t *nbricks_out, void *stream);
+
+/*
  * sdf_closest_points -- the closest point transform proper: for every cell whose
  * closest-triangle id (as written by sdf_compute on the same grid) is >= 0, the point of that
  * triangle nearest to the cell centre; +INFINITY in all three components elsewhere.

@@ -22,7 +22,7 @@ SDF_OK, SDF_EINVAL, SDF_ENOTCLOSED, SDF_EORIENT, SDF_EDEGENERATE, SDF_ENOMEM, SD
 TABLE_CORNER_VID, TABLE_HALFEDGE_ADJ, TABLE_FACE_NORMAL, TABLE_VERTEX_REC, TABLE_EDGE_REC, \
     TABLE_VERTEX_MINTRI = range(6)
 
-EXPORTS = ("sdf_create", "sdf_transform", "sdf_compute", "sdf_compute_host", "sdf_zslab", "sdf_compute_zslab", "sdf_fill_interior", "sdf_closest_points", "sdf_stats", "sdf_get_table",
+EXPORTS = ("sdf_create", "sdf_transform", "sdf_compute", "sdf_compute_host", "sdf_compute_sparse", "sdf_compute_sparse_host", "sdf_zslab", "sdf_compute_zslab", "sdf_fill_interior", "sdf_closest_points", "sdf_stats", "sdf_get_table",
            "sdf_destroy", "sdf_strerror", "sdf_last_cuda_error", "sdf_version",
            "sdf_enable_timing", "sdf_get_timings", "sdf_launch_count", "sdf_measure_fp32_peak",
            "sdf_read_stl", "sdf_free_host", "sdf_write_stl", "sdf_write_grid")
@@ -93,6 +93,11 @@ def lib():
     L.sdf_transform.argtypes = [vp, C.c_int64, C.c_int, C.POINTER(_Allocator), C.POINTER(C.c_float), C.c_float, C.c_int, C.c_int,
                                 C.c_int, C.c_float, vp, vp, vp, C.POINTER(vp)]
     L.sdf_transform.restype = C.c_int
+    L.sdf_compute_sparse.argtypes = [vp, C.POINTER(C.c_float), C.c_float, C.c_int, C.c_int, C.c_int, C.c_float, C.c_int64, vp, vp, vp,
+                                     C.POINTER(C.c_int64), vp]
+    L.sdf_compute_sparse.restype = C.c_int
+    L.sdf_compute_sparse_host.argtypes = L.sdf_compute_sparse.argtypes
+    L.sdf_compute_sparse_host.restype = C.c_int
     L.sdf_zslab.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.sdf_zslab.restype = C.c_int
     L.sdf_compute_zslab.argtypes = [vp, C.POINTER(C.c_float), C.c_float, C.c_int, C.c_int, C.c_int, C.c_float, C.c_int, C.c_int,
@@ -425,6 +430,47 @@ def sdf_get_table(mesh: Mesh, which: int) -> np.ndarray:
     if st != SDF_OK:
         raise SdfError(st, "sdf_get_table")
     return out
+
+
+def sdf_brick_count(mesh: Mesh, origin, h, dims, band, stream=None) -> int:
+    """Number of 8x8x8 bricks the band reaches on this grid (sdf_compute_sparse with capacity 0: counts, writes nothing)."""
+    _torch()
+    o = (C.c_float * 3)(*[float(v) for v in origin])
+    n = C.c_int64(0)
+    st = lib().sdf_compute_sparse(mesh.handle, o, float(h), int(dims[0]), int(dims[1]), int(dims[2]), float(band), 0, None, None,
+                                  None, C.byref(n), C.c_void_p(_stream_ptr(stream)))
+    if st not in (SDF_OK, SDF_ENOMEM):
+        raise SdfError(st, "sdf_compute_sparse")
+    return int(n.value)
+
+
+def sdf_compute_sparse(mesh: Mesh, origin, h, dims, band, brick_ids=None, dist_bricks=None, tri_bricks=None, stream=None):
+    """Band-sparse output: (n, brick_ids int32[cap], dist_bricks float32[cap,512], tri_bricks int32[cap,512]).  Device tensors
+    (allocated here for the exact count if not given) or pinned / plain CPU tensors (then the library stages and copies)."""
+    torch = _torch()
+    if dist_bricks is None:
+        cap = sdf_brick_count(mesh, origin, h, dims, band, stream=stream)
+        brick_ids = torch.empty((max(cap, 1),), dtype=torch.int32, device="cuda")
+        dist_bricks = torch.empty((max(cap, 1), 512), dtype=torch.float32, device="cuda")
+        tri_bricks = torch.empty((max(cap, 1), 512), dtype=torch.int32, device="cuda")
+    cap = int(dist_bricks.shape[0])
+    if not (brick_ids.dtype == torch.int32 and dist_bricks.dtype == torch.float32 and tri_bricks.dtype == torch.int32):
+        raise TypeError("brick_ids / tri_bricks must be int32, dist_bricks float32")
+    if not (brick_ids.is_contiguous() and dist_bricks.is_contiguous() and tri_bricks.is_contiguous()):
+        raise ValueError("outputs must be contiguous")
+    if brick_ids.numel() < cap or tri_bricks.shape != dist_bricks.shape or dist_bricks.shape[1] != 512:
+        raise ValueError("outputs must be [cap], [cap,512], [cap,512]")
+    on_dev = dist_bricks.is_cuda
+    if brick_ids.is_cuda != on_dev or tri_bricks.is_cuda != on_dev:
+        raise ValueError("outputs must live on the same side")
+    o = (C.c_float * 3)(*[float(v) for v in origin])
+    n = C.c_int64(0)
+    fn = lib().sdf_compute_sparse if on_dev else lib().sdf_compute_sparse_host
+    st = fn(mesh.handle, o, float(h), int(dims[0]), int(dims[1]), int(dims[2]), float(band), cap, C.c_void_p(brick_ids.data_ptr()),
+            C.c_void_p(dist_bricks.data_ptr()), C.c_void_p(tri_bricks.data_ptr()), C.byref(n), C.c_void_p(_stream_ptr(stream)))
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_compute_sparse")
+    return int(n.value), brick_ids, dist_bricks, tri_bricks
 
 
 def sdf_measure_fp32_peak(stream=None):

@@ -300,6 +300,57 @@ int sdf_compute_host(sdf_mesh *m, const float origin[3], float h, int nx, int ny
     return s;
 }
 
+int sdf_compute_sparse(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz, float band, int64_t brick_cap,
+                       int32_t *brick_ids, float *dist_bricks, int32_t *tri_bricks, int64_t *nbricks_out, void *stream) {
+    if (nbricks_out) *nbricks_out = 0;
+    if (!m || !nbricks_out || brick_cap < 0) return SDF_EINVAL;
+    if (brick_cap > 0 && (!brick_ids || !dist_bricks || !tri_bricks)) return SDF_EINVAL;
+    if (((uintptr_t)dist_bricks & 15) || ((uintptr_t)tri_bricks & 15)) return SDF_EINVAL;
+    GridParams g;
+    CKS(make_grid(origin, h, nx, ny, nz, band, nullptr, nullptr, &g));
+    SparseOut sp = {brick_cap, brick_ids, dist_bricks, tri_bricks, 0};
+    const int s = run_compute(m, g, nullptr, nullptr, (cudaStream_t)stream, false, &sp);
+    *nbricks_out = sp.count;
+    return s;
+}
+
+int sdf_compute_sparse_host(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int nz, float band,
+                            int64_t brick_cap, int32_t *brick_ids_host, float *dist_bricks_host, int32_t *tri_bricks_host,
+                            int64_t *nbricks_out, void *stream) {
+    if (nbricks_out) *nbricks_out = 0;
+    if (!m || !nbricks_out || brick_cap < 0) return SDF_EINVAL;
+    if (brick_cap > 0 && (!brick_ids_host || !dist_bricks_host || !tri_bricks_host)) return SDF_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    GridParams g;
+    CKS(make_grid(origin, h, nx, ny, nz, band, nullptr, nullptr, &g));
+    // device staging for brick_cap bricks: ids, distances, triangle ids in one block
+    const size_t cap = (size_t)(brick_cap > 0 ? brick_cap : 0);
+    void *blk = nullptr;
+    Carver c(nullptr);
+    c.take<float>(cap * BRICK_CELLS); c.take<int>(cap * BRICK_CELLS); c.take<int>(cap + 1);
+    int s = dev_alloc(&m->alloc, &blk, c.off, st);
+    if (s != SDF_OK) return s;
+    Carver d(blk);
+    float *dd = d.take<float>(cap * BRICK_CELLS);
+    int *dt = d.take<int>(cap * BRICK_CELLS);
+    int *di = d.take<int>(cap + 1);
+    SparseOut sp = {brick_cap, di, dd, dt, 0};
+    s = run_compute(m, g, nullptr, nullptr, st, false, &sp);
+    *nbricks_out = sp.count;
+    if (s == SDF_OK && sp.count > 0) {
+        const size_t n = (size_t)sp.count;
+        cudaError_t e = cudaMemcpyAsync(brick_ids_host, di, n * sizeof(int), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(dist_bricks_host, dd, n * BRICK_CELLS * sizeof(float), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(tri_bricks_host, dt, n * BRICK_CELLS * sizeof(int), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { g_last_cuda_error = (int)e; (void)cudaGetLastError(); s = SDF_ECUDA; }
+    } else if (s == SDF_OK) {
+        cudaStreamSynchronize(st);
+    }
+    dev_free(&m->alloc, blk, st);
+    return s;
+}
+
 int sdf_stats(sdf_mesh *m, sdf_stats_t *o) {
     if (!m || !o) return SDF_EINVAL;
     CK(cudaStreamSynchronize(m->last_stream));

@@ -201,7 +201,10 @@ void stage_mark(sdf_mesh *m, int stage, int which, cudaStream_t st);
 
 // stages (features.cu / compute.cu)
 int build_features(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st);
-int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st, bool prefilled = false);
+// band-sparse output of run_compute (sdf_compute_sparse): bricks instead of dense grids
+struct SparseOut { int64_t cap; int *ids; float *dist; int *tri; int64_t count; };
+int run_compute(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st, bool prefilled = false,
+                SparseOut *sp = nullptr);
 int start_prefill(sdf_mesh *m, const GridParams &g, float *dist, int *tri, cudaStream_t st);
 int maybe_prefill(sdf_mesh *m, int point, cudaStream_t st);
 int maybe_alloc_brick_ws(sdf_mesh *m, cudaStream_t st);

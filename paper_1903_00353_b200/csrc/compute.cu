@@ -497,7 +497,10 @@ __device__ __forceinline__ CellOut finish_cell(const MeshView &mv, const GridPar
 // test is clear is unpacked on the spot; the others (a few per cent) are queued in shared memory and spread over the
 // threads afterwards -- the sign pass is the expensive, divergent part.  Only row segments that hold a populated
 // cell are written: the sentinel fill has been there before.
+// SPARSE: the brick goes out whole (sentinels included) at its slot of a band-sparse output, [slot][512] cells in the
+// scratch's own order (k&7, j&7, i&7; x fastest) -- sdf_compute_sparse; no dense grid, no sentinel fill.
 #define EB_BT 128
+template <bool SPARSE>
 __global__ void __launch_bounds__(EB_BT, 12) emit_bricks_kernel(MeshView mv, GridParams g, const int *__restrict__ list,
                                                             const u64 *__restrict__ scratch,
                                                             float *__restrict__ dist, int *__restrict__ tri,
@@ -542,7 +545,11 @@ __global__ void __launch_bounds__(EB_BT, 12) emit_bricks_kernel(MeshView mv, Gri
         const bool other = __shfl_xor_sync(0xffffffffu, any ? 1 : 0, 1) != 0;     // (every lane takes part: no short circuit)
         const bool seg = any || other;
         const int i = bx * 8 + (c0 & 7), j = by * 8 + ((c0 >> 3) & 7), k = bz * 8 + (c0 >> 6);
-        if (seg && j < g.ny && k < g.nz) {
+        if (SPARSE) {
+            const size_t o = (size_t)slot * BRICK_CELLS + c0;
+            *(float4 *)(dist + o) = make_float4(od[0], od[1], od[2], od[3]);
+            *(int4 *)(tri + o) = make_int4(ot[0], ot[1], ot[2], ot[3]);
+        } else if (seg && j < g.ny && k < g.nz) {
             const size_t o = ((size_t)k * g.ny + j) * g.nx + i;
             if (g.vec4 && i + 3 < g.nx) {
                 *(float4 *)(dist + o) = make_float4(od[0], od[1], od[2], od[3]);
@@ -561,7 +568,7 @@ __global__ void __launch_bounds__(EB_BT, 12) emit_bricks_kernel(MeshView mv, Gri
         const int i = bx * 8 + (c & 7), j = by * 8 + ((c >> 3) & 7), k = bz * 8 + (c >> 6);
         const CellOut o = finish_cell(mv, g, i, j, k, s_pack[q], recheck);
         if (o.t >= 0) {
-            const size_t idx = ((size_t)k * g.ny + j) * g.nx + i;
+            const size_t idx = SPARSE ? (size_t)slot * BRICK_CELLS + c : ((size_t)k * g.ny + j) * g.nx + i;
             dist[idx] = o.d; tri[idx] = o.t;
             band++;
         }
@@ -752,7 +759,7 @@ int maybe_prepare_bricks(sdf_mesh *m, cudaStream_t st, cudaStream_t vs, bool mar
     return SDF_OK;
 }
 
-int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cudaStream_t st, bool prefilled) {
+int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cudaStream_t st, bool prefilled, SparseOut *sp) {
     GridParams g = g_in;
     {
         // a mesh with few polyhedra cannot fill the GPU with one lane per polyhedron: hand more
@@ -774,7 +781,8 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
         if (!(prefilled && i == SDF_T_FILL)) m->ev_set[i] = false;
     // the fill is forked here (or, fill_mode 4, after the host crossing below) unless sdf_transform
     // already started it ahead of the feature construction
-    const bool forked = prefilled || g.fill_mode < 2 || g.fill_mode == 4;
+    if (sp) g.fill_mode = 5;                       // band-sparse output: no dense grid to fill
+    const bool forked = !sp && (prefilled || g.fill_mode < 2 || g.fill_mode == 4);
     auto fork_fill = [&]() -> int { return fork_sentinel_fill(m, g, dist, tri, st, true); };
     auto launch_fill = [&](cudaStream_t fs) -> int { return fork_sentinel_fill(m, g, dist, tri, fs, false); };
     if (prefilled) {}
@@ -797,6 +805,15 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
     // fork the fill first: its CTAs claim their SMs while the GPU is still empty (the scratch
     // allocation and its clear come next), before the evaluate blocks flood it
     if (g.fill_mode == 4 && !prefilled) CKS(fork_fill());
+    if (sp) {
+        sp->count = (int64_t)bricks;
+        m->h_ctr[CTR_BRICKS] = bricks;
+        m->last_bricks_total = nbricks;
+        m->last_stream = st;
+        if ((int64_t)bricks > sp->cap) return SDF_ENOMEM;          // the caller learns the count and comes back
+        dist = sp->dist; tri = sp->tri;
+        if (bricks) CK(cudaMemcpyAsync(sp->ids, m->brick_list, sizeof(int) * (size_t)bricks, cudaMemcpyDeviceToDevice, st));
+    }
     CKS(ensure(m, &m->scratch, &m->scratch_cap, (size_t)(bricks ? bricks : 1) * BRICK_CELLS, st));
     stage_mark(m, SDF_T_CLEAR, 0, st);
     if (bricks) CK(cudaMemsetAsync(m->scratch, 0xFF, (size_t)bricks * BRICK_CELLS * sizeof(u64), st));
@@ -824,7 +841,9 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
     else if (g.fill_mode == 2) CKS(launch_fill(st));
     if (bricks) {
         stage_mark(m, SDF_T_EMIT, 0, st);
-        KL; emit_bricks_kernel<<<(unsigned)bricks, EB_BT, 0, st>>>(mv, g, m->brick_list, m->scratch, dist, tri, m->d_ctr);
+        KL;
+        if (sp) emit_bricks_kernel<true><<<(unsigned)bricks, EB_BT, 0, st>>>(mv, g, m->brick_list, m->scratch, dist, tri, m->d_ctr);
+        else emit_bricks_kernel<false><<<(unsigned)bricks, EB_BT, 0, st>>>(mv, g, m->brick_list, m->scratch, dist, tri, m->d_ctr);
         stage_mark(m, SDF_T_EMIT, 1, st);
     }
     CK(cudaGetLastError());
