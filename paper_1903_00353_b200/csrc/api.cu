@@ -181,6 +181,8 @@ static int make_grid(const float origin[3], float h, int nx, int ny, int nz, flo
     g->fill_depth = fd ? atoi(fd) : 8;
     g->fill_issuers = fi ? atoi(fi) : 4;
     if (g->fill_issuers < 1 || g->fill_issuers > 4) g->fill_issuers = 4;
+    const char *sh = getenv("SDF_SCRATCH_HINT");
+    g->scratch_hint = (sh && sh[0] == '0') ? 0 : 1;
     const char *fck = getenv("SDF_FILL_CHUNK_LOG2");
     g->fill_chunk_log2 = fck ? atoi(fck) : 12;
     if (g->fill_chunk_log2 < 11 || g->fill_chunk_log2 > 14) g->fill_chunk_log2 = 12;

@@ -122,6 +122,7 @@ struct GridParams {
     int fill_prio;                  // side stream at the highest priority
     int fill_ctas;                  // TMA fill: CTAs launched per SM (one per SM survives)
     int fill_depth, fill_issuers;   // TMA fill: chunk pairs in flight per issuing lane, issuing lanes per SM
+    int scratch_hint;               // L2 evict-last hint on the scratch atomics (default on)
     int fill_chunk_log2;            // TMA fill: log2 of the bytes per bulk copy (11..14)
     int fill_sm_share;              // TMA fill: SMs out of every 8 that stream (8 = all; fewer = throttled, ablation)
 };

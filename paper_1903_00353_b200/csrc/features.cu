@@ -71,33 +71,6 @@ __global__ void __launch_bounds__(FB) bbox_sample_kernel(const float *__restrict
     }
 }
 
-__device__ __forceinline__ u32 spread3(u32 v) {           // 5 bits -> every third bit
-    v &= 31u;
-    v = (v | (v << 8)) & 0x100Fu;
-    v = (v | (v << 4)) & 0x10C3u;
-    v = (v | (v << 2)) & 0x1249u;
-    return v;
-}
-
-// 15-bit Morton key of the first corner (32 bins per axis over the sampled box)
-__global__ void __launch_bounds__(FB) bin_key_kernel(const float *__restrict__ in, int F, const int *__restrict__ bbox,
-                                                     u32 *__restrict__ keys, u32 *__restrict__ vals) {
-    int t = blockIdx.x * FB + threadIdx.x;
-    if (t >= F) return;
-    const float *p = in + 9 * (size_t)t;
-    u32 q[3];
-#pragma unroll
-    for (int i = 0; i < 3; i++) {
-        const float lo = ord2f(bbox[i]), hi = ord2f(bbox[3 + i]);
-        const float w = hi - lo;
-        float f = (w > 0.0f && isfinite(w)) ? (p[i] - lo) / w * 32.0f : 0.0f;
-        f = fminf(fmaxf(f, 0.0f), 31.0f);                 // NaN -> 0; outliers -> end bins
-        q[i] = (u32)f;
-    }
-    keys[t] = spread3(q[0]) | (spread3(q[1]) << 1) | (spread3(q[2]) << 2);
-    vals[t] = (u32)t;
-}
-
 __global__ void __launch_bounds__(FB) identity_perm_kernel(int F, u32 *__restrict__ perm) {
     int t = blockIdx.x * FB + threadIdx.x;
     if (t < F) perm[t] = (u32)t;
