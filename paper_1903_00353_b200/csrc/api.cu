@@ -360,11 +360,12 @@ int sdf_stats(sdf_mesh *m, sdf_stats_t *o) {
     CK(cudaMemcpy(all, m->d_ctr, sizeof(u64) * CTR_TOTAL, cudaMemcpyDeviceToHost));
     memcpy(m->h_ctr, all, sizeof(u64) * CTR_COUNT);
     u64 *c = m->h_ctr;
-    c[CTR_POLY] = c[CTR_TESTED] = c[CTR_ACCEPTED] = c[CTR_ITEMS] = 0;
+    c[CTR_POLY] = c[CTR_TESTED] = c[CTR_ACCEPTED] = c[CTR_ITEMS] = c[CTR_BAND] = c[CTR_RECHECK] = 0;
     for (int s = 0; s < CTR_SLOTS; s++) {
         const u64 *q = all + CTR_SPREAD + s * 8;
         c[CTR_POLY] += q[SP_POLY]; c[CTR_TESTED] += q[SP_TESTED];
         c[CTR_ACCEPTED] += q[SP_ACCEPTED]; c[CTR_ITEMS] += q[SP_ROWS];
+        c[CTR_BAND] += q[SP_BAND]; c[CTR_RECHECK] += q[SP_RECHECK];
     }
     memset(o, 0, sizeof(*o));
     o->F = m->F; o->V = m->V; o->E = m->E;

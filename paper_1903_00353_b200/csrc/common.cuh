@@ -47,7 +47,7 @@ enum {
     CTR_BIGCUR = CTR_SPREAD + CTR_SLOTS * 8,     // evaluate_big_kernel: one fetch cursor per row slice
     CTR_TOTAL = CTR_BIGCUR + 8
 };
-enum { SP_POLY = 0, SP_TESTED, SP_ACCEPTED, SP_ROWS };
+enum { SP_POLY = 0, SP_TESTED, SP_ACCEPTED, SP_ROWS, SP_BAND, SP_RECHECK };
 
 // ---------------------------------------------------------------------------------------
 // feature tables (HBM layout)

@@ -505,12 +505,14 @@ __global__ void __launch_bounds__(EB_BT, 12) emit_bricks_kernel(MeshView mv, Gri
                                                             const u64 *__restrict__ scratch,
                                                             float *__restrict__ dist, int *__restrict__ tri,
                                                             u64 *__restrict__ ctr) {
+    // every warp owns a quarter of the brick (two z-slices, 128 cells) and its own queue: no block-wide rendezvous
+    // (the barriers were 52 % of this kernel's stall samples)
     __shared__ u64 s_pack[BRICK_CELLS];
     __shared__ unsigned short s_cell[BRICK_CELLS];
-    __shared__ u32 s_n, s_stat[2];
-    const int tid = threadIdx.x;
-    if (tid == 0) { s_n = 0; s_stat[0] = s_stat[1] = 0; }
-    __syncthreads();
+    __shared__ u32 s_n[EB_BT / 32];
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    if (lane == 0) s_n[w] = 0;
+    __syncwarp();
     const int slot = blockIdx.x;
     const int b = list[slot];
     const int bx = b % g.nbx, by = (b / g.nbx) % g.nby, bz = b / (g.nbx * g.nby);
@@ -536,7 +538,7 @@ __global__ void __launch_bounds__(EB_BT, 12) emit_bricks_kernel(MeshView mv, Gri
                 any = true;
                 band++;
             } else {
-                const u32 q = atomicAdd(&s_n, 1u);
+                const u32 q = 128u * (u32)w + atomicAdd(&s_n[w], 1u);
                 s_pack[q] = p[c];
                 s_cell[q] = (unsigned short)(c0 + c);
             }
@@ -561,24 +563,28 @@ __global__ void __launch_bounds__(EB_BT, 12) emit_bricks_kernel(MeshView mv, Gri
             }
         }
     }
-    __syncthreads();        // the segment stores above come before the single-cell stores below
-    const int n = (int)s_n;
-    for (int q = tid; q < n; q += EB_BT) {
-        const int c = s_cell[q];
+    __syncwarp();           // the warp's segment stores above come before its single-cell stores below (same warp, same cells)
+    const int n = (int)s_n[w];
+    for (int q = lane; q < n; q += 32) {
+        const int c = s_cell[128 * w + q];
         const int i = bx * 8 + (c & 7), j = by * 8 + ((c >> 3) & 7), k = bz * 8 + (c >> 6);
-        const CellOut o = finish_cell(mv, g, i, j, k, s_pack[q], recheck);
+        const CellOut o = finish_cell(mv, g, i, j, k, s_pack[128 * w + q], recheck);
         if (o.t >= 0) {
             const size_t idx = SPARSE ? (size_t)slot * BRICK_CELLS + c : ((size_t)k * g.ny + j) * g.nx + i;
             dist[idx] = o.d; tri[idx] = o.t;
             band++;
         }
     }
-    if (band) atomicAdd(&s_stat[0], band);
-    if (recheck) atomicAdd(&s_stat[1], recheck);
-    __syncthreads();
-    if (tid == 0) {
-        if (s_stat[0]) atomicAdd(&ctr[CTR_BAND], (u64)s_stat[0]);
-        if (s_stat[1]) atomicAdd(&ctr[CTR_RECHECK], (u64)s_stat[1]);
+    // statistics: warp sums into counters spread over CTR_SLOTS lines (same-address atomics serialise in L2)
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+        band += __shfl_xor_sync(0xffffffffu, band, o);
+        recheck += __shfl_xor_sync(0xffffffffu, recheck, o);
+    }
+    if (lane == 0) {
+        u64 *sp = ctr + CTR_SPREAD + ((blockIdx.x * (EB_BT / 32) + w) & (CTR_SLOTS - 1)) * 8;
+        if (band) atomicAdd(sp + SP_BAND, (u64)band);
+        if (recheck) atomicAdd(sp + SP_RECHECK, (u64)recheck);
     }
 }
 
