@@ -27,6 +27,7 @@
  * SDF_FILL_MODE=0..4, SDF_SCHEDULER=serial | dynamic[:N], SDF_RUFF=cone, SDF_NO_BINNING=1,
  * SDF_CREATE_FORK=0 (vertex stage on the caller's stream), SDF_SMOOTH_SIN=x (edges / vertices whose normals span less
  * than asin(x) get no wedge / cone of their own, their faces' prisms are widened instead; default 1/32, 0 = off), SDF_FILLINT_PLAIN=1 (interior fill without the blank map);
+ * SDF_FILL_SM_SHARE=1..8 / SDF_FILL_CHUNK_LOG2=11..14 / SDF_SCRATCH_HINT=0 (sentinel-fill and scratch ablations);
  * see DESIGN.md.
  */
 #ifndef PAPER_1903_00353_SDF_H
@@ -103,9 +104,14 @@ typedef struct sdf_stats_t {
  *   ntri      1 .. 2^29
  *   a         device allocator, or NULL
  *   stream    cudaStream_t (0 = legacy default stream).  The call synchronises the stream
- *             twice (the vertex count mid-way, the validation flags before returning).
- * The library works on a spatially binned copy of the soup (coarse Morton order); every
- * triangle id it reports is the caller's.
+ *             once, before returning (validation flags and the counts of vertices, wedges and
+ *             cones; the per-vertex tables are sized by V <= 3F/2 + 64, which every closed
+ *             surface meets, so no count is needed mid-way).
+ * The library works on a spatially ordered copy of the soup (fine Morton order); every
+ * triangle id it reports is the caller's.  Vertex ids (sdf_get_table) and the order of the edge
+ * records depend on the order in which thread blocks run; no value of the output grids does.
+ * SDF_BUILDER=tile selects the tile-local builder (shared-memory weld / pairing per spatial tile;
+ * bit-identical tables and grids, measured slower on a B200: an ablation).
  *   out       receives the handle on SDF_OK; set to NULL otherwise.
  * Errors: SDF_EINVAL, SDF_ENOTCLOSED, SDF_EORIENT, SDF_EDEGENERATE, SDF_ENOMEM, SDF_ECUDA.
  */
@@ -148,17 +154,18 @@ int sdf_compute(sdf_mesh *m, const float origin[3], float h, int nx, int ny, int
  * feature construction lets the dense sentinel write of both grids (A8a:
  * +INFINITY / -1 outside the band), which depends on nothing but the output
  * pointers, start earlier: environment SDF_PREFILL_AT = 1 (before A0), 2 (before the edge table),
- * 3 (before edge pairing), 4 (default: where sdf_compute forks it, beside A5-A7).  On a B200 the
- * early starts LOSE (the feature kernels stall under the fill's write stream), so
- * they are an ablation, not the default.  What the single call does gain: the brick marking and
- * its prefix sum (A6a) run on the vertex stream beside the edge stage and their total returns with
- * the validation flags -- one stream synchronisation fewer than the two calls (
- * SDF_HOIST_BRICKS=0 switches that off).
+ * 3 (before edge pairing), 4 (default: behind the last feature kernel, under the host crossing),
+ * 5 (after the crossing, where sdf_compute forks it).  On a B200 the starts 1-3 LOSE: the feature
+ * kernels and the fill are bound by the same memory pipe and take the sum of their times whatever
+ * the fill's rate, so they are an ablation.  What the single call does gain: the
+ * brick marking and its prefix sum (A6a) run inside the feature construction and their total
+ * returns with the validation flags -- ONE stream synchronisation for the whole call against two
+ * for the two calls (SDF_HOIST_BRICKS=0 switches that off).
  *
  *   tri_xyz, ntri, on_device, a      as for sdf_create
  *   origin, h, nx, ny, nz, band      as for sdf_compute
  *   dist_out, tri_out                DEVICE, caller-owned, as for sdf_compute; overwritten entirely
- *   stream                           cudaStream_t; synchronised twice (sdf_create's two crossings)
+ *   stream                           cudaStream_t; synchronised once (flags, counts and the brick total together)
  *   out                              receives the handle (for sdf_stats, further sdf_compute calls ...) on
  *                                    SDF_OK; NULL otherwise, and then the output grids hold unspecified values
  *                                    (the fill has been waited for: nothing is left in flight).
