@@ -610,7 +610,7 @@ static int fork_sentinel_fill(sdf_mesh *m, const GridParams &g, float *dist, int
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const int64_t N = (int64_t)g.nx * g.ny * g.nz;
     const int vec = (((uintptr_t)dist & 15) == 0) && (((uintptr_t)tri & 15) == 0);
-    if (!m->fill_state) CKS(dev_alloc(&m->alloc, (void **)&m->fill_state, sizeof(u32) * FILL_STATE_WORDS, st));
+    static_assert(FILL_STATE_WORDS == 1024, "fill_state is carved out of slab_f with 1024 words (features.cu)");
     auto launch_fill = [&](cudaStream_t fs) -> int {
         stage_mark(m, SDF_T_FILL, 0, fs);
         if (vec && g.fill_mode != 1) {
@@ -746,7 +746,6 @@ int maybe_begin_bricks(sdf_mesh *m, cudaStream_t st, const GridParams **g_dev, u
     if (!m->hoist_g) return SDF_OK;
     CKS(alloc_brick_ws(m, *m->hoist_g, st));
     CKS(reset_bricks(m, *m->hoist_g, st));
-    if (!m->hoist_g_dev) CKS(dev_alloc(&m->alloc, (void **)&m->hoist_g_dev, sizeof(GridParams), st));
     CK(cudaMemcpyAsync(m->hoist_g_dev, m->hoist_g, sizeof(GridParams), cudaMemcpyHostToDevice, st));
     *g_dev = m->hoist_g_dev;
     *flag = m->brick_flag;

@@ -652,6 +652,8 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
         m->vsm = c.take<unsigned char>((size_t)vcap);
         m->d_ctr = c.take<u64>(CTR_TOTAL);
         m->d_flags = c.take<int>(4);
+        m->fill_state = c.take<u32>(1024);                   // (small blocks of their own would each cost an allocator call)
+        m->hoist_g_dev = c.take<GridParams>(1);
         if (pass == 0) CKS(dev_alloc(al, &m->slab_f, c.off, st));
     }
     CK(cudaMemsetAsync(m->d_ctr, 0, sizeof(u64) * CTR_TOTAL, st));
@@ -783,6 +785,8 @@ static int build_features_tile(sdf_mesh *m, const float *tri, int on_device, cud
         m->vsm = c.take<unsigned char>((size_t)vcap);
         m->d_ctr = c.take<u64>(CTR_TOTAL);
         m->d_flags = c.take<int>(4);
+        m->fill_state = c.take<u32>(1024);                   // (small blocks of their own would each cost an allocator call)
+        m->hoist_g_dev = c.take<GridParams>(1);
         if (pass == 0) CKS(dev_alloc(al, &m->slab_f, c.off, st));
     }
     CK(cudaMemsetAsync(m->d_ctr, 0, sizeof(u64) * CTR_TOTAL, st));
