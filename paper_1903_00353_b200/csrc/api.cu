@@ -94,7 +94,7 @@ void sdf_destroy(sdf_mesh *m) {
     if (m->ev_join) cudaEventDestroy(m->ev_join);
     if (m->ev_ffork) cudaEventDestroy(m->ev_ffork);
     if (m->ev_fjoin) cudaEventDestroy(m->ev_fjoin);
-    void *ptrs[] = {m->slab_f, m->slab_v, m->slab_ws, m->scratch, m->cp_state};      // (fill_state, hoist_g_dev: views into slab_f)
+    void *ptrs[] = {m->slab_f, m->slab_ws, m->scratch, m->cp_state};      // (fill_state, hoist_g_dev: views into slab_f)
     for (size_t i = 0; i < sizeof(ptrs) / sizeof(ptrs[0]); i++) dev_free(&m->alloc, ptrs[i], st);
     for (int i = 0; i < SDF_T_COUNT; i++)
         for (int w = 0; w < 2; w++)

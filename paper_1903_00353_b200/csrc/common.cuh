@@ -135,8 +135,7 @@ struct sdf_mesh {
     int64_t F, E, V;
     // device memory comes in a few slabs carved into tables (one allocator call each: the
     // caller's allocator may be a slow host callback)
-    void *slab_f;            // F-sized feature tables + counters
-    void *slab_v;            // V-sized feature tables
+    void *slab_f;            // every persistent feature table (per-vertex ones sized by V <= 3F/2 + 64) + counters
     void *slab_ws; size_t slab_ws_cap;     // per-compute workspace (bytes), grown on demand
     // feature tables (device, views into the slabs)
     float *soup;             // [F][9] canonicalised copy of the input

@@ -836,12 +836,9 @@ static int build_features_tile(sdf_mesh *m, const float *tri, int on_device, cud
     }
     CK(cudaMemsetAsync(wtab, 0xFF, (size_t)((char *)(etab + cape) - (char *)wtab), st));
     CKS(order_triangles(src, F, ow, (u32 *)m->perm, st));
-    static bool attr_set = false;
-    if (!attr_set) {
-        CK(cudaFuncSetAttribute(tile_geom_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileGeomSmem)));
-        CK(cudaFuncSetAttribute(tile_cone_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileConeSmem)));
-        attr_set = true;
-    }
+    // (per call: the attribute belongs to the current device, and the two calls cost a few microseconds)
+    CK(cudaFuncSetAttribute(tile_geom_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileGeomSmem)));
+    CK(cudaFuncSetAttribute(tile_cone_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileConeSmem)));
     // A1: weld inside the tiles, the tiles' unique vertices through the global table
     KL; tile_weld_kernel<<<ntiles, TB, 0, st>>>(src, m->perm, (int)F, m->soup, m->inv_perm, wtab, capw - 1, tt, vcorner, vacc,
                                               vcosq, vcospos, vside, m->vmint, vcap, m->d_ctr, m->d_flags);
