@@ -6,9 +6,9 @@
 //
 // Differences from the paper's design: hashed exact-bit vertex keys instead of
 // lossy 30-bit Morton codes, exact (min,max) vertex-id edge keys instead
-// of concatenated Morton codes, own radix sort instead of thrust
-// (PAPER.md:336), order-independent fixed-point atomics instead of the per-group serial
-// regrouping.
+// of concatenated Morton codes, a one-pass counting sort of the triangles by a
+// fine Morton bin instead of thrust::sort_by_key on the features, order-independent
+// fixed-point atomics instead of the per-group serial regrouping.
 #include "primitives.cuh"
 #include "evaluate.cuh"
 #include <math.h>

@@ -1,15 +1,19 @@
-// tile_features.cuh -- tile-local feature builder (included by features.cu; the default of sdf_create).
+// tile_features.cuh -- included by features.cu.  Holds (1) what both feature builders share: the edge classifier
+// (edge_class_of), the record writer, edge_pair_record_kernel (pairing through the global half-edge table, class and
+// wedge record in one pass -- the default builder runs it over every half-edge) and vertex_axis64; (2) the TILE-LOCAL
+// builder, SDF_BUILDER=tile: an ablation, bit-identical to the default builder in every table and grid
+// (tests/test_gpu_features.py) and measured slower on a B200 (C4 3.84 against 3.28 ms).
 //
 // The paper regroups the unordered STL entries with a Morton sort and a per-group serial pass and
-// names that regrouping as its bottleneck.  The first builder of this library (kept below in
-// features.cu as SDF_BUILDER=global) welded vertices and paired half-edges through hash tables in global memory: every
-// one of the 3F corners costs 6-8 random L2 sectors and the kernels run at the L2 sector rate of a B200 (~370 G
-// sectors/s measured, profiles/r2_atomics.md), i.e. 24x the algorithmic bytes.
+// names that regrouping as its bottleneck.  The default builder (features.cu) welds vertices and
+// pairs half-edges through hash tables in global memory: every one of the 3F corners costs several random L2 sectors
+// (478 M sectors for 144 MB of input at C4, profiles/r2_atomics.md).  The tile-local builder was the attempt to keep
+// that traffic on chip:
 //
-// Here the soup is first put in a coarse spatial order (the 15-bit Morton binning of features.cu) and then cut into
-// tiles of TT consecutive triangles -- a compact patch of surface.  Inside a tile everything happens in shared memory:
+// The soup is put in a fine Morton order (the one-pass counting sort of features.cu) and cut into tiles of TT
+// consecutive triangles.  Inside a tile everything happens in shared memory:
 //   T1 tile_weld_kernel   gather + canonicalise the tile, weld its corners in a shared-memory hash table (exact bits),
-//                         then only the tile's UNIQUE vertices (~1/5 of its corners) go through the global weld table
+//                         then only the tile's UNIQUE vertices (~1/4 of its corners) go through the global weld table
 //                         (find-or-insert; the inserter takes a vertex id from a counter and resets the accumulators)
 //   T3 tile_geom_kernel   vertex ids of the corners, fp64 face normals and corner angles, the angle-weighted normal
 //                         sums (eq.8) combined per tile vertex in shared memory (32-bit limbs) and added
@@ -19,8 +23,11 @@
 //   T4 edge_pair_record_kernel   the boundary half-edges: pairing through the global table, class + record in one pass
 //   T5 tile_cone_kernel   cone angle (eq.9), side bits and lowest triangle id,
 //                         combined per tile vertex in shared memory, one global atomic each per tile vertex
-// Vertex ids and the order of the edge records depend on the order in which blocks run; nothing that reaches the
-// output does (ids written to the grids are the caller's triangle ids, all sums are integer).
+// It halves the L2 sectors (223 M) and loses on instructions and occupancy: 44-69 KB of shared memory and 76-80 registers
+// per thread, 300 M warp instructions in tile_geom_kernel alone; and a run of a space-filling curve is several patches,
+// not one: 54 % of a tile's vertices also occur in another tile.
+// Vertex ids and the order of the edge records depend on the order in which blocks run (both builders); nothing that
+// reaches the output does (ids written to the grids are the caller's triangle ids, all sums are integer).
 #pragma once
 
 #define TT 512                 // triangles per tile
