@@ -16,7 +16,7 @@ CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libsdf_b200.so")
 SOURCES = ["api.cu", "features.cu", "compute.cu", "fill.cu", "stl_io.cu", "peaks.cu"]
 RDC_SOURCES = ["cdp.cu"]          # device-side launches (the dynamic-parallelism ablation): relocatable device code
-HEADERS = ["common.cuh", "primitives.cuh", "evaluate.cuh", os.path.join("..", "..", "include", "sdf.h")]
+HEADERS = ["common.cuh", "primitives.cuh", "evaluate.cuh", "tile_features.cuh", os.path.join("..", "..", "include", "sdf.h")]
 ARCH_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a"]
 NVCC_FLAGS = ARCH_FLAGS + ["-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
 LINK_FLAGS = ARCH_FLAGS + ["-shared", "-Xcompiler", "-fPIC", "--cudart", "static", "-lcudadevrt"]

@@ -2,7 +2,7 @@
 // (edge_class_of), the record writer, edge_pair_record_kernel (pairing through the global half-edge table, class and
 // wedge record in one pass -- the default builder runs it over every half-edge) and vertex_axis64; (2) the TILE-LOCAL
 // builder, SDF_BUILDER=tile: an ablation, bit-identical to the default builder in every table and grid
-// (tests/test_gpu_features.py) and measured slower on a B200 (C4 3.84 against 3.28 ms).
+// (tests/test_gpu_features.py) and measured slower on a B200 (C4 3.84 against 3.36 ms when the two were compared).
 //
 // The paper regroups the unordered STL entries with a Morton sort and a per-group serial pass and
 // names that regrouping as its bottleneck.  The default builder (features.cu) welds vertices and
