@@ -178,14 +178,17 @@ static int make_grid(const float origin[3], float h, int nx, int ny, int nz, flo
     const char *fl = getenv("SDF_FILL_CTAS");
     g->fill_ctas = fl ? atoi(fl) : 32;
     if (g->fill_ctas < 1 || g->fill_ctas > 64) g->fill_ctas = 32;
-    g->fill_depth = fd ? atoi(fd) : 8;
-    g->fill_issuers = fi ? atoi(fi) : 4;
-    if (g->fill_issuers < 1 || g->fill_issuers > 4) g->fill_issuers = 4;
+    // one issuing lane per SM, 8 KiB bulk copies, three pairs in flight: the fewer bulk stores are queued in L2 the less
+    // the kernels beside the fill are held up (4 lanes x 9 pairs of 4 KiB: C4 3.27 -> 3.20 ms, C5 4.22 -> 4.12; alone the
+    // fill runs at 7.3 TB/s either way; profiles/r2_ablations.md)
+    g->fill_depth = fd ? atoi(fd) : 2;
+    g->fill_issuers = fi ? atoi(fi) : 1;
+    if (g->fill_issuers < 1 || g->fill_issuers > 4) g->fill_issuers = 1;
     const char *sh = getenv("SDF_SCRATCH_HINT");
     g->scratch_hint = (sh && sh[0] == '0') ? 0 : 1;
     const char *fck = getenv("SDF_FILL_CHUNK_LOG2");
-    g->fill_chunk_log2 = fck ? atoi(fck) : 12;
-    if (g->fill_chunk_log2 < 11 || g->fill_chunk_log2 > 14) g->fill_chunk_log2 = 12;
+    g->fill_chunk_log2 = fck ? atoi(fck) : 13;
+    if (g->fill_chunk_log2 < 11 || g->fill_chunk_log2 > 14) g->fill_chunk_log2 = 13;
     const char *fsh = getenv("SDF_FILL_SM_SHARE");
     g->fill_sm_share = fsh ? atoi(fsh) : 8;
     if (g->fill_sm_share < 1 || g->fill_sm_share > 8) g->fill_sm_share = 8;

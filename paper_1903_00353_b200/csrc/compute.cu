@@ -373,14 +373,15 @@ __global__ void __launch_bounds__(FILL_BT) fill_kernel(float *__restrict__ dist,
     }
 }
 
-// TMA variant (the default): one CTA per SM keeps two 4 KiB sentinel tiles in shared memory and
-// one lane per warp streams them to HBM with bulk asynchronous copies (cp.async.bulk, SASS
-// UBLKCP), L2 evict-first.  It needs 4 warps and 8 KiB of shared memory per SM, so the kernels
-// of A5-A7 keep (almost) the whole SM while 8 B/cell stream out underneath them.
+// TMA variant (the default): one CTA per SM keeps two sentinel tiles (8 KiB each by default) in shared memory and
+// one lane streams them to HBM with bulk asynchronous copies (cp.async.bulk, SASS UBLKCP), L2 evict-first.  It
+// needs 4 warps and 16-32 KiB of shared memory per SM, so the kernels of A5-A7 keep (almost) the whole SM while
+// 8 B/cell stream out underneath them.
 #define FILL_TMA_BT 128
-#define FILL_TMA_CHUNK 4096      // default bytes per bulk copy (runtime: bits 16.. of the `issuers` argument hold log2).  The size sets the balance with the kernels running beside
-                                 // the fill: 2 KiB starves them (evaluate 1.46 -> 1.96 ms at C4), 16 KiB yields to them
-                                 // (fill 1.55 ms); alone the fill does 7.3 TB/s at 4 KiB
+// bytes per bulk copy: runtime, bits 16.. of the `issuers` argument hold log2 (SDF_FILL_CHUNK_LOG2, default 13); issuing
+// lanes = bits 0..7 (SDF_FILL_ISSUERS, default 1); pairs in flight per lane = DEPTH + 1 (SDF_FILL_DEPTH, default 2).
+// What matters beside another kernel is how many bulk stores are queued in L2 at a time: with one lane the fill both
+// runs faster alone (1.18 against 1.22 ms at C4) and holds the evaluate kernels up less (profiles/r2_ablations.md).
 // fill_state: [0] = next batch (dynamic fetch), [1 + smid] = SM already has a fill CTA.  More
 // CTAs than SMs are launched and the first to arrive on an SM claims it; the others exit at
 // once.  (With one CTA per SM by count only, a busy GPU stacked several fill CTAs on the few
@@ -989,10 +990,12 @@ int run_closest_points(sdf_mesh *m, const GridParams &g, const int *tri, float *
         if (!m->cp_state) CKS(dev_alloc(&m->alloc, (void **)&m->cp_state, sizeof(u32) * FILL_STATE_WORDS, st));
         CK(cudaMemsetAsync(m->cp_state, 0, sizeof(u32) * FILL_STATE_WORDS, st));
         const int64_t half = 3 * n / 2;
-        int64_t bq = (half / (FILL_TMA_CHUNK / 4)) / ((int64_t)sms * 4 * 8);
-        const int batch = (int)(bq < 1 ? 1 : (bq > FILL_BATCH_BYTES / FILL_TMA_CHUNK ? FILL_BATCH_BYTES / FILL_TMA_CHUNK : bq));
-        KL; fill_tma_kernel<8><<<(unsigned)(sms * 4), FILL_TMA_BT, 0, st>>>(cp, (int *)(cp + half), half, 4 | (8 << 8) | (12 << 16), batch, m->cp_state,
-                                                                         0x7F800000u, 0x7F800000u);
+        const int chunk = 1 << g.fill_chunk_log2;
+        int64_t bq = (half / (chunk / 4)) / ((int64_t)sms * g.fill_issuers * 8);
+        const int batch = (int)(bq < 1 ? 1 : (bq > FILL_BATCH_BYTES / chunk ? FILL_BATCH_BYTES / chunk : bq));
+        KL; fill_tma_kernel<2><<<(unsigned)(sms * 4), FILL_TMA_BT, 0, st>>>(cp, (int *)(cp + half), half,
+                                                                         g.fill_issuers | (8 << 8) | (g.fill_chunk_log2 << 16), batch,
+                                                                         m->cp_state, 0x7F800000u, 0x7F800000u);
         KL; closest_points_sparse_kernel<<<(unsigned)((n / 4 + 256 * CPS_LOADS - 1) / (256 * CPS_LOADS)), 256, 0, st>>>(mv, g, tri, cp, n);
         CK(cudaGetLastError());
         m->last_stream = st;
