@@ -92,6 +92,7 @@ void sdf_destroy(sdf_mesh *m) {
     if (m->side) cudaStreamSynchronize(m->side);      // shared, process-lifetime stream: not destroyed here
     if (m->ev_fork) cudaEventDestroy(m->ev_fork);
     if (m->ev_join) cudaEventDestroy(m->ev_join);
+    if (m->ev_bjoin) cudaEventDestroy(m->ev_bjoin);
     if (m->ev_ffork) cudaEventDestroy(m->ev_ffork);
     if (m->ev_fjoin) cudaEventDestroy(m->ev_fjoin);
     void *ptrs[] = {m->slab_f, m->slab_ws, m->scratch, m->cp_state};      // (fill_state, hoist_g_dev: views into slab_f)

@@ -172,6 +172,7 @@ struct sdf_mesh {
     cudaStream_t last_stream;
     cudaStream_t side;                // library-owned stream of the sentinel fill (A8a)
     cudaEvent_t ev_fork, ev_join;
+    cudaEvent_t ev_bjoin;             // join of the brick stream (hoisted A6a beside the edge and vertex stages)
     // sdf_transform: sentinel fill still to be started at stage boundary pre_at of build_features (0 = none pending)
     const GridParams *pre_g; float *pre_dist; int *pre_tri; int pre_at;
     // sdf_transform: A6a (brick marks + scan) still to be run by build_features / already run for the next run_compute

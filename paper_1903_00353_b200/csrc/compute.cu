@@ -15,12 +15,41 @@
 
 #include "evaluate.cuh"
 
-// A6a (evaluate.cuh mark_triangle_bricks): one thread per triangle
+// A6a (evaluate.cuh): four threads per triangle.  The first decides whether the triangle is small (one box of a few
+// bricks: it marks them, the other three leave after one shuffle); the four boxes of a larger one go to one thread each
+// (one thread walking all four in turn: 56 us for the 20480 triangles of C2, 0.2 ms at C5; the whole warp walking one
+// triangle's boxes after another was tried too and is slower still: C3 0.41 -> 0.47 ms).
+// SPLIT = false: a thread per triangle does it all (meshes of millions of sub-cell triangles, where three of the four
+// threads would only add waves).
+template <bool SPLIT>
 __global__ void __launch_bounds__(256) brick_mark_kernel(MeshView mv, GridParams g,
                                                          unsigned char *__restrict__ brick_flag) {
-    const int64_t t = (int64_t)blockIdx.x * 256 + threadIdx.x;
-    if (t >= mv.F) return;
-    mark_triangle_bricks(g, mv.soup + 9 * t, mv.fn + 3 * t, brick_flag);
+    const int64_t gid = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (!SPLIT) {
+        if (gid < mv.F) mark_triangle_bricks(g, mv.soup + 9 * gid, mv.fn + 3 * gid, brick_flag);
+        return;
+    }
+    const int64_t t = gid >> 2;
+    const int q = (int)(gid & 3), lane = threadIdx.x & 31;
+    const bool valid = t < mv.F;
+    float T[9], N[3];
+    int small = 1;
+    if (valid && q == 0) {
+#pragma unroll
+        for (int i = 0; i < 9; i++) T[i] = mv.soup[9 * t + i];
+        small = mark_triangle_small(g, T, brick_flag) ? 1 : 0;
+    }
+    small = __shfl_sync(0xffffffffu, small, lane & ~3);
+    if (small || !valid) return;
+    if (q) {
+#pragma unroll
+        for (int i = 0; i < 9; i++) T[i] = mv.soup[9 * t + i];
+    }
+#pragma unroll
+    for (int i = 0; i < 3; i++) N[i] = mv.fn[3 * t + i];
+    float mn[3], mx[3];
+    triangle_part_box(g, T, N, q, mn, mx);
+    mark_box(g, mn, mx, brick_flag);
 }
 
 struct BrickIn {
@@ -726,7 +755,8 @@ static int scan_bricks(sdf_mesh *m, const GridParams &g, cudaStream_t ps, bool m
     stage_mark(m, SDF_T_CLIP_SCAN, 0, ps);
     if (!marked) {
         const MeshView mv = make_view(m);
-        KL; brick_mark_kernel<<<(unsigned)((mv.F + 255) / 256), 256, 0, ps>>>(mv, g, m->brick_flag);
+        if (mv.F >= (1 << 21)) { KL; brick_mark_kernel<false><<<(unsigned)((mv.F + 255) / 256), 256, 0, ps>>>(mv, g, m->brick_flag); }
+        else { KL; brick_mark_kernel<true><<<(unsigned)((4 * (int64_t)mv.F + 255) / 256), 256, 0, ps>>>(mv, g, m->brick_flag); }
     }
     CKS(launch_scan(BrickIn{m->brick_flag}, BrickOut{m->brick_table, m->brick_list}, nbricks, m->scan_ws, m->d_ctr + CTR_BRICKS, ps));
     CK(cudaGetLastError());

@@ -124,8 +124,10 @@ __device__ __forceinline__ void mark_box(const GridParams &g, const float *mn, c
                 if (!*f) *f = 1;            // mostly already set: a cached read, not a write
             }
 }
-__device__ __forceinline__ void mark_triangle_bricks(const GridParams &g, const float *T, const float *N,
-                                                     unsigned char *__restrict__ brick_flag) {
+// A small triangle (or the AABB debug mode): its box grown by the reach holds all four boxes and costs no extra brick.
+// Marks it and returns true; false for a larger triangle (nothing marked).
+__device__ __forceinline__ bool mark_triangle_small(const GridParams &g, const float *T,
+                                                    unsigned char *__restrict__ brick_flag) {
     const float rb = g.rb, eps = g.eps;
     float lo[3], hi[3], mn[3], mx[3];
     float ext_max = 0.0f;
@@ -134,27 +136,41 @@ __device__ __forceinline__ void mark_triangle_bricks(const GridParams &g, const 
         lo[i] = fminf(T[i], fminf(T[3 + i], T[6 + i])); hi[i] = fmaxf(T[i], fmaxf(T[3 + i], T[6 + i]));
         ext_max = fmaxf(ext_max, hi[i] - lo[i]);
     }
-    if (g.aabb_mode || ext_max <= 4.0f * g.h) {
-        // small triangle: its box grown by the reach holds all four boxes and costs no extra brick
+    if (!(g.aabb_mode || ext_max <= 4.0f * g.h)) return false;
 #pragma unroll
-        for (int i = 0; i < 3; i++) { mn[i] = lo[i] - rb - eps; mx[i] = hi[i] + rb + eps; }
-        mark_box(g, mn, mx, brick_flag);
-        return;
-    }
-#pragma unroll
-    for (int i = 0; i < 3; i++) {
-        float ext = rb * fabsf(N[i]);
-        mn[i] = lo[i] - ext - eps; mx[i] = hi[i] + ext + eps;
-    }
+    for (int i = 0; i < 3; i++) { mn[i] = lo[i] - rb - eps; mx[i] = hi[i] + rb + eps; }
     mark_box(g, mn, mx, brick_flag);
+    return true;
+}
+// box q of a larger triangle: 0 = the slab box, 1..3 = the box of edge q-1 grown by the reach
+__device__ __forceinline__ void triangle_part_box(const GridParams &g, const float *T, const float *N, int q,
+                                                  float *mn, float *mx) {
+    const float rb = g.rb, eps = g.eps;
+    if (q == 0) {
 #pragma unroll
-    for (int k = 0; k < 3; k++) {
+        for (int i = 0; i < 3; i++) {
+            const float lo = fminf(T[i], fminf(T[3 + i], T[6 + i])), hi = fmaxf(T[i], fmaxf(T[3 + i], T[6 + i]));
+            const float ext = rb * fabsf(N[i]);
+            mn[i] = lo - ext - eps; mx[i] = hi + ext + eps;
+        }
+    } else {
+        const int k = q - 1;
         const float *A = T + 3 * k, *B = T + 3 * (k == 2 ? 0 : k + 1);
 #pragma unroll
         for (int i = 0; i < 3; i++) {
             mn[i] = fminf(A[i], B[i]) - rb - eps;
             mx[i] = fmaxf(A[i], B[i]) + rb + eps;
         }
+    }
+}
+// one thread, all boxes (tri_geom_kernel: C4-like meshes of sub-cell triangles, one box each)
+__device__ __forceinline__ void mark_triangle_bricks(const GridParams &g, const float *T, const float *N,
+                                                     unsigned char *__restrict__ brick_flag) {
+    if (mark_triangle_small(g, T, brick_flag)) return;
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+        float mn[3], mx[3];
+        triangle_part_box(g, T, N, q, mn, mx);
         mark_box(g, mn, mx, brick_flag);
     }
 }

@@ -539,17 +539,21 @@ static int classify_edge_errors(sdf_mesh *m, int nc, TmpPool &tmp, cudaStream_t 
     return SDF_OK;
 }
 
-// the library's second stream (vertex stage beside the edge stage): forked from st, drained on early returns
-static int fork_vertex_stream(sdf_mesh *m, cudaStream_t st, cudaStream_t *vs_out, StreamDrain &drain) {
+// the library's second and third stream (vertex stage and hoisted A6a beside the edge stage): forked from st, drained
+// on early returns
+static int fork_vertex_stream(sdf_mesh *m, cudaStream_t st, cudaStream_t *vs_out, StreamDrain &drain,
+                              cudaStream_t *bs_out = nullptr, StreamDrain *bdrain = nullptr) {
     *vs_out = st;
+    if (bs_out) *bs_out = st;
     const char *cf = getenv("SDF_CREATE_FORK");
     if (cf && cf[0] == '0') return SDF_OK;
-    static cudaStream_t g_vs = nullptr;
+    static cudaStream_t g_vs = nullptr, g_bs = nullptr;
     static int g_vs_dev = -1;
     int dev = 0;
     CK(cudaGetDevice(&dev));
     if (!g_vs || g_vs_dev != dev) {
         CK(cudaStreamCreateWithFlags(&g_vs, cudaStreamNonBlocking));
+        CK(cudaStreamCreateWithFlags(&g_bs, cudaStreamNonBlocking));
         g_vs_dev = dev;
     }
     if (!m->ev_fork) CK(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
@@ -558,6 +562,12 @@ static int fork_vertex_stream(sdf_mesh *m, cudaStream_t st, cudaStream_t *vs_out
     CK(cudaStreamWaitEvent(g_vs, m->ev_fork, 0));
     drain.s = g_vs; drain.armed = true;
     *vs_out = g_vs;
+    if (bs_out && bdrain && m->hoist_g) {
+        if (!m->ev_bjoin) CK(cudaEventCreateWithFlags(&m->ev_bjoin, cudaEventDisableTiming));
+        CK(cudaStreamWaitEvent(g_bs, m->ev_fork, 0));
+        bdrain->s = g_bs; bdrain->armed = true;
+        *bs_out = g_bs;
+    }
     return SDF_OK;
 }
 
@@ -628,7 +638,7 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
     const int nc = (int)(3 * F);
     const sdf_allocator *al = &m->alloc;
     TmpPool tmp(al, st);
-    StreamDrain drain;
+    StreamDrain drain, bdrain;
     m->E = nc / 2;
     // every vertex of a closed surface has at least two corners, so V <= 3F/2; the per-vertex tables are sized by that
     // bound (no host crossing for the count) and a soup with more vertices is flagged not closed by ingest_weld_kernel
@@ -725,12 +735,19 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
     KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wvid, slot, (int)F, m->cvid, m->fn, vacc, etab, cape - 1, m->d_flags,
                                                     mark_g, mark_flag);
     // the vertex stage needs only what tri_geom wrote: it runs on a second stream beside the edge stage
-    cudaStream_t vs = st;
-    CKS(fork_vertex_stream(m, st, &vs, drain));
+    // (and A6a -- brick marks unless tri_geom made them, scan -- on a third one: it needs the soup and the normals only)
+    cudaStream_t vs = st, bs = st;
+    CKS(fork_vertex_stream(m, st, &vs, drain, &bs, &bdrain));
     CKS(maybe_prefill(m, 3, st));
     // pairing, classes and wedge records in one pass
     KL; edge_pair_record_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, etab, cape - 1, m->adj, m->soup, m->fn, m->perm,
                                                             smooth_sin, m->erec, (int)m->E, (int *)m->fsm, m->d_ctr, m->d_flags);
+    CKS(maybe_prepare_bricks(m, st, bs, mark_g != nullptr));
+    if (bs != st && bs != vs) {
+        CK(cudaEventRecord(m->ev_bjoin, bs));
+        CK(cudaStreamWaitEvent(st, m->ev_bjoin, 0));
+        bdrain.armed = false;
+    }
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_EDGES, 1, st);
 
@@ -742,7 +759,6 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
                                                            vcospos, smooth_sin, m->vrec, m->vsm, m->cone_list, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_VERTICES, 1, vs);
-    CKS(maybe_prepare_bricks(m, st, vs, mark_g != nullptr));
     if (vs != st) {
         CK(cudaEventRecord(m->ev_join, vs));
         CK(cudaStreamWaitEvent(st, m->ev_join, 0));
@@ -754,7 +770,7 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
 }
 
 // ===================================================================================================
-// the tile-local builder (default; tile_features.cuh)
+// the tile-local builder (SDF_BUILDER=tile, an ablation; tile_features.cuh)
 // ===================================================================================================
 static int build_features_tile(sdf_mesh *m, const float *tri, int on_device, cudaStream_t st) {
     const int64_t F = m->F;
