@@ -743,11 +743,7 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
     KL; edge_pair_record_kernel<<<blocks_for(F), FB, 0, st>>>(m->cvid, (int)F, etab, cape - 1, m->adj, m->soup, m->fn, m->perm,
                                                             smooth_sin, m->erec, (int)m->E, (int *)m->fsm, m->d_ctr, m->d_flags);
     CKS(maybe_prepare_bricks(m, st, bs, mark_g != nullptr));
-    if (bs != st && bs != vs) {
-        CK(cudaEventRecord(m->ev_bjoin, bs));
-        CK(cudaStreamWaitEvent(st, m->ev_bjoin, 0));
-        bdrain.armed = false;
-    }
+    if (bs != st) CK(cudaEventRecord(m->ev_bjoin, bs));
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_EDGES, 1, st);
 
@@ -759,6 +755,10 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
                                                            vcospos, smooth_sin, m->vrec, m->vsm, m->cone_list, m->d_ctr);
     CK(cudaGetLastError());
     stage_mark(m, SDF_T_VERTICES, 1, vs);
+    if (bs != st) {
+        CK(cudaStreamWaitEvent(st, m->ev_bjoin, 0));
+        bdrain.armed = false;
+    }
     if (vs != st) {
         CK(cudaEventRecord(m->ev_join, vs));
         CK(cudaStreamWaitEvent(st, m->ev_join, 0));
