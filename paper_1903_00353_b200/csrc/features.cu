@@ -277,6 +277,14 @@ __global__ void __launch_bounds__(FB, TG_MINB) tri_geom_kernel(const float *__re
         v[k] = (int)wvid[slot[3 * (size_t)t + k]];
         cvid[3 * (size_t)t + k] = v[k];
     }
+    // forward half-edges (ascending ids): the first probe of each is loaded now and waited for after the fp64 work
+    u32 eh[3], ecur[3];
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const int k1 = (k + 1) % 3;
+        eh[k] = edge_hash((u32)v[k], (u32)v[k1]) & emask;
+        ecur[k] = (v[k] < v[k1]) ? __ldcg(etab + eh[k]) : 0u;
+    }
     double n[3], p[3][3];
     bool ok = tri_normal64(T, n, p);
     // PAPER.md:137 "we disallow faces of zero area".  (A repeated vertex IS a zero area, exactly: equal corners give a zero
@@ -303,18 +311,27 @@ __global__ void __launch_bounds__(FB, TG_MINB) tri_geom_kernel(const float *__re
             for (int i = 0; i < 3; i++)
                 atomicAdd(&vacc[3 * (size_t)v[k] + i], (u64)(long long)llrint(alpha * n[i] * FIXSCALE));
         }
-        // half-edge 3t+k goes corner k -> k+1; forward = ascending ids.  Forward
-        // half-edges take the first empty slot of the edge table on their probe sequence (no key
-        // check: a valid mesh has one forward half-edge per key, and a duplicate just leaves an
-        // entry nobody claims, which the pair count exposes)
-        if (v[k] < v[k1]) {
-            // (a table laid out along the vertex ids, so that the probes of an edge's two triangles hit L2, was measured:
-            // it halves the DRAM reads of the two edge kernels and makes them slower -- their stalls are the round
-            // trips of the L2 atomics themselves, and clustered homes lengthen the probe sequences)
-            u32 h = edge_hash((u32)v[k], (u32)v[k1]) & emask;
-            while (__ldcg(etab + h) != EMPTY32 || atomicCAS(etab + h, EMPTY32, (u32)(3 * t + k)) != EMPTY32)
-                h = (h + 1) & emask;
-        }
+    }
+    // half-edge 3t+k goes corner k -> k+1; forward = ascending ids.  Forward
+    // half-edges take the first empty slot of the edge table on their probe sequence (no key
+    // check: a valid mesh has one forward half-edge per key, and a duplicate just leaves an
+    // entry nobody claims, which the pair count exposes).  The three first claims go out together.
+    // (a table laid out along the vertex ids, so that the probes of an edge's two triangles hit L2, was measured:
+    // it halves the DRAM reads of the two edge kernels and makes them slower -- their stalls are the round
+    // trips of the L2 atomics themselves, and clustered homes lengthen the probe sequences)
+    u32 got[3];
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const int k1 = (k + 1) % 3;
+        got[k] = EMPTY32;                                    // EMPTY32 = placed (or not a forward half-edge)
+        if (v[k] < v[k1]) got[k] = (ecur[k] == EMPTY32) ? atomicCAS(etab + eh[k], EMPTY32, (u32)(3 * t + k)) : ecur[k];
+    }
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        if (got[k] == EMPTY32) continue;
+        u32 h = eh[k];
+        do h = (h + 1) & emask;
+        while (__ldcg(etab + h) != EMPTY32 || atomicCAS(etab + h, EMPTY32, (u32)(3 * t + k)) != EMPTY32);
     }
 }
 
