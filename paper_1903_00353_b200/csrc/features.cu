@@ -685,8 +685,6 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
     }
     CK(cudaMemsetAsync(m->d_ctr, 0, sizeof(u64) * CTR_TOTAL, st));
     CK(cudaMemsetAsync(m->d_flags, 0, sizeof(int) * 4, st));
-    CK(cudaMemsetAsync(m->adj, 0xFF, sizeof(int) * 3 * F, st));
-    CK(cudaMemsetAsync(m->fsm, 0, sizeof(float) * (size_t)F, st));
 
     // smooth features get no polyhedron of their own (common.cuh, SMOOTH_SIN_DEFAULT); SDF_SMOOTH_SIN=0 switches that off
     float smooth_sin = SMOOTH_SIN_DEFAULT;
@@ -729,8 +727,21 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
         CK(cudaMemcpyAsync(staging, tri, sizeof(float) * 9 * F, cudaMemcpyHostToDevice, st));
         src = staging;
     }
-    CK(cudaMemsetAsync(wtab, 0xFF, (size_t)((char *)(etab + cape) - (char *)wtab), st));
-    CKS(order_triangles(src, F, ow, (u32 *)m->perm, st));
+    // the table resets (0.2 GB at C4) run on the second stream beside the latency-bound ordering kernels
+    {
+        cudaStream_t ms = st;
+        StreamDrain mdrain;
+        if (ow.on) CKS(fork_vertex_stream(m, st, &ms, mdrain));        // (small meshes: the fork costs more than it hides)
+        CK(cudaMemsetAsync(wtab, 0xFF, (size_t)((char *)(etab + cape) - (char *)wtab), ms));
+        CK(cudaMemsetAsync(m->adj, 0xFF, sizeof(int) * 3 * F, ms));
+        CK(cudaMemsetAsync(m->fsm, 0, sizeof(float) * (size_t)F, ms));
+        CKS(order_triangles(src, F, ow, (u32 *)m->perm, st));
+        if (ms != st) {
+            CK(cudaEventRecord(m->ev_join, ms));
+            CK(cudaStreamWaitEvent(st, m->ev_join, 0));
+            mdrain.armed = false;
+        }
+    }
     WeldTab wt = {wtab, capw - 1, 0u, ow.cnt, ow.bbox, ow.bits, (u32)F};
     {
         const char *ul = getenv("SDF_UNIFORM_TABLES");
