@@ -48,7 +48,8 @@ enum {
     SDF_EDEGENERATE = 4,  /* zero-area triangle or repeated vertex in a triangle */
     SDF_ENOMEM      = 5,  /* device (or host staging) allocation failed */
     SDF_ECUDA       = 6,  /* CUDA runtime error / no device; see sdf_last_cuda_error() */
-    SDF_EIO         = 7   /* file cannot be opened / read / written, or is not a valid STL file */
+    SDF_EIO         = 7,  /* file cannot be opened / read / written, or is not a valid STL file */
+    SDF_ETOOBIG     = 8   /* sdf_fill_interior_static: the grid needs more scratch than the static array holds */
 };
 
 /* Opaque handle: device-resident feature tables of one mesh.  Owned by the library,
@@ -270,6 +271,22 @@ int sdf_closest_points(sdf_mesh *m, const float origin[3], float h, int nx, int 
  * Errors: SDF_EINVAL, SDF_ENOMEM, SDF_ECUDA.
  */
 int sdf_fill_interior(float *dist, int nx, int ny, int nz, float band, void *stream);
+
+/*
+ * sdf_fill_interior_static -- sdf_fill_interior for callers that must not allocate: code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid cudaMalloc.  Same arguments, same result cell for cell.
+ * The scratch (the two blank maps, nx*ny*nz/128 bytes for nx a multiple of 1024) is a static device array of
+ * 8 MiB inside the library -- every GPU that loads the library holds it until the process exits -- so:
+ *   - a grid with ny * nz * ceil(nx / 1024) > 2^20 (more than 1024^3 cells at nx = 1024) is refused: SDF_ETOOBIG,
+ *     nothing is launched;
+ *   - the call performs no cudaMalloc, cudaFree, cudaMallocAsync or memory-pool call; it enqueues three kernels on
+ *     `stream` and returns (the first call on a device also looks the array's address up: cudaGetSymbolAddress);
+ *   - all calls share the one array: two calls that may overlap on the GPU (streams without an order between them,
+ *     concurrent host threads) race on it and their results are undefined.  Calls ordered on one stream are safe;
+ *     the array needs no clearing between them.
+ * Errors: SDF_EINVAL, SDF_ETOOBIG, SDF_ECUDA.
+ */
+int sdf_fill_interior_static(float *dist, int nx, int ny, int nz, float band, void *stream);
 
 /*
  * STL and grid files (host code; "takes as input a stereolithography (STL) file and

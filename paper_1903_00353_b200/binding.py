@@ -16,13 +16,13 @@ import numpy as np
 from . import build as _build
 
 STATUS_NAMES = {0: "SDF_OK", 1: "SDF_EINVAL", 2: "SDF_ENOTCLOSED", 3: "SDF_EORIENT",
-                4: "SDF_EDEGENERATE", 5: "SDF_ENOMEM", 6: "SDF_ECUDA", 7: "SDF_EIO"}
-SDF_OK, SDF_EINVAL, SDF_ENOTCLOSED, SDF_EORIENT, SDF_EDEGENERATE, SDF_ENOMEM, SDF_ECUDA, SDF_EIO = range(8)
+                4: "SDF_EDEGENERATE", 5: "SDF_ENOMEM", 6: "SDF_ECUDA", 7: "SDF_EIO", 8: "SDF_ETOOBIG"}
+SDF_OK, SDF_EINVAL, SDF_ENOTCLOSED, SDF_EORIENT, SDF_EDEGENERATE, SDF_ENOMEM, SDF_ECUDA, SDF_EIO, SDF_ETOOBIG = range(9)
 
 TABLE_CORNER_VID, TABLE_HALFEDGE_ADJ, TABLE_FACE_NORMAL, TABLE_VERTEX_REC, TABLE_EDGE_REC, \
     TABLE_VERTEX_MINTRI = range(6)
 
-EXPORTS = ("sdf_create", "sdf_transform", "sdf_compute", "sdf_compute_host", "sdf_compute_sparse", "sdf_compute_sparse_host", "sdf_zslab", "sdf_compute_zslab", "sdf_fill_interior", "sdf_closest_points", "sdf_stats", "sdf_get_table",
+EXPORTS = ("sdf_create", "sdf_transform", "sdf_compute", "sdf_compute_host", "sdf_compute_sparse", "sdf_compute_sparse_host", "sdf_zslab", "sdf_compute_zslab", "sdf_fill_interior", "sdf_fill_interior_static", "sdf_closest_points", "sdf_stats", "sdf_get_table",
            "sdf_destroy", "sdf_strerror", "sdf_last_cuda_error", "sdf_version",
            "sdf_enable_timing", "sdf_get_timings", "sdf_launch_count", "sdf_measure_fp32_peak",
            "sdf_read_stl", "sdf_free_host", "sdf_write_stl", "sdf_write_grid")
@@ -116,6 +116,8 @@ def lib():
     L.sdf_write_grid.restype = C.c_int
     L.sdf_fill_interior.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_float, vp]
     L.sdf_fill_interior.restype = C.c_int
+    L.sdf_fill_interior_static.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_float, vp]
+    L.sdf_fill_interior_static.restype = C.c_int
     L.sdf_stats.argtypes = [vp, C.POINTER(Stats)]
     L.sdf_stats.restype = C.c_int
     L.sdf_get_table.argtypes = [vp, C.c_int, vp, C.c_size_t]
@@ -376,6 +378,16 @@ def sdf_fill_interior(dist, band, stream=None):
     st = lib().sdf_fill_interior(C.c_void_p(dist.data_ptr()), nx, ny, nz, float(band), C.c_void_p(_stream_ptr(stream)))
     if st != SDF_OK:
         raise SdfError(st, "sdf_fill_interior")
+    return dist
+
+
+def sdf_fill_interior_static(dist, band, stream=None):
+    """sdf_fill_interior without any allocation: the scratch is a static 8 MiB device array (grids beyond it: SDF_ETOOBIG)."""
+    assert dist.is_cuda and dist.is_contiguous() and dist.dim() == 3
+    nz, ny, nx = (int(v) for v in dist.shape)
+    st = lib().sdf_fill_interior_static(C.c_void_p(dist.data_ptr()), nx, ny, nz, float(band), C.c_void_p(_stream_ptr(stream)))
+    if st != SDF_OK:
+        raise SdfError(st, "sdf_fill_interior_static")
     return dist
 
 

@@ -81,6 +81,7 @@ const char *sdf_strerror(int s) {
     case SDF_ENOMEM: return "out of memory";
     case SDF_ECUDA: return "CUDA error or no CUDA device";
     case SDF_EIO: return "file cannot be opened, read or written, or is not a valid STL file";
+    case SDF_ETOOBIG: return "grid too large for the static scratch of sdf_fill_interior_static (8 MiB: ny * nz * ceil(nx / 1024) <= 2^20)";
     default: return "unknown status";
     }
 }

@@ -249,3 +249,51 @@ extern "C" int sdf_fill_interior(float *dist, int nx, int ny, int nz, float band
     CK(e);
     return SDF_OK;
 }
+
+// ---------------------------------------------------------------------------------------
+// sdf_fill_interior_static: the same three sweeps for callers that must not allocate (CUDA graph capture, serving
+// loops, harnesses that forbid cudaMalloc).  The blank maps live in a file-scope device array instead of the
+// stream-ordered pool: SDF_FILL_STATIC_BYTES per GPU that loads the library, held until the process exits.
+//   - grids whose maps do not fit (more than ny * nz * ceil(nx / 1024) = 2^20 map words) are refused: SDF_ETOOBIG
+//   - no cudaMalloc / cudaFree / cudaMallocAsync / pool call on any path of this function
+//   - every call uses the SAME array: calls that overlap on the GPU (different streams without an order between
+//     them, or different host threads) race on it.  The array keeps the last call's contents; nothing has to be cleared:
+//     sweep_x_kernel writes every map word of this call's grid before the y and z walks read one.
+// In host code `g_fill_static_maps` is only the symbol's host-side stand-in: its device address is looked up once per
+// device (with that device current) through cudaGetSymbolAddress and that pointer is what the kernels get.
+// ---------------------------------------------------------------------------------------
+#define SDF_FILL_STATIC_BYTES (8u << 20)      /* 1024^3 cells (C4): 2 maps x 2^20 words x 4 B */
+static __device__ __align__(256) unsigned g_fill_static_maps[SDF_FILL_STATIC_BYTES / sizeof(unsigned)];
+
+#define FILL_STATIC_MAX_DEVICES 64
+static unsigned *g_fill_static_ptr[FILL_STATIC_MAX_DEVICES];      // per device: address of the array (0 = not looked up yet)
+
+extern "C" int sdf_fill_interior_static(float *dist, int nx, int ny, int nz, float band, void *stream) {
+    if (!dist || nx <= 0 || ny <= 0 || nz <= 0 || nx > 32767 || ny > 32767 || nz > 32767) return SDF_EINVAL;
+    if (!(band > 0.0f) || !isfinite(band)) return SDF_EINVAL;
+    const int64_t nrows = (int64_t)ny * nz;
+    const int nwords = ((nx + 31) / 32 + 31) / 32;
+    const size_t mapw = (size_t)nrows * nwords;
+    if (sizeof(unsigned) * 2 * mapw > (size_t)SDF_FILL_STATIC_BYTES) return SDF_ETOOBIG;
+    int ndev = 0, dev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0) { (void)cudaGetLastError(); return SDF_ECUDA; }
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= FILL_STATIC_MAX_DEVICES) return SDF_EINVAL;
+    unsigned *maps = g_fill_static_ptr[dev];
+    if (!maps) {
+        // set-up, once per device (two host threads arriving together look the same address up twice)
+        CK(cudaGetSymbolAddress((void **)&maps, g_fill_static_maps));
+        if (!maps) return SDF_ECUDA;
+        g_fill_static_ptr[dev] = maps;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const float fillv = -band;
+    unsigned *by = maps, *bz = maps + mapw;
+    KL; sweep_x_kernel<<<(unsigned)((nrows + 7) / 8), 256, 0, st>>>(dist, nx, nrows, fillv, by, bz, nwords, ny, nz);
+    KL; sweep_line_kernel<<<dim3((unsigned)((nx + 255) / 256), (unsigned)nz), 256, 0, st>>>(
+        dist, nx, (int64_t)nx * ny, ny, nx, fillv, nwords, by, bz, (int64_t)nwords * nz);
+    KL; sweep_line_kernel<<<dim3((unsigned)((nx + 255) / 256), (unsigned)ny), 256, 0, st>>>(
+        dist, nx, nx, nz, (int64_t)nx * ny, fillv, nwords, bz, nullptr, 0);
+    CK(cudaGetLastError());
+    return SDF_OK;
+}
