@@ -186,6 +186,9 @@ static int make_grid(const float origin[3], float h, int nx, int ny, int nz, flo
     g->fill_depth = fd ? atoi(fd) : 2;
     g->fill_issuers = fi ? atoi(fi) : 1;
     if (g->fill_issuers < 1 || g->fill_issuers > 4) g->fill_issuers = 1;
+    const char *ec = getenv("SDF_EVAL_CHUNK");
+    g->eval_chunk = ec ? atoi(ec) : 256;            // SDF_EVAL_CHUNK=0: faces, then wedges, then cones (C5: 3.99 against 3.95 ms)
+    if (g->eval_chunk < 0 || g->eval_chunk > (1 << 20)) g->eval_chunk = 256;
     const char *sh = getenv("SDF_SCRATCH_HINT");
     g->scratch_hint = (sh && sh[0] == '0') ? 0 : 1;
     const char *fck = getenv("SDF_FILL_CHUNK_LOG2");

@@ -261,6 +261,30 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
     }
 }
 
+// The order in which the warps of evaluate_small_kernel take the polyhedra.  The index space is [faces | wedges | cones],
+// each class roughly along the Morton order of the triangles; taken front to back the grid is swept three times and a
+// scratch sector has left L2 (the sentinel fill streams through it meanwhile) before the next class comes by.  So the
+// warps are dealt out in `chunks` rounds: round k takes the k-th part of the faces, of the wedges and of the cones --
+// one sweep over space, the three classes of a region close together in time.
+struct EvalOrder {
+    int64_t chunks;         // 0: plain order
+    int64_t wf, we, wc;     // warps per round for faces / wedges / cones
+    __device__ __forceinline__ int64_t poly_of(int64_t W, int ppw, int lane, const MeshView &mv) const {
+        if (lane >= ppw) return -1;
+        if (!chunks) {
+            const int64_t p = W * ppw + lane;
+            return p < mv.P ? p : -1;
+        }
+        const int64_t per = wf + we + wc, k = W / per, r = W - k * per;
+        int64_t lo, hi, wi;
+        if (r < wf) { wi = k * wf + r; lo = 0; hi = mv.F; }
+        else if (r < wf + we) { wi = k * we + (r - wf); lo = mv.F; hi = (int64_t)mv.F + mv.E; }
+        else { wi = k * wc + (r - wf - we); lo = (int64_t)mv.F + mv.E; hi = mv.P; }
+        const int64_t p = lo + wi * ppw + lane;
+        return p < hi ? p : -1;
+    }
+};
+
 #define ES_WARPS 4
 #ifndef ES_MINB
 #define ES_MINB 9
@@ -270,17 +294,17 @@ __global__ void __launch_bounds__(32 * ES_WARPS, SERIAL ? 1 : ES_MINB) evaluate_
                                                                        u32 *__restrict__ big_list,
                                                                        const int *__restrict__ table,
                                                                        u64 *__restrict__ scratch, u64 *__restrict__ ctr,
-                                                                       int ppw) {
+                                                                       int ppw, EvalOrder eo) {
     // ppw = polyhedra per warp: 32, or fewer when the mesh has few polyhedra (more warps for the
     // same rows: a mesh of 1e5 medium polyhedra otherwise leaves each scheduler 5 long-running warps)
     __shared__ float s_rec[ES_WARPS][32][RR_WORDS];
     __shared__ int s_ex[ES_WARPS][33];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int64_t p = ((int64_t)blockIdx.x * ES_WARPS + w) * ppw + lane;
+    const int64_t p = eo.poly_of((int64_t)blockIdx.x * ES_WARPS + w, ppw, lane, mv);
     int rows = 0;
     bool live = false, direct = false;
     PolyHdr Hd;
-    if (lane < ppw && p < mv.P) {
+    if (p >= 0) {
         PolyHdr H;
         live = poly_aabv(mv, g, p, H);
         if (live) {
@@ -883,14 +907,23 @@ int run_compute(sdf_mesh *m, const GridParams &g_in, float *dist, int *tri, cuda
     if (bricks) {
         stage_mark(m, SDF_T_EVALUATE, 0, st);
         const int ppw = P < (1 << 17) ? 4 : (P < (1 << 20) ? 8 : 32);
-        const int64_t nblk = (P + (int64_t)ppw * ES_WARPS - 1) / ((int64_t)ppw * ES_WARPS);
+        int64_t nblk = (P + (int64_t)ppw * ES_WARPS - 1) / ((int64_t)ppw * ES_WARPS);
+        EvalOrder eo = {0, 0, 0, 0};
+        if (g.eval_chunk > 0 && (mv.E > 0 || mv.NC > 0) && P >= (1 << 17)) {
+            const int64_t nf = (mv.F + ppw - 1) / ppw, ne = ((int64_t)mv.E + ppw - 1) / ppw, nc = ((int64_t)mv.NC + ppw - 1) / ppw;
+            int64_t K = (nf + ne + nc) / g.eval_chunk;
+            if (K < 1) K = 1;
+            eo.chunks = K;
+            eo.wf = (nf + K - 1) / K; eo.we = (ne + K - 1) / K; eo.wc = (nc + K - 1) / K;
+            nblk = (K * (eo.wf + eo.we + eo.wc) + ES_WARPS - 1) / ES_WARPS;
+        }
         const unsigned split = P < 65536 ? EBIG_SPLIT : (P < (1 << 20) ? 2 : 1);
         if (g.cdp) {
             CKS(run_cdp_evaluate(m, mv, g, st));
         } else {
         KL;
-        if (g.serial_loop) evaluate_small_kernel<true><<<(unsigned)nblk, 32 * ES_WARPS, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr, ppw);
-        else evaluate_small_kernel<false><<<(unsigned)nblk, 32 * ES_WARPS, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr, ppw);
+        if (g.serial_loop) evaluate_small_kernel<true><<<(unsigned)nblk, 32 * ES_WARPS, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr, ppw, eo);
+        else evaluate_small_kernel<false><<<(unsigned)nblk, 32 * ES_WARPS, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr, ppw, eo);
         KL; evaluate_big_kernel<<<dim3((unsigned)(sms * 4 / split), split), EBIG_BT, 0, st>>>(mv, g, m->big_list, m->brick_table, m->scratch, m->d_ctr);
         }
         stage_mark(m, SDF_T_EVALUATE, 1, st);
