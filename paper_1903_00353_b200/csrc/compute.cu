@@ -813,8 +813,7 @@ static int scan_bricks(sdf_mesh *m, const GridParams &g, cudaStream_t ps, bool m
 // sdf_transform, before build_features forks the vertex stream (tile builder: the marking kernel runs later)
 int maybe_alloc_brick_ws(sdf_mesh *m, cudaStream_t st) {
     if (!m->hoist_g) return SDF_OK;
-    CKS(alloc_brick_ws(m, *m->hoist_g, st));
-    return reset_bricks(m, *m->hoist_g, st);
+    return alloc_brick_ws(m, *m->hoist_g, st);          // (the resets go with the marking kernel: maybe_prepare_bricks)
 }
 
 // sdf_transform, global builder: workspace + reset on `st`, and a device copy of the grid for tri_geom_kernel, which
@@ -836,6 +835,7 @@ int maybe_prepare_bricks(sdf_mesh *m, cudaStream_t st, cudaStream_t vs, bool mar
     const GridParams *g = m->hoist_g;
     m->hoist_g = nullptr;
     (void)st;
+    if (!marked) CKS(reset_bricks(m, *g, vs));          // off the caller's stream: two fewer operations in front of the edge stage
     CKS(scan_bricks(m, *g, vs, marked));
     stage_mark(m, SDF_T_CLIP_SCAN, 1, vs);
     m->bricks_ready = true;        // the total travels with the validation flags (the host crossing)

@@ -267,9 +267,13 @@ __global__ void __launch_bounds__(FB, TG_MINB) tri_geom_kernel(const float *__re
                                                       float *__restrict__ fn, u64 *__restrict__ vacc,
                                                       u32 *etab, u32 emask, int *__restrict__ flags,
                                                       const GridParams *__restrict__ mark_g,
-                                                      unsigned char *__restrict__ brick_flag) {
+                                                      unsigned char *__restrict__ brick_flag,
+                                                      int *__restrict__ adj, float *__restrict__ fsm) {
     int t = blockIdx.x * FB + threadIdx.x;
     if (t >= F) return;
+    // what the pairing kernel (next on this stream) expects: no partner yet, no smooth edge absorbed yet
+    adj[3 * (size_t)t] = -1; adj[3 * (size_t)t + 1] = -1; adj[3 * (size_t)t + 2] = -1;
+    fsm[t] = 0.0f;
     const float *T = soup + 9 * (size_t)t;
     int v[3];
 #pragma unroll
@@ -592,9 +596,21 @@ static int fork_vertex_stream(sdf_mesh *m, cudaStream_t st, cudaStream_t *vs_out
 // sdf_transform, the brick total of the hoisted A6a)
 static int finish_features(sdf_mesh *m, int nc, int vcap, TmpPool &tmp, cudaStream_t st) {
     int hflags[4] = {0, 0, 0, 0};
-    CK(cudaMemcpyAsync(hflags, m->d_flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(m->h_ctr, m->d_ctr, sizeof(u64) * CTR_COUNT, cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
+    {
+        // counters and flags are adjacent in the slab: one copy
+        const size_t span = (size_t)((char *)(m->d_flags + 4) - (char *)m->d_ctr);
+        u64 both[CTR_TOTAL + 64];
+        if (span <= sizeof(both) && (char *)m->d_flags > (char *)m->d_ctr) {
+            CK(cudaMemcpyAsync(both, m->d_ctr, span, cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+            memcpy(m->h_ctr, both, sizeof(u64) * CTR_COUNT);
+            memcpy(hflags, (char *)both + ((char *)m->d_flags - (char *)m->d_ctr), sizeof(hflags));
+        } else {
+            CK(cudaMemcpyAsync(hflags, m->d_flags, sizeof(hflags), cudaMemcpyDeviceToHost, st));
+            CK(cudaMemcpyAsync(m->h_ctr, m->d_ctr, sizeof(u64) * CTR_COUNT, cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+        }
+    }
     int status = status_from_flags(hflags[0]);
     m->V = (int64_t)(m->h_ctr[CTR_V] < (u64)vcap ? m->h_ctr[CTR_V] : (u64)vcap);
     m->Elive = (int64_t)m->h_ctr[CTR_ELIVE];
@@ -683,8 +699,7 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
         m->hoist_g_dev = c.take<GridParams>(1);
         if (pass == 0) CKS(dev_alloc(al, &m->slab_f, c.off, st));
     }
-    CK(cudaMemsetAsync(m->d_ctr, 0, sizeof(u64) * CTR_TOTAL, st));
-    CK(cudaMemsetAsync(m->d_flags, 0, sizeof(int) * 4, st));
+    CK(cudaMemsetAsync(m->d_ctr, 0, (size_t)((char *)(m->d_flags + 4) - (char *)m->d_ctr), st));      // counters and flags: adjacent
 
     // smooth features get no polyhedron of their own (common.cuh, SMOOTH_SIN_DEFAULT); SDF_SMOOTH_SIN=0 switches that off
     float smooth_sin = SMOOTH_SIN_DEFAULT;
@@ -733,8 +748,6 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
         StreamDrain mdrain;
         if (ow.on) CKS(fork_vertex_stream(m, st, &ms, mdrain));        // (small meshes: the fork costs more than it hides)
         CK(cudaMemsetAsync(wtab, 0xFF, (size_t)((char *)(etab + cape) - (char *)wtab), ms));
-        CK(cudaMemsetAsync(m->adj, 0xFF, sizeof(int) * 3 * F, ms));
-        CK(cudaMemsetAsync(m->fsm, 0, sizeof(float) * (size_t)F, ms));
         CKS(order_triangles(src, F, ow, (u32 *)m->perm, st));
         if (ms != st) {
             CK(cudaEventRecord(m->ev_join, ms));
@@ -761,7 +774,7 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
     if (F >= ((int64_t)1 << 21)) CKS(maybe_begin_bricks(m, st, &mark_g, &mark_flag));   // (big triangles mark hundreds of bricks per thread: C5 loses 0.14 ms)
     else CKS(maybe_alloc_brick_ws(m, st));
     KL; tri_geom_kernel<<<blocks_for(F), FB, 0, st>>>(m->soup, wvid, slot, (int)F, m->cvid, m->fn, vacc, etab, cape - 1, m->d_flags,
-                                                    mark_g, mark_flag);
+                                                    mark_g, mark_flag, m->adj, m->fsm);
     // the vertex stage needs only what tri_geom wrote: it runs on a second stream beside the edge stage
     // (and A6a -- brick marks unless tri_geom made them, scan -- on a third one: it needs the soup and the normals only)
     cudaStream_t vs = st, bs = st;
