@@ -194,6 +194,11 @@ struct Carver {
     }
 };
 
+// the library's fork / join events come from a process-wide pool (creating and destroying five per handle was a tenth of
+// the host time of a small sdf_transform); thread-safe; an event goes back when its handle is destroyed
+int ev_get(cudaEvent_t *e);          // no-op if *e is set already
+void ev_put(cudaEvent_t *e);
+
 // allocation through the handle's allocator
 int dev_alloc(const sdf_allocator *a, void **p, size_t bytes, cudaStream_t st);
 void dev_free(const sdf_allocator *a, void *p, cudaStream_t st);

@@ -165,7 +165,8 @@ __global__ void __launch_bounds__(FB) ingest_weld_kernel(const float *__restrict
                                                          int *__restrict__ vcorner, u64 *__restrict__ vacc,
                                                          long long *__restrict__ vcosq, long long *__restrict__ vcospos,
                                                          int *__restrict__ vside, int *__restrict__ vmint, int vcap,
-                                                         u64 *ctr, int *__restrict__ flags) {
+                                                         u64 *ctr, int *__restrict__ flags, int *__restrict__ perm_identity) {
+    // perm == nullptr: the internal order is the caller's (small meshes are not sorted) and perm_identity is filled here
     __shared__ u32 s_nins, s_base;
     if (threadIdx.x == 0) s_nins = 0;
     __syncthreads();
@@ -174,7 +175,8 @@ __global__ void __launch_bounds__(FB) ingest_weld_kernel(const float *__restrict
     u32 h = 0;
     if (c < ncorner) {
         const int i = c / 3, k = c - 3 * i;
-        const int t = perm[i];
+        const int t = perm ? perm[i] : i;
+        if (!perm && k == 0) perm_identity[i] = i;
         const float *p = in + 9 * (size_t)t + 3 * k;
         float x = p[0], y = p[1], z = p[2];
         if (!(isfinite(x) && isfinite(y) && isfinite(z))) atomicOr(flags, ERRB_NONFINITE);
@@ -191,7 +193,7 @@ __global__ void __launch_bounds__(FB) ingest_weld_kernel(const float *__restrict
                 if (cur == EMPTY32) { inserted = true; break; }
             }
             const int ci = (int)cur / 3, ck = (int)cur - 3 * ci;
-            const float *q = in + 9 * (size_t)perm[ci] + 3 * ck;
+            const float *q = in + 9 * (size_t)(perm ? perm[ci] : ci) + 3 * ck;
             if (canon_bits(q[0]) == bx && canon_bits(q[1]) == by && canon_bits(q[2]) == bz) break;
             wtab_next(wt, bx, by, bz, h, np);
         }
@@ -577,14 +579,14 @@ static int fork_vertex_stream(sdf_mesh *m, cudaStream_t st, cudaStream_t *vs_out
         CK(cudaStreamCreateWithFlags(&g_bs, cudaStreamNonBlocking));
         g_vs_dev = dev;
     }
-    if (!m->ev_fork) CK(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
-    if (!m->ev_join) CK(cudaEventCreateWithFlags(&m->ev_join, cudaEventDisableTiming));
+    CKS(ev_get(&m->ev_fork));
+    CKS(ev_get(&m->ev_join));
     CK(cudaEventRecord(m->ev_fork, st));
     CK(cudaStreamWaitEvent(g_vs, m->ev_fork, 0));
     drain.s = g_vs; drain.armed = true;
     *vs_out = g_vs;
     if (bs_out && bdrain && m->hoist_g) {
-        if (!m->ev_bjoin) CK(cudaEventCreateWithFlags(&m->ev_bjoin, cudaEventDisableTiming));
+        CKS(ev_get(&m->ev_bjoin));
         CK(cudaStreamWaitEvent(g_bs, m->ev_fork, 0));
         bdrain->s = g_bs; bdrain->armed = true;
         *bs_out = g_bs;
@@ -748,7 +750,7 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
         StreamDrain mdrain;
         if (ow.on) CKS(fork_vertex_stream(m, st, &ms, mdrain));        // (small meshes: the fork costs more than it hides)
         CK(cudaMemsetAsync(wtab, 0xFF, (size_t)((char *)(etab + cape) - (char *)wtab), ms));
-        CKS(order_triangles(src, F, ow, (u32 *)m->perm, st));
+        if (ow.on) CKS(order_triangles(src, F, ow, (u32 *)m->perm, st));      // (not sorted: ingest_weld_kernel fills the identity)
         if (ms != st) {
             CK(cudaEventRecord(m->ev_join, ms));
             CK(cudaStreamWaitEvent(st, m->ev_join, 0));
@@ -760,8 +762,8 @@ static int build_features_global(sdf_mesh *m, const float *tri, int on_device, c
         const char *ul = getenv("SDF_UNIFORM_TABLES");
         if (ow.on && !(ul && ul[0] == '1') && capw >= 4096) wt.scale = (u32)((((u64)capw - 1024) << 12) / (u64)F);
     }
-    KL; ingest_weld_kernel<<<blocks_for(nc), FB, 0, st>>>(src, m->perm, nc, m->soup, m->inv_perm, wt, slot, wvid, vcorner,
-                                                        vacc, vcosq, vcospos, vside, m->vmint, vcap, m->d_ctr, m->d_flags);
+    KL; ingest_weld_kernel<<<blocks_for(nc), FB, 0, st>>>(src, ow.on ? m->perm : nullptr, nc, m->soup, m->inv_perm, wt, slot, wvid, vcorner,
+                                                        vacc, vcosq, vcospos, vside, m->vmint, vcap, m->d_ctr, m->d_flags, m->perm);
     stage_mark(m, SDF_T_INGEST_WELD, 1, st);
 
     // ---- A3 (per triangle), A2 edge table
