@@ -112,6 +112,9 @@ __device__ __forceinline__ void cell_range(float mn, float mx, float o, float in
 // those four boxes per triangle (corners + normal only) covers every cell the evaluation can touch.
 __device__ __forceinline__ void mark_box(const GridParams &g, const float *mn, const float *mx,
                                          unsigned char *__restrict__ brick_flag) {
+    // a non-finite corner (the soup is being rejected with SDF_EINVAL anyway) would turn into whole-axis ranges: a thread
+    // walking every brick of the grid, per such triangle
+    if (!isfinite(mn[0] + mn[1] + mn[2] + mx[0] + mx[1] + mx[2])) return;
     int i0, i1, j0, j1, k0, k1;
     cell_range(mn[0], mx[0], g.ox, g.inv_h, g.nx, i0, i1);
     cell_range(mn[1], mx[1], g.oy, g.inv_h, g.ny, j0, j1);

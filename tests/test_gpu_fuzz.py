@@ -182,3 +182,30 @@ def test_mass_defects_stay_in_bounds(oracle_mod, name, scale):
         assert torch.equal(t0, t1) and torch.equal(d0.view(torch.int32), d1.view(torch.int32)), vi
         m1.destroy()
     m0.destroy()
+
+
+def test_many_non_finite_triangles_are_rejected_quickly():
+    """ADVICE r1 (features.cu first crossing): a soup full of Inf / NaN corners is flagged by the ingest kernel, but
+    sdf_transform's hoisted brick marking still sees it -- a non-finite box must not turn into a walk over every brick
+    of the grid per triangle.  SDF_EINVAL, in milliseconds, and a valid mesh afterwards is untouched."""
+    import time
+    from paper_1903_00353_b200 import binding as B
+    w = f32_grid(W.config("C2"))
+    good = np.ascontiguousarray(w.soup)
+    m0, d0, t0 = B.compute_workload(w)
+    torch.cuda.synchronize()
+    r = np.random.default_rng(99)
+    for bad_value in (np.inf, -np.inf, np.nan):
+        s = good.copy()
+        hit = r.random(len(s)) < 0.5
+        s[hit, r.integers(0, 3, hit.sum()), r.integers(0, 3, hit.sum())] = bad_value
+        t_start = time.perf_counter()
+        with pytest.raises(B.SdfError) as e:
+            B.sdf_transform(torch.from_numpy(s).cuda(), w.origin, w.h, w.dims, w.band)
+        torch.cuda.synchronize()
+        assert e.value.status == B.SDF_EINVAL
+        assert time.perf_counter() - t_start < 2.0
+    m1, d1, t1 = B.compute_workload(w)
+    torch.cuda.synchronize()
+    assert torch.equal(t0, t1) and torch.equal(d0.view(torch.int32), d1.view(torch.int32))
+    m0.destroy(); m1.destroy()
