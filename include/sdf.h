@@ -28,7 +28,7 @@
  * SDF_CREATE_FORK=0 (vertex stage on the caller's stream), SDF_SMOOTH_SIN=x (edges / vertices whose normals span less
  * than asin(x) get no wedge / cone of their own, their faces' prisms are widened instead; default 1/32, 0 = off), SDF_FILLINT_PLAIN=1 (interior fill without the blank map);
  * SDF_FILL_SM_SHARE=1..8 / SDF_FILL_CHUNK_LOG2=11..14 / SDF_FILL_ISSUERS=1..4 / SDF_FILL_DEPTH / SDF_SCRATCH_HINT=0 (sentinel-fill and scratch
- * ablations); SDF_EVAL_CHUNK=n (warps per round in which faces, wedges and cones of a region are evaluated together; 0 = class after class);
+ * ablations); SDF_ROW_CLIP=n (rows longer than n cells are clipped analytically before the walk; default 2), SDF_EVAL_CHUNK=n (warps per round in which faces, wedges and cones of a region are evaluated together; 0 = class after class);
  * see DESIGN.md.
  */
 #ifndef PAPER_1903_00353_SDF_H

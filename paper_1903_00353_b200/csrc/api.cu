@@ -212,6 +212,9 @@ static int make_grid(const float origin[3], float h, int nx, int ny, int nz, flo
     g->fill_depth = fd ? atoi(fd) : 2;
     g->fill_issuers = fi ? atoi(fi) : 1;
     if (g->fill_issuers < 1 || g->fill_issuers > 4) g->fill_issuers = 1;
+    const char *rcl = getenv("SDF_ROW_CLIP");
+    g->row_clip = rcl ? atoi(rcl) : 2;              // (8, the first setting: C4 3.15 against 3.13 ms, C3 0.379 / 0.370, C2 0.248 / 0.241)
+    if (g->row_clip < 0 || g->row_clip > 1024) g->row_clip = 2;
     const char *ec = getenv("SDF_EVAL_CHUNK");
     g->eval_chunk = ec ? atoi(ec) : 256;            // SDF_EVAL_CHUNK=0: faces, then wedges, then cones (C5: 3.99 against 3.95 ms)
     if (g->eval_chunk < 0 || g->eval_chunk > (1 << 20)) g->eval_chunk = 256;

@@ -81,7 +81,7 @@ struct BrickOut {
 // ---- small polyhedra: compact record + incremental scan conversion of a grid row.
 // Along a grid row every half-space test of PAPER.md:246-252 is linear in the cell index,
 // s(di) = base + di * g, so a row costs one set-up (the j,k terms) and one FMA + compare per
-// plane and cell; rows longer than ROW_CLIP_NI cells are first clipped analytically (a convex
+// plane and cell; rows longer than g.row_clip cells (2; SDF_ROW_CLIP) are first clipped analytically (a convex
 // body meets a line in one interval).  Cells that pass get the distance from the canonical
 // expressions (cell position by one fmaf, differences first, dot_rn), so a distance does not
 // depend on which path evaluated it.
@@ -95,7 +95,6 @@ struct BrickOut {
 #define RR_INV_NJ 27     // float 1 / nj
 #define RR_TIDX 28       // faces: internal triangle index (the eps-margin path re-reads the corners)
 #define RR_WORDS 29      // odd stride: records of different owners fall in different banks
-#define ROW_CLIP_NI 8
 
 __device__ __forceinline__ void build_row_record(const MeshView &mv, const GridParams &g, int64_t p, const PolyHdr &H,
                                                  float *rec) {
@@ -176,7 +175,7 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
         const float b1 = fmaf(m1.x, rx0, fmaf(m1.y, ry, m1.z * rz)) - rec[15], g1 = m1.x * h;
         const float b2 = fmaf(m2.x, rx0, fmaf(m2.y, ry, m2.z * rz)) - rec[16], g2 = m2.x * h;
         const float bn = fmaf(n.x, rx0, fmaf(n.y, ry, n.z * rz)), gn = n.x * h;
-        if (ni > ROW_CLIP_NI && !g.aabb_mode) {
+        if (ni > g.row_clip && !g.aabb_mode) {
             float lo = 0.0f, hi = (float)db;
             clip_lin(b0, g0, t0, lo, hi); clip_lin(b1, g1, t1, lo, hi); clip_lin(b2, g2, t2, lo, hi);
             clip_lin(bn, gn, reach, lo, hi); clip_lin(-bn, -gn, reach, lo, hi);
@@ -212,7 +211,7 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
         const float bt = fmaf(u.x, rx0, fmaf(u.y, ry, u.z * rz)), gt = u.x * h;
         const float b1 = fmaf(w1.x, rx0, fmaf(w1.y, ry, w1.z * rz)), g1 = w1.x * h;
         const float b2 = fmaf(w2.x, rx0, fmaf(w2.y, ry, w2.z * rz)), g2 = w2.x * h;
-        if (ni > ROW_CLIP_NI) {
+        if (ni > g.row_clip) {
             float lo = 0.0f, hi = (float)db;
             clip_lin(bt, gt, eps, lo, hi); clip_lin(L - bt, -gt, eps, lo, hi);
             clip_lin(b1, g1, eps, lo, hi); clip_lin(b2, g2, eps, lo, hi);
