@@ -533,6 +533,13 @@ __device__ __forceinline__ CellOut finish_cell(const MeshView &mv, const GridPar
         V3<double> Q;
         double D = tri_closest<double>(X - A, E0, EC, Nn, rg, Q);
         if (!(D < g.dband)) return o;                         // strictly inside the band
+        // a distance that fp64 cannot tell from zero (a cell centre on a vertex, an edge, a face: |n . r| of an in-plane r is
+        // rounding noise of ~1e-16 |r|) is zero, and a zero has no sign -- not -1e-17 or +1e-17 by the luck of the rounding
+        {
+            const V3<double> R = X - A;
+            const double scale = fabs(R.x) + fabs(R.y) + fabs(R.z) + fabs(E0.x) + fabs(E0.y) + fabs(E0.z) + fabs(EC.x) + fabs(EC.y) + fabs(EC.z);
+            if (D <= 4e-15 * scale) D = 0.0;
+        }
         V3<double> PN;
         if (rg == RG_FACE) PN = Nn;
         else if (rg <= RG_E2) PN = ld3d(N) + ld3d(mv.fn + 3 * (size_t)(mv.adj[3 * (size_t)t + (rg - RG_E0)] / 3));

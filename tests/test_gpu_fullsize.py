@@ -138,3 +138,58 @@ def test_scale_36m_triangles():
     assert st["edges_convex"] + st["edges_concave"] + st["edges_flat"] == st["E"]
     _whole_grid_properties(w, d, tr, st)
     assert abs(st["band_cells"] - 5_186_000) < 2_000          # C4's surface, C4's band
+
+
+def test_grid_with_more_than_2_to_32_cells(oracle_mod):
+    """A 1664 x 1664 x 1600 grid (4.43e9 cells > 2^32; 35 GB of output): linear cell indices need 64 bits in the fill, the
+    emit pass, the sparse output and the closest-point pass.  A small sphere sits at the far corner, so every populated
+    cell has a linear index beyond 2^32.  Grid spacing and origin are powers of two: a crop of the grid has bit-identical
+    cell positions, so the window around the sphere must equal a compute of that window alone bit for bit, which in turn is
+    compared with the oracle; everything outside the window must be sentinels."""
+    from paper_1903_00353_b200 import binding as B
+    nx, ny, nz = 1664, 1664, 1600
+    h = 2.0 ** -10
+    v, t = W.icosphere_mesh(3, 28 * h)
+    centre = np.array([(nx - 48) * h, (ny - 48) * h, (nz - 48) * h])
+    soup = W.soup_from_indexed(v + centre, t, np.random.default_rng(5))
+    w = f32_grid(W.Workload("huge", soup, (0.0, 0.0, 0.0), h, (nx, ny, nz), 3 * h))
+    assert nx * ny * nz > 2 ** 32
+    m, d, tr = B.compute_workload(w)
+    torch.cuda.synchronize()
+    lo = (nx - 96, ny - 96, nz - 96)
+    c = w.crop(lo, (96, 96, 96))
+    # the window against the oracle
+    om = oracle_mod.Mesh(c.soup)
+    dref, tref = om.sdf(c.origin, c.h, c.dims, c.band)
+    dwin = d[lo[2]:, lo[1]:, lo[0]:].contiguous().cpu().numpy()
+    twin = tr[lo[2]:, lo[1]:, lo[0]:].contiguous().cpu().numpy()
+    # the tolerance is the whole grid's (1e-5 h + 1e-6 diag: the window's coordinates are ~1.6, not ~0.1)
+    import types
+    cw = types.SimpleNamespace(h=c.h, band=c.band, diag=w.diag, ntri=c.ntri, dims=c.dims, origin=c.origin)
+    res = compare_to_oracle(dwin, twin, dref, tref, cw, om)
+    assert res["ok"], str({k: v for k, v in res.items() if not isinstance(v, (list, np.ndarray))})
+    populated = int(np.isfinite(dref).sum())
+    assert populated > 20000
+    # ... and against the same window computed alone (bit for bit)
+    m2, d2, t2 = B.compute_workload(c)
+    torch.cuda.synchronize()
+    assert np.array_equal(d2.cpu().numpy().view(np.int32), dwin.view(np.int32)) and np.array_equal(t2.cpu().numpy(), twin)
+    # nothing populated outside the window, and sentinels everywhere else (also in the first cells and past index 2^32)
+    assert int(torch.isfinite(d).sum()) == int(np.isfinite(dwin).sum())
+    assert int((tr >= 0).sum()) == int((twin >= 0).sum())
+    flat_d, flat_t = d.view(-1), tr.view(-1)
+    for pos in (0, 1, 2 ** 31 - 1, 2 ** 31, 2 ** 32 - 1, 2 ** 32, 2 ** 32 + 1):
+        assert torch.isinf(flat_d[pos]) and int(flat_t[pos]) == -1
+    assert bool(torch.all(torch.isinf(d[0]))) and bool(torch.all(tr[0] == -1))
+    # the band-sparse output and the closest points of the same call sequence agree with the dense grids
+    nb, ids, sd, st_ = B.sdf_compute_sparse(m, w.origin, w.h, w.dims, w.band)
+    torch.cuda.synchronize()
+    assert nb > 0 and int(torch.isfinite(sd[:nb]).sum()) == int(np.isfinite(dwin).sum())
+    cp = B.sdf_closest_points(m, w.origin, w.h, w.dims, tr)
+    torch.cuda.synchronize()
+    assert int(torch.isfinite(cp[..., 0]).sum()) == int((twin >= 0).sum())
+    B.sdf_fill_interior(d, w.band)
+    torch.cuda.synchronize()
+    inside = int((d == -np.float32(w.band)).sum())
+    assert inside > 1000 and bool(torch.all(torch.isinf(d[0])))
+    m.destroy(); m2.destroy()

@@ -512,3 +512,27 @@ def test_fp32_peak_microbenchmark():
     from paper_1903_00353_b200 import binding as B
     tf, sms = B.sdf_measure_fp32_peak()
     assert sms > 0 and 0.5 * sms * 128 * 2 * 1.0e9 / 1e12 < tf < sms * 128 * 2 * 2.3e9 / 1e12, (tf, sms)
+
+
+@pytest.mark.parametrize("subdiv", [1, 2, 3])
+def test_cell_centres_on_vertices_and_edges_of_a_generic_mesh(oracle_mod, subdiv):
+    """Cell centres that coincide with vertices (the six axis vertices of an icosphere of radius 16 h centred on a grid
+    point) and with points of edges (the midpoints of the octahedral edges, at subdiv >= 1 vertices themselves; at any
+    level the x-axis crossings): the exact distance is 0 there, and a zero has no sign.  The faces around them have
+    irrational normals, so n . r of an in-plane r is rounding noise: the sign pass must report 0, as the definition
+    does, not +-1e-17."""
+    n, h = 64, 2.0 ** -5
+    v, t = W.icosphere_mesh(subdiv, 16 * h)
+    c = np.array([32 * h, 32 * h, 32 * h])
+    w = W.Workload("onvertex", W.soup_from_indexed(v + c, t, np.random.default_rng(subdiv)), (0.0, 0.0, 0.0), h, (n, n, n), 3 * h)
+    res = check_parity(w, oracle_mod)
+    _assert_ok(res)
+    om = oracle_mod.Mesh(f32_grid(w).soup)
+    d_ref, _ = om.sdf(w.origin, w.h, w.dims, w.band)
+    assert int((d_ref == 0).sum()) >= 6
+    from paper_1903_00353_b200 import binding as B
+    m, d, tr = B.compute_workload(f32_grid(w))
+    dz = d.cpu().numpy()
+    assert np.array_equal(dz == 0, d_ref == 0)
+    assert not np.signbit(dz[dz == 0]).any()
+    m.destroy()
