@@ -103,3 +103,47 @@ def test_transform_errors_leave_no_handle():
     with pytest.raises(B.SdfError):
         B.sdf_transform(soup, w.origin, w.h, w.dims, w.band)
     torch.cuda.synchronize()
+
+
+def test_two_host_threads_on_two_streams():
+    """include/sdf.h: distinct handles on distinct streams are independent (the library's side streams are shared, its
+    events pooled): two host threads run sdf_transform / sdf_compute_sparse / destroy in a loop, each on its own stream
+    and workload; every result must equal the one the same call gives alone, bit for bit."""
+    import threading
+    from paper_1903_00353_b200 import binding as B
+    ws = [f32_grid(W.config("C2", 0.5)), f32_grid(W.config("C3", 0.3)), f32_grid(W.config("C5", 0.08))]
+    ref = []
+    for w in ws:                                          # also creates the library-wide state (first calls: serial)
+        m, d, t = B.compute_workload(w)
+        torch.cuda.synchronize()
+        ref.append((d.clone(), t.clone()))
+        m.destroy()
+    errors = []
+
+    def worker(idx):
+        try:
+            w = ws[idx]
+            st = torch.cuda.Stream()
+            soup = torch.from_numpy(np.ascontiguousarray(w.soup)).cuda()
+            torch.cuda.synchronize()
+            for it in range(12):
+                with torch.cuda.stream(st):
+                    m, d, t = B.sdf_transform(soup, w.origin, w.h, w.dims, w.band, stream=st)
+                    nb, ids, sd, stt = B.sdf_compute_sparse(m, w.origin, w.h, w.dims, w.band, stream=st)
+                st.synchronize()
+                if not (torch.equal(d.view(torch.int32), ref[idx][0].view(torch.int32)) and torch.equal(t, ref[idx][1])):
+                    errors.append((idx, it, "dense"))
+                if int(torch.isfinite(sd[:nb]).sum()) != int(torch.isfinite(ref[idx][0]).sum()):
+                    errors.append((idx, it, "sparse"))
+                m.destroy()
+        except Exception as e:                            # noqa: BLE001 -- reported through the list
+            errors.append((idx, repr(e)))
+
+    threads = [threading.Thread(target=worker, args=(i,)) for i in range(len(ws))]
+    for th in threads:
+        th.start()
+    for th in threads:
+        th.join(timeout=120)
+    assert not any(th.is_alive() for th in threads)
+    torch.cuda.synchronize()
+    assert not errors, errors[:5]
