@@ -24,21 +24,23 @@ void stage_mark(sdf_mesh *m, int stage, int which, cudaStream_t st) {
 #include <vector>
 static std::mutex g_ev_mutex;
 static std::vector<cudaEvent_t> g_ev_pool[64];      // per device: idle events (cudaEventDisableTiming)
-int ev_get(cudaEvent_t *e) {
+int ev_get(sdf_mesh *m, cudaEvent_t *e) {
     if (*e) return SDF_OK;
     int dev = 0;
     CK(cudaGetDevice(&dev));
-    if (dev >= 0 && dev < 64) {
+    if (!m->ev_dev1) m->ev_dev1 = dev + 1;
+    if (m->ev_dev1 == dev + 1 && dev >= 0 && dev < 64) {
         std::lock_guard<std::mutex> lk(g_ev_mutex);
         if (!g_ev_pool[dev].empty()) { *e = g_ev_pool[dev].back(); g_ev_pool[dev].pop_back(); return SDF_OK; }
     }
     CK(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
     return SDF_OK;
 }
-void ev_put(cudaEvent_t *e) {
+void ev_put(sdf_mesh *m, cudaEvent_t *e) {
     if (!*e) return;
     int dev = -1;
-    if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64) {
+    // back to the pool of the device it was taken on (a handle used on another device keeps its events out of the pools)
+    if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64 && m->ev_dev1 == dev + 1) {
         std::lock_guard<std::mutex> lk(g_ev_mutex);
         if (g_ev_pool[dev].size() < 256) { g_ev_pool[dev].push_back(*e); *e = nullptr; return; }
     }
@@ -117,11 +119,11 @@ void sdf_destroy(sdf_mesh *m) {
     cudaStream_t st = m->last_stream;
     cudaStreamSynchronize(st);
     if (m->side) cudaStreamSynchronize(m->side);      // shared, process-lifetime stream: not destroyed here
-    ev_put(&m->ev_fork);
-    ev_put(&m->ev_join);
-    ev_put(&m->ev_bjoin);
-    ev_put(&m->ev_ffork);
-    ev_put(&m->ev_fjoin);
+    ev_put(m, &m->ev_fork);
+    ev_put(m, &m->ev_join);
+    ev_put(m, &m->ev_bjoin);
+    ev_put(m, &m->ev_ffork);
+    ev_put(m, &m->ev_fjoin);
     void *ptrs[] = {m->slab_f, m->slab_ws, m->scratch, m->cp_state};      // (fill_state, hoist_g_dev: views into slab_f)
     for (size_t i = 0; i < sizeof(ptrs) / sizeof(ptrs[0]); i++) dev_free(&m->alloc, ptrs[i], st);
     for (int i = 0; i < SDF_T_COUNT; i++)

@@ -174,6 +174,7 @@ struct sdf_mesh {
     cudaStream_t last_stream;
     cudaStream_t side;                // library-owned stream of the sentinel fill (A8a)
     cudaEvent_t ev_fork, ev_join;
+    int ev_dev1;                      // 1 + device the handle's pooled events belong to (0: none taken yet)
     cudaEvent_t ev_bjoin;             // join of the brick stream (hoisted A6a beside the edge and vertex stages)
     // sdf_transform: sentinel fill still to be started at stage boundary pre_at of build_features (0 = none pending)
     const GridParams *pre_g; float *pre_dist; int *pre_tri; int pre_at;
@@ -197,8 +198,9 @@ struct Carver {
 
 // the library's fork / join events come from a process-wide pool (creating and destroying five per handle was a tenth of
 // the host time of a small sdf_transform); thread-safe; an event goes back when its handle is destroyed
-int ev_get(cudaEvent_t *e);          // no-op if *e is set already
-void ev_put(cudaEvent_t *e);
+struct sdf_mesh;
+int ev_get(sdf_mesh *m, cudaEvent_t *e);          // no-op if *e is set already
+void ev_put(sdf_mesh *m, cudaEvent_t *e);
 
 // allocation through the handle's allocator
 int dev_alloc(const sdf_allocator *a, void **p, size_t bytes, cudaStream_t st);

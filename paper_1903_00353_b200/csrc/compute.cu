@@ -738,8 +738,8 @@ static int fork_sentinel_fill(sdf_mesh *m, const GridParams &g, float *dist, int
         }
         m->side = g_side;
     }
-    CKS(ev_get(&m->ev_ffork));
-    CKS(ev_get(&m->ev_fjoin));
+    CKS(ev_get(m, &m->ev_ffork));
+    CKS(ev_get(m, &m->ev_fjoin));
     CK(cudaEventRecord(m->ev_ffork, st));
     CK(cudaStreamWaitEvent(m->side, m->ev_ffork, 0));
     CKS(launch_fill(m->side));

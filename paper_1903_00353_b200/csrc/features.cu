@@ -579,14 +579,14 @@ static int fork_vertex_stream(sdf_mesh *m, cudaStream_t st, cudaStream_t *vs_out
         CK(cudaStreamCreateWithFlags(&g_bs, cudaStreamNonBlocking));
         g_vs_dev = dev;
     }
-    CKS(ev_get(&m->ev_fork));
-    CKS(ev_get(&m->ev_join));
+    CKS(ev_get(m, &m->ev_fork));
+    CKS(ev_get(m, &m->ev_join));
     CK(cudaEventRecord(m->ev_fork, st));
     CK(cudaStreamWaitEvent(g_vs, m->ev_fork, 0));
     drain.s = g_vs; drain.armed = true;
     *vs_out = g_vs;
     if (bs_out && bdrain && m->hoist_g) {
-        CKS(ev_get(&m->ev_bjoin));
+        CKS(ev_get(m, &m->ev_bjoin));
         CK(cudaStreamWaitEvent(g_bs, m->ev_fork, 0));
         bdrain->s = g_bs; bdrain->armed = true;
         *bs_out = g_bs;
