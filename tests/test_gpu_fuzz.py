@@ -71,6 +71,46 @@ def test_fuzz_parity_and_fill(oracle_mod, seed):
     assert populated > 100000
 
 
+def _aligned_case(r):
+    """Vertices and cell centres on a common power-of-two lattice (spheres whose axis vertices, boxes and cube fans whose
+    faces and edges pass through cell centres): many exactly-zero distances and exact ties between features."""
+    mk = [lambda: W.icosphere_mesh(int(r.integers(0, 4)), 1.0), lambda: W.box_mesh((0.5, 0.25, 0.75)), lambda: W.tetrahedron_mesh(1.0),
+          lambda: W.cube_fan_mesh((int(r.integers(0, 3)), int(r.integers(0, 3)), int(r.integers(0, 3))))]
+    v, t = mk[int(r.integers(0, len(mk)))]()
+    nn = int(r.integers(16, 64))
+    h = 2.0 ** -int(r.integers(3, 7))
+    radius = int(r.integers(2, nn // 3 + 1)) * h
+    centre = np.array([int(x) * h for x in r.integers(nn // 3, 2 * nn // 3, 3)])
+    soup = W.soup_from_indexed(v * radius + centre, t, r)
+    return f32_grid(W.Workload("aligned", soup, (0.0, 0.0, 0.0), h, (nn, nn, nn), float(r.integers(1, 5)) * h))
+
+
+def test_fuzz_lattice_aligned_meshes(oracle_mod):
+    """Cell centres on vertices, edges and faces: the exact distance is 0 there.  The library reports +0 (DESIGN.md sec.7 (iii));
+    the oracle +0 or +-1e-16 (its fp64 noise), which clause 3 of the harness waives.  1,100 of 12,400 such cases differed in
+    exactly that way before the waiver, none in any other way; the suite keeps 150."""
+    from paper_1903_00353_b200 import binding as B
+    zeros = 0
+    for c in range(150):
+        w = _aligned_case(np.random.default_rng(31 * 100003 + c))
+        om = oracle_mod.Mesh(w.soup)
+        d_ref, t_ref = om.sdf(w.origin, w.h, w.dims, w.band)
+        m, d, tr = B.sdf_transform(torch.from_numpy(np.ascontiguousarray(w.soup)).cuda(), w.origin, w.h, w.dims, w.band)
+        d_np = d.cpu().numpy()
+        res = compare_to_oracle(d_np, tr.cpu().numpy(), d_ref, t_ref, w, om)
+        assert res["ok"] and all(res[k] == 0 for k in KEYS), (c, w.dims, w.band / w.h, {k: res[k] for k in KEYS})
+        z = d_np == 0
+        zeros += int(z.sum())
+        assert not np.signbit(d_np[z]).any()                  # a zero is +0
+        assert np.all(np.abs(d_ref[z]) <= 1e-12 * w.diag)       # ... and only where the oracle's distance is zero too
+        # (the converse holds to fp32 resolution only: on a coplanar patch a cell can lie 1e-9 outside the triangle whose
+        # fp32 candidate won and inside its neighbour -- the sign pass re-decides on the winning triangle, DESIGN.md sec.7)
+        on = np.abs(d_ref) <= 1e-12 * w.diag
+        assert np.all(np.abs(d_np[on]) <= 1e-7 * w.diag) and int(z[on].sum()) >= 0.97 * int(on.sum())
+        m.destroy()
+    assert zeros > 1000
+
+
 @pytest.mark.parametrize("seed", [201, 202])
 def test_fuzz_wide_bands_partial_overlap_closest_points(oracle_mod, seed):
     from paper_1903_00353_b200 import binding as B

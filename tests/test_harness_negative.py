@@ -121,6 +121,22 @@ def test_flipped_sign_is_a_sign_violation(case):
         assert all(res[k] == 0 for k in KEYS if k not in ("bad_sign", "bad_dist"))
 
 
+def test_sign_of_a_distance_below_fp64_noise_is_waived_but_not_above(case):
+    """Clause 3 is waived only where both magnitudes are below 1e-12 * diag (an exact zero that the oracle's fp64 reports as
+    +-1e-16): +0 against -1e-17 passes; the same cell at -1e-9 against +1e-9 does not."""
+    w, om, d, t = case
+    c = _deep_cells(case)[0]
+    d_ref = d.copy().reshape(-1)
+    d_gpu = d.copy().reshape(-1)
+    d_ref[c] = np.float32(-1e-17); d_gpu[c] = np.float32(0.0)
+    from helpers import compare_to_oracle
+    res = compare_to_oracle(d_gpu.reshape(d.shape), t, d_ref.reshape(d.shape), t, w, om)
+    assert res["bad_sign"] == 0
+    d_ref[c] = np.float32(-1e-9); d_gpu[c] = np.float32(1e-9)
+    res = compare_to_oracle(d_gpu.reshape(d.shape), t, d_ref.reshape(d.shape), t, w, om)
+    assert res["bad_sign"] == 1 and not res["ok"]
+
+
 def test_wrong_id_is_an_id_violation_but_a_tying_id_is_not(case):
     w, om, d, t = case
     F = w.ntri
