@@ -590,6 +590,10 @@ __global__ void __launch_bounds__(EB_BT, 8) emit_bricks_kernel(MeshView mv, Grid
 #pragma unroll
     for (int r = 0; r < 4; r++) {
         const u64 p[4] = {ld[2 * r].x, ld[2 * r].y, ld[2 * r + 1].x, ld[2 * r + 1].y};
+        // two z-slices without a candidate (a band sheet rarely crosses all eight slices of a brick): nothing to unpack or write
+        if (__all_sync(0xffffffffu, (u32)((p[0] & p[1] & p[2] & p[3]) >> 32) == 0xFFFFFFFFu)) {
+            if (!SPARSE) continue;
+        }
         const int c0 = 128 * r + 4 * lane;
         float od[4];
         int ot[4];
