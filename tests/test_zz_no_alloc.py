@@ -66,7 +66,7 @@ def test_static_fill_allocates_nothing_and_rejects_large_grids():
     B.sdf_fill_interior_static(work, 0.5)
     torch.cuda.synchronize()
     free1, _ = torch.cuda.mem_get_info()
-    assert free1 == free0                                   # nothing taken from (or returned to) the driver
+    assert free1 >= free0                                   # nothing taken from the driver (a pool trimming itself meanwhile may return some)
     # the largest grid that fits: ny * nz * ceil(nx / 1024) = 2^20 map words; one row more does not
     fits = torch.full((1024, 1024, 32), float("inf"), dtype=torch.float32, device="cuda")
     fits[500, 500, 7] = -1.0
