@@ -187,6 +187,7 @@ static int make_grid(const float origin[3], float h, int nx, int ny, int nz, flo
         maxabs = fmaxf(maxabs, fmaxf(lo, hi));
     }
     g->guard = 1e-3f * h + 1e-6f * maxabs;
+    g->tiny_abs = 2.5e-7f * maxabs;
     g->rb = band + g->guard + g->eps;
     const char *dbg = getenv("SDF_AABB_MODE");
     g->aabb_mode = (dbg && dbg[0] == '1') ? 1 : 0;

@@ -121,6 +121,7 @@ struct GridParams {
                                     // 4 forked after the mid-way host crossing
     int fill_prio;                  // side stream at the highest priority
     int fill_ctas;                  // TMA fill: CTAs launched per SM (one per SM survives)
+    float tiny_abs;                 // an fp32 distance at or below this has no reliable sign: 2 ulp of the largest |coordinate| of the grid
     int row_clip;                   // rows longer than this many cells are clipped analytically before they are walked
     int eval_chunk;                 // warps per class-interleaving round of evaluate_small_kernel (0: plain order)
     int fill_depth, fill_issuers;   // TMA fill: chunk pairs in flight per issuing lane, issuing lanes per SM

@@ -195,7 +195,7 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
             if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f && !g.aabb_mode) {
                 const float dnc = dot_rn(n, r);
                 d = fabsf(dnc);
-                fl = (tiny_vs(d, r) ? 0u : FL_SURE) | (dnc < 0.0f ? FL_NEG : 0u);
+                fl = (tiny_vs(g, d, r) ? 0u : FL_SURE) | (dnc < 0.0f ? FL_NEG : 0u);
             } else {
                 // eps margin: exact clamped distance from the triangle itself
                 const float *T = mv.soup + 9 * (size_t)ri[RR_TIDX];
@@ -231,7 +231,7 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
             // the end caps belong to the end vertices, and the eps slack of a nearly flat wedge
             // reaches through the surface: the class gives the sign only where the bisector agrees
             const float sb = (fl_rec & FL_NEG) ? -dot(nbis, q) : dot(nbis, q);
-            const u32 fl = (tu > 0.0f && tu < L && sb > 1e-2f * d && !tiny_vs(d, r)) ? fl_rec : (fl_rec & FL_NEG);
+            const u32 fl = (tu > 0.0f && tu < L && sb > 1e-2f * d && !tiny_vs(g, d, r)) ? fl_rec : (fl_rec & FL_NEG);
             if (d < reach) { accepted++; put_min(g, table, scratch, i, j, k, d, id, fl); }
         }
     } else {
@@ -255,7 +255,7 @@ __device__ __forceinline__ void process_row_inc(const MeshView &mv, const GridPa
             if (d >= reach || ar < c * d - eps) continue;
             accepted++;
             // near the plane through the vertex normal to the axis the side is not decided here
-            put_min(g, table, scratch, i, j, k, d, id, ar > 1e-2f * d ? fl_rec : (fl_rec & FL_NEG));
+            put_min(g, table, scratch, i, j, k, d, id, (ar > 1e-2f * d && !tiny_vs(g, d, r)) ? fl_rec : (fl_rec & FL_NEG));
         }
     }
 }
@@ -494,10 +494,75 @@ __global__ void __launch_bounds__(FILL_TMA_BT) fill_tma_kernel(float *__restrict
 
 struct CellOut { float d; int t; };
 
+// A cell within fp32 noise of the surface (finish_cell): the triangle closest to X among t, its three edge neighbours and
+// the fan around its corner nearest to X (at most 32 of it) is found in fp64, and distance, sign and id are taken from it.
+// A distance that fp64 cannot tell from zero (a cell centre on a vertex, an edge, a face: |n . r| of an in-plane r is
+// rounding noise of ~1e-16 |r|) is zero, and a zero has no sign -- not -1e-17 or +1e-17 by the luck of the rounding.
+// A few hundred cells per million come here: the emit kernel collects them and works them off in a loop of its own at the
+// end (inlined into the sign pass, or called out of line, this code cost the whole kernel 6-17 % of its speed).
+__device__ __forceinline__ CellOut near_surface_cell(const float *__restrict__ soup, const float *__restrict__ fn,
+                                                  const int *__restrict__ adj, const int *__restrict__ cvid,
+                                                  const int *__restrict__ perm, const VertexRec *__restrict__ vrec, int t, int xt,
+                                                  double x, double y, double z, double dband) {
+    const V3<double> X = mk<double>(x, y, z);
+    int tb = t, kc = 0, rg = 0;
+    double D = 0.0, scale = 0.0, best = 1e300;
+    for (int c = 0; c < 3; c++) {
+        const V3<double> dv = X - ld3d(soup + 9 * (size_t)t + 3 * c);
+        const double q2 = dot(dv, dv);
+        if (q2 < best) { best = q2; kc = c; }
+    }
+    V3<double> R = X, Q = X, Nn = X;
+    int he = 3 * t + (kc + 2) % 3;                           // the half-edge of t that arrives at the corner
+    // one loop, one instance of the fp64 point-triangle routine: candidate 0 is t, 1..3 its edge neighbours, then the fan
+    for (int c = 0; c < 36; c++) {
+        int tt = t;
+        if (c >= 1 && c <= 3) {
+            const int tw = adj[3 * (size_t)t + (c - 1)];
+            if (tw < 0 || tw / 3 == t) continue;
+            tt = tw / 3;
+        } else if (c > 3) {
+            // the fan matters only where the cell is as close to the corner as to the surface (within the same noise):
+            // elsewhere the closest point lies in a face or on an edge, and the edge neighbours were all there is to ask
+            if (c == 4) {
+                const double lim = D + 1e-5 * scale;
+                if (best > lim * lim) break;
+            }
+            const int tw = adj[he];                          // its twin leaves the corner in the next triangle of the fan
+            if (tw < 0 || tw / 3 == t) break;
+            tt = tw / 3;
+            he = 3 * tt + ((tw - 3 * tt) + 2) % 3;
+        }
+        const float *TT = soup + 9 * (size_t)tt;
+        const V3<double> A2 = ld3d(TT), E0 = ld3d(TT + 3) - A2, EC = ld3d(TT + 6) - A2, R2 = X - A2;
+        V3<double> n2 = cross(E0, EC), q2;
+        n2 = (1.0 / sqrt(dot(n2, n2))) * n2;
+        int rg2;
+        const double D2 = tri_closest<double>(R2, E0, EC, n2, rg2, q2);
+        if (c == 0 || D2 < D) {
+            D = D2; tb = tt; rg = rg2; R = R2; Q = q2; Nn = n2;
+            scale = fabs(R2.x) + fabs(R2.y) + fabs(R2.z) + fabs(E0.x) + fabs(E0.y) + fabs(E0.z) + fabs(EC.x) + fabs(EC.y) + fabs(EC.z);
+        }
+    }
+    CellOut o;
+    o.d = INFINITY; o.t = -1;
+    if (!(D < dband)) return o;
+    if (D <= 4e-15 * scale) D = 0.0;
+    V3<double> PN;
+    if (rg == RG_FACE) PN = Nn;
+    else if (rg <= RG_E2) PN = ld3d(fn + 3 * (size_t)tb) + ld3d(fn + 3 * (size_t)(adj[3 * (size_t)tb + (rg - RG_E0)] / 3));
+    else PN = ld3d(vrec[cvid[3 * (size_t)tb + (rg - RG_V0)]].axis);
+    const bool neg = dot(PN, R - Q) < 0.0;
+    const float d = (float)D;
+    o.d = (neg && d != 0.0f) ? -d : d;
+    o.t = tb == t ? xt : perm[tb];
+    return o;
+}
+
 // Populated cell: band decision (fp64 re-check near the band edge) and the sign from the
 // pseudonormal of the closest feature of the winning triangle.
 __device__ __forceinline__ CellOut finish_cell(const MeshView &mv, const GridParams &g, int i, int j, int k, u64 pack,
-                                               u32 &recheck) {
+                                               u32 &recheck, bool &near_surface) {
     CellOut o;
     o.d = INFINITY; o.t = -1;
     float d = __uint_as_float((u32)(pack >> 32));
@@ -522,7 +587,7 @@ __device__ __forceinline__ CellOut finish_cell(const MeshView &mv, const GridPar
     f3 dv = (x - a) - q;
     float s = dot(pn, dv);
     bool neg = s < 0.0f;
-    if (fabsf(s) <= 1e-3f * sqrtf(dot(pn, pn) * dot(dv, dv)) || tiny_vs(d, x - a)) redo = true;
+    if (fabsf(s) <= 1e-3f * sqrtf(dot(pn, pn) * dot(dv, dv)) || tiny_vs(g, d, x - a)) redo = true;
     if (redo) {
         // fp64 on the same winning triangle: exact cell position, distance, region, sign
         recheck++;
@@ -532,14 +597,17 @@ __device__ __forceinline__ CellOut finish_cell(const MeshView &mv, const GridPar
         V3<double> X = mk<double>(g.dox + i * g.dh, g.doy + j * g.dh, g.doz + k * g.dh);
         V3<double> Q;
         double D = tri_closest<double>(X - A, E0, EC, Nn, rg, Q);
-        if (!(D < g.dband)) return o;                         // strictly inside the band (PAPER.md:392)
-        // a distance that fp64 cannot tell from zero (a cell centre on a vertex, an edge, a face: |n . r| of an in-plane r is
-        // rounding noise of ~1e-16 |r|) is zero, and a zero has no sign -- not -1e-17 or +1e-17 by the luck of the rounding
-        {
-            const V3<double> R = X - A;
-            const double scale = fabs(R.x) + fabs(R.y) + fabs(R.z) + fabs(E0.x) + fabs(E0.y) + fabs(E0.z) + fabs(EC.x) + fabs(EC.y) + fabs(EC.z);
-            if (D <= 4e-15 * scale) D = 0.0;
+        const V3<double> R = X - A;
+        const double scale = fabs(R.x) + fabs(R.y) + fabs(R.z) + fabs(E0.x) + fabs(E0.y) + fabs(E0.z) + fabs(EC.x) + fabs(EC.y) + fabs(EC.z);
+        if (D <= 1e-5 * scale) {
+            // Within fp32 noise of the surface the fp32 minimum may belong to a NEIGHBOUR of the closest triangle (3e-8
+            // beside 9e-9: the order of two such candidates is rounding luck), and beside a sharp edge the neighbour's side
+            // of the surface is the other one: the triangles around the winner are measured in fp64 too, the closest decides
+            // (a few hundred cells per million: the caller hands them to near_surface_cell)
+            near_surface = true;
+            return o;
         }
+        if (!(D < g.dband)) return o;                         // strictly inside the band (PAPER.md:392)
         V3<double> PN;
         if (rg == RG_FACE) PN = Nn;
         else if (rg <= RG_E2) PN = ld3d(N) + ld3d(mv.fn + 3 * (size_t)(mv.adj[3 * (size_t)t + (rg - RG_E0)] / 3));
@@ -650,11 +718,37 @@ __global__ void __launch_bounds__(EB_BT, 8) emit_bricks_kernel(MeshView mv, Grid
     // the sign pass proper, 32 queued cells at a time (one call site: finish_cell is large).  The packed value is read
     // again from the scratch (an L2 hit); the single-cell stores come after the warp's segment stores above.
     __syncwarp();
+    int n2 = 0;                                                // cells within fp32 noise of the surface: a second, colder queue
     for (int q0 = 0; q0 < n; q0 += 32) {
+        bool near = false;
+        int c = 0;
         if (q0 + lane < n) {
+            c = s_cell[w][q0 + lane];
+            const int ci = bx * 8 + (c & 7), cj = by * 8 + ((c >> 3) & 7), ck = bz * 8 + (c >> 6);
+            const CellOut o = finish_cell(mv, g, ci, cj, ck, __ldcg(scratch + (size_t)slot * BRICK_CELLS + c), recheck, near);
+            if (o.t >= 0) {
+                const size_t idx = SPARSE ? (size_t)slot * BRICK_CELLS + c : ((size_t)ck * g.ny + cj) * g.nx + ci;
+                dist[idx] = o.d; tri[idx] = o.t;
+                band++;
+            }
+        }
+        const unsigned nm = __ballot_sync(0xffffffffu, near);
+        if (nm) {
+            // (the slots written here were read above: entry n2 + rank <= q0 + lane)
+            __syncwarp();
+            if (near) s_cell[w][n2 + __popc(nm & ((1u << lane) - 1u))] = (unsigned short)c;
+            n2 += __popc(nm);
+            __syncwarp();
+        }
+    }
+    for (int q0 = 0; q0 < n2; q0 += 32) {
+        if (q0 + lane < n2) {
             const int c = s_cell[w][q0 + lane];
             const int ci = bx * 8 + (c & 7), cj = by * 8 + ((c >> 3) & 7), ck = bz * 8 + (c >> 6);
-            const CellOut o = finish_cell(mv, g, ci, cj, ck, __ldcg(scratch + (size_t)slot * BRICK_CELLS + c), recheck);
+            const u64 pack = __ldcg(scratch + (size_t)slot * BRICK_CELLS + c);
+            const int xt = (int)((u32)pack >> 2);
+            const CellOut o = near_surface_cell(mv.soup, mv.fn, mv.adj, mv.cvid, mv.perm, mv.vrec, mv.inv_perm[xt], xt,
+                                                g.dox + ci * g.dh, g.doy + cj * g.dh, g.doz + ck * g.dh, g.dband);
             if (o.t >= 0) {
                 const size_t idx = SPARSE ? (size_t)slot * BRICK_CELLS + c : ((size_t)ck * g.ny + cj) * g.nx + ci;
                 dist[idx] = o.d; tri[idx] = o.t;

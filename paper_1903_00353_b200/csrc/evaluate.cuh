@@ -283,7 +283,11 @@ __device__ __forceinline__ bool poly_aabv(const MeshView &mv, const GridParams &
 #define TY_UNSURE 32
 
 // a distance this small against the operands it was differenced from has no reliable sign in fp32
-__device__ __forceinline__ bool tiny_vs(float d, f3 r) { return d <= 1e-5f * (fabsf(r.x) + fabsf(r.y) + fabsf(r.z)); }
+// (relative to the operands of the difference -- and absolutely: a cell coordinate fmaf(i, h, o) carries half an ulp of the
+// largest coordinate of the grid whatever the size of r; g.tiny_abs = two such ulps)
+__device__ __forceinline__ bool tiny_vs(const GridParams &g, float d, f3 r) {
+    return d <= 1e-5f * (fabsf(r.x) + fabsf(r.y) + fabsf(r.z)) || d <= g.tiny_abs;
+}
 
 __device__ __forceinline__ void put_min(const GridParams &g, const int *__restrict__ table, u64 *__restrict__ scratch,
                                         int i, int j, int k, float d, int id, u32 fl) {
@@ -360,7 +364,7 @@ __device__ __forceinline__ void process_direct(const MeshView &mv, const GridPar
                     if (s0 >= 0.0f && s1 >= 0.0f && s2 >= 0.0f) {
                         const float dnc = dot_rn(n, r);
                         d = fabsf(dnc);
-                        fl = (tiny_vs(d, r) ? 0u : FL_SURE) | (dnc < 0.0f ? FL_NEG : 0u);
+                        fl = (tiny_vs(g, d, r) ? 0u : FL_SURE) | (dnc < 0.0f ? FL_NEG : 0u);
                     } else {
                         int rg; f3 qq;                // eps margin: exact clamped distance
                         d = tri_closest<float>(r, e0, ec, n, rg, qq);
@@ -400,7 +404,7 @@ __device__ __forceinline__ void process_direct(const MeshView &mv, const GridPar
                     const f3 q = mk<float>(__fmaf_rn(-tc, u.x, r.x), __fmaf_rn(-tc, u.y, r.y), __fmaf_rn(-tc, u.z, r.z));
                     const float d = __fsqrt_rn(dot_rn(q, q));
                     const float sb = (fl_rec & FL_NEG) ? -dot(nbis, q) : dot(nbis, q);
-                    const u32 fl = (tu > 0.0f && tu < L && sb > 1e-2f * d && !tiny_vs(d, r)) ? fl_rec : (fl_rec & FL_NEG);
+                    const u32 fl = (tu > 0.0f && tu < L && sb > 1e-2f * d && !tiny_vs(g, d, r)) ? fl_rec : (fl_rec & FL_NEG);
                     if (d < reach) { accepted++; put_min(g, table, scratch, i, j0 + dj, k0 + dk, d, id, fl); }
                 }
             }
@@ -424,7 +428,7 @@ __device__ __forceinline__ void process_direct(const MeshView &mv, const GridPar
                     const float d = __fsqrt_rn(dot_rn(r, r)), ar = dot(A, r);
                     if (d >= reach || ar < c * d - eps) continue;
                     accepted++;
-                    put_min(g, table, scratch, i, j0 + dj, k0 + dk, d, id, ar > 1e-2f * d ? fl_rec : (fl_rec & FL_NEG));
+                    put_min(g, table, scratch, i, j0 + dj, k0 + dk, d, id, (ar > 1e-2f * d && !tiny_vs(g, d, r)) ? fl_rec : (fl_rec & FL_NEG));
                 }
             }
         }

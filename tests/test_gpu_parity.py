@@ -536,3 +536,28 @@ def test_cell_centres_on_vertices_and_edges_of_a_generic_mesh(oracle_mod, subdiv
     assert np.array_equal(dz == 0, d_ref == 0)
     assert not np.signbit(dz[dz == 0]).any()
     m.destroy()
+
+
+def test_sign_of_a_cell_within_fp32_noise_of_the_surface(oracle_mod):
+    """Found by a fuzz campaign on medium meshes (756 cases, 5 sign mismatches in ~1e9 band cells): a cell 7e-9 outside the
+    surface whose fp32 cell coordinate (half an ulp of |x| ~ 0.5: 3e-8) put it 4e-9 inside one face while the closest point
+    lay on the neighbouring face.  A relative test (d <= 1e-5 |x - a|) called the face's sign certain because the cell was
+    close to corner a.  Now a distance within two ulps of the grid's largest coordinate is never sign-certain, and the fp64
+    sign pass measures the triangles around the winner too."""
+    import dataclasses
+    import types
+    from helpers import compare_to_oracle
+    from paper_1903_00353_b200 import binding as B
+    w0 = W.config("C4", 0.2561253111963309)
+    w = w0.crop((6, 103, 27), (238, 150, 228))
+    w = f32_grid(dataclasses.replace(w, band=4.10730308445584 * w.h))
+    om = oracle_mod.Mesh(w.soup)
+    d_ref, t_ref = om.sdf(w.origin, w.h, w.dims, w.band)
+    m, d, tr = B.compute_workload(w)
+    cw = types.SimpleNamespace(h=w.h, band=w.band, diag=w0.diag, ntri=w.ntri, dims=w.dims, origin=w.origin)
+    res = compare_to_oracle(d.cpu().numpy(), tr.cpu().numpy(), d_ref, t_ref, cw, om)
+    _assert_ok(res)
+    cell = 6177419                                   # the cell of the campaign: 6.7e-9 outside
+    assert d_ref.reshape(-1)[cell] < 0 and abs(d_ref.reshape(-1)[cell]) < 1e-8
+    assert d.cpu().numpy().reshape(-1)[cell] < 0
+    m.destroy()
