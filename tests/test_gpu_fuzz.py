@@ -4,8 +4,10 @@ and shifted, on random ragged grids (5..150 cells per axis, spacing and origin n
 bands (0.6..12 cells).  Every case must meet the four north_star clauses, and sdf_fill_interior on its result
 must equal the oracle's sweeps bit for bit.  (10,800 such cases were run once with zero failures, also under the
 ablation switches, and 11,000 more with multi-body meshes, bands up to 80 cells, grids that only partly meet the
-mesh and the closest-point call; the suite keeps 700 of them.  Round 2's final build: 62,000 more with new seeds, through
-sdf_create + sdf_compute and through sdf_transform, a fifth of them lattice-aligned: see test_fuzz_lattice_aligned_meshes.)"""
+mesh and the closest-point call; the suite keeps 700 of them.  Round 2: 62,000 more with new seeds, through sdf_create +
+sdf_compute and through sdf_transform, a fifth of them lattice-aligned (test_fuzz_lattice_aligned_meshes), and 756 medium-size
+ones -- random windows of C2..C5 at 130,000 to 370,000 triangles, ~1e9 band cells -- which found the five near-surface sign
+errors of test_sign_of_a_cell_within_fp32_noise_of_the_surface; after that fix 60,800 small and 1,011 medium cases: none.)"""
 import numpy as np
 import pytest
 import torch
