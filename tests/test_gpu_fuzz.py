@@ -7,7 +7,9 @@ ablation switches, and 11,000 more with multi-body meshes, bands up to 80 cells,
 mesh and the closest-point call; the suite keeps 700 of them.  Round 2: 62,000 more with new seeds, through sdf_create +
 sdf_compute and through sdf_transform, a fifth of them lattice-aligned (test_fuzz_lattice_aligned_meshes), and 756 medium-size
 ones -- random windows of C2..C5 at 130,000 to 370,000 triangles, ~1e9 band cells -- which found the five near-surface sign
-errors of test_sign_of_a_cell_within_fp32_noise_of_the_surface; after that fix 60,800 small and 1,011 medium cases: none.)"""
+errors of test_sign_of_a_cell_within_fp32_noise_of_the_surface; after that fix 60,800 small and 1,011 medium cases, 83,650 small
+ones under SDF_SCHEDULER=serial | dynamic, SDF_BUILDER=tile and SDF_SMOOTH_SIN=0, and 2,184 through the closest-point, z-slab and
+host-output calls: none.)"""
 import numpy as np
 import pytest
 import torch
